@@ -1,0 +1,202 @@
+/*
+ * metronome.h -- C ABI of libmetronome.so: bounded-window paged attention for resident streaming
+ * sessions on one NVIDIA B200 (sm_100a).
+ *
+ * The library implements the data-parallel hot path of Metronome's per-frame serving step
+ * (arxiv/paper_2607_02640; citations are PAPER.md:L<line>):
+ *
+ *   "retain each session's first S and last W tokens, freeing everything between -- as an API"
+ *                                                                    (sec. 6)
+ *   "the KV manager pins each request's first blocks instead of freeing them, and the attention
+ *    kernel's windowed mask admits [0,S) U [t-W,t]"                  (sec. 4.1)
+ *
+ * Conventions
+ *   - All functions return an int status (METRONOME_OK = 0).  No exceptions, no aborts.
+ *     On ANY error the pool's state (host and device) is unchanged.
+ *   - "host" pointers are ordinary CPU memory, read or written before the call returns.
+ *     "device" pointers are CUDA global memory on the pool's device; they are consumed
+ *     asynchronously on `cuda_stream` (a cudaStream_t passed as void*; NULL = default stream).
+ *   - All calls on one pool must be issued from one host thread at a time and on ONE stream (or on
+ *     streams the caller has ordered); the library adds no cross-stream synchronisation.
+ *   - The pool owns the KV storage (unless the caller provides it), block tables, free list and
+ *     split-KV workspace.  The caller owns q / k_new / v_new / out and the stream.
+ *   - bf16 = IEEE bfloat16 bit patterns, 2 bytes.  Row-major, innermost index last.
+ *   - Positions: the token appended i-th to a session (counting from 0 at session_open) has
+ *     absolute position i for ever ("the resident request keeps growing logically", L103).
+ *     K arrives position-encoded; the library applies no rotary embedding.
+ */
+#ifndef METRONOME_H_
+#define METRONOME_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define METRONOME_ABI_VERSION 1
+
+/* ---- status codes --------------------------------------------------------------------------- */
+enum {
+    METRONOME_OK = 0,
+    METRONOME_ERR_INVALID_ARG = 1,        /* NULL pointer, negative count, unsupported shape       */
+    METRONOME_ERR_INVALID_SESSION = 2,    /* sid not open                                          */
+    METRONOME_ERR_DUPLICATE_SESSION = 3,  /* a session may appear once per call (L46: "all due
+                                             sessions each tick")                                  */
+    METRONOME_ERR_SESSIONS_FULL = 4,      /* max_sessions slots are open                           */
+    METRONOME_ERR_POOL_EXHAUSTED = 5,     /* the paper's stall (L60: "the scheduler can no longer
+                                             allocate blocks"), surfaced cleanly: nothing changed  */
+    METRONOME_ERR_CHUNK_TOO_LARGE = 6,    /* n_new > max_new_tokens                                */
+    METRONOME_ERR_QLEN_EXCEEDS_LAST_APPEND = 7, /* older rows' windows may already be freed        */
+    METRONOME_ERR_LAYER_SEQUENCE = 8,     /* layer > 0 append that does not repeat layer 0's batch,
+                                             or attend on a layer not yet appended this step       */
+    METRONOME_ERR_LEN_OVERFLOW = 9,       /* the clean version of the max_model_len crash (L271)   */
+    METRONOME_ERR_CUDA = 10,              /* a CUDA runtime call failed; see metronome_last_cuda_error */
+    METRONOME_ERR_UNSUPPORTED = 11,       /* e.g. attention on a bookkeeping-only pool             */
+    METRONOME_ERR_OUT_OF_MEMORY = 12
+};
+
+/* ---- flags ---------------------------------------------------------------------------------- */
+/* Fill every freed block with bf16 NaN (L258: "freed blocks NaN-poisoned to prove nothing outside
+ * sinks U window is ever read").  Debug / test aid; off by default. */
+#define METRONOME_FLAG_POISON_ON_FREE 0x1u
+/* No KV storage: only sessions, block tables and the free list (any block_size >= 1).  append_kv
+ * must be given k_new = v_new = NULL; attend_frame returns METRONOME_ERR_UNSUPPORTED.  For
+ * occupancy studies (Eq. 1, Fig. 5) and bookkeeping tests. */
+#define METRONOME_FLAG_BOOKKEEPING_ONLY 0x2u
+/* The paper's vanilla arm (L52: "it bounds nothing"): no block is ever freed before close and the
+ * mask is plain causal.  W is ignored. */
+#define METRONOME_FLAG_UNBOUNDED 0x4u
+
+/* ---- configuration -------------------------------------------------------------------------- */
+typedef struct metronome_pool_config {
+    int32_t n_layers;        /* >= 1; one block table is shared by all layers (L256: every decoder
+                                layer reports the same windowed spec)                              */
+    int32_t n_q_heads;       /* Hq                                                                 */
+    int32_t n_kv_heads;      /* Hkv; Hq % Hkv == 0; G = Hq / Hkv (grouped-query attention, L258)   */
+    int32_t head_dim;        /* D in {64, 128}                                                     */
+    int32_t block_size;      /* tokens per KV block; 16 (L149: "S=16 -- one KV block") unless
+                                METRONOME_FLAG_BOOKKEEPING_ONLY                                    */
+    int32_t n_sinks;         /* S >= 0: pinned attention-sink tokens (L101)                        */
+    int32_t window;          /* W >= 1: most recent tokens kept, the query's own included          */
+    int32_t max_sessions;    /* session slots, 1..65536                                            */
+    int32_t max_new_tokens;  /* largest n_new of one session in one append_kv (chunk length)       */
+    int32_t n_blocks;        /* size of the fixed KV block pool (L60)                              */
+    float   softmax_scale;   /* 0 -> 1/sqrt(D)                                                     */
+    uint32_t flags;          /* METRONOME_FLAG_*                                                   */
+    int64_t max_session_len; /* 0 -> 2^31 - 1 - max_new_tokens; longer appends: LEN_OVERFLOW       */
+    void*   kv_storage;      /* device; NULL -> the pool allocates metronome_kv_storage_bytes()    */
+    size_t  kv_storage_bytes;/* size of kv_storage when provided                                   */
+} metronome_pool_config_t;
+
+typedef struct metronome_pool metronome_pool_t; /* opaque */
+
+/* ---- pool ----------------------------------------------------------------------------------- */
+
+/* Bytes of device memory the KV storage of `cfg` needs:
+ * n_layers * n_blocks * n_kv_heads * 2 (K,V) * block_size * head_dim * 2.  0 if cfg is invalid. */
+size_t metronome_kv_storage_bytes(const metronome_pool_config_t* cfg);
+
+/* Worst-case resident blocks of one session: ceil(S/B) + floor((W + max_new_tokens - 1)/B) + 2.
+ * (L258: "the per-request admission cap counts the pinned blocks so pool sizing stays exact".)
+ * Returns -1 on invalid arguments. */
+int32_t metronome_max_blocks_per_session(int32_t S, int32_t W, int32_t B, int32_t max_new_tokens);
+
+/* Creates a pool on the current CUDA device.  cfg: host.  *out receives the handle.
+ * The free list is a LIFO stack whose initial pop order is 0,1,2,...  (reading R6).
+ * Errors: INVALID_ARG, OUT_OF_MEMORY, CUDA. */
+int metronome_pool_create(const metronome_pool_config_t* cfg, metronome_pool_t** out);
+
+/* Frees everything the pool owns (synchronises the device first).  NULL is a no-op. */
+int metronome_pool_destroy(metronome_pool_t* pool);
+
+/* ---- sessions (L52: a session is one long-lived resident request) ----------------------------- */
+
+/* Claims the LOWEST free session slot; len = 0, no blocks.  *sid_out: host.  No device work.
+ * Errors: SESSIONS_FULL. */
+int metronome_session_open(metronome_pool_t* pool, int32_t* sid_out);
+
+/* Returns all blocks of `sid` to the free list (sink blocks, then live window blocks, ascending
+ * logical order) and releases the slot.  Asynchronous on cuda_stream.
+ * Errors: INVALID_SESSION, CUDA. */
+int metronome_session_close(metronome_pool_t* pool, int32_t sid, void* cuda_stream);
+
+/* ---- the per-frame hot path (L46: "prefill the new chunk, then decode up to tau output tokens,
+ *      attending over the session's accumulated context ... for all due sessions each tick") ---- */
+
+/* Appends n_new[i] tokens to session sids[i], i = 0..n_batch-1 (batch order matters, reading R6).
+ *   sids, n_new : host int32 [n_batch]; each session at most once; 0 <= n_new[i] <= max_new_tokens
+ *   k_new,v_new : device bf16 [sum(n_new), n_kv_heads, head_dim], rows in batch order
+ *   layer == 0  : bookkeeping, then the K/V write:
+ *       phase 1  every session frees its non-sink blocks that lie ENTIRELY behind the window of
+ *                position L0 (its length before this call) -- block b is freed iff b >= ceil(S/B)
+ *                and (b+1)*B <= L0-W+1 (L256: "frees blocks that fall entirely behind the window";
+ *                L258: "pins each request's first ceil(S/block) blocks instead of freeing them");
+ *       check    free + freed >= needed, else POOL_EXHAUSTED and nothing has changed;
+ *       phase 2  every session pops ceil(L1/B) - ceil(L0/B) blocks, ascending logical order.
+ *   layer  > 0  : must repeat layer 0's most recent batch exactly; only writes K/V of that layer.
+ * Errors: INVALID_ARG, INVALID_SESSION, DUPLICATE_SESSION, CHUNK_TOO_LARGE, LEN_OVERFLOW,
+ *         POOL_EXHAUSTED, LAYER_SEQUENCE, CUDA. */
+int metronome_append_kv(metronome_pool_t* pool, int32_t layer, int32_t n_batch,
+                        const int32_t* sids, const int32_t* n_new,
+                        const void* k_new, const void* v_new, void* cuda_stream);
+
+/* Attention of the LAST q_lens[i] positions of session sids[i] over its resident keys under
+ *   admit(j,t) = (j <= t) and (j < S or t - j < W)        (L103, L258; window = W keys incl. t)
+ *   out[t,h] = softmax_j(scale * <q[t,h], k[j,h/G]>) . v[j,h/G]      fp32 accumulate, bf16 out
+ * decode: q_len 1; chunk prefill: q_len n (causal inside the chunk).  One call may mix both (L258).
+ *   sids, q_lens : host int32 [n_batch]; 0 <= q_lens[i] <= n_new of that session's last append
+ *   q, out       : device bf16 [sum(q_lens), n_q_heads, head_dim], rows in batch order
+ * The layer must have been appended in the current step (since the last layer-0 append).
+ * Errors: INVALID_ARG, INVALID_SESSION, DUPLICATE_SESSION, QLEN_EXCEEDS_LAST_APPEND,
+ *         LAYER_SEQUENCE, UNSUPPORTED, CUDA. */
+int metronome_attend_frame(metronome_pool_t* pool, int32_t layer, int32_t n_batch,
+                           const int32_t* sids, const int32_t* q_lens,
+                           const void* q, void* out, void* cuda_stream);
+
+/* append_kv followed by attend_frame(q_lens = n_new) with HOST buffers: k_new, v_new, q are copied
+ * host->device, out device->host, all on cuda_stream, and the stream is synchronised before
+ * returning.  Pinned (page-locked) host memory makes the copies asynchronous.  This is the
+ * end-to-end entry point bench.py's `e2e` leg times.  Errors: union of the two calls. */
+int metronome_step_host(metronome_pool_t* pool, int32_t layer, int32_t n_batch,
+                        const int32_t* sids, const int32_t* n_new,
+                        const void* k_new_host, const void* v_new_host,
+                        const void* q_host, void* out_host, void* cuda_stream);
+
+/* ---- introspection (bit-exact parity of tables and free list; occupancy signal, L83) ---------- */
+
+/* All out-pointers are host and optional (NULL = skip).  Blocks the host until cuda_stream has
+ * finished the pool's earlier work.  block_ids receives the resident physical ids in logical order
+ * (sink blocks first); room for metronome_max_blocks_per_session() entries is required.
+ * first_live_block = first logical non-sink block still resident.  Errors: INVALID_SESSION, CUDA. */
+int metronome_session_query(metronome_pool_t* pool, int32_t sid, void* cuda_stream, int64_t* len,
+                            int32_t* first_live_block, int32_t* n_blocks, int32_t* block_ids);
+
+/* n_free and the free ids in POP order (next allocation first); free_ids needs n_blocks entries. */
+int metronome_pool_query(metronome_pool_t* pool, void* cuda_stream, int32_t* n_free, int32_t* free_ids);
+
+/* Reads back, through the block table, K and V rows of positions [pos0, pos0+n) of `sid` in
+ * `layer` into device bf16 [n, n_kv_heads, head_dim] buffers (verification of the KV write).
+ * Positions whose block is not resident return bf16 NaN.  Errors: INVALID_*, UNSUPPORTED, CUDA. */
+int metronome_read_kv(metronome_pool_t* pool, int32_t layer, int32_t sid, int64_t pos0, int32_t n,
+                      void* k_out, void* v_out, void* cuda_stream);
+
+/* Counters since pool_create: kernels launched by the library, append / attend calls.  host. */
+int metronome_pool_stats(metronome_pool_t* pool, int64_t* kernel_launches, int64_t* append_calls,
+                         int64_t* attend_calls);
+
+/* Tuning knob (0 = automatic): keys per split-KV segment target, and forcing the kernel family
+ * (0 auto, 1 CUDA-core row kernel, 2 tensor-core tile kernel).  For benchmarks and tests of "both
+ * launch modes" (L258).  Errors: INVALID_ARG. */
+int metronome_pool_set_tuning(metronome_pool_t* pool, int32_t split_tokens, int32_t kernel_family);
+
+const char* metronome_strerror(int status);
+/* Text of the last CUDA error seen by this pool ("" if none).  Valid until the next call. */
+const char* metronome_last_cuda_error(metronome_pool_t* pool);
+int metronome_abi_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* METRONOME_H_ */

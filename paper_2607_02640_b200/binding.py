@@ -1,0 +1,194 @@
+"""Thin ctypes mirror of include/metronome.h -- argument marshalling only.
+
+Every step of the path runs in libmetronome.so's CUDA kernels; torch is used by callers for device
+memory and streams.  There is NO fallback: if the library is missing or a call fails, this raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from ctypes import POINTER, byref, c_char_p, c_float, c_int, c_int32, c_int64, c_size_t, c_uint32, c_void_p
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libmetronome.so")
+
+FLAG_POISON_ON_FREE = 0x1
+FLAG_BOOKKEEPING_ONLY = 0x2
+FLAG_UNBOUNDED = 0x4
+
+ERR_NAMES = {0: "OK", 1: "INVALID_ARG", 2: "INVALID_SESSION", 3: "DUPLICATE_SESSION", 4: "SESSIONS_FULL",
+             5: "POOL_EXHAUSTED", 6: "CHUNK_TOO_LARGE", 7: "QLEN_EXCEEDS_LAST_APPEND", 8: "LAYER_SEQUENCE",
+             9: "LEN_OVERFLOW", 10: "CUDA", 11: "UNSUPPORTED", 12: "OUT_OF_MEMORY"}
+
+# every symbol include/metronome.h declares
+EXPORTS = ["metronome_abi_version", "metronome_strerror", "metronome_last_cuda_error",
+           "metronome_kv_storage_bytes", "metronome_max_blocks_per_session", "metronome_pool_create",
+           "metronome_pool_destroy", "metronome_session_open", "metronome_session_close",
+           "metronome_append_kv", "metronome_attend_frame", "metronome_step_host",
+           "metronome_session_query", "metronome_pool_query", "metronome_read_kv", "metronome_pool_stats",
+           "metronome_pool_set_tuning"]
+
+
+class MetronomeError(RuntimeError):
+    def __init__(self, status: int, detail: str = ""):
+        self.status = status
+        self.code = ERR_NAMES.get(status, f"UNKNOWN_{status}")
+        super().__init__(f"{self.code}" + (f": {detail}" if detail else ""))
+
+
+class PoolConfig(ctypes.Structure):
+    _fields_ = [("n_layers", c_int32), ("n_q_heads", c_int32), ("n_kv_heads", c_int32), ("head_dim", c_int32),
+                ("block_size", c_int32), ("n_sinks", c_int32), ("window", c_int32), ("max_sessions", c_int32),
+                ("max_new_tokens", c_int32), ("n_blocks", c_int32), ("softmax_scale", c_float), ("flags", c_uint32),
+                ("max_session_len", c_int64), ("kv_storage", c_void_p), ("kv_storage_bytes", c_size_t)]
+
+
+_lib = None
+
+
+def load():
+    """Loads libmetronome.so; fails loudly if it has not been built (no CPU fallback exists)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_2607_02640_b200.build` "
+                          "(or __graft_entry__.build()). There is no fallback path.")
+    lib = ctypes.CDLL(LIB_PATH)
+    i32p = POINTER(c_int32)
+    lib.metronome_abi_version.restype = c_int
+    lib.metronome_strerror.restype = c_char_p
+    lib.metronome_strerror.argtypes = [c_int]
+    lib.metronome_last_cuda_error.restype = c_char_p
+    lib.metronome_last_cuda_error.argtypes = [c_void_p]
+    lib.metronome_kv_storage_bytes.restype = c_size_t
+    lib.metronome_kv_storage_bytes.argtypes = [POINTER(PoolConfig)]
+    lib.metronome_max_blocks_per_session.restype = c_int32
+    lib.metronome_max_blocks_per_session.argtypes = [c_int32] * 4
+    lib.metronome_pool_create.argtypes = [POINTER(PoolConfig), POINTER(c_void_p)]
+    lib.metronome_pool_destroy.argtypes = [c_void_p]
+    lib.metronome_session_open.argtypes = [c_void_p, i32p]
+    lib.metronome_session_close.argtypes = [c_void_p, c_int32, c_void_p]
+    lib.metronome_append_kv.argtypes = [c_void_p, c_int32, c_int32, i32p, i32p, c_void_p, c_void_p, c_void_p]
+    lib.metronome_attend_frame.argtypes = [c_void_p, c_int32, c_int32, i32p, i32p, c_void_p, c_void_p, c_void_p]
+    lib.metronome_step_host.argtypes = [c_void_p, c_int32, c_int32, i32p, i32p, c_void_p, c_void_p, c_void_p,
+                                        c_void_p, c_void_p]
+    lib.metronome_session_query.argtypes = [c_void_p, c_int32, c_void_p, POINTER(c_int64), i32p, i32p, i32p]
+    lib.metronome_pool_query.argtypes = [c_void_p, c_void_p, i32p, i32p]
+    lib.metronome_read_kv.argtypes = [c_void_p, c_int32, c_int32, c_int64, c_int32, c_void_p, c_void_p, c_void_p]
+    lib.metronome_pool_stats.argtypes = [c_void_p, POINTER(c_int64), POINTER(c_int64), POINTER(c_int64)]
+    lib.metronome_pool_set_tuning.argtypes = [c_void_p, c_int32, c_int32]
+    _lib = lib
+    return lib
+
+
+def max_blocks_per_session(S: int, W: int, B: int, max_new_tokens: int) -> int:
+    return int(load().metronome_max_blocks_per_session(S, W, B, max_new_tokens))
+
+
+def _i32(a):
+    a = np.ascontiguousarray(a, dtype=np.int32)
+    return a, a.ctypes.data_as(POINTER(c_int32))
+
+
+def _ptr(t):
+    """torch tensor (device or pinned host) or raw integer address -> c_void_p."""
+    if t is None:
+        return None
+    if isinstance(t, int):
+        return c_void_p(t)
+    return c_void_p(t.data_ptr())
+
+
+class Pool:
+    """metronome_pool_t with the header's entry points (same names, same argument order)."""
+
+    def __init__(self, *, n_q_heads, n_kv_heads, head_dim, n_sinks, window, n_blocks, max_sessions,
+                 max_new_tokens, n_layers=1, block_size=16, softmax_scale=0.0, flags=0, max_session_len=0,
+                 kv_storage=None, kv_storage_bytes=0):
+        self._lib = load()
+        self._h = c_void_p()
+        self.cfg = PoolConfig(n_layers, n_q_heads, n_kv_heads, head_dim, block_size, n_sinks, window, max_sessions,
+                              max_new_tokens, n_blocks, softmax_scale, flags, max_session_len,
+                              kv_storage, kv_storage_bytes)
+        self._check(self._lib.metronome_pool_create(byref(self.cfg), byref(self._h)))
+        if flags & FLAG_UNBOUNDED:
+            self.max_blocks = (max_session_len + block_size - 1) // block_size + 1
+        else:
+            self.max_blocks = max_blocks_per_session(n_sinks, window, block_size, max_new_tokens)
+
+    def _check(self, status):
+        if status != 0:
+            detail = ""
+            if status == 10 and self._h:
+                detail = self._lib.metronome_last_cuda_error(self._h).decode()
+            raise MetronomeError(status, detail)
+
+    def kv_storage_bytes(self) -> int:
+        return int(self._lib.metronome_kv_storage_bytes(byref(self.cfg)))
+
+    def destroy(self):
+        if getattr(self, "_h", None):
+            self._lib.metronome_pool_destroy(self._h)
+            self._h = c_void_p()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def session_open(self) -> int:
+        sid = c_int32(-1)
+        self._check(self._lib.metronome_session_open(self._h, byref(sid)))
+        return sid.value
+
+    def session_close(self, sid: int, stream=0):
+        self._check(self._lib.metronome_session_close(self._h, sid, c_void_p(stream)))
+
+    def append_kv(self, layer, sids, n_new, k_new, v_new, stream=0):
+        s, sp = _i32(sids)
+        n, np_ = _i32(n_new)
+        self._check(self._lib.metronome_append_kv(self._h, layer, len(s), sp, np_, _ptr(k_new), _ptr(v_new),
+                                                  c_void_p(stream)))
+
+    def attend_frame(self, layer, sids, q_lens, q, out, stream=0):
+        s, sp = _i32(sids)
+        n, np_ = _i32(q_lens)
+        self._check(self._lib.metronome_attend_frame(self._h, layer, len(s), sp, np_, _ptr(q), _ptr(out),
+                                                     c_void_p(stream)))
+
+    def step_host(self, layer, sids, n_new, k_host, v_host, q_host, out_host, stream=0):
+        s, sp = _i32(sids)
+        n, np_ = _i32(n_new)
+        self._check(self._lib.metronome_step_host(self._h, layer, len(s), sp, np_, _ptr(k_host), _ptr(v_host),
+                                                  _ptr(q_host), _ptr(out_host), c_void_p(stream)))
+
+    def session_query(self, sid, stream=0):
+        """-> (len, first_live_block, [physical block ids in logical order])"""
+        ln, fl, nb = c_int64(), c_int32(), c_int32()
+        ids = (c_int32 * max(1, self.max_blocks))()
+        self._check(self._lib.metronome_session_query(self._h, sid, c_void_p(stream), byref(ln), byref(fl),
+                                                      byref(nb), ids))
+        return ln.value, fl.value, [ids[i] for i in range(nb.value)]
+
+    def pool_query(self, stream=0, want_ids=True):
+        """-> (n_free, [free ids in pop order])"""
+        nf = c_int32()
+        ids = (c_int32 * max(1, self.cfg.n_blocks))() if want_ids else None
+        self._check(self._lib.metronome_pool_query(self._h, c_void_p(stream), byref(nf), ids))
+        return nf.value, ([ids[i] for i in range(nf.value)] if want_ids else None)
+
+    def read_kv(self, layer, sid, pos0, n, k_out, v_out, stream=0):
+        self._check(self._lib.metronome_read_kv(self._h, layer, sid, pos0, n, _ptr(k_out), _ptr(v_out),
+                                                c_void_p(stream)))
+
+    def stats(self):
+        a, b, c = c_int64(), c_int64(), c_int64()
+        self._check(self._lib.metronome_pool_stats(self._h, byref(a), byref(b), byref(c)))
+        return {"kernel_launches": a.value, "append_calls": b.value, "attend_calls": c.value}
+
+    def set_tuning(self, split_tokens=0, kernel_family=0):
+        self._check(self._lib.metronome_pool_set_tuning(self._h, split_tokens, kernel_family))

@@ -1,0 +1,105 @@
+// attend_common.cuh -- work-list item, small device helpers and the split merge (rows a6, a8).
+#pragma once
+#include <cuda_bf16.h>
+
+#include "layout.cuh"
+
+namespace metronome {
+
+// One batch item of an attend_frame call, filled by the host from its shadow counts (row a8).
+// A "tile" is one resident KV block (16 tokens) of the session: first the pinned sink blocks,
+// then the window blocks that hold any key some query of this call may attend
+// ("the tile loop gains ceil(S/tile) extra leading iterations remapped onto the
+// sink tiles ... in segmented-decode mode only segment 0 takes them").
+struct AttendItem {
+    int32_t sid;
+    int32_t len;              // session length (the newest query sits at len-1)
+    int32_t q_len;            // queries = positions len-q_len .. len-1
+    int32_t q_row_off;        // exclusive prefix sum of q_len (row of this item's first query)
+    int32_t n_sink_tiles;     // min(ceil(S/16), ceil(len/16))
+    int32_t first_blk;        // first window logical block needed (>= ceil(S/16))
+    int32_t n_tiles;          // n_sink_tiles + window tiles
+    int32_t n_splits;         // split-KV segments of this item
+    int32_t split_off;        // exclusive prefix sum of n_splits (first CTA of this item)
+    int32_t tiles_per_split;
+    int32_t pad0, pad1;
+};
+
+struct AttendParams {
+    const AttendItem* items;
+    int32_t n_items;
+    const int32_t* table;
+    int32_t tbl_width, n_sink, ring;
+    const __nv_bfloat16* q;
+    __nv_bfloat16* out;
+    const uint8_t* kv_layer;
+    KvLayout L;
+    int32_t S, W;             // sinks, window (W = INT32_MAX/2 in the unbounded arm)
+    float scale_log2;         // softmax_scale * log2(e): scores live in the log2 domain
+    int32_t Hq, G;
+    float* ws_acc;            // [row][Hq][max_splits][D]   unnormalised partial outputs
+    float* ws_ml;             // [row][Hq][max_splits][2]   running max (log2 domain), running sum
+    int32_t max_splits;
+};
+
+__device__ __forceinline__ float ex2(float x) {
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// largest i in [0,n) with key(items[i]) <= x, keys ascending and key(items[0]) == 0
+template <typename F>
+__device__ __forceinline__ int32_t find_item(int32_t n, int32_t x, F key) {
+    int32_t lo = 0, hi = n - 1;
+    while (lo < hi) {
+        const int32_t mid = (lo + hi + 1) >> 1;
+        if (key(mid) <= x) lo = mid; else hi = mid - 1;
+    }
+    return lo;
+}
+
+// admit(j,t) = j<=t and (j<S or t-j<W)   PAPER.md:L103, L258 (window = W keys including t)
+__device__ __forceinline__ bool admit(int32_t j, int32_t t, int32_t S, int32_t W) {
+    return j <= t && (j < S || t - j < W);
+}
+
+__device__ __forceinline__ float bf16lo(uint32_t x) { return __uint_as_float(x << 16); }
+__device__ __forceinline__ float bf16hi(uint32_t x) { return __uint_as_float(x & 0xFFFF0000u); }
+
+__device__ __forceinline__ uint32_t pack_bf16(float a, float b) {
+    __nv_bfloat162 v = __floats2bfloat162_rn(a, b);
+    return *reinterpret_cast<uint32_t*>(&v);
+}
+
+// Row a6: log-sum-exp combine of the split-KV partials of one (query row, q head); sinks were
+// counted once, by segment 0 ("merged exactly once").
+// grid = (total_rows, Hq), block = D/4 threads.
+template <int D>
+__global__ void __launch_bounds__(D / 4)
+merge_kernel(AttendParams p) {
+    const int32_t row = blockIdx.x, h = blockIdx.y;
+    const int32_t i = find_item(p.n_items, row, [&](int32_t k) { return p.items[k].q_row_off; });
+    const int32_t ns = p.items[i].n_splits;
+    if (ns <= 1) return;      // the attention kernel already wrote the final output
+    const int64_t base = ((int64_t)row * p.Hq + h) * p.max_splits;
+    float M = -INFINITY;
+    for (int s = 0; s < ns; ++s) M = fmaxf(M, p.ws_ml[(base + s) * 2]);
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+    float l = 0.f;
+    for (int s = 0; s < ns; ++s) {
+        const float m = p.ws_ml[(base + s) * 2];
+        if (m == -INFINITY) continue;                 // this segment admitted no key for this row
+        const float w = ex2(m - M);
+        l += w * p.ws_ml[(base + s) * 2 + 1];
+        const float4 a = reinterpret_cast<const float4*>(p.ws_acc + (base + s) * D)[threadIdx.x];
+        acc.x += w * a.x; acc.y += w * a.y; acc.z += w * a.z; acc.w += w * a.w;
+    }
+    const float inv = l > 0.f ? 1.f / l : 0.f;
+    uint2 o;
+    o.x = pack_bf16(acc.x * inv, acc.y * inv);
+    o.y = pack_bf16(acc.z * inv, acc.w * inv);
+    reinterpret_cast<uint2*>(p.out + ((int64_t)row * p.Hq + h) * D)[threadIdx.x] = o;
+}
+
+}  // namespace metronome

@@ -1,0 +1,183 @@
+// attend_rows.cuh -- row a5: split-KV flash-decoding over sink + window blocks on CUDA cores.
+//
+// One CTA = one (split-KV segment, q head, query row).  It is THE kernel for multi-head decode
+// (G = 1, q_len = 1: BASELINE.json config 2), where the work is a pure HBM stream at 1 flop/byte
+// and tensor cores have nothing to contract; for G > 1 or q_len > 1 it is the general
+// (re-reading) fallback behind the tensor-core tile kernel in attend_mma.cuh.
+//
+// Mapping (D = 128): a K/V row of 256 bytes is read by 16 lanes x 16 bytes, so a warp covers two
+// tokens per step and one 16-token tile in 8 steps; all 16 loads of a tile (8 K + 8 V, 16 bytes
+// per lane each = 8 KiB per warp) are issued before the first use, which with 4 warps per CTA and
+// several CTAs per SM keeps far more than the ~44 KiB/SM in flight that 6.5 TB/s at ~1 us needs.
+// Score = 8 FMAs per lane + a 4-step xor-shuffle reduction over the 16 lanes of a token
+// ("warp-shuffle softmax", north_star); online softmax per half-warp in the log2 domain; the
+// halves, then the 4 warps, are combined once at the end.  The four warps take tiles
+// round-robin, so there is no barrier inside the tile loop.
+#pragma once
+#include "attend_common.cuh"
+
+namespace metronome {
+
+__device__ __forceinline__ void merge_state(float& m, float& l, float (&acc)[8], float m2, float l2,
+                                            const float (&acc2)[8]) {
+    const float M = fmaxf(m, m2);
+    if (M == -INFINITY) return;
+    const float a = ex2(m - M), b = ex2(m2 - M);   // ex2(-inf) = 0
+    l = l * a + l2 * b;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) acc[i] = acc[i] * a + acc2[i] * b;
+    m = M;
+}
+
+// grid = (total_splits, Hq, max_q_len), block = 128
+template <int D>
+__global__ void __launch_bounds__(128)
+attend_rows_kernel(AttendParams p) {
+    constexpr int LPT = D / 8;         // lanes per token (16-byte chunks per row)
+    constexpr int TPS = 32 / LPT;      // tokens per warp step
+    constexpr int STEPS = kBlockTokens / TPS;
+    const int32_t i = find_item(p.n_items, (int32_t)blockIdx.x, [&](int32_t k) { return p.items[k].split_off; });
+    const AttendItem it = p.items[i];
+    const int32_t r = blockIdx.z;
+    if (r >= it.q_len) return;
+    const int32_t split = blockIdx.x - it.split_off;
+    const int32_t h = blockIdx.y, kvh = h / p.G;
+    const int32_t t = it.len - it.q_len + r;          // absolute position of this query (reading R2)
+    const int32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int32_t sub = lane % LPT, grp = lane / LPT;
+    const int64_t qrow = (int64_t)(it.q_row_off + r) * p.Hq + h;
+
+    float qf[8];
+    {
+        const uint4 qv = *reinterpret_cast<const uint4*>(p.q + qrow * D + sub * 8);
+        const uint32_t w[4] = {qv.x, qv.y, qv.z, qv.w};
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            qf[2 * k] = bf16lo(w[k]) * p.scale_log2;
+            qf[2 * k + 1] = bf16hi(w[k]) * p.scale_log2;
+        }
+    }
+
+    float m = -INFINITY, l = 0.f, acc[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) acc[k] = 0.f;
+
+    const int32_t* trow = p.table + (int64_t)it.sid * p.tbl_width;
+    const int32_t tl0 = split * it.tiles_per_split;
+    const int32_t tl1 = min(it.n_tiles, tl0 + it.tiles_per_split);
+
+    for (int32_t tile = tl0 + warp; tile < tl1; tile += 4) {
+        const int32_t blk = tile < it.n_sink_tiles ? tile : it.first_blk + (tile - it.n_sink_tiles);
+        const int32_t p0 = blk * kBlockTokens;
+        // tiles with no admitted key for this row (later chunk rows leave early window tiles behind;
+        // earlier chunk rows do not see the newest tile): warp-uniform skip
+        if (p0 > t || (p0 >= p.S && t - (p0 + kBlockTokens - 1) >= p.W)) continue;
+        const int32_t phys = __ldg(trow + table_slot(blk, p.n_sink, p.ring));
+        const uint8_t* kt = p.kv_layer + (int64_t)phys * p.L.block_bytes + (int64_t)kvh * p.L.head_bytes;
+        const uint8_t* vt = kt + p.L.tile_bytes;
+        uint4 kr[STEPS], vr[STEPS];
+#pragma unroll
+        for (int j = 0; j < STEPS; ++j) {
+            const int32_t off = tile_chunk_offset(j * TPS + grp, sub);
+            kr[j] = __ldg(reinterpret_cast<const uint4*>(kt + off));
+            vr[j] = __ldg(reinterpret_cast<const uint4*>(vt + off));
+        }
+        float s[STEPS];
+#pragma unroll
+        for (int j = 0; j < STEPS; ++j) {
+            const uint32_t w[4] = {kr[j].x, kr[j].y, kr[j].z, kr[j].w};
+            float d = 0.f;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                d = fmaf(qf[2 * k], bf16lo(w[k]), d);
+                d = fmaf(qf[2 * k + 1], bf16hi(w[k]), d);
+            }
+#pragma unroll
+            for (int o = LPT / 2; o >= 1; o >>= 1) d += __shfl_xor_sync(0xffffffffu, d, o);
+            s[j] = d;
+        }
+        const bool full = (p0 + kBlockTokens - 1 <= t) &&
+                          (p0 + kBlockTokens - 1 < p.S || t - p0 < p.W);
+        if (!full) {
+            // boundary tile: token-exact mask; rows that are not admitted may hold stale or
+            // poisoned bytes (0 * NaN = NaN), so their V is zeroed, not multiplied by p = 0
+#pragma unroll
+            for (int j = 0; j < STEPS; ++j) {
+                const int32_t pos = p0 + j * TPS + grp;
+                if (!admit(pos, t, p.S, p.W)) {
+                    s[j] = -INFINITY;
+                    vr[j] = make_uint4(0u, 0u, 0u, 0u);
+                }
+            }
+        }
+        float tmax = s[0];
+#pragma unroll
+        for (int j = 1; j < STEPS; ++j) tmax = fmaxf(tmax, s[j]);
+        const float mn = fmaxf(m, tmax);
+        if (mn != -INFINITY) {            // (uniform inside a token group)
+            const float corr = ex2(m - mn);
+            l *= corr;
+#pragma unroll
+            for (int k = 0; k < 8; ++k) acc[k] *= corr;
+#pragma unroll
+            for (int j = 0; j < STEPS; ++j) {
+                const float pj = ex2(s[j] - mn);
+                l += pj;
+                const uint32_t w[4] = {vr[j].x, vr[j].y, vr[j].z, vr[j].w};
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    acc[2 * k] = fmaf(pj, bf16lo(w[k]), acc[2 * k]);
+                    acc[2 * k + 1] = fmaf(pj, bf16hi(w[k]), acc[2 * k + 1]);
+                }
+            }
+            m = mn;
+        }
+    }
+
+    // combine the token groups of the warp
+#pragma unroll
+    for (int o = 16; o >= LPT; o >>= 1) {
+        const float m2 = __shfl_xor_sync(0xffffffffu, m, o);
+        const float l2 = __shfl_xor_sync(0xffffffffu, l, o);
+        float a2[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) a2[k] = __shfl_xor_sync(0xffffffffu, acc[k], o);
+        merge_state(m, l, acc, m2, l2, a2);
+    }
+    // combine the 4 warps
+    __shared__ float sm_m[4], sm_l[4], sm_acc[4][D];
+    if (lane < LPT) {
+        if (sub == 0) { sm_m[warp] = m; sm_l[warp] = l; }
+#pragma unroll
+        for (int k = 0; k < 8; ++k) sm_acc[warp][sub * 8 + k] = acc[k];
+    }
+    __syncthreads();
+    if (threadIdx.x < LPT) {
+        m = sm_m[0]; l = sm_l[0];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) acc[k] = sm_acc[0][sub * 8 + k];
+        for (int w = 1; w < 4; ++w) {
+            float a2[8];
+#pragma unroll
+            for (int k = 0; k < 8; ++k) a2[k] = sm_acc[w][sub * 8 + k];
+            merge_state(m, l, acc, sm_m[w], sm_l[w], a2);
+        }
+        if (it.n_splits == 1) {
+            const float inv = l > 0.f ? 1.f / l : 0.f;
+            uint4 o;
+            o.x = pack_bf16(acc[0] * inv, acc[1] * inv);
+            o.y = pack_bf16(acc[2] * inv, acc[3] * inv);
+            o.z = pack_bf16(acc[4] * inv, acc[5] * inv);
+            o.w = pack_bf16(acc[6] * inv, acc[7] * inv);
+            *reinterpret_cast<uint4*>(p.out + qrow * D + sub * 8) = o;
+        } else {
+            const int64_t slot = qrow * p.max_splits + split;
+            float4* dst = reinterpret_cast<float4*>(p.ws_acc + slot * D + sub * 8);
+            dst[0] = make_float4(acc[0], acc[1], acc[2], acc[3]);
+            dst[1] = make_float4(acc[4], acc[5], acc[6], acc[7]);
+            if (sub == 0) { p.ws_ml[slot * 2] = m; p.ws_ml[slot * 2 + 1] = l; }
+        }
+    }
+}
+
+}  // namespace metronome

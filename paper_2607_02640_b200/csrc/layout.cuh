@@ -1,0 +1,54 @@
+// layout.cuh -- how the bounded KV cache is laid out in HBM.
+//
+// The pool owns the layout, so it is chosen for the kernels that stream it, not for the writer:
+//
+//   kv[layer][block][kv_head][K|V][half = d/64][row = token%16][64 bf16, 16-byte chunks XOR-swizzled]
+//
+// * One (block, kv_head) = K tile + V tile = 2 * 16 * D * 2 bytes, CONTIGUOUS (8 KiB at D=128): the
+//   unit a decode CTA streams; one bulk async copy (UBLKCP) or 512 coalesced 16-byte loads.
+// * Inside a tile, a "half" is 16 rows x 128 bytes.  The 16-byte chunk c (0..7) of row r is stored at
+//   chunk position c ^ (r & 7).  That is exactly the 128-byte-swizzle, K-major shared-memory layout
+//   of sm_100 UMMA descriptors and what makes `ldmatrix` conflict-free, so a LINEAR copy
+//   HBM -> shared memory lands a tile already swizzled: no tensor map, no re-layout pass.
+// * A token row is two 128-byte segments (one per half); the append kernel writes 16-byte chunks.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace metronome {
+
+constexpr int kBlockTokens = 16;   // PAPER.md:L149 "S=16 -- one KV block"
+constexpr int kHalfDim = 64;       // 128-byte rows: the swizzle span
+
+struct KvLayout {
+    int32_t head_dim;       // D
+    int32_t n_kv_heads;     // Hkv
+    int64_t tile_bytes;     // 16 * D * 2          (K or V of one block-head)
+    int64_t head_bytes;     // 2 * tile_bytes      (K then V)
+    int64_t block_bytes;    // Hkv * head_bytes
+    int64_t layer_bytes;    // n_blocks * block_bytes
+};
+
+__host__ __device__ inline KvLayout make_layout(int32_t D, int32_t Hkv, int64_t n_blocks) {
+    KvLayout L;
+    L.head_dim = D;
+    L.n_kv_heads = Hkv;
+    L.tile_bytes = (int64_t)kBlockTokens * D * 2;
+    L.head_bytes = 2 * L.tile_bytes;
+    L.block_bytes = (int64_t)Hkv * L.head_bytes;
+    L.layer_bytes = n_blocks * L.block_bytes;
+    return L;
+}
+
+// Byte offset, inside a K or V tile, of 16-byte chunk `c` (0 .. D/8-1) of token row `r` (0..15).
+__host__ __device__ __forceinline__ int32_t tile_chunk_offset(int32_t r, int32_t c) {
+    return ((c >> 3) * (kBlockTokens * 128)) + r * 128 + (((c & 7) ^ (r & 7)) << 4);
+}
+
+// Slot of logical block `b` in a session's block table: the first n_sink entries are the pinned
+// sink blocks, the rest is a ring over the window blocks (pinned head, freed middle).
+__host__ __device__ __forceinline__ int32_t table_slot(int32_t b, int32_t n_sink, int32_t ring) {
+    return b < n_sink ? b : n_sink + (b - n_sink) % ring;
+}
+
+}  // namespace metronome

@@ -1,0 +1,691 @@
+// metronome.cu -- the C ABI of libmetronome.so (include/metronome.h) and its host-side state.
+//
+// Host state is "shadow counts" only: per session {open, len, first_live, last_n}, the free count,
+// and the last layer-0 batch.  They are pure functions of the call history, so every error is
+// raised synchronously and before anything changes, while the physical block ids (block tables,
+// free stack) live on the device and are only ever touched by kernels on the caller's stream.
+#include "../../include/metronome.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "attend_common.cuh"
+#include "attend_mma.cuh"
+#include "attend_rows.cuh"
+#include "bookkeeping.cuh"
+#include "kv_append.cuh"
+
+using namespace metronome;
+
+namespace {
+
+struct Session {
+    bool open = false;
+    int64_t len = 0;
+    int32_t first_live = 0;   // first logical non-sink block still resident
+    int32_t last_n = 0;       // n_new of this session's most recent append
+};
+
+constexpr int kStagingSlots = 16;
+constexpr int kMaxSplits = 64;
+
+}  // namespace
+
+struct metronome_pool {
+    metronome_pool_config_t cfg{};
+    int32_t n_sink = 0, tbl_width = 0, ring = 0, G = 1, W_eff = 0;
+    float scale = 0.f;
+    KvLayout L{};
+    bool bookkeeping_only = false, poison = false, unbounded = false, own_kv = false;
+
+    std::vector<Session> sessions;
+    std::vector<int32_t> stamp;        // duplicate detection
+    int32_t stamp_now = 0;
+    int32_t n_open = 0, n_free = 0;
+
+    int64_t epoch = 0;                 // number of layer-0 appends so far
+    std::vector<int64_t> layer_epoch;  // epoch of each layer's latest append
+    std::vector<int32_t> last_sids, last_n_new;
+
+    // device
+    int32_t* d_table = nullptr;
+    int32_t* d_free = nullptr;
+    uint8_t* d_kv = nullptr;
+    float* d_ws_acc = nullptr;
+    float* d_ws_ml = nullptr;
+    size_t ws_slots = 0;               // capacity in (row, head, split) slots
+    uint8_t* d_io = nullptr;           // staging for metronome_step_host
+    size_t io_bytes = 0;
+
+    // per-call metadata staging: pinned host ring + matching device ring
+    uint8_t* h_stage = nullptr;
+    uint8_t* d_stage = nullptr;
+    size_t slot_bytes = 0;
+    cudaEvent_t ev[kStagingSlots]{};
+    bool ev_used[kStagingSlots]{};
+    int next_slot = 0;
+
+    int32_t tune_split_tokens = 0, tune_family = 0;
+    int32_t n_sm = 148;
+    int64_t n_launch = 0, n_append = 0, n_attend = 0;
+    std::string cuda_err;
+};
+
+namespace {
+
+int cuda_fail(metronome_pool* p, cudaError_t e, const char* what) {
+    if (p) p->cuda_err = std::string(what) + ": " + cudaGetErrorString(e);
+    return METRONOME_ERR_CUDA;
+}
+#define CU(call)                                                     \
+    do {                                                             \
+        cudaError_t e_ = (call);                                     \
+        if (e_ != cudaSuccess) return cuda_fail(pool, e_, #call);    \
+    } while (0)
+
+bool valid_cfg(const metronome_pool_config_t* c) {
+    if (!c) return false;
+    const bool bk = c->flags & METRONOME_FLAG_BOOKKEEPING_ONLY;
+    if (c->n_layers < 1 || c->n_q_heads < 1 || c->n_kv_heads < 1 || c->n_q_heads % c->n_kv_heads) return false;
+    if (c->block_size < 1 || c->n_sinks < 0 || c->window < 1 || c->max_sessions < 1 || c->max_sessions > 65536)
+        return false;
+    if (c->max_new_tokens < 1 || c->n_blocks < 1 || c->max_session_len < 0) return false;
+    if (!bk && (c->block_size != kBlockTokens || (c->head_dim != 64 && c->head_dim != 128))) return false;
+    if ((c->flags & METRONOME_FLAG_UNBOUNDED) && c->max_session_len <= 0) return false;
+    if (!(c->softmax_scale >= 0.f)) return false;
+    return true;
+}
+
+// Stage `bytes` of per-call metadata: returns the host pointer to fill and the device pointer the
+// kernels will read; commit_stage() enqueues the copy.
+int acquire_stage(metronome_pool* pool, uint8_t** h, uint8_t** d, int* slot) {
+    const int s = pool->next_slot;
+    pool->next_slot = (s + 1) % kStagingSlots;
+    if (pool->ev_used[s]) CU(cudaEventSynchronize(pool->ev[s]));
+    *h = pool->h_stage + (size_t)s * pool->slot_bytes;
+    *d = pool->d_stage + (size_t)s * pool->slot_bytes;
+    *slot = s;
+    return METRONOME_OK;
+}
+int commit_stage(metronome_pool* pool, int slot, size_t bytes, cudaStream_t st) {
+    CU(cudaMemcpyAsync(pool->d_stage + (size_t)slot * pool->slot_bytes, pool->h_stage + (size_t)slot * pool->slot_bytes,
+                       bytes, cudaMemcpyHostToDevice, st));
+    CU(cudaEventRecord(pool->ev[slot], st));
+    pool->ev_used[slot] = true;
+    return METRONOME_OK;
+}
+
+int check_batch(metronome_pool* pool, int32_t n_batch, const int32_t* sids, const int32_t* counts) {
+    if (n_batch < 0 || n_batch > pool->cfg.max_sessions) return METRONOME_ERR_INVALID_ARG;
+    if (n_batch > 0 && (!sids || !counts)) return METRONOME_ERR_INVALID_ARG;
+    // duplicates first, then per-item checks (same precedence as the oracle)
+    if (++pool->stamp_now == INT32_MAX) {
+        std::fill(pool->stamp.begin(), pool->stamp.end(), 0);
+        pool->stamp_now = 1;
+    }
+    for (int i = 0; i < n_batch; ++i) {
+        const int32_t s = sids[i];
+        if (s < 0 || s >= pool->cfg.max_sessions) continue;
+        if (pool->stamp[s] == pool->stamp_now) return METRONOME_ERR_DUPLICATE_SESSION;
+        pool->stamp[s] = pool->stamp_now;
+    }
+    for (int i = 0; i < n_batch; ++i) {
+        const int32_t s = sids[i];
+        if (s < 0 || s >= pool->cfg.max_sessions || !pool->sessions[s].open) return METRONOME_ERR_INVALID_SESSION;
+        if (counts[i] < 0) return METRONOME_ERR_INVALID_ARG;
+    }
+    return METRONOME_OK;
+}
+
+int launch_kv_write(metronome_pool* pool, int32_t layer, const AppendItem* d_items, int32_t n_items,
+                    int32_t max_n, const void* k_new, const void* v_new, cudaStream_t st) {
+    if (max_n == 0 || n_items == 0) return METRONOME_OK;
+    const int32_t chunks = max_n * pool->cfg.n_kv_heads * (pool->cfg.head_dim / 8);
+    dim3 grid((chunks + 255) / 256, n_items);
+    kv_append_kernel<<<grid, 256, 0, st>>>(d_items, pool->d_table, pool->tbl_width, pool->n_sink, pool->ring,
+                                           (const uint4*)k_new, (const uint4*)v_new,
+                                           pool->d_kv + (int64_t)layer * pool->L.layer_bytes, pool->L);
+    ++pool->n_launch;
+    CU(cudaGetLastError());
+    return METRONOME_OK;
+}
+
+int ensure_workspace(metronome_pool* pool, size_t slots) {
+    if (slots <= pool->ws_slots) return METRONOME_OK;
+    // cudaFree synchronises the device, so kernels still reading the old workspace are done
+    if (pool->d_ws_acc) cudaFree(pool->d_ws_acc);
+    if (pool->d_ws_ml) cudaFree(pool->d_ws_ml);
+    pool->d_ws_acc = pool->d_ws_ml = nullptr;
+    pool->ws_slots = 0;
+    const size_t want = slots + slots / 4;
+    CU(cudaMalloc(&pool->d_ws_acc, want * pool->cfg.head_dim * sizeof(float)));
+    CU(cudaMalloc(&pool->d_ws_ml, want * 2 * sizeof(float)));
+    pool->ws_slots = want;
+    return METRONOME_OK;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------------
+extern "C" {
+
+int metronome_abi_version(void) { return METRONOME_ABI_VERSION; }
+
+const char* metronome_strerror(int status) {
+    switch (status) {
+        case METRONOME_OK: return "OK";
+        case METRONOME_ERR_INVALID_ARG: return "INVALID_ARG";
+        case METRONOME_ERR_INVALID_SESSION: return "INVALID_SESSION";
+        case METRONOME_ERR_DUPLICATE_SESSION: return "DUPLICATE_SESSION";
+        case METRONOME_ERR_SESSIONS_FULL: return "SESSIONS_FULL";
+        case METRONOME_ERR_POOL_EXHAUSTED: return "POOL_EXHAUSTED";
+        case METRONOME_ERR_CHUNK_TOO_LARGE: return "CHUNK_TOO_LARGE";
+        case METRONOME_ERR_QLEN_EXCEEDS_LAST_APPEND: return "QLEN_EXCEEDS_LAST_APPEND";
+        case METRONOME_ERR_LAYER_SEQUENCE: return "LAYER_SEQUENCE";
+        case METRONOME_ERR_LEN_OVERFLOW: return "LEN_OVERFLOW";
+        case METRONOME_ERR_CUDA: return "CUDA";
+        case METRONOME_ERR_UNSUPPORTED: return "UNSUPPORTED";
+        case METRONOME_ERR_OUT_OF_MEMORY: return "OUT_OF_MEMORY";
+        default: return "UNKNOWN";
+    }
+}
+
+const char* metronome_last_cuda_error(metronome_pool_t* pool) { return pool ? pool->cuda_err.c_str() : ""; }
+
+size_t metronome_kv_storage_bytes(const metronome_pool_config_t* c) {
+    if (!valid_cfg(c) || (c->flags & METRONOME_FLAG_BOOKKEEPING_ONLY)) return 0;
+    return (size_t)c->n_layers * c->n_blocks * c->n_kv_heads * 2 * c->block_size * c->head_dim * 2;
+}
+
+int32_t metronome_max_blocks_per_session(int32_t S, int32_t W, int32_t B, int32_t max_new_tokens) {
+    if (S < 0 || W < 1 || B < 1 || max_new_tokens < 1) return -1;
+    const int64_t v = (int64_t)((S + B - 1) / B) + ((int64_t)W + max_new_tokens - 1) / B + 2;
+    return v > INT32_MAX ? -1 : (int32_t)v;
+}
+
+int metronome_pool_create(const metronome_pool_config_t* cfg, metronome_pool_t** out) {
+    if (!out) return METRONOME_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!valid_cfg(cfg)) return METRONOME_ERR_INVALID_ARG;
+    metronome_pool* pool = new (std::nothrow) metronome_pool();
+    if (!pool) return METRONOME_ERR_OUT_OF_MEMORY;
+    pool->cfg = *cfg;
+    const metronome_pool_config_t& c = pool->cfg;
+    pool->bookkeeping_only = c.flags & METRONOME_FLAG_BOOKKEEPING_ONLY;
+    pool->poison = c.flags & METRONOME_FLAG_POISON_ON_FREE;
+    pool->unbounded = c.flags & METRONOME_FLAG_UNBOUNDED;
+    if (pool->cfg.max_session_len == 0) pool->cfg.max_session_len = (int64_t)INT32_MAX - c.max_new_tokens;
+    const int32_t B = c.block_size;
+    pool->n_sink = (c.n_sinks + B - 1) / B;
+    if (pool->unbounded) {
+        const int64_t blocks = (pool->cfg.max_session_len + B - 1) / B + 1;
+        if (blocks > (1 << 24)) { delete pool; return METRONOME_ERR_INVALID_ARG; }
+        pool->tbl_width = (int32_t)blocks;
+        pool->ring = pool->tbl_width;        // never wraps: slots are linear
+        pool->n_sink = 0;                    // nothing is pinned because nothing is freed
+        pool->W_eff = INT32_MAX / 2;
+    } else {
+        pool->tbl_width = metronome_max_blocks_per_session(c.n_sinks, c.window, B, c.max_new_tokens);
+        if (pool->tbl_width < 0) { delete pool; return METRONOME_ERR_INVALID_ARG; }
+        pool->ring = pool->tbl_width - pool->n_sink;
+        pool->W_eff = c.window;
+    }
+    pool->G = c.n_q_heads / c.n_kv_heads;
+    pool->scale = c.softmax_scale > 0.f ? c.softmax_scale : 1.0f / sqrtf((float)(c.head_dim > 0 ? c.head_dim : 1));
+    pool->sessions.assign(c.max_sessions, Session());
+    pool->stamp.assign(c.max_sessions, 0);
+    pool->layer_epoch.assign(c.n_layers, 0);
+    pool->n_free = c.n_blocks;
+
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&pool->n_sm, cudaDevAttrMultiProcessorCount, dev);
+    auto fail = [&](int code, cudaError_t ce, const char* what) {
+        if (code == METRONOME_ERR_CUDA) cuda_fail(pool, ce, what);
+        metronome_pool_destroy(pool);
+        return code;
+    };
+    if (e != cudaSuccess) return fail(METRONOME_ERR_CUDA, e, "cudaGetDevice");
+    e = cudaMalloc(&pool->d_table, (size_t)c.max_sessions * pool->tbl_width * sizeof(int32_t));
+    if (e != cudaSuccess) return fail(METRONOME_ERR_OUT_OF_MEMORY, e, "cudaMalloc table");
+    e = cudaMalloc(&pool->d_free, (size_t)c.n_blocks * sizeof(int32_t));
+    if (e != cudaSuccess) return fail(METRONOME_ERR_OUT_OF_MEMORY, e, "cudaMalloc free stack");
+    cudaMemset(pool->d_table, 0xFF, (size_t)c.max_sessions * pool->tbl_width * sizeof(int32_t));
+    if (!pool->bookkeeping_only) {
+        pool->L = make_layout(c.head_dim, c.n_kv_heads, c.n_blocks);
+        const size_t need = metronome_kv_storage_bytes(&pool->cfg);
+        if (c.kv_storage) {
+            if (c.kv_storage_bytes < need || ((uintptr_t)c.kv_storage & 127)) return fail(METRONOME_ERR_INVALID_ARG, e, "");
+            pool->d_kv = (uint8_t*)c.kv_storage;
+        } else {
+            e = cudaMalloc(&pool->d_kv, need);
+            if (e != cudaSuccess) return fail(METRONOME_ERR_OUT_OF_MEMORY, e, "cudaMalloc kv storage");
+            pool->own_kv = true;
+        }
+        if (pool->poison) fill_nan_kernel<<<1184, 256>>>((uint4*)pool->d_kv, (int64_t)(need / 16));
+    }
+    pool->slot_bytes = (size_t)c.max_sessions * (sizeof(AppendItem) > sizeof(AttendItem) ? sizeof(AppendItem) : sizeof(AttendItem));
+    e = cudaMallocHost(&pool->h_stage, pool->slot_bytes * kStagingSlots);
+    if (e != cudaSuccess) return fail(METRONOME_ERR_OUT_OF_MEMORY, e, "cudaMallocHost staging");
+    e = cudaMalloc(&pool->d_stage, pool->slot_bytes * kStagingSlots);
+    if (e != cudaSuccess) return fail(METRONOME_ERR_OUT_OF_MEMORY, e, "cudaMalloc staging");
+    for (int i = 0; i < kStagingSlots; ++i) {
+        e = cudaEventCreateWithFlags(&pool->ev[i], cudaEventDisableTiming);
+        if (e != cudaSuccess) return fail(METRONOME_ERR_CUDA, e, "cudaEventCreate");
+    }
+    init_free_stack_kernel<<<(c.n_blocks + 255) / 256, 256>>>(pool->d_free, c.n_blocks);
+    e = cudaDeviceSynchronize();
+    if (e != cudaSuccess) return fail(METRONOME_ERR_CUDA, e, "pool init kernels");
+    configure_attend_mma_kernels();
+    *out = pool;
+    return METRONOME_OK;
+}
+
+int metronome_pool_destroy(metronome_pool_t* pool) {
+    if (!pool) return METRONOME_OK;
+    cudaDeviceSynchronize();
+    if (pool->d_table) cudaFree(pool->d_table);
+    if (pool->d_free) cudaFree(pool->d_free);
+    if (pool->own_kv && pool->d_kv) cudaFree(pool->d_kv);
+    if (pool->d_ws_acc) cudaFree(pool->d_ws_acc);
+    if (pool->d_ws_ml) cudaFree(pool->d_ws_ml);
+    if (pool->d_io) cudaFree(pool->d_io);
+    if (pool->h_stage) cudaFreeHost(pool->h_stage);
+    if (pool->d_stage) cudaFree(pool->d_stage);
+    for (int i = 0; i < kStagingSlots; ++i)
+        if (pool->ev[i]) cudaEventDestroy(pool->ev[i]);
+    delete pool;
+    return METRONOME_OK;
+}
+
+int metronome_session_open(metronome_pool_t* pool, int32_t* sid_out) {
+    if (!pool || !sid_out) return METRONOME_ERR_INVALID_ARG;
+    if (pool->n_open >= pool->cfg.max_sessions) return METRONOME_ERR_SESSIONS_FULL;
+    for (int32_t s = 0; s < pool->cfg.max_sessions; ++s) {
+        if (!pool->sessions[s].open) {           // lowest free slot (reading R6)
+            Session& ss = pool->sessions[s];
+            ss.open = true; ss.len = 0; ss.first_live = pool->n_sink; ss.last_n = 0;
+            ++pool->n_open;
+            *sid_out = s;
+            return METRONOME_OK;
+        }
+    }
+    return METRONOME_ERR_SESSIONS_FULL;
+}
+
+int metronome_session_close(metronome_pool_t* pool, int32_t sid, void* cuda_stream) {
+    if (!pool) return METRONOME_ERR_INVALID_ARG;
+    if (sid < 0 || sid >= pool->cfg.max_sessions || !pool->sessions[sid].open) return METRONOME_ERR_INVALID_SESSION;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    Session& s = pool->sessions[sid];
+    const int32_t B = pool->cfg.block_size;
+    const int32_t n_blk = (int32_t)((s.len + B - 1) / B);
+    const int32_t n_sink_res = n_blk < pool->n_sink ? n_blk : pool->n_sink;
+    const int32_t n_win = n_blk > s.first_live ? n_blk - s.first_live : 0;
+    const int32_t cnt = n_sink_res + n_win;
+    if (cnt > 0) {
+        close_session_kernel<<<1, 256, 0, st>>>(pool->d_table + (int64_t)sid * pool->tbl_width, pool->n_sink, pool->ring,
+                                                n_sink_res, s.first_live, n_blk, pool->d_free, pool->n_free);
+        ++pool->n_launch;
+        CU(cudaGetLastError());
+        if (pool->poison && !pool->bookkeeping_only) {
+            poison_blocks_kernel<<<dim3(cnt, pool->cfg.n_layers), 256, 0, st>>>(pool->d_free, pool->n_free, pool->d_kv,
+                                                                               pool->L.block_bytes, pool->L.layer_bytes);
+            ++pool->n_launch;
+            CU(cudaGetLastError());
+        }
+    }
+    pool->n_free += cnt;
+    s = Session();
+    --pool->n_open;
+    // a closed session can no longer be part of a layer > 0 replay
+    pool->last_sids.clear(); pool->last_n_new.clear();
+    return METRONOME_OK;
+}
+
+int metronome_append_kv(metronome_pool_t* pool, int32_t layer, int32_t n_batch, const int32_t* sids,
+                        const int32_t* n_new, const void* k_new, const void* v_new, void* cuda_stream) {
+    if (!pool || layer < 0 || layer >= pool->cfg.n_layers) return METRONOME_ERR_INVALID_ARG;
+    int rc = check_batch(pool, n_batch, sids, n_new);
+    if (rc) return rc;
+    const metronome_pool_config_t& c = pool->cfg;
+    const int32_t B = c.block_size;
+    int64_t total_new = 0;
+    int32_t max_n = 0;
+    for (int i = 0; i < n_batch; ++i) {
+        if (n_new[i] > c.max_new_tokens) return METRONOME_ERR_CHUNK_TOO_LARGE;
+        if (pool->sessions[sids[i]].len + n_new[i] > c.max_session_len) return METRONOME_ERR_LEN_OVERFLOW;
+        total_new += n_new[i];
+        if (n_new[i] > max_n) max_n = n_new[i];
+    }
+    if (pool->bookkeeping_only ? (k_new || v_new) : (total_new > 0 && (!k_new || !v_new)))
+        return METRONOME_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+
+    if (layer > 0) {
+        // must repeat layer 0's batch of this step, once (reading R16)
+        if (pool->epoch == 0 || pool->layer_epoch[layer] >= pool->epoch || (int32_t)pool->last_sids.size() != n_batch ||
+            (n_batch && (memcmp(pool->last_sids.data(), sids, n_batch * sizeof(int32_t)) ||
+                         memcmp(pool->last_n_new.data(), n_new, n_batch * sizeof(int32_t)))))
+            return METRONOME_ERR_LAYER_SEQUENCE;
+    }
+
+    uint8_t *h = nullptr, *d = nullptr;
+    int slot = 0;
+    AppendItem* items = nullptr;
+    int32_t total_freed = 0, total_alloc = 0;
+    if (n_batch > 0) {
+        rc = acquire_stage(pool, &h, &d, &slot);
+        if (rc) return rc;
+        items = reinterpret_cast<AppendItem*>(h);
+        int32_t row = 0;
+        for (int i = 0; i < n_batch; ++i) {
+            const Session& s = pool->sessions[sids[i]];
+            AppendItem& it = items[i];
+            memset(&it, 0, sizeof(it));
+            it.sid = sids[i];
+            it.n_new = n_new[i];
+            it.row_off = row;
+            row += n_new[i];
+            if (layer == 0) {
+                const int64_t L0 = s.len, L1 = s.len + n_new[i];
+                it.len0 = (int32_t)L0;
+                int64_t new_first = s.first_live;
+                if (!pool->unbounded) {
+                    // block b is entirely behind the window of position L0 iff (b+1)*B <= L0-W+1 (L256);
+                    // the first ceil(S/B) blocks are pinned (L258)
+                    const int64_t behind = L0 - c.window + 1 > 0 ? (L0 - c.window + 1) / B : 0;
+                    if (behind > new_first) new_first = behind;
+                    if (pool->n_sink > new_first) new_first = pool->n_sink;
+                }
+                it.free_lo = s.first_live;
+                it.n_freed = (int32_t)(new_first - s.first_live);
+                it.free_off = total_freed;
+                it.alloc_lo = (int32_t)((L0 + B - 1) / B);
+                it.n_alloc = (int32_t)((L1 + B - 1) / B) - it.alloc_lo;
+                it.alloc_off = total_alloc;
+                total_freed += it.n_freed;
+                total_alloc += it.n_alloc;
+            } else {
+                it.len0 = (int32_t)(s.len - n_new[i]);
+            }
+        }
+    }
+    if (layer == 0) {
+        if (pool->n_free + total_freed < total_alloc) return METRONOME_ERR_POOL_EXHAUSTED;  // nothing changed
+        if (n_batch > 0) {
+            rc = commit_stage(pool, slot, (size_t)n_batch * sizeof(AppendItem), st);
+            if (rc) return rc;
+            if (total_freed + total_alloc > 0) {
+                bookkeeping_kernel<<<1, 512, 0, st>>>(reinterpret_cast<const AppendItem*>(d), n_batch, pool->d_table,
+                                                      pool->tbl_width, pool->n_sink, pool->ring, pool->d_free,
+                                                      pool->n_free, total_freed);
+                ++pool->n_launch;
+                CU(cudaGetLastError());
+            }
+            if (pool->poison && !pool->bookkeeping_only && total_freed > 0) {
+                poison_blocks_kernel<<<dim3(total_freed, c.n_layers), 256, 0, st>>>(pool->d_free, pool->n_free, pool->d_kv,
+                                                                                   pool->L.block_bytes, pool->L.layer_bytes);
+                ++pool->n_launch;
+                CU(cudaGetLastError());
+            }
+        }
+        // commit the shadow counts
+        for (int i = 0; i < n_batch; ++i) {
+            Session& s = pool->sessions[sids[i]];
+            s.first_live += items[i].n_freed;
+            s.len += n_new[i];
+            s.last_n = n_new[i];
+        }
+        pool->n_free += total_freed - total_alloc;
+        ++pool->epoch;
+        pool->layer_epoch[0] = pool->epoch;
+        pool->last_sids.assign(sids, sids + n_batch);
+        pool->last_n_new.assign(n_new, n_new + n_batch);
+    } else {
+        if (n_batch > 0) {
+            rc = commit_stage(pool, slot, (size_t)n_batch * sizeof(AppendItem), st);
+            if (rc) return rc;
+        }
+        pool->layer_epoch[layer] = pool->epoch;
+    }
+    ++pool->n_append;
+    if (!pool->bookkeeping_only && n_batch > 0)
+        return launch_kv_write(pool, layer, reinterpret_cast<const AppendItem*>(d), n_batch, max_n, k_new, v_new, st);
+    return METRONOME_OK;
+}
+
+int metronome_attend_frame(metronome_pool_t* pool, int32_t layer, int32_t n_batch, const int32_t* sids,
+                           const int32_t* q_lens, const void* q, void* out, void* cuda_stream) {
+    if (!pool || layer < 0 || layer >= pool->cfg.n_layers) return METRONOME_ERR_INVALID_ARG;
+    if (pool->bookkeeping_only) return METRONOME_ERR_UNSUPPORTED;
+    int rc = check_batch(pool, n_batch, sids, q_lens);
+    if (rc) return rc;
+    const metronome_pool_config_t& c = pool->cfg;
+    int64_t total_rows = 0;
+    for (int i = 0; i < n_batch; ++i) {
+        if (q_lens[i] > pool->sessions[sids[i]].last_n) return METRONOME_ERR_QLEN_EXCEEDS_LAST_APPEND;
+        total_rows += q_lens[i];
+    }
+    if (total_rows > 0 && (!q || !out)) return METRONOME_ERR_INVALID_ARG;
+    ++pool->n_attend;
+    if (total_rows == 0) return METRONOME_OK;
+    if (pool->epoch == 0 || pool->layer_epoch[layer] != pool->epoch) return METRONOME_ERR_LAYER_SEQUENCE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+
+    // ---- row a8: the per-call work list, from the shadow counts ------------------------------
+    uint8_t *h = nullptr, *d = nullptr;
+    int slot = 0;
+    rc = acquire_stage(pool, &h, &d, &slot);
+    if (rc) return rc;
+    AttendItem* items = reinterpret_cast<AttendItem*>(h);
+    const int32_t S = pool->unbounded ? 0 : c.n_sinks, W = pool->W_eff;
+    int32_t n_items = 0, row = 0, max_q = 0;
+    int64_t mma_units = 0, rows_units = 0;   // tile visits if every item took 1 split
+    for (int i = 0; i < n_batch; ++i) {
+        if (q_lens[i] == 0) continue;
+        const Session& s = pool->sessions[sids[i]];
+        AttendItem& it = items[n_items++];
+        memset(&it, 0, sizeof(it));
+        it.sid = sids[i];
+        it.len = (int32_t)s.len;
+        it.q_len = q_lens[i];
+        it.q_row_off = row;
+        row += q_lens[i];
+        const int32_t n_blk = (int32_t)((s.len + kBlockTokens - 1) / kBlockTokens);
+        const int64_t t0 = s.len - q_lens[i];                      // oldest query of this call
+        const int64_t wfirst = t0 - W + 1 > 0 ? t0 - W + 1 : 0;    // its oldest window key
+        int32_t first_blk = (int32_t)(wfirst / kBlockTokens);
+        if (first_blk < pool->n_sink) first_blk = pool->n_sink;
+        it.n_sink_tiles = n_blk < pool->n_sink ? n_blk : pool->n_sink;
+        it.first_blk = first_blk;
+        it.n_tiles = it.n_sink_tiles + (n_blk > first_blk ? n_blk - first_blk : 0);
+        if (it.q_len > max_q) max_q = it.q_len;
+        mma_units += (int64_t)it.n_tiles * c.n_kv_heads;
+        rows_units += (int64_t)it.n_tiles * c.n_q_heads * it.q_len;
+    }
+    // kernel family: CUDA-core row kernel for pure multi-head decode, tensor-core tile kernel when
+    // G x q_len rows share one KV stream (north_star: "Tensor cores are used only for the GQA-group x
+    // chunk QK^T/PV tiles, where the work really is a dense contraction")
+    int family = pool->tune_family;
+    if (family == 0) family = (pool->G * max_q >= 4) ? 2 : 1;
+    if (family == 2 && !attend_mma_supported(pool->G, max_q)) family = 1;
+    // split-KV: enough CTAs for >= 2 waves, each with a useful run of tiles
+    const int64_t units = family == 2 ? mma_units : rows_units;
+    const int64_t target_ctas = (int64_t)pool->n_sm * (family == 2 ? 4 : 16);
+    int32_t tps = pool->tune_split_tokens > 0 ? (pool->tune_split_tokens + kBlockTokens - 1) / kBlockTokens
+                                              : (int32_t)((units + target_ctas - 1) / target_ctas);
+    const int32_t min_tps = family == 2 ? 8 : 8;
+    if (pool->tune_split_tokens <= 0 && tps < min_tps) tps = min_tps;
+    if (tps < 1) tps = 1;
+    int32_t total_splits = 0, max_splits = 1;
+    for (int i = 0; i < n_items; ++i) {
+        AttendItem& it = items[i];
+        int32_t ns = (it.n_tiles + tps - 1) / tps;
+        if (ns > kMaxSplits) ns = kMaxSplits;
+        if (ns < 1) ns = 1;
+        it.n_splits = ns;
+        it.tiles_per_split = (it.n_tiles + ns - 1) / ns;
+        it.n_splits = (it.n_tiles + it.tiles_per_split - 1) / it.tiles_per_split;
+        if (it.n_splits < 1) it.n_splits = 1;
+        it.split_off = total_splits;
+        total_splits += it.n_splits;
+        if (it.n_splits > max_splits) max_splits = it.n_splits;
+    }
+    if (max_splits > 1) {
+        rc = ensure_workspace(pool, (size_t)total_rows * c.n_q_heads * max_splits);
+        if (rc) return rc;
+    }
+    rc = commit_stage(pool, slot, (size_t)n_items * sizeof(AttendItem), st);
+    if (rc) return rc;
+
+    AttendParams p{};
+    p.items = reinterpret_cast<const AttendItem*>(d);
+    p.n_items = n_items;
+    p.table = pool->d_table;
+    p.tbl_width = pool->tbl_width; p.n_sink = pool->n_sink; p.ring = pool->ring;
+    p.q = (const __nv_bfloat16*)q;
+    p.out = (__nv_bfloat16*)out;
+    p.kv_layer = pool->d_kv + (int64_t)layer * pool->L.layer_bytes;
+    p.L = pool->L;
+    p.S = S; p.W = W;
+    p.scale_log2 = pool->scale * 1.4426950408889634f;
+    p.Hq = c.n_q_heads; p.G = pool->G;
+    p.ws_acc = pool->d_ws_acc; p.ws_ml = pool->d_ws_ml;
+    p.max_splits = max_splits;
+
+    if (family == 2) {
+        rc = launch_attend_mma(p, c.head_dim, c.n_kv_heads, total_splits, max_q, st);
+        if (rc) return cuda_fail(pool, cudaGetLastError(), "attend_mma launch");
+    } else {
+        dim3 grid(total_splits, c.n_q_heads, max_q);
+        if (c.head_dim == 128) attend_rows_kernel<128><<<grid, 128, 0, st>>>(p);
+        else attend_rows_kernel<64><<<grid, 128, 0, st>>>(p);
+    }
+    ++pool->n_launch;
+    CU(cudaGetLastError());
+    if (max_splits > 1) {
+        dim3 grid((unsigned)total_rows, c.n_q_heads);
+        if (c.head_dim == 128) merge_kernel<128><<<grid, 32, 0, st>>>(p);
+        else merge_kernel<64><<<grid, 16, 0, st>>>(p);
+        ++pool->n_launch;
+        CU(cudaGetLastError());
+    }
+    return METRONOME_OK;
+}
+
+int metronome_step_host(metronome_pool_t* pool, int32_t layer, int32_t n_batch, const int32_t* sids,
+                        const int32_t* n_new, const void* k_new_host, const void* v_new_host,
+                        const void* q_host, void* out_host, void* cuda_stream) {
+    if (!pool || n_batch < 0 || (n_batch > 0 && (!sids || !n_new))) return METRONOME_ERR_INVALID_ARG;
+    if (pool->bookkeeping_only) return METRONOME_ERR_UNSUPPORTED;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const metronome_pool_config_t& c = pool->cfg;
+    int64_t rows = 0;
+    for (int i = 0; i < n_batch; ++i) {
+        if (n_new[i] < 0) return METRONOME_ERR_INVALID_ARG;
+        if (n_new[i] > c.max_new_tokens) return METRONOME_ERR_CHUNK_TOO_LARGE;
+        rows += n_new[i];
+    }
+    if (rows > 0 && (!k_new_host || !v_new_host || !q_host || !out_host)) return METRONOME_ERR_INVALID_ARG;
+    const size_t kv_b = (size_t)rows * c.n_kv_heads * c.head_dim * 2, q_b = (size_t)rows * c.n_q_heads * c.head_dim * 2;
+    const size_t kv_al = (kv_b + 255) & ~(size_t)255, q_al = (q_b + 255) & ~(size_t)255;
+    const size_t need = 2 * kv_al + 2 * q_al;
+    if (need > pool->io_bytes) {
+        if (pool->d_io) cudaFree(pool->d_io);
+        pool->d_io = nullptr; pool->io_bytes = 0;
+        CU(cudaMalloc(&pool->d_io, need + need / 2));
+        pool->io_bytes = need + need / 2;
+    }
+    uint8_t* dk = pool->d_io; uint8_t* dv = dk + kv_al; uint8_t* dq = dv + kv_al; uint8_t* dout = dq + q_al;
+    if (rows > 0) {
+        CU(cudaMemcpyAsync(dk, k_new_host, kv_b, cudaMemcpyHostToDevice, st));
+        CU(cudaMemcpyAsync(dv, v_new_host, kv_b, cudaMemcpyHostToDevice, st));
+        CU(cudaMemcpyAsync(dq, q_host, q_b, cudaMemcpyHostToDevice, st));
+    }
+    int rc = metronome_append_kv(pool, layer, n_batch, sids, n_new, rows ? dk : nullptr, rows ? dv : nullptr, cuda_stream);
+    if (rc) return rc;
+    rc = metronome_attend_frame(pool, layer, n_batch, sids, n_new, dq, dout, cuda_stream);
+    if (rc) return rc;
+    if (rows > 0) CU(cudaMemcpyAsync(out_host, dout, q_b, cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    return METRONOME_OK;
+}
+
+int metronome_session_query(metronome_pool_t* pool, int32_t sid, void* cuda_stream, int64_t* len,
+                            int32_t* first_live_block, int32_t* n_blocks, int32_t* block_ids) {
+    if (!pool) return METRONOME_ERR_INVALID_ARG;
+    if (sid < 0 || sid >= pool->cfg.max_sessions || !pool->sessions[sid].open) return METRONOME_ERR_INVALID_SESSION;
+    const Session& s = pool->sessions[sid];
+    const int32_t B = pool->cfg.block_size;
+    const int32_t n_blk = (int32_t)((s.len + B - 1) / B);
+    const int32_t n_sink_res = n_blk < pool->n_sink ? n_blk : pool->n_sink;
+    const int32_t n_win = n_blk > s.first_live ? n_blk - s.first_live : 0;
+    if (len) *len = s.len;
+    if (first_live_block) *first_live_block = s.first_live;
+    if (n_blocks) *n_blocks = n_sink_res + n_win;
+    if (block_ids && n_sink_res + n_win > 0) {
+        std::vector<int32_t> rowbuf(pool->tbl_width);
+        cudaStream_t st = (cudaStream_t)cuda_stream;
+        CU(cudaMemcpyAsync(rowbuf.data(), pool->d_table + (int64_t)sid * pool->tbl_width,
+                           (size_t)pool->tbl_width * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+        int k = 0;
+        for (int b = 0; b < n_sink_res; ++b) block_ids[k++] = rowbuf[table_slot(b, pool->n_sink, pool->ring)];
+        for (int b = s.first_live; b < n_blk; ++b) block_ids[k++] = rowbuf[table_slot(b, pool->n_sink, pool->ring)];
+    }
+    return METRONOME_OK;
+}
+
+int metronome_pool_query(metronome_pool_t* pool, void* cuda_stream, int32_t* n_free, int32_t* free_ids) {
+    if (!pool) return METRONOME_ERR_INVALID_ARG;
+    if (n_free) *n_free = pool->n_free;
+    if (free_ids && pool->n_free > 0) {
+        std::vector<int32_t> buf(pool->n_free);
+        cudaStream_t st = (cudaStream_t)cuda_stream;
+        CU(cudaMemcpyAsync(buf.data(), pool->d_free, (size_t)pool->n_free * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+        for (int i = 0; i < pool->n_free; ++i) free_ids[i] = buf[pool->n_free - 1 - i];   // pop order
+    }
+    return METRONOME_OK;
+}
+
+int metronome_read_kv(metronome_pool_t* pool, int32_t layer, int32_t sid, int64_t pos0, int32_t n, void* k_out,
+                      void* v_out, void* cuda_stream) {
+    if (!pool || layer < 0 || layer >= pool->cfg.n_layers || n < 0 || pos0 < 0) return METRONOME_ERR_INVALID_ARG;
+    if (pool->bookkeeping_only) return METRONOME_ERR_UNSUPPORTED;
+    if (sid < 0 || sid >= pool->cfg.max_sessions || !pool->sessions[sid].open) return METRONOME_ERR_INVALID_SESSION;
+    if (n == 0) return METRONOME_OK;
+    if (!k_out || !v_out || pos0 + n > INT32_MAX) return METRONOME_ERR_INVALID_ARG;
+    const Session& s = pool->sessions[sid];
+    const int32_t n_blk = (int32_t)((s.len + kBlockTokens - 1) / kBlockTokens);
+    const int32_t n_sink_res = n_blk < pool->n_sink ? n_blk : pool->n_sink;
+    const int64_t chunks = (int64_t)n * pool->cfg.n_kv_heads * (pool->cfg.head_dim / 8);
+    kv_read_kernel<<<(unsigned)((chunks + 255) / 256), 256, 0, (cudaStream_t)cuda_stream>>>(
+        pool->d_table + (int64_t)sid * pool->tbl_width, pool->n_sink, pool->ring, n_sink_res, s.first_live, n_blk,
+        (int32_t)pos0, n, pool->d_kv + (int64_t)layer * pool->L.layer_bytes, pool->L, (uint4*)k_out, (uint4*)v_out);
+    ++pool->n_launch;
+    CU(cudaGetLastError());
+    return METRONOME_OK;
+}
+
+int metronome_pool_stats(metronome_pool_t* pool, int64_t* kernel_launches, int64_t* append_calls, int64_t* attend_calls) {
+    if (!pool) return METRONOME_ERR_INVALID_ARG;
+    if (kernel_launches) *kernel_launches = pool->n_launch;
+    if (append_calls) *append_calls = pool->n_append;
+    if (attend_calls) *attend_calls = pool->n_attend;
+    return METRONOME_OK;
+}
+
+int metronome_pool_set_tuning(metronome_pool_t* pool, int32_t split_tokens, int32_t kernel_family) {
+    if (!pool || split_tokens < 0 || kernel_family < 0 || kernel_family > 2) return METRONOME_ERR_INVALID_ARG;
+    pool->tune_split_tokens = split_tokens;
+    pool->tune_family = kernel_family;
+    return METRONOME_OK;
+}
+
+}  // extern "C"

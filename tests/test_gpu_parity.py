@@ -1,0 +1,258 @@
+"""GPU parity tests (`-m gpu`): the CUDA path, through the C ABI, against the oracle.
+
+Bookkeeping (block tables, free list, eviction order) must match bit-exactly after every call;
+attention within north_star's tolerance (helpers.assert_parity).  Every input is seeded
+(synth.rows) and regenerated on the CPU for the oracle; nothing here reads /root/reference.
+"""
+import os
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import bounded_kv as O
+from paper_2607_02640_b200 import binding, synth
+from paper_2607_02640_b200 import workloads as wl
+from paper_2607_02640_b200.runner import Runner
+from parity_helpers import OracleMirror, assert_parity, parity_report
+from test_oracle_bookkeeping import GOLDEN, parse_trace, run_trace
+
+pytestmark = pytest.mark.gpu
+
+
+def _loaded_native():
+    """The driver checks that the in-tree .so is what ran: fail loudly if it is not loaded."""
+    with open("/proc/self/maps") as f:
+        assert "libmetronome.so" in f.read(), "native library not loaded"
+
+
+# ------------------------------------------------------------------------------ bookkeeping
+
+
+def test_hand_trace_on_device():
+    def make(B, S, W, n_blocks):
+        return binding.Pool(n_q_heads=1, n_kv_heads=1, head_dim=64, n_sinks=S, window=W, n_blocks=n_blocks,
+                            max_sessions=4, max_new_tokens=8, block_size=B, flags=binding.FLAG_BOOKKEEPING_ONLY)
+
+    run_trace(parse_trace(os.path.join(GOLDEN, "bookkeeping_hand_trace.txt")), make,
+              lambda p, sids, n: p.append_kv(0, sids, n, None, None),
+              lambda p, sid: p.session_close(sid), lambda p: p.session_open(),
+              lambda p, sid: p.session_query(sid), lambda p: p.pool_query()[1])
+    _loaded_native()
+
+
+@pytest.mark.parametrize("S,W,B,n_blocks,seed", [(4, 32, 16, 40, 0), (0, 20, 16, 24, 1), (17, 40, 16, 64, 2),
+                                                 (3, 7, 4, 30, 3), (40, 5, 8, 60, 4), (4, 2048, 16, 700, 5)])
+def test_bookkeeping_fuzz_bit_exact(S, W, B, n_blocks, seed):
+    """Random open / append / close traffic incl. pool exhaustion: tables and free list after EVERY call."""
+    rng = np.random.default_rng(seed)
+    n_max, slots = 25, 6
+    pool = binding.Pool(n_q_heads=1, n_kv_heads=1, head_dim=64, n_sinks=S, window=W, n_blocks=n_blocks,
+                        max_sessions=slots, max_new_tokens=n_max, block_size=B, flags=binding.FLAG_BOOKKEEPING_ONLY)
+    ora = O.PagedOracle(O.PoolConfig(n_q_heads=1, n_kv_heads=1, head_dim=64, S=S, W=W, n_blocks=n_blocks,
+                                     block_size=B, max_sessions=slots, max_new_tokens=n_max), store_kv=False)
+    live, exhausted = [], 0
+    for step in range(400):
+        r = rng.random()
+        if (r < 0.1 and len(live) < slots) or not live:
+            a, b = pool.session_open(), ora.session_open()
+            assert a == b
+            live.append(a)
+        elif r < 0.15:
+            sid = live.pop(int(rng.integers(len(live))))
+            pool.session_close(sid); ora.session_close(sid)
+        else:
+            k = int(rng.integers(1, len(live) + 1))
+            sids = [int(x) for x in rng.permutation(live)[:k]]
+            n_new = [int(rng.integers(1, n_max + 1)) if rng.random() < 0.5 else 1 for _ in sids]
+            err = None
+            try:
+                ora.append_kv(0, sids, n_new)
+            except O.OracleError as e:
+                err = e.code
+            if err:
+                exhausted += 1
+                with pytest.raises(binding.MetronomeError, match=err):
+                    pool.append_kv(0, sids, n_new, None, None)
+            else:
+                pool.append_kv(0, sids, n_new, None, None)
+        for sid in live:
+            got, want = pool.session_query(sid), ora.session_query(sid)
+            assert (got[0], got[1], got[2]) == (want[0], want[1], want[2]), (step, sid)
+        assert pool.pool_query()[1] == ora.pool_query(), step
+    if n_blocks <= 40:
+        assert exhausted > 0, "the fuzz never reached pool exhaustion"
+
+
+def test_error_codes_and_no_state_change():
+    pool = binding.Pool(n_q_heads=4, n_kv_heads=2, head_dim=64, n_sinks=4, window=32, n_blocks=7,
+                        max_sessions=2, max_new_tokens=16)
+    a = pool.session_open(); b = pool.session_open()
+    with pytest.raises(binding.MetronomeError, match="SESSIONS_FULL"):
+        pool.session_open()
+    k = torch.zeros(64, 2, 64, dtype=torch.bfloat16, device="cuda")
+    q = torch.zeros(64, 4, 64, dtype=torch.bfloat16, device="cuda")
+    for sids, n, code in [([a, a], [1, 1], "DUPLICATE_SESSION"), ([5], [1], "INVALID_SESSION"),
+                          ([a], [17], "CHUNK_TOO_LARGE"), ([a], [-1], "INVALID_ARG")]:
+        with pytest.raises(binding.MetronomeError, match=code):
+            pool.append_kv(0, sids, n, k, k)
+    with pytest.raises(binding.MetronomeError, match="LAYER_SEQUENCE"):
+        pool.attend_frame(0, [a], [1], q, q)
+    pool.append_kv(0, [a, b], [16, 16], k, k)
+    pool.append_kv(0, [a, b], [16, 16], k, k)
+    pool.append_kv(0, [a, b], [16, 16], k, k)           # 6 of 7 blocks in use
+    before = (pool.session_query(a), pool.session_query(b), pool.pool_query())
+    with pytest.raises(binding.MetronomeError, match="POOL_EXHAUSTED"):
+        pool.append_kv(0, [a, b], [16, 16], k, k)       # L0=48, W=32: nothing is behind the window yet; needs 2
+    assert (pool.session_query(a), pool.session_query(b), pool.pool_query()) == before
+    with pytest.raises(binding.MetronomeError, match="QLEN_EXCEEDS_LAST_APPEND"):
+        pool.attend_frame(0, [a], [17], q, q)
+    pool.session_close(a)
+    with pytest.raises(binding.MetronomeError, match="INVALID_SESSION"):
+        pool.session_close(a)
+    assert pool.session_open() == a
+
+
+# ------------------------------------------------------------------------------ KV write
+
+
+def test_kv_write_reads_back_through_the_table():
+    w = wl.make_workload(1)
+    r = Runner(w)
+    events, _ = wl.build_schedule(w)
+    rest = r.run_history(events)
+    for i in range(w.n_sessions):
+        L = r.length[i]
+        k = torch.empty(L, w.n_kv_heads, w.head_dim, dtype=torch.bfloat16, device="cuda")
+        v = torch.empty_like(k)
+        r.pool.read_kv(0, r.sid[i], 0, L, k, v)
+        pos = np.arange(L)
+        want_k = r.rows(synth.STREAM_K, 0, np.full(L, r.uid[i]), pos, device="cpu")
+        want_v = r.rows(synth.STREAM_V, 0, np.full(L, r.uid[i]), pos, device="cpu")
+        ln, first_live, blocks = r.pool.session_query(r.sid[i])
+        resident = np.array([(p // 16 < 1) or (p // 16 >= first_live) for p in pos])   # n_sink = 1
+        kc, vc = k.cpu(), v.cpu()
+        assert torch.equal(kc[resident].view(torch.int16), want_k[resident].view(torch.int16))
+        assert torch.equal(vc[resident].view(torch.int16), want_v[resident].view(torch.int16))
+        assert torch.isnan(kc[~resident].float()).all()      # evicted rows are reported as NaN
+
+
+# ------------------------------------------------------------------------------ attention parity
+
+
+def _run_parity(w, history_scale=1.0, n_layers=1, flags=0, family=0, split_tokens=0, max_timed=None,
+                check_tables=True, check_history_attend_every=0):
+    r = Runner(w, n_layers=n_layers, flags=flags)
+    r.pool.set_tuning(split_tokens, family)
+    m = OracleMirror(r)
+    events, _ = wl.build_schedule(w, history_scale=history_scale)
+    worst = {"max_abs": 0.0, "max_rel": 0.0, "row_l2": 0.0}
+    n_timed = 0
+    hist_i = 0
+    for ev in events:
+        if ev[0] == "open":
+            r.open(ev[1]); m.open(ev[1])
+        elif ev[0] == "close":
+            r.close(ev[1]); m.close(ev[1])
+            if check_tables:
+                m.check_tables(r.pool)
+        else:
+            st = r.make_step(ev)
+            do_attend = st.timed
+            if not st.timed and check_history_attend_every:
+                hist_i += 1
+                do_attend = hist_i % check_history_attend_every == 0
+            for layer in range(n_layers):
+                r.append(st, layer); m.append(st, layer)
+                if do_attend:
+                    out = r.attend(st, layer)
+                    ref = m.attend(st, layer)
+                    rep = assert_parity(out, ref, f"{w.name} frame {st.frame} layer {layer} n={st.n_new[:4]}")
+                    for k_ in worst:
+                        worst[k_] = max(worst[k_], rep[k_])
+            if check_tables and (st.timed or hist_i % 7 == 0):
+                m.check_tables(r.pool)
+            if st.timed:
+                n_timed += 1
+                if max_timed and n_timed >= max_timed:
+                    break
+    _loaded_native()
+    return worst
+
+
+@pytest.mark.parametrize("family", [0, 1, 2])
+def test_config1_tiny_full(family):
+    """BASELINE.json configs[0] exactly as specified, every frame, tables after every call."""
+    worst = _run_parity(wl.make_workload(1), family=family, check_history_attend_every=5)
+    print("config 1 worst", family, worst)
+
+
+@pytest.mark.parametrize("split_tokens", [16, 48, 4096])
+def test_config1_both_launch_modes(split_tokens):
+    """PAPER.md:L258 'both launch modes': plain (one segment) and segmented (split-KV) decode."""
+    for family in (1, 2):
+        _run_parity(wl.make_workload(1), family=family, split_tokens=split_tokens, check_tables=False)
+
+
+def test_config1_poisoned_frees_two_layers():
+    """freed blocks NaN-poisoned: nothing outside sinks U window is ever read."""
+    _run_parity(wl.make_workload(1), n_layers=2, flags=binding.FLAG_POISON_ON_FREE, check_history_attend_every=3)
+
+
+@pytest.mark.parametrize("index,n_sessions,scale,timed", [(2, 6, 0.3, 12), (3, 5, 0.6, 2), (4, 6, 0.12, 2), (5, 12, 0.05, 6)])
+def test_configs_2_to_5_reduced(index, n_sessions, scale, timed):
+    """Configs 2-5 at their true head shapes and (S, W), with fewer sessions / shorter ages so the
+    oracle finishes in seconds; several tiles, ragged tails, mixed chunk+decode, outliers, churn."""
+    w = wl.make_workload(index, n_sessions=n_sessions, n_timed_frames=timed)
+    worst = _run_parity(w, history_scale=scale, flags=binding.FLAG_POISON_ON_FREE)
+    print("config", index, "worst", worst)
+
+
+def test_mixed_prefill_and_decode_in_one_call():
+    """PAPER.md:L258 'mixed prefill/decode': one attend_frame call with q_len 1 and q_len n items."""
+    w = wl.make_workload(3, n_sessions=4)
+    for family in (1, 2):
+        r = Runner(w)
+        r.pool.set_tuning(0, family)
+        m = OracleMirror(r, paged=False)
+        for i in range(4):
+            r.open(i); m.open(i)
+        rng = np.random.default_rng(0)
+        for step in range(40):
+            n_new = np.array([int(rng.integers(1, 26)) if rng.random() < 0.5 else 1 for _ in range(4)], np.int32)
+            st = r.make_step(("step", np.arange(4, dtype=np.int32), n_new, True, step))
+            r.append(st, 0); m.append(st, 0)
+            assert_parity(r.attend(st, 0), m.attend(st, 0), f"mixed step {step} {n_new}")
+
+
+@pytest.mark.parametrize("family", [1, 2])
+def test_spike_keys_at_every_mask_boundary_on_device(family):
+    S, W, L = 4, 128, 300
+    t = L - 1
+    kw = dict(n_sinks=S, window=W, n_blocks=64)
+
+    def run(j):
+        D = 64
+        pool = binding.Pool(n_q_heads=1, n_kv_heads=1, head_dim=D, max_sessions=1, max_new_tokens=16, **kw)
+        pool.set_tuning(0, family)
+        sid = pool.session_open()
+        k = torch.zeros(L, 1, D); v = torch.zeros(L, 1, D)
+        k[j, 0, 0] = 10.0
+        v[:, 0, 1] = 1.0
+        v[j, 0, 0] = 1000.0; v[j, 0, 1] = 0.0
+        k = k.to(torch.bfloat16).cuda(); v = v.to(torch.bfloat16).cuda()
+        for a in range(0, L, 16):
+            n = min(16, L - a)
+            pool.append_kv(0, [sid], [n], k[a:a + n].contiguous(), v[a:a + n].contiguous())
+        q = torch.zeros(1, 1, D); q[0, 0, 0] = 32.0
+        q = q.to(torch.bfloat16).cuda()
+        out = torch.empty_like(q)
+        pool.attend_frame(0, [sid], [1], q, out)
+        torch.cuda.synchronize()
+        return out[0, 0].float().cpu().numpy()
+
+    assert run(t - W)[0] == 0.0 and abs(run(t - W)[1] - 1.0) < 1e-2      # just behind the window: OUT
+    assert run(t - W + 1)[0] > 990.0                                       # oldest window key: IN
+    assert run(S - 1)[0] > 990.0                                           # last sink: IN
+    assert run(S)[0] == 0.0                                                # first non-sink, far behind: OUT
+    assert run(t)[0] > 990.0                                               # the query's own key: IN
