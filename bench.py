@@ -1,0 +1,431 @@
+#!/usr/bin/env python
+"""bench.py -- session-frames/s and windowed-attention HBM GB/s on synthetic Metronome sessions.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl reference]
+
+A "step" is one frame of the whole hot path for every due session on one layer:
+append_kv (evict + allocate + KV write) then attend_frame (work list, attention, merge).
+At N=1 the workload is BASELINE.json configs[1] (Moshi-shaped: 128 sessions, 32Q/32KV, D=128,
+S=4, W=750, ages U{1..3750}); histories are built through the library first (untimed).
+Prints ONE JSON line (contract in the task statement): `value` = whole-job session-frames/s with
+inputs resident in HBM, `e2e` = the same through metronome_step_host with pinned HOST buffers,
+`roofline` for the dominant kernel (attention), `cpu_baseline` = the oracle on the host cores.
+
+N > 1 (launched by torch.distributed.run): replicas only -- one pool per GPU, sessions never
+cross GPUs, no data-path collective; max-over-ranks time, `"scaling": "weak"`.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+RANK = int(os.environ.get("RANK", "0"))
+LOCAL_RANK = int(os.environ.get("LOCAL_RANK", "0"))
+WORLD = int(os.environ.get("WORLD_SIZE", "1"))
+
+METRIC = "session_frames_per_sec"
+UNIT = "session-frames/s (per layer)"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=400)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="metronome", choices=["metronome", "reference"])
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config index 1..5 (2 = the metric's)")
+    ap.add_argument("--history-scale", type=float, default=1.0)
+    ap.add_argument("--sessions", type=int, default=0, help="override the session count (0 = the config's)")
+    ap.add_argument("--family", type=int, default=0, help="0 auto, 1 CUDA-core rows, 2 tensor-core tiles")
+    ap.add_argument("--split-tokens", type=int, default=0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        p = json.load(open(path))
+        return float(p["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """SM clock and throttle reasons sampled DURING the timed region (NVML, a polling thread)."""
+
+    def __init__(self, gpu_index: int, period_s: float = 0.01):
+        import threading
+        self.sm, self.reasons, self.max_mhz, self.err = [], set(), None, None
+        self._stop = threading.Event()
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(gpu_index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception as e:          # noqa: BLE001
+            self.err = f"nvml unavailable: {e}"
+            self.nv = None
+        self.period = period_s
+        self.t = threading.Thread(target=self._loop, daemon=True)
+        if self.nv:
+            self.t.start()
+
+    def _loop(self):
+        nv = self.nv
+        names = {"hw_slowdown": getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8),
+                 "hw_thermal_slowdown": getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40),
+                 "sw_thermal_slowdown": getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20),
+                 "sw_power_cap": getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4)}
+        while not self._stop.is_set():
+            try:
+                self.sm.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                try:
+                    mask = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:       # noqa: BLE001
+                    mask = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for k, bit in names.items():
+                    if mask & bit:
+                        self.reasons.add(k)
+            except Exception as e:      # noqa: BLE001
+                self.err = str(e)
+                break
+            self._stop.wait(self.period)
+
+    def stop(self):
+        self._stop.set()
+        if self.nv:
+            self.t.join(timeout=2)
+        sm = sorted(self.sm)
+        out = {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": self.max_mhz, "samples": len(sm),
+               "reasons": sorted(self.reasons)}
+        if self.err:
+            out["note"] = self.err
+        return out
+
+
+def algorithmic_bytes(w, lengths, n_new):
+    """per session keys_read x Hkv x 4D (K+V bf16) + q and out rows.
+    keys_read = min(len, S+W) for decode; for a chunk the union over its rows min(L1, S+W+n-1)."""
+    total = 0
+    for L, n in zip(lengths, n_new):
+        L, n = int(L), int(n)
+        keys = min(L, w.S + w.W + n - 1)
+        total += keys * w.n_kv_heads * 4 * w.head_dim + n * w.n_q_heads * 4 * w.head_dim
+    return total
+
+
+def cpu_baseline(w, runner, steps_sample, budget_s=15.0, n_threads=None):
+    """The oracle as it stands, on this box's host cores, on a bounded sample of the same workload:
+    a seeded subset of sessions at their real ages, one attend per timed step until the budget."""
+    import numpy as np
+    import torch
+    from oracle import bounded_kv as O
+    from paper_2607_02640_b200 import synth
+    n_threads = n_threads or O.max_threads()
+    rng = np.random.default_rng(w.seed + 99)
+    locs = sorted(runner.length)
+    pick = [int(x) for x in rng.permutation(locs)[:min(8, len(locs))]]
+    sample = []
+    for i in pick:
+        L = runner.length[i]
+        n = int(steps_sample.get(i, 1))
+        # only sinks + the union window can be admitted: regenerate exactly those rows on the CPU
+        lo = max(0, L - n - w.W + 1)
+        pos = np.concatenate([np.arange(0, min(w.S, lo)), np.arange(lo, L)]).astype(np.int64)
+        uid = np.full(len(pos), runner.uid[i], np.int64)
+        k = synth.to_u16(runner.rows(synth.STREAM_K, 0, uid, pos, device="cpu"))
+        v = synth.to_u16(runner.rows(synth.STREAM_V, 0, uid, pos, device="cpu"))
+        qpos = np.arange(L - n, L, dtype=np.int64)
+        q = synth.to_u16(runner.rows(synth.STREAM_Q, 0, np.full(n, runner.uid[i], np.int64), qpos, device="cpu"))
+        sample.append((q, qpos, k, v, pos))
+    t0 = time.perf_counter()
+    frames = 0
+    while True:
+        for q, qpos, k, v, pos in sample:
+            O.attend(q, qpos, k, v, pos, w.S, w.W, None, "f32", False, n_threads)
+        frames += len(sample)
+        el = time.perf_counter() - t0
+        if el >= budget_s or frames >= 100000:
+            break
+    return {"value": frames / el, "unit": UNIT, "cores": int(n_threads), "kind": "oracle",
+            "sample": f"{len(sample)} seeded sessions of config {w.index} at their real ages, attention only "
+                      f"(oracle_attend_f32, OpenMP over rows x heads), repeated for {el:.1f} s = {frames} session-frames"}
+
+
+def run_reference(args):
+    """--impl reference: the oracle (there is no reference implementation to install).
+    Each step is a bounded sample of the workload; rank 0 only."""
+    if RANK != 0:
+        return
+    import numpy as np
+    from oracle import bounded_kv as O
+    from paper_2607_02640_b200 import synth
+    from paper_2607_02640_b200 import workloads as wl
+    w = wl.make_workload(args.config)
+    rng = np.random.default_rng(w.seed)
+    n_threads = O.max_threads()
+    # same age recipe as the workload, 8 seeded sessions per step, attention of one frame
+    import torch
+
+    def rows(tag, uid, pos, heads):
+        return synth.to_u16(synth.rows(w.seed, tag, 0, torch.from_numpy(uid), torch.from_numpy(pos), heads, w.head_dim))
+
+    sample = []
+    for i in range(8):
+        L = int(rng.integers(1, 3751)) if w.index == 2 else int(rng.integers(1, 150 * 33))
+        n = 1
+        lo = max(0, L - n - w.W + 1)
+        pos = np.concatenate([np.arange(0, min(w.S, lo)), np.arange(lo, L)]).astype(np.int64)
+        uid = np.full(len(pos), i, np.int64)
+        qpos = np.arange(L - n, L, dtype=np.int64)
+        sample.append((rows(synth.STREAM_Q, np.full(n, i, np.int64), qpos, w.n_q_heads), qpos,
+                       rows(synth.STREAM_K, uid, pos, w.n_kv_heads), rows(synth.STREAM_V, uid, pos, w.n_kv_heads), pos))
+
+    def step():
+        for q, qpos, k, v, pos in sample:
+            O.attend(q, qpos, k, v, pos, w.S, w.W, None, "f32", False, n_threads)
+
+    for _ in range(args.warmup):
+        step()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step()
+    el = time.perf_counter() - t0
+    value = len(sample) * args.steps / el
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * el / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": f"config {w.index} ({w.name}), bounded sample: 8 seeded sessions per step, attention only"},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": int(n_threads), "kind": "oracle",
+                             "sample": "8 seeded sessions per step, one decode attend each"},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    # one process per GPU: make this rank's GPU the only visible one BEFORE CUDA initialises, so the
+    # library (static cudart) and torch agree on "device 0"
+    if WORLD > 1 and "CUDA_VISIBLE_DEVICES" not in os.environ:
+        os.environ["CUDA_VISIBLE_DEVICES"] = str(LOCAL_RANK)
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_2607_02640_b200 import build as _build
+    _build.build_library()
+    from paper_2607_02640_b200 import synth
+    from paper_2607_02640_b200 import workloads as wl
+    from paper_2607_02640_b200.runner import Runner
+
+    assert torch.cuda.is_available(), "bench.py needs a GPU (there is no CPU fallback for the product path)"
+    torch.cuda.set_device(0)
+    if WORLD > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", 0))
+
+    K, W = args.steps, max(args.warmup, 3)
+    # a bench "step" = one FRAME (all its sub-steps: chunk prefill + decode steps) for every due
+    # session; every phase needs fresh frames: warm-up + timed + profiled + e2e warm-up + e2e timed
+    need = 2 * W + 3 * K
+    w = wl.make_workload(args.config, n_sessions=args.sessions or None, n_timed_frames=need)
+    events, info = wl.build_schedule(w, history_scale=args.history_scale)
+    r = Runner(w, n_layers=1)
+    r.pool.set_tuning(args.split_tokens, args.family)
+    t_hist = time.perf_counter()
+    rest = r.run_history(events)
+    torch.cuda.synchronize()
+    t_hist = time.perf_counter() - t_hist
+    frames, cur, cur_fid = [], [], None       # a frame = its opens/closes, then its steps
+    for ev in rest:
+        fid = ev[4] if ev[0] == "step" else None
+        if cur and cur_fid is not None and fid != cur_fid:
+            frames.append(cur)
+            cur, cur_fid = [], None
+        cur.append(ev)
+        if fid is not None:
+            cur_fid = fid
+    if cur and cur_fid is not None:
+        frames.append(cur)
+    assert len(frames) >= need, (len(frames), need)
+
+    def prepare(frs):
+        """Resolve the frames' steps and generate their inputs in HBM before the timed region."""
+        out = []
+        for fr in frs:
+            for ev in fr:
+                if ev[0] == "open":
+                    r.open(ev[1]); continue
+                if ev[0] == "close":
+                    out.append(("close", r.sid[ev[1]], ev[1])); continue
+                st = r.make_step(ev)
+                k = r.rows(synth.STREAM_K, 0, st.uid_rows, st.pos_rows)
+                v = r.rows(synth.STREAM_V, 0, st.uid_rows, st.pos_rows)
+                q = r.rows(synth.STREAM_Q, 0, st.uid_rows, st.pos_rows)
+                lens_after = [r.length[int(i)] for i in st.local]
+                out.append((st, k, v, q, torch.empty_like(q), lens_after))
+        return out
+
+    def run(prepped):
+        for item in prepped:
+            if item[0] == "close":
+                r.pool.session_close(item[1]); continue
+            st, k, v, q, o, _ = item
+            r.pool.append_kv(0, st.sids, st.n_new, k, v)
+            r.pool.attend_frame(0, st.sids, st.n_new, q, o)
+
+    def finish_closes(prepped):
+        for item in prepped:
+            if item[0] == "close":
+                i = item[2]
+                r.sid.pop(i, None); r.uid.pop(i, None); r.length.pop(i, None)
+
+    def session_frames(frs):
+        return sum(len({int(i) for ev in fr if ev[0] == "step" for i in ev[1]}) for fr in frs)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if WORLD > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    cursor = 0
+
+    def take(n):
+        nonlocal cursor
+        frs = frames[cursor:cursor + n]
+        cursor += n
+        return frs
+
+    # ---- device-resident timing: W warm-up steps, then EXACTLY K timed steps ----
+    warm_f, timed_f = take(W), take(K)
+    warm = prepare(warm_f)
+    run(warm)
+    finish_closes(warm)
+    timed = prepare(timed_f)
+    barrier()
+    gpu_index = int(os.environ.get("CUDA_VISIBLE_DEVICES", str(LOCAL_RANK)).split(",")[0] or 0)
+    sampler = ClockSampler(gpu_index) if RANK == 0 else None
+    launches0 = r.pool.stats()["kernel_launches"]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.nvtx.range_push("metronome_timed")     # lets `ncu --nvtx --nvtx-include` pick this region
+    e0.record()
+    run(timed)
+    e1.record()
+    torch.cuda.nvtx.range_pop()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop() if sampler else None
+    launches = r.pool.stats()["kernel_launches"] - launches0
+    if WORLD > 1:
+        t = torch.tensor([ms], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    finish_closes(timed)
+    value = WORLD * session_frames(timed_f) / (ms * 1e-3)
+
+    # ---- roofline of the dominant kernel: same steps again with the library's event brackets ----
+    prof = prepare(take(K))
+    r.pool.set_profiling(True)
+    run(prof)
+    torch.cuda.synchronize()
+    k_ms, k_n = r.pool.read_profile()
+    r.pool.set_profiling(False)
+    finish_closes(prof)
+    alg_bytes = sum(algorithmic_bytes(w, it[5], it[0].n_new) for it in prof if it[0] != "close")
+    n_prof_steps = sum(1 for it in prof if it[0] != "close")
+    peak, peak_src = peaks()
+    achieved = alg_bytes / (k_ms * 1e-3) / 1e9 if k_ms > 0 else 0.0
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        traffic = json.load(open(tpath)).get(f"config{w.index}")
+    roofline = {"bound": "hbm", "kernel": "attend_rows_kernel<128>" if w.n_q_heads == w.n_kv_heads else "attend_mma_kernel",
+                "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
+                "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes / max(k_n, 1),
+                "kernel_ms_avg": k_ms / max(k_n, 1), "kernel_share_of_step": k_ms / ms if ms > 0 else None,
+                "frac_of_nominal_8TBs": achieved / 8000.0}
+
+    # ---- end to end: HOST buffers through metronome_step_host, copies inside the timed region ----
+    e2e = None
+    if not args.no_e2e:
+        def to_host(prepped):
+            out = []
+            for item in prepped:
+                if item[0] == "close":
+                    out.append(item); continue
+                st, k, v, q, o, _ = item
+                out.append((st, k.cpu().pin_memory(), v.cpu().pin_memory(), q.cpu().pin_memory(),
+                            torch.empty(q.shape, dtype=q.dtype).pin_memory()))
+            return out
+
+        def run_host(hp):
+            chk = 0.0
+            for item in hp:
+                if item[0] == "close":
+                    r.pool.session_close(item[1]); continue
+                st, k, v, q, o = item
+                r.pool.step_host(0, st.sids, st.n_new, k, v, q, o)   # synchronises; `o` is on the host
+                chk += float(o[0, 0, 0])
+            return chk
+        hw_f, ht_f = take(W), take(K)
+        hw = to_host(prepare(hw_f))
+        run_host(hw)
+        finish_closes(hw)
+        ht = to_host(prepare(ht_f))
+        barrier()
+        t0 = time.perf_counter()
+        run_host(ht)
+        el = time.perf_counter() - t0
+        if WORLD > 1:
+            t = torch.tensor([el], device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            el = float(t.item())
+        hsteps = [it for it in ht if it[0] != "close"]
+        h2d = sum(k.numel() * 2 + v.numel() * 2 + q.numel() * 2 for _, k, v, q, _ in hsteps) / K
+        d2h = sum(o.numel() * 2 for *_, o in hsteps) / K
+        e2e = {"value": WORLD * session_frames(ht_f) / el, "unit": UNIT, "h2d_bytes_per_step": h2d,
+               "d2h_bytes_per_step": d2h, "ms_per_step": 1e3 * el / K,
+               "api": "metronome_step_host (pinned host buffers)"}
+
+    if RANK != 0:
+        if WORLD > 1:
+            dist.destroy_process_group()
+        return
+    cpu = None
+    if not args.no_cpu_baseline and WORLD == 1:
+        last = [it for it in timed if it[0] != "close"][-1][0]
+        cpu = cpu_baseline(w, r, {int(i): int(n) for i, n in zip(last.local, last.n_new)})
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": WORLD, "steps": K, "warmup": W,
+        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "bf16 in, f32 accumulate", "data": "synthetic",
+        "config": {"workload": f"BASELINE.json configs[{w.index - 1}] {w.name}: {w.n_sessions} sessions, "
+                               f"{w.n_q_heads}Q/{w.n_kv_heads}KV, D={w.head_dim}, S={w.S}, W={w.W}, block 16",
+                   "sessions_per_gpu": w.n_sessions, "n_layers": 1, "parallelism": f"replicas x{WORLD}",
+                   "history_scale": args.history_scale,
+                   "l2": "inputs larger than L2: every step streams each session's whole window "
+                         f"({alg_bytes / max(k_n, 1) / 1e6:.0f} MB per step vs 126 MB L2), no flush needed",
+                   "history_build_s": round(t_hist, 2)},
+        "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
+        "attention_gbs": achieved,
+    }
+    print(json.dumps(line), flush=True)
+    if WORLD > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

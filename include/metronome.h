@@ -191,6 +191,14 @@ int metronome_pool_stats(metronome_pool_t* pool, int64_t* kernel_launches, int64
  * launch modes" (L258).  Errors: INVALID_ARG. */
 int metronome_pool_set_tuning(metronome_pool_t* pool, int32_t split_tokens, int32_t kernel_family);
 
+/* Measurement aid.  While enabled, attend_frame brackets its attention kernel (the dominant
+ * kernel; not the metadata copy, not the merge) with CUDA events on the caller's stream.
+ * read_profile waits for those events, returns the summed kernel time in milliseconds and the
+ * number of bracketed launches since the last reset, and (reset != 0) clears them.  host. */
+int metronome_pool_set_profiling(metronome_pool_t* pool, int32_t enable);
+int metronome_pool_read_profile(metronome_pool_t* pool, double* attend_kernel_ms, int64_t* attend_kernel_launches,
+                                int32_t reset);
+
 const char* metronome_strerror(int status);
 /* Text of the last CUDA error seen by this pool ("" if none).  Valid until the next call. */
 const char* metronome_last_cuda_error(metronome_pool_t* pool);

@@ -28,7 +28,7 @@ EXPORTS = ["metronome_abi_version", "metronome_strerror", "metronome_last_cuda_e
            "metronome_pool_destroy", "metronome_session_open", "metronome_session_close",
            "metronome_append_kv", "metronome_attend_frame", "metronome_step_host",
            "metronome_session_query", "metronome_pool_query", "metronome_read_kv", "metronome_pool_stats",
-           "metronome_pool_set_tuning"]
+           "metronome_pool_set_tuning", "metronome_pool_set_profiling", "metronome_pool_read_profile"]
 
 
 class MetronomeError(RuntimeError):
@@ -80,6 +80,8 @@ def load():
     lib.metronome_read_kv.argtypes = [c_void_p, c_int32, c_int32, c_int64, c_int32, c_void_p, c_void_p, c_void_p]
     lib.metronome_pool_stats.argtypes = [c_void_p, POINTER(c_int64), POINTER(c_int64), POINTER(c_int64)]
     lib.metronome_pool_set_tuning.argtypes = [c_void_p, c_int32, c_int32]
+    lib.metronome_pool_set_profiling.argtypes = [c_void_p, c_int32]
+    lib.metronome_pool_read_profile.argtypes = [c_void_p, POINTER(ctypes.c_double), POINTER(c_int64), c_int32]
     _lib = lib
     return lib
 
@@ -192,3 +194,12 @@ class Pool:
 
     def set_tuning(self, split_tokens=0, kernel_family=0):
         self._check(self._lib.metronome_pool_set_tuning(self._h, split_tokens, kernel_family))
+
+    def set_profiling(self, enable: bool):
+        self._check(self._lib.metronome_pool_set_profiling(self._h, int(enable)))
+
+    def read_profile(self, reset=True):
+        """-> (summed attention-kernel milliseconds, bracketed launches)"""
+        ms, n = ctypes.c_double(), c_int64()
+        self._check(self._lib.metronome_pool_read_profile(self._h, byref(ms), byref(n), int(reset)))
+        return ms.value, n.value

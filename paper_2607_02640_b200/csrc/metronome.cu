@@ -69,6 +69,11 @@ struct metronome_pool {
     bool ev_used[kStagingSlots]{};
     int next_slot = 0;
 
+    // profiling (metronome_pool_set_profiling): event pairs around the attention kernel
+    bool profiling = false;
+    std::vector<cudaEvent_t> prof_ev;  // start, stop, start, stop, ...
+    size_t prof_used = 0;
+
     int32_t tune_split_tokens = 0, tune_family = 0;
     int32_t n_sm = 148;
     int64_t n_launch = 0, n_append = 0, n_attend = 0;
@@ -280,7 +285,8 @@ int metronome_pool_create(const metronome_pool_config_t* cfg, metronome_pool_t**
     init_free_stack_kernel<<<(c.n_blocks + 255) / 256, 256>>>(pool->d_free, c.n_blocks);
     e = cudaDeviceSynchronize();
     if (e != cudaSuccess) return fail(METRONOME_ERR_CUDA, e, "pool init kernels");
-    configure_attend_mma_kernels();
+    e = configure_attend_mma_kernels();
+    if (e != cudaSuccess) return fail(METRONOME_ERR_CUDA, e, "cudaFuncSetAttribute");
     *out = pool;
     return METRONOME_OK;
 }
@@ -298,6 +304,7 @@ int metronome_pool_destroy(metronome_pool_t* pool) {
     if (pool->d_stage) cudaFree(pool->d_stage);
     for (int i = 0; i < kStagingSlots; ++i)
         if (pool->ev[i]) cudaEventDestroy(pool->ev[i]);
+    for (cudaEvent_t e : pool->prof_ev) cudaEventDestroy(e);
     delete pool;
     return METRONOME_OK;
 }
@@ -558,6 +565,16 @@ int metronome_attend_frame(metronome_pool_t* pool, int32_t layer, int32_t n_batc
     p.ws_acc = pool->d_ws_acc; p.ws_ml = pool->d_ws_ml;
     p.max_splits = max_splits;
 
+    if (pool->profiling) {
+        if (pool->prof_used + 2 > pool->prof_ev.size()) {
+            cudaEvent_t a, b;
+            CU(cudaEventCreate(&a));
+            CU(cudaEventCreate(&b));
+            pool->prof_ev.push_back(a);
+            pool->prof_ev.push_back(b);
+        }
+        CU(cudaEventRecord(pool->prof_ev[pool->prof_used], st));
+    }
     if (family == 2) {
         rc = launch_attend_mma(p, c.head_dim, c.n_kv_heads, total_splits, max_q, st);
         if (rc) return cuda_fail(pool, cudaGetLastError(), "attend_mma launch");
@@ -568,6 +585,10 @@ int metronome_attend_frame(metronome_pool_t* pool, int32_t layer, int32_t n_batc
     }
     ++pool->n_launch;
     CU(cudaGetLastError());
+    if (pool->profiling) {
+        CU(cudaEventRecord(pool->prof_ev[pool->prof_used + 1], st));
+        pool->prof_used += 2;
+    }
     if (max_splits > 1) {
         dim3 grid((unsigned)total_rows, c.n_q_heads);
         if (c.head_dim == 128) merge_kernel<128><<<grid, 32, 0, st>>>(p);
@@ -678,6 +699,28 @@ int metronome_pool_stats(metronome_pool_t* pool, int64_t* kernel_launches, int64
     if (kernel_launches) *kernel_launches = pool->n_launch;
     if (append_calls) *append_calls = pool->n_append;
     if (attend_calls) *attend_calls = pool->n_attend;
+    return METRONOME_OK;
+}
+
+int metronome_pool_set_profiling(metronome_pool_t* pool, int32_t enable) {
+    if (!pool) return METRONOME_ERR_INVALID_ARG;
+    pool->profiling = enable != 0;
+    return METRONOME_OK;
+}
+
+int metronome_pool_read_profile(metronome_pool_t* pool, double* attend_kernel_ms, int64_t* attend_kernel_launches,
+                                int32_t reset) {
+    if (!pool) return METRONOME_ERR_INVALID_ARG;
+    double ms = 0.0;
+    for (size_t i = 0; i + 1 < pool->prof_used; i += 2) {
+        CU(cudaEventSynchronize(pool->prof_ev[i + 1]));
+        float t = 0.f;
+        CU(cudaEventElapsedTime(&t, pool->prof_ev[i], pool->prof_ev[i + 1]));
+        ms += t;
+    }
+    if (attend_kernel_ms) *attend_kernel_ms = ms;
+    if (attend_kernel_launches) *attend_kernel_launches = (int64_t)(pool->prof_used / 2);
+    if (reset) pool->prof_used = 0;
     return METRONOME_OK;
 }
 
