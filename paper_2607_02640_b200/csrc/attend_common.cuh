@@ -22,7 +22,8 @@ struct AttendItem {
     int32_t n_splits;         // split-KV segments of this item
     int32_t split_off;        // exclusive prefix sum of n_splits (first CTA of this item)
     int32_t tiles_per_split;
-    int32_t pad0, pad1;
+    int32_t tile_off;         // exclusive prefix sum of n_tiles over the items of this launch
+    int32_t class_row_off;    // exclusive prefix sum of q_len over the items of this launch
 };
 
 struct AttendParams {
@@ -74,15 +75,16 @@ __device__ __forceinline__ uint32_t pack_bf16(float a, float b) {
 
 // Row a6: log-sum-exp combine of the split-KV partials of one (query row, q head); sinks were
 // counted once, by segment 0 ("merged exactly once").
-// grid = (total_rows, Hq), block = D/4 threads.
+// grid = (rows of this launch's items, Hq), block = D/4 threads.
 template <int D>
 __global__ void __launch_bounds__(D / 4)
 merge_kernel(AttendParams p) {
-    const int32_t row = blockIdx.x, h = blockIdx.y;
-    const int32_t i = find_item(p.n_items, row, [&](int32_t k) { return p.items[k].q_row_off; });
+    const int32_t h = blockIdx.y;
+    const int32_t i = find_item(p.n_items, (int32_t)blockIdx.x, [&](int32_t k) { return p.items[k].class_row_off; });
     const int32_t ns = p.items[i].n_splits;
     if (ns <= 1) return;      // the attention kernel already wrote the final output
-    const int64_t base = ((int64_t)row * p.Hq + h) * p.max_splits;
+    const int64_t row = p.items[i].q_row_off + ((int32_t)blockIdx.x - p.items[i].class_row_off);
+    const int64_t base = (row * p.Hq + h) * p.max_splits;
     float M = -INFINITY;
     for (int s = 0; s < ns; ++s) M = fmaxf(M, p.ws_ml[(base + s) * 2]);
     float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -99,7 +101,7 @@ merge_kernel(AttendParams p) {
     uint2 o;
     o.x = pack_bf16(acc.x * inv, acc.y * inv);
     o.y = pack_bf16(acc.z * inv, acc.w * inv);
-    reinterpret_cast<uint2*>(p.out + ((int64_t)row * p.Hq + h) * D)[threadIdx.x] = o;
+    reinterpret_cast<uint2*>(p.out + (row * p.Hq + h) * D)[threadIdx.x] = o;
 }
 
 }  // namespace metronome

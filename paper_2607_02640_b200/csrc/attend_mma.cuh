@@ -1,20 +1,35 @@
-// attend_mma.cuh -- rows a5 (GQA decode) and a7 (chunk prefill): tensor-core tile kernel.
+// attend_mma.cuh -- rows a5 (GQA decode) and a7 (chunk prefill) on the tensor cores.
 //
-// One CTA = one (split-KV segment, KV head).  The R = G x q_len query rows that share this KV head
-// (GQA group x chunk rows; "grouped-query attention", "mixed prefill/decode") form
-// up to 13 m16 row tiles, one per compute warp; the KV stream is read from HBM ONCE for all of
-// them.  A producer warp streams the sink tiles first and then the window tiles
-// ("extra leading iterations remapped onto the sink tiles ... accumulating them
-// first is exact") into a shared-memory ring with bulk async copies (cp.async.bulk -> UBLKCP, one
-// 8 KiB copy per (block, head) because layout.cuh keeps K|V of a block-head contiguous and
-// pre-swizzled), completion counted on mbarriers; compute warps release stages on "empty"
-// mbarriers.  Per 16-key tile a warp does S = Q K^T (mma.sync m16n8k16 bf16, K fragments by
-// ldmatrix), the token-exact union mask on boundary tiles only, an online softmax in the log2
-// domain with a warp-uniform skip of the rescale, and O += P V (V fragments by ldmatrix.trans).
+// The R = G x q_len query rows that share one KV head (GQA group x chunk rows; PAPER.md:L258
+// "grouped-query attention", "mixed prefill/decode") are cut into m16 row tiles, so the KV stream
+// is read from HBM ONCE for all of them.  Two kernels share the per-tile arithmetic (WarpTile):
 //
-// Why mma.sync and not tcgen05 here (round 1): decode has R <= 16 rows, one m16 tile at AI = G
-// flop/byte, far below what needs UMMA; the chunk tiles (R <= 208) are the candidate for a
-// tcgen05 path ("next").  The HBM layout is already UMMA's SWIZZLE_128B K-major.
+//   attend_gqa_kernel   R <= 16 (decode).  HBM-bound at G flop/byte.  The flattened list of
+//                       (item, KV head, tile) work is cut into EQUAL contiguous ranges, one per
+//                       CTA of a grid sized n_SM x CTAs/SM ("stream-K": ragged session ages cannot
+//                       unbalance the SMs); inside a CTA four warps take tiles round-robin, each
+//                       with a PRIVATE ring of bulk async copies (no CTA barrier in the loop),
+//                       and are merged through shared memory once per (item, head) piece.
+//   attend_mma_kernel   R <= 208 (chunk prefill).  One CTA per (segment, KV head), one compute warp
+//                       per m16 row tile, a producer warp streaming 64-key stages for all of them.
+//
+// Data movement: one cp.async.bulk (SASS UBLKCP) of 2*16*D*2 bytes per (block, head) -- layout.cuh
+// keeps K|V of a block-head contiguous and pre-swizzled -- completion counted on an mbarrier.
+// Sinks go first ("extra leading iterations remapped onto the sink tiles ...
+// accumulating them first is exact"); in split mode only the piece that holds them takes them.
+//
+// Per 16-key tile: S = Q K^T (mma.sync m16n8k16 bf16, K fragments by ldmatrix), token-exact union
+// mask on boundary tiles only, online softmax in the log2 domain with a warp-uniform skip of the
+// rescale, O += P V (V fragments by ldmatrix.trans).  Two accuracy devices, both on the tensor core:
+//   * the softmax denominator is accumulated from the SAME rounded P that multiplies V (an extra n8
+//     tile against a ones matrix), so numerator and denominator see identical weights;
+//   * P is split into bf16 hi + lo parts, and the lo MMA is issued only for tiles that hold a key
+//     whose weight exceeds 1/64 of the running sum (warp-uniform vote): peaky softmax rows (config
+//     4's x20 outlier channels) get ~2^-17 weights, flat rows pay nothing.
+//
+// Why mma.sync and not tcgen05 (round 1): decode is one m16 tile at G flop/byte; the chunk tiles are
+// the candidate for a tcgen05/TMEM path.  The HBM layout is already UMMA's
+// SWIZZLE_128B K-major.
 #pragma once
 #include "attend_common.cuh"
 
@@ -58,26 +73,197 @@ __device__ __forceinline__ void mma_bf16(float (&c)[4], const uint32_t (&a)[4], 
                  : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
 }
 
+// ------------------------------------------------------------------------------------------------
+// One m16 row tile, per-thread view.  Row rho = 16*mtile + lane/4 (a) and +8 (b); rho = r*G + g:
+// query row r of the call (position t_first + r), member g of the GQA group.
+template <int D>
+struct WarpTile {
+    static constexpr int KSTEPS = D / 16;   // k-steps of Q K^T
+    static constexpr int NT = D / 8;        // n8 tiles of P V
+    uint32_t qa[KSTEPS][4];
+    float o[NT][4];
+    float m_a, m_b;                          // running max per row, log2 domain (-inf: nothing admitted yet)
+    float lsum[4];                           // [0] row a, [2] row b: running sum, accumulated by the tensor core
+    int32_t ta, tb;                          // absolute position of rows a / b (-1: padding row, admits nothing)
+    int32_t t_min, t_max;                    // positions spanned by the tile's valid rows (warp-uniform)
+    bool va, vb;
+    int64_t qrow_a, qrow_b;                  // (query row, q head) flattened: row of q / out
+
+    __device__ __forceinline__ void init(const AttendParams& p, const AttendItem& it, int32_t kvh, int32_t mtile,
+                                         int32_t lane) {
+        const int32_t R = it.q_len * p.G;
+        const int32_t t_first = it.len - it.q_len;            // reading R15: the last q_len positions
+        const int32_t rho_a = 16 * mtile + (lane >> 2), rho_b = rho_a + 8;
+        va = rho_a < R; vb = rho_b < R;
+        const int32_t ra = rho_a / p.G, rb = rho_b / p.G;
+        ta = va ? t_first + ra : -1;
+        tb = vb ? t_first + rb : -1;
+        qrow_a = (int64_t)(it.q_row_off + ra) * p.Hq + kvh * p.G + (rho_a - ra * p.G);
+        qrow_b = (int64_t)(it.q_row_off + rb) * p.Hq + kvh * p.G + (rho_b - rb * p.G);
+        t_min = t_first + (16 * mtile) / p.G;
+        t_max = t_first + (min(R, 16 * mtile + 16) - 1) / p.G;
+        const uint32_t* pa = reinterpret_cast<const uint32_t*>(p.q + qrow_a * D);
+        const uint32_t* pb = reinterpret_cast<const uint32_t*>(p.q + qrow_b * D);
+        const int32_t c = lane & 3;
+#pragma unroll
+        for (int kk = 0; kk < KSTEPS; ++kk) {
+            qa[kk][0] = va ? __ldg(pa + kk * 8 + c) : 0u;
+            qa[kk][1] = vb ? __ldg(pb + kk * 8 + c) : 0u;
+            qa[kk][2] = va ? __ldg(pa + kk * 8 + 4 + c) : 0u;
+            qa[kk][3] = vb ? __ldg(pb + kk * 8 + 4 + c) : 0u;
+        }
+        reset();
+    }
+    __device__ __forceinline__ void reset() {
+#pragma unroll
+        for (int n = 0; n < NT; ++n) { o[n][0] = o[n][1] = o[n][2] = o[n][3] = 0.f; }
+        m_a = m_b = -INFINITY;
+        lsum[0] = lsum[1] = lsum[2] = lsum[3] = 0.f;
+    }
+
+    // true when no key of the 16-token tile at position p0 is admitted for any row (warp-uniform)
+    __device__ __forceinline__ bool skips(const AttendParams& p, int32_t p0) const {
+        return p0 > t_max || (p0 >= p.S && t_min - (p0 + kBlockTokens - 1) >= p.W);
+    }
+
+    // one 16-key tile: kt / vt are shared-memory addresses of the swizzled K and V tiles
+    __device__ __forceinline__ void step(const AttendParams& p, int32_t len, uint32_t kt, uint32_t vt, int32_t p0,
+                                         int32_t lane) {
+        const int32_t mat = lane >> 3, r8 = lane & 7;
+        const int32_t k_row = r8 + ((mat >> 1) << 3), k_cs = mat & 1;   // K: (rows 0-7 | 8-15) x (chunk, chunk+1)
+        const int32_t v_row = r8 + ((mat & 1) << 3), v_cs = mat >> 1;   // V: (chunk, chunk+1) x (rows 0-7 | 8-15)
+        const int32_t col0 = (lane & 3) * 2;
+        // ---- S = Q K^T: two n8 tiles ----
+        float s0[4] = {0.f, 0.f, 0.f, 0.f}, s1[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+        for (int kk = 0; kk < KSTEPS; ++kk) {
+            uint32_t b0, b1, b2, b3;
+            ldsm_x4(kt + tile_chunk_offset(k_row, 2 * kk + k_cs), b0, b1, b2, b3);
+            mma_bf16(s0, qa[kk], b0, b1);
+            mma_bf16(s1, qa[kk], b2, b3);
+        }
+        // ---- union mask, boundary tiles only ----
+        const bool full = (p0 + kBlockTokens - 1 <= t_min) && (p0 + kBlockTokens - 1 < p.S || t_max - p0 < p.W);
+        if (!full) {
+            const int32_t ja = p0 + col0, jb = ja + 8;
+            s0[0] = admit(ja, ta, p.S, p.W) ? s0[0] : -INFINITY;
+            s0[1] = admit(ja + 1, ta, p.S, p.W) ? s0[1] : -INFINITY;
+            s0[2] = admit(ja, tb, p.S, p.W) ? s0[2] : -INFINITY;
+            s0[3] = admit(ja + 1, tb, p.S, p.W) ? s0[3] : -INFINITY;
+            s1[0] = admit(jb, ta, p.S, p.W) ? s1[0] : -INFINITY;
+            s1[1] = admit(jb + 1, ta, p.S, p.W) ? s1[1] : -INFINITY;
+            s1[2] = admit(jb, tb, p.S, p.W) ? s1[2] : -INFINITY;
+            s1[3] = admit(jb + 1, tb, p.S, p.W) ? s1[3] : -INFINITY;
+        }
+        // ---- online softmax (log2 domain) ----
+        float mx_a = fmaxf(fmaxf(s0[0], s0[1]), fmaxf(s1[0], s1[1]));
+        float mx_b = fmaxf(fmaxf(s0[2], s0[3]), fmaxf(s1[2], s1[3]));
+        mx_a = fmaxf(mx_a, __shfl_xor_sync(0xffffffffu, mx_a, 1));
+        mx_a = fmaxf(mx_a, __shfl_xor_sync(0xffffffffu, mx_a, 2));
+        mx_b = fmaxf(mx_b, __shfl_xor_sync(0xffffffffu, mx_b, 1));
+        mx_b = fmaxf(mx_b, __shfl_xor_sync(0xffffffffu, mx_b, 2));
+        const float mn_a = fmaxf(m_a, mx_a * p.scale_log2), mn_b = fmaxf(m_b, mx_b * p.scale_log2);
+        if (__any_sync(0xffffffffu, (mn_a != m_a) || (mn_b != m_b))) {
+            const float ca = mn_a == -INFINITY ? 1.f : ex2(m_a - mn_a);
+            const float cb = mn_b == -INFINITY ? 1.f : ex2(m_b - mn_b);
+            lsum[0] *= ca; lsum[1] *= ca; lsum[2] *= cb; lsum[3] *= cb;
+#pragma unroll
+            for (int n = 0; n < NT; ++n) { o[n][0] *= ca; o[n][1] *= ca; o[n][2] *= cb; o[n][3] *= cb; }
+            m_a = mn_a; m_b = mn_b;
+        }
+        // a row with nothing admitted so far keeps m = -inf: subtract 0 instead (its p are all 0)
+        const float sub_a = m_a == -INFINITY ? 0.f : m_a, sub_b = m_b == -INFINITY ? 0.f : m_b;
+        float pr[8];
+        pr[0] = ex2(fmaf(s0[0], p.scale_log2, -sub_a)); pr[1] = ex2(fmaf(s0[1], p.scale_log2, -sub_a));
+        pr[2] = ex2(fmaf(s0[2], p.scale_log2, -sub_b)); pr[3] = ex2(fmaf(s0[3], p.scale_log2, -sub_b));
+        pr[4] = ex2(fmaf(s1[0], p.scale_log2, -sub_a)); pr[5] = ex2(fmaf(s1[1], p.scale_log2, -sub_a));
+        pr[6] = ex2(fmaf(s1[2], p.scale_log2, -sub_b)); pr[7] = ex2(fmaf(s1[3], p.scale_log2, -sub_b));
+        uint32_t hi[4], lo[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            hi[k] = pack_bf16(pr[2 * k], pr[2 * k + 1]);     // [0] row a keys col0.., [1] row b, [2] row a keys 8+col0.., [3] row b
+            lo[k] = pack_bf16(pr[2 * k] - bf16lo(hi[k]), pr[2 * k + 1] - bf16hi(hi[k]));
+        }
+        // lo part only where a key carries more than 1/64 of the running sum (warp-uniform)
+        const float pm_a = fmaxf(fmaxf(pr[0], pr[1]), fmaxf(pr[4], pr[5]));
+        const float pm_b = fmaxf(fmaxf(pr[2], pr[3]), fmaxf(pr[6], pr[7]));
+        const bool need_lo = __any_sync(0xffffffffu, (pm_a * 64.f > lsum[0]) || (pm_b * 64.f > lsum[2]));
+        constexpr uint32_t kOnes = 0x3F803F80u;              // bf16 (1, 1)
+        mma_bf16(lsum, hi, kOnes, kOnes);
+        if (need_lo) mma_bf16(lsum, lo, kOnes, kOnes);
+        // ---- O += P V; V rows past the session's length hold stale / poisoned bytes (0 * NaN) ----
+        const int32_t nvalid = len - p0;                     // < 16 only in the session's last block
+        uint32_t mk0 = 0xFFFFFFFFu, mk1 = 0xFFFFFFFFu;
+        if (nvalid < kBlockTokens) {
+            mk0 = (col0 < nvalid ? 0x0000FFFFu : 0u) | (col0 + 1 < nvalid ? 0xFFFF0000u : 0u);
+            mk1 = (col0 + 8 < nvalid ? 0x0000FFFFu : 0u) | (col0 + 9 < nvalid ? 0xFFFF0000u : 0u);
+        }
+#pragma unroll
+        for (int n = 0; n < NT; n += 2) {
+            uint32_t b0, b1, b2, b3;
+            ldsm_x4_t(vt + tile_chunk_offset(v_row, n + v_cs), b0, b1, b2, b3);
+            if (nvalid < kBlockTokens) { b0 &= mk0; b1 &= mk1; b2 &= mk0; b3 &= mk1; }
+            mma_bf16(o[n], hi, b0, b1);
+            mma_bf16(o[n + 1], hi, b2, b3);
+            if (need_lo) {
+                mma_bf16(o[n], lo, b0, b1);
+                mma_bf16(o[n + 1], lo, b2, b3);
+            }
+        }
+    }
+
+    // final bf16 output (the piece covered every tile of this (item, head))
+    __device__ __forceinline__ void store_final(const AttendParams& p, int32_t lane) const {
+        const float ia = lsum[0] > 0.f ? 1.f / lsum[0] : 0.f, ib = lsum[2] > 0.f ? 1.f / lsum[2] : 0.f;
+        uint32_t* oa = reinterpret_cast<uint32_t*>(p.out + qrow_a * D);
+        uint32_t* ob = reinterpret_cast<uint32_t*>(p.out + qrow_b * D);
+#pragma unroll
+        for (int n = 0; n < NT; ++n) {
+            if (va) oa[n * 4 + (lane & 3)] = pack_bf16(o[n][0] * ia, o[n][1] * ia);
+            if (vb) ob[n * 4 + (lane & 3)] = pack_bf16(o[n][2] * ib, o[n][3] * ib);
+        }
+    }
+    // unnormalised partial (acc, m, l) of one split-KV piece
+    __device__ __forceinline__ void store_partial(const AttendParams& p, int32_t piece, int32_t lane) const {
+        const int64_t slot_a = qrow_a * p.max_splits + piece, slot_b = qrow_b * p.max_splits + piece;
+        float2* wa = reinterpret_cast<float2*>(p.ws_acc + slot_a * D);
+        float2* wb = reinterpret_cast<float2*>(p.ws_acc + slot_b * D);
+#pragma unroll
+        for (int n = 0; n < NT; ++n) {
+            if (va) wa[n * 4 + (lane & 3)] = make_float2(o[n][0], o[n][1]);
+            if (vb) wb[n * 4 + (lane & 3)] = make_float2(o[n][2], o[n][3]);
+        }
+        if ((lane & 3) == 0) {
+            if (va) { p.ws_ml[slot_a * 2] = m_a; p.ws_ml[slot_a * 2 + 1] = lsum[0]; }
+            if (vb) { p.ws_ml[slot_b * 2] = m_b; p.ws_ml[slot_b * 2 + 1] = lsum[2]; }
+        }
+    }
+};
+
+// logical block and first token position of tile `tile` of an item (sinks first, then the window)
+__device__ __forceinline__ int32_t tile_block(const AttendItem& it, int32_t tile) {
+    return tile < it.n_sink_tiles ? tile : it.first_blk + (tile - it.n_sink_tiles);
+}
+
+// ================================================================================================
+// Chunk prefill: one CTA per (segment, KV head); NW compute warps (one m16 row tile each) + 1 producer.
 template <int D, int NW>
 struct MmaCfg {
-    static constexpr int KS = NW == 1 ? 2 : 4;          // key tiles (blocks) per pipeline stage
-    static constexpr int NS = NW == 1 ? 4 : 3;          // stages
+    static constexpr int KS = 4;                        // key tiles (blocks) per pipeline stage
+    static constexpr int NS = 3;                        // stages
     static constexpr int kHeadBytes = 2 * kBlockTokens * D * 2;
     static constexpr int kStageBytes = KS * kHeadBytes;
     static constexpr int kSmemBytes = NS * kStageBytes + 2 * NS * 8 + 128;
     static constexpr int kThreads = 32 * (NW + 1);
 };
 
-// grid = (total_splits, Hkv); block = 32 * (NW + 1): NW compute warps + 1 producer warp.
+// grid = (total_splits of the chunk-class items, Hkv)
 template <int D, int NW>
 __global__ void __launch_bounds__(MmaCfg<D, NW>::kThreads, 1)
 attend_mma_kernel(AttendParams p) {
     using C = MmaCfg<D, NW>;
-    constexpr int KSTEPS = D / 16;       // k-steps of Q K^T
-    constexpr int NT = D / 8;            // n-tiles of P V
     extern __shared__ __align__(128) uint8_t smem_raw[];
-    // 128-byte aligned stage buffers (rows of a tile are 128-byte swizzle atoms)
-    const uint32_t smem_base = (smem_u32(smem_raw) + 127u) & ~127u;
+    const uint32_t smem_base = (smem_u32(smem_raw) + 127u) & ~127u;     // tiles are 128-byte swizzle atoms
     const uint32_t bar_full = smem_base + C::NS * C::kStageBytes;
     const uint32_t bar_empty = bar_full + C::NS * 8;
 
@@ -86,7 +272,7 @@ attend_mma_kernel(AttendParams p) {
     const int32_t split = blockIdx.x - it.split_off;
     const int32_t kvh = blockIdx.y;
     const int32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int32_t R = it.q_len * p.G;                       // query rows sharing this KV head
+    const int32_t R = it.q_len * p.G;
     const int32_t nw_active = (R + 15) >> 4;                // compute warps with at least one row
     const int32_t tl0 = split * it.tiles_per_split;
     const int32_t tl1 = min(it.n_tiles, tl0 + it.tiles_per_split);
@@ -112,9 +298,7 @@ attend_mma_kernel(AttendParams p) {
             if (lane == 0) mbar_expect_tx(bar_full + 8 * slot, (uint32_t)nt * C::kHeadBytes);
             __syncwarp();
             if (lane < nt) {
-                const int32_t tile = t0 + lane;
-                const int32_t blk = tile < it.n_sink_tiles ? tile : it.first_blk + (tile - it.n_sink_tiles);
-                const int32_t phys = __ldg(trow + table_slot(blk, p.n_sink, p.ring));
+                const int32_t phys = __ldg(trow + table_slot(tile_block(it, t0 + lane), p.n_sink, p.ring));
                 const uint8_t* src = p.kv_layer + (int64_t)phys * p.L.block_bytes + (int64_t)kvh * p.L.head_bytes;
                 bulk_g2s(smem_base + slot * C::kStageBytes + lane * C::kHeadBytes, src, C::kHeadBytes, bar_full + 8 * slot);
             }
@@ -124,162 +308,216 @@ attend_mma_kernel(AttendParams p) {
     if (warp >= nw_active) return;
 
     // -------------------------------- compute warps --------------------------------
-    // rows of this warp's m16 tile: rho_a = 16*warp + lane/4, rho_b = rho_a + 8; rho = r*G + g
-    const int32_t t_first = it.len - it.q_len;              // position of query row 0 (reading R15)
-    const int32_t rho_a = 16 * warp + (lane >> 2), rho_b = rho_a + 8;
-    const bool va = rho_a < R, vb = rho_b < R;
-    const int32_t ra = rho_a / p.G, rb = rho_b / p.G;
-    const int32_t ta = va ? t_first + ra : -1, tb = vb ? t_first + rb : -1;   // -1: admits nothing
-    const int64_t qrow_a = (int64_t)(it.q_row_off + ra) * p.Hq + kvh * p.G + (rho_a - ra * p.G);
-    const int64_t qrow_b = (int64_t)(it.q_row_off + rb) * p.Hq + kvh * p.G + (rho_b - rb * p.G);
-    // positions spanned by the valid rows of this warp (warp-uniform)
-    const int32_t r_lo = (16 * warp) / p.G, r_hi = (min(R, 16 * warp + 16) - 1) / p.G;
-    const int32_t t_min = t_first + r_lo, t_max = t_first + r_hi;
-
-    uint32_t qa[KSTEPS][4];
-    {
-        const uint32_t* pa = reinterpret_cast<const uint32_t*>(p.q + qrow_a * D);
-        const uint32_t* pb = reinterpret_cast<const uint32_t*>(p.q + qrow_b * D);
-        const int32_t c = lane & 3;
-#pragma unroll
-        for (int kk = 0; kk < KSTEPS; ++kk) {
-            qa[kk][0] = va ? __ldg(pa + kk * 8 + c) : 0u;
-            qa[kk][1] = vb ? __ldg(pb + kk * 8 + c) : 0u;
-            qa[kk][2] = va ? __ldg(pa + kk * 8 + 4 + c) : 0u;
-            qa[kk][3] = vb ? __ldg(pb + kk * 8 + 4 + c) : 0u;
-        }
-    }
-
-    float o[NT][4];
-#pragma unroll
-    for (int n = 0; n < NT; ++n) { o[n][0] = o[n][1] = o[n][2] = o[n][3] = 0.f; }
-    // running max per row (log2 domain) and running sum.  The sum is accumulated BY THE TENSOR CORE
-    // from the same bf16-rounded P that multiplies V (one extra n8 tile against a ones matrix), so
-    // numerator and denominator see identical weights: with one dominant key (outlier channels,
-    // config 4) the rounding of P cancels instead of scaling the output.
-    float m_a = -INFINITY, m_b = -INFINITY;
-    float lsum[4] = {0.f, 0.f, 0.f, 0.f};
-    constexpr uint32_t kOnes = 0x3F803F80u;   // bf16 (1, 1)
-
-    // ldmatrix lane roles
-    const int32_t mat = lane >> 3, r8 = lane & 7;
-    const int32_t k_row = r8 + ((mat >> 1) << 3), k_cs = mat & 1;      // K: matrices (rows 0-7|8-15) x (chunk, chunk+1)
-    const int32_t v_row = r8 + ((mat & 1) << 3), v_cs = mat >> 1;      // V: matrices (chunk, chunk+1) x (rows 0-7|8-15)
-    const int32_t col0 = (lane & 3) * 2;
-
+    WarpTile<D> wt;
+    wt.init(p, it, kvh, warp, lane);
     for (int32_t s = 0; s < n_stage; ++s) {
         const int32_t slot = s % C::NS;
         mbar_wait(bar_full + 8 * slot, (s / C::NS) & 1);
         const int32_t tbase = tl0 + s * C::KS;
         const int32_t nt = min(C::KS, tl1 - tbase);
         for (int32_t j = 0; j < nt; ++j) {
-            const int32_t tile = tbase + j;
-            const int32_t blk = tile < it.n_sink_tiles ? tile : it.first_blk + (tile - it.n_sink_tiles);
-            const int32_t p0 = blk * kBlockTokens;
-            // no admitted key for any row of this warp: skip (warp-uniform)
-            if (p0 > t_max || (p0 >= p.S && t_min - (p0 + kBlockTokens - 1) >= p.W)) continue;
+            const int32_t p0 = tile_block(it, tbase + j) * kBlockTokens;
+            if (wt.skips(p, p0)) continue;
             const uint32_t kt = smem_base + slot * C::kStageBytes + j * C::kHeadBytes;
-            const uint32_t vt = kt + kBlockTokens * D * 2;
-
-            // ---- S = Q K^T over this 16-key tile: two n8 tiles ----
-            float s0[4] = {0.f, 0.f, 0.f, 0.f}, s1[4] = {0.f, 0.f, 0.f, 0.f};
-#pragma unroll
-            for (int kk = 0; kk < KSTEPS; ++kk) {
-                uint32_t b0, b1, b2, b3;
-                ldsm_x4(kt + tile_chunk_offset(k_row, 2 * kk + k_cs), b0, b1, b2, b3);
-                mma_bf16(s0, qa[kk], b0, b1);
-                mma_bf16(s1, qa[kk], b2, b3);
-            }
-            // ---- mask (boundary tiles only) ----
-            const bool full = (p0 + kBlockTokens - 1 <= t_min) &&
-                              (p0 + kBlockTokens - 1 < p.S || t_max - p0 < p.W);
-            if (!full) {
-                const int32_t ja = p0 + col0, jb = ja + 8;
-                s0[0] = admit(ja, ta, p.S, p.W) ? s0[0] : -INFINITY;
-                s0[1] = admit(ja + 1, ta, p.S, p.W) ? s0[1] : -INFINITY;
-                s0[2] = admit(ja, tb, p.S, p.W) ? s0[2] : -INFINITY;
-                s0[3] = admit(ja + 1, tb, p.S, p.W) ? s0[3] : -INFINITY;
-                s1[0] = admit(jb, ta, p.S, p.W) ? s1[0] : -INFINITY;
-                s1[1] = admit(jb + 1, ta, p.S, p.W) ? s1[1] : -INFINITY;
-                s1[2] = admit(jb, tb, p.S, p.W) ? s1[2] : -INFINITY;
-                s1[3] = admit(jb + 1, tb, p.S, p.W) ? s1[3] : -INFINITY;
-            }
-            // ---- online softmax (log2 domain) ----
-            float mx_a = fmaxf(fmaxf(s0[0], s0[1]), fmaxf(s1[0], s1[1]));
-            float mx_b = fmaxf(fmaxf(s0[2], s0[3]), fmaxf(s1[2], s1[3]));
-            mx_a = fmaxf(mx_a, __shfl_xor_sync(0xffffffffu, mx_a, 1));
-            mx_a = fmaxf(mx_a, __shfl_xor_sync(0xffffffffu, mx_a, 2));
-            mx_b = fmaxf(mx_b, __shfl_xor_sync(0xffffffffu, mx_b, 1));
-            mx_b = fmaxf(mx_b, __shfl_xor_sync(0xffffffffu, mx_b, 2));
-            const float mn_a = fmaxf(m_a, mx_a * p.scale_log2), mn_b = fmaxf(m_b, mx_b * p.scale_log2);
-            const bool grow = (mn_a != m_a) || (mn_b != m_b);
-            if (__any_sync(0xffffffffu, grow)) {
-                const float ca = mn_a == -INFINITY ? 1.f : ex2(m_a - mn_a);
-                const float cb = mn_b == -INFINITY ? 1.f : ex2(m_b - mn_b);
-                lsum[0] *= ca; lsum[1] *= ca; lsum[2] *= cb; lsum[3] *= cb;
-#pragma unroll
-                for (int n = 0; n < NT; ++n) { o[n][0] *= ca; o[n][1] *= ca; o[n][2] *= cb; o[n][3] *= cb; }
-                m_a = mn_a; m_b = mn_b;
-            }
-            // a row with nothing admitted so far keeps m = -inf: use 0 as the subtrahend (p = 0)
-            const float sub_a = m_a == -INFINITY ? 0.f : m_a, sub_b = m_b == -INFINITY ? 0.f : m_b;
-            const float p00 = ex2(fmaf(s0[0], p.scale_log2, -sub_a)), p01 = ex2(fmaf(s0[1], p.scale_log2, -sub_a));
-            const float p02 = ex2(fmaf(s0[2], p.scale_log2, -sub_b)), p03 = ex2(fmaf(s0[3], p.scale_log2, -sub_b));
-            const float p10 = ex2(fmaf(s1[0], p.scale_log2, -sub_a)), p11 = ex2(fmaf(s1[1], p.scale_log2, -sub_a));
-            const float p12 = ex2(fmaf(s1[2], p.scale_log2, -sub_b)), p13 = ex2(fmaf(s1[3], p.scale_log2, -sub_b));
-            uint32_t pa[4];
-            pa[0] = pack_bf16(p00, p01);   // row a, keys col0..col0+1
-            pa[1] = pack_bf16(p02, p03);   // row b
-            pa[2] = pack_bf16(p10, p11);   // row a, keys 8+col0..
-            pa[3] = pack_bf16(p12, p13);   // row b
-            mma_bf16(lsum, pa, kOnes, kOnes);
-            // ---- O += P V ; rows of V past the session's length hold stale / poisoned bytes ----
-            const int32_t nvalid = it.len - p0;           // < 16 only in the session's last block
-            uint32_t mk0 = 0xFFFFFFFFu, mk1 = 0xFFFFFFFFu;
-            if (nvalid < kBlockTokens) {
-                mk0 = (col0 < nvalid ? 0x0000FFFFu : 0u) | (col0 + 1 < nvalid ? 0xFFFF0000u : 0u);
-                mk1 = (col0 + 8 < nvalid ? 0x0000FFFFu : 0u) | (col0 + 9 < nvalid ? 0xFFFF0000u : 0u);
-            }
-#pragma unroll
-            for (int n = 0; n < NT; n += 2) {
-                uint32_t b0, b1, b2, b3;
-                ldsm_x4_t(vt + tile_chunk_offset(v_row, n + v_cs), b0, b1, b2, b3);
-                if (nvalid < kBlockTokens) { b0 &= mk0; b1 &= mk1; b2 &= mk0; b3 &= mk1; }
-                mma_bf16(o[n], pa, b0, b1);
-                mma_bf16(o[n + 1], pa, b2, b3);
-            }
+            wt.step(p, it.len, kt, kt + kBlockTokens * D * 2, p0, lane);
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(bar_empty + 8 * slot);
     }
+    if (it.n_splits == 1) wt.store_final(p, lane);
+    else wt.store_partial(p, split, lane);
+}
 
-    // ---- epilogue ----
-    const float l_a = lsum[0], l_b = lsum[2];     // every column of the ones tile holds the row sum
-    if (it.n_splits == 1) {
-        const float ia = l_a > 0.f ? 1.f / l_a : 0.f, ib = l_b > 0.f ? 1.f / l_b : 0.f;
-        uint32_t* oa = reinterpret_cast<uint32_t*>(p.out + qrow_a * D);
-        uint32_t* ob = reinterpret_cast<uint32_t*>(p.out + qrow_b * D);
+// ================================================================================================
+// GQA decode (R <= 16): stream-K partition of the flattened (item, KV head, tile) list.
+template <int D>
+struct GqaCfg {
+    static constexpr int NWARP = 4;
+    static constexpr int NS = 2;                        // private stages per warp, one 16-key tile each
+    static constexpr int kHeadBytes = 2 * kBlockTokens * D * 2;
+    static constexpr int kWarpBytes = NS * kHeadBytes;
+    static constexpr int kSmemBytes = NWARP * kWarpBytes + NWARP * NS * 8 + 128;
+    static constexpr int kThreads = 32 * NWARP;
+    // the merge of the 4 warps reuses the rings: 16 rows x (D + 2) floats per warp must fit
+    static_assert(16 * (D + 2) * 4 <= kWarpBytes, "merge scratch does not fit a warp's ring");
+};
+
+struct GqaPlan {
+    int32_t n_kv_heads;
+    int64_t total_tiles;      // Hkv * sum of the items' n_tiles
+    int64_t tiles_per_cta;    // ceil(total_tiles / gridDim.x)
+};
+
+// piece index of CTA `cta` within the (item, head) pair whose global tile range starts at pair_lo
+__device__ __forceinline__ int32_t gqa_first_cta(int64_t pair_lo, int64_t q) { return (int32_t)(pair_lo / q); }
+
+// grid = n_SM * CTAs/SM (<= total tiles), block = 128.  items[].tile_off = exclusive prefix of n_tiles.
+template <int D>
+__global__ void __launch_bounds__(GqaCfg<D>::kThreads)
+attend_gqa_kernel(AttendParams p, GqaPlan plan) {
+    using C = GqaCfg<D>;
+    extern __shared__ __align__(128) uint8_t smem_raw[];
+    const uint32_t smem_base = (smem_u32(smem_raw) + 127u) & ~127u;
+    uint8_t* smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
+    const int32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const uint32_t ring = smem_base + warp * C::kWarpBytes;
+    const uint32_t bars = smem_base + C::NWARP * C::kWarpBytes + warp * C::NS * 8;
+    if (lane == 0) {
+        for (int s = 0; s < C::NS; ++s) mbar_init(bars + 8 * s, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    uint32_t phase_bits = 0;                             // parity of each private stage
+
+    const int64_t q = plan.tiles_per_cta;
+    int64_t g = (int64_t)blockIdx.x * q;
+    const int64_t g_end = min(plan.total_tiles, g + q);
+    const int32_t Hkv = plan.n_kv_heads;
+
+    while (g < g_end) {
+        // ---- the (item, head) pair that holds global tile g, and this CTA's piece of it ----
+        int32_t i = 0;
+        {
+            int32_t lo = 0, hi = p.n_items - 1;        // largest i with tile_off[i] * Hkv <= g
+            while (lo < hi) {
+                const int32_t mid = (lo + hi + 1) >> 1;
+                if ((int64_t)p.items[mid].tile_off * Hkv <= g) lo = mid; else hi = mid - 1;
+            }
+            i = lo;
+        }
+        const AttendItem it = p.items[i];
+        const int64_t item_lo = (int64_t)it.tile_off * Hkv;
+        const int32_t kvh = (int32_t)((g - item_lo) / it.n_tiles);
+        const int64_t pair_lo = item_lo + (int64_t)kvh * it.n_tiles;
+        const int32_t a = (int32_t)(g - pair_lo);
+        const int32_t b = (int32_t)min((int64_t)it.n_tiles, g_end - pair_lo);
+        const int32_t first_cta = gqa_first_cta(pair_lo, q);
+        const int32_t last_cta = gqa_first_cta(pair_lo + it.n_tiles - 1, q);
+
+        WarpTile<D> wt;
+        wt.init(p, it, kvh, 0, lane);
+        const int32_t* trow = p.table + (int64_t)it.sid * p.tbl_width;
+        const uint8_t* head_base = p.kv_layer + (int64_t)kvh * p.L.head_bytes;
+        // this warp's tiles: a + warp, a + warp + 4, ...   (private ring, prologue fills NS stages)
+        const int32_t n_mine = (b - a - warp + C::NWARP - 1) / C::NWARP;
+        auto issue = [&](int32_t k) {      // k-th tile of this warp -> stage k % NS
+            if (lane == 0) {
+                const int32_t tile = a + warp + k * C::NWARP;
+                const int32_t phys = __ldg(trow + table_slot(tile_block(it, tile), p.n_sink, p.ring));
+                const uint32_t bar = bars + 8 * (k % C::NS);
+                mbar_expect_tx(bar, C::kHeadBytes);
+                bulk_g2s(ring + (k % C::NS) * C::kHeadBytes, head_base + (int64_t)phys * p.L.block_bytes, C::kHeadBytes, bar);
+            }
+        };
+        for (int32_t k = 0; k < min(n_mine, C::NS); ++k) issue(k);
+        for (int32_t k = 0; k < n_mine; ++k) {
+            const int32_t st = k % C::NS;
+            mbar_wait(bars + 8 * st, (phase_bits >> st) & 1u);
+            phase_bits ^= 1u << st;
+            const int32_t p0 = tile_block(it, a + warp + k * C::NWARP) * kBlockTokens;
+            const uint32_t kt = ring + st * C::kHeadBytes;
+            if (!wt.skips(p, p0)) wt.step(p, it.len, kt, kt + kBlockTokens * D * 2, p0, lane);
+            __syncwarp();                                  // every lane is done reading the stage
+            if (k + C::NS < n_mine) issue(k + C::NS);
+        }
+        // ---- merge the four warps through shared memory (their rings are idle now) ----
+        __syncthreads();
+        float* scratch = reinterpret_cast<float*>(smem_gen + warp * C::kWarpBytes);   // [16][D + 2]
+        {
+            const int32_t ra = lane >> 2, c = (lane & 3) * 2;
 #pragma unroll
-        for (int n = 0; n < NT; ++n) {
-            if (va) oa[n * 4 + (lane & 3)] = pack_bf16(o[n][0] * ia, o[n][1] * ia);
-            if (vb) ob[n * 4 + (lane & 3)] = pack_bf16(o[n][2] * ib, o[n][3] * ib);
+            for (int n = 0; n < WarpTile<D>::NT; ++n) {
+                *reinterpret_cast<float2*>(scratch + ra * (D + 2) + n * 8 + c) = make_float2(wt.o[n][0], wt.o[n][1]);
+                *reinterpret_cast<float2*>(scratch + (ra + 8) * (D + 2) + n * 8 + c) = make_float2(wt.o[n][2], wt.o[n][3]);
+            }
+            if ((lane & 3) == 0) {
+                scratch[ra * (D + 2) + D] = wt.m_a; scratch[ra * (D + 2) + D + 1] = wt.lsum[0];
+                scratch[(ra + 8) * (D + 2) + D] = wt.m_b; scratch[(ra + 8) * (D + 2) + D + 1] = wt.lsum[2];
+            }
         }
-    } else {
-        const int64_t slot_a = qrow_a * p.max_splits + split, slot_b = qrow_b * p.max_splits + split;
-        float2* wa = reinterpret_cast<float2*>(p.ws_acc + slot_a * D);
-        float2* wb = reinterpret_cast<float2*>(p.ws_acc + slot_b * D);
+        __syncthreads();
+        {
+            // 128 threads: row = tid / 8 (16 rows), 8 threads x (D/8) consecutive dims each
+            const int32_t row = threadIdx.x >> 3, sub = threadIdx.x & 7;
+            const int32_t R = it.q_len * p.G;
+            if (row < R) {
+                const float* sc = reinterpret_cast<const float*>(smem_gen);
+                float M = -INFINITY;
 #pragma unroll
-        for (int n = 0; n < NT; ++n) {
-            if (va) wa[n * 4 + (lane & 3)] = make_float2(o[n][0], o[n][1]);
-            if (vb) wb[n * 4 + (lane & 3)] = make_float2(o[n][2], o[n][3]);
+                for (int w = 0; w < C::NWARP; ++w) M = fmaxf(M, sc[w * (C::kWarpBytes / 4) + row * (D + 2) + D]);
+                float wgt[C::NWARP], l = 0.f;
+#pragma unroll
+                for (int w = 0; w < C::NWARP; ++w) {
+                    const float mw = sc[w * (C::kWarpBytes / 4) + row * (D + 2) + D];
+                    wgt[w] = (mw == -INFINITY) ? 0.f : ex2(mw - M);
+                    l += wgt[w] * sc[w * (C::kWarpBytes / 4) + row * (D + 2) + D + 1];
+                }
+                const int32_t r = row / p.G, gq = row - r * p.G;
+                const int64_t qrow = (int64_t)(it.q_row_off + r) * p.Hq + kvh * p.G + gq;
+                constexpr int DPT = D / 8;                    // dims per thread
+                float acc[DPT];
+#pragma unroll
+                for (int d = 0; d < DPT; ++d) {
+                    float v = 0.f;
+#pragma unroll
+                    for (int w = 0; w < C::NWARP; ++w) v += wgt[w] * sc[w * (C::kWarpBytes / 4) + row * (D + 2) + sub * DPT + d];
+                    acc[d] = v;
+                }
+                if (first_cta == last_cta) {
+                    const float inv = l > 0.f ? 1.f / l : 0.f;
+                    uint32_t* dst = reinterpret_cast<uint32_t*>(p.out + qrow * D + sub * DPT);
+#pragma unroll
+                    for (int d = 0; d < DPT; d += 2) dst[d >> 1] = pack_bf16(acc[d] * inv, acc[d + 1] * inv);
+                } else {
+                    const int64_t slot = qrow * p.max_splits + ((int32_t)blockIdx.x - first_cta);
+                    float* dst = p.ws_acc + slot * D + sub * DPT;
+#pragma unroll
+                    for (int d = 0; d < DPT; ++d) dst[d] = acc[d];
+                    if (sub == 0) { p.ws_ml[slot * 2] = M; p.ws_ml[slot * 2 + 1] = l; }
+                }
+            }
         }
-        if ((lane & 3) == 0) {
-            if (va) { p.ws_ml[slot_a * 2] = m_a; p.ws_ml[slot_a * 2 + 1] = l_a; }
-            if (vb) { p.ws_ml[slot_b * 2] = m_b; p.ws_ml[slot_b * 2 + 1] = l_b; }
-        }
+        // scratch (generic-proxy stores) is dead before the rings are refilled by the async proxy
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncthreads();
+        g = pair_lo + b;
     }
 }
 
+// Merge of the stream-K pieces of the decode-class items.  grid = (n decode-class rows, Hq), block = D/4.
+template <int D>
+__global__ void __launch_bounds__(D / 4)
+merge_gqa_kernel(AttendParams p, GqaPlan plan) {
+    const int32_t h = blockIdx.y;
+    const int32_t i = find_item(p.n_items, (int32_t)blockIdx.x, [&](int32_t k) { return p.items[k].class_row_off; });
+    const AttendItem it = p.items[i];
+    const int32_t kvh = h / p.G;
+    const int64_t pair_lo = ((int64_t)it.tile_off * plan.n_kv_heads) + (int64_t)kvh * it.n_tiles;
+    const int32_t first_cta = gqa_first_cta(pair_lo, plan.tiles_per_cta);
+    const int32_t ns = gqa_first_cta(pair_lo + it.n_tiles - 1, plan.tiles_per_cta) - first_cta + 1;
+    if (ns <= 1) return;
+    const int64_t grow = (int64_t)it.q_row_off + ((int32_t)blockIdx.x - it.class_row_off);
+    const int64_t base = (grow * p.Hq + h) * p.max_splits;
+    float M = -INFINITY;
+    for (int s = 0; s < ns; ++s) M = fmaxf(M, p.ws_ml[(base + s) * 2]);
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+    float l = 0.f;
+    for (int s = 0; s < ns; ++s) {
+        const float m = p.ws_ml[(base + s) * 2];
+        if (m == -INFINITY) continue;
+        const float w = ex2(m - M);
+        l += w * p.ws_ml[(base + s) * 2 + 1];
+        const float4 a = reinterpret_cast<const float4*>(p.ws_acc + (base + s) * D)[threadIdx.x];
+        acc.x += w * a.x; acc.y += w * a.y; acc.z += w * a.z; acc.w += w * a.w;
+    }
+    const float inv = l > 0.f ? 1.f / l : 0.f;
+    uint2 o;
+    o.x = pack_bf16(acc.x * inv, acc.y * inv);
+    o.y = pack_bf16(acc.z * inv, acc.w * inv);
+    reinterpret_cast<uint2*>(p.out + (grow * p.Hq + h) * D)[threadIdx.x] = o;
+}
+
+// ------------------------------------------------------------------------------------------------
 constexpr int kMmaMaxRows = 13 * 16;
 
 inline bool attend_mma_supported(int32_t G, int32_t max_q) { return (int64_t)G * max_q <= kMmaMaxRows; }
@@ -292,35 +530,40 @@ inline cudaError_t configure_one() {
 
 inline cudaError_t configure_attend_mma_kernels() {
     cudaError_t e;
-    if ((e = configure_one<128, 1>()) != cudaSuccess) return e;
     if ((e = configure_one<128, 4>()) != cudaSuccess) return e;
     if ((e = configure_one<128, 8>()) != cudaSuccess) return e;
     if ((e = configure_one<128, 13>()) != cudaSuccess) return e;
-    if ((e = configure_one<64, 1>()) != cudaSuccess) return e;
     if ((e = configure_one<64, 4>()) != cudaSuccess) return e;
     if ((e = configure_one<64, 8>()) != cudaSuccess) return e;
     if ((e = configure_one<64, 13>()) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(attend_gqa_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  GqaCfg<128>::kSmemBytes)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(attend_gqa_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  GqaCfg<64>::kSmemBytes)) != cudaSuccess) return e;
     return cudaSuccess;
 }
 
-template <int D>
-inline int launch_attend_mma_d(const AttendParams& p, int32_t Hkv, int32_t total_splits, int32_t max_rows,
-                               cudaStream_t st) {
+// chunk-class items (16 < R <= 208): p.items / p.n_items must point at them
+inline void launch_attend_mma(const AttendParams& p, int32_t D, int32_t Hkv, int32_t total_splits, int32_t max_rows,
+                              cudaStream_t st) {
     dim3 grid(total_splits, Hkv);
-    if (max_rows <= 16) attend_mma_kernel<D, 1><<<grid, MmaCfg<D, 1>::kThreads, MmaCfg<D, 1>::kSmemBytes, st>>>(p);
-    else if (max_rows <= 64) attend_mma_kernel<D, 4><<<grid, MmaCfg<D, 4>::kThreads, MmaCfg<D, 4>::kSmemBytes, st>>>(p);
-    else if (max_rows <= 128) attend_mma_kernel<D, 8><<<grid, MmaCfg<D, 8>::kThreads, MmaCfg<D, 8>::kSmemBytes, st>>>(p);
-    else attend_mma_kernel<D, 13><<<grid, MmaCfg<D, 13>::kThreads, MmaCfg<D, 13>::kSmemBytes, st>>>(p);
-    return 0;
+#define METRONOME_LAUNCH_MMA(DD)                                                                                   \
+    if (max_rows <= 64) attend_mma_kernel<DD, 4><<<grid, MmaCfg<DD, 4>::kThreads, MmaCfg<DD, 4>::kSmemBytes, st>>>(p); \
+    else if (max_rows <= 128) attend_mma_kernel<DD, 8><<<grid, MmaCfg<DD, 8>::kThreads, MmaCfg<DD, 8>::kSmemBytes, st>>>(p); \
+    else attend_mma_kernel<DD, 13><<<grid, MmaCfg<DD, 13>::kThreads, MmaCfg<DD, 13>::kSmemBytes, st>>>(p);
+    if (D == 128) { METRONOME_LAUNCH_MMA(128) } else { METRONOME_LAUNCH_MMA(64) }
+#undef METRONOME_LAUNCH_MMA
 }
 
-// returns 0 when a kernel was launched
-inline int launch_attend_mma(const AttendParams& p, int32_t D, int32_t Hkv, int32_t total_splits, int32_t max_q,
-                             cudaStream_t st) {
-    const int32_t max_rows = p.G * max_q;
-    if (max_rows > kMmaMaxRows) return 1;
-    return D == 128 ? launch_attend_mma_d<128>(p, Hkv, total_splits, max_rows, st)
-                    : launch_attend_mma_d<64>(p, Hkv, total_splits, max_rows, st);
+// decode-class items (R <= 16)
+inline void launch_attend_gqa(const AttendParams& p, const GqaPlan& plan, int32_t D, int32_t n_ctas, cudaStream_t st) {
+    if (D == 128) attend_gqa_kernel<128><<<n_ctas, GqaCfg<128>::kThreads, GqaCfg<128>::kSmemBytes, st>>>(p, plan);
+    else attend_gqa_kernel<64><<<n_ctas, GqaCfg<64>::kThreads, GqaCfg<64>::kSmemBytes, st>>>(p, plan);
+}
+inline void launch_merge_gqa(const AttendParams& p, const GqaPlan& plan, int32_t D, int32_t n_rows, cudaStream_t st) {
+    dim3 grid(n_rows, p.Hq);
+    if (D == 128) merge_gqa_kernel<128><<<grid, 32, 0, st>>>(p, plan);
+    else merge_gqa_kernel<64><<<grid, 16, 0, st>>>(p, plan);
 }
 
 }  // namespace metronome

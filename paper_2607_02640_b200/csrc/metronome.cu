@@ -485,18 +485,38 @@ int metronome_attend_frame(metronome_pool_t* pool, int32_t layer, int32_t n_batc
     cudaStream_t st = (cudaStream_t)cuda_stream;
 
     // ---- row a8: the per-call work list, from the shadow counts ------------------------------
+    // Kernel families (north_star: "Tensor cores are used only for the GQA-group x chunk QK^T/PV
+    // tiles, where the work really is a dense contraction"):
+    //   rows   CUDA-core row kernel: pure multi-head decode (G x q_len < 4 for every item), and the
+    //          general fallback
+    //   gqa    tensor-core stream-K decode kernel: items with R = G x q_len <= 16
+    //   chunk  tensor-core chunk-prefill kernel:   items with 16 < R <= 208
+    int32_t max_q = 0;
+    for (int i = 0; i < n_batch; ++i)
+        if (q_lens[i] > max_q) max_q = q_lens[i];
+    int family = pool->tune_family;
+    if (family == 0) family = (pool->G * max_q >= 4) ? 2 : 1;
+    if (family == 2 && !attend_mma_supported(pool->G, max_q)) family = 1;
+
     uint8_t *h = nullptr, *d = nullptr;
     int slot = 0;
     rc = acquire_stage(pool, &h, &d, &slot);
     if (rc) return rc;
     AttendItem* items = reinterpret_cast<AttendItem*>(h);
     const int32_t S = pool->unbounded ? 0 : c.n_sinks, W = pool->W_eff;
-    int32_t n_items = 0, row = 0, max_q = 0;
-    int64_t mma_units = 0, rows_units = 0;   // tile visits if every item took 1 split
+    // class 0 = rows kernel or gqa kernel (placed first), class 1 = chunk kernel (placed after)
+    int32_t n_cls[2] = {0, 0};
+    if (family == 2)
+        for (int i = 0; i < n_batch; ++i)
+            if (q_lens[i] > 0) ++n_cls[pool->G * q_lens[i] > 16 ? 1 : 0];
+    int32_t fill[2] = {0, n_cls[0]};
+    int32_t row = 0, n_items = 0;
     for (int i = 0; i < n_batch; ++i) {
         if (q_lens[i] == 0) continue;
         const Session& s = pool->sessions[sids[i]];
-        AttendItem& it = items[n_items++];
+        const int cls = (family == 2 && pool->G * q_lens[i] > 16) ? 1 : 0;
+        AttendItem& it = items[family == 2 ? fill[cls]++ : n_items];
+        ++n_items;
         memset(&it, 0, sizeof(it));
         it.sid = sids[i];
         it.len = (int32_t)s.len;
@@ -511,37 +531,62 @@ int metronome_attend_frame(metronome_pool_t* pool, int32_t layer, int32_t n_batc
         it.n_sink_tiles = n_blk < pool->n_sink ? n_blk : pool->n_sink;
         it.first_blk = first_blk;
         it.n_tiles = it.n_sink_tiles + (n_blk > first_blk ? n_blk - first_blk : 0);
-        if (it.q_len > max_q) max_q = it.q_len;
-        mma_units += (int64_t)it.n_tiles * c.n_kv_heads;
-        rows_units += (int64_t)it.n_tiles * c.n_q_heads * it.q_len;
     }
-    // kernel family: CUDA-core row kernel for pure multi-head decode, tensor-core tile kernel when
-    // G x q_len rows share one KV stream (north_star: "Tensor cores are used only for the GQA-group x
-    // chunk QK^T/PV tiles, where the work really is a dense contraction")
-    int family = pool->tune_family;
-    if (family == 0) family = (pool->G * max_q >= 4) ? 2 : 1;
-    if (family == 2 && !attend_mma_supported(pool->G, max_q)) family = 1;
-    // split-KV: enough CTAs for >= 2 waves, each with a useful run of tiles
-    const int64_t units = family == 2 ? mma_units : rows_units;
-    const int64_t target_ctas = (int64_t)pool->n_sm * (family == 2 ? 4 : 16);
-    int32_t tps = pool->tune_split_tokens > 0 ? (pool->tune_split_tokens + kBlockTokens - 1) / kBlockTokens
-                                              : (int32_t)((units + target_ctas - 1) / target_ctas);
-    const int32_t min_tps = family == 2 ? 8 : 8;
-    if (pool->tune_split_tokens <= 0 && tps < min_tps) tps = min_tps;
-    if (tps < 1) tps = 1;
-    int32_t total_splits = 0, max_splits = 1;
-    for (int i = 0; i < n_items; ++i) {
-        AttendItem& it = items[i];
-        int32_t ns = (it.n_tiles + tps - 1) / tps;
-        if (ns > kMaxSplits) ns = kMaxSplits;
-        if (ns < 1) ns = 1;
-        it.n_splits = ns;
-        it.tiles_per_split = (it.n_tiles + ns - 1) / ns;
-        it.n_splits = (it.n_tiles + it.tiles_per_split - 1) / it.tiles_per_split;
-        if (it.n_splits < 1) it.n_splits = 1;
-        it.split_off = total_splits;
-        total_splits += it.n_splits;
-        if (it.n_splits > max_splits) max_splits = it.n_splits;
+    if (family != 2) { n_cls[0] = n_items; n_cls[1] = 0; }
+
+    // per-class prefix sums, split-KV plan
+    int32_t total_splits[2] = {0, 0}, max_splits = 1, cls_rows[2] = {0, 0}, cls_max_q[2] = {0, 0};
+    int64_t cls_tiles[2] = {0, 0};
+    GqaPlan gplan{};
+    int32_t gqa_ctas = 0;
+    for (int cls = 0; cls < 2; ++cls) {
+        AttendItem* its = items + (cls == 0 ? 0 : n_cls[0]);
+        const int32_t n = n_cls[cls];
+        if (n == 0) continue;
+        int64_t units = 0;           // tile visits of this class's CTAs if nothing were split
+        for (int i = 0; i < n; ++i) {
+            its[i].tile_off = (int32_t)cls_tiles[cls];
+            its[i].class_row_off = cls_rows[cls];
+            cls_tiles[cls] += its[i].n_tiles;
+            cls_rows[cls] += its[i].q_len;
+            if (its[i].q_len > cls_max_q[cls]) cls_max_q[cls] = its[i].q_len;
+            units += (int64_t)its[i].n_tiles * (family == 2 ? c.n_kv_heads : c.n_q_heads * its[i].q_len);
+        }
+        if (family == 2 && cls == 0) {
+            // stream-K: equal contiguous tile ranges over a grid of n_SM x 3 CTAs
+            gplan.n_kv_heads = c.n_kv_heads;
+            gplan.total_tiles = cls_tiles[0] * c.n_kv_heads;
+            int64_t ctas = (int64_t)pool->n_sm * 3;
+            const int64_t min_tiles = pool->tune_split_tokens > 0 ? (pool->tune_split_tokens + 15) / 16 : 8;
+            if (ctas > (gplan.total_tiles + min_tiles - 1) / min_tiles) ctas = (gplan.total_tiles + min_tiles - 1) / min_tiles;
+            if (pool->tune_split_tokens > 0) ctas = (gplan.total_tiles + min_tiles - 1) / min_tiles;
+            if (ctas < 1) ctas = 1;
+            gplan.tiles_per_cta = (gplan.total_tiles + ctas - 1) / ctas;
+            gqa_ctas = (int32_t)((gplan.total_tiles + gplan.tiles_per_cta - 1) / gplan.tiles_per_cta);
+            for (int i = 0; i < n; ++i) {
+                const int32_t pieces = (int32_t)((its[i].n_tiles + gplan.tiles_per_cta - 1) / gplan.tiles_per_cta) + 1;
+                its[i].n_splits = pieces;      // upper bound on the pieces of one (item, head) pair
+                if (pieces > max_splits) max_splits = pieces;
+            }
+            continue;
+        }
+        // segments sized for >= 2 waves of CTAs, each with a useful run of tiles
+        const int64_t target_ctas = (int64_t)pool->n_sm * (family == 2 ? 4 : 16);
+        int32_t tps = pool->tune_split_tokens > 0 ? (pool->tune_split_tokens + kBlockTokens - 1) / kBlockTokens
+                                                  : (int32_t)((units + target_ctas - 1) / target_ctas);
+        if (pool->tune_split_tokens <= 0 && tps < 8) tps = 8;
+        if (tps < 1) tps = 1;
+        for (int i = 0; i < n; ++i) {
+            AttendItem& it = its[i];
+            int32_t ns = (it.n_tiles + tps - 1) / tps;
+            if (ns > kMaxSplits) ns = kMaxSplits;
+            if (ns < 1) ns = 1;
+            it.tiles_per_split = (it.n_tiles + ns - 1) / ns;
+            it.n_splits = (it.n_tiles + it.tiles_per_split - 1) / it.tiles_per_split;
+            it.split_off = total_splits[cls];
+            total_splits[cls] += it.n_splits;
+            if (it.n_splits > max_splits) max_splits = it.n_splits;
+        }
     }
     if (max_splits > 1) {
         rc = ensure_workspace(pool, (size_t)total_rows * c.n_q_heads * max_splits);
@@ -551,8 +596,6 @@ int metronome_attend_frame(metronome_pool_t* pool, int32_t layer, int32_t n_batc
     if (rc) return rc;
 
     AttendParams p{};
-    p.items = reinterpret_cast<const AttendItem*>(d);
-    p.n_items = n_items;
     p.table = pool->d_table;
     p.tbl_width = pool->tbl_width; p.n_sink = pool->n_sink; p.ring = pool->ring;
     p.q = (const __nv_bfloat16*)q;
@@ -575,22 +618,49 @@ int metronome_attend_frame(metronome_pool_t* pool, int32_t layer, int32_t n_batc
         }
         CU(cudaEventRecord(pool->prof_ev[pool->prof_used], st));
     }
+    const AttendItem* d_items = reinterpret_cast<const AttendItem*>(d);
+    bool merge_cls[2] = {false, false};
     if (family == 2) {
-        rc = launch_attend_mma(p, c.head_dim, c.n_kv_heads, total_splits, max_q, st);
-        if (rc) return cuda_fail(pool, cudaGetLastError(), "attend_mma launch");
+        if (n_cls[0] > 0) {
+            p.items = d_items; p.n_items = n_cls[0];
+            launch_attend_gqa(p, gplan, c.head_dim, gqa_ctas, st);
+            ++pool->n_launch;
+            CU(cudaGetLastError());
+            merge_cls[0] = gqa_ctas > 1;
+        }
+        if (n_cls[1] > 0) {
+            p.items = d_items + n_cls[0]; p.n_items = n_cls[1];
+            launch_attend_mma(p, c.head_dim, c.n_kv_heads, total_splits[1], pool->G * cls_max_q[1], st);
+            ++pool->n_launch;
+            CU(cudaGetLastError());
+            for (int i = 0; i < n_cls[1]; ++i)
+                if (items[n_cls[0] + i].n_splits > 1) merge_cls[1] = true;
+        }
     } else {
-        dim3 grid(total_splits, c.n_q_heads, max_q);
+        p.items = d_items; p.n_items = n_items;
+        dim3 grid(total_splits[0], c.n_q_heads, cls_max_q[0]);
         if (c.head_dim == 128) attend_rows_kernel<128><<<grid, 128, 0, st>>>(p);
         else attend_rows_kernel<64><<<grid, 128, 0, st>>>(p);
+        ++pool->n_launch;
+        CU(cudaGetLastError());
+        for (int i = 0; i < n_items; ++i)
+            if (items[i].n_splits > 1) merge_cls[0] = true;
     }
-    ++pool->n_launch;
-    CU(cudaGetLastError());
     if (pool->profiling) {
         CU(cudaEventRecord(pool->prof_ev[pool->prof_used + 1], st));
         pool->prof_used += 2;
     }
-    if (max_splits > 1) {
-        dim3 grid((unsigned)total_rows, c.n_q_heads);
+    // ---- row a6: combine the split-KV partials ----
+    if (family == 2 && merge_cls[0]) {
+        p.items = d_items; p.n_items = n_cls[0];
+        launch_merge_gqa(p, gplan, c.head_dim, cls_rows[0], st);
+        ++pool->n_launch;
+        CU(cudaGetLastError());
+    }
+    for (int cls = (family == 2 ? 1 : 0); cls < 2; ++cls) {
+        if (!merge_cls[cls] || (family != 2 && cls == 1)) continue;
+        p.items = d_items + (cls == 0 ? 0 : n_cls[0]); p.n_items = n_cls[cls];
+        dim3 grid((unsigned)cls_rows[cls], c.n_q_heads);
         if (c.head_dim == 128) merge_kernel<128><<<grid, 32, 0, st>>>(p);
         else merge_kernel<64><<<grid, 16, 0, st>>>(p);
         ++pool->n_launch;
