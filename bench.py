@@ -227,7 +227,7 @@ def main():
     import torch.distributed as dist
     from paper_2607_02640_b200 import build as _build
     _build.build_library()
-    from paper_2607_02640_b200 import synth
+    from paper_2607_02640_b200 import replicas, synth
     from paper_2607_02640_b200 import workloads as wl
     from paper_2607_02640_b200.runner import Runner
 
@@ -242,7 +242,7 @@ def main():
     need = 2 * W + 3 * K
     w = wl.make_workload(args.config, n_sessions=args.sessions or None, n_timed_frames=need)
     events, info = wl.build_schedule(w, history_scale=args.history_scale)
-    r = Runner(w, n_layers=1)
+    r = Runner(w, n_layers=1, uid_base=replicas.uid_base(RANK))
     r.pool.set_tuning(args.split_tokens, args.family)
     t_hist = time.perf_counter()
     rest = r.run_history(events)
@@ -329,12 +329,8 @@ def main():
     ms = e0.elapsed_time(e1)
     clocks = sampler.stop() if sampler else None
     launches = r.pool.stats()["kernel_launches"] - launches0
-    if WORLD > 1:
-        t = torch.tensor([ms], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
     finish_closes(timed)
-    value = WORLD * session_frames(timed_f) / (ms * 1e-3)
+    value, ms = replicas.aggregate(ms, session_frames(timed_f), device="cuda")   # max over ranks, sum of frames
 
     # ---- roofline of the dominant kernel: same steps again with the library's event brackets ----
     prof = prepare(take(K))
@@ -389,14 +385,12 @@ def main():
         t0 = time.perf_counter()
         run_host(ht)
         el = time.perf_counter() - t0
-        if WORLD > 1:
-            t = torch.tensor([el], device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            el = float(t.item())
+        e2e_value, el_ms = replicas.aggregate(el * 1e3, session_frames(ht_f), device="cuda")
+        el = el_ms * 1e-3
         hsteps = [it for it in ht if it[0] != "close"]
         h2d = sum(k.numel() * 2 + v.numel() * 2 + q.numel() * 2 for _, k, v, q, _ in hsteps) / K
         d2h = sum(o.numel() * 2 for *_, o in hsteps) / K
-        e2e = {"value": WORLD * session_frames(ht_f) / el, "unit": UNIT, "h2d_bytes_per_step": h2d,
+        e2e = {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d,
                "d2h_bytes_per_step": d2h, "ms_per_step": 1e3 * el / K,
                "api": "metronome_step_host (pinned host buffers)"}
 

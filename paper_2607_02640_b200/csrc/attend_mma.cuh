@@ -24,8 +24,9 @@
 //   * the softmax denominator is accumulated from the SAME rounded P that multiplies V (an extra n8
 //     tile against a ones matrix), so numerator and denominator see identical weights;
 //   * P is split into bf16 hi + lo parts, and the lo MMA is issued only for tiles that hold a key
-//     whose weight exceeds 1/64 of the running sum (warp-uniform vote): peaky softmax rows (config
-//     4's x20 outlier channels) get ~2^-17 weights, flat rows pay nothing.
+//     whose weight exceeds 1/32 (chunk) or 1/256 (decode, where the MMA is free) of the running sum
+//     (warp-uniform vote): peaky softmax rows (config 4's x20 outlier channels) get ~2^-17 weights,
+//     flat rows pay almost nothing.
 //
 // Why mma.sync and not tcgen05 (round 1): decode is one m16 tile at G flop/byte; the chunk tiles are
 // the candidate for a tcgen05/TMEM path.  The HBM layout is already UMMA's
@@ -127,6 +128,8 @@ struct WarpTile {
     }
 
     // one 16-key tile: kt / vt are shared-memory addresses of the swizzled K and V tiles
+    // kLoInv: the lo part of P is issued when some key's weight exceeds 1/kLoInv of the running sum
+    template <int kLoInv>
     __device__ __forceinline__ void step(const AttendParams& p, int32_t len, uint32_t kt, uint32_t vt, int32_t p0,
                                          int32_t lane) {
         const int32_t mat = lane >> 3, r8 = lane & 7;
@@ -184,10 +187,10 @@ struct WarpTile {
             hi[k] = pack_bf16(pr[2 * k], pr[2 * k + 1]);     // [0] row a keys col0.., [1] row b, [2] row a keys 8+col0.., [3] row b
             lo[k] = pack_bf16(pr[2 * k] - bf16lo(hi[k]), pr[2 * k + 1] - bf16hi(hi[k]));
         }
-        // lo part only where a key carries more than 1/64 of the running sum (warp-uniform)
+        // lo part only where a key carries more than 1/kLoInv of the running sum (warp-uniform)
         const float pm_a = fmaxf(fmaxf(pr[0], pr[1]), fmaxf(pr[4], pr[5]));
         const float pm_b = fmaxf(fmaxf(pr[2], pr[3]), fmaxf(pr[6], pr[7]));
-        const bool need_lo = __any_sync(0xffffffffu, (pm_a * 64.f > lsum[0]) || (pm_b * 64.f > lsum[2]));
+        const bool need_lo = __any_sync(0xffffffffu, (pm_a * (float)kLoInv > lsum[0]) || (pm_b * (float)kLoInv > lsum[2]));
         constexpr uint32_t kOnes = 0x3F803F80u;              // bf16 (1, 1)
         mma_bf16(lsum, hi, kOnes, kOnes);
         if (need_lo) mma_bf16(lsum, lo, kOnes, kOnes);
@@ -319,7 +322,7 @@ attend_mma_kernel(AttendParams p) {
             const int32_t p0 = tile_block(it, tbase + j) * kBlockTokens;
             if (wt.skips(p, p0)) continue;
             const uint32_t kt = smem_base + slot * C::kStageBytes + j * C::kHeadBytes;
-            wt.step(p, it.len, kt, kt + kBlockTokens * D * 2, p0, lane);
+            wt.template step<32>(p, it.len, kt, kt + kBlockTokens * D * 2, p0, lane);
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(bar_empty + 8 * slot);
@@ -416,7 +419,7 @@ attend_gqa_kernel(AttendParams p, GqaPlan plan) {
             phase_bits ^= 1u << st;
             const int32_t p0 = tile_block(it, a + warp + k * C::NWARP) * kBlockTokens;
             const uint32_t kt = ring + st * C::kHeadBytes;
-            if (!wt.skips(p, p0)) wt.step(p, it.len, kt, kt + kBlockTokens * D * 2, p0, lane);
+            if (!wt.skips(p, p0)) wt.template step<256>(p, it.len, kt, kt + kBlockTokens * D * 2, p0, lane);
             __syncwarp();                                  // every lane is done reading the stage
             if (k + C::NS < n_mine) issue(k + C::NS);
         }

@@ -30,7 +30,7 @@ class Step:
 
 class Runner:
     def __init__(self, w: Workload, n_layers: int = 1, flags: int = 0, device: str = "cuda",
-                 softmax_scale: float = 0.0):
+                 softmax_scale: float = 0.0, uid_base: int = 0):
         self.w = w
         self.n_layers = n_layers
         self.device = torch.device(device)
@@ -41,7 +41,7 @@ class Runner:
         self.sid = {}            # local index -> library sid
         self.uid = {}            # local index -> unique session uid (fresh on every open)
         self.length = {}         # local index -> tokens so far
-        self._next_uid = 0
+        self._next_uid = uid_base    # replicas draw different inputs (replicas.uid_base)
         oc = w.outlier_channels()
         self.outliers = torch.from_numpy(oc).to(self.device) if oc.size else None
 
