@@ -1,0 +1,554 @@
+// attend_umma.cuh -- row a7 (chunk prefill) on the 5th-generation tensor cores: tcgen05.mma with
+// TMEM accumulators (SASS UTCHMMA / LDTM / STTM), operands staged by bulk async copies (UBLKCP).
+//
+// The R = G x q_len query rows that share one KV head ("grouped-query attention",
+// "mixed prefill/decode"; L46 "prefill the new chunk") are a real dense contraction against the
+// session's sink + window keys: S = Q K^T and O = P V with M = 128-row tiles.  One CTA owns one
+// (item, KV head, split-KV segment) and streams its KV ONCE from HBM in stages of 8 blocks
+// (128 keys):
+//
+//   warp 0      producer: per stage, bulk copies of the K tiles (one 2 KB copy per 64-dim half, so
+//               the halves of 8 blocks form one UMMA K-major operand) and of the V tiles (4 KB each;
+//               a V tile as laid out in HBM already IS a SWIZZLE_128B MN-major operand of one
+//               K=16 MMA), into a 5-deep ring of 32 KB buffers, mbarrier complete_tx
+//   warp 1      MMA issuer (one elected lane) + TMEM allocator:
+//                 S_s = Q_s K_j^T   (SS form, D/16 instructions 128x128x16)  -> TMEM, fp32
+//                 O_s += P_s V_j    (TS form: P is read from TMEM, V from shared memory)
+//               completion is signalled with tcgen05.commit on mbarriers
+//   warps 2-5   softmax warpgroup of slot 0, warps 6-9 of slot 1: ONE THREAD PER QUERY ROW
+//               (tcgen05.ld 32x32b): token-exact union mask on boundary stages, row max and row sum
+//               without any shuffle, exp2 in the log2 domain, P rounded to bf16 and written back to
+//               TMEM over S (tcgen05.st), lazy rescale of O (only when the max moved by > 2^8)
+//
+// Two slots (S, P and O regions in TMEM: 2 x (128 + D) columns of the 512) ping-pong so the tensor
+// pipe, the MUFU pipe and the copy engine overlap:
+//   R > 128  : slot s = rows [128 s, 128 s + 128), both slots see every key stage
+//   R <= 128 : both slots hold the same rows; slot s takes key stages j = s (mod 2); the two
+//              partial (O, m, l) are merged through shared memory at the end
+// Sinks go first, in segment 0 only; a single segment writes the final bf16 output,
+// several write unnormalised partials for merge_kernel (row a6).
+//
+// Roofline: at R = 200 (config 3) the step is ~200 flop/byte against a ridge of ~250: HBM-bound
+// with the tensor pipe ~70 % busy; the mma.sync predecessor (attend_mma_kernel) was 7x off.
+#pragma once
+#include "attend_mma.cuh"
+
+namespace metronome {
+
+template <int D>
+struct UmmaCfg {
+    static constexpr int KS = 8;                          // KV blocks per stage (128 keys)
+    static constexpr int NBUF = 5;                        // ring buffers (each one K or one V stage)
+    static constexpr int NH = D / 64;                     // 64-dim halves (128-byte swizzle span)
+    static constexpr int kTileBytes = kBlockTokens * D * 2;   // K or V of one (block, head)
+    static constexpr int kBufBytes = KS * kTileBytes;     // 32 KB at D = 128
+    static constexpr int kHalfBytes = 128 * 128;          // [128 rows or keys][64 dims]
+    static constexpr int kQBytes = 128 * D * 2;           // Q rows of one slot
+    static constexpr int kBarOff = 2 * kQBytes + NBUF * kBufBytes;
+    static constexpr int kMlOff = kBarOff + 256;          // (m, l) of slot 1 for the in-CTA merge
+    static constexpr int kSmemBytes = kMlOff + 1024 + 1024;   // + alignment slack
+    static constexpr int kThreads = 320;
+    static constexpr int kTmemCols = 512;
+    static constexpr int kColS = 0, kColO = 256;          // S_s at 128 s; O_s at 256 + D s
+    static_assert(kSmemBytes <= 232448, "shared memory budget");
+};
+
+// ---- tcgen05 / UMMA primitives --------------------------------------------------------------
+// shared-memory matrix descriptor, SWIZZLE_128B (cute::UMMA::SmemDescriptor bit layout)
+__device__ __forceinline__ uint64_t umma_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
+    return (uint64_t)((saddr >> 4) & 0x3FFFu) | ((uint64_t)((lbo_bytes >> 4) & 0x3FFFu) << 16) |
+           ((uint64_t)((sbo_bytes >> 4) & 0x3FFFu) << 32) | ((uint64_t)1 << 46) | ((uint64_t)2 << 61);
+}
+// instruction descriptor, kind::f16: bf16 x bf16 -> f32, M = 128
+__host__ __device__ constexpr uint32_t umma_idesc(int n, bool b_mn_major) {
+    return (1u << 4) | (1u << 7) | (1u << 10) | ((b_mn_major ? 1u : 0u) << 16) | ((uint32_t)(n >> 3) << 17) |
+           ((uint32_t)(128 >> 4) << 24);
+}
+__device__ __forceinline__ void umma_ss(uint32_t d_tmem, uint64_t a, uint64_t b, uint32_t idesc, uint32_t accum) {
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                 "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+                 ::"r"(d_tmem), "l"(a), "l"(b), "r"(idesc), "r"(accum) : "memory");
+}
+__device__ __forceinline__ void umma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b, uint32_t idesc, uint32_t accum) {
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                 "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
+                 ::"r"(d_tmem), "r"(a_tmem), "l"(b), "r"(idesc), "r"(accum) : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint32_t bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void named_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+__device__ __forceinline__ void named_arrive(int id, int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+
+// barrier with an OR-reduction of a predicate over its `n` participating threads
+__device__ __forceinline__ bool named_sync_or(int id, int n, bool pred) {
+    uint32_t out;
+    asm volatile("{\n\t.reg .pred p, q;\n\tsetp.ne.u32 q, %1, 0;\n\tbar.red.or.pred p, %2, %3, q;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                 : "=r"(out) : "r"((uint32_t)pred), "r"(id), "r"(n) : "memory");
+    return out != 0;
+}
+
+// 32 lanes x 32 consecutive 32-bit columns: thread i of the warp gets lane (quarter base + i)
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t* r) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+                 "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+                   "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]),
+                   "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]),
+                   "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+                 : "r"(taddr));
+}
+__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t* r) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
+                 "{%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31,%32};"
+                 ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]),
+                   "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]),
+                   "r"(r[16]), "r"(r[17]), "r"(r[18]), "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]),
+                   "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]), "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31])
+                 : "memory");
+}
+__device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+
+// Order in which the ring is filled and drained (producer and MMA warp agree on it):
+//   two row tiles : K0 V0 K1 V1 ...            (S_0, S_1 of stage j+1 are issued around P V of stage j)
+//   one row tile  : K0 K1 V0 K2 V1 ... V(n-1)  (slots alternate stages, so K is needed one stage ahead)
+__device__ __forceinline__ int32_t umma_entry_k(bool two, int32_t j) { return two ? 2 * j : (j == 0 ? 0 : 2 * j - 1); }
+__device__ __forceinline__ int32_t umma_entry_v(bool two, int32_t j, int32_t n) {
+    return two ? 2 * j + 1 : (j == n - 1 ? 2 * n - 1 : 2 * j + 2);
+}
+
+// grid = (Hkv, total segments of the chunk-class items), block = 320, one CTA per SM
+template <int D>
+__global__ void __launch_bounds__(UmmaCfg<D>::kThreads, 1)
+attend_umma_kernel(AttendParams p) {
+    using C = UmmaCfg<D>;
+    extern __shared__ __align__(1024) uint8_t smem_umma[];
+    const uint32_t base = (smem_u32(smem_umma) + 1023u) & ~1023u;       // swizzle atoms are 1024-byte aligned
+    uint8_t* gen = smem_umma + (base - smem_u32(smem_umma));
+    const uint32_t sQ = base, sRing = base + 2 * C::kQBytes, sBar = base + C::kBarOff;
+    auto bar_full = [&](int b) { return sBar + 8u * b; };
+    auto bar_empty = [&](int b) { return sBar + 8u * (C::NBUF + b); };
+    auto bar_s = [&](int s) { return sBar + 8u * (2 * C::NBUF + s); };          // S_s ready   (MMA -> softmax)
+    auto bar_p = [&](int s) { return sBar + 8u * (2 * C::NBUF + 2 + s); };      // P_s written (softmax -> MMA)
+    auto bar_o = [&](int s) { return sBar + 8u * (2 * C::NBUF + 4 + s); };      // last P V of slot s done
+    volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(gen + C::kBarOff + 2 * 8 * C::NBUF + 6 * 8);
+    volatile uint32_t* lo_flag = tmem_slot + 2;                                 // [slot]: P_lo of this stage is valid
+
+    const int32_t kvh = blockIdx.x;
+    const int32_t i = find_item(p.n_items, (int32_t)blockIdx.y, [&](int32_t k) { return p.items[k].split_off; });
+    const AttendItem it = p.items[i];
+    const int32_t split = (int32_t)blockIdx.y - it.split_off;
+    const int32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int32_t R = it.q_len * p.G;
+    const bool two = R > 128;
+    const int32_t tl0 = split * it.tiles_per_split;
+    const int32_t tl1 = min(it.n_tiles, tl0 + it.tiles_per_split);
+    const int32_t n_stage = (tl1 - tl0 + C::KS - 1) / C::KS;
+    const int32_t t_first = it.len - it.q_len;                          // reading R15: the last q_len positions
+
+    if (warp == 0) {
+        // ================================ producer ================================
+        if (lane == 0) {
+            for (int b = 0; b < C::NBUF; ++b) { mbar_init(bar_full(b), 1); mbar_init(bar_empty(b), 1); }
+            for (int s = 0; s < 2; ++s) { mbar_init(bar_s(s), 1); mbar_init(bar_p(s), 4); mbar_init(bar_o(s), 1); }
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        }
+        __syncwarp();
+        named_arrive(1, C::kThreads);
+        const int32_t* trow = p.table + (int64_t)it.sid * p.tbl_width;
+        const uint8_t* head_base = p.kv_layer + (int64_t)kvh * p.L.head_bytes;
+        for (int32_t e = 0; e < 2 * n_stage; ++e) {
+            bool is_v;
+            int32_t j;
+            if (two) { is_v = e & 1; j = e >> 1; }
+            else if (e == 0) { is_v = false; j = 0; }
+            else if (e == 2 * n_stage - 1) { is_v = true; j = n_stage - 1; }
+            else if (e & 1) { is_v = false; j = (e + 1) >> 1; }
+            else { is_v = true; j = (e >> 1) - 1; }
+            const int32_t b = e % C::NBUF, k = e / C::NBUF;
+            if (k >= 1) mbar_wait(bar_empty(b), (k - 1) & 1);
+            const int32_t t0 = tl0 + j * C::KS;
+            const int32_t nt = min(C::KS, tl1 - t0);
+            if (lane == 0) mbar_expect_tx(bar_full(b), (uint32_t)nt * C::kTileBytes);
+            __syncwarp();
+            const uint32_t dst = sRing + b * C::kBufBytes;
+            if (is_v) {
+                if (lane < nt) {
+                    const int32_t phys = __ldg(trow + table_slot(tile_block(it, t0 + lane), p.n_sink, p.ring));
+                    bulk_g2s(dst + lane * C::kTileBytes, head_base + (int64_t)phys * p.L.block_bytes + p.L.tile_bytes,
+                             C::kTileBytes, bar_full(b));
+                }
+            } else if (lane < nt * C::NH) {
+                const int32_t blk = lane / C::NH, h = lane % C::NH;
+                const int32_t phys = __ldg(trow + table_slot(tile_block(it, t0 + blk), p.n_sink, p.ring));
+                bulk_g2s(dst + h * C::kHalfBytes + blk * 2048, head_base + (int64_t)phys * p.L.block_bytes + h * 2048, 2048,
+                         bar_full(b));
+            }
+        }
+        return;
+    }
+
+    if (warp == 1) {
+        // ================================ MMA issuer ================================
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;"
+                     ::"r"(smem_u32(const_cast<uint32_t*>(tmem_slot))), "r"(C::kTmemCols));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+        tc_fence_before();
+        named_sync(1, C::kThreads);
+        tc_fence_after();
+        const uint32_t tmem = *tmem_slot;
+        constexpr uint32_t idesc_qk = umma_idesc(128, false);
+        constexpr uint32_t idesc_pv = umma_idesc(D, true);
+
+        auto wait_full = [&](int32_t e) {
+            mbar_wait(bar_full(e % C::NBUF), (e / C::NBUF) & 1);
+            tc_fence_after();
+        };
+        auto release = [&](int32_t e) { if (lane == 0) umma_commit(bar_empty(e % C::NBUF)); };
+        // S_slot = Q_qslot K^T over the K stage in ring entry e
+        auto issue_qk = [&](int32_t slot, int32_t qslot, int32_t e) {
+            if (lane == 0) {
+                const uint32_t kb = sRing + (e % C::NBUF) * C::kBufBytes, qb = sQ + qslot * C::kQBytes;
+#pragma unroll
+                for (int kk = 0; kk < D / 16; ++kk) {
+                    const uint32_t off = (kk >> 2) * C::kHalfBytes + (kk & 3) * 32;
+                    umma_ss(tmem + C::kColS + 128 * slot, umma_desc(qb + off, 16, 1024), umma_desc(kb + off, 16, 1024),
+                            idesc_qk, kk > 0);
+                }
+                umma_commit(bar_s(slot));
+            }
+            __syncwarp();
+        };
+        // O_slot (+)= P_slot V over the V stage in ring entry e: one K=16 MMA per valid block
+        // (P = bf16 hi [+ bf16 lo when the softmax warps flagged a peaky stage]: columns 0-63 / 64-127 of S_slot)
+        auto issue_pv = [&](int32_t slot, int32_t e, int32_t nt, bool accumulate) {
+            if (lane == 0) {
+                const uint32_t vb = sRing + (e % C::NBUF) * C::kBufBytes;
+                const bool lo = lo_flag[slot] != 0;
+                for (int32_t b = 0; b < nt; ++b)
+                    umma_ts(tmem + C::kColO + D * slot, tmem + C::kColS + 128 * slot + 8 * b,
+                            umma_desc(vb + b * C::kTileBytes, 2048, 1024), idesc_pv, (accumulate || b > 0) ? 1u : 0u);
+                if (lo)
+                    for (int32_t b = 0; b < nt; ++b)
+                        umma_ts(tmem + C::kColO + D * slot, tmem + C::kColS + 128 * slot + 64 + 8 * b,
+                                umma_desc(vb + b * C::kTileBytes, 2048, 1024), idesc_pv, 1u);
+            }
+            __syncwarp();
+        };
+        // V rows past the session's length hold stale or poisoned bytes (0 * NaN = NaN): zero them
+        auto fix_ragged_v = [&](int32_t e, int32_t t0, int32_t nt) {
+            const int32_t last = it.n_tiles - 1, nvalid = it.len & (kBlockTokens - 1);
+            if (nvalid == 0 || last < t0 || last >= t0 + nt) return;
+            uint8_t* vt = gen + 2 * C::kQBytes + (e % C::NBUF) * C::kBufBytes + (last - t0) * C::kTileBytes;
+            const int32_t per_row = C::NH * 8;
+            for (int32_t idx = lane; idx < (kBlockTokens - nvalid) * per_row; idx += 32) {
+                const int32_t row = nvalid + idx / per_row, rem = idx % per_row;
+                *reinterpret_cast<uint4*>(vt + (rem >> 3) * 2048 + row * 128 + (rem & 7) * 16) = make_uint4(0u, 0u, 0u, 0u);
+            }
+            fence_async_smem();
+            __syncwarp();
+        };
+        auto stage_nt = [&](int32_t j) { return min(C::KS, tl1 - (tl0 + j * C::KS)); };
+
+        if (two) {
+            int32_t ek = umma_entry_k(true, 0);
+            wait_full(ek);
+            issue_qk(0, 0, ek);
+            issue_qk(1, 1, ek);
+            release(ek);
+            for (int32_t j = 0; j < n_stage; ++j) {
+                const int32_t ev = umma_entry_v(true, j, n_stage), nt = stage_nt(j);
+                const bool more = j + 1 < n_stage;
+                wait_full(ev);
+                fix_ragged_v(ev, tl0 + j * C::KS, nt);
+                mbar_wait(bar_p(0), j & 1);
+                tc_fence_after();
+                issue_pv(0, ev, nt, j > 0);
+                if (!more && lane == 0) umma_commit(bar_o(0));
+                if (more) {
+                    ek = umma_entry_k(true, j + 1);
+                    wait_full(ek);
+                    issue_qk(0, 0, ek);
+                }
+                mbar_wait(bar_p(1), j & 1);
+                tc_fence_after();
+                issue_pv(1, ev, nt, j > 0);
+                release(ev);
+                if (!more && lane == 0) umma_commit(bar_o(1));
+                if (more) {
+                    issue_qk(1, 1, ek);
+                    release(ek);
+                }
+            }
+        } else {
+            for (int32_t j = 0; j < min(2, n_stage); ++j) {
+                const int32_t ek = umma_entry_k(false, j);
+                wait_full(ek);
+                issue_qk(j, 0, ek);
+                release(ek);
+            }
+            for (int32_t j = 0; j < n_stage; ++j) {
+                const int32_t s = j & 1, ev = umma_entry_v(false, j, n_stage), nt = stage_nt(j);
+                wait_full(ev);
+                fix_ragged_v(ev, tl0 + j * C::KS, nt);
+                mbar_wait(bar_p(s), (j >> 1) & 1);
+                tc_fence_after();
+                issue_pv(s, ev, nt, j >= 2);
+                release(ev);
+                if (j + 2 >= n_stage && lane == 0) umma_commit(bar_o(s));
+                if (j + 2 < n_stage) {
+                    const int32_t ek = umma_entry_k(false, j + 2);
+                    wait_full(ek);
+                    issue_qk(s, 0, ek);
+                    release(ek);
+                }
+            }
+        }
+        // every softmax warp has finished reading TMEM
+        named_sync(2, C::kThreads - 32);
+        tc_fence_after();
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(C::kTmemCols));
+        return;
+    }
+
+    // ================================ softmax warps ================================
+    const int32_t slot = (warp - 2) >> 2, quarter = warp & 3;       // TMEM lanes 32 (warp % 4) .. + 31
+    const int32_t row = quarter * 32 + lane;
+    const int32_t tile_row0 = two ? 128 * slot : 0;
+    const int32_t rho = tile_row0 + row;                              // rho = r * G + g
+    const bool valid = rho < R;
+    const int32_t rq = rho / p.G, gq = rho - rq * p.G;
+    const int32_t t = valid ? t_first + rq : -1;                      // -1: padding row, admits nothing
+    const bool warp_active = tile_row0 + quarter * 32 < R;
+    const int32_t t_wmin = t_first + (tile_row0 + quarter * 32) / p.G;
+    const int32_t t_wmax = t_first + (min(R, tile_row0 + quarter * 32 + 32) - 1) / p.G;
+
+    // ---- Q rows -> shared memory, K-major SWIZZLE_128B, one [128][64] region per 64-dim half ----
+    {
+        const int32_t tid2 = threadIdx.x - 64;
+        const int32_t n_rows = two ? 256 : 128;
+        constexpr int CPR = D / 8;                                    // 16-byte chunks per row
+        for (int32_t idx = tid2; idx < n_rows * CPR; idx += 256) {
+            const int32_t rr = idx / CPR, c = idx % CPR;
+            uint4 v = make_uint4(0u, 0u, 0u, 0u);
+            if (rr < R) {
+                const int32_t r2 = rr / p.G, g2 = rr - r2 * p.G;
+                v = __ldg(reinterpret_cast<const uint4*>(p.q + ((int64_t)(it.q_row_off + r2) * p.Hq + kvh * p.G + g2) * D) + c);
+            }
+            *reinterpret_cast<uint4*>(gen + (rr >> 7) * C::kQBytes + (c >> 3) * C::kHalfBytes + (rr & 127) * 128 +
+                                      (((c & 7) ^ (rr & 7)) << 4)) = v;
+        }
+        fence_async_smem();
+    }
+    named_sync(1, C::kThreads);
+    tc_fence_after();
+    const uint32_t tmem = *tmem_slot;
+    const uint32_t lane_base = (uint32_t)(quarter * 32) << 16;
+    const uint32_t tS = tmem + lane_base + C::kColS + 128 * slot;     // S (fp32) and, over it, P (bf16 x 2 per column)
+    const uint32_t tO = tmem + lane_base + C::kColO + D * slot;
+
+    float m_run = -INFINITY, m_used = -INFINITY, l = 0.f;
+    int32_t n_it = 0;
+    for (int32_t j = two ? 0 : slot; j < n_stage; j += two ? 1 : 2, ++n_it) {
+        mbar_wait(bar_s(slot), n_it & 1);
+        tc_fence_after();
+        uint32_t s[128];
+        float sub = 0.f;
+        bool need_lo = false;
+        if (warp_active) {
+#pragma unroll
+            for (int c = 0; c < 4; ++c) tmem_ld32(tS + 32 * c, s + 32 * c);
+            tmem_wait_ld();
+            const int32_t t0 = tl0 + j * C::KS;
+            const int32_t nt = min(C::KS, tl1 - t0);
+            // a stage needs no mask when every key of it is admitted for every row of this warp
+            bool full = nt == C::KS;
+            for (int32_t b = 0; b < nt && full; ++b) {
+                const int32_t pe = tile_block(it, t0 + b) * kBlockTokens + kBlockTokens - 1;
+                full = pe <= t_wmin && (pe < p.S || t_wmax - (pe - (kBlockTokens - 1)) < p.W);
+            }
+            if (!full) {
+#pragma unroll
+                for (int b = 0; b < C::KS; ++b) {
+                    const int32_t p0 = b < nt ? tile_block(it, t0 + b) * kBlockTokens : INT32_MAX / 2;
+#pragma unroll
+                    for (int c = 0; c < kBlockTokens; ++c)
+                        if (!admit(p0 + c, t, p.S, p.W)) s[b * kBlockTokens + c] = 0xFF800000u;   // -inf
+                }
+            }
+            float mx0 = -INFINITY, mx1 = -INFINITY, mx2 = -INFINITY, mx3 = -INFINITY;
+#pragma unroll
+            for (int c = 0; c < 128; c += 4) {
+                mx0 = fmaxf(mx0, __uint_as_float(s[c]));
+                mx1 = fmaxf(mx1, __uint_as_float(s[c + 1]));
+                mx2 = fmaxf(mx2, __uint_as_float(s[c + 2]));
+                mx3 = fmaxf(mx3, __uint_as_float(s[c + 3]));
+            }
+            const float mx = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * p.scale_log2;
+            m_run = fmaxf(m_run, mx);
+            if (n_it == 0) {
+                m_used = m_run;                                       // O_s is still empty
+            } else {
+                // lazy rescale: keep the stale reference max while it is within 2^8 of the true one
+                const bool need = (m_run - m_used) > 8.f;             // (-inf) - (-inf) = NaN -> false
+                if (__any_sync(0xffffffffu, need)) {
+                    const float f = (need && m_used != -INFINITY) ? ex2(m_used - m_run) : 1.f;
+                    l *= f;
+#pragma unroll
+                    for (int c = 0; c < D / 32; ++c) {
+                        uint32_t o[32];
+                        tmem_ld32(tO + 32 * c, o);
+                        tmem_wait_ld();
+#pragma unroll
+                        for (int k = 0; k < 32; ++k) o[k] = __float_as_uint(__uint_as_float(o[k]) * f);
+                        tmem_st32(tO + 32 * c, o);
+                    }
+                    if (need) m_used = m_run;
+                }
+            }
+            sub = m_used == -INFINITY ? 0.f : m_used;                 // nothing admitted yet: every p is 0
+            // a key that carries more than 1/32 of the running sum: P needs its bf16 lo part too
+            need_lo = valid && ex2(mx - sub) * 32.f > l;
+        }
+        const bool lo = named_sync_or(4 + slot, 128, need_lo);        // one decision for the slot's 128 rows
+        if (warp_active) {
+            uint32_t pk[64];
+            if (lo) {
+                uint32_t pl[64];
+#pragma unroll
+                for (int k = 0; k < 64; ++k) {
+                    const float p0 = ex2(fmaf(__uint_as_float(s[2 * k]), p.scale_log2, -sub));
+                    const float p1 = ex2(fmaf(__uint_as_float(s[2 * k + 1]), p.scale_log2, -sub));
+                    pk[k] = pack_bf16(p0, p1);
+                    pl[k] = pack_bf16(p0 - bf16lo(pk[k]), p1 - bf16hi(pk[k]));
+                    l += (bf16lo(pk[k]) + bf16lo(pl[k])) + (bf16hi(pk[k]) + bf16hi(pl[k]));
+                }
+                tmem_st32(tS + 64, pl);
+                tmem_st32(tS + 96, pl + 32);
+            } else {
+#pragma unroll
+                for (int k = 0; k < 64; ++k) {
+                    const float p0 = ex2(fmaf(__uint_as_float(s[2 * k]), p.scale_log2, -sub));
+                    const float p1 = ex2(fmaf(__uint_as_float(s[2 * k + 1]), p.scale_log2, -sub));
+                    pk[k] = pack_bf16(p0, p1);
+                    l += bf16lo(pk[k]) + bf16hi(pk[k]);               // the denominator sees the rounded weights
+                }
+            }
+            tmem_st32(tS, pk);
+            tmem_st32(tS + 32, pk + 32);
+            tmem_wait_st();
+        }
+        if (quarter == 0 && lane == 0) lo_flag[slot] = lo ? 1u : 0u;
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar_p(slot));
+    }
+
+    // ---- epilogue ----
+    const int64_t qrow = (int64_t)(it.q_row_off + rq) * p.Hq + kvh * p.G + gq;
+    float* ml1 = reinterpret_cast<float*>(gen + C::kMlOff);
+    auto store_row = [&](const float (&o)[D], float m, float lsum) {
+        if (!valid) return;
+        if (it.n_splits == 1) {
+            const float inv = lsum > 0.f ? 1.f / lsum : 0.f;
+            uint4* dst = reinterpret_cast<uint4*>(p.out + qrow * D);
+#pragma unroll
+            for (int c = 0; c < D / 8; ++c)
+                dst[c] = make_uint4(pack_bf16(o[8 * c] * inv, o[8 * c + 1] * inv), pack_bf16(o[8 * c + 2] * inv, o[8 * c + 3] * inv),
+                                    pack_bf16(o[8 * c + 4] * inv, o[8 * c + 5] * inv), pack_bf16(o[8 * c + 6] * inv, o[8 * c + 7] * inv));
+        } else {
+            const int64_t ws = qrow * p.max_splits + split;
+            float4* dst = reinterpret_cast<float4*>(p.ws_acc + ws * D);
+#pragma unroll
+            for (int c = 0; c < D / 4; ++c) dst[c] = make_float4(o[4 * c], o[4 * c + 1], o[4 * c + 2], o[4 * c + 3]);
+            p.ws_ml[ws * 2] = m;
+            p.ws_ml[ws * 2 + 1] = lsum;
+        }
+    };
+    auto load_o = [&](float (&o)[D]) {
+#pragma unroll
+        for (int c = 0; c < D / 32; ++c) tmem_ld32(tO + 32 * c, reinterpret_cast<uint32_t*>(o) + 32 * c);
+        tmem_wait_ld();
+    };
+    if (two) {
+        if (n_it > 0) {
+            mbar_wait(bar_o(slot), 0);
+            tc_fence_after();
+            if (warp_active) {
+                float o[D];
+                load_o(o);
+                store_row(o, m_used, l);
+            }
+        }
+    } else {
+        // both slots' MMAs are complete before the Q region is reused for the exchange
+        mbar_wait(bar_o(0), 0);
+        if (n_stage >= 2) mbar_wait(bar_o(1), 0);
+        tc_fence_after();
+        constexpr int NCH = D / 4;                                     // float4 chunks per row
+        float4* ex = reinterpret_cast<float4*>(gen) + row * NCH;
+        if (slot == 1) {
+            if (n_it > 0 && warp_active) {
+                float o[D];
+                load_o(o);
+#pragma unroll
+                for (int c = 0; c < NCH; ++c) ex[(c ^ row) & (NCH - 1)] = make_float4(o[4 * c], o[4 * c + 1], o[4 * c + 2], o[4 * c + 3]);
+                ml1[2 * row] = m_used;
+                ml1[2 * row + 1] = l;
+            }
+            __threadfence_block();
+            named_arrive(3, 256);
+        } else {
+            float o[D];
+            if (warp_active) load_o(o);
+            named_sync(3, 256);
+            if (warp_active) {
+                if (n_stage >= 2) {
+                    const float m1 = ml1[2 * row], l1 = ml1[2 * row + 1];
+                    const float M = fmaxf(m_used, m1);
+                    const float a0 = m_used == -INFINITY ? 0.f : ex2(m_used - M);
+                    const float a1 = m1 == -INFINITY ? 0.f : ex2(m1 - M);
+#pragma unroll
+                    for (int c = 0; c < NCH; ++c) {
+                        const float4 b = ex[(c ^ row) & (NCH - 1)];
+                        o[4 * c] = a0 * o[4 * c] + a1 * b.x;
+                        o[4 * c + 1] = a0 * o[4 * c + 1] + a1 * b.y;
+                        o[4 * c + 2] = a0 * o[4 * c + 2] + a1 * b.z;
+                        o[4 * c + 3] = a0 * o[4 * c + 3] + a1 * b.w;
+                    }
+                    l = a0 * l + a1 * l1;
+                    m_used = M;
+                }
+                store_row(o, m_used, l);
+            }
+        }
+    }
+    tc_fence_before();
+    named_arrive(2, C::kThreads - 32);
+}
+
+// ------------------------------------------------------------------------------------------------
+constexpr int kUmmaMaxRows = 256;
+
+inline bool attend_umma_supported(int32_t G, int32_t max_q) { return (int64_t)G * max_q <= kUmmaMaxRows; }
+
+inline cudaError_t configure_attend_umma_kernels() {
+    cudaError_t e;
+    if ((e = cudaFuncSetAttribute(attend_umma_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  UmmaCfg<128>::kSmemBytes)) != cudaSuccess) return e;
+    return cudaFuncSetAttribute(attend_umma_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                UmmaCfg<64>::kSmemBytes);
+}
+
+// chunk-class items (16 < R <= 256): p.items / p.n_items must point at them
+inline void launch_attend_umma(const AttendParams& p, int32_t D, int32_t Hkv, int32_t total_splits, cudaStream_t st) {
+    dim3 grid(Hkv, total_splits);
+    if (D == 128) attend_umma_kernel<128><<<grid, UmmaCfg<128>::kThreads, UmmaCfg<128>::kSmemBytes, st>>>(p);
+    else attend_umma_kernel<64><<<grid, UmmaCfg<64>::kThreads, UmmaCfg<64>::kSmemBytes, st>>>(p);
+}
+
+}  // namespace metronome

@@ -8,6 +8,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <algorithm>
 #include <cstring>
 #include <new>
 #include <string>
@@ -16,6 +17,7 @@
 #include "attend_common.cuh"
 #include "attend_mma.cuh"
 #include "attend_rows.cuh"
+#include "attend_umma.cuh"
 #include "bookkeeping.cuh"
 #include "kv_append.cuh"
 
@@ -286,6 +288,7 @@ int metronome_pool_create(const metronome_pool_config_t* cfg, metronome_pool_t**
     e = cudaDeviceSynchronize();
     if (e != cudaSuccess) return fail(METRONOME_ERR_CUDA, e, "pool init kernels");
     e = configure_attend_mma_kernels();
+    if (e == cudaSuccess) e = configure_attend_umma_kernels();
     if (e != cudaSuccess) return fail(METRONOME_ERR_CUDA, e, "cudaFuncSetAttribute");
     *out = pool;
     return METRONOME_OK;
@@ -490,13 +493,17 @@ int metronome_attend_frame(metronome_pool_t* pool, int32_t layer, int32_t n_batc
     //   rows   CUDA-core row kernel: pure multi-head decode (G x q_len < 4 for every item), and the
     //          general fallback
     //   gqa    tensor-core stream-K decode kernel: items with R = G x q_len <= 16
-    //   chunk  tensor-core chunk-prefill kernel:   items with 16 < R <= 208
+    //   chunk  tcgen05 / TMEM chunk-prefill kernel: items with 16 < R <= 256
+    //          (tuning family 3: its mma.sync predecessor, R <= 208, kept for A/B measurements)
     int32_t max_q = 0;
     for (int i = 0; i < n_batch; ++i)
         if (q_lens[i] > max_q) max_q = q_lens[i];
     int family = pool->tune_family;
+    const bool legacy_chunk = family == 3;
+    if (family == 3) family = 2;
     if (family == 0) family = (pool->G * max_q >= 4) ? 2 : 1;
-    if (family == 2 && !attend_mma_supported(pool->G, max_q)) family = 1;
+    if (family == 2 && !(legacy_chunk ? attend_mma_supported(pool->G, max_q) : attend_umma_supported(pool->G, max_q)))
+        family = 1;
 
     uint8_t *h = nullptr, *d = nullptr;
     int slot = 0;
@@ -533,6 +540,10 @@ int metronome_attend_frame(metronome_pool_t* pool, int32_t layer, int32_t n_batc
         it.n_tiles = it.n_sink_tiles + (n_blk > first_blk ? n_blk - first_blk : 0);
     }
     if (family != 2) { n_cls[0] = n_items; n_cls[1] = 0; }
+    // chunk class: longest first, so the hardware's in-order CTA dispatch packs the short ones last
+    if (family == 2 && !legacy_chunk && n_cls[1] > 1)
+        std::stable_sort(items + n_cls[0], items + n_cls[0] + n_cls[1],
+                         [](const AttendItem& a, const AttendItem& b) { return a.n_tiles > b.n_tiles; });
 
     // per-class prefix sums, split-KV plan
     int32_t total_splits[2] = {0, 0}, max_splits = 1, cls_rows[2] = {0, 0}, cls_max_q[2] = {0, 0};
@@ -575,6 +586,12 @@ int metronome_attend_frame(metronome_pool_t* pool, int32_t layer, int32_t n_batc
         int32_t tps = pool->tune_split_tokens > 0 ? (pool->tune_split_tokens + kBlockTokens - 1) / kBlockTokens
                                                   : (int32_t)((units + target_ctas - 1) / target_ctas);
         if (pool->tune_split_tokens <= 0 && tps < 8) tps = 8;
+        if (family == 2 && !legacy_chunk && pool->tune_split_tokens <= 0) {
+            // tcgen05 chunk kernel, one CTA per SM: whole (item, head) pairs when they alone give
+            // >= 3 CTAs per SM (no partials to merge), else whole 128-key stages, >= 4 per segment
+            if ((int64_t)n * c.n_kv_heads >= 3 * (int64_t)pool->n_sm) tps = INT32_MAX / 2;
+            else tps = std::max(32, (tps + 7) / 8 * 8);
+        }
         if (tps < 1) tps = 1;
         for (int i = 0; i < n; ++i) {
             AttendItem& it = its[i];
@@ -630,7 +647,8 @@ int metronome_attend_frame(metronome_pool_t* pool, int32_t layer, int32_t n_batc
         }
         if (n_cls[1] > 0) {
             p.items = d_items + n_cls[0]; p.n_items = n_cls[1];
-            launch_attend_mma(p, c.head_dim, c.n_kv_heads, total_splits[1], pool->G * cls_max_q[1], st);
+            if (legacy_chunk) launch_attend_mma(p, c.head_dim, c.n_kv_heads, total_splits[1], pool->G * cls_max_q[1], st);
+            else launch_attend_umma(p, c.head_dim, c.n_kv_heads, total_splits[1], st);
             ++pool->n_launch;
             CU(cudaGetLastError());
             for (int i = 0; i < n_cls[1]; ++i)
@@ -795,7 +813,7 @@ int metronome_pool_read_profile(metronome_pool_t* pool, double* attend_kernel_ms
 }
 
 int metronome_pool_set_tuning(metronome_pool_t* pool, int32_t split_tokens, int32_t kernel_family) {
-    if (!pool || split_tokens < 0 || kernel_family < 0 || kernel_family > 2) return METRONOME_ERR_INVALID_ARG;
+    if (!pool || split_tokens < 0 || kernel_family < 0 || kernel_family > 3) return METRONOME_ERR_INVALID_ARG;
     pool->tune_split_tokens = split_tokens;
     pool->tune_family = kernel_family;
     return METRONOME_OK;
