@@ -17,7 +17,7 @@
 //               completion is signalled with tcgen05.commit on mbarriers
 //   warps 2-5   softmax warpgroup of slot 0, warps 6-9 of slot 1: ONE THREAD PER QUERY ROW
 //               (tcgen05.ld 32x32b): token-exact union mask on boundary stages, row max and row sum
-//               without any shuffle, exp2 in the log2 domain, P rounded to bf16 and written back to
+//               without any shuffle, exp2 in the log2 domain, P split into bf16 hi + lo and written back to
 //               TMEM over S (tcgen05.st), lazy rescale of O (only when the max moved by > 2^8)
 //
 // Two slots (S, P and O regions in TMEM: 2 x (128 + D) columns of the 512) ping-pong so the tensor
@@ -34,6 +34,20 @@
 #include "attend_mma.cuh"
 
 namespace metronome {
+
+// Timeline probe for the microbenchmark harness (compiled out of the library): clock64 stamps of
+// one CTA's roles.
+#ifdef METRONOME_TRACE
+__device__ long long g_trace[4 * 1024];
+__device__ int g_trace_cta = 0;
+#define MTRACE(role, idx)                                                                        \
+    do {                                                                                        \
+        if (blockIdx.x == 0 && (int)blockIdx.y == g_trace_cta && (threadIdx.x & 31) == 0 && (idx) < 1024) \
+            g_trace[(role) * 1024 + (idx)] = clock64();                                         \
+    } while (0)
+#else
+#define MTRACE(role, idx) do { } while (0)
+#endif
 
 template <int D>
 struct UmmaCfg {
@@ -59,10 +73,15 @@ __device__ __forceinline__ uint64_t umma_desc(uint32_t saddr, uint32_t lbo_bytes
     return (uint64_t)((saddr >> 4) & 0x3FFFu) | ((uint64_t)((lbo_bytes >> 4) & 0x3FFFu) << 16) |
            ((uint64_t)((sbo_bytes >> 4) & 0x3FFFu) << 32) | ((uint64_t)1 << 46) | ((uint64_t)2 << 61);
 }
-// instruction descriptor, kind::f16: bf16 x bf16 -> f32, M = 128
-__host__ __device__ constexpr uint32_t umma_idesc(int n, bool b_mn_major) {
-    return (1u << 4) | (1u << 7) | (1u << 10) | ((b_mn_major ? 1u : 0u) << 16) | ((uint32_t)(n >> 3) << 17) |
-           ((uint32_t)(128 >> 4) << 24);
+// instruction descriptor, kind::f16: (bf16 | fp16) A x bf16 B -> f32, M = 128
+__host__ __device__ constexpr uint32_t umma_idesc(int n, bool b_mn_major, bool a_fp16 = false) {
+    return (1u << 4) | ((a_fp16 ? 0u : 1u) << 7) | (1u << 10) | ((b_mn_major ? 1u : 0u) << 16) |
+           ((uint32_t)(n >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+}
+__device__ __forceinline__ uint32_t pack_f16(float a, float b) {
+    uint32_t r;
+    asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(b), "f"(a));     // a -> low half
+    return r;
 }
 __device__ __forceinline__ void umma_ss(uint32_t d_tmem, uint64_t a, uint64_t b, uint32_t idesc, uint32_t accum) {
     asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
@@ -83,14 +102,6 @@ __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.a
 __device__ __forceinline__ void named_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 __device__ __forceinline__ void named_arrive(int id, int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 
-// barrier with an OR-reduction of a predicate over its `n` participating threads
-__device__ __forceinline__ bool named_sync_or(int id, int n, bool pred) {
-    uint32_t out;
-    asm volatile("{\n\t.reg .pred p, q;\n\tsetp.ne.u32 q, %1, 0;\n\tbar.red.or.pred p, %2, %3, q;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-                 : "=r"(out) : "r"((uint32_t)pred), "r"(id), "r"(n) : "memory");
-    return out != 0;
-}
-
 // 32 lanes x 32 consecutive 32-bit columns: thread i of the warp gets lane (quarter base + i)
 __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t* r) {
     asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 "
@@ -108,6 +119,13 @@ __device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t* r) {
                    "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]),
                    "r"(r[16]), "r"(r[17]), "r"(r[18]), "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]),
                    "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]), "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31])
+                 : "memory");
+}
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t* r) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], "
+                 "{%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
+                 ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]),
+                   "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
                  : "memory");
 }
 __device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
@@ -136,7 +154,6 @@ attend_umma_kernel(AttendParams p) {
     auto bar_p = [&](int s) { return sBar + 8u * (2 * C::NBUF + 2 + s); };      // P_s written (softmax -> MMA)
     auto bar_o = [&](int s) { return sBar + 8u * (2 * C::NBUF + 4 + s); };      // last P V of slot s done
     volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(gen + C::kBarOff + 2 * 8 * C::NBUF + 6 * 8);
-    volatile uint32_t* lo_flag = tmem_slot + 2;                                 // [slot]: P_lo of this stage is valid
 
     const int32_t kvh = blockIdx.x;
     const int32_t i = find_item(p.n_items, (int32_t)blockIdx.y, [&](int32_t k) { return p.items[k].split_off; });
@@ -224,18 +241,16 @@ attend_umma_kernel(AttendParams p) {
             __syncwarp();
         };
         // O_slot (+)= P_slot V over the V stage in ring entry e: one K=16 MMA per valid block
-        // (P = bf16 hi [+ bf16 lo when the softmax warps flagged a peaky stage]: columns 0-63 / 64-127 of S_slot)
+        // (P = bf16 hi + bf16 lo: per 32-column chunk of S_slot, hi in columns 0-15, lo in 16-31)
         auto issue_pv = [&](int32_t slot, int32_t e, int32_t nt, bool accumulate) {
             if (lane == 0) {
                 const uint32_t vb = sRing + (e % C::NBUF) * C::kBufBytes;
-                const bool lo = lo_flag[slot] != 0;
-                for (int32_t b = 0; b < nt; ++b)
-                    umma_ts(tmem + C::kColO + D * slot, tmem + C::kColS + 128 * slot + 8 * b,
-                            umma_desc(vb + b * C::kTileBytes, 2048, 1024), idesc_pv, (accumulate || b > 0) ? 1u : 0u);
-                if (lo)
-                    for (int32_t b = 0; b < nt; ++b)
-                        umma_ts(tmem + C::kColO + D * slot, tmem + C::kColS + 128 * slot + 64 + 8 * b,
-                                umma_desc(vb + b * C::kTileBytes, 2048, 1024), idesc_pv, 1u);
+                for (int32_t b = 0; b < nt; ++b) {
+                    const uint32_t pa = tmem + C::kColS + 128 * slot + 32 * (b >> 1) + 8 * (b & 1);
+                    const uint64_t vd = umma_desc(vb + b * C::kTileBytes, 2048, 1024);
+                    umma_ts(tmem + C::kColO + D * slot, pa, vd, idesc_pv, (accumulate || b > 0) ? 1u : 0u);
+                    umma_ts(tmem + C::kColO + D * slot, pa + 16, vd, idesc_pv, 1u);
+                }
             }
             __syncwarp();
         };
@@ -264,9 +279,11 @@ attend_umma_kernel(AttendParams p) {
                 const int32_t ev = umma_entry_v(true, j, n_stage), nt = stage_nt(j);
                 const bool more = j + 1 < n_stage;
                 wait_full(ev);
+                MTRACE(1, 4 * j + 2);
                 fix_ragged_v(ev, tl0 + j * C::KS, nt);
                 mbar_wait(bar_p(0), j & 1);
                 tc_fence_after();
+                MTRACE(1, 4 * j + 3);
                 issue_pv(0, ev, nt, j > 0);
                 if (!more && lane == 0) umma_commit(bar_o(0));
                 if (more) {
@@ -274,8 +291,10 @@ attend_umma_kernel(AttendParams p) {
                     wait_full(ek);
                     issue_qk(0, 0, ek);
                 }
+                MTRACE(1, 4 * j + 4);
                 mbar_wait(bar_p(1), j & 1);
                 tc_fence_after();
+                MTRACE(1, 4 * j + 5);
                 issue_pv(1, ev, nt, j > 0);
                 release(ev);
                 if (!more && lane == 0) umma_commit(bar_o(1));
@@ -316,6 +335,7 @@ attend_umma_kernel(AttendParams p) {
     }
 
     // ================================ softmax warps ================================
+    if ((warp & 3) == 0) MTRACE(2 + ((warp - 2) >> 2), 1002);
     const int32_t slot = (warp - 2) >> 2, quarter = warp & 3;       // TMEM lanes 32 (warp % 4) .. + 31
     const int32_t row = quarter * 32 + lane;
     const int32_t tile_row0 = two ? 128 * slot : 0;
@@ -332,62 +352,88 @@ attend_umma_kernel(AttendParams p) {
         const int32_t tid2 = threadIdx.x - 64;
         const int32_t n_rows = two ? 256 : 128;
         constexpr int CPR = D / 8;                                    // 16-byte chunks per row
+        // 16-byte cp.async per chunk: all of a thread's copies are in flight together
         for (int32_t idx = tid2; idx < n_rows * CPR; idx += 256) {
             const int32_t rr = idx / CPR, c = idx % CPR;
-            uint4 v = make_uint4(0u, 0u, 0u, 0u);
+            const uint32_t dst = (rr >> 7) * C::kQBytes + (c >> 3) * C::kHalfBytes + (rr & 127) * 128 + (((c & 7) ^ (rr & 7)) << 4);
             if (rr < R) {
                 const int32_t r2 = rr / p.G, g2 = rr - r2 * p.G;
-                v = __ldg(reinterpret_cast<const uint4*>(p.q + ((int64_t)(it.q_row_off + r2) * p.Hq + kvh * p.G + g2) * D) + c);
+                const __nv_bfloat16* src = p.q + ((int64_t)(it.q_row_off + r2) * p.Hq + kvh * p.G + g2) * D + c * 8;
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sQ + dst), "l"(src) : "memory");
+            } else {
+                *reinterpret_cast<uint4*>(gen + dst) = make_uint4(0u, 0u, 0u, 0u);
             }
-            *reinterpret_cast<uint4*>(gen + (rr >> 7) * C::kQBytes + (c >> 3) * C::kHalfBytes + (rr & 127) * 128 +
-                                      (((c & 7) ^ (rr & 7)) << 4)) = v;
         }
+        asm volatile("cp.async.commit_group;\n\tcp.async.wait_group 0;" ::: "memory");
         fence_async_smem();
     }
     named_sync(1, C::kThreads);
     tc_fence_after();
+    if ((warp & 3) == 0) MTRACE(2 + ((warp - 2) >> 2), 1003);
     const uint32_t tmem = *tmem_slot;
     const uint32_t lane_base = (uint32_t)(quarter * 32) << 16;
     const uint32_t tS = tmem + lane_base + C::kColS + 128 * slot;     // S (fp32) and, over it, P (bf16 x 2 per column)
     const uint32_t tO = tmem + lane_base + C::kColO + D * slot;
 
-    float m_run = -INFINITY, m_used = -INFINITY, l = 0.f;
+    // One stage of one slot, per thread = per query row: 128 scores in TMEM.  The scores are read
+    // in 32-column chunks, twice (pass 1: row max; pass 2: exp2, round, write P), with the next
+    // chunk's tcgen05.ld in flight while the current one is processed: ~100 live registers instead
+    // of 128 scores + 128 weights (which spilled), and P chunk c (16 columns) lands on columns the
+    // pass has already consumed.
+    float m_run = -INFINITY, m_used = -INFINITY;
+    float l0 = 0.f, l1 = 0.f, l2 = 0.f, l3 = 0.f;                     // four partial sums (ILP)
     int32_t n_it = 0;
     for (int32_t j = two ? 0 : slot; j < n_stage; j += two ? 1 : 2, ++n_it) {
+        if (quarter == 0) MTRACE(2 + slot, 16 * n_it + 0);
         mbar_wait(bar_s(slot), n_it & 1);
         tc_fence_after();
-        uint32_t s[128];
+        if (quarter == 0) MTRACE(2 + slot, 16 * n_it + 1);
         float sub = 0.f;
-        bool need_lo = false;
+        bool full = true;
+        const int32_t t0 = tl0 + j * C::KS;
+        const int32_t nt = min(C::KS, tl1 - t0);
+        auto mask_chunk = [&](uint32_t (&s)[32], int c) {
+#pragma unroll
+            for (int bb = 0; bb < 2; ++bb) {
+                const int32_t b = 2 * c + bb;
+                const int32_t p0 = b < nt ? tile_block(it, t0 + b) * kBlockTokens : INT32_MAX / 2;
+#pragma unroll
+                for (int k = 0; k < kBlockTokens; ++k)
+                    if (!admit(p0 + k, t, p.S, p.W)) s[bb * kBlockTokens + k] = 0xFF800000u;   // -inf
+            }
+        };
+        uint32_t sa[32], sb[32];
         if (warp_active) {
-#pragma unroll
-            for (int c = 0; c < 4; ++c) tmem_ld32(tS + 32 * c, s + 32 * c);
-            tmem_wait_ld();
-            const int32_t t0 = tl0 + j * C::KS;
-            const int32_t nt = min(C::KS, tl1 - t0);
+            tmem_ld32(tS, sa);
             // a stage needs no mask when every key of it is admitted for every row of this warp
-            bool full = nt == C::KS;
-            for (int32_t b = 0; b < nt && full; ++b) {
-                const int32_t pe = tile_block(it, t0 + b) * kBlockTokens + kBlockTokens - 1;
-                full = pe <= t_wmin && (pe < p.S || t_wmax - (pe - (kBlockTokens - 1)) < p.W);
-            }
-            if (!full) {
-#pragma unroll
-                for (int b = 0; b < C::KS; ++b) {
-                    const int32_t p0 = b < nt ? tile_block(it, t0 + b) * kBlockTokens : INT32_MAX / 2;
-#pragma unroll
-                    for (int c = 0; c < kBlockTokens; ++c)
-                        if (!admit(p0 + c, t, p.S, p.W)) s[b * kBlockTokens + c] = 0xFF800000u;   // -inf
-                }
-            }
+            // (window tiles are consecutive logical blocks; a stage that holds sink tiles takes the mask)
+            const int32_t p_first = tile_block(it, t0) * kBlockTokens;
+            full = nt == C::KS && t0 >= it.n_sink_tiles && p_first + C::KS * kBlockTokens - 1 <= t_wmin &&
+                   t_wmax - p_first < p.W;
+            // ---- pass 1: row max ----
             float mx0 = -INFINITY, mx1 = -INFINITY, mx2 = -INFINITY, mx3 = -INFINITY;
+            auto max_chunk = [&](uint32_t (&cur)[32], uint32_t (&nxt)[32], int c) {
+                tmem_wait_ld();
+                if (c < 3) tmem_ld32(tS + 32 * (c + 1), nxt);
+                if (!full) mask_chunk(cur, c);
 #pragma unroll
-            for (int c = 0; c < 128; c += 4) {
-                mx0 = fmaxf(mx0, __uint_as_float(s[c]));
-                mx1 = fmaxf(mx1, __uint_as_float(s[c + 1]));
-                mx2 = fmaxf(mx2, __uint_as_float(s[c + 2]));
-                mx3 = fmaxf(mx3, __uint_as_float(s[c + 3]));
-            }
+                for (int k = 0; k < 32; k += 4) {
+                    mx0 = fmaxf(mx0, __uint_as_float(cur[k]));
+                    mx1 = fmaxf(mx1, __uint_as_float(cur[k + 1]));
+                    mx2 = fmaxf(mx2, __uint_as_float(cur[k + 2]));
+                    mx3 = fmaxf(mx3, __uint_as_float(cur[k + 3]));
+                }
+                if (quarter == 0) MTRACE(2 + slot, 16 * n_it + 2 + c);
+            };
+#ifndef EXP_NOPASS1
+            max_chunk(sa, sb, 0);
+            max_chunk(sb, sa, 1);
+            max_chunk(sa, sb, 2);
+            max_chunk(sb, sa, 3);
+#else
+            tmem_wait_ld(); mx0 = 8.f;
+#endif
+            tmem_ld32(tS, sa);                                        // pass 2, chunk 0: in flight over the rescale
             const float mx = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * p.scale_log2;
             m_run = fmaxf(m_run, mx);
             if (n_it == 0) {
@@ -397,57 +443,58 @@ attend_umma_kernel(AttendParams p) {
                 const bool need = (m_run - m_used) > 8.f;             // (-inf) - (-inf) = NaN -> false
                 if (__any_sync(0xffffffffu, need)) {
                     const float f = (need && m_used != -INFINITY) ? ex2(m_used - m_run) : 1.f;
-                    l *= f;
+                    l0 *= f; l1 *= f; l2 *= f; l3 *= f;
+                    tmem_wait_ld();                                   // (chunk 0 of pass 2 has landed in sa)
 #pragma unroll
                     for (int c = 0; c < D / 32; ++c) {
-                        uint32_t o[32];
-                        tmem_ld32(tO + 32 * c, o);
+                        tmem_ld32(tO + 32 * c, sb);
                         tmem_wait_ld();
 #pragma unroll
-                        for (int k = 0; k < 32; ++k) o[k] = __float_as_uint(__uint_as_float(o[k]) * f);
-                        tmem_st32(tO + 32 * c, o);
+                        for (int k = 0; k < 32; ++k) sb[k] = __float_as_uint(__uint_as_float(sb[k]) * f);
+                        tmem_st32(tO + 32 * c, sb);
                     }
                     if (need) m_used = m_run;
                 }
             }
             sub = m_used == -INFINITY ? 0.f : m_used;                 // nothing admitted yet: every p is 0
-            // a key that carries more than 1/32 of the running sum: P needs its bf16 lo part too
-            need_lo = valid && ex2(mx - sub) * 32.f > l;
-        }
-        const bool lo = named_sync_or(4 + slot, 128, need_lo);        // one decision for the slot's 128 rows
-        if (warp_active) {
-            uint32_t pk[64];
-            if (lo) {
-                uint32_t pl[64];
+            if (quarter == 0) MTRACE(2 + slot, 16 * n_it + 6);
+            // ---- pass 2: p = 2^(s * scale - m); P = bf16 hi + bf16 lo (2^-17 weights: the x20 outlier
+            // channels of config 4 need more than bf16's 2^-9), hi | lo of chunk c over S columns
+            // [32c, 32c+16) | [32c+16, 32c+32), which the pass has just consumed ----
+            auto exp_chunk = [&](uint32_t (&cur)[32], uint32_t (&nxt)[32], int c) {
+                tmem_wait_ld();
+                if (c < 3) tmem_ld32(tS + 32 * (c + 1), nxt);
+                if (!full) mask_chunk(cur, c);
+                uint32_t pk[32];
 #pragma unroll
-                for (int k = 0; k < 64; ++k) {
-                    const float p0 = ex2(fmaf(__uint_as_float(s[2 * k]), p.scale_log2, -sub));
-                    const float p1 = ex2(fmaf(__uint_as_float(s[2 * k + 1]), p.scale_log2, -sub));
+                for (int k = 0; k < 16; k += 2) {
+                    const float p0 = ex2(fmaf(__uint_as_float(cur[2 * k]), p.scale_log2, -sub));
+                    const float p1 = ex2(fmaf(__uint_as_float(cur[2 * k + 1]), p.scale_log2, -sub));
+                    const float p2 = ex2(fmaf(__uint_as_float(cur[2 * k + 2]), p.scale_log2, -sub));
+                    const float p3 = ex2(fmaf(__uint_as_float(cur[2 * k + 3]), p.scale_log2, -sub));
                     pk[k] = pack_bf16(p0, p1);
-                    pl[k] = pack_bf16(p0 - bf16lo(pk[k]), p1 - bf16hi(pk[k]));
-                    l += (bf16lo(pk[k]) + bf16lo(pl[k])) + (bf16hi(pk[k]) + bf16hi(pl[k]));
+                    pk[k + 1] = pack_bf16(p2, p3);
+                    pk[16 + k] = pack_bf16(p0 - bf16lo(pk[k]), p1 - bf16hi(pk[k]));
+                    pk[17 + k] = pack_bf16(p2 - bf16lo(pk[k + 1]), p3 - bf16hi(pk[k + 1]));
+                    l0 += p0; l1 += p1; l2 += p2; l3 += p3;
                 }
-                tmem_st32(tS + 64, pl);
-                tmem_st32(tS + 96, pl + 32);
-            } else {
-#pragma unroll
-                for (int k = 0; k < 64; ++k) {
-                    const float p0 = ex2(fmaf(__uint_as_float(s[2 * k]), p.scale_log2, -sub));
-                    const float p1 = ex2(fmaf(__uint_as_float(s[2 * k + 1]), p.scale_log2, -sub));
-                    pk[k] = pack_bf16(p0, p1);
-                    l += bf16lo(pk[k]) + bf16hi(pk[k]);               // the denominator sees the rounded weights
-                }
-            }
-            tmem_st32(tS, pk);
-            tmem_st32(tS + 32, pk + 32);
+                tmem_st32(tS + 32 * c, pk);
+                if (quarter == 0) MTRACE(2 + slot, 16 * n_it + 8 + c);
+            };
+            exp_chunk(sa, sb, 0);
+            exp_chunk(sb, sa, 1);
+            exp_chunk(sa, sb, 2);
+            exp_chunk(sb, sa, 3);
             tmem_wait_st();
         }
-        if (quarter == 0 && lane == 0) lo_flag[slot] = lo ? 1u : 0u;
+        if (quarter == 0) MTRACE(2 + slot, 16 * n_it + 12);
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(bar_p(slot));
     }
+    float l = (l0 + l1) + (l2 + l3);
 
+    if (quarter == 0) MTRACE(2 + slot, 1000);
     // ---- epilogue ----
     const int64_t qrow = (int64_t)(it.q_row_off + rq) * p.Hq + kvh * p.G + gq;
     float* ml1 = reinterpret_cast<float*>(gen + C::kMlOff);
@@ -527,6 +574,7 @@ attend_umma_kernel(AttendParams p) {
             }
         }
     }
+    if (quarter == 0) MTRACE(2 + slot, 1001);
     tc_fence_before();
     named_arrive(2, C::kThreads - 32);
 }
