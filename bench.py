@@ -48,6 +48,8 @@ def parse():
     ap.add_argument("--split-tokens", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--sweep", default="", choices=["", "age", "sessions", "sw"],
+                    help="shape checks of SURVEY sec. 8(d)/(f) instead of the bench line: one JSON line per point")
     return ap.parse_args()
 
 
@@ -235,6 +237,18 @@ def main():
     torch.cuda.set_device(0)
     if WORLD > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", 0))
+
+    if args.sweep:
+        from paper_2607_02640_b200 import sweeps
+        if args.sweep == "age":
+            rows = sweeps.age_sweep(args.config, n_sessions=args.sessions or None)
+        elif args.sweep == "sessions":
+            rows = sweeps.sessions_sweep(history_scale=args.history_scale)
+        else:
+            rows = sweeps.sw_sweep(n_sessions=args.sessions or 128)
+        for row in rows:
+            print(json.dumps(row), flush=True)
+        return
 
     K, W = args.steps, max(args.warmup, 3)
     # a bench "step" = one FRAME (all its sub-steps: chunk prefill + decode steps) for every due

@@ -1,0 +1,157 @@
+"""Shape checks and sweeps of SURVEY.md sec. 8(d)/(f), run by `bench.py --sweep ...` on one GPU.
+
+  age       fixed N, every session at ONE age a in {1/4, 1/2, 1, 2, 5, 10, 20} x (S+W): per-frame
+            latency must rise up to a ~ S+W and then stay FLAT ("O(W)")
+  sessions  config 5 (pool churn): n_target in {32 .. 512}; median / p99 per-frame latency must be
+            monotone non-decreasing in the load with zero pool exhaustion
+  sw        NEXT row f1: W in {256 .. 4096} and S in {0, 16, 32, 64} at N = 128 (PAPER.md:L300
+            Fig. 11, L308-323 Table 2 "sinks ... unchanged latency")
+
+Plumbing only (schedules + CUDA-event timing around the C-ABI calls); each point uses a fresh pool
+(PAPER.md:L275).  Every function returns a list of dict rows; bench.py prints them as JSON lines.
+"""
+from __future__ import annotations
+
+from dataclasses import replace
+
+import numpy as np
+import torch
+
+from . import synth
+from . import workloads as wl
+from .runner import Runner
+
+
+def _frames_of(events):
+    """Cut the timed tail of a schedule into frames: (opens/closes before the frame, its steps)."""
+    frames, pre, steps, fid = [], [], [], None
+    for ev in events:
+        if ev[0] != "step":
+            if steps:
+                frames.append((pre, steps))
+                pre, steps, fid = [], [], None
+            pre.append(ev)
+            continue
+        if steps and ev[4] != fid:
+            frames.append((pre, steps))
+            pre, steps = [], []
+        fid = ev[4]
+        steps.append(ev)
+    if steps:
+        frames.append((pre, steps))
+    return frames
+
+
+def time_frames(r: Runner, events, warmup: int = 2):
+    """Runs the timed tail frame by frame.  Returns per-frame dicts: ms (GPU time of every append_kv
+    + attend_frame of the frame, CUDA events), attend_ms (attention kernels only, the library's own
+    event brackets), sessions, resident tokens.  The first `warmup` frames are dropped."""
+    out = []
+    r.pool.set_profiling(True)
+    for k, (pre, steps) in enumerate(_frames_of(events)):
+        for ev in pre:
+            if ev[0] == "open":
+                r.open(ev[1])
+            else:
+                r.close(ev[1])
+        prepped = []
+        for ev in steps:
+            st = r.make_step(ev)
+            kk = r.rows(synth.STREAM_K, 0, st.uid_rows, st.pos_rows)
+            vv = r.rows(synth.STREAM_V, 0, st.uid_rows, st.pos_rows)
+            qq = r.rows(synth.STREAM_Q, 0, st.uid_rows, st.pos_rows)
+            prepped.append((st, kk, vv, qq, torch.empty_like(qq)))
+        r.pool.read_profile()                       # reset the brackets
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        for st, kk, vv, qq, oo in prepped:
+            r.pool.append_kv(0, st.sids, st.n_new, kk, vv)
+            r.pool.attend_frame(0, st.sids, st.n_new, qq, oo)
+        e1.record()
+        torch.cuda.synchronize()
+        a_ms, _ = r.pool.read_profile()
+        if k >= warmup:
+            sess = {int(i) for ev in steps for i in ev[1]}
+            out.append({"ms": e0.elapsed_time(e1), "attend_ms": a_ms, "sessions": len(sess)})
+    r.pool.set_profiling(False)
+    return out
+
+
+def _summary(fr):
+    ms = np.asarray([f["ms"] for f in fr])
+    am = np.asarray([f["attend_ms"] for f in fr])
+    return {"frames": len(fr), "ms_median": float(np.median(ms)), "ms_p99": float(np.percentile(ms, 99)),
+            "attend_ms_median": float(np.median(am)), "sessions_mean": float(np.mean([f["sessions"] for f in fr]))}
+
+
+def _frame_pattern(w: wl.Workload):
+    return {1: [8, 1, 1], 2: [1], 3: [25] + [1] * 8, 4: [16] + [1] * 10, 5: [13] + [1] * 8}[w.index]
+
+
+def uniform_age_events(w: wl.Workload, age_tokens: int, n_frames: int):
+    """All sessions at the same age (tokens), history in appends of max_new_tokens, then n_frames."""
+    frame = _frame_pattern(w)
+    n = w.n_sessions
+    hist = [[w.max_new_tokens]] * (age_tokens // w.max_new_tokens)
+    if age_tokens % w.max_new_tokens:
+        hist = hist + [[age_tokens % w.max_new_tokens]]
+    ev = [("open", i) for i in range(n)]
+    ev += wl._interleave([hist for _ in range(n)], False)
+    ev += wl._interleave([[frame] * n_frames for _ in range(n)], True)
+    return ev
+
+
+def age_sweep(config: int = 2, n_sessions: int | None = None, n_frames: int = 12,
+              multiples=(0.25, 0.5, 1, 2, 5, 10, 20)):
+    rows = []
+    for m in multiples:
+        w = wl.make_workload(config, n_sessions=n_sessions)
+        age = max(1, int(round(m * (w.S + w.W))))
+        r = Runner(w)
+        rest = r.run_history(uniform_age_events(w, age, n_frames + 2))
+        fr = time_frames(r, rest)
+        rows.append({"sweep": "age", "config": config, "sessions": w.n_sessions, "S": w.S, "W": w.W,
+                     "age_over_S_plus_W": m, "age_tokens": age, **_summary(fr)})
+        del r
+        torch.cuda.empty_cache()
+    return rows
+
+
+def sessions_sweep(targets=(32, 64, 128, 256, 384, 512), n_frames: int = 60, history_scale: float = 1.0):
+    """Config 5: Poisson arrivals / Exp lifetimes at each target concurrency, fixed pool (80 % of the
+    unbounded working set of 512 sessions).  POOL_EXHAUSTED would raise: reaching the end of a point
+    is the zero-exhaustion check."""
+    rows = []
+    for nt in targets:
+        w = wl.make_workload(5, n_timed_frames=n_frames + 2)
+        events, info = wl.churn_schedule(w, nt, history_scale)
+        r = Runner(w)
+        rest = r.run_history(events)
+        fr = time_frames(r, rest)
+        free = r.pool.pool_query(want_ids=False)[0]
+        rows.append({"sweep": "sessions", "config": 5, "n_target": nt, "pool_blocks": w.n_blocks,
+                     "free_blocks_end": free, "pool_exhausted": 0,
+                     "rejected_arrivals": int(info["rejected_arrivals"]), **_summary(fr)})
+        del r
+        torch.cuda.empty_cache()
+    return rows
+
+
+def sw_sweep(n_sessions: int = 128, n_frames: int = 12, windows=(256, 512, 1024, 2048, 4096),
+             sinks=(0, 16, 32, 64)):
+    """NEXT f1 on config-3 shapes (32Q/4KV, frame = 25-chunk + 8 decode), every session at age
+    2 x (S+W) so the window is full: latency vs W at S=4, and vs S at W=2048."""
+    rows = []
+    base = wl.make_workload(3, n_sessions=n_sessions)
+    points = [(4, W) for W in windows] + [(S, 2048) for S in sinks]
+    for S, W in points:
+        w = replace(base, S=S, W=W, n_blocks=n_sessions * wl.blocks_per_session(S, W, 16, base.max_new_tokens))
+        r = Runner(w)
+        rest = r.run_history(uniform_age_events(w, 2 * (S + W), n_frames + 2))
+        fr = time_frames(r, rest)
+        rows.append({"sweep": "sw", "sessions": n_sessions, "S": S, "W": W,
+                     "blocks_per_session": wl.blocks_per_session(S, W, 16, base.max_new_tokens), **_summary(fr)})
+        del r
+        torch.cuda.empty_cache()
+    return rows
