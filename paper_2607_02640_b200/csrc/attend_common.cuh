@@ -41,6 +41,7 @@ struct AttendParams {
     float* ws_acc;            // [row][Hq][max_splits][D]   unnormalised partial outputs
     float* ws_ml;             // [row][Hq][max_splits][2]   running max (log2 domain), running sum
     int32_t max_splits;
+    int32_t* tickets;         // [item][Hkv] arrival counters of the stream-K pieces (zero between launches)
 };
 
 __device__ __forceinline__ float ex2(float x) {

@@ -473,10 +473,52 @@ attend_gqa_kernel(AttendParams p, GqaPlan plan) {
                     for (int d = 0; d < DPT; d += 2) dst[d >> 1] = pack_bf16(acc[d] * inv, acc[d + 1] * inv);
                 } else {
                     const int64_t slot = qrow * p.max_splits + ((int32_t)blockIdx.x - first_cta);
-                    float* dst = p.ws_acc + slot * D + sub * DPT;
+                    float4* dst = reinterpret_cast<float4*>(p.ws_acc + slot * D + sub * DPT);
 #pragma unroll
-                    for (int d = 0; d < DPT; ++d) dst[d] = acc[d];
-                    if (sub == 0) { p.ws_ml[slot * 2] = M; p.ws_ml[slot * 2 + 1] = l; }
+                    for (int d = 0; d < DPT; d += 4) __stcg(dst + (d >> 2), make_float4(acc[d], acc[d + 1], acc[d + 2], acc[d + 3]));
+                    if (sub == 0) __stcg(reinterpret_cast<float2*>(p.ws_ml + slot * 2), make_float2(M, l));
+                }
+            }
+            // ---- row a6, fused: the LAST piece of this (item, head) to arrive combines them all
+            // ("merged exactly once"); the ticket counter resets itself ----
+            if (first_cta != last_cta) {                       // CTA-uniform
+                __shared__ int32_t s_ticket;
+                int32_t* ticket = p.tickets + (int64_t)i * Hkv + kvh;
+                __threadfence();
+                __syncthreads();
+                if (threadIdx.x == 0) s_ticket = atomicAdd(ticket, 1);
+                __syncthreads();
+                const int32_t ns = last_cta - first_cta + 1;
+                if (s_ticket == ns - 1) {
+                    __threadfence();
+                    if (row < R) {
+                        const int32_t r = row / p.G, gq = row - r * p.G;
+                        const int64_t qrow = (int64_t)(it.q_row_off + r) * p.Hq + kvh * p.G + gq;
+                        const int64_t base = qrow * p.max_splits;
+                        constexpr int DPT = D / 8;
+                        float Mx = -INFINITY;
+                        for (int32_t s2 = 0; s2 < ns; ++s2) Mx = fmaxf(Mx, __ldcg(p.ws_ml + (base + s2) * 2));
+                        float acc[DPT], l = 0.f;
+#pragma unroll
+                        for (int d = 0; d < DPT; ++d) acc[d] = 0.f;
+                        for (int32_t s2 = 0; s2 < ns; ++s2) {
+                            const float2 ml = __ldcg(reinterpret_cast<const float2*>(p.ws_ml + (base + s2) * 2));
+                            if (ml.x == -INFINITY) continue;      // this piece admitted no key for this row
+                            const float w = ex2(ml.x - Mx);
+                            l += w * ml.y;
+                            const float4* src = reinterpret_cast<const float4*>(p.ws_acc + (base + s2) * D + sub * DPT);
+#pragma unroll
+                            for (int d = 0; d < DPT; d += 4) {
+                                const float4 a = __ldcg(src + (d >> 2));
+                                acc[d] += w * a.x; acc[d + 1] += w * a.y; acc[d + 2] += w * a.z; acc[d + 3] += w * a.w;
+                            }
+                        }
+                        const float inv = l > 0.f ? 1.f / l : 0.f;
+                        uint32_t* dst = reinterpret_cast<uint32_t*>(p.out + qrow * D + sub * DPT);
+#pragma unroll
+                        for (int d = 0; d < DPT; d += 2) dst[d >> 1] = pack_bf16(acc[d] * inv, acc[d + 1] * inv);
+                    }
+                    if (threadIdx.x == 0) *ticket = 0;
                 }
             }
         }
@@ -485,39 +527,6 @@ attend_gqa_kernel(AttendParams p, GqaPlan plan) {
         __syncthreads();
         g = pair_lo + b;
     }
-}
-
-// Merge of the stream-K pieces of the decode-class items.  grid = (n decode-class rows, Hq), block = D/4.
-template <int D>
-__global__ void __launch_bounds__(D / 4)
-merge_gqa_kernel(AttendParams p, GqaPlan plan) {
-    const int32_t h = blockIdx.y;
-    const int32_t i = find_item(p.n_items, (int32_t)blockIdx.x, [&](int32_t k) { return p.items[k].class_row_off; });
-    const AttendItem it = p.items[i];
-    const int32_t kvh = h / p.G;
-    const int64_t pair_lo = ((int64_t)it.tile_off * plan.n_kv_heads) + (int64_t)kvh * it.n_tiles;
-    const int32_t first_cta = gqa_first_cta(pair_lo, plan.tiles_per_cta);
-    const int32_t ns = gqa_first_cta(pair_lo + it.n_tiles - 1, plan.tiles_per_cta) - first_cta + 1;
-    if (ns <= 1) return;
-    const int64_t grow = (int64_t)it.q_row_off + ((int32_t)blockIdx.x - it.class_row_off);
-    const int64_t base = (grow * p.Hq + h) * p.max_splits;
-    float M = -INFINITY;
-    for (int s = 0; s < ns; ++s) M = fmaxf(M, p.ws_ml[(base + s) * 2]);
-    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-    float l = 0.f;
-    for (int s = 0; s < ns; ++s) {
-        const float m = p.ws_ml[(base + s) * 2];
-        if (m == -INFINITY) continue;
-        const float w = ex2(m - M);
-        l += w * p.ws_ml[(base + s) * 2 + 1];
-        const float4 a = reinterpret_cast<const float4*>(p.ws_acc + (base + s) * D)[threadIdx.x];
-        acc.x += w * a.x; acc.y += w * a.y; acc.z += w * a.z; acc.w += w * a.w;
-    }
-    const float inv = l > 0.f ? 1.f / l : 0.f;
-    uint2 o;
-    o.x = pack_bf16(acc.x * inv, acc.y * inv);
-    o.y = pack_bf16(acc.z * inv, acc.w * inv);
-    reinterpret_cast<uint2*>(p.out + (grow * p.Hq + h) * D)[threadIdx.x] = o;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -563,10 +572,4 @@ inline void launch_attend_gqa(const AttendParams& p, const GqaPlan& plan, int32_
     if (D == 128) attend_gqa_kernel<128><<<n_ctas, GqaCfg<128>::kThreads, GqaCfg<128>::kSmemBytes, st>>>(p, plan);
     else attend_gqa_kernel<64><<<n_ctas, GqaCfg<64>::kThreads, GqaCfg<64>::kSmemBytes, st>>>(p, plan);
 }
-inline void launch_merge_gqa(const AttendParams& p, const GqaPlan& plan, int32_t D, int32_t n_rows, cudaStream_t st) {
-    dim3 grid(n_rows, p.Hq);
-    if (D == 128) merge_gqa_kernel<128><<<grid, 32, 0, st>>>(p, plan);
-    else merge_gqa_kernel<64><<<grid, 16, 0, st>>>(p, plan);
-}
-
 }  // namespace metronome

@@ -59,6 +59,7 @@ struct metronome_pool {
     uint8_t* d_kv = nullptr;
     float* d_ws_acc = nullptr;
     float* d_ws_ml = nullptr;
+    int32_t* d_tickets = nullptr;      // [max_sessions][Hkv], zero between launches
     size_t ws_slots = 0;               // capacity in (row, head, split) slots
     uint8_t* d_io = nullptr;           // staging for metronome_step_host
     size_t io_bytes = 0;
@@ -276,6 +277,9 @@ int metronome_pool_create(const metronome_pool_config_t* cfg, metronome_pool_t**
         if (pool->poison) fill_nan_kernel<<<1184, 256>>>((uint4*)pool->d_kv, (int64_t)(need / 16));
     }
     pool->slot_bytes = (size_t)c.max_sessions * (sizeof(AppendItem) > sizeof(AttendItem) ? sizeof(AppendItem) : sizeof(AttendItem));
+    e = cudaMalloc(&pool->d_tickets, (size_t)c.max_sessions * c.n_kv_heads * sizeof(int32_t));
+    if (e != cudaSuccess) return fail(METRONOME_ERR_OUT_OF_MEMORY, e, "cudaMalloc tickets");
+    cudaMemset(pool->d_tickets, 0, (size_t)c.max_sessions * c.n_kv_heads * sizeof(int32_t));
     e = cudaMallocHost(&pool->h_stage, pool->slot_bytes * kStagingSlots);
     if (e != cudaSuccess) return fail(METRONOME_ERR_OUT_OF_MEMORY, e, "cudaMallocHost staging");
     e = cudaMalloc(&pool->d_stage, pool->slot_bytes * kStagingSlots);
@@ -298,6 +302,7 @@ int metronome_pool_destroy(metronome_pool_t* pool) {
     if (!pool) return METRONOME_OK;
     cudaDeviceSynchronize();
     if (pool->d_table) cudaFree(pool->d_table);
+    if (pool->d_tickets) cudaFree(pool->d_tickets);
     if (pool->d_free) cudaFree(pool->d_free);
     if (pool->own_kv && pool->d_kv) cudaFree(pool->d_kv);
     if (pool->d_ws_acc) cudaFree(pool->d_ws_acc);
@@ -624,6 +629,7 @@ int metronome_attend_frame(metronome_pool_t* pool, int32_t layer, int32_t n_batc
     p.Hq = c.n_q_heads; p.G = pool->G;
     p.ws_acc = pool->d_ws_acc; p.ws_ml = pool->d_ws_ml;
     p.max_splits = max_splits;
+    p.tickets = pool->d_tickets;
 
     if (pool->profiling) {
         if (pool->prof_used + 2 > pool->prof_ev.size()) {
@@ -643,7 +649,6 @@ int metronome_attend_frame(metronome_pool_t* pool, int32_t layer, int32_t n_batc
             launch_attend_gqa(p, gplan, c.head_dim, gqa_ctas, st);
             ++pool->n_launch;
             CU(cudaGetLastError());
-            merge_cls[0] = gqa_ctas > 1;
         }
         if (n_cls[1] > 0) {
             p.items = d_items + n_cls[0]; p.n_items = n_cls[1];
@@ -669,12 +674,6 @@ int metronome_attend_frame(metronome_pool_t* pool, int32_t layer, int32_t n_batc
         pool->prof_used += 2;
     }
     // ---- row a6: combine the split-KV partials ----
-    if (family == 2 && merge_cls[0]) {
-        p.items = d_items; p.n_items = n_cls[0];
-        launch_merge_gqa(p, gplan, c.head_dim, cls_rows[0], st);
-        ++pool->n_launch;
-        CU(cudaGetLastError());
-    }
     for (int cls = (family == 2 ? 1 : 0); cls < 2; ++cls) {
         if (!merge_cls[cls] || (family != 2 && cls == 1)) continue;
         p.items = d_items + (cls == 0 ? 0 : n_cls[0]); p.n_items = n_cls[cls];
