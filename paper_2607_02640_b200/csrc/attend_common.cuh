@@ -41,6 +41,7 @@ struct AttendParams {
     float* ws_acc;            // [row][Hq][max_splits][D]   unnormalised partial outputs
     float* ws_ml;             // [row][Hq][max_splits][2]   running max (log2 domain), running sum
     int32_t max_splits;
+    int32_t pdl_early;        // let the next kernel on the stream start launching right away (PDL)
     int32_t* tickets;         // [item][Hkv] arrival counters of the stream-K pieces (zero between launches)
 };
 
@@ -80,6 +81,8 @@ __device__ __forceinline__ uint32_t pack_bf16(float a, float b) {
 template <int D>
 __global__ void __launch_bounds__(D / 4)
 merge_kernel(AttendParams p) {
+    if (p.pdl_early) pdl_launch_dependents();
+    pdl_wait();
     const int32_t h = blockIdx.y;
     const int32_t i = find_item(p.n_items, (int32_t)blockIdx.x, [&](int32_t k) { return p.items[k].class_row_off; });
     const int32_t ns = p.items[i].n_splits;

@@ -265,6 +265,8 @@ template <int D, int NW>
 __global__ void __launch_bounds__(MmaCfg<D, NW>::kThreads, 1)
 attend_mma_kernel(AttendParams p) {
     using C = MmaCfg<D, NW>;
+    if (p.pdl_early) pdl_launch_dependents();
+    pdl_wait();
     extern __shared__ __align__(128) uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 127u) & ~127u;     // tiles are 128-byte swizzle atoms
     const uint32_t bar_full = smem_base + C::NS * C::kStageBytes;
@@ -359,6 +361,8 @@ template <int D>
 __global__ void __launch_bounds__(GqaCfg<D>::kThreads)
 attend_gqa_kernel(AttendParams p, GqaPlan plan) {
     using C = GqaCfg<D>;
+    if (p.pdl_early) pdl_launch_dependents();
+    pdl_wait();                  // the work list and this step's K/V rows come from the append kernel
     extern __shared__ __align__(128) uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 127u) & ~127u;
     uint8_t* smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
@@ -568,8 +572,9 @@ inline void launch_attend_mma(const AttendParams& p, int32_t D, int32_t Hkv, int
 }
 
 // decode-class items (R <= 16)
-inline void launch_attend_gqa(const AttendParams& p, const GqaPlan& plan, int32_t D, int32_t n_ctas, cudaStream_t st) {
-    if (D == 128) attend_gqa_kernel<128><<<n_ctas, GqaCfg<128>::kThreads, GqaCfg<128>::kSmemBytes, st>>>(p, plan);
-    else attend_gqa_kernel<64><<<n_ctas, GqaCfg<64>::kThreads, GqaCfg<64>::kSmemBytes, st>>>(p, plan);
+inline cudaError_t launch_attend_gqa(const AttendParams& p, const GqaPlan& plan, int32_t D, int32_t n_ctas, cudaStream_t st,
+                                     bool pdl = false) {
+    if (D == 128) return launch_kernel(attend_gqa_kernel<128>, dim3(n_ctas), GqaCfg<128>::kThreads, GqaCfg<128>::kSmemBytes, st, pdl, p, plan);
+    return launch_kernel(attend_gqa_kernel<64>, dim3(n_ctas), GqaCfg<64>::kThreads, GqaCfg<64>::kSmemBytes, st, pdl, p, plan);
 }
 }  // namespace metronome

@@ -33,6 +33,8 @@ __device__ __forceinline__ void merge_state(float& m, float& l, float (&acc)[8],
 template <int D>
 __global__ void __launch_bounds__(128)
 attend_rows_kernel(AttendParams p) {
+    if (p.pdl_early) pdl_launch_dependents();
+    pdl_wait();                  // the work list and this step's K/V rows come from the append kernel
     constexpr int LPT = D / 8;         // lanes per token (16-byte chunks per row)
     constexpr int TPS = 32 / LPT;      // tokens per warp step
     constexpr int STEPS = kBlockTokens / TPS;

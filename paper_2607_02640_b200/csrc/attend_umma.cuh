@@ -144,6 +144,8 @@ template <int D>
 __global__ void __launch_bounds__(UmmaCfg<D>::kThreads, 1)
 attend_umma_kernel(AttendParams p) {
     using C = UmmaCfg<D>;
+    if (p.pdl_early) pdl_launch_dependents();
+    pdl_wait();                  // the work list and this step's K/V rows come from the append kernel
     extern __shared__ __align__(1024) uint8_t smem_umma[];
     const uint32_t base = (smem_u32(smem_umma) + 1023u) & ~1023u;       // swizzle atoms are 1024-byte aligned
     uint8_t* gen = smem_umma + (base - smem_u32(smem_umma));
@@ -593,10 +595,11 @@ inline cudaError_t configure_attend_umma_kernels() {
 }
 
 // chunk-class items (16 < R <= 256): p.items / p.n_items must point at them
-inline void launch_attend_umma(const AttendParams& p, int32_t D, int32_t Hkv, int32_t total_splits, cudaStream_t st) {
+inline cudaError_t launch_attend_umma(const AttendParams& p, int32_t D, int32_t Hkv, int32_t total_splits, cudaStream_t st,
+                                      bool pdl = false) {
     dim3 grid(Hkv, total_splits);
-    if (D == 128) attend_umma_kernel<128><<<grid, UmmaCfg<128>::kThreads, UmmaCfg<128>::kSmemBytes, st>>>(p);
-    else attend_umma_kernel<64><<<grid, UmmaCfg<64>::kThreads, UmmaCfg<64>::kSmemBytes, st>>>(p);
+    if (D == 128) return launch_kernel(attend_umma_kernel<128>, grid, UmmaCfg<128>::kThreads, UmmaCfg<128>::kSmemBytes, st, pdl, p);
+    return launch_kernel(attend_umma_kernel<64>, grid, UmmaCfg<64>::kThreads, UmmaCfg<64>::kSmemBytes, st, pdl, p);
 }
 
 }  // namespace metronome

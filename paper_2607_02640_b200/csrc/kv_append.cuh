@@ -38,6 +38,133 @@ kv_append_kernel(const AppendItem* __restrict__ items, const int32_t* __restrict
     *reinterpret_cast<uint4*>(tile + L.tile_bytes + off) = vv;
 }
 
+// ------------------------------------------------------------------------------------------------
+// One launch per append_kv call: rows a2 + a3 (bookkeeping) and a4 (KV scatter) fused, and the
+// attention work list of the same step (row a8) carried to the device on the way.
+//
+// grid = (ceil(max_n_new * Hkv * D/8 / 256), n_items + 1), block = 256.
+//   CTA (0, 0)    the bookkeeping CTA: the two phases of bookkeeping.cuh over the whole batch, then
+//                 it publishes `epoch` in *bk_flag (release).  It is the first CTA in dispatch
+//                 order and waits on nobody.  It also copies the step's AttendItems host -> device.
+//   CTA (x, y>0)  scatter CTAs of item y-1.  Only items that allocate a block in this call
+//                 (n_alloc > 0) read a table entry the bookkeeping CTA writes: they spin on the flag.
+// `items` (and `attend_src`) point into the pool's PINNED HOST staging ring: the kernel reads the
+// per-call metadata over the bus itself, so there is no separate H2D copy on the stream, and those
+// reads are issued BEFORE griddepcontrol.wait, i.e. while the previous kernel is still running when
+// the launch is programmatic (PDL).
+struct AppendParams {
+    const AppendItem* items;
+    int32_t n_items;
+    int32_t* table;
+    int32_t tbl_width, n_sink, ring;
+    int32_t* free_stack;
+    int32_t n_free0, total_freed;
+    int32_t do_bookkeeping;        // 0: layers > 0, or nothing to free / allocate, or done by bookkeeping_kernel
+    int32_t* bk_flag;
+    int32_t epoch;
+    int32_t pdl_early;
+    const uint4* attend_src;       // AttendItems of this step (host), attend_n16 x 16 bytes; may be null
+    uint4* attend_dst;
+    int32_t attend_n16;
+    const uint4* k_new;
+    const uint4* v_new;
+    uint8_t* kv_layer;             // null: metadata only
+    KvLayout L;
+};
+
+constexpr int kAppendSmemItems = 1024;       // AppendItems the bookkeeping CTA stages in shared memory
+
+__global__ void __launch_bounds__(256)
+append_fused_kernel(const AppendParams a) {
+    extern __shared__ __align__(16) uint8_t smem_items[];
+    if (a.pdl_early) pdl_launch_dependents();
+    if (blockIdx.y == 0) {
+        if (blockIdx.x != 0) return;
+        // ---- bookkeeping CTA ----
+        constexpr int kPre = 8;                        // 8 x 256 x 16 B = 682 AttendItems in registers
+        uint4 pre[kPre];
+#pragma unroll
+        for (int k = 0; k < kPre; ++k) {
+            const int32_t idx = k * 256 + (int32_t)threadIdx.x;
+            if (idx < a.attend_n16) pre[k] = a.attend_src[idx];
+        }
+        const bool staged = a.do_bookkeeping && a.n_items <= kAppendSmemItems;
+        if (staged) {
+            const uint4* src = reinterpret_cast<const uint4*>(a.items);
+            uint4* dst = reinterpret_cast<uint4*>(smem_items);
+            const int32_t n16 = a.n_items * (int32_t)(sizeof(AppendItem) / 16);
+            for (int32_t idx = threadIdx.x; idx < n16; idx += 256) dst[idx] = src[idx];
+        }
+        pdl_wait();
+#pragma unroll
+        for (int k = 0; k < kPre; ++k) {
+            const int32_t idx = k * 256 + (int32_t)threadIdx.x;
+            if (idx < a.attend_n16) a.attend_dst[idx] = pre[k];
+        }
+        for (int32_t idx = kPre * 256 + threadIdx.x; idx < a.attend_n16; idx += 256) a.attend_dst[idx] = a.attend_src[idx];
+        if (!a.do_bookkeeping) return;
+        __syncthreads();
+        const AppendItem* items = staged ? reinterpret_cast<const AppendItem*>(smem_items) : a.items;
+        // phase 1: evict (a2) -- PAPER.md:L256 "frees blocks that fall entirely behind the window"
+        for (int i = threadIdx.x; i < a.n_items; i += 256) {
+            const AppendItem it = items[i];
+            const int32_t* row = a.table + (int64_t)it.sid * a.tbl_width;
+            for (int k = 0; k < it.n_freed; ++k)
+                a.free_stack[a.n_free0 + it.free_off + k] = row[table_slot(it.free_lo + k, a.n_sink, a.ring)];
+        }
+        __syncthreads();
+        // phase 2: allocate (a3) -- pops from the top of the stack, batch order, ascending logical block
+        const int32_t top = a.n_free0 + a.total_freed - 1;
+        for (int i = threadIdx.x; i < a.n_items; i += 256) {
+            const AppendItem it = items[i];
+            int32_t* row = a.table + (int64_t)it.sid * a.tbl_width;
+            for (int k = 0; k < it.n_alloc; ++k)
+                row[table_slot(it.alloc_lo + k, a.n_sink, a.ring)] = a.free_stack[top - (it.alloc_off + k)];
+        }
+        __threadfence();
+        __syncthreads();
+        if (threadIdx.x == 0) asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(a.bk_flag), "r"(a.epoch) : "memory");
+        return;
+    }
+    // ---- scatter CTAs (a4) ----
+    if (!a.kv_layer) return;
+    const AppendItem it = a.items[blockIdx.y - 1];
+    const int32_t chunks_per_row = a.L.head_dim >> 3;
+    const int32_t chunks_per_tok = a.L.n_kv_heads * chunks_per_row;
+    const int32_t idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (blockIdx.x * (int32_t)blockDim.x >= it.n_new * chunks_per_tok) return;      // CTA-uniform
+    const bool active = idx < it.n_new * chunks_per_tok;
+    const int32_t tok = idx / chunks_per_tok;
+    const int32_t rem = idx - tok * chunks_per_tok;
+    const int32_t h = rem / chunks_per_row;
+    const int32_t c = rem - h * chunks_per_row;
+    const int64_t src = (int64_t)(it.row_off + tok) * chunks_per_tok + rem;
+    pdl_wait();                                       // k_new / v_new may come from the previous kernel
+    uint4 kk = make_uint4(0u, 0u, 0u, 0u), vv = kk;
+    if (active) {
+        kk = __ldg(a.k_new + src);
+        vv = __ldg(a.v_new + src);
+    }
+    if (a.do_bookkeeping && it.n_alloc > 0) {
+        if (threadIdx.x == 0) {
+            int32_t seen;
+            do {
+                asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(seen) : "l"(a.bk_flag) : "memory");
+                if (seen != a.epoch) __nanosleep(100);
+            } while (seen != a.epoch);
+        }
+        __syncthreads();
+    }
+    if (!active) return;
+    const int32_t pos = it.len0 + tok;
+    const int32_t blk = pos / kBlockTokens, r = pos % kBlockTokens;
+    const int32_t phys = __ldcg(a.table + (int64_t)it.sid * a.tbl_width + table_slot(blk, a.n_sink, a.ring));
+    uint8_t* tile = a.kv_layer + (int64_t)phys * a.L.block_bytes + (int64_t)h * a.L.head_bytes;
+    const int32_t off = tile_chunk_offset(r, c);
+    *reinterpret_cast<uint4*>(tile + off) = kk;
+    *reinterpret_cast<uint4*>(tile + a.L.tile_bytes + off) = vv;
+}
+
 // grid = ceil(n * Hkv * D/8 / 256); positions whose block is not resident give bf16 NaN.
 __global__ void __launch_bounds__(256)
 kv_read_kernel(const int32_t* __restrict__ row, int32_t n_sink, int32_t ring, int32_t n_sink_res,

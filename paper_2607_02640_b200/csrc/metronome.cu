@@ -8,6 +8,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <algorithm>
 #include <cstring>
 #include <new>
@@ -32,8 +33,27 @@ struct Session {
     int32_t last_n = 0;       // n_new of this session's most recent append
 };
 
-constexpr int kStagingSlots = 16;
+constexpr int kStagingSlots = 64;      // per-call metadata slots (pinned host + device twin)
+constexpr int kStagingGroup = 8;       // one completion event per 8 slots: an event between two kernels
+                                       // would break their programmatic (PDL) launch edge
 constexpr int kMaxSplits = 64;
+
+// Row a8: the launch plan of one attend_frame call (host side of the work list).  Items of class 0
+// go to the row kernel or the GQA decode kernel, items of class 1 (placed after them) to the chunk
+// kernel.
+struct AttendPlan {
+    bool valid = false;
+    int64_t epoch = -1;               // pool epoch the plan was made for (cached plans only)
+    int family = 1;                   // 1 CUDA-core rows, 2 tensor-core (gqa + chunk)
+    bool legacy_chunk = false;        // tuning family 3: mma.sync chunk kernel
+    int32_t n_items = 0;
+    int32_t n_cls[2] = {0, 0}, total_splits[2] = {0, 0}, cls_rows[2] = {0, 0}, cls_max_q[2] = {0, 0};
+    bool merge_cls[2] = {false, false};
+    int32_t max_splits = 1;
+    GqaPlan gplan{};
+    int32_t gqa_ctas = 0;
+    int64_t total_rows = 0;
+};
 
 }  // namespace
 
@@ -52,6 +72,7 @@ struct metronome_pool {
     int64_t epoch = 0;                 // number of layer-0 appends so far
     std::vector<int64_t> layer_epoch;  // epoch of each layer's latest append
     std::vector<int32_t> last_sids, last_n_new;
+    AttendPlan cached_plan;            // plan of attend_frame(q_lens = n_new) for the latest layer-0 append
 
     // device
     int32_t* d_table = nullptr;
@@ -60,6 +81,8 @@ struct metronome_pool {
     float* d_ws_acc = nullptr;
     float* d_ws_ml = nullptr;
     int32_t* d_tickets = nullptr;      // [max_sessions][Hkv], zero between launches
+    int32_t* d_bk_flag = nullptr;      // epoch of the last bookkeeping the fused append kernel finished
+    AttendItem* d_attend_items = nullptr;   // [max_sessions], written by the append kernel (cached plan)
     size_t ws_slots = 0;               // capacity in (row, head, split) slots
     uint8_t* d_io = nullptr;           // staging for metronome_step_host
     size_t io_bytes = 0;
@@ -68,8 +91,8 @@ struct metronome_pool {
     uint8_t* h_stage = nullptr;
     uint8_t* d_stage = nullptr;
     size_t slot_bytes = 0;
-    cudaEvent_t ev[kStagingSlots]{};
-    bool ev_used[kStagingSlots]{};
+    cudaEvent_t ev[kStagingSlots / kStagingGroup]{};
+    bool ev_used[kStagingSlots / kStagingGroup]{};
     int next_slot = 0;
 
     // profiling (metronome_pool_set_profiling): event pairs around the attention kernel
@@ -113,18 +136,26 @@ bool valid_cfg(const metronome_pool_config_t* c) {
 int acquire_stage(metronome_pool* pool, uint8_t** h, uint8_t** d, int* slot) {
     const int s = pool->next_slot;
     pool->next_slot = (s + 1) % kStagingSlots;
-    if (pool->ev_used[s]) CU(cudaEventSynchronize(pool->ev[s]));
+    // entering a group: every call that used it one lap ago must have been consumed by the GPU
+    // (calls on a pool are stream-ordered: the event after the group's last call covers them all)
+    if (s % kStagingGroup == 0 && pool->ev_used[s / kStagingGroup]) CU(cudaEventSynchronize(pool->ev[s / kStagingGroup]));
     *h = pool->h_stage + (size_t)s * pool->slot_bytes;
     *d = pool->d_stage + (size_t)s * pool->slot_bytes;
     *slot = s;
     return METRONOME_OK;
 }
+// after the last kernel / copy that reads the slot has been enqueued
+int release_stage(metronome_pool* pool, int slot, cudaStream_t st) {
+    if (slot % kStagingGroup == kStagingGroup - 1) {
+        CU(cudaEventRecord(pool->ev[slot / kStagingGroup], st));
+        pool->ev_used[slot / kStagingGroup] = true;
+    }
+    return METRONOME_OK;
+}
 int commit_stage(metronome_pool* pool, int slot, size_t bytes, cudaStream_t st) {
     CU(cudaMemcpyAsync(pool->d_stage + (size_t)slot * pool->slot_bytes, pool->h_stage + (size_t)slot * pool->slot_bytes,
                        bytes, cudaMemcpyHostToDevice, st));
-    CU(cudaEventRecord(pool->ev[slot], st));
-    pool->ev_used[slot] = true;
-    return METRONOME_OK;
+    return release_stage(pool, slot, st);
 }
 
 int check_batch(metronome_pool* pool, int32_t n_batch, const int32_t* sids, const int32_t* counts) {
@@ -149,19 +180,6 @@ int check_batch(metronome_pool* pool, int32_t n_batch, const int32_t* sids, cons
     return METRONOME_OK;
 }
 
-int launch_kv_write(metronome_pool* pool, int32_t layer, const AppendItem* d_items, int32_t n_items,
-                    int32_t max_n, const void* k_new, const void* v_new, cudaStream_t st) {
-    if (max_n == 0 || n_items == 0) return METRONOME_OK;
-    const int32_t chunks = max_n * pool->cfg.n_kv_heads * (pool->cfg.head_dim / 8);
-    dim3 grid((chunks + 255) / 256, n_items);
-    kv_append_kernel<<<grid, 256, 0, st>>>(d_items, pool->d_table, pool->tbl_width, pool->n_sink, pool->ring,
-                                           (const uint4*)k_new, (const uint4*)v_new,
-                                           pool->d_kv + (int64_t)layer * pool->L.layer_bytes, pool->L);
-    ++pool->n_launch;
-    CU(cudaGetLastError());
-    return METRONOME_OK;
-}
-
 int ensure_workspace(metronome_pool* pool, size_t slots) {
     if (slots <= pool->ws_slots) return METRONOME_OK;
     // cudaFree synchronises the device, so kernels still reading the old workspace are done
@@ -173,6 +191,209 @@ int ensure_workspace(metronome_pool* pool, size_t slots) {
     CU(cudaMalloc(&pool->d_ws_acc, want * pool->cfg.head_dim * sizeof(float)));
     CU(cudaMalloc(&pool->d_ws_ml, want * 2 * sizeof(float)));
     pool->ws_slots = want;
+    return METRONOME_OK;
+}
+
+// ---- row a8: the per-call work list, from the shadow counts ------------------------------------
+// Kernel families (north_star: "Tensor cores are used only for the GQA-group x chunk QK^T/PV tiles,
+// where the work really is a dense contraction"):
+//   rows   CUDA-core row kernel: pure multi-head decode (G x q_len < 4 for every item), and the
+//          general fallback
+//   gqa    tensor-core stream-K decode kernel: items with R = G x q_len <= 16
+//   chunk  tcgen05 / TMEM chunk-prefill kernel: items with 16 < R <= 256
+//          (tuning family 3: its mma.sync predecessor, R <= 208, kept for A/B measurements)
+// Fills items[0 .. plan.n_items) (host memory) and the plan; grows the split workspace if needed.
+int plan_attend(metronome_pool* pool, int32_t n_batch, const int32_t* sids, const int32_t* q_lens, AttendItem* items,
+                AttendPlan& pl) {
+    const metronome_pool_config_t& c = pool->cfg;
+    pl = AttendPlan();
+    int32_t max_q = 0;
+    for (int i = 0; i < n_batch; ++i) {
+        if (q_lens[i] > max_q) max_q = q_lens[i];
+        pl.total_rows += q_lens[i];
+    }
+    int family = pool->tune_family;
+    const bool legacy_chunk = family == 3;
+    if (family == 3) family = 2;
+    if (family == 0) family = (pool->G * max_q >= 4) ? 2 : 1;
+    if (family == 2 && !(legacy_chunk ? attend_mma_supported(pool->G, max_q) : attend_umma_supported(pool->G, max_q)))
+        family = 1;
+    pl.family = family;
+    pl.legacy_chunk = legacy_chunk;
+
+    const int32_t W = pool->W_eff;
+    int32_t* n_cls = pl.n_cls;
+    if (family == 2)
+        for (int i = 0; i < n_batch; ++i)
+            if (q_lens[i] > 0) ++n_cls[pool->G * q_lens[i] > 16 ? 1 : 0];
+    int32_t fill[2] = {0, n_cls[0]};
+    int32_t row = 0, n_items = 0;
+    for (int i = 0; i < n_batch; ++i) {
+        if (q_lens[i] == 0) continue;
+        const Session& s = pool->sessions[sids[i]];
+        const int cls = (family == 2 && pool->G * q_lens[i] > 16) ? 1 : 0;
+        AttendItem& it = items[family == 2 ? fill[cls]++ : n_items];
+        ++n_items;
+        memset(&it, 0, sizeof(it));
+        it.sid = sids[i];
+        it.len = (int32_t)s.len;
+        it.q_len = q_lens[i];
+        it.q_row_off = row;
+        row += q_lens[i];
+        const int32_t n_blk = (int32_t)((s.len + kBlockTokens - 1) / kBlockTokens);
+        const int64_t t0 = s.len - q_lens[i];                      // oldest query of this call
+        const int64_t wfirst = t0 - W + 1 > 0 ? t0 - W + 1 : 0;    // its oldest window key
+        int32_t first_blk = (int32_t)(wfirst / kBlockTokens);
+        if (first_blk < pool->n_sink) first_blk = pool->n_sink;
+        it.n_sink_tiles = n_blk < pool->n_sink ? n_blk : pool->n_sink;
+        it.first_blk = first_blk;
+        it.n_tiles = it.n_sink_tiles + (n_blk > first_blk ? n_blk - first_blk : 0);
+    }
+    pl.n_items = n_items;
+    if (family != 2) { n_cls[0] = n_items; n_cls[1] = 0; }
+    // chunk class: longest first, so the hardware's in-order CTA dispatch packs the short ones last
+    if (family == 2 && !legacy_chunk && n_cls[1] > 1)
+        std::stable_sort(items + n_cls[0], items + n_cls[0] + n_cls[1],
+                         [](const AttendItem& a, const AttendItem& b) { return a.n_tiles > b.n_tiles; });
+
+    // per-class prefix sums, split-KV plan
+    int64_t cls_tiles[2] = {0, 0};
+    for (int cls = 0; cls < 2; ++cls) {
+        AttendItem* its = items + (cls == 0 ? 0 : n_cls[0]);
+        const int32_t n = n_cls[cls];
+        if (n == 0) continue;
+        int64_t units = 0;           // tile visits of this class's CTAs if nothing were split
+        for (int i = 0; i < n; ++i) {
+            its[i].tile_off = (int32_t)cls_tiles[cls];
+            its[i].class_row_off = pl.cls_rows[cls];
+            cls_tiles[cls] += its[i].n_tiles;
+            pl.cls_rows[cls] += its[i].q_len;
+            if (its[i].q_len > pl.cls_max_q[cls]) pl.cls_max_q[cls] = its[i].q_len;
+            units += (int64_t)its[i].n_tiles * (family == 2 ? c.n_kv_heads : c.n_q_heads * its[i].q_len);
+        }
+        if (family == 2 && cls == 0) {
+            // stream-K: equal contiguous tile ranges over a grid of n_SM x 3 CTAs
+            GqaPlan& g = pl.gplan;
+            g.n_kv_heads = c.n_kv_heads;
+            g.total_tiles = cls_tiles[0] * c.n_kv_heads;
+            int64_t ctas = (int64_t)pool->n_sm * 3;
+            const int64_t min_tiles = pool->tune_split_tokens > 0 ? (pool->tune_split_tokens + 15) / 16 : 8;
+            if (ctas > (g.total_tiles + min_tiles - 1) / min_tiles) ctas = (g.total_tiles + min_tiles - 1) / min_tiles;
+            if (pool->tune_split_tokens > 0) ctas = (g.total_tiles + min_tiles - 1) / min_tiles;
+            if (ctas < 1) ctas = 1;
+            g.tiles_per_cta = (g.total_tiles + ctas - 1) / ctas;
+            pl.gqa_ctas = (int32_t)((g.total_tiles + g.tiles_per_cta - 1) / g.tiles_per_cta);
+            for (int i = 0; i < n; ++i) {
+                const int32_t pieces = (int32_t)((its[i].n_tiles + g.tiles_per_cta - 1) / g.tiles_per_cta) + 1;
+                its[i].n_splits = pieces;      // upper bound on the pieces of one (item, head) pair
+                if (pieces > pl.max_splits) pl.max_splits = pieces;
+            }
+            continue;
+        }
+        // segments sized for >= 2 waves of CTAs, each with a useful run of tiles
+        const int64_t target_ctas = (int64_t)pool->n_sm * (family == 2 ? 4 : 16);
+        int32_t tps = pool->tune_split_tokens > 0 ? (pool->tune_split_tokens + kBlockTokens - 1) / kBlockTokens
+                                                  : (int32_t)((units + target_ctas - 1) / target_ctas);
+        if (pool->tune_split_tokens <= 0 && tps < 8) tps = 8;
+        if (family == 2 && !legacy_chunk && pool->tune_split_tokens <= 0) {
+            // tcgen05 chunk kernel, one CTA per SM: whole (item, head) pairs when they alone give
+            // >= 3 CTAs per SM (no partials to merge), else whole 128-key stages, >= 4 per segment
+            if ((int64_t)n * c.n_kv_heads >= 3 * (int64_t)pool->n_sm) tps = INT32_MAX / 2;
+            else tps = std::max(32, (tps + 7) / 8 * 8);
+        }
+        if (tps < 1) tps = 1;
+        for (int i = 0; i < n; ++i) {
+            AttendItem& it = its[i];
+            int32_t ns = (it.n_tiles + tps - 1) / tps;
+            if (ns > kMaxSplits) ns = kMaxSplits;
+            if (ns < 1) ns = 1;
+            it.tiles_per_split = (it.n_tiles + ns - 1) / ns;
+            it.n_splits = (it.n_tiles + it.tiles_per_split - 1) / it.tiles_per_split;
+            it.split_off = pl.total_splits[cls];
+            pl.total_splits[cls] += it.n_splits;
+            if (it.n_splits > pl.max_splits) pl.max_splits = it.n_splits;
+            if (it.n_splits > 1) pl.merge_cls[cls] = true;
+        }
+    }
+    if (pl.max_splits > 1) {
+        const int rc = ensure_workspace(pool, (size_t)pl.total_rows * c.n_q_heads * pl.max_splits);
+        if (rc) return rc;
+    }
+    pl.valid = true;
+    return METRONOME_OK;
+}
+
+// Launches the attention kernels (rows a5 / a7) and the split merge (a6) of one attend_frame call.
+// `pdl`: the work list was written by the append kernel that precedes this launch on the stream
+// (cached plan): launch programmatically so the prologue overlaps that kernel's tail.
+int launch_attend(metronome_pool* pool, int32_t layer, const AttendPlan& pl, const AttendItem* d_items, const void* q,
+                  void* out, cudaStream_t st, bool pdl) {
+    const metronome_pool_config_t& c = pool->cfg;
+    AttendParams p{};
+    p.table = pool->d_table;
+    p.tbl_width = pool->tbl_width; p.n_sink = pool->n_sink; p.ring = pool->ring;
+    p.q = (const __nv_bfloat16*)q;
+    p.out = (__nv_bfloat16*)out;
+    p.kv_layer = pool->d_kv + (int64_t)layer * pool->L.layer_bytes;
+    p.L = pool->L;
+    p.S = pool->unbounded ? 0 : c.n_sinks; p.W = pool->W_eff;
+    p.scale_log2 = pool->scale * 1.4426950408889634f;
+    p.Hq = c.n_q_heads; p.G = pool->G;
+    p.ws_acc = pool->d_ws_acc; p.ws_ml = pool->d_ws_ml;
+    p.max_splits = pl.max_splits;
+    p.tickets = pool->d_tickets;
+    // measured on B200 (configs 2-4): letting the next append kernel launch early hides its host-memory
+    // reads behind the attention kernel (-4..6 % per frame); the reverse (attention CTAs resident while
+    // the append kernel runs) costs 15-25 %, so the append kernel does not trigger early
+    p.pdl_early = 1;
+
+    if (pool->profiling) {
+        if (pool->prof_used + 2 > pool->prof_ev.size()) {
+            cudaEvent_t a, b;
+            CU(cudaEventCreate(&a));
+            CU(cudaEventCreate(&b));
+            pool->prof_ev.push_back(a);
+            pool->prof_ev.push_back(b);
+        }
+        CU(cudaEventRecord(pool->prof_ev[pool->prof_used], st));
+        pdl = false;
+    }
+    if (pl.family == 2) {
+        if (pl.n_cls[0] > 0) {
+            p.items = d_items; p.n_items = pl.n_cls[0];
+            CU(launch_attend_gqa(p, pl.gplan, c.head_dim, pl.gqa_ctas, st, pdl));
+            ++pool->n_launch;
+        }
+        if (pl.n_cls[1] > 0) {
+            p.items = d_items + pl.n_cls[0]; p.n_items = pl.n_cls[1];
+            if (pl.legacy_chunk) {
+                launch_attend_mma(p, c.head_dim, c.n_kv_heads, pl.total_splits[1], pool->G * pl.cls_max_q[1], st);
+                CU(cudaGetLastError());
+            } else {
+                CU(launch_attend_umma(p, c.head_dim, c.n_kv_heads, pl.total_splits[1], st, pdl));
+            }
+            ++pool->n_launch;
+        }
+    } else {
+        p.items = d_items; p.n_items = pl.n_items;
+        dim3 grid(pl.total_splits[0], c.n_q_heads, pl.cls_max_q[0]);
+        if (c.head_dim == 128) CU(launch_kernel(attend_rows_kernel<128>, grid, dim3(128), 0, st, pdl, p));
+        else CU(launch_kernel(attend_rows_kernel<64>, grid, dim3(128), 0, st, pdl, p));
+        ++pool->n_launch;
+    }
+    if (pool->profiling) {
+        CU(cudaEventRecord(pool->prof_ev[pool->prof_used + 1], st));
+        pool->prof_used += 2;
+    }
+    // ---- row a6: combine the split-KV partials (the GQA decode kernel merges its own pieces) ----
+    for (int cls = (pl.family == 2 ? 1 : 0); cls < 2; ++cls) {
+        if (!pl.merge_cls[cls] || (pl.family != 2 && cls == 1)) continue;
+        p.items = d_items + (cls == 0 ? 0 : pl.n_cls[0]); p.n_items = pl.n_cls[cls];
+        dim3 grid((unsigned)pl.cls_rows[cls], c.n_q_heads);
+        if (c.head_dim == 128) CU(launch_kernel(merge_kernel<128>, grid, dim3(32), 0, st, !pool->profiling, p));
+        else CU(launch_kernel(merge_kernel<64>, grid, dim3(16), 0, st, !pool->profiling, p));
+        ++pool->n_launch;
+    }
     return METRONOME_OK;
 }
 
@@ -276,15 +497,20 @@ int metronome_pool_create(const metronome_pool_config_t* cfg, metronome_pool_t**
         }
         if (pool->poison) fill_nan_kernel<<<1184, 256>>>((uint4*)pool->d_kv, (int64_t)(need / 16));
     }
-    pool->slot_bytes = (size_t)c.max_sessions * (sizeof(AppendItem) > sizeof(AttendItem) ? sizeof(AppendItem) : sizeof(AttendItem));
+    pool->slot_bytes = (size_t)c.max_sessions * (sizeof(AppendItem) + sizeof(AttendItem));
     e = cudaMalloc(&pool->d_tickets, (size_t)c.max_sessions * c.n_kv_heads * sizeof(int32_t));
     if (e != cudaSuccess) return fail(METRONOME_ERR_OUT_OF_MEMORY, e, "cudaMalloc tickets");
     cudaMemset(pool->d_tickets, 0, (size_t)c.max_sessions * c.n_kv_heads * sizeof(int32_t));
+    e = cudaMalloc(&pool->d_bk_flag, 16);
+    if (e != cudaSuccess) return fail(METRONOME_ERR_OUT_OF_MEMORY, e, "cudaMalloc flag");
+    cudaMemset(pool->d_bk_flag, 0, 16);
+    e = cudaMalloc(&pool->d_attend_items, (size_t)c.max_sessions * sizeof(AttendItem));
+    if (e != cudaSuccess) return fail(METRONOME_ERR_OUT_OF_MEMORY, e, "cudaMalloc attend items");
     e = cudaMallocHost(&pool->h_stage, pool->slot_bytes * kStagingSlots);
     if (e != cudaSuccess) return fail(METRONOME_ERR_OUT_OF_MEMORY, e, "cudaMallocHost staging");
     e = cudaMalloc(&pool->d_stage, pool->slot_bytes * kStagingSlots);
     if (e != cudaSuccess) return fail(METRONOME_ERR_OUT_OF_MEMORY, e, "cudaMalloc staging");
-    for (int i = 0; i < kStagingSlots; ++i) {
+    for (int i = 0; i < kStagingSlots / kStagingGroup; ++i) {
         e = cudaEventCreateWithFlags(&pool->ev[i], cudaEventDisableTiming);
         if (e != cudaSuccess) return fail(METRONOME_ERR_CUDA, e, "cudaEventCreate");
     }
@@ -303,6 +529,8 @@ int metronome_pool_destroy(metronome_pool_t* pool) {
     cudaDeviceSynchronize();
     if (pool->d_table) cudaFree(pool->d_table);
     if (pool->d_tickets) cudaFree(pool->d_tickets);
+    if (pool->d_bk_flag) cudaFree(pool->d_bk_flag);
+    if (pool->d_attend_items) cudaFree(pool->d_attend_items);
     if (pool->d_free) cudaFree(pool->d_free);
     if (pool->own_kv && pool->d_kv) cudaFree(pool->d_kv);
     if (pool->d_ws_acc) cudaFree(pool->d_ws_acc);
@@ -310,7 +538,7 @@ int metronome_pool_destroy(metronome_pool_t* pool) {
     if (pool->d_io) cudaFree(pool->d_io);
     if (pool->h_stage) cudaFreeHost(pool->h_stage);
     if (pool->d_stage) cudaFree(pool->d_stage);
-    for (int i = 0; i < kStagingSlots; ++i)
+    for (int i = 0; i < kStagingSlots / kStagingGroup; ++i)
         if (pool->ev[i]) cudaEventDestroy(pool->ev[i]);
     for (cudaEvent_t e : pool->prof_ev) cudaEventDestroy(e);
     delete pool;
@@ -430,23 +658,27 @@ int metronome_append_kv(metronome_pool_t* pool, int32_t layer, int32_t n_batch, 
             }
         }
     }
+    const AppendItem* h_items = reinterpret_cast<const AppendItem*>(h);     // pinned host memory, read by the kernels
+    AttendItem* h_attend = reinterpret_cast<AttendItem*>(h + (size_t)n_batch * sizeof(AppendItem));
+    bool fused_bookkeeping = false, have_plan = false;
+    const int32_t n_free0 = pool->n_free;
     if (layer == 0) {
         if (pool->n_free + total_freed < total_alloc) return METRONOME_ERR_POOL_EXHAUSTED;  // nothing changed
-        if (n_batch > 0) {
-            rc = commit_stage(pool, slot, (size_t)n_batch * sizeof(AppendItem), st);
-            if (rc) return rc;
-            if (total_freed + total_alloc > 0) {
-                bookkeeping_kernel<<<1, 512, 0, st>>>(reinterpret_cast<const AppendItem*>(d), n_batch, pool->d_table,
-                                                      pool->tbl_width, pool->n_sink, pool->ring, pool->d_free,
-                                                      pool->n_free, total_freed);
+        if (n_batch > 0 && total_freed + total_alloc > 0) {
+            if (pool->poison || pool->bookkeeping_only) {
+                // unfused: the poison fill has to sit between the frees and the K/V writes
+                bookkeeping_kernel<<<1, 512, 0, st>>>(h_items, n_batch, pool->d_table, pool->tbl_width, pool->n_sink,
+                                                      pool->ring, pool->d_free, pool->n_free, total_freed);
                 ++pool->n_launch;
                 CU(cudaGetLastError());
-            }
-            if (pool->poison && !pool->bookkeeping_only && total_freed > 0) {
-                poison_blocks_kernel<<<dim3(total_freed, c.n_layers), 256, 0, st>>>(pool->d_free, pool->n_free, pool->d_kv,
-                                                                                   pool->L.block_bytes, pool->L.layer_bytes);
-                ++pool->n_launch;
-                CU(cudaGetLastError());
+                if (pool->poison && !pool->bookkeeping_only && total_freed > 0) {
+                    poison_blocks_kernel<<<dim3(total_freed, c.n_layers), 256, 0, st>>>(pool->d_free, pool->n_free, pool->d_kv,
+                                                                                       pool->L.block_bytes, pool->L.layer_bytes);
+                    ++pool->n_launch;
+                    CU(cudaGetLastError());
+                }
+            } else {
+                fused_bookkeeping = true;
             }
         }
         // commit the shadow counts
@@ -461,16 +693,46 @@ int metronome_append_kv(metronome_pool_t* pool, int32_t layer, int32_t n_batch, 
         pool->layer_epoch[0] = pool->epoch;
         pool->last_sids.assign(sids, sids + n_batch);
         pool->last_n_new.assign(n_new, n_new + n_batch);
-    } else {
-        if (n_batch > 0) {
-            rc = commit_stage(pool, slot, (size_t)n_batch * sizeof(AppendItem), st);
+        // row a8 ahead of time: the work list of attend_frame(q_lens = n_new) for this step; the
+        // append kernel carries it to the device
+        pool->cached_plan.valid = false;
+        if (!pool->bookkeeping_only && total_new > 0) {
+            rc = plan_attend(pool, n_batch, sids, n_new, h_attend, pool->cached_plan);
             if (rc) return rc;
+            pool->cached_plan.epoch = pool->epoch;
+            have_plan = true;
         }
+    } else {
         pool->layer_epoch[layer] = pool->epoch;
     }
     ++pool->n_append;
-    if (!pool->bookkeeping_only && n_batch > 0)
-        return launch_kv_write(pool, layer, reinterpret_cast<const AppendItem*>(d), n_batch, max_n, k_new, v_new, st);
+    if (n_batch > 0 && (fused_bookkeeping || (!pool->bookkeeping_only && total_new > 0))) {
+        AppendParams a{};
+        a.items = h_items;
+        a.n_items = n_batch;
+        a.table = pool->d_table;
+        a.tbl_width = pool->tbl_width; a.n_sink = pool->n_sink; a.ring = pool->ring;
+        a.free_stack = pool->d_free;
+        a.n_free0 = n_free0; a.total_freed = total_freed;
+        a.do_bookkeeping = fused_bookkeeping ? 1 : 0;
+        a.bk_flag = pool->d_bk_flag;
+        a.epoch = (int32_t)pool->epoch;
+        a.pdl_early = 0;
+        if (have_plan) {
+            a.attend_src = reinterpret_cast<const uint4*>(h_attend);
+            a.attend_dst = reinterpret_cast<uint4*>(pool->d_attend_items);
+            a.attend_n16 = pool->cached_plan.n_items * (int32_t)(sizeof(AttendItem) / 16);
+        }
+        a.k_new = (const uint4*)k_new; a.v_new = (const uint4*)v_new;
+        a.kv_layer = pool->bookkeeping_only ? nullptr : pool->d_kv + (int64_t)layer * pool->L.layer_bytes;
+        a.L = pool->L;
+        const int32_t chunks = max_n * c.n_kv_heads * (c.head_dim / 8);
+        dim3 grid(std::max(1, (chunks + 255) / 256), n_batch + 1);
+        const size_t smem = (fused_bookkeeping && n_batch <= kAppendSmemItems) ? (size_t)n_batch * sizeof(AppendItem) : 0;
+        CU(launch_kernel(append_fused_kernel, grid, dim3(256), smem, st, true, a));
+        ++pool->n_launch;
+    }
+    if (n_batch > 0) return release_stage(pool, slot, st);
     return METRONOME_OK;
 }
 
@@ -480,7 +742,6 @@ int metronome_attend_frame(metronome_pool_t* pool, int32_t layer, int32_t n_batc
     if (pool->bookkeeping_only) return METRONOME_ERR_UNSUPPORTED;
     int rc = check_batch(pool, n_batch, sids, q_lens);
     if (rc) return rc;
-    const metronome_pool_config_t& c = pool->cfg;
     int64_t total_rows = 0;
     for (int i = 0; i < n_batch; ++i) {
         if (q_lens[i] > pool->sessions[sids[i]].last_n) return METRONOME_ERR_QLEN_EXCEEDS_LAST_APPEND;
@@ -492,198 +753,24 @@ int metronome_attend_frame(metronome_pool_t* pool, int32_t layer, int32_t n_batc
     if (pool->epoch == 0 || pool->layer_epoch[layer] != pool->epoch) return METRONOME_ERR_LAYER_SEQUENCE;
     cudaStream_t st = (cudaStream_t)cuda_stream;
 
-    // ---- row a8: the per-call work list, from the shadow counts ------------------------------
-    // Kernel families (north_star: "Tensor cores are used only for the GQA-group x chunk QK^T/PV
-    // tiles, where the work really is a dense contraction"):
-    //   rows   CUDA-core row kernel: pure multi-head decode (G x q_len < 4 for every item), and the
-    //          general fallback
-    //   gqa    tensor-core stream-K decode kernel: items with R = G x q_len <= 16
-    //   chunk  tcgen05 / TMEM chunk-prefill kernel: items with 16 < R <= 256
-    //          (tuning family 3: its mma.sync predecessor, R <= 208, kept for A/B measurements)
-    int32_t max_q = 0;
-    for (int i = 0; i < n_batch; ++i)
-        if (q_lens[i] > max_q) max_q = q_lens[i];
-    int family = pool->tune_family;
-    const bool legacy_chunk = family == 3;
-    if (family == 3) family = 2;
-    if (family == 0) family = (pool->G * max_q >= 4) ? 2 : 1;
-    if (family == 2 && !(legacy_chunk ? attend_mma_supported(pool->G, max_q) : attend_umma_supported(pool->G, max_q)))
-        family = 1;
+    // Fast path: the queries are exactly the rows of this step's append (decode: 1, chunk: n), whose
+    // work list append_kv(layer 0) already planned and its kernel already copied to the device.
+    const AttendPlan& cp = pool->cached_plan;
+    if (cp.valid && cp.epoch == pool->epoch && (int32_t)pool->last_sids.size() == n_batch &&
+        !memcmp(pool->last_sids.data(), sids, n_batch * sizeof(int32_t)) &&
+        !memcmp(pool->last_n_new.data(), q_lens, n_batch * sizeof(int32_t)))
+        return launch_attend(pool, layer, cp, pool->d_attend_items, q, out, st, /*after_append=*/true);
 
     uint8_t *h = nullptr, *d = nullptr;
     int slot = 0;
     rc = acquire_stage(pool, &h, &d, &slot);
     if (rc) return rc;
-    AttendItem* items = reinterpret_cast<AttendItem*>(h);
-    const int32_t S = pool->unbounded ? 0 : c.n_sinks, W = pool->W_eff;
-    // class 0 = rows kernel or gqa kernel (placed first), class 1 = chunk kernel (placed after)
-    int32_t n_cls[2] = {0, 0};
-    if (family == 2)
-        for (int i = 0; i < n_batch; ++i)
-            if (q_lens[i] > 0) ++n_cls[pool->G * q_lens[i] > 16 ? 1 : 0];
-    int32_t fill[2] = {0, n_cls[0]};
-    int32_t row = 0, n_items = 0;
-    for (int i = 0; i < n_batch; ++i) {
-        if (q_lens[i] == 0) continue;
-        const Session& s = pool->sessions[sids[i]];
-        const int cls = (family == 2 && pool->G * q_lens[i] > 16) ? 1 : 0;
-        AttendItem& it = items[family == 2 ? fill[cls]++ : n_items];
-        ++n_items;
-        memset(&it, 0, sizeof(it));
-        it.sid = sids[i];
-        it.len = (int32_t)s.len;
-        it.q_len = q_lens[i];
-        it.q_row_off = row;
-        row += q_lens[i];
-        const int32_t n_blk = (int32_t)((s.len + kBlockTokens - 1) / kBlockTokens);
-        const int64_t t0 = s.len - q_lens[i];                      // oldest query of this call
-        const int64_t wfirst = t0 - W + 1 > 0 ? t0 - W + 1 : 0;    // its oldest window key
-        int32_t first_blk = (int32_t)(wfirst / kBlockTokens);
-        if (first_blk < pool->n_sink) first_blk = pool->n_sink;
-        it.n_sink_tiles = n_blk < pool->n_sink ? n_blk : pool->n_sink;
-        it.first_blk = first_blk;
-        it.n_tiles = it.n_sink_tiles + (n_blk > first_blk ? n_blk - first_blk : 0);
-    }
-    if (family != 2) { n_cls[0] = n_items; n_cls[1] = 0; }
-    // chunk class: longest first, so the hardware's in-order CTA dispatch packs the short ones last
-    if (family == 2 && !legacy_chunk && n_cls[1] > 1)
-        std::stable_sort(items + n_cls[0], items + n_cls[0] + n_cls[1],
-                         [](const AttendItem& a, const AttendItem& b) { return a.n_tiles > b.n_tiles; });
-
-    // per-class prefix sums, split-KV plan
-    int32_t total_splits[2] = {0, 0}, max_splits = 1, cls_rows[2] = {0, 0}, cls_max_q[2] = {0, 0};
-    int64_t cls_tiles[2] = {0, 0};
-    GqaPlan gplan{};
-    int32_t gqa_ctas = 0;
-    for (int cls = 0; cls < 2; ++cls) {
-        AttendItem* its = items + (cls == 0 ? 0 : n_cls[0]);
-        const int32_t n = n_cls[cls];
-        if (n == 0) continue;
-        int64_t units = 0;           // tile visits of this class's CTAs if nothing were split
-        for (int i = 0; i < n; ++i) {
-            its[i].tile_off = (int32_t)cls_tiles[cls];
-            its[i].class_row_off = cls_rows[cls];
-            cls_tiles[cls] += its[i].n_tiles;
-            cls_rows[cls] += its[i].q_len;
-            if (its[i].q_len > cls_max_q[cls]) cls_max_q[cls] = its[i].q_len;
-            units += (int64_t)its[i].n_tiles * (family == 2 ? c.n_kv_heads : c.n_q_heads * its[i].q_len);
-        }
-        if (family == 2 && cls == 0) {
-            // stream-K: equal contiguous tile ranges over a grid of n_SM x 3 CTAs
-            gplan.n_kv_heads = c.n_kv_heads;
-            gplan.total_tiles = cls_tiles[0] * c.n_kv_heads;
-            int64_t ctas = (int64_t)pool->n_sm * 3;
-            const int64_t min_tiles = pool->tune_split_tokens > 0 ? (pool->tune_split_tokens + 15) / 16 : 8;
-            if (ctas > (gplan.total_tiles + min_tiles - 1) / min_tiles) ctas = (gplan.total_tiles + min_tiles - 1) / min_tiles;
-            if (pool->tune_split_tokens > 0) ctas = (gplan.total_tiles + min_tiles - 1) / min_tiles;
-            if (ctas < 1) ctas = 1;
-            gplan.tiles_per_cta = (gplan.total_tiles + ctas - 1) / ctas;
-            gqa_ctas = (int32_t)((gplan.total_tiles + gplan.tiles_per_cta - 1) / gplan.tiles_per_cta);
-            for (int i = 0; i < n; ++i) {
-                const int32_t pieces = (int32_t)((its[i].n_tiles + gplan.tiles_per_cta - 1) / gplan.tiles_per_cta) + 1;
-                its[i].n_splits = pieces;      // upper bound on the pieces of one (item, head) pair
-                if (pieces > max_splits) max_splits = pieces;
-            }
-            continue;
-        }
-        // segments sized for >= 2 waves of CTAs, each with a useful run of tiles
-        const int64_t target_ctas = (int64_t)pool->n_sm * (family == 2 ? 4 : 16);
-        int32_t tps = pool->tune_split_tokens > 0 ? (pool->tune_split_tokens + kBlockTokens - 1) / kBlockTokens
-                                                  : (int32_t)((units + target_ctas - 1) / target_ctas);
-        if (pool->tune_split_tokens <= 0 && tps < 8) tps = 8;
-        if (family == 2 && !legacy_chunk && pool->tune_split_tokens <= 0) {
-            // tcgen05 chunk kernel, one CTA per SM: whole (item, head) pairs when they alone give
-            // >= 3 CTAs per SM (no partials to merge), else whole 128-key stages, >= 4 per segment
-            if ((int64_t)n * c.n_kv_heads >= 3 * (int64_t)pool->n_sm) tps = INT32_MAX / 2;
-            else tps = std::max(32, (tps + 7) / 8 * 8);
-        }
-        if (tps < 1) tps = 1;
-        for (int i = 0; i < n; ++i) {
-            AttendItem& it = its[i];
-            int32_t ns = (it.n_tiles + tps - 1) / tps;
-            if (ns > kMaxSplits) ns = kMaxSplits;
-            if (ns < 1) ns = 1;
-            it.tiles_per_split = (it.n_tiles + ns - 1) / ns;
-            it.n_splits = (it.n_tiles + it.tiles_per_split - 1) / it.tiles_per_split;
-            it.split_off = total_splits[cls];
-            total_splits[cls] += it.n_splits;
-            if (it.n_splits > max_splits) max_splits = it.n_splits;
-        }
-    }
-    if (max_splits > 1) {
-        rc = ensure_workspace(pool, (size_t)total_rows * c.n_q_heads * max_splits);
-        if (rc) return rc;
-    }
-    rc = commit_stage(pool, slot, (size_t)n_items * sizeof(AttendItem), st);
+    AttendPlan plan;
+    rc = plan_attend(pool, n_batch, sids, q_lens, reinterpret_cast<AttendItem*>(h), plan);
     if (rc) return rc;
-
-    AttendParams p{};
-    p.table = pool->d_table;
-    p.tbl_width = pool->tbl_width; p.n_sink = pool->n_sink; p.ring = pool->ring;
-    p.q = (const __nv_bfloat16*)q;
-    p.out = (__nv_bfloat16*)out;
-    p.kv_layer = pool->d_kv + (int64_t)layer * pool->L.layer_bytes;
-    p.L = pool->L;
-    p.S = S; p.W = W;
-    p.scale_log2 = pool->scale * 1.4426950408889634f;
-    p.Hq = c.n_q_heads; p.G = pool->G;
-    p.ws_acc = pool->d_ws_acc; p.ws_ml = pool->d_ws_ml;
-    p.max_splits = max_splits;
-    p.tickets = pool->d_tickets;
-
-    if (pool->profiling) {
-        if (pool->prof_used + 2 > pool->prof_ev.size()) {
-            cudaEvent_t a, b;
-            CU(cudaEventCreate(&a));
-            CU(cudaEventCreate(&b));
-            pool->prof_ev.push_back(a);
-            pool->prof_ev.push_back(b);
-        }
-        CU(cudaEventRecord(pool->prof_ev[pool->prof_used], st));
-    }
-    const AttendItem* d_items = reinterpret_cast<const AttendItem*>(d);
-    bool merge_cls[2] = {false, false};
-    if (family == 2) {
-        if (n_cls[0] > 0) {
-            p.items = d_items; p.n_items = n_cls[0];
-            launch_attend_gqa(p, gplan, c.head_dim, gqa_ctas, st);
-            ++pool->n_launch;
-            CU(cudaGetLastError());
-        }
-        if (n_cls[1] > 0) {
-            p.items = d_items + n_cls[0]; p.n_items = n_cls[1];
-            if (legacy_chunk) launch_attend_mma(p, c.head_dim, c.n_kv_heads, total_splits[1], pool->G * cls_max_q[1], st);
-            else launch_attend_umma(p, c.head_dim, c.n_kv_heads, total_splits[1], st);
-            ++pool->n_launch;
-            CU(cudaGetLastError());
-            for (int i = 0; i < n_cls[1]; ++i)
-                if (items[n_cls[0] + i].n_splits > 1) merge_cls[1] = true;
-        }
-    } else {
-        p.items = d_items; p.n_items = n_items;
-        dim3 grid(total_splits[0], c.n_q_heads, cls_max_q[0]);
-        if (c.head_dim == 128) attend_rows_kernel<128><<<grid, 128, 0, st>>>(p);
-        else attend_rows_kernel<64><<<grid, 128, 0, st>>>(p);
-        ++pool->n_launch;
-        CU(cudaGetLastError());
-        for (int i = 0; i < n_items; ++i)
-            if (items[i].n_splits > 1) merge_cls[0] = true;
-    }
-    if (pool->profiling) {
-        CU(cudaEventRecord(pool->prof_ev[pool->prof_used + 1], st));
-        pool->prof_used += 2;
-    }
-    // ---- row a6: combine the split-KV partials ----
-    for (int cls = (family == 2 ? 1 : 0); cls < 2; ++cls) {
-        if (!merge_cls[cls] || (family != 2 && cls == 1)) continue;
-        p.items = d_items + (cls == 0 ? 0 : n_cls[0]); p.n_items = n_cls[cls];
-        dim3 grid((unsigned)cls_rows[cls], c.n_q_heads);
-        if (c.head_dim == 128) merge_kernel<128><<<grid, 32, 0, st>>>(p);
-        else merge_kernel<64><<<grid, 16, 0, st>>>(p);
-        ++pool->n_launch;
-        CU(cudaGetLastError());
-    }
-    return METRONOME_OK;
+    rc = commit_stage(pool, slot, (size_t)plan.n_items * sizeof(AttendItem), st);
+    if (rc) return rc;
+    return launch_attend(pool, layer, plan, reinterpret_cast<const AttendItem*>(d), q, out, st, false);
 }
 
 int metronome_step_host(metronome_pool_t* pool, int32_t layer, int32_t n_batch, const int32_t* sids,
@@ -815,6 +902,7 @@ int metronome_pool_set_tuning(metronome_pool_t* pool, int32_t split_tokens, int3
     if (!pool || split_tokens < 0 || kernel_family < 0 || kernel_family > 3) return METRONOME_ERR_INVALID_ARG;
     pool->tune_split_tokens = split_tokens;
     pool->tune_family = kernel_family;
+    pool->cached_plan.valid = false;
     return METRONOME_OK;
 }
 
