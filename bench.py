@@ -275,6 +275,11 @@ def main():
         frames.append(cur)
     assert len(frames) >= need, (len(frames), need)
 
+    # Sessions that open and close inside the timed frames (config 5, pool churn) need the frames
+    # prepared one at a time (an open needs the slot an earlier frame's close frees): the GPU time of
+    # the K frames is then the sum of K event brackets instead of one.
+    churn = any(ev[0] != "step" for fr in frames for ev in fr)
+
     def prepare(frs):
         """Resolve the frames' steps and generate their inputs in HBM before the timed region."""
         out = []
@@ -283,6 +288,8 @@ def main():
                 if ev[0] == "open":
                     r.open(ev[1]); continue
                 if ev[0] == "close":
+                    if churn:
+                        r.close(ev[1]); continue       # frees the slot a later open of this frame needs
                     out.append(("close", r.sid[ev[1]], ev[1])); continue
                 st = r.make_step(ev)
                 k = r.rows(synth.STREAM_K, 0, st.uid_rows, st.pos_rows)
@@ -324,36 +331,56 @@ def main():
         return frs
 
     # ---- device-resident timing: W warm-up steps, then EXACTLY K timed steps ----
+
+    def run_frames(frs):
+        """-> (prepared items, GPU milliseconds)"""
+        if not churn:
+            prepped = prepare(frs)
+            barrier()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            run(prepped)
+            e1.record()
+            barrier()
+            return prepped, e0.elapsed_time(e1)
+        total, allp = 0.0, []
+        for fr in frs:
+            prepped = prepare([fr])
+            barrier()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            run(prepped)
+            e1.record()
+            barrier()
+            total += e0.elapsed_time(e1)
+            finish_closes(prepped)
+            allp += prepped
+        return allp, total
+
     warm_f, timed_f = take(W), take(K)
-    warm = prepare(warm_f)
-    run(warm)
-    finish_closes(warm)
-    timed = prepare(timed_f)
-    barrier()
+    warm, _ = run_frames(warm_f)
+    if not churn:
+        finish_closes(warm)
     gpu_index = int(os.environ.get("CUDA_VISIBLE_DEVICES", str(LOCAL_RANK)).split(",")[0] or 0)
     sampler = ClockSampler(gpu_index) if RANK == 0 else None
     launches0 = r.pool.stats()["kernel_launches"]
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.nvtx.range_push("metronome_timed")     # lets `ncu --nvtx --nvtx-include` pick this region
-    e0.record()
-    run(timed)
-    e1.record()
+    timed, ms = run_frames(timed_f)
     torch.cuda.nvtx.range_pop()
-    barrier()
-    ms = e0.elapsed_time(e1)
     clocks = sampler.stop() if sampler else None
     launches = r.pool.stats()["kernel_launches"] - launches0
-    finish_closes(timed)
+    if not churn:
+        finish_closes(timed)
     value, ms = replicas.aggregate(ms, session_frames(timed_f), device="cuda")   # max over ranks, sum of frames
 
     # ---- roofline of the dominant kernel: same steps again with the library's event brackets ----
-    prof = prepare(take(K))
     r.pool.set_profiling(True)
-    run(prof)
+    prof, _ = run_frames(take(K))
     torch.cuda.synchronize()
     k_ms, k_n = r.pool.read_profile()
     r.pool.set_profiling(False)
-    finish_closes(prof)
+    if not churn:
+        finish_closes(prof)
     alg_bytes = sum(algorithmic_bytes(w, it[5], it[0].n_new) for it in prof if it[0] != "close")
     n_prof_steps = sum(1 for it in prof if it[0] != "close")
     peak, peak_src = peaks()
@@ -362,7 +389,7 @@ def main():
     tpath = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tpath):
         traffic = json.load(open(tpath)).get(f"config{w.index}")
-    roofline = {"bound": "hbm", "kernel": "attend_rows_kernel<128>" if w.n_q_heads == w.n_kv_heads else "attend_mma_kernel",
+    roofline = {"bound": "hbm", "kernel": "attend_rows_kernel<128>" if w.n_q_heads == w.n_kv_heads else "attend_gqa_kernel (decode) + attend_umma_kernel (chunk)",
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes / max(k_n, 1),
                 "kernel_ms_avg": k_ms / max(k_n, 1), "kernel_share_of_step": k_ms / ms if ms > 0 else None,
@@ -370,7 +397,7 @@ def main():
 
     # ---- end to end: HOST buffers through metronome_step_host, copies inside the timed region ----
     e2e = None
-    if not args.no_e2e:
+    if not args.no_e2e and not churn:       # (config 5 is a latency sweep workload: no host arm)
         def to_host(prepped):
             out = []
             for item in prepped:
