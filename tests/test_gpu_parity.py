@@ -273,3 +273,58 @@ def test_spike_keys_at_every_mask_boundary_on_device(family):
     assert run(S - 1)[0] > 990.0                                           # last sink: IN
     assert run(S)[0] == 0.0                                                # first non-sink, far behind: OUT
     assert run(t)[0] > 990.0                                               # the query's own key: IN
+
+
+def test_attend_on_a_reordered_subset_with_shorter_queries():
+    """attend_frame need not repeat the append's batch: a reordered subset of the sessions, with
+    q_len <= the rows just appended (reading R15), takes the library's general path (work list built
+    and uploaded by attend_frame itself instead of the one planned at append time)."""
+    from paper_2607_02640_b200.runner import Step
+    w = wl.make_workload(3, n_sessions=5)
+    for family in (1, 2):
+        r = Runner(w)
+        r.pool.set_tuning(0, family)
+        m = OracleMirror(r, paged=False)
+        for i in range(5):
+            r.open(i); m.open(i)
+        rng = np.random.default_rng(3)
+        for step in range(30):
+            n_new = np.array([int(rng.integers(2, 26)) for _ in range(5)], np.int32)
+            st = r.make_step(("step", np.arange(5, dtype=np.int32), n_new, True, step))
+            r.append(st, 0); m.append(st, 0)
+            keep = rng.permutation(5)[: int(rng.integers(1, 5))]
+            q_lens = np.array([int(rng.integers(1, n_new[i] + 1)) for i in keep], np.int32)
+            uid = np.repeat(np.asarray([r.uid[int(i)] for i in keep], np.int64), q_lens)
+            pos = np.concatenate([np.arange(r.length[int(i)] - int(n), r.length[int(i)], dtype=np.int64)
+                                  for i, n in zip(keep, q_lens)])
+            sub = Step(keep.astype(np.int32), np.asarray([r.sid[int(i)] for i in keep], np.int32), q_lens, uid, pos,
+                       True, step)
+            assert_parity(r.attend(sub, 0), m.attend(sub, 0), f"subset step {step} keep={keep} q={q_lens}")
+    _loaded_native()
+
+
+def test_bookkeeping_with_more_sessions_than_the_kernel_stages():
+    """> 1024 sessions in one append call: the fused append kernel's bookkeeping CTA reads the batch
+    from memory instead of its shared-memory copy; tables and free list stay bit-exact."""
+    n = 1500
+    pool = binding.Pool(n_q_heads=2, n_kv_heads=1, head_dim=64, n_sinks=4, window=32, n_blocks=n * 5, max_sessions=n,
+                        max_new_tokens=16)
+    cfg = O.PoolConfig(n_q_heads=2, n_kv_heads=1, head_dim=64, S=4, W=32, n_blocks=n * 5, block_size=16,
+                       max_sessions=n, max_new_tokens=16)
+    ora = O.PagedOracle(cfg)
+    sids = [pool.session_open() for _ in range(n)]
+    assert sids == [ora.session_open() for _ in range(n)]
+    rng = np.random.default_rng(5)
+    for step in range(8):
+        n_new = rng.integers(0, 17, size=n).astype(np.int32)
+        rows = int(n_new.sum())
+        k = torch.zeros(rows, 1, 64, dtype=torch.bfloat16, device="cuda")
+        pool.append_kv(0, sids, n_new, k, k)
+        kz = np.zeros((rows, 1, 64), np.uint16)
+        ora.append_kv(0, sids, [int(x) for x in n_new], kz, kz)
+    n_free, ids = pool.pool_query()
+    assert ids == ora.pool_query()
+    for s in sids[::37]:
+        got, want = pool.session_query(s), ora.session_query(s)
+        assert (got[0], got[1], list(got[2])) == (want[0], want[1], list(want[2]))
+    _loaded_native()
