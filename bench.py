@@ -332,28 +332,25 @@ def main():
 
     # ---- device-resident timing: W warm-up steps, then EXACTLY K timed steps ----
 
-    def run_frames(frs):
-        """-> (prepared items, GPU milliseconds)"""
-        if not churn:
-            prepped = prepare(frs)
-            barrier()
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record()
-            run(prepped)
-            e1.record()
-            barrier()
-            return prepped, e0.elapsed_time(e1)
+    def run_frames(frs, nvtx=None):
+        """-> (prepared items, GPU milliseconds).  `nvtx` names the range around the library calls
+        only (input generation stays outside), so `ncu --nvtx --nvtx-include` lists just our kernels."""
         total, allp = 0.0, []
-        for fr in frs:
-            prepped = prepare([fr])
+        for group in ([[fr] for fr in frs] if churn else [frs]):
+            prepped = prepare(group)
             barrier()
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            if nvtx:
+                torch.cuda.nvtx.range_push(nvtx)
             e0.record()
             run(prepped)
             e1.record()
+            if nvtx:
+                torch.cuda.nvtx.range_pop()
             barrier()
             total += e0.elapsed_time(e1)
-            finish_closes(prepped)
+            if churn:
+                finish_closes(prepped)
             allp += prepped
         return allp, total
 
@@ -364,9 +361,7 @@ def main():
     gpu_index = int(os.environ.get("CUDA_VISIBLE_DEVICES", str(LOCAL_RANK)).split(",")[0] or 0)
     sampler = ClockSampler(gpu_index) if RANK == 0 else None
     launches0 = r.pool.stats()["kernel_launches"]
-    torch.cuda.nvtx.range_push("metronome_timed")     # lets `ncu --nvtx --nvtx-include` pick this region
-    timed, ms = run_frames(timed_f)
-    torch.cuda.nvtx.range_pop()
+    timed, ms = run_frames(timed_f, nvtx="metronome_timed")
     clocks = sampler.stop() if sampler else None
     launches = r.pool.stats()["kernel_launches"] - launches0
     if not churn:
@@ -388,7 +383,8 @@ def main():
     traffic = None
     tpath = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tpath):
-        traffic = json.load(open(tpath)).get(f"config{w.index}")
+        tj = json.load(open(tpath))
+        traffic = tj.get(f"config{w.index}", tj.get(f"config{w.index}_decode"))
     roofline = {"bound": "hbm", "kernel": "attend_rows_kernel<128>" if w.n_q_heads == w.n_kv_heads else "attend_gqa_kernel (decode) + attend_umma_kernel (chunk)",
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes / max(k_n, 1),
