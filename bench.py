@@ -48,7 +48,7 @@ def parse():
     ap.add_argument("--split-tokens", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--sweep", default="", choices=["", "age", "sessions", "sw"],
+    ap.add_argument("--sweep", default="", choices=["", "age", "sessions", "sw", "occupancy"],
                     help="shape checks of SURVEY sec. 8(d)/(f) instead of the bench line: one JSON line per point")
     return ap.parse_args()
 
@@ -244,6 +244,8 @@ def main():
             rows = sweeps.age_sweep(args.config, n_sessions=args.sessions or None)
         elif args.sweep == "sessions":
             rows = sweeps.sessions_sweep(history_scale=args.history_scale)
+        elif args.sweep == "occupancy":
+            rows = sweeps.occupancy_trace(n_sessions=args.sessions or 128)
         else:
             rows = sweeps.sw_sweep(n_sessions=args.sessions or 128)
         for row in rows:

@@ -821,7 +821,11 @@ int metronome_session_query(metronome_pool_t* pool, int32_t sid, void* cuda_stre
     const int32_t n_sink_res = n_blk < pool->n_sink ? n_blk : pool->n_sink;
     const int32_t n_win = n_blk > s.first_live ? n_blk - s.first_live : 0;
     if (len) *len = s.len;
-    if (first_live_block) *first_live_block = s.first_live;
+    // the unbounded arm pins nothing internally (nothing is ever freed), but reports the same
+    // "first non-sink block" = ceil(S / block) as the bounded rule of session_open (SURVEY 8(c) rule 2)
+    if (first_live_block)
+        *first_live_block = pool->unbounded ? (pool->cfg.n_sinks + pool->cfg.block_size - 1) / pool->cfg.block_size
+                                            : s.first_live;
     if (n_blocks) *n_blocks = n_sink_res + n_win;
     if (block_ids && n_sink_res + n_win > 0) {
         std::vector<int32_t> rowbuf(pool->tbl_width);

@@ -30,14 +30,15 @@ class Step:
 
 class Runner:
     def __init__(self, w: Workload, n_layers: int = 1, flags: int = 0, device: str = "cuda",
-                 softmax_scale: float = 0.0, uid_base: int = 0):
+                 softmax_scale: float = 0.0, uid_base: int = 0, max_session_len: int = 0):
         self.w = w
         self.n_layers = n_layers
         self.device = torch.device(device)
         self.pool = binding.Pool(n_q_heads=w.n_q_heads, n_kv_heads=w.n_kv_heads, head_dim=w.head_dim,
                                  n_sinks=w.S, window=w.W, n_blocks=w.n_blocks, max_sessions=w.slots,
                                  max_new_tokens=w.max_new_tokens, n_layers=n_layers,
-                                 block_size=w.block_size, softmax_scale=softmax_scale, flags=flags)
+                                 block_size=w.block_size, softmax_scale=softmax_scale, flags=flags,
+                                 max_session_len=max_session_len)
         self.sid = {}            # local index -> library sid
         self.uid = {}            # local index -> unique session uid (fresh on every open)
         self.length = {}         # local index -> tokens so far

@@ -4,6 +4,10 @@
             latency must rise up to a ~ S+W and then stay FLAT ("O(W)")
   sessions  config 5 (pool churn): n_target in {32 .. 512}; median / p99 per-frame latency must be
             monotone non-decreasing in the load with zero pool exhaustion
+  occupancy NEXT row f2: the unbounded arm (METRONOME_FLAG_UNBOUNDED) against the windowed one on the
+            same pool and traffic: occupancy rho(t) = rho0 + N r t until POOL_EXHAUSTED at
+            t_sat = (1 - rho0) / (N r) (Eq. 1, L83 Fig. 5) vs. the windowed plateau
+            rho0 + N s(W)
   sw        NEXT row f1: W in {256 .. 4096} and S in {0, 16, 32, 64} at N = 128 (PAPER.md:L300
             Fig. 11, L308-323 Table 2 "sinks ... unchanged latency")
 
@@ -152,6 +156,64 @@ def sw_sweep(n_sessions: int = 128, n_frames: int = 12, windows=(256, 512, 1024,
         fr = time_frames(r, rest)
         rows.append({"sweep": "sw", "sessions": n_sessions, "S": S, "W": W,
                      "blocks_per_session": wl.blocks_per_session(S, W, 16, base.max_new_tokens), **_summary(fr)})
+        del r
+        torch.cuda.empty_cache()
+    return rows
+
+
+def occupancy_trace(n_sessions: int = 128, n_frames: int = 200):
+    """NEXT f2 on config-3 shapes: N sessions, every frame appends 25 + 8 x 1 tokens (r = 33 tokens per
+    session and frame), pool = 2 x N x the windowed per-session cap.  Unbounded arm: runs until the library
+    returns POOL_EXHAUSTED and compares that frame with Eq. 1's closed form (a block is held from its
+    first token, hence the ceil).  Windowed arm: same traffic, 3 x longer, plateau.  Occupancy is read
+    from the device free list after every frame (metronome_pool_query)."""
+    from . import binding
+    base = wl.make_workload(3, n_sessions=n_sessions)
+    frame = _frame_pattern(base)
+    r_tok = sum(frame)
+    rows = []
+    for arm in ("unbounded", "windowed"):
+        flags = binding.FLAG_UNBOUNDED if arm == "unbounded" else 0
+        w = replace(base, n_blocks=2 * base.n_blocks)
+        r = Runner(w, flags=flags, max_session_len=(n_frames + 2) * r_tok if arm == "unbounded" else 0)
+        for i in range(n_sessions):
+            r.open(i)
+        trace, exhausted_at = [], None
+        for f in range(n_frames):
+            try:
+                for n in frame:
+                    st = r.make_step(("step", np.arange(n_sessions, dtype=np.int32), np.full(n_sessions, n, np.int32), True, f))
+                    r.append(st, 0)
+                    r.attend(st, 0)
+            except binding.MetronomeError as e:
+                assert "POOL_EXHAUSTED" in str(e), e
+                exhausted_at = f
+                break
+            trace.append(1.0 - r.pool.pool_query(want_ids=False)[0] / w.n_blocks)
+        # Eq. 1 with r in blocks per frame: the frame in which ceil(L/16) summed over sessions first
+        # exceeds the pool (all sessions are in lockstep, so per session: ceil(L/16) > n_blocks / N)
+        per_session = w.n_blocks // n_sessions
+        t_sat = None
+        if arm == "unbounded":
+            L, t = 0, 0
+            while True:
+                ok = True
+                for n in frame:
+                    if -(-(L + n) // 16) > per_session:
+                        ok = False
+                        break
+                    L += n
+                if not ok:
+                    break
+                t += 1
+            t_sat = t
+        slope = float(np.polyfit(np.arange(len(trace[:20])), trace[:20], 1)[0]) if len(trace) >= 20 else None
+        rows.append({"sweep": "occupancy", "arm": arm, "sessions": n_sessions, "pool_blocks": w.n_blocks,
+                     "tokens_per_session_frame": r_tok, "frames_run": len(trace), "pool_exhausted_at_frame": exhausted_at,
+                     "eq1_t_sat_frame": t_sat, "eq1_slope_per_frame": n_sessions * r_tok / 16 / w.n_blocks,
+                     "fit_slope_first_20_frames": slope, "occupancy_end": trace[-1] if trace else None,
+                     "occupancy_max": max(trace) if trace else None,
+                     "occupancy_every_10th_frame": [round(x, 4) for x in trace[::10]]})
         del r
         torch.cuda.empty_cache()
     return rows

@@ -328,3 +328,38 @@ def test_bookkeeping_with_more_sessions_than_the_kernel_stages():
         got, want = pool.session_query(s), ora.session_query(s)
         assert (got[0], got[1], list(got[2])) == (want[0], want[1], list(want[2]))
     _loaded_native()
+
+
+def test_unbounded_arm_matches_the_oracle_until_the_pool_is_exhausted():
+    """NEXT f2 (Eq. 1): METRONOME_FLAG_UNBOUNDED keeps every block (W = infinity, nothing
+    pinned, nothing freed): attention = plain causal attention over the whole history, occupancy grows
+    linearly, and the append that does not fit returns POOL_EXHAUSTED with nothing changed."""
+    from dataclasses import replace
+    w = replace(wl.make_workload(1), n_blocks=4 * 9)
+    for family in (1, 2):
+        r = Runner(w, flags=binding.FLAG_UNBOUNDED, max_session_len=4096)
+        r.pool.set_tuning(0, family)
+        m = OracleMirror(r, unbounded=True)
+        for i in range(4):
+            r.open(i); m.open(i)
+        exhausted = False
+        for step in range(40):
+            n_new = np.array([8, 1, 5, 3], np.int32)
+            ev = ("step", np.arange(4, dtype=np.int32), n_new, True, step)
+            lengths = dict(r.length)
+            st = r.make_step(ev)
+            try:
+                r.append(st, 0)
+            except binding.MetronomeError as e:
+                assert e.code == "POOL_EXHAUSTED"
+                with pytest.raises(O.OracleError):
+                    m.append(st, 0)
+                r.length.update(lengths)
+                exhausted = True
+                break
+            m.append(st, 0)
+            assert_parity(r.attend(st, 0), m.attend(st, 0), f"unbounded step {step}")
+            m.check_tables(r.pool)
+        assert exhausted
+        m.check_tables(r.pool)
+    _loaded_native()
