@@ -4,32 +4,30 @@
 // The R = G x q_len query rows that share one KV head ("grouped-query attention",
 // "mixed prefill/decode"; L46 "prefill the new chunk") are a real dense contraction against the
 // session's sink + window keys: S = Q K^T and O = P V with M = 128-row tiles.  One CTA owns one
-// (item, KV head, split-KV segment) and streams its KV ONCE from HBM in stages of 8 blocks
-// (128 keys):
+// (item, KV head, split-KV segment) and streams its KV ONCE from HBM in half-stages of 4 blocks
+// (64 keys):
 //
-//   warp 0      producer: per stage, bulk copies of the K tiles (one 2 KB copy per 64-dim half, so
-//               the halves of 8 blocks form one UMMA K-major operand) and of the V tiles (4 KB each;
-//               a V tile as laid out in HBM already IS a SWIZZLE_128B MN-major operand of one
-//               K=16 MMA), into a 5-deep ring of 32 KB buffers, mbarrier complete_tx
-//   warp 1      MMA issuer (one elected lane) + TMEM allocator:
-//                 S_s = Q_s K_j^T   (SS form, D/16 instructions 128x128x16)  -> TMEM, fp32
-//                 O_s += P_s V_j    (TS form: P is read from TMEM, V from shared memory)
-//               completion is signalled with tcgen05.commit on mbarriers
-//   warps 2-5   softmax warpgroup of slot 0, warps 6-9 of slot 1: ONE THREAD PER QUERY ROW
-//               (tcgen05.ld 32x32b): token-exact union mask on boundary stages, row max and row sum
-//               without any shuffle, exp2 in the log2 domain, P split into bf16 hi + lo and written back to
-//               TMEM over S (tcgen05.st), lazy rescale of O (only when the max moved by > 2^8)
+//   warp 0      producer: per half-stage, bulk copies of the K tiles (one 2 KB copy per 64-dim half,
+//               so the halves of 4 blocks form one UMMA K-major operand) and of the V tiles (a V
+//               tile as laid out in HBM already IS a SWIZZLE_128B MN-major operand of one K=16
+//               MMA), into a ring of 16 KB buffers, mbarrier complete_tx
+//   warps 1, 2  MMA issuers, one per slot (warp 1 also allocates TMEM); per half-stage h:
+//                 S = Q K_h^T   (SS form, D/16 instructions 128x64x16)   -> one of TWO S buffers
+//                 O += P_h V_h  (TS form: P read from TMEM, V from shared memory; hi and lo parts)
+//               S is double buffered, so Q K^T of half-stage h+1 is issued BEFORE P V of h: the
+//               softmax warps never wait for the tensor pipe in steady state
+//   warps 4-7   softmax warpgroup of slot 0, warps 8-11 of slot 1: ONE THREAD PER QUERY ROW
+//               (tcgen05.ld 32x32b, 64 scores in registers): token-exact union mask on boundary
+//               half-stages, row max and row sum without any shuffle, exp2 in the log2 domain, P split
+//               into bf16 hi + lo and written back over the S buffer (tcgen05.st), lazy rescale of
+//               O (only when the max moved by > 2^8, after the previous P V has completed)
 //
-// Two slots (S, P and O regions in TMEM: 2 x (128 + D) columns of the 512) ping-pong so the tensor
-// pipe, the MUFU pipe and the copy engine overlap:
-//   R > 128  : slot s = rows [128 s, 128 s + 128), both slots see every key stage
-//   R <= 128 : both slots hold the same rows; slot s takes key stages j = s (mod 2); the two
+// Two slots (TMEM: 2 x (2 x 64 S/P + D O) columns of the 512):
+//   R > 128  : slot s = rows [128 s, 128 s + 128), both slots see every half-stage
+//   R <= 128 : both slots hold the same rows; slot s takes half-stages h = s (mod 2); the two
 //              partial (O, m, l) are merged through shared memory at the end
 // Sinks go first, in segment 0 only; a single segment writes the final bf16 output,
 // several write unnormalised partials for merge_kernel (row a6).
-//
-// Roofline: at R = 200 (config 3) the step is ~200 flop/byte against a ridge of ~250: HBM-bound
-// with the tensor pipe ~70 % busy; the mma.sync predecessor (attend_mma_kernel) was 7x off.
 #pragma once
 #include "attend_mma.cuh"
 
@@ -51,19 +49,20 @@ __device__ int g_trace_cta = 0;
 
 template <int D>
 struct UmmaCfg {
-    static constexpr int KS = 8;                          // KV blocks per stage (128 keys)
-    static constexpr int NBUF = 5;                        // ring buffers (each one K or one V stage)
+    static constexpr int KS = 4;                          // KV blocks per half-stage (64 keys)
     static constexpr int NH = D / 64;                     // 64-dim halves (128-byte swizzle span)
     static constexpr int kTileBytes = kBlockTokens * D * 2;   // K or V of one (block, head)
-    static constexpr int kBufBytes = KS * kTileBytes;     // 32 KB at D = 128
-    static constexpr int kHalfBytes = 128 * 128;          // [128 rows or keys][64 dims]
+    static constexpr int kBufBytes = KS * kTileBytes;     // 16 KB at D = 128: one K or one V half-stage
+    static constexpr int kKHalfBytes = KS * kBlockTokens * 128;   // [64 keys][64 dims]
+    static constexpr int kQHalfBytes = 128 * 128;         // [128 rows][64 dims]
     static constexpr int kQBytes = 128 * D * 2;           // Q rows of one slot
+    static constexpr int NBUF = D == 128 ? 10 : 12;       // ring buffers
     static constexpr int kBarOff = 2 * kQBytes + NBUF * kBufBytes;
-    static constexpr int kMlOff = kBarOff + 256;          // (m, l) of slot 1 for the in-CTA merge
+    static constexpr int kMlOff = kBarOff + 512;          // (m, l) of slot 1 for the in-CTA merge
     static constexpr int kSmemBytes = kMlOff + 1024 + 1024;   // + alignment slack
-    static constexpr int kThreads = 320;
+    static constexpr int kThreads = 384;
     static constexpr int kTmemCols = 512;
-    static constexpr int kColS = 0, kColO = 256;          // S_s at 128 s; O_s at 256 + D s
+    static constexpr int kColS = 0, kColO = 256;          // S buffers of slot s at 128 s + {0, 64}; O_s at 256 + D s
     static_assert(kSmemBytes <= 232448, "shared memory budget");
 };
 
@@ -128,18 +127,41 @@ __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t* r) {
                    "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
                  : "memory");
 }
+// packed fp32 x 2 arithmetic (sm_100: FFMA2 / FADD2): half the issue slots of the softmax inner loop
+__device__ __forceinline__ uint64_t f2_pack(float lo, float hi) {
+    uint64_t r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void f2_unpack(uint64_t v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ uint64_t f2_fma(uint64_t a, uint64_t b, uint64_t c) {
+    uint64_t d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ uint64_t f2_add(uint64_t a, uint64_t b) {
+    uint64_t d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ uint64_t f2_sub(uint64_t a, uint64_t b) {
+    uint64_t d;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
 __device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 
-// Order in which the ring is filled and drained (producer and MMA warp agree on it):
-//   two row tiles : K0 V0 K1 V1 ...            (S_0, S_1 of stage j+1 are issued around P V of stage j)
-//   one row tile  : K0 K1 V0 K2 V1 ... V(n-1)  (slots alternate stages, so K is needed one stage ahead)
-__device__ __forceinline__ int32_t umma_entry_k(bool two, int32_t j) { return two ? 2 * j : (j == 0 ? 0 : 2 * j - 1); }
-__device__ __forceinline__ int32_t umma_entry_v(bool two, int32_t j, int32_t n) {
-    return two ? 2 * j + 1 : (j == n - 1 ? 2 * n - 1 : 2 * j + 2);
-}
 
-// grid = (Hkv, total segments of the chunk-class items), block = 320, one CTA per SM
+// Order in which the ring is filled and drained.  Each slot runs Q K^T one half-stage ahead of P V:
+//   R > 128  (both slots consume every entry): K0 K1 V0 K2 V1 ... K(n-1) V(n-2) V(n-1)
+//   R <= 128 (slot s consumes half-stages h = s mod 2): the same order over PAIRS (2j, 2j+1), each
+//            pair entry expanded into its two half-stages; a missing last half-stage is a phantom
+//            entry (no bytes) so that the indices stay closed-form
+__device__ __forceinline__ int32_t umma_seq_k(int32_t j) { return j == 0 ? 0 : 2 * j - 1; }
+__device__ __forceinline__ int32_t umma_seq_v(int32_t j, int32_t n) { return j == n - 1 ? 2 * n - 1 : 2 * j + 2; }
+
+// grid = (Hkv, total segments of the chunk-class items), block = 384, one CTA per SM
 template <int D>
 __global__ void __launch_bounds__(UmmaCfg<D>::kThreads, 1)
 attend_umma_kernel(AttendParams p) {
@@ -152,10 +174,11 @@ attend_umma_kernel(AttendParams p) {
     const uint32_t sQ = base, sRing = base + 2 * C::kQBytes, sBar = base + C::kBarOff;
     auto bar_full = [&](int b) { return sBar + 8u * b; };
     auto bar_empty = [&](int b) { return sBar + 8u * (C::NBUF + b); };
-    auto bar_s = [&](int s) { return sBar + 8u * (2 * C::NBUF + s); };          // S_s ready   (MMA -> softmax)
-    auto bar_p = [&](int s) { return sBar + 8u * (2 * C::NBUF + 2 + s); };      // P_s written (softmax -> MMA)
-    auto bar_o = [&](int s) { return sBar + 8u * (2 * C::NBUF + 4 + s); };      // last P V of slot s done
-    volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(gen + C::kBarOff + 2 * 8 * C::NBUF + 6 * 8);
+    auto bar_s = [&](int s, int buf) { return sBar + 8u * (2 * C::NBUF + 2 * s + buf); };       // S ready  (MMA -> softmax)
+    auto bar_p = [&](int s, int buf) { return sBar + 8u * (2 * C::NBUF + 4 + 2 * s + buf); };   // P written (softmax -> MMA)
+    auto bar_pv = [&](int s) { return sBar + 8u * (2 * C::NBUF + 8 + s); };                     // P V of a half-stage done
+    auto bar_o = [&](int s) { return sBar + 8u * (2 * C::NBUF + 10 + s); };                     // last P V of slot s done
+    volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(gen + C::kBarOff + 8 * (2 * C::NBUF + 12));
 
     const int32_t kvh = blockIdx.x;
     const int32_t i = find_item(p.n_items, (int32_t)blockIdx.y, [&](int32_t k) { return p.items[k].split_off; });
@@ -166,31 +189,46 @@ attend_umma_kernel(AttendParams p) {
     const bool two = R > 128;
     const int32_t tl0 = split * it.tiles_per_split;
     const int32_t tl1 = min(it.n_tiles, tl0 + it.tiles_per_split);
-    const int32_t n_stage = (tl1 - tl0 + C::KS - 1) / C::KS;
+    const int32_t n_half = (tl1 - tl0 + C::KS - 1) / C::KS;             // half-stages of this segment
+    const int32_t n_pair = (n_half + 1) >> 1;
     const int32_t t_first = it.len - it.q_len;                          // reading R15: the last q_len positions
+    // ring entry of K / V of half-stage h (see umma_seq_k / umma_seq_v)
+    auto entry_k = [&](int32_t h) { return two ? umma_seq_k(h) : 2 * umma_seq_k(h >> 1) + (h & 1); };
+    auto entry_v = [&](int32_t h) { return two ? umma_seq_v(h, n_half) : 2 * umma_seq_v(h >> 1, n_pair) + (h & 1); };
 
     if (warp == 0) {
         // ================================ producer ================================
         if (lane == 0) {
-            for (int b = 0; b < C::NBUF; ++b) { mbar_init(bar_full(b), 1); mbar_init(bar_empty(b), 1); }
-            for (int s = 0; s < 2; ++s) { mbar_init(bar_s(s), 1); mbar_init(bar_p(s), 4); mbar_init(bar_o(s), 1); }
+            for (int b = 0; b < C::NBUF; ++b) { mbar_init(bar_full(b), 1); mbar_init(bar_empty(b), two ? 2 : 1); }
+            for (int s = 0; s < 2; ++s) {
+                for (int buf = 0; buf < 2; ++buf) { mbar_init(bar_s(s, buf), 1); mbar_init(bar_p(s, buf), 4); }
+                mbar_init(bar_pv(s), 1);
+                mbar_init(bar_o(s), 1);
+            }
             asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         }
         __syncwarp();
         named_arrive(1, C::kThreads);
         const int32_t* trow = p.table + (int64_t)it.sid * p.tbl_width;
         const uint8_t* head_base = p.kv_layer + (int64_t)kvh * p.L.head_bytes;
-        for (int32_t e = 0; e < 2 * n_stage; ++e) {
+        const int32_t n_entries = two ? 2 * n_half : 4 * n_pair;
+        for (int32_t e = 0; e < n_entries; ++e) {
+            // invert the order: which (K | V, half-stage) is entry e
+            const int32_t es = two ? e : e >> 1, ns = two ? n_half : n_pair;
             bool is_v;
             int32_t j;
-            if (two) { is_v = e & 1; j = e >> 1; }
-            else if (e == 0) { is_v = false; j = 0; }
-            else if (e == 2 * n_stage - 1) { is_v = true; j = n_stage - 1; }
-            else if (e & 1) { is_v = false; j = (e + 1) >> 1; }
-            else { is_v = true; j = (e >> 1) - 1; }
+            if (es == 0) { is_v = false; j = 0; }
+            else if (es == 2 * ns - 1) { is_v = true; j = ns - 1; }
+            else if (es & 1) { is_v = false; j = (es + 1) >> 1; }
+            else { is_v = true; j = (es >> 1) - 1; }
+            const int32_t h = two ? j : 2 * j + (e & 1);
             const int32_t b = e % C::NBUF, k = e / C::NBUF;
             if (k >= 1) mbar_wait(bar_empty(b), (k - 1) & 1);
-            const int32_t t0 = tl0 + j * C::KS;
+            if (h >= n_half) {                                        // phantom half-stage of an odd count
+                if (lane == 0) mbar_arrive(bar_full(b));
+                continue;
+            }
+            const int32_t t0 = tl0 + h * C::KS;
             const int32_t nt = min(C::KS, tl1 - t0);
             if (lane == 0) mbar_expect_tx(bar_full(b), (uint32_t)nt * C::kTileBytes);
             __syncwarp();
@@ -202,57 +240,65 @@ attend_umma_kernel(AttendParams p) {
                              C::kTileBytes, bar_full(b));
                 }
             } else if (lane < nt * C::NH) {
-                const int32_t blk = lane / C::NH, h = lane % C::NH;
+                const int32_t blk = lane / C::NH, hh = lane % C::NH;
                 const int32_t phys = __ldg(trow + table_slot(tile_block(it, t0 + blk), p.n_sink, p.ring));
-                bulk_g2s(dst + h * C::kHalfBytes + blk * 2048, head_base + (int64_t)phys * p.L.block_bytes + h * 2048, 2048,
+                bulk_g2s(dst + hh * C::kKHalfBytes + blk * 2048, head_base + (int64_t)phys * p.L.block_bytes + hh * 2048, 2048,
                          bar_full(b));
             }
         }
         return;
     }
+    if (warp == 3) {                                                  // spare warp of the first warpgroup
+        named_arrive(1, C::kThreads);
+        return;
+    }
 
-    if (warp == 1) {
-        // ================================ MMA issuer ================================
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;"
-                     ::"r"(smem_u32(const_cast<uint32_t*>(tmem_slot))), "r"(C::kTmemCols));
-        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    if (warp == 1 || warp == 2) {
+        // ================================ MMA issuer of slot `slot` ================================
+        const int32_t slot = warp - 1;
+        if (warp == 1) {
+            asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;"
+                         ::"r"(smem_u32(const_cast<uint32_t*>(tmem_slot))), "r"(C::kTmemCols));
+            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+        }
         tc_fence_before();
         named_sync(1, C::kThreads);
         tc_fence_after();
         const uint32_t tmem = *tmem_slot;
-        constexpr uint32_t idesc_qk = umma_idesc(128, false);
+        constexpr uint32_t idesc_qk = umma_idesc(C::KS * kBlockTokens, false);
         constexpr uint32_t idesc_pv = umma_idesc(D, true);
+        const uint32_t tSbase = tmem + C::kColS + 128 * slot, tOacc = tmem + C::kColO + D * slot;
+        const uint32_t qb = sQ + (two ? slot : 0) * C::kQBytes;
 
         auto wait_full = [&](int32_t e) {
             mbar_wait(bar_full(e % C::NBUF), (e / C::NBUF) & 1);
             tc_fence_after();
         };
         auto release = [&](int32_t e) { if (lane == 0) umma_commit(bar_empty(e % C::NBUF)); };
-        // S_slot = Q_qslot K^T over the K stage in ring entry e
-        auto issue_qk = [&](int32_t slot, int32_t qslot, int32_t e) {
+        // S[buf] = Q K^T over the K half-stage in ring entry e
+        auto issue_qk = [&](int32_t buf, int32_t e) {
             if (lane == 0) {
-                const uint32_t kb = sRing + (e % C::NBUF) * C::kBufBytes, qb = sQ + qslot * C::kQBytes;
+                const uint32_t kb = sRing + (e % C::NBUF) * C::kBufBytes;
 #pragma unroll
-                for (int kk = 0; kk < D / 16; ++kk) {
-                    const uint32_t off = (kk >> 2) * C::kHalfBytes + (kk & 3) * 32;
-                    umma_ss(tmem + C::kColS + 128 * slot, umma_desc(qb + off, 16, 1024), umma_desc(kb + off, 16, 1024),
-                            idesc_qk, kk > 0);
-                }
-                umma_commit(bar_s(slot));
+                for (int kk = 0; kk < D / 16; ++kk)
+                    umma_ss(tSbase + 64 * buf, umma_desc(qb + (kk >> 2) * C::kQHalfBytes + (kk & 3) * 32, 16, 1024),
+                            umma_desc(kb + (kk >> 2) * C::kKHalfBytes + (kk & 3) * 32, 16, 1024), idesc_qk, kk > 0);
+                umma_commit(bar_s(slot, buf));
             }
             __syncwarp();
         };
-        // O_slot (+)= P_slot V over the V stage in ring entry e: one K=16 MMA per valid block
-        // (P = bf16 hi + bf16 lo: per 32-column chunk of S_slot, hi in columns 0-15, lo in 16-31)
-        auto issue_pv = [&](int32_t slot, int32_t e, int32_t nt, bool accumulate) {
+        // O (+)= P V over the V half-stage in ring entry e: per valid block one K=16 MMA for the hi part of P
+        // and one for the lo part (per 32-column chunk of the S buffer: hi in columns 0-15, lo in 16-31)
+        auto issue_pv = [&](int32_t buf, int32_t e, int32_t nt, bool accumulate) {
             if (lane == 0) {
                 const uint32_t vb = sRing + (e % C::NBUF) * C::kBufBytes;
                 for (int32_t b = 0; b < nt; ++b) {
-                    const uint32_t pa = tmem + C::kColS + 128 * slot + 32 * (b >> 1) + 8 * (b & 1);
+                    const uint32_t pa = tSbase + 64 * buf + 32 * (b >> 1) + 8 * (b & 1);
                     const uint64_t vd = umma_desc(vb + b * C::kTileBytes, 2048, 1024);
-                    umma_ts(tmem + C::kColO + D * slot, pa, vd, idesc_pv, (accumulate || b > 0) ? 1u : 0u);
-                    umma_ts(tmem + C::kColO + D * slot, pa + 16, vd, idesc_pv, 1u);
+                    umma_ts(tOacc, pa, vd, idesc_pv, (accumulate || b > 0) ? 1u : 0u);
+                    umma_ts(tOacc, pa + 16, vd, idesc_pv, 1u);
                 }
+                umma_commit(bar_pv(slot));
             }
             __syncwarp();
         };
@@ -269,76 +315,54 @@ attend_umma_kernel(AttendParams p) {
             fence_async_smem();
             __syncwarp();
         };
-        auto stage_nt = [&](int32_t j) { return min(C::KS, tl1 - (tl0 + j * C::KS)); };
-
-        if (two) {
-            int32_t ek = umma_entry_k(true, 0);
-            wait_full(ek);
-            issue_qk(0, 0, ek);
-            issue_qk(1, 1, ek);
-            release(ek);
-            for (int32_t j = 0; j < n_stage; ++j) {
-                const int32_t ev = umma_entry_v(true, j, n_stage), nt = stage_nt(j);
-                const bool more = j + 1 < n_stage;
-                wait_full(ev);
-                MTRACE(1, 4 * j + 2);
-                fix_ragged_v(ev, tl0 + j * C::KS, nt);
-                mbar_wait(bar_p(0), j & 1);
-                tc_fence_after();
-                MTRACE(1, 4 * j + 3);
-                issue_pv(0, ev, nt, j > 0);
-                if (!more && lane == 0) umma_commit(bar_o(0));
-                if (more) {
-                    ek = umma_entry_k(true, j + 1);
-                    wait_full(ek);
-                    issue_qk(0, 0, ek);
-                }
-                MTRACE(1, 4 * j + 4);
-                mbar_wait(bar_p(1), j & 1);
-                tc_fence_after();
-                MTRACE(1, 4 * j + 5);
-                issue_pv(1, ev, nt, j > 0);
-                release(ev);
-                if (!more && lane == 0) umma_commit(bar_o(1));
-                if (more) {
-                    issue_qk(1, 1, ek);
-                    release(ek);
-                }
-            }
-        } else {
-            for (int32_t j = 0; j < min(2, n_stage); ++j) {
-                const int32_t ek = umma_entry_k(false, j);
+        // this slot's half-stages: h(k) = k (two) or 2 k + slot
+        const int32_t n_mine = two ? n_half : (n_half - slot + 1) >> 1;
+        auto half_of = [&](int32_t k) { return two ? k : 2 * k + slot; };
+        for (int32_t k = 0; k < min(2, n_mine); ++k) {
+            const int32_t e = entry_k(half_of(k));
+            wait_full(e);
+            issue_qk(k, e);
+            release(e);
+        }
+        for (int32_t k = 0; k < n_mine; ++k) {
+            const int32_t h = half_of(k), e = entry_v(h), buf = k & 1;
+            const int32_t t0 = tl0 + h * C::KS, nt = min(C::KS, tl1 - t0);
+            MTRACE(slot, 4 * k);
+            wait_full(e);
+            MTRACE(slot, 4 * k + 1);
+            fix_ragged_v(e, t0, nt);
+            mbar_wait(bar_p(slot, buf), (k >> 1) & 1);
+            tc_fence_after();
+            MTRACE(slot, 4 * k + 2);
+            issue_pv(buf, e, nt, k > 0);
+            release(e);
+            if (k == n_mine - 1 && lane == 0) umma_commit(bar_o(slot));
+            if (k + 2 < n_mine) {
+                const int32_t ek = entry_k(half_of(k + 2));
                 wait_full(ek);
-                issue_qk(j, 0, ek);
+                issue_qk(buf, ek);
                 release(ek);
             }
-            for (int32_t j = 0; j < n_stage; ++j) {
-                const int32_t s = j & 1, ev = umma_entry_v(false, j, n_stage), nt = stage_nt(j);
-                wait_full(ev);
-                fix_ragged_v(ev, tl0 + j * C::KS, nt);
-                mbar_wait(bar_p(s), (j >> 1) & 1);
-                tc_fence_after();
-                issue_pv(s, ev, nt, j >= 2);
-                release(ev);
-                if (j + 2 >= n_stage && lane == 0) umma_commit(bar_o(s));
-                if (j + 2 < n_stage) {
-                    const int32_t ek = umma_entry_k(false, j + 2);
-                    wait_full(ek);
-                    issue_qk(s, 0, ek);
-                    release(ek);
-                }
-            }
+            MTRACE(slot, 4 * k + 3);
         }
-        // every softmax warp has finished reading TMEM
-        named_sync(2, C::kThreads - 32);
-        tc_fence_after();
-        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(C::kTmemCols));
+        // a phantom half-stage (R <= 128, odd count) belongs to slot 1: hand its two entries back
+        if (!two && slot == 1 && (n_half & 1)) {
+            const int32_t ek = entry_k(n_half), ev = entry_v(n_half);
+            wait_full(ek); if (lane == 0) mbar_arrive(bar_empty(ek % C::NBUF));
+            wait_full(ev); if (lane == 0) mbar_arrive(bar_empty(ev % C::NBUF));
+        }
+        if (warp == 1) {
+            // every softmax warp has finished reading TMEM
+            named_sync(2, 32 + 256);
+            tc_fence_after();
+            asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(C::kTmemCols));
+        }
         return;
     }
 
     // ================================ softmax warps ================================
-    if ((warp & 3) == 0) MTRACE(2 + ((warp - 2) >> 2), 1002);
-    const int32_t slot = (warp - 2) >> 2, quarter = warp & 3;       // TMEM lanes 32 (warp % 4) .. + 31
+    if ((warp & 3) == 0) MTRACE(2 + ((warp - 4) >> 2), 1002);
+    const int32_t slot = (warp - 4) >> 2, quarter = warp & 3;       // TMEM lanes 32 (warp % 4) .. + 31
     const int32_t row = quarter * 32 + lane;
     const int32_t tile_row0 = two ? 128 * slot : 0;
     const int32_t rho = tile_row0 + row;                              // rho = r * G + g
@@ -351,13 +375,13 @@ attend_umma_kernel(AttendParams p) {
 
     // ---- Q rows -> shared memory, K-major SWIZZLE_128B, one [128][64] region per 64-dim half ----
     {
-        const int32_t tid2 = threadIdx.x - 64;
+        const int32_t tid2 = threadIdx.x - 128;
         const int32_t n_rows = two ? 256 : 128;
         constexpr int CPR = D / 8;                                    // 16-byte chunks per row
         // 16-byte cp.async per chunk: all of a thread's copies are in flight together
         for (int32_t idx = tid2; idx < n_rows * CPR; idx += 256) {
             const int32_t rr = idx / CPR, c = idx % CPR;
-            const uint32_t dst = (rr >> 7) * C::kQBytes + (c >> 3) * C::kHalfBytes + (rr & 127) * 128 + (((c & 7) ^ (rr & 7)) << 4);
+            const uint32_t dst = (rr >> 7) * C::kQBytes + (c >> 3) * C::kQHalfBytes + (rr & 127) * 128 + (((c & 7) ^ (rr & 7)) << 4);
             if (rr < R) {
                 const int32_t r2 = rr / p.G, g2 = rr - r2 * p.G;
                 const __nv_bfloat16* src = p.q + ((int64_t)(it.q_row_off + r2) * p.Hq + kvh * p.G + g2) * D + c * 8;
@@ -371,132 +395,124 @@ attend_umma_kernel(AttendParams p) {
     }
     named_sync(1, C::kThreads);
     tc_fence_after();
-    if ((warp & 3) == 0) MTRACE(2 + ((warp - 2) >> 2), 1003);
+    if ((warp & 3) == 0) MTRACE(2 + ((warp - 4) >> 2), 1003);
     const uint32_t tmem = *tmem_slot;
     const uint32_t lane_base = (uint32_t)(quarter * 32) << 16;
-    const uint32_t tS = tmem + lane_base + C::kColS + 128 * slot;     // S (fp32) and, over it, P (bf16 x 2 per column)
+    const uint32_t tS = tmem + lane_base + C::kColS + 128 * slot;     // two 64-column S buffers; P (bf16 hi | lo) goes over S
     const uint32_t tO = tmem + lane_base + C::kColO + D * slot;
 
-    // One stage of one slot, per thread = per query row: 128 scores in TMEM.  The scores are read
-    // in 32-column chunks, twice (pass 1: row max; pass 2: exp2, round, write P), with the next
-    // chunk's tcgen05.ld in flight while the current one is processed: ~100 live registers instead
-    // of 128 scores + 128 weights (which spilled), and P chunk c (16 columns) lands on columns the
-    // pass has already consumed.
+    // One half-stage of one slot, per thread = per query row: 64 scores, read ONCE into registers
+    // (two tcgen05.ld of 32 columns), row max, exp2, and P written back over the columns just read.
     float m_run = -INFINITY, m_used = -INFINITY;
     float l0 = 0.f, l1 = 0.f, l2 = 0.f, l3 = 0.f;                     // four partial sums (ILP)
-    int32_t n_it = 0;
-    for (int32_t j = two ? 0 : slot; j < n_stage; j += two ? 1 : 2, ++n_it) {
-        if (quarter == 0) MTRACE(2 + slot, 16 * n_it + 0);
-        mbar_wait(bar_s(slot), n_it & 1);
+    const int32_t n_mine = two ? n_half : (n_half - slot + 1) >> 1;
+    for (int32_t k = 0; k < n_mine; ++k) {
+        const int32_t h = two ? k : 2 * k + slot, buf = k & 1;
+        if (quarter == 0) MTRACE(2 + slot, 4 * k);
+        mbar_wait(bar_s(slot, buf), (k >> 1) & 1);
         tc_fence_after();
-        if (quarter == 0) MTRACE(2 + slot, 16 * n_it + 1);
-        float sub = 0.f;
-        bool full = true;
-        const int32_t t0 = tl0 + j * C::KS;
-        const int32_t nt = min(C::KS, tl1 - t0);
-        auto mask_chunk = [&](uint32_t (&s)[32], int c) {
-#pragma unroll
-            for (int bb = 0; bb < 2; ++bb) {
-                const int32_t b = 2 * c + bb;
-                const int32_t p0 = b < nt ? tile_block(it, t0 + b) * kBlockTokens : INT32_MAX / 2;
-#pragma unroll
-                for (int k = 0; k < kBlockTokens; ++k)
-                    if (!admit(p0 + k, t, p.S, p.W)) s[bb * kBlockTokens + k] = 0xFF800000u;   // -inf
-            }
-        };
-        uint32_t sa[32], sb[32];
+        if (quarter == 0) MTRACE(2 + slot, 4 * k + 1);
         if (warp_active) {
-            tmem_ld32(tS, sa);
-            // a stage needs no mask when every key of it is admitted for every row of this warp
-            // (window tiles are consecutive logical blocks; a stage that holds sink tiles takes the mask)
+            const uint32_t tSb = tS + 64 * buf;
+            uint32_t sa[32], sb[32];
+            tmem_ld32(tSb, sa);
+            tmem_ld32(tSb + 32, sb);
+            const int32_t t0 = tl0 + h * C::KS;
+            const int32_t nt = min(C::KS, tl1 - t0);
+            // a half-stage needs no mask when every key of it is admitted for every row of this warp
+            // (window tiles are consecutive logical blocks; one that holds sink tiles takes the mask)
             const int32_t p_first = tile_block(it, t0) * kBlockTokens;
-            full = nt == C::KS && t0 >= it.n_sink_tiles && p_first + C::KS * kBlockTokens - 1 <= t_wmin &&
-                   t_wmax - p_first < p.W;
-            // ---- pass 1: row max ----
-            float mx0 = -INFINITY, mx1 = -INFINITY, mx2 = -INFINITY, mx3 = -INFINITY;
-            auto max_chunk = [&](uint32_t (&cur)[32], uint32_t (&nxt)[32], int c) {
-                tmem_wait_ld();
-                if (c < 3) tmem_ld32(tS + 32 * (c + 1), nxt);
-                if (!full) mask_chunk(cur, c);
+            const bool full = nt == C::KS && t0 >= it.n_sink_tiles && p_first + C::KS * kBlockTokens - 1 <= t_wmin &&
+                              t_wmax - p_first < p.W;
+            tmem_wait_ld();
+            if (!full) {
+                auto mask_chunk = [&](uint32_t (&s)[32], int c) {
 #pragma unroll
-                for (int k = 0; k < 32; k += 4) {
-                    mx0 = fmaxf(mx0, __uint_as_float(cur[k]));
-                    mx1 = fmaxf(mx1, __uint_as_float(cur[k + 1]));
-                    mx2 = fmaxf(mx2, __uint_as_float(cur[k + 2]));
-                    mx3 = fmaxf(mx3, __uint_as_float(cur[k + 3]));
-                }
-                if (quarter == 0) MTRACE(2 + slot, 16 * n_it + 2 + c);
-            };
-#ifndef EXP_NOPASS1
-            max_chunk(sa, sb, 0);
-            max_chunk(sb, sa, 1);
-            max_chunk(sa, sb, 2);
-            max_chunk(sb, sa, 3);
-#else
-            tmem_wait_ld(); mx0 = 8.f;
-#endif
-            tmem_ld32(tS, sa);                                        // pass 2, chunk 0: in flight over the rescale
+                    for (int bb = 0; bb < 2; ++bb) {
+                        const int32_t b = 2 * c + bb;
+                        const int32_t p0 = b < nt ? tile_block(it, t0 + b) * kBlockTokens : INT32_MAX / 2;
+#pragma unroll
+                        for (int kk = 0; kk < kBlockTokens; ++kk)
+                            if (!admit(p0 + kk, t, p.S, p.W)) s[bb * kBlockTokens + kk] = 0xFF800000u;   // -inf
+                    }
+                };
+                mask_chunk(sa, 0);
+                mask_chunk(sb, 1);
+            }
+            float mx0 = -INFINITY, mx1 = -INFINITY, mx2 = -INFINITY, mx3 = -INFINITY;
+#pragma unroll
+            for (int kk = 0; kk < 32; kk += 2) {
+                mx0 = fmaxf(mx0, __uint_as_float(sa[kk]));
+                mx1 = fmaxf(mx1, __uint_as_float(sa[kk + 1]));
+                mx2 = fmaxf(mx2, __uint_as_float(sb[kk]));
+                mx3 = fmaxf(mx3, __uint_as_float(sb[kk + 1]));
+            }
             const float mx = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * p.scale_log2;
             m_run = fmaxf(m_run, mx);
-            if (n_it == 0) {
-                m_used = m_run;                                       // O_s is still empty
+            if (k == 0) {
+                m_used = m_run;                                       // O is still empty
             } else {
                 // lazy rescale: keep the stale reference max while it is within 2^8 of the true one
                 const bool need = (m_run - m_used) > 8.f;             // (-inf) - (-inf) = NaN -> false
                 if (__any_sync(0xffffffffu, need)) {
+                    // S is double buffered, so P V of the previous half-stage may still be running
+                    mbar_wait(bar_pv(slot), (k - 1) & 1);
+                    tc_fence_after();
                     const float f = (need && m_used != -INFINITY) ? ex2(m_used - m_run) : 1.f;
                     l0 *= f; l1 *= f; l2 *= f; l3 *= f;
-                    tmem_wait_ld();                                   // (chunk 0 of pass 2 has landed in sa)
 #pragma unroll
                     for (int c = 0; c < D / 32; ++c) {
-                        tmem_ld32(tO + 32 * c, sb);
+                        uint32_t o[32];
+                        tmem_ld32(tO + 32 * c, o);
                         tmem_wait_ld();
 #pragma unroll
-                        for (int k = 0; k < 32; ++k) sb[k] = __float_as_uint(__uint_as_float(sb[k]) * f);
-                        tmem_st32(tO + 32 * c, sb);
+                        for (int kk = 0; kk < 32; ++kk) o[kk] = __float_as_uint(__uint_as_float(o[kk]) * f);
+                        tmem_st32(tO + 32 * c, o);
                     }
                     if (need) m_used = m_run;
                 }
             }
-            sub = m_used == -INFINITY ? 0.f : m_used;                 // nothing admitted yet: every p is 0
-            if (quarter == 0) MTRACE(2 + slot, 16 * n_it + 6);
-            // ---- pass 2: p = 2^(s * scale - m); P = bf16 hi + bf16 lo (2^-17 weights: the x20 outlier
-            // channels of config 4 need more than bf16's 2^-9), hi | lo of chunk c over S columns
-            // [32c, 32c+16) | [32c+16, 32c+32), which the pass has just consumed ----
-            auto exp_chunk = [&](uint32_t (&cur)[32], uint32_t (&nxt)[32], int c) {
-                tmem_wait_ld();
-                if (c < 3) tmem_ld32(tS + 32 * (c + 1), nxt);
-                if (!full) mask_chunk(cur, c);
+            const float sub = m_used == -INFINITY ? 0.f : m_used;     // nothing admitted yet: every p is 0
+            // p = 2^(s * scale - m); P = bf16 hi + bf16 lo (2^-17 weights: the x20 outlier channels of
+            // config 4 need more than bf16's 2^-9); hi | lo of chunk c over S columns [32c, +16) | [32c+16, +32)
+            const uint64_t scale2 = f2_pack(p.scale_log2, p.scale_log2), nsub2 = f2_pack(-sub, -sub);
+            uint64_t lA = f2_pack(l0, l1), lB = f2_pack(l2, l3);
+            auto exp_chunk = [&](uint32_t (&cur)[32], int c) {
                 uint32_t pk[32];
 #pragma unroll
-                for (int k = 0; k < 16; k += 2) {
-                    const float p0 = ex2(fmaf(__uint_as_float(cur[2 * k]), p.scale_log2, -sub));
-                    const float p1 = ex2(fmaf(__uint_as_float(cur[2 * k + 1]), p.scale_log2, -sub));
-                    const float p2 = ex2(fmaf(__uint_as_float(cur[2 * k + 2]), p.scale_log2, -sub));
-                    const float p3 = ex2(fmaf(__uint_as_float(cur[2 * k + 3]), p.scale_log2, -sub));
-                    pk[k] = pack_bf16(p0, p1);
-                    pk[k + 1] = pack_bf16(p2, p3);
-                    pk[16 + k] = pack_bf16(p0 - bf16lo(pk[k]), p1 - bf16hi(pk[k]));
-                    pk[17 + k] = pack_bf16(p2 - bf16lo(pk[k + 1]), p3 - bf16hi(pk[k + 1]));
-                    l0 += p0; l1 += p1; l2 += p2; l3 += p3;
+                for (int kk = 0; kk < 16; kk += 2) {
+                    float x0, x1, x2, x3;
+                    f2_unpack(f2_fma(f2_pack(__uint_as_float(cur[2 * kk]), __uint_as_float(cur[2 * kk + 1])), scale2, nsub2), x0, x1);
+                    f2_unpack(f2_fma(f2_pack(__uint_as_float(cur[2 * kk + 2]), __uint_as_float(cur[2 * kk + 3])), scale2, nsub2), x2, x3);
+                    const float p0 = ex2(x0), p1 = ex2(x1), p2 = ex2(x2), p3 = ex2(x3);
+                    pk[kk] = pack_bf16(p0, p1);
+                    pk[kk + 1] = pack_bf16(p2, p3);
+                    const uint64_t pa = f2_pack(p0, p1), pb = f2_pack(p2, p3);
+                    float d0, d1, d2, d3;
+                    f2_unpack(f2_sub(pa, f2_pack(bf16lo(pk[kk]), bf16hi(pk[kk]))), d0, d1);
+                    f2_unpack(f2_sub(pb, f2_pack(bf16lo(pk[kk + 1]), bf16hi(pk[kk + 1]))), d2, d3);
+                    pk[16 + kk] = pack_bf16(d0, d1);
+                    pk[17 + kk] = pack_bf16(d2, d3);
+                    lA = f2_add(lA, pa);
+                    lB = f2_add(lB, pb);
                 }
-                tmem_st32(tS + 32 * c, pk);
-                if (quarter == 0) MTRACE(2 + slot, 16 * n_it + 8 + c);
+                tmem_st32(tSb + 32 * c, pk);
             };
-            exp_chunk(sa, sb, 0);
-            exp_chunk(sb, sa, 1);
-            exp_chunk(sa, sb, 2);
-            exp_chunk(sb, sa, 3);
+            exp_chunk(sa, 0);
+            exp_chunk(sb, 1);
+            f2_unpack(lA, l0, l1);
+            f2_unpack(lB, l2, l3);
             tmem_wait_st();
         }
-        if (quarter == 0) MTRACE(2 + slot, 16 * n_it + 12);
+        if (quarter == 0) MTRACE(2 + slot, 4 * k + 2);
         tc_fence_before();
         __syncwarp();
-        if (lane == 0) mbar_arrive(bar_p(slot));
+        if (lane == 0) mbar_arrive(bar_p(slot, buf));
     }
-    float l = (l0 + l1) + (l2 + l3);
-
     if (quarter == 0) MTRACE(2 + slot, 1000);
+    float l = (l0 + l1) + (l2 + l3);
+    const int32_t n_it = n_mine;
+
     // ---- epilogue ----
     const int64_t qrow = (int64_t)(it.q_row_off + rq) * p.Hq + kvh * p.G + gq;
     float* ml1 = reinterpret_cast<float*>(gen + C::kMlOff);
@@ -536,7 +552,7 @@ attend_umma_kernel(AttendParams p) {
     } else {
         // both slots' MMAs are complete before the Q region is reused for the exchange
         mbar_wait(bar_o(0), 0);
-        if (n_stage >= 2) mbar_wait(bar_o(1), 0);
+        if (n_half >= 2) mbar_wait(bar_o(1), 0);
         tc_fence_after();
         constexpr int NCH = D / 4;                                     // float4 chunks per row
         float4* ex = reinterpret_cast<float4*>(gen) + row * NCH;
@@ -556,7 +572,7 @@ attend_umma_kernel(AttendParams p) {
             if (warp_active) load_o(o);
             named_sync(3, 256);
             if (warp_active) {
-                if (n_stage >= 2) {
+                if (n_half >= 2) {
                     const float m1 = ml1[2 * row], l1 = ml1[2 * row + 1];
                     const float M = fmaxf(m_used, m1);
                     const float a0 = m_used == -INFINITY ? 0.f : ex2(m_used - M);
@@ -578,7 +594,7 @@ attend_umma_kernel(AttendParams p) {
     }
     if (quarter == 0) MTRACE(2 + slot, 1001);
     tc_fence_before();
-    named_arrive(2, C::kThreads - 32);
+    named_arrive(2, 32 + 256);
 }
 
 // ------------------------------------------------------------------------------------------------
