@@ -48,6 +48,9 @@ def parse():
     ap.add_argument("--split-tokens", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--layers", type=int, default=1,
+                    help="KV pools cycled per sub-step (a model runs its 30-50 layers one after the other: with >= 4 "
+                         "layers consecutive passes over one layer's pool cannot hit in the 126 MB L2, SURVEY 8(d))")
     ap.add_argument("--sweep", default="", choices=["", "age", "sessions", "sw", "occupancy"],
                     help="shape checks of SURVEY sec. 8(d)/(f) instead of the bench line: one JSON line per point")
     return ap.parse_args()
@@ -258,7 +261,8 @@ def main():
     need = 2 * W + 3 * K
     w = wl.make_workload(args.config, n_sessions=args.sessions or None, n_timed_frames=need)
     events, info = wl.build_schedule(w, history_scale=args.history_scale)
-    r = Runner(w, n_layers=1, uid_base=replicas.uid_base(RANK))
+    NL = max(1, args.layers)
+    r = Runner(w, n_layers=NL, uid_base=replicas.uid_base(RANK))
     r.pool.set_tuning(args.split_tokens, args.family)
     t_hist = time.perf_counter()
     rest = r.run_history(events)
@@ -306,8 +310,9 @@ def main():
             if item[0] == "close":
                 r.pool.session_close(item[1]); continue
             st, k, v, q, o, _ = item
-            r.pool.append_kv(0, st.sids, st.n_new, k, v)
-            r.pool.attend_frame(0, st.sids, st.n_new, q, o)
+            for layer in range(NL):                   # the same rows stand in for every layer's K/V/Q
+                r.pool.append_kv(layer, st.sids, st.n_new, k, v)
+                r.pool.attend_frame(layer, st.sids, st.n_new, q, o)
 
     def finish_closes(prepped):
         for item in prepped:
@@ -368,7 +373,7 @@ def main():
     launches = r.pool.stats()["kernel_launches"] - launches0
     if not churn:
         finish_closes(timed)
-    value, ms = replicas.aggregate(ms, session_frames(timed_f), device="cuda")   # max over ranks, sum of frames
+    value, ms = replicas.aggregate(ms, session_frames(timed_f) * NL, device="cuda")  # max over ranks; per layer
 
     # ---- roofline of the dominant kernel: same steps again with the library's event brackets ----
     r.pool.set_profiling(True)
@@ -378,7 +383,7 @@ def main():
     r.pool.set_profiling(False)
     if not churn:
         finish_closes(prof)
-    alg_bytes = sum(algorithmic_bytes(w, it[5], it[0].n_new) for it in prof if it[0] != "close")
+    alg_bytes = NL * sum(algorithmic_bytes(w, it[5], it[0].n_new) for it in prof if it[0] != "close")
     n_prof_steps = sum(1 for it in prof if it[0] != "close")
     peak, peak_src = peaks()
     achieved = alg_bytes / (k_ms * 1e-3) / 1e9 if k_ms > 0 else 0.0
@@ -395,7 +400,7 @@ def main():
 
     # ---- end to end: HOST buffers through metronome_step_host, copies inside the timed region ----
     e2e = None
-    if not args.no_e2e and not churn:       # (config 5 is a latency sweep workload: no host arm)
+    if not args.no_e2e and not churn and NL == 1:       # (config 5 is a latency sweep workload: no host arm)
         def to_host(prepped):
             out = []
             for item in prepped:
@@ -447,7 +452,7 @@ def main():
         "dtype": "bf16 in, f32 accumulate", "data": "synthetic",
         "config": {"workload": f"BASELINE.json configs[{w.index - 1}] {w.name}: {w.n_sessions} sessions, "
                                f"{w.n_q_heads}Q/{w.n_kv_heads}KV, D={w.head_dim}, S={w.S}, W={w.W}, block 16",
-                   "sessions_per_gpu": w.n_sessions, "n_layers": 1, "parallelism": f"replicas x{WORLD}",
+                   "sessions_per_gpu": w.n_sessions, "n_layers": NL, "parallelism": f"replicas x{WORLD}",
                    "history_scale": args.history_scale,
                    "l2": "inputs larger than L2: every step streams each session's whole window "
                          f"({alg_bytes / max(k_n, 1) / 1e6:.0f} MB per step vs 126 MB L2), no flush needed",
