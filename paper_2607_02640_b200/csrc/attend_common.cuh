@@ -42,6 +42,8 @@ struct AttendParams {
     float* ws_ml;             // [row][Hq][max_splits][2]   running max (log2 domain), running sum
     int32_t max_splits;
     int32_t pdl_early;        // let the next kernel on the stream start launching right away (PDL)
+    const int32_t* range_item; // GQA decode: item that holds the first tile of each range (null: binary search)
+    int32_t* gqa_ctr;         // [2] claim / exit counters of the GQA decode kernel's dynamic ranges (zero between launches)
     int32_t* tickets;         // [item][Hkv] arrival counters of the stream-K pieces (zero between launches)
 };
 

@@ -347,14 +347,30 @@ struct GqaCfg {
     static_assert(16 * (D + 2) * 4 <= kWarpBytes, "merge scratch does not fit a warp's ring");
 };
 
+// The flattened tile list [0, total_tiles) is cut into RANGES in two regimes:
+//   static   ranges 0 .. n_static-1, q1 tiles each, cover [0, g1): range r belongs to CTA r
+//   dynamic  ranges n_static .. n_total-1, q2 (< q1) tiles each, cover [g1, total): claimed with an
+//            atomic counter by whichever CTA finishes early.  SMs do not stream at the same speed
+//            (equal static shares finished 63..95 us apart on a B200), so the last ~20 % of the
+//            work is handed out in small pieces.
 struct GqaPlan {
     int32_t n_kv_heads;
     int64_t total_tiles;      // Hkv * sum of the items' n_tiles
-    int64_t tiles_per_cta;    // ceil(total_tiles / gridDim.x)
+    int64_t q1, g1;           // static regime
+    int64_t q2;               // dynamic regime
+    int32_t n_static, n_total;
+    __host__ __device__ int64_t range_lo(int32_t r) const { return r < n_static ? r * q1 : g1 + (int64_t)(r - n_static) * q2; }
+    __host__ __device__ int64_t range_hi(int32_t r) const {
+        const int64_t hi = r < n_static ? (r + 1) * q1 : g1 + (int64_t)(r - n_static + 1) * q2;
+        const int64_t cap = r < n_static ? g1 : total_tiles;
+        return hi < cap ? hi : cap;
+    }
+    __host__ __device__ int32_t range_of(int64_t g) const {
+        return g < g1 ? (int32_t)(g / q1) : n_static + (int32_t)((g - g1) / q2);
+    }
+    // upper bound on the pieces one (item, head) pair of n tiles can be cut into
+    __host__ __device__ int32_t max_pieces(int32_t n) const { return (int32_t)((n + q2 - 1) / q2) + 2; }
 };
-
-// piece index of CTA `cta` within the (item, head) pair whose global tile range starts at pair_lo
-__device__ __forceinline__ int32_t gqa_first_cta(int64_t pair_lo, int64_t q) { return (int32_t)(pair_lo / q); }
 
 // grid = n_SM * CTAs/SM (<= total tiles), block = 128.  items[].tile_off = exclusive prefix of n_tiles.
 template <int D>
@@ -376,33 +392,36 @@ attend_gqa_kernel(AttendParams p, GqaPlan plan) {
     __syncthreads();
     uint32_t phase_bits = 0;                             // parity of each private stage
 
-    const int64_t q = plan.tiles_per_cta;
-    int64_t g = (int64_t)blockIdx.x * q;
-    const int64_t g_end = min(plan.total_tiles, g + q);
     const int32_t Hkv = plan.n_kv_heads;
-
+    __shared__ int32_t s_range;
+    int32_t range = blockIdx.x;                          // first the CTA's static range, then claimed ones
+    while (range < plan.n_total) {
+    int64_t g = plan.range_lo(range);
+    const int64_t g_end = plan.range_hi(range);
+    // the item that holds the range's first tile: from the host's table, else by binary search
+    // (largest i with tile_off[i] * Hkv <= g); later pairs of the range follow without a search
+    int32_t i = 0;
+    if (p.range_item) {
+        i = p.range_item[range];
+    } else {
+        int32_t lo = 0, hi = p.n_items - 1;
+        while (lo < hi) {
+            const int32_t mid = (lo + hi + 1) >> 1;
+            if ((int64_t)p.items[mid].tile_off * Hkv <= g) lo = mid; else hi = mid - 1;
+        }
+        i = lo;
+    }
     while (g < g_end) {
         // ---- the (item, head) pair that holds global tile g, and this CTA's piece of it ----
-        int32_t i = 0;
-        {
-            int32_t lo = 0, hi = p.n_items - 1;        // largest i with tile_off[i] * Hkv <= g
-            while (lo < hi) {
-                const int32_t mid = (lo + hi + 1) >> 1;
-                if ((int64_t)p.items[mid].tile_off * Hkv <= g) lo = mid; else hi = mid - 1;
-            }
-            i = lo;
-        }
         const AttendItem it = p.items[i];
         const int64_t item_lo = (int64_t)it.tile_off * Hkv;
         const int32_t kvh = (int32_t)((g - item_lo) / it.n_tiles);
         const int64_t pair_lo = item_lo + (int64_t)kvh * it.n_tiles;
         const int32_t a = (int32_t)(g - pair_lo);
         const int32_t b = (int32_t)min((int64_t)it.n_tiles, g_end - pair_lo);
-        const int32_t first_cta = gqa_first_cta(pair_lo, q);
-        const int32_t last_cta = gqa_first_cta(pair_lo + it.n_tiles - 1, q);
+        const int32_t first_cta = plan.range_of(pair_lo);                      // first / last range of this pair
+        const int32_t last_cta = plan.range_of(pair_lo + it.n_tiles - 1);
 
-        WarpTile<D> wt;
-        wt.init(p, it, kvh, 0, lane);
         const int32_t* trow = p.table + (int64_t)it.sid * p.tbl_width;
         const uint8_t* head_base = p.kv_layer + (int64_t)kvh * p.L.head_bytes;
         // this warp's tiles: a + warp, a + warp + 4, ...   (private ring, prologue fills NS stages)
@@ -417,6 +436,8 @@ attend_gqa_kernel(AttendParams p, GqaPlan plan) {
             }
         };
         for (int32_t k = 0; k < min(n_mine, C::NS); ++k) issue(k);
+        WarpTile<D> wt;                                   // (Q rows are fetched while the first tiles fly)
+        wt.init(p, it, kvh, 0, lane);
         for (int32_t k = 0; k < n_mine; ++k) {
             const int32_t st = k % C::NS;
             mbar_wait(bars + 8 * st, (phase_bits >> st) & 1u);
@@ -476,7 +497,7 @@ attend_gqa_kernel(AttendParams p, GqaPlan plan) {
 #pragma unroll
                     for (int d = 0; d < DPT; d += 2) dst[d >> 1] = pack_bf16(acc[d] * inv, acc[d + 1] * inv);
                 } else {
-                    const int64_t slot = qrow * p.max_splits + ((int32_t)blockIdx.x - first_cta);
+                    const int64_t slot = qrow * p.max_splits + (range - first_cta);
                     float4* dst = reinterpret_cast<float4*>(p.ws_acc + slot * D + sub * DPT);
 #pragma unroll
                     for (int d = 0; d < DPT; d += 4) __stcg(dst + (d >> 2), make_float4(acc[d], acc[d + 1], acc[d + 2], acc[d + 3]));
@@ -530,6 +551,18 @@ attend_gqa_kernel(AttendParams p, GqaPlan plan) {
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncthreads();
         g = pair_lo + b;
+        if (kvh + 1 == Hkv) ++i;                          // (a pair left unfinished ends the range anyway)
+    }
+    // ---- next range: one of the small dynamic ones, first come first served ----
+    if (plan.n_total == plan.n_static) break;
+    if (threadIdx.x == 0) s_range = plan.n_static + atomicAdd(p.gqa_ctr, 1);
+    __syncthreads();
+    range = s_range;
+    }
+    // every CTA leaves through exactly one failed claim: the last one out zeroes the counters for
+    // the next launch
+    if (plan.n_total != plan.n_static && threadIdx.x == 0) {
+        if (atomicAdd(p.gqa_ctr + 1, 1) == (int32_t)gridDim.x - 1) { p.gqa_ctr[0] = 0; p.gqa_ctr[1] = 0; }
     }
 }
 

@@ -37,6 +37,7 @@ constexpr int kStagingSlots = 64;      // per-call metadata slots (pinned host +
 constexpr int kStagingGroup = 8;       // one completion event per 8 slots: an event between two kernels
                                        // would break their programmatic (PDL) launch edge
 constexpr int kMaxSplits = 64;
+constexpr int kMaxRangeItems = 4096;   // GQA decode ranges whose start item travels with the work list
 
 // Row a8: the launch plan of one attend_frame call (host side of the work list).  Items of class 0
 // go to the row kernel or the GQA decode kernel, items of class 1 (placed after them) to the chunk
@@ -52,6 +53,7 @@ struct AttendPlan {
     int32_t max_splits = 1;
     GqaPlan gplan{};
     int32_t gqa_ctas = 0;
+    int32_t n_range_items = 0;        // int32 entries after the AttendItems (0: kernels search)
     int64_t total_rows = 0;
 };
 
@@ -272,7 +274,8 @@ int plan_attend(metronome_pool* pool, int32_t n_batch, const int32_t* sids, cons
             units += (int64_t)its[i].n_tiles * (family == 2 ? c.n_kv_heads : c.n_q_heads * its[i].q_len);
         }
         if (family == 2 && cls == 0) {
-            // stream-K: equal contiguous tile ranges over a grid of n_SM x 3 CTAs
+            // stream-K: one wave of n_SM x 3 CTAs, equal static ranges (one per CTA); for long shares the
+            // last 10 % of the flattened tile list is cut into small ranges claimed dynamically.
             GqaPlan& g = pl.gplan;
             g.n_kv_heads = c.n_kv_heads;
             g.total_tiles = cls_tiles[0] * c.n_kv_heads;
@@ -281,10 +284,29 @@ int plan_attend(metronome_pool* pool, int32_t n_batch, const int32_t* sids, cons
             if (ctas > (g.total_tiles + min_tiles - 1) / min_tiles) ctas = (g.total_tiles + min_tiles - 1) / min_tiles;
             if (pool->tune_split_tokens > 0) ctas = (g.total_tiles + min_tiles - 1) / min_tiles;
             if (ctas < 1) ctas = 1;
-            g.tiles_per_cta = (g.total_tiles + ctas - 1) / ctas;
-            pl.gqa_ctas = (int32_t)((g.total_tiles + g.tiles_per_cta - 1) / g.tiles_per_cta);
+            const int64_t share = (g.total_tiles + ctas - 1) / ctas;
+            // measured on B200: the dynamic tail pays (-2 % on config 5) only when a CTA's share is long
+            // (>= 512 tiles = 4 MB); for shorter shares the restart of a claimed range costs more than the
+            // imbalance it removes (configs 3 and 4: +3..7 %), so they stay fully static
+            const bool dynamic = pool->tune_split_tokens <= 0 && share >= 512;
+            g.q1 = dynamic ? (share * 9 + 9) / 10 : share;
+            g.n_static = (int32_t)(dynamic ? ctas : (g.total_tiles + g.q1 - 1) / g.q1);
+            g.g1 = std::min<int64_t>(g.total_tiles, g.q1 * g.n_static);
+            g.q2 = dynamic ? std::max<int64_t>(8, g.q1 / 6) : g.q1;
+            g.n_total = g.n_static + (int32_t)((g.total_tiles - g.g1 + g.q2 - 1) / g.q2);
+            pl.gqa_ctas = g.n_static;
+            if (g.n_total <= kMaxRangeItems) {
+                int32_t* range_item = reinterpret_cast<int32_t*>(items + n_items);    // after ALL items
+                int32_t ii = 0;
+                for (int32_t r = 0; r < g.n_total; ++r) {
+                    const int64_t lo = g.range_lo(r);
+                    while (ii + 1 < n && (int64_t)its[ii + 1].tile_off * c.n_kv_heads <= lo) ++ii;
+                    range_item[r] = ii;
+                }
+                pl.n_range_items = g.n_total;
+            }
             for (int i = 0; i < n; ++i) {
-                const int32_t pieces = (int32_t)((its[i].n_tiles + g.tiles_per_cta - 1) / g.tiles_per_cta) + 1;
+                const int32_t pieces = g.max_pieces(its[i].n_tiles);
                 its[i].n_splits = pieces;      // upper bound on the pieces of one (item, head) pair
                 if (pieces > pl.max_splits) pl.max_splits = pieces;
             }
@@ -342,6 +364,8 @@ int launch_attend(metronome_pool* pool, int32_t layer, const AttendPlan& pl, con
     p.ws_acc = pool->d_ws_acc; p.ws_ml = pool->d_ws_ml;
     p.max_splits = pl.max_splits;
     p.tickets = pool->d_tickets;
+    p.range_item = pl.n_range_items ? reinterpret_cast<const int32_t*>(d_items + pl.n_items) : nullptr;
+    p.gqa_ctr = pool->d_bk_flag + 2;              // same 16-byte allocation: [flag, -, claims, exits]
     // measured on B200 (configs 2-4): letting the next append kernel launch early hides its host-memory
     // reads behind the attention kernel (-4..6 % per frame); the reverse (attention CTAs resident while
     // the append kernel runs) costs 15-25 %, so the append kernel does not trigger early
@@ -497,14 +521,14 @@ int metronome_pool_create(const metronome_pool_config_t* cfg, metronome_pool_t**
         }
         if (pool->poison) fill_nan_kernel<<<1184, 256>>>((uint4*)pool->d_kv, (int64_t)(need / 16));
     }
-    pool->slot_bytes = (size_t)c.max_sessions * (sizeof(AppendItem) + sizeof(AttendItem));
+    pool->slot_bytes = (size_t)c.max_sessions * (sizeof(AppendItem) + sizeof(AttendItem)) + kMaxRangeItems * sizeof(int32_t) + 16;
     e = cudaMalloc(&pool->d_tickets, (size_t)c.max_sessions * c.n_kv_heads * sizeof(int32_t));
     if (e != cudaSuccess) return fail(METRONOME_ERR_OUT_OF_MEMORY, e, "cudaMalloc tickets");
     cudaMemset(pool->d_tickets, 0, (size_t)c.max_sessions * c.n_kv_heads * sizeof(int32_t));
     e = cudaMalloc(&pool->d_bk_flag, 16);
     if (e != cudaSuccess) return fail(METRONOME_ERR_OUT_OF_MEMORY, e, "cudaMalloc flag");
     cudaMemset(pool->d_bk_flag, 0, 16);
-    e = cudaMalloc(&pool->d_attend_items, (size_t)c.max_sessions * sizeof(AttendItem));
+    e = cudaMalloc(&pool->d_attend_items, (size_t)c.max_sessions * sizeof(AttendItem) + kMaxRangeItems * sizeof(int32_t) + 16);
     if (e != cudaSuccess) return fail(METRONOME_ERR_OUT_OF_MEMORY, e, "cudaMalloc attend items");
     e = cudaMallocHost(&pool->h_stage, pool->slot_bytes * kStagingSlots);
     if (e != cudaSuccess) return fail(METRONOME_ERR_OUT_OF_MEMORY, e, "cudaMallocHost staging");
@@ -721,7 +745,7 @@ int metronome_append_kv(metronome_pool_t* pool, int32_t layer, int32_t n_batch, 
         if (have_plan) {
             a.attend_src = reinterpret_cast<const uint4*>(h_attend);
             a.attend_dst = reinterpret_cast<uint4*>(pool->d_attend_items);
-            a.attend_n16 = pool->cached_plan.n_items * (int32_t)(sizeof(AttendItem) / 16);
+            a.attend_n16 = (int32_t)((pool->cached_plan.n_items * sizeof(AttendItem) + pool->cached_plan.n_range_items * sizeof(int32_t) + 15) / 16);
         }
         a.k_new = (const uint4*)k_new; a.v_new = (const uint4*)v_new;
         a.kv_layer = pool->bookkeeping_only ? nullptr : pool->d_kv + (int64_t)layer * pool->L.layer_bytes;
@@ -768,7 +792,7 @@ int metronome_attend_frame(metronome_pool_t* pool, int32_t layer, int32_t n_batc
     AttendPlan plan;
     rc = plan_attend(pool, n_batch, sids, q_lens, reinterpret_cast<AttendItem*>(h), plan);
     if (rc) return rc;
-    rc = commit_stage(pool, slot, (size_t)plan.n_items * sizeof(AttendItem), st);
+    rc = commit_stage(pool, slot, (size_t)plan.n_items * sizeof(AttendItem) + (size_t)plan.n_range_items * sizeof(int32_t), st);
     if (rc) return rc;
     return launch_attend(pool, layer, plan, reinterpret_cast<const AttendItem*>(d), q, out, st, false);
 }
