@@ -181,7 +181,10 @@ attend_umma_kernel(AttendParams p) {
     volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(gen + C::kBarOff + 8 * (2 * C::NBUF + 12));
 
     const int32_t kvh = blockIdx.x;
-    const int32_t i = find_item(p.n_items, (int32_t)blockIdx.y, [&](int32_t k) { return p.items[k].split_off; });
+    // (no item is split when the grid has one row per item: no search)
+    const int32_t i = (int32_t)gridDim.y == p.n_items
+                          ? (int32_t)blockIdx.y
+                          : find_item(p.n_items, (int32_t)blockIdx.y, [&](int32_t k) { return p.items[k].split_off; });
     const AttendItem it = p.items[i];
     const int32_t split = (int32_t)blockIdx.y - it.split_off;
     const int32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
