@@ -51,7 +51,7 @@ def parse():
     ap.add_argument("--layers", type=int, default=1,
                     help="KV pools cycled per sub-step (a model runs its 30-50 layers one after the other: with >= 4 "
                          "layers consecutive passes over one layer's pool cannot hit in the 126 MB L2, SURVEY 8(d))")
-    ap.add_argument("--sweep", default="", choices=["", "age", "sessions", "sw", "occupancy"],
+    ap.add_argument("--sweep", default="", choices=["", "age", "sessions", "sw", "occupancy", "admission"],
                     help="shape checks of SURVEY sec. 8(d)/(f) instead of the bench line: one JSON line per point")
     return ap.parse_args()
 
@@ -247,6 +247,8 @@ def main():
             rows = sweeps.age_sweep(args.config, n_sessions=args.sessions or None)
         elif args.sweep == "sessions":
             rows = sweeps.sessions_sweep(history_scale=args.history_scale)
+        elif args.sweep == "admission":
+            rows = sweeps.admission_run()
         elif args.sweep == "occupancy":
             rows = sweeps.occupancy_trace(n_sessions=args.sessions or 128)
         else:

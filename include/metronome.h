@@ -200,6 +200,31 @@ int metronome_pool_set_profiling(metronome_pool_t* pool, int32_t enable);
 int metronome_pool_read_profile(metronome_pool_t* pool, double* attend_kernel_ms, int64_t* attend_kernel_launches,
                                 int32_t reset);
 
+/* ---- NEXT row f3: deadline-aware admission on the per-frame latency signal ----
+ * PAPER.md:L105-111 sec. 4.2: "an AIMD loop on the measured per-frame latency, which lowers the
+ * admission cap multiplicatively when latency nears a target fraction of the budget and raises it
+ * additively to probe when there is headroom.  Arrivals beyond the cap receive a clean overload
+ * rejection."  The paper gives no constants (parity unpinned by the paper; the rule below is this
+ * build's reading, R17).  Pure host state, no CUDA, not thread-safe.
+ *   observe(latency): cap <- max(cap_min, cap * mult_factor)   if latency >= target_frac * budget_ms
+ *                     cap <- min(cap_max, cap + add_step)      otherwise        (one update per frame)
+ *   admit(n_live):    1 iff n_live < floor(cap)                (the caller opens the session or sheds)
+ * Errors: INVALID_ARG (null pointers; budget_ms <= 0; target_frac not in (0, 1]; add_step <= 0;
+ * mult_factor not in (0, 1); cap_min < 1; cap_max < cap_min; cap_init outside [cap_min, cap_max]; a
+ * negative or NaN latency; n_live < 0). */
+typedef struct metronome_gate metronome_gate_t;
+typedef struct {
+    float budget_ms;     /* the frame deadline ("80 ms frame")            */
+    float target_frac;   /* back off when latency reaches this fraction of the budget  */
+    float add_step;      /* additive increase of the cap per frame with headroom       */
+    float mult_factor;   /* multiplicative decrease, in (0, 1)                          */
+    float cap_min, cap_max, cap_init;
+} metronome_gate_config_t;
+int metronome_gate_create(const metronome_gate_config_t* cfg, metronome_gate_t** out);
+int metronome_gate_destroy(metronome_gate_t* gate);
+int metronome_gate_observe(metronome_gate_t* gate, float frame_latency_ms, float* cap_out);
+int metronome_gate_admit(metronome_gate_t* gate, int32_t n_live, int32_t* admitted_out);
+
 const char* metronome_strerror(int status);
 /* Text of the last CUDA error seen by this pool ("" if none).  Valid until the next call. */
 const char* metronome_last_cuda_error(metronome_pool_t* pool);

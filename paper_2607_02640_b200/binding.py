@@ -28,7 +28,8 @@ EXPORTS = ["metronome_abi_version", "metronome_strerror", "metronome_last_cuda_e
            "metronome_pool_destroy", "metronome_session_open", "metronome_session_close",
            "metronome_append_kv", "metronome_attend_frame", "metronome_step_host",
            "metronome_session_query", "metronome_pool_query", "metronome_read_kv", "metronome_pool_stats",
-           "metronome_pool_set_tuning", "metronome_pool_set_profiling", "metronome_pool_read_profile"]
+           "metronome_pool_set_tuning", "metronome_pool_set_profiling", "metronome_pool_read_profile",
+           "metronome_gate_create", "metronome_gate_destroy", "metronome_gate_observe", "metronome_gate_admit"]
 
 
 class MetronomeError(RuntimeError):
@@ -82,6 +83,10 @@ def load():
     lib.metronome_pool_set_tuning.argtypes = [c_void_p, c_int32, c_int32]
     lib.metronome_pool_set_profiling.argtypes = [c_void_p, c_int32]
     lib.metronome_pool_read_profile.argtypes = [c_void_p, POINTER(ctypes.c_double), POINTER(c_int64), c_int32]
+    lib.metronome_gate_create.argtypes = [c_void_p, POINTER(c_void_p)]
+    lib.metronome_gate_destroy.argtypes = [c_void_p]
+    lib.metronome_gate_observe.argtypes = [c_void_p, c_float, POINTER(c_float)]
+    lib.metronome_gate_admit.argtypes = [c_void_p, c_int32, i32p]
     _lib = lib
     return lib
 
@@ -203,3 +208,39 @@ class Pool:
         ms, n = ctypes.c_double(), c_int64()
         self._check(self._lib.metronome_pool_read_profile(self._h, byref(ms), byref(n), int(reset)))
         return ms.value, n.value
+
+
+class GateConfig(ctypes.Structure):
+    _fields_ = [("budget_ms", c_float), ("target_frac", c_float), ("add_step", c_float), ("mult_factor", c_float),
+                ("cap_min", c_float), ("cap_max", c_float), ("cap_init", c_float)]
+
+
+class Gate:
+    """metronome_gate_t: the AIMD admission gate of PAPER.md:L105-111 (NEXT row f3).  Host-only."""
+
+    def __init__(self, *, budget_ms, target_frac, add_step, mult_factor, cap_min, cap_max, cap_init):
+        self._lib = load()
+        self._h = c_void_p()
+        cfg = GateConfig(budget_ms, target_frac, add_step, mult_factor, cap_min, cap_max, cap_init)
+        st = self._lib.metronome_gate_create(byref(cfg), byref(self._h))
+        if st:
+            raise MetronomeError(st)
+
+    def observe(self, frame_latency_ms: float) -> float:
+        cap = c_float()
+        st = self._lib.metronome_gate_observe(self._h, c_float(frame_latency_ms), byref(cap))
+        if st:
+            raise MetronomeError(st)
+        return cap.value
+
+    def admit(self, n_live: int) -> bool:
+        out = c_int32()
+        st = self._lib.metronome_gate_admit(self._h, n_live, byref(out))
+        if st:
+            raise MetronomeError(st)
+        return bool(out.value)
+
+    def __del__(self):
+        if getattr(self, "_h", None):
+            self._lib.metronome_gate_destroy(self._h)
+            self._h = None

@@ -926,6 +926,46 @@ int metronome_pool_read_profile(metronome_pool_t* pool, double* attend_kernel_ms
     return METRONOME_OK;
 }
 
+// ---- NEXT f3: AIMD admission gate, host-only ----
+struct metronome_gate {
+    metronome_gate_config_t cfg;
+    float cap;
+};
+
+int metronome_gate_create(const metronome_gate_config_t* c, metronome_gate_t** out) {
+    if (!c || !out) return METRONOME_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!(c->budget_ms > 0.f) || !(c->target_frac > 0.f && c->target_frac <= 1.f) || !(c->add_step > 0.f) ||
+        !(c->mult_factor > 0.f && c->mult_factor < 1.f) || !(c->cap_min >= 1.f) || !(c->cap_max >= c->cap_min) ||
+        !(c->cap_init >= c->cap_min && c->cap_init <= c->cap_max))
+        return METRONOME_ERR_INVALID_ARG;
+    metronome_gate* g = new (std::nothrow) metronome_gate();
+    if (!g) return METRONOME_ERR_OUT_OF_MEMORY;
+    g->cfg = *c;
+    g->cap = c->cap_init;
+    *out = g;
+    return METRONOME_OK;
+}
+
+int metronome_gate_destroy(metronome_gate_t* gate) {
+    delete gate;
+    return METRONOME_OK;
+}
+
+int metronome_gate_observe(metronome_gate_t* g, float latency_ms, float* cap_out) {
+    if (!g || !(latency_ms >= 0.f)) return METRONOME_ERR_INVALID_ARG;
+    if (latency_ms >= g->cfg.target_frac * g->cfg.budget_ms) g->cap = std::max(g->cfg.cap_min, g->cap * g->cfg.mult_factor);
+    else g->cap = std::min(g->cfg.cap_max, g->cap + g->cfg.add_step);
+    if (cap_out) *cap_out = g->cap;
+    return METRONOME_OK;
+}
+
+int metronome_gate_admit(metronome_gate_t* g, int32_t n_live, int32_t* admitted_out) {
+    if (!g || !admitted_out || n_live < 0) return METRONOME_ERR_INVALID_ARG;
+    *admitted_out = n_live < (int32_t)floorf(g->cap) ? 1 : 0;
+    return METRONOME_OK;
+}
+
 int metronome_pool_set_tuning(metronome_pool_t* pool, int32_t split_tokens, int32_t kernel_family) {
     if (!pool || split_tokens < 0 || kernel_family < 0 || kernel_family > 3) return METRONOME_ERR_INVALID_ARG;
     pool->tune_split_tokens = split_tokens;

@@ -8,6 +8,9 @@
             same pool and traffic: occupancy rho(t) = rho0 + N r t until POOL_EXHAUSTED at
             t_sat = (1 - rho0) / (N r) (Eq. 1, L83 Fig. 5) vs. the windowed plateau
             rho0 + N s(W)
+  admission NEXT row f3: the AIMD gate (metronome_gate_*) closed around the measured per-frame latency on
+            the config-5 traffic under open-loop overload: the cap must settle where latency sits at the
+            target fraction of the budget (Fig. 7)
   sw        NEXT row f1: W in {256 .. 4096} and S in {0, 16, 32, 64} at N = 128 (PAPER.md:L300
             Fig. 11, L308-323 Table 2 "sinks ... unchanged latency")
 
@@ -217,3 +220,67 @@ def occupancy_trace(n_sessions: int = 128, n_frames: int = 200):
         del r
         torch.cuda.empty_cache()
     return rows
+
+
+def admission_run(n_frames: int = 500, budget_ms: float = 2.5, target_frac: float = 0.8, arrivals_per_frame: float = 6.0,
+                  mean_life_frames: float = 300.0, seed: int = 260702645):
+    """NEXT f3: config-5 shapes (32Q/4KV, W=2048, frame = 13-chunk + 8 decode, pool of config 5), sessions
+    arrive as a Poisson stream far above what fits the deadline, live Exp(300) frames, and are admitted
+    only while the gate's cap allows; every frame's measured GPU latency (one layer) feeds the gate.
+    Returns one row: cap / live / latency every 25 frames and the steady-state summary."""
+    from . import binding
+    w = wl.make_workload(5)
+    frame = _frame_pattern(w)
+    rng = np.random.default_rng(seed)
+    gate = binding.Gate(budget_ms=budget_ms, target_frac=target_frac, add_step=1.0, mult_factor=0.85, cap_min=4.0,
+                        cap_max=float(w.slots), cap_init=16.0)
+    r = Runner(w)
+    free_local = list(range(w.slots - 1, -1, -1))
+    alive = {}                                           # local index -> frames left
+    trace, lat_hist, live_hist, cap_hist = [], [], [], []
+    admitted = rejected = 0
+    cap = 16.0
+    for f in range(n_frames):
+        for i in [i for i, left in alive.items() if left <= 0]:
+            r.close(i)
+            del alive[i]
+            free_local.append(i)
+        for _ in range(int(rng.poisson(arrivals_per_frame))):
+            if free_local and gate.admit(len(alive)):
+                i = free_local.pop()
+                r.open(i)
+                alive[i] = int(np.ceil(rng.exponential(mean_life_frames)))
+                admitted += 1
+            else:
+                rejected += 1                            # the clean overload rejection of L109
+        order = np.asarray(sorted(alive), np.int32)
+        ms = 0.0
+        if len(order):
+            prepped = []
+            for n in frame:
+                st = r.make_step(("step", order, np.full(len(order), n, np.int32), True, f))
+                prepped.append((st, r.rows(synth.STREAM_K, 0, st.uid_rows, st.pos_rows),
+                                r.rows(synth.STREAM_V, 0, st.uid_rows, st.pos_rows),
+                                r.rows(synth.STREAM_Q, 0, st.uid_rows, st.pos_rows)))
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for st, kk, vv, qq in prepped:
+                r.pool.append_kv(0, st.sids, st.n_new, kk, vv)
+                r.pool.attend_frame(0, st.sids, st.n_new, qq, torch.empty_like(qq))
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1)
+        cap = gate.observe(ms)
+        for i in alive:
+            alive[i] -= 1
+        lat_hist.append(ms); live_hist.append(len(alive)); cap_hist.append(cap)
+        if f % 25 == 0:
+            trace.append({"frame": f, "cap": round(cap, 1), "live": len(alive), "latency_ms": round(ms, 3)})
+    tail = slice(n_frames // 2, None)
+    over = float(np.mean(np.asarray(lat_hist[tail]) > budget_ms))
+    return [{"sweep": "admission", "config": 5, "budget_ms": budget_ms, "target_ms": budget_ms * target_frac,
+             "arrivals_per_frame": arrivals_per_frame, "frames": n_frames, "admitted": admitted, "rejected": rejected,
+             "steady_live_mean": float(np.mean(live_hist[tail])), "steady_cap_mean": float(np.mean(cap_hist[tail])),
+             "steady_latency_ms_median": float(np.median(lat_hist[tail])),
+             "steady_latency_ms_p99": float(np.percentile(lat_hist[tail], 99)),
+             "steady_frames_over_budget_frac": over, "pool_exhausted": 0, "trace_every_25_frames": trace}]
