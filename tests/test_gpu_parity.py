@@ -363,3 +363,45 @@ def test_unbounded_arm_matches_the_oracle_until_the_pool_is_exhausted():
         assert exhausted
         m.check_tables(r.pool)
     _loaded_native()
+
+
+@pytest.mark.parametrize("q_len", [4, 25])
+def test_chunk_kernel_with_score_jumps_between_half_stages(q_len):
+    """Chunk-prefill kernel (tcgen05 path: R = 8 x q_len = 32 rows, one row tile, and 200 rows, two row
+    tiles) on keys whose scores jump by far more than 2^8 from one 64-key half-stage to a later one: the
+    lazy rescale of the TMEM accumulator (after the previous P V has completed) and the -inf handling of
+    rows that admit nothing in a half-stage must hold.  Seeded inputs built here; the oracle gets the
+    same bf16 bits."""
+    S, W, D, G = 4, 256, 128, 8
+    rng = np.random.default_rng(11 + q_len)
+    pool = binding.Pool(n_q_heads=G, n_kv_heads=1, head_dim=D, n_sinks=S, window=W, n_blocks=64, max_sessions=2,
+                        max_new_tokens=25)
+    pool.set_tuning(0, 2)
+    cfg = O.PoolConfig(n_q_heads=G, n_kv_heads=1, head_dim=D, S=S, W=W, n_blocks=64, block_size=16, max_sessions=2,
+                       max_new_tokens=25)
+    ora = O.DefinitionOracle(cfg)
+    sid = pool.session_open()
+    assert sid == ora.session_open()
+    direction = rng.standard_normal(D).astype(np.float32)
+    direction /= np.linalg.norm(direction)
+    total, worst = 0, 0.0
+    for step in range(40):
+        n = q_len if step % 3 else min(25, q_len + 5)
+        k = 0.3 * rng.standard_normal((n, 1, D)).astype(np.float32)
+        v = rng.standard_normal((n, 1, D)).astype(np.float32)
+        for j in range(n):                       # every ~37th key is a spike, each taller than the last
+            if (total + j) % 37 == 36:
+                k[j, 0] = direction * (4.0 + 0.5 * ((total + j) // 37))
+                v[j, 0] = 50.0 * np.sign(rng.standard_normal(D))
+        q = (0.3 * rng.standard_normal((n, G, D)) + 30.0 * direction).astype(np.float32)
+        kb, vb, qb = (torch.from_numpy(a).to(torch.bfloat16).cuda() for a in (k, v, q))
+        pool.append_kv(0, [sid], [n], kb, vb)
+        ora.append_kv(0, [sid], [n], synth.to_u16(kb), synth.to_u16(vb))
+        out = torch.empty_like(qb)
+        pool.attend_frame(0, [sid], [n], qb, out)
+        ref = ora.attend_frame(0, [sid], [n], synth.to_u16(qb))
+        rep = assert_parity(out, ref, f"spiky chunk step {step} n={n}", unit_scale=False)
+        worst = max(worst, rep["row_l2"])
+        total += n
+    print("spiky chunk worst row l2", worst)
+    _loaded_native()
