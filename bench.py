@@ -379,7 +379,7 @@ def main():
 
     # ---- roofline of the dominant kernel: same steps again with the library's event brackets ----
     r.pool.set_profiling(True)
-    prof, _ = run_frames(take(K))
+    prof, prof_ms = run_frames(take(K))      # (its own GPU time: the share below is within this pass)
     torch.cuda.synchronize()
     k_ms, k_n = r.pool.read_profile()
     r.pool.set_profiling(False)
@@ -397,7 +397,7 @@ def main():
     roofline = {"bound": "hbm", "kernel": "attend_rows_kernel<128>" if w.n_q_heads == w.n_kv_heads else "attend_gqa_kernel (decode) + attend_umma_kernel (chunk)",
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes / max(k_n, 1),
-                "kernel_ms_avg": k_ms / max(k_n, 1), "kernel_share_of_step": k_ms / ms if ms > 0 else None,
+                "kernel_ms_avg": k_ms / max(k_n, 1), "kernel_share_of_step": k_ms / prof_ms if prof_ms > 0 else None,
                 "frac_of_nominal_8TBs": achieved / 8000.0}
 
     # ---- end to end: HOST buffers through metronome_step_host, copies inside the timed region ----

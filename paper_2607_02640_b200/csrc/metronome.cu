@@ -95,6 +95,9 @@ struct metronome_pool {
     size_t slot_bytes = 0;
     cudaEvent_t ev[kStagingSlots / kStagingGroup]{};
     bool ev_used[kStagingSlots / kStagingGroup]{};
+    bool group_dirty[kStagingSlots / kStagingGroup]{};   // slots of the group handed out since its last event
+    cudaStream_t last_stream = nullptr;
+    bool have_stream = false;
     int next_slot = 0;
 
     // profiling (metronome_pool_set_profiling): event pairs around the attention kernel
@@ -138,20 +141,31 @@ bool valid_cfg(const metronome_pool_config_t* c) {
 int acquire_stage(metronome_pool* pool, uint8_t** h, uint8_t** d, int* slot) {
     const int s = pool->next_slot;
     pool->next_slot = (s + 1) % kStagingSlots;
-    // entering a group: every call that used it one lap ago must have been consumed by the GPU
-    // (calls on a pool are stream-ordered: the event after the group's last call covers them all)
-    if (s % kStagingGroup == 0 && pool->ev_used[s / kStagingGroup]) CU(cudaEventSynchronize(pool->ev[s / kStagingGroup]));
+    if (s % kStagingGroup == 0) {
+        // Entering a group.  (1) Close the group just left: one event on the stream of its last call
+        // covers all its slots (calls on a pool are stream-ordered).  Doing it here, not after each
+        // call, keeps events from sitting between an append kernel and its attention kernel (that
+        // would break their programmatic launch edge) and also covers calls that returned an error.
+        const int prev = ((s + kStagingSlots - kStagingGroup) % kStagingSlots) / kStagingGroup;
+        if (pool->group_dirty[prev] && pool->have_stream) {
+            CU(cudaEventRecord(pool->ev[prev], pool->last_stream));
+            pool->ev_used[prev] = true;
+            pool->group_dirty[prev] = false;
+        }
+        // (2) every call that used this group one lap ago must have been consumed by the GPU
+        if (pool->ev_used[s / kStagingGroup]) CU(cudaEventSynchronize(pool->ev[s / kStagingGroup]));
+    }
+    pool->group_dirty[s / kStagingGroup] = true;
     *h = pool->h_stage + (size_t)s * pool->slot_bytes;
     *d = pool->d_stage + (size_t)s * pool->slot_bytes;
     *slot = s;
     return METRONOME_OK;
 }
-// after the last kernel / copy that reads the slot has been enqueued
+// after the last kernel / copy that reads the slot has been enqueued on `st`
 int release_stage(metronome_pool* pool, int slot, cudaStream_t st) {
-    if (slot % kStagingGroup == kStagingGroup - 1) {
-        CU(cudaEventRecord(pool->ev[slot / kStagingGroup], st));
-        pool->ev_used[slot / kStagingGroup] = true;
-    }
+    (void)slot;
+    pool->last_stream = st;
+    pool->have_stream = true;
     return METRONOME_OK;
 }
 int commit_stage(metronome_pool* pool, int slot, size_t bytes, cudaStream_t st) {
