@@ -399,6 +399,12 @@ def main():
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes / max(k_n, 1),
                 "kernel_ms_avg": k_ms / max(k_n, 1), "kernel_share_of_step": k_ms / prof_ms if prof_ms > 0 else None,
                 "frac_of_nominal_8TBs": achieved / 8000.0}
+    if RANK == 0:
+        # read-only stream microbenchmark in the same job: a second, read-only denominator
+        from paper_2607_02640_b200 import binding as _b
+        rs = _b.stream_read_gbs(4 << 30, 5)
+        roofline["read_stream_gbs"] = rs
+        roofline["frac_of_read_stream"] = achieved / rs if rs > 0 else None
 
     # ---- end to end: HOST buffers through metronome_step_host, copies inside the timed region ----
     e2e = None

@@ -225,6 +225,14 @@ int metronome_gate_destroy(metronome_gate_t* gate);
 int metronome_gate_observe(metronome_gate_t* gate, float frame_latency_ms, float* cap_out);
 int metronome_gate_admit(metronome_gate_t* gate, int32_t n_live, int32_t* admitted_out);
 
+/* Measurement aid ("plus a read-only stream microbenchmark run in the same job").
+ * Streams `bytes` of a scratch device buffer (allocated and freed inside) `reps` times with 16-byte
+ * loads from every SM and returns the best read-only bandwidth in GB/s in *gbs_out: the ceiling a pure
+ * KV stream can reach on this GPU, next to the read+write copy figure of MEASURED_PEAKS.json.
+ * Blocking; uses the current device and `cuda_stream`.  Errors: INVALID_ARG (bytes < 1 MiB, reps < 1,
+ * null), OUT_OF_MEMORY, CUDA. */
+int metronome_stream_read_gbs(size_t bytes, int32_t reps, void* cuda_stream, double* gbs_out);
+
 const char* metronome_strerror(int status);
 /* Text of the last CUDA error seen by this pool ("" if none).  Valid until the next call. */
 const char* metronome_last_cuda_error(metronome_pool_t* pool);

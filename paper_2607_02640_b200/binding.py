@@ -29,7 +29,8 @@ EXPORTS = ["metronome_abi_version", "metronome_strerror", "metronome_last_cuda_e
            "metronome_append_kv", "metronome_attend_frame", "metronome_step_host",
            "metronome_session_query", "metronome_pool_query", "metronome_read_kv", "metronome_pool_stats",
            "metronome_pool_set_tuning", "metronome_pool_set_profiling", "metronome_pool_read_profile",
-           "metronome_gate_create", "metronome_gate_destroy", "metronome_gate_observe", "metronome_gate_admit"]
+           "metronome_gate_create", "metronome_gate_destroy", "metronome_gate_observe", "metronome_gate_admit",
+           "metronome_stream_read_gbs"]
 
 
 class MetronomeError(RuntimeError):
@@ -87,6 +88,7 @@ def load():
     lib.metronome_gate_destroy.argtypes = [c_void_p]
     lib.metronome_gate_observe.argtypes = [c_void_p, c_float, POINTER(c_float)]
     lib.metronome_gate_admit.argtypes = [c_void_p, c_int32, i32p]
+    lib.metronome_stream_read_gbs.argtypes = [c_size_t, c_int32, c_void_p, POINTER(ctypes.c_double)]
     _lib = lib
     return lib
 
@@ -208,6 +210,15 @@ class Pool:
         ms, n = ctypes.c_double(), c_int64()
         self._check(self._lib.metronome_pool_read_profile(self._h, byref(ms), byref(n), int(reset)))
         return ms.value, n.value
+
+
+def stream_read_gbs(n_bytes: int = 4 << 30, reps: int = 5, stream=0) -> float:
+    """Read-only HBM stream microbenchmark (best of `reps`), GB/s."""
+    out = ctypes.c_double()
+    st = load().metronome_stream_read_gbs(n_bytes, reps, c_void_p(stream), byref(out))
+    if st:
+        raise MetronomeError(st)
+    return out.value
 
 
 class GateConfig(ctypes.Structure):

@@ -940,6 +940,44 @@ int metronome_pool_read_profile(metronome_pool_t* pool, double* attend_kernel_ms
     return METRONOME_OK;
 }
 
+// ---- measurement aid: read-only HBM stream ----
+int metronome_stream_read_gbs(size_t bytes, int32_t reps, void* cuda_stream, double* gbs_out) {
+    if (bytes < (1u << 20) || reps < 1 || !gbs_out) return METRONOME_ERR_INVALID_ARG;
+    metronome_pool* pool = nullptr;                      // (CU() reports through a pool; none here)
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    uint4* buf = nullptr;
+    unsigned int* sink = nullptr;
+    const int64_t n16 = (int64_t)(bytes / 16);
+    if (cudaMalloc(&buf, (size_t)n16 * 16) != cudaSuccess) return METRONOME_ERR_OUT_OF_MEMORY;
+    if (cudaMalloc(&sink, 4) != cudaSuccess) { cudaFree(buf); return METRONOME_ERR_OUT_OF_MEMORY; }
+    int dev = 0, n_sm = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    cudaMemsetAsync(buf, 1, (size_t)n16 * 16, st);
+    cudaMemsetAsync(sink, 0, 4, st);
+    double best = 0.0;
+    cudaError_t err = cudaSuccess;
+    for (int r = 0; r < reps + 1 && err == cudaSuccess; ++r) {          // first pass is a warm-up
+        cudaEventRecord(e0, st);
+        stream_read_kernel<<<n_sm * 8, 512, 0, st>>>(buf, n16, sink);
+        cudaEventRecord(e1, st);
+        err = cudaEventSynchronize(e1);
+        float ms = 0.f;
+        if (err == cudaSuccess) err = cudaEventElapsedTime(&ms, e0, e1);
+        if (r > 0 && ms > 0.f) best = std::max(best, (double)n16 * 16.0 / (ms * 1e-3) / 1e9);
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(buf);
+    cudaFree(sink);
+    if (err != cudaSuccess) return cuda_fail(pool, err, "stream_read");
+    *gbs_out = best;
+    return METRONOME_OK;
+}
+
 // ---- NEXT f3: AIMD admission gate, host-only ----
 struct metronome_gate {
     metronome_gate_config_t cfg;
