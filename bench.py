@@ -405,6 +405,8 @@ def main():
         rs = _b.stream_read_gbs(4 << 30, 5)
         roofline["read_stream_gbs"] = rs
         roofline["frac_of_read_stream"] = achieved / rs if rs > 0 else None
+        roofline["note"] = ("peak is the driver's copy figure (read + write); a read-only stream on the same GPU "
+                            "reaches read_stream_gbs, so frac can exceed 1: frac_of_read_stream is the tighter bound")
 
     # ---- end to end: HOST buffers through metronome_step_host, copies inside the timed region ----
     e2e = None

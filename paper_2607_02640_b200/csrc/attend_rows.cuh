@@ -29,7 +29,7 @@ __device__ __forceinline__ void merge_state(float& m, float& l, float (&acc)[8],
     m = M;
 }
 
-// grid = (total_splits, Hq, max_q_len), block = 128
+// grid = (Hq, total_splits, max_q_len), block = 128
 template <int D>
 __global__ void __launch_bounds__(128)
 attend_rows_kernel(AttendParams p) {
@@ -38,12 +38,15 @@ attend_rows_kernel(AttendParams p) {
     constexpr int LPT = D / 8;         // lanes per token (16-byte chunks per row)
     constexpr int TPS = 32 / LPT;      // tokens per warp step
     constexpr int STEPS = kBlockTokens / TPS;
-    const int32_t i = find_item(p.n_items, (int32_t)blockIdx.x, [&](int32_t k) { return p.items[k].split_off; });
+    // heads vary fastest across the grid: CTAs that run together read neighbouring 8 KiB tiles of the same
+    // KV blocks
+    const int32_t seg = (int32_t)blockIdx.y;
+    const int32_t i = find_item(p.n_items, seg, [&](int32_t k) { return p.items[k].split_off; });
     const AttendItem it = p.items[i];
     const int32_t r = blockIdx.z;
     if (r >= it.q_len) return;
-    const int32_t split = blockIdx.x - it.split_off;
-    const int32_t h = blockIdx.y, kvh = h / p.G;
+    const int32_t split = seg - it.split_off;
+    const int32_t h = blockIdx.x, kvh = h / p.G;
     const int32_t t = it.len - it.q_len + r;          // absolute position of this query (reading R2)
     const int32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int32_t sub = lane % LPT, grp = lane / LPT;

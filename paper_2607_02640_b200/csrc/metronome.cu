@@ -414,7 +414,7 @@ int launch_attend(metronome_pool* pool, int32_t layer, const AttendPlan& pl, con
         }
     } else {
         p.items = d_items; p.n_items = pl.n_items;
-        dim3 grid(pl.total_splits[0], c.n_q_heads, pl.cls_max_q[0]);
+        dim3 grid(c.n_q_heads, pl.total_splits[0], pl.cls_max_q[0]);
         if (c.head_dim == 128) CU(launch_kernel(attend_rows_kernel<128>, grid, dim3(128), 0, st, pdl, p));
         else CU(launch_kernel(attend_rows_kernel<64>, grid, dim3(128), 0, st, pdl, p));
         ++pool->n_launch;
