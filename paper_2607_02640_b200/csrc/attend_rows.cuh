@@ -71,22 +71,38 @@ attend_rows_kernel(AttendParams p) {
     const int32_t tl0 = split * it.tiles_per_split;
     const int32_t tl1 = min(it.n_tiles, tl0 + it.tiles_per_split);
 
-    for (int32_t tile = tl0 + warp; tile < tl1; tile += 4) {
-        const int32_t blk = tile < it.n_sink_tiles ? tile : it.first_blk + (tile - it.n_sink_tiles);
-        const int32_t p0 = blk * kBlockTokens;
-        // tiles with no admitted key for this row (later chunk rows leave early window tiles behind;
-        // earlier chunk rows do not see the newest tile): warp-uniform skip
-        if (p0 > t || (p0 >= p.S && t - (p0 + kBlockTokens - 1) >= p.W)) continue;
-        const int32_t phys = __ldg(trow + table_slot(blk, p.n_sink, p.ring));
-        const uint8_t* kt = p.kv_layer + (int64_t)phys * p.L.block_bytes + (int64_t)kvh * p.L.head_bytes;
-        const uint8_t* vt = kt + p.L.tile_bytes;
-        uint4 kr[STEPS], vr[STEPS];
+    // Software pipeline: the K rows of the NEXT tile are requested as soon as the scores of the current
+    // tile are out of the K registers, its V rows as soon as P V is done with the V registers, so a
+    // warp keeps ~8 KiB in flight through its whole compute phase (not only while it waits).
+    auto block_of = [&](int32_t tile) { return tile < it.n_sink_tiles ? tile : it.first_blk + (tile - it.n_sink_tiles); };
+    // next tile >= `tile` (stride 4) with at least one admitted key for this row; tl1 if none.  Later chunk
+    // rows leave early window tiles behind, earlier chunk rows do not see the newest tile.
+    auto next_valid = [&](int32_t tile) {
+        for (; tile < tl1; tile += 4) {
+            const int32_t p0 = block_of(tile) * kBlockTokens;
+            if (!(p0 > t || (p0 >= p.S && t - (p0 + kBlockTokens - 1) >= p.W))) break;
+        }
+        return tile;
+    };
+    auto tile_ptr = [&](int32_t tile) {
+        const int32_t phys = __ldg(trow + table_slot(block_of(tile), p.n_sink, p.ring));
+        return p.kv_layer + (int64_t)phys * p.L.block_bytes + (int64_t)kvh * p.L.head_bytes;
+    };
+    uint4 kr[STEPS], vr[STEPS];
+    int32_t tile = next_valid(tl0 + warp);
+    if (tile < tl1) {
+        const uint8_t* kt = tile_ptr(tile);
 #pragma unroll
         for (int j = 0; j < STEPS; ++j) {
             const int32_t off = tile_chunk_offset(j * TPS + grp, sub);
             kr[j] = __ldg(reinterpret_cast<const uint4*>(kt + off));
-            vr[j] = __ldg(reinterpret_cast<const uint4*>(vt + off));
+            vr[j] = __ldg(reinterpret_cast<const uint4*>(kt + p.L.tile_bytes + off));
         }
+    }
+    while (tile < tl1) {
+        const int32_t p0 = block_of(tile) * kBlockTokens;
+        const int32_t nxt = next_valid(tile + 4);
+        const uint8_t* kt_next = nxt < tl1 ? tile_ptr(nxt) : nullptr;
         float s[STEPS];
 #pragma unroll
         for (int j = 0; j < STEPS; ++j) {
@@ -100,6 +116,11 @@ attend_rows_kernel(AttendParams p) {
 #pragma unroll
             for (int o = LPT / 2; o >= 1; o >>= 1) d += __shfl_xor_sync(0xffffffffu, d, o);
             s[j] = d;
+        }
+        if (kt_next) {
+#pragma unroll
+            for (int j = 0; j < STEPS; ++j)
+                kr[j] = __ldg(reinterpret_cast<const uint4*>(kt_next + tile_chunk_offset(j * TPS + grp, sub)));
         }
         const bool full = (p0 + kBlockTokens - 1 <= t) &&
                           (p0 + kBlockTokens - 1 < p.S || t - p0 < p.W);
@@ -137,6 +158,12 @@ attend_rows_kernel(AttendParams p) {
             }
             m = mn;
         }
+        if (kt_next) {
+#pragma unroll
+            for (int j = 0; j < STEPS; ++j)
+                vr[j] = __ldg(reinterpret_cast<const uint4*>(kt_next + p.L.tile_bytes + tile_chunk_offset(j * TPS + grp, sub)));
+        }
+        tile = nxt;
     }
 
     // combine the token groups of the warp
