@@ -405,3 +405,33 @@ def test_chunk_kernel_with_score_jumps_between_half_stages(q_len):
         total += n
     print("spiky chunk worst row l2", worst)
     _loaded_native()
+
+
+def test_empty_batches_and_zero_length_items():
+    """Degenerate calls: an empty batch, and a batch in which some sessions append 0 tokens / ask for 0
+    query rows, must be accepted, leave those sessions untouched and give the other sessions' rows
+    exactly what they get alone (parity with the oracle)."""
+    from paper_2607_02640_b200.runner import Step
+    w = wl.make_workload(3, n_sessions=4)
+    for family in (1, 2):
+        r = Runner(w)
+        r.pool.set_tuning(0, family)
+        m = OracleMirror(r)
+        for i in range(4):
+            r.open(i); m.open(i)
+        empty = np.zeros(0, np.int32)
+        z = torch.zeros(0, w.n_kv_heads, w.head_dim, dtype=torch.bfloat16, device="cuda")
+        zq = torch.zeros(0, w.n_q_heads, w.head_dim, dtype=torch.bfloat16, device="cuda")
+        r.pool.append_kv(0, empty, empty, z, z)
+        r.pool.attend_frame(0, empty, empty, zq, zq)
+        rng = np.random.default_rng(9)
+        for step in range(24):
+            n_new = np.array([int(rng.integers(0, 26)) if rng.random() < 0.7 else 0 for _ in range(4)], np.int32)
+            st = r.make_step(("step", np.arange(4, dtype=np.int32), n_new, True, step))
+            r.append(st, 0); m.append(st, 0)
+            if n_new.sum() == 0:
+                r.pool.attend_frame(0, st.sids, st.n_new, zq, zq)
+            else:
+                assert_parity(r.attend(st, 0), m.attend(st, 0), f"zero-length items step {step} {n_new}")
+            m.check_tables(r.pool)
+    _loaded_native()
