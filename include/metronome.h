@@ -187,8 +187,8 @@ int metronome_pool_stats(metronome_pool_t* pool, int64_t* kernel_launches, int64
                          int64_t* attend_calls);
 
 /* Tuning knob (0 = automatic): keys per split-KV segment target, and forcing the kernel family
- * (0 auto, 1 CUDA-core row kernel, 2 tensor-core kernels, 3 = 2 with the mma.sync predecessor of the
- * tcgen05 chunk-prefill kernel).  For benchmarks and tests of "both launch modes" (L258).
+ * (0 auto, 1 CUDA-core row kernel, 2 tensor-core kernels: mma.sync GQA decode + tcgen05 chunk prefill).
+ * For benchmarks and tests of "both launch modes" (L258).
  * Errors: INVALID_ARG. */
 int metronome_pool_set_tuning(metronome_pool_t* pool, int32_t split_tokens, int32_t kernel_family);
 

@@ -1,36 +1,34 @@
-// attend_mma.cuh -- rows a5 (GQA decode) and a7 (chunk prefill) on the tensor cores.
+// attend_mma.cuh -- row a5 (+ a6) for grouped-query decode, on the tensor cores (mma.sync).
 //
-// The R = G x q_len query rows that share one KV head (GQA group x chunk rows; PAPER.md:L258
-// "grouped-query attention", "mixed prefill/decode") are cut into m16 row tiles, so the KV stream
-// is read from HBM ONCE for all of them.  Two kernels share the per-tile arithmetic (WarpTile):
+// The R = G x q_len <= 16 query rows that share one KV head ("grouped-query
+// attention") form one m16 row tile, so the KV stream is read from HBM ONCE for the whole group.
 //
-//   attend_gqa_kernel   R <= 16 (decode).  HBM-bound at G flop/byte.  The flattened list of
-//                       (item, KV head, tile) work is cut into EQUAL contiguous ranges, one per
-//                       CTA of a grid sized n_SM x CTAs/SM ("stream-K": ragged session ages cannot
-//                       unbalance the SMs); inside a CTA four warps take tiles round-robin, each
-//                       with a PRIVATE ring of bulk async copies (no CTA barrier in the loop),
-//                       and are merged through shared memory once per (item, head) piece.
-//   attend_mma_kernel   R <= 208 (chunk prefill).  One CTA per (segment, KV head), one compute warp
-//                       per m16 row tile, a producer warp streaming 64-key stages for all of them.
+//   attend_gqa_kernel   HBM-bound at G flop/byte.  The flattened list of (item, KV head, tile)
+//                       work is cut into EQUAL contiguous ranges, one per CTA of a single wave of
+//                       n_SM x 3 CTAs ("stream-K": ragged session ages cannot unbalance the SMs);
+//                       inside a CTA four warps take tiles round-robin, each with a PRIVATE ring
+//                       of bulk async copies (no CTA barrier in the tile loop), and are merged
+//                       through shared memory once per (item, head) piece.
 //
 // Data movement: one cp.async.bulk (SASS UBLKCP) of 2*16*D*2 bytes per (block, head) -- layout.cuh
 // keeps K|V of a block-head contiguous and pre-swizzled -- completion counted on an mbarrier.
 // Sinks go first ("extra leading iterations remapped onto the sink tiles ...
 // accumulating them first is exact"); in split mode only the piece that holds them takes them.
 //
-// Per 16-key tile: S = Q K^T (mma.sync m16n8k16 bf16, K fragments by ldmatrix), token-exact union
-// mask on boundary tiles only, online softmax in the log2 domain with a warp-uniform skip of the
-// rescale, O += P V (V fragments by ldmatrix.trans).  Two accuracy devices, both on the tensor core:
+// Per 16-key tile (WarpTile): S = Q K^T (mma.sync m16n8k16 bf16, K fragments by ldmatrix),
+// token-exact union mask on boundary tiles only, online softmax in the log2 domain with a
+// warp-uniform skip of the rescale, O += P V (V fragments by ldmatrix.trans).  Two accuracy devices,
+// both on the tensor core:
 //   * the softmax denominator is accumulated from the SAME rounded P that multiplies V (an extra n8
 //     tile against a ones matrix), so numerator and denominator see identical weights;
 //   * P is split into bf16 hi + lo parts, and the lo MMA is issued only for tiles that hold a key
-//     whose weight exceeds 1/32 (chunk) or 1/256 (decode, where the MMA is free) of the running sum
-//     (warp-uniform vote): peaky softmax rows (config 4's x20 outlier channels) get ~2^-17 weights,
-//     flat rows pay almost nothing.
+//     whose weight exceeds 1/256 of the running sum (warp-uniform vote; the MMA is free in a
+//     bandwidth-bound kernel): peaky softmax rows (config 4's x20 outlier channels) get ~2^-17
+//     weights, flat rows pay almost nothing.
 //
-// Why mma.sync and not tcgen05 (round 1): decode is one m16 tile at G flop/byte; the chunk tiles are
-// the candidate for a tcgen05/TMEM path.  The HBM layout is already UMMA's
-// SWIZZLE_128B K-major.
+// Why mma.sync here and tcgen05 only for the chunk (attend_umma.cuh): decode is ONE m16 tile per KV
+// head at G flop/byte; a 128-row UMMA tile would be > 87 % padding.  The shared helpers of this file
+// (mbarrier / bulk-copy wrappers, tile_block) are used by the chunk kernel too.
 #pragma once
 #include "attend_common.cuh"
 
@@ -246,91 +244,6 @@ struct WarpTile {
 // logical block and first token position of tile `tile` of an item (sinks first, then the window)
 __device__ __forceinline__ int32_t tile_block(const AttendItem& it, int32_t tile) {
     return tile < it.n_sink_tiles ? tile : it.first_blk + (tile - it.n_sink_tiles);
-}
-
-// ================================================================================================
-// Chunk prefill: one CTA per (segment, KV head); NW compute warps (one m16 row tile each) + 1 producer.
-template <int D, int NW>
-struct MmaCfg {
-    static constexpr int KS = 4;                        // key tiles (blocks) per pipeline stage
-    static constexpr int NS = 3;                        // stages
-    static constexpr int kHeadBytes = 2 * kBlockTokens * D * 2;
-    static constexpr int kStageBytes = KS * kHeadBytes;
-    static constexpr int kSmemBytes = NS * kStageBytes + 2 * NS * 8 + 128;
-    static constexpr int kThreads = 32 * (NW + 1);
-};
-
-// grid = (total_splits of the chunk-class items, Hkv)
-template <int D, int NW>
-__global__ void __launch_bounds__(MmaCfg<D, NW>::kThreads, 1)
-attend_mma_kernel(AttendParams p) {
-    using C = MmaCfg<D, NW>;
-    if (p.pdl_early) pdl_launch_dependents();
-    pdl_wait();
-    extern __shared__ __align__(128) uint8_t smem_raw[];
-    const uint32_t smem_base = (smem_u32(smem_raw) + 127u) & ~127u;     // tiles are 128-byte swizzle atoms
-    const uint32_t bar_full = smem_base + C::NS * C::kStageBytes;
-    const uint32_t bar_empty = bar_full + C::NS * 8;
-
-    const int32_t i = find_item(p.n_items, (int32_t)blockIdx.x, [&](int32_t k) { return p.items[k].split_off; });
-    const AttendItem it = p.items[i];
-    const int32_t split = blockIdx.x - it.split_off;
-    const int32_t kvh = blockIdx.y;
-    const int32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int32_t R = it.q_len * p.G;
-    const int32_t nw_active = (R + 15) >> 4;                // compute warps with at least one row
-    const int32_t tl0 = split * it.tiles_per_split;
-    const int32_t tl1 = min(it.n_tiles, tl0 + it.tiles_per_split);
-    const int32_t n_stage = (tl1 - tl0 + C::KS - 1) / C::KS;
-
-    if (threadIdx.x == 0) {
-        for (int s = 0; s < C::NS; ++s) {
-            mbar_init(bar_full + 8 * s, 1);
-            mbar_init(bar_empty + 8 * s, nw_active);
-        }
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
-    __syncthreads();
-
-    if (warp == NW) {
-        // ------------------------------ producer warp ------------------------------
-        const int32_t* trow = p.table + (int64_t)it.sid * p.tbl_width;
-        for (int32_t s = 0; s < n_stage; ++s) {
-            const int32_t slot = s % C::NS;
-            if (s >= C::NS) mbar_wait(bar_empty + 8 * slot, ((s / C::NS) - 1) & 1);
-            const int32_t t0 = tl0 + s * C::KS;
-            const int32_t nt = min(C::KS, tl1 - t0);
-            if (lane == 0) mbar_expect_tx(bar_full + 8 * slot, (uint32_t)nt * C::kHeadBytes);
-            __syncwarp();
-            if (lane < nt) {
-                const int32_t phys = __ldg(trow + table_slot(tile_block(it, t0 + lane), p.n_sink, p.ring));
-                const uint8_t* src = p.kv_layer + (int64_t)phys * p.L.block_bytes + (int64_t)kvh * p.L.head_bytes;
-                bulk_g2s(smem_base + slot * C::kStageBytes + lane * C::kHeadBytes, src, C::kHeadBytes, bar_full + 8 * slot);
-            }
-        }
-        return;
-    }
-    if (warp >= nw_active) return;
-
-    // -------------------------------- compute warps --------------------------------
-    WarpTile<D> wt;
-    wt.init(p, it, kvh, warp, lane);
-    for (int32_t s = 0; s < n_stage; ++s) {
-        const int32_t slot = s % C::NS;
-        mbar_wait(bar_full + 8 * slot, (s / C::NS) & 1);
-        const int32_t tbase = tl0 + s * C::KS;
-        const int32_t nt = min(C::KS, tl1 - tbase);
-        for (int32_t j = 0; j < nt; ++j) {
-            const int32_t p0 = tile_block(it, tbase + j) * kBlockTokens;
-            if (wt.skips(p, p0)) continue;
-            const uint32_t kt = smem_base + slot * C::kStageBytes + j * C::kHeadBytes;
-            wt.template step<32>(p, it.len, kt, kt + kBlockTokens * D * 2, p0, lane);
-        }
-        __syncwarp();
-        if (lane == 0) mbar_arrive(bar_empty + 8 * slot);
-    }
-    if (it.n_splits == 1) wt.store_final(p, lane);
-    else wt.store_partial(p, split, lane);
 }
 
 // ================================================================================================
@@ -567,41 +480,12 @@ attend_gqa_kernel(AttendParams p, GqaPlan plan) {
 }
 
 // ------------------------------------------------------------------------------------------------
-constexpr int kMmaMaxRows = 13 * 16;
-
-inline bool attend_mma_supported(int32_t G, int32_t max_q) { return (int64_t)G * max_q <= kMmaMaxRows; }
-
-template <int D, int NW>
-inline cudaError_t configure_one() {
-    return cudaFuncSetAttribute(attend_mma_kernel<D, NW>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                MmaCfg<D, NW>::kSmemBytes);
-}
-
 inline cudaError_t configure_attend_mma_kernels() {
     cudaError_t e;
-    if ((e = configure_one<128, 4>()) != cudaSuccess) return e;
-    if ((e = configure_one<128, 8>()) != cudaSuccess) return e;
-    if ((e = configure_one<128, 13>()) != cudaSuccess) return e;
-    if ((e = configure_one<64, 4>()) != cudaSuccess) return e;
-    if ((e = configure_one<64, 8>()) != cudaSuccess) return e;
-    if ((e = configure_one<64, 13>()) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(attend_gqa_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                   GqaCfg<128>::kSmemBytes)) != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(attend_gqa_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  GqaCfg<64>::kSmemBytes)) != cudaSuccess) return e;
-    return cudaSuccess;
-}
-
-// chunk-class items (16 < R <= 208): p.items / p.n_items must point at them
-inline void launch_attend_mma(const AttendParams& p, int32_t D, int32_t Hkv, int32_t total_splits, int32_t max_rows,
-                              cudaStream_t st) {
-    dim3 grid(total_splits, Hkv);
-#define METRONOME_LAUNCH_MMA(DD)                                                                                   \
-    if (max_rows <= 64) attend_mma_kernel<DD, 4><<<grid, MmaCfg<DD, 4>::kThreads, MmaCfg<DD, 4>::kSmemBytes, st>>>(p); \
-    else if (max_rows <= 128) attend_mma_kernel<DD, 8><<<grid, MmaCfg<DD, 8>::kThreads, MmaCfg<DD, 8>::kSmemBytes, st>>>(p); \
-    else attend_mma_kernel<DD, 13><<<grid, MmaCfg<DD, 13>::kThreads, MmaCfg<DD, 13>::kSmemBytes, st>>>(p);
-    if (D == 128) { METRONOME_LAUNCH_MMA(128) } else { METRONOME_LAUNCH_MMA(64) }
-#undef METRONOME_LAUNCH_MMA
+    return cudaFuncSetAttribute(attend_gqa_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                GqaCfg<64>::kSmemBytes);
 }
 
 // decode-class items (R <= 16)

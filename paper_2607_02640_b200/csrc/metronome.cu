@@ -46,7 +46,6 @@ struct AttendPlan {
     bool valid = false;
     int64_t epoch = -1;               // pool epoch the plan was made for (cached plans only)
     int family = 1;                   // 1 CUDA-core rows, 2 tensor-core (gqa + chunk)
-    bool legacy_chunk = false;        // tuning family 3: mma.sync chunk kernel
     int32_t n_items = 0;
     int32_t n_cls[2] = {0, 0}, total_splits[2] = {0, 0}, cls_rows[2] = {0, 0}, cls_max_q[2] = {0, 0};
     bool merge_cls[2] = {false, false};
@@ -217,7 +216,6 @@ int ensure_workspace(metronome_pool* pool, size_t slots) {
 //          general fallback
 //   gqa    tensor-core stream-K decode kernel: items with R = G x q_len <= 16
 //   chunk  tcgen05 / TMEM chunk-prefill kernel: items with 16 < R <= 256
-//          (tuning family 3: its mma.sync predecessor, R <= 208, kept for A/B measurements)
 // Fills items[0 .. plan.n_items) (host memory) and the plan; grows the split workspace if needed.
 int plan_attend(metronome_pool* pool, int32_t n_batch, const int32_t* sids, const int32_t* q_lens, AttendItem* items,
                 AttendPlan& pl) {
@@ -229,13 +227,10 @@ int plan_attend(metronome_pool* pool, int32_t n_batch, const int32_t* sids, cons
         pl.total_rows += q_lens[i];
     }
     int family = pool->tune_family;
-    const bool legacy_chunk = family == 3;
-    if (family == 3) family = 2;
     if (family == 0) family = (pool->G * max_q >= 4) ? 2 : 1;
-    if (family == 2 && !(legacy_chunk ? attend_mma_supported(pool->G, max_q) : attend_umma_supported(pool->G, max_q)))
+    if (family == 2 && !attend_umma_supported(pool->G, max_q))
         family = 1;
     pl.family = family;
-    pl.legacy_chunk = legacy_chunk;
 
     const int32_t W = pool->W_eff;
     int32_t* n_cls = pl.n_cls;
@@ -268,7 +263,7 @@ int plan_attend(metronome_pool* pool, int32_t n_batch, const int32_t* sids, cons
     pl.n_items = n_items;
     if (family != 2) { n_cls[0] = n_items; n_cls[1] = 0; }
     // chunk class: longest first, so the hardware's in-order CTA dispatch packs the short ones last
-    if (family == 2 && !legacy_chunk && n_cls[1] > 1)
+    if (family == 2 && n_cls[1] > 1)
         std::stable_sort(items + n_cls[0], items + n_cls[0] + n_cls[1],
                          [](const AttendItem& a, const AttendItem& b) { return a.n_tiles > b.n_tiles; });
 
@@ -331,7 +326,7 @@ int plan_attend(metronome_pool* pool, int32_t n_batch, const int32_t* sids, cons
         int32_t tps = pool->tune_split_tokens > 0 ? (pool->tune_split_tokens + kBlockTokens - 1) / kBlockTokens
                                                   : (int32_t)((units + target_ctas - 1) / target_ctas);
         if (pool->tune_split_tokens <= 0 && tps < 8) tps = 8;
-        if (family == 2 && !legacy_chunk && pool->tune_split_tokens <= 0) {
+        if (family == 2 && pool->tune_split_tokens <= 0) {
             // tcgen05 chunk kernel, one CTA per SM: whole (item, head) pairs when they alone give
             // >= 3 CTAs per SM (no partials to merge), else whole 128-key stages, >= 4 per segment
             if ((int64_t)n * c.n_kv_heads >= 3 * (int64_t)pool->n_sm) tps = INT32_MAX / 2;
@@ -404,12 +399,7 @@ int launch_attend(metronome_pool* pool, int32_t layer, const AttendPlan& pl, con
         }
         if (pl.n_cls[1] > 0) {
             p.items = d_items + pl.n_cls[0]; p.n_items = pl.n_cls[1];
-            if (pl.legacy_chunk) {
-                launch_attend_mma(p, c.head_dim, c.n_kv_heads, pl.total_splits[1], pool->G * pl.cls_max_q[1], st);
-                CU(cudaGetLastError());
-            } else {
-                CU(launch_attend_umma(p, c.head_dim, c.n_kv_heads, pl.total_splits[1], st, pdl));
-            }
+            CU(launch_attend_umma(p, c.head_dim, c.n_kv_heads, pl.total_splits[1], st, pdl));
             ++pool->n_launch;
         }
     } else {
@@ -1019,7 +1009,7 @@ int metronome_gate_admit(metronome_gate_t* g, int32_t n_live, int32_t* admitted_
 }
 
 int metronome_pool_set_tuning(metronome_pool_t* pool, int32_t split_tokens, int32_t kernel_family) {
-    if (!pool || split_tokens < 0 || kernel_family < 0 || kernel_family > 3) return METRONOME_ERR_INVALID_ARG;
+    if (!pool || split_tokens < 0 || kernel_family < 0 || kernel_family > 2) return METRONOME_ERR_INVALID_ARG;
     pool->tune_split_tokens = split_tokens;
     pool->tune_family = kernel_family;
     pool->cached_plan.valid = false;
