@@ -324,6 +324,7 @@ attend_gqa_kernel(AttendParams p, GqaPlan plan) {
         }
         i = lo;
     }
+    int32_t pre = 0;        // 1: the first tile of the coming pair is already in flight, in stage 1
     while (g < g_end) {
         // ---- the (item, head) pair that holds global tile g, and this CTA's piece of it ----
         const AttendItem it = p.items[i];
@@ -339,20 +340,22 @@ attend_gqa_kernel(AttendParams p, GqaPlan plan) {
         const uint8_t* head_base = p.kv_layer + (int64_t)kvh * p.L.head_bytes;
         // this warp's tiles: a + warp, a + warp + 4, ...   (private ring, prologue fills NS stages)
         const int32_t n_mine = (b - a - warp + C::NWARP - 1) / C::NWARP;
-        auto issue = [&](int32_t k) {      // k-th tile of this warp -> stage k % NS
+        const int32_t sbase = pre;         // k-th tile of this warp -> stage (k + sbase) % NS
+        auto issue = [&](int32_t k) {
             if (lane == 0) {
                 const int32_t tile = a + warp + k * C::NWARP;
                 const int32_t phys = __ldg(trow + table_slot(tile_block(it, tile), p.n_sink, p.ring));
-                const uint32_t bar = bars + 8 * (k % C::NS);
+                const int32_t st = (k + sbase) % C::NS;
+                const uint32_t bar = bars + 8 * st;
                 mbar_expect_tx(bar, C::kHeadBytes);
-                bulk_g2s(ring + (k % C::NS) * C::kHeadBytes, head_base + (int64_t)phys * p.L.block_bytes, C::kHeadBytes, bar);
+                bulk_g2s(ring + st * C::kHeadBytes, head_base + (int64_t)phys * p.L.block_bytes, C::kHeadBytes, bar);
             }
         };
-        for (int32_t k = 0; k < min(n_mine, C::NS); ++k) issue(k);
+        for (int32_t k = pre; k < min(n_mine, C::NS); ++k) issue(k);
         WarpTile<D> wt;                                   // (Q rows are fetched while the first tiles fly)
         wt.init(p, it, kvh, 0, lane);
         for (int32_t k = 0; k < n_mine; ++k) {
-            const int32_t st = k % C::NS;
+            const int32_t st = (k + sbase) % C::NS;
             mbar_wait(bars + 8 * st, (phase_bits >> st) & 1u);
             phase_bits ^= 1u << st;
             const int32_t p0 = tile_block(it, a + warp + k * C::NWARP) * kBlockTokens;
@@ -361,19 +364,46 @@ attend_gqa_kernel(AttendParams p, GqaPlan plan) {
             __syncwarp();                                  // every lane is done reading the stage
             if (k + C::NS < n_mine) issue(k + C::NS);
         }
+        // ---- while the warps are merged below, the first tile of the NEXT pair of this range is
+        // already on its way: the merge scratch of R <= 15 rows fits the warp's stage 0, so stage 1
+        // takes that tile now (saves the table -> HBM round trip after every (item, head) boundary) ----
+        const int32_t R_rows = it.q_len * p.G;
+        pre = 0;
+        if (R_rows * (D + 2) * 4 <= C::kHeadBytes && b == it.n_tiles && pair_lo + b < g_end) {
+            const bool same = kvh + 1 < Hkv;
+            const int32_t i2 = same ? i : i + 1;
+            const int32_t sid2 = same ? it.sid : p.items[i2].sid;
+            const int32_t nt2 = same ? it.n_tiles : p.items[i2].n_tiles;
+            const int32_t sink2 = same ? it.n_sink_tiles : p.items[i2].n_sink_tiles;
+            const int32_t first2 = same ? it.first_blk : p.items[i2].first_blk;
+            const int32_t b2 = (int32_t)min((int64_t)nt2, g_end - (pair_lo + b));
+            if (warp < b2) {
+                if (lane == 0) {
+                    const int32_t blk = warp < sink2 ? warp : first2 + (warp - sink2);
+                    const int32_t phys = __ldg(p.table + (int64_t)sid2 * p.tbl_width + table_slot(blk, p.n_sink, p.ring));
+                    const uint32_t bar = bars + 8;
+                    mbar_expect_tx(bar, C::kHeadBytes);
+                    bulk_g2s(ring + C::kHeadBytes,
+                             p.kv_layer + (int64_t)phys * p.L.block_bytes + (int64_t)(same ? kvh + 1 : 0) * p.L.head_bytes,
+                             C::kHeadBytes, bar);
+                }
+                pre = 1;
+            }
+        }
         // ---- merge the four warps through shared memory (their rings are idle now) ----
         __syncthreads();
-        float* scratch = reinterpret_cast<float*>(smem_gen + warp * C::kWarpBytes);   // [16][D + 2]
+        float* scratch = reinterpret_cast<float*>(smem_gen + warp * C::kWarpBytes);   // [R][D + 2], rows < R only
         {
             const int32_t ra = lane >> 2, c = (lane & 3) * 2;
+            const bool wa = ra < R_rows, wb = ra + 8 < R_rows;
 #pragma unroll
             for (int n = 0; n < WarpTile<D>::NT; ++n) {
-                *reinterpret_cast<float2*>(scratch + ra * (D + 2) + n * 8 + c) = make_float2(wt.o[n][0], wt.o[n][1]);
-                *reinterpret_cast<float2*>(scratch + (ra + 8) * (D + 2) + n * 8 + c) = make_float2(wt.o[n][2], wt.o[n][3]);
+                if (wa) *reinterpret_cast<float2*>(scratch + ra * (D + 2) + n * 8 + c) = make_float2(wt.o[n][0], wt.o[n][1]);
+                if (wb) *reinterpret_cast<float2*>(scratch + (ra + 8) * (D + 2) + n * 8 + c) = make_float2(wt.o[n][2], wt.o[n][3]);
             }
             if ((lane & 3) == 0) {
-                scratch[ra * (D + 2) + D] = wt.m_a; scratch[ra * (D + 2) + D + 1] = wt.lsum[0];
-                scratch[(ra + 8) * (D + 2) + D] = wt.m_b; scratch[(ra + 8) * (D + 2) + D + 1] = wt.lsum[2];
+                if (wa) { scratch[ra * (D + 2) + D] = wt.m_a; scratch[ra * (D + 2) + D + 1] = wt.lsum[0]; }
+                if (wb) { scratch[(ra + 8) * (D + 2) + D] = wt.m_b; scratch[(ra + 8) * (D + 2) + D + 1] = wt.lsum[2]; }
             }
         }
         __syncthreads();
