@@ -42,10 +42,28 @@ struct AttendParams {
     float* ws_ml;             // [row][Hq][max_splits][2]   running max (log2 domain), running sum
     int32_t max_splits;
     int32_t pdl_early;        // let the next kernel on the stream start launching right away (PDL)
+    const int32_t* items_flag; // work list of epoch items_epoch is on the device once *items_flag == items_epoch
+    int32_t items_epoch;      // -1: the list came by a copy / plain launch: wait for the predecessor at the top
     const int32_t* range_item; // GQA decode: item that holds the first tile of each range (null: binary search)
     int32_t* gqa_ctr;         // [2] claim / exit counters of the GQA decode kernel's dynamic ranges (zero between launches)
     int32_t* tickets;         // [item][Hkv] arrival counters of the stream-K pieces (zero between launches)
 };
+
+// Start of an attention kernel.  In early mode (items_epoch >= 0: launched programmatically behind an
+// append kernel that triggered its dependents at once) the kernel may run NEXT TO the kernels before
+// it: it only waits for its work list here, streams every block the append does not touch, and calls
+// pdl_wait() before the first FRESH block of an item (blocks that hold the rows appended in this
+// step: logical block >= (len - q_len) / 16) and before it writes anything.  Otherwise the
+// predecessor is waited for right away.  One thread per CTA; the caller syncs.
+__device__ __forceinline__ void wait_work_list(const AttendParams& p) {
+    if (p.items_epoch < 0) { pdl_wait(); return; }
+    int32_t seen;                       // (>=: a later step's list may already be out, in the other buffer)
+    do {
+        asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(seen) : "l"(p.items_flag) : "memory");
+        if (seen - p.items_epoch < 0) __nanosleep(64);
+    } while (seen - p.items_epoch < 0);
+}
+__device__ __forceinline__ int32_t fresh_block(const AttendItem& it) { return (it.len - it.q_len) / kBlockTokens; }
 
 __device__ __forceinline__ float ex2(float x) {
     float y;

@@ -34,7 +34,9 @@ template <int D>
 __global__ void __launch_bounds__(128)
 attend_rows_kernel(AttendParams p) {
     if (p.pdl_early) pdl_launch_dependents();
-    pdl_wait();                  // the work list and this step's K/V rows come from the append kernel
+    if (threadIdx.x == 0) wait_work_list(p);
+    __syncthreads();
+    if (p.items_epoch < 0) pdl_wait();
     constexpr int LPT = D / 8;         // lanes per token (16-byte chunks per row)
     constexpr int TPS = 32 / LPT;      // tokens per warp step
     constexpr int STEPS = kBlockTokens / TPS;
@@ -84,7 +86,9 @@ attend_rows_kernel(AttendParams p) {
         }
         return tile;
     };
+    const int32_t fresh = fresh_block(it);
     auto tile_ptr = [&](int32_t tile) {
+        if (block_of(tile) >= fresh) pdl_wait();        // rows (and maybe the block) of this step's append
         const int32_t phys = __ldg(trow + table_slot(block_of(tile), p.n_sink, p.ring));
         return p.kv_layer + (int64_t)phys * p.L.block_bytes + (int64_t)kvh * p.L.head_bytes;
     };
@@ -166,6 +170,7 @@ attend_rows_kernel(AttendParams p) {
         tile = nxt;
     }
 
+    pdl_wait();       // nothing is written before the predecessor (and the kernels before it) are over
     // combine the token groups of the warp
 #pragma unroll
     for (int o = 16; o >= LPT; o >>= 1) {

@@ -62,7 +62,9 @@ struct AppendParams {
     int32_t do_bookkeeping;        // 0: layers > 0, or nothing to free / allocate, or done by bookkeeping_kernel
     int32_t* bk_flag;
     int32_t epoch;
-    int32_t pdl_early;
+    int32_t pdl_early;             // early mode: let the dependent (attention) kernel launch right away
+    int32_t* items_flag;           // [0] <- epoch once the AttendItems are on the device; [4] <- epoch once past the wait
+    int32_t gate_epoch;            // early mode: items_flag[4] must have reached this before the buffer is reused
     const uint4* attend_src;       // AttendItems of this step (host), attend_n16 x 16 bytes; may be null
     uint4* attend_dst;
     int32_t attend_n16;
@@ -95,15 +97,47 @@ append_fused_kernel(const AppendParams a) {
             const int32_t n16 = a.n_items * (int32_t)(sizeof(AppendItem) / 16);
             for (int32_t idx = threadIdx.x; idx < n16; idx += 256) dst[idx] = src[idx];
         }
-        pdl_wait();
+        // The attention work list goes to the device, then *items_flag <- epoch (release).
+        //  - early mode (pdl_early: the row kernel may start before this kernel has passed its own
+        //    wait, to overlap its ramp-up with the previous attention kernel's tail): the copy is made
+        //    BEFORE the wait, into one of two buffers (epoch parity).  The reader of that buffer was the
+        //    attention kernel two steps back; it is over once the previous append kernel got past ITS
+        //    wait, which an early-mode kernel publishes in items_flag[4] (gate_epoch: the previous append's
+        //    epoch if it ran in early mode, else 0 = no gate: a kernel that is not in early mode lets its
+        //    attention kernel start only when it has completed).
+        //  - otherwise: after the wait.
+        auto copy_items = [&]() {
 #pragma unroll
-        for (int k = 0; k < kPre; ++k) {
-            const int32_t idx = k * 256 + (int32_t)threadIdx.x;
-            if (idx < a.attend_n16) a.attend_dst[idx] = pre[k];
+            for (int k = 0; k < kPre; ++k) {
+                const int32_t idx = k * 256 + (int32_t)threadIdx.x;
+                if (idx < a.attend_n16) a.attend_dst[idx] = pre[k];
+            }
+            for (int32_t idx = kPre * 256 + threadIdx.x; idx < a.attend_n16; idx += 256) a.attend_dst[idx] = a.attend_src[idx];
+        };
+        if (a.pdl_early) {
+            if (threadIdx.x == 0) {
+                int32_t seen;
+                do {
+                    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(seen) : "l"(a.items_flag + 4) : "memory");
+                    if (seen - a.gate_epoch < 0) __nanosleep(64);
+                } while (seen - a.gate_epoch < 0);
+            }
+            __syncthreads();
+            copy_items();
+            __threadfence();
+            __syncthreads();
+            if (threadIdx.x == 0)
+                asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(a.items_flag), "r"(a.epoch) : "memory");
         }
-        for (int32_t idx = kPre * 256 + threadIdx.x; idx < a.attend_n16; idx += 256) a.attend_dst[idx] = a.attend_src[idx];
+        pdl_wait();
+        if (a.pdl_early) {
+            if (threadIdx.x == 0)
+                asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(a.items_flag + 4), "r"(a.epoch) : "memory");
+        } else {
+            copy_items();          // (the kernel boundary publishes it: the attention kernel waits for this kernel at its top)
+        }
         if (!a.do_bookkeeping) return;
-        __syncthreads();
+        __syncthreads();          // the staged AppendItems are complete in shared memory
         const AppendItem* items = staged ? reinterpret_cast<const AppendItem*>(smem_items) : a.items;
         // phase 1: evict (a2) -- PAPER.md:L256 "frees blocks that fall entirely behind the window"
         for (int i = threadIdx.x; i < a.n_items; i += 256) {

@@ -53,6 +53,7 @@ struct AttendPlan {
     GqaPlan gplan{};
     int32_t gqa_ctas = 0;
     int32_t n_range_items = 0;        // int32 entries after the AttendItems (0: kernels search)
+    bool early = false;               // the append kernel of this step runs in early mode (see append_fused_kernel)
     int64_t total_rows = 0;
 };
 
@@ -82,8 +83,10 @@ struct metronome_pool {
     float* d_ws_acc = nullptr;
     float* d_ws_ml = nullptr;
     int32_t* d_tickets = nullptr;      // [max_sessions][Hkv], zero between launches
-    int32_t* d_bk_flag = nullptr;      // epoch of the last bookkeeping the fused append kernel finished
-    AttendItem* d_attend_items = nullptr;   // [max_sessions], written by the append kernel (cached plan)
+    int32_t* d_bk_flag = nullptr;      // [0] bookkeeping epoch, [1] work-list epoch, [2..3] GQA claim counters, [5] past-wait epoch
+    int32_t last_early_epoch = 0;      // epoch of the previous append kernel if it ran in early mode, else 0
+    AttendItem* d_attend_items = nullptr;   // 2 x [max_sessions] (+ range items), written by the append kernel (cached plan)
+    size_t attend_buf_bytes = 0;
     size_t ws_slots = 0;               // capacity in (row, head, split) slots
     uint8_t* d_io = nullptr;           // staging for metronome_step_host
     size_t io_bytes = 0;
@@ -376,9 +379,13 @@ int launch_attend(metronome_pool* pool, int32_t layer, const AttendPlan& pl, con
     p.range_item = pl.n_range_items ? reinterpret_cast<const int32_t*>(d_items + pl.n_items) : nullptr;
     p.gqa_ctr = pool->d_bk_flag + 2;              // same 16-byte allocation: [flag, -, claims, exits]
     // measured on B200 (configs 2-4): letting the next append kernel launch early hides its host-memory
-    // reads behind the attention kernel (-4..6 % per frame); the reverse (attention CTAs resident while
-    // the append kernel runs) costs 15-25 %, so the append kernel does not trigger early
+    // reads behind the attention kernel (-4..6 % per frame)
     p.pdl_early = 1;
+    // behind the fused append kernel of the same step the attention kernels may start early (they wait for
+    // their work list, stream the untouched blocks, and wait for the append before the fresh ones); with the
+    // poison fill or the profiling brackets in between, and on the general path, they wait at the top
+    p.items_flag = pool->d_bk_flag + 1;
+    p.items_epoch = (pdl && pl.early && !pool->profiling) ? (int32_t)pl.epoch : -1;
 
     if (pool->profiling) {
         if (pool->prof_used + 2 > pool->prof_ev.size()) {
@@ -529,10 +536,11 @@ int metronome_pool_create(const metronome_pool_config_t* cfg, metronome_pool_t**
     e = cudaMalloc(&pool->d_tickets, (size_t)c.max_sessions * c.n_kv_heads * sizeof(int32_t));
     if (e != cudaSuccess) return fail(METRONOME_ERR_OUT_OF_MEMORY, e, "cudaMalloc tickets");
     cudaMemset(pool->d_tickets, 0, (size_t)c.max_sessions * c.n_kv_heads * sizeof(int32_t));
-    e = cudaMalloc(&pool->d_bk_flag, 16);
+    e = cudaMalloc(&pool->d_bk_flag, 64);
     if (e != cudaSuccess) return fail(METRONOME_ERR_OUT_OF_MEMORY, e, "cudaMalloc flag");
-    cudaMemset(pool->d_bk_flag, 0, 16);
-    e = cudaMalloc(&pool->d_attend_items, (size_t)c.max_sessions * sizeof(AttendItem) + kMaxRangeItems * sizeof(int32_t) + 16);
+    cudaMemset(pool->d_bk_flag, 0, 64);
+    pool->attend_buf_bytes = (((size_t)c.max_sessions * sizeof(AttendItem) + kMaxRangeItems * sizeof(int32_t) + 16) + 255) & ~(size_t)255;
+    e = cudaMalloc(&pool->d_attend_items, 2 * pool->attend_buf_bytes);      // two buffers, by epoch parity
     if (e != cudaSuccess) return fail(METRONOME_ERR_OUT_OF_MEMORY, e, "cudaMalloc attend items");
     e = cudaMallocHost(&pool->h_stage, pool->slot_bytes * kStagingSlots);
     if (e != cudaSuccess) return fail(METRONOME_ERR_OUT_OF_MEMORY, e, "cudaMallocHost staging");
@@ -745,10 +753,17 @@ int metronome_append_kv(metronome_pool_t* pool, int32_t layer, int32_t n_batch, 
         a.do_bookkeeping = fused_bookkeeping ? 1 : 0;
         a.bk_flag = pool->d_bk_flag;
         a.epoch = (int32_t)pool->epoch;
-        a.pdl_early = 0;
+        // early mode (measured on B200): only for the row kernel (pure multi-head decode, config 2: -5 %);
+        // with the GQA decode / chunk kernels resident next to the append kernel configs 4 and 5 lose 20 %
+        const bool early = have_plan && pool->cached_plan.family == 1 && !pool->poison && !pool->profiling;
+        pool->cached_plan.early = early;
+        a.pdl_early = early ? 1 : 0;
+        a.items_flag = pool->d_bk_flag + 1;
+        a.gate_epoch = pool->last_early_epoch;
+        pool->last_early_epoch = early ? (int32_t)pool->epoch : 0;
         if (have_plan) {
             a.attend_src = reinterpret_cast<const uint4*>(h_attend);
-            a.attend_dst = reinterpret_cast<uint4*>(pool->d_attend_items);
+            a.attend_dst = reinterpret_cast<uint4*>(reinterpret_cast<uint8_t*>(pool->d_attend_items) + (pool->epoch & 1) * pool->attend_buf_bytes);
             a.attend_n16 = (int32_t)((pool->cached_plan.n_items * sizeof(AttendItem) + pool->cached_plan.n_range_items * sizeof(int32_t) + 15) / 16);
         }
         a.k_new = (const uint4*)k_new; a.v_new = (const uint4*)v_new;
@@ -787,7 +802,10 @@ int metronome_attend_frame(metronome_pool_t* pool, int32_t layer, int32_t n_batc
     if (cp.valid && cp.epoch == pool->epoch && (int32_t)pool->last_sids.size() == n_batch &&
         !memcmp(pool->last_sids.data(), sids, n_batch * sizeof(int32_t)) &&
         !memcmp(pool->last_n_new.data(), q_lens, n_batch * sizeof(int32_t)))
-        return launch_attend(pool, layer, cp, pool->d_attend_items, q, out, st, /*after_append=*/true);
+        return launch_attend(pool, layer, cp,
+                             reinterpret_cast<const AttendItem*>(reinterpret_cast<const uint8_t*>(pool->d_attend_items) +
+                                                                 (cp.epoch & 1) * pool->attend_buf_bytes),
+                             q, out, st, /*after_append=*/true);
 
     uint8_t *h = nullptr, *d = nullptr;
     int slot = 0;
