@@ -435,3 +435,37 @@ def test_empty_batches_and_zero_length_items():
                 assert_parity(r.attend(st, 0), m.attend(st, 0), f"zero-length items step {step} {n_new}")
             m.check_tables(r.pool)
     _loaded_native()
+
+
+def test_early_mode_decode_with_constant_eviction_and_reuse():
+    """Multi-head decode runs in 'early mode': the row kernel of step k streams the blocks the append of
+    step k does not touch while that append (and the tail of step k-1's attention) is still running.
+    A small window makes every session free a block every 16 steps, and the freed blocks are reused at
+    once by other sessions, so a read of a stale or reassigned block would show.  300 back-to-back
+    steps, every output and every table against the oracle."""
+    from dataclasses import replace
+    w = replace(wl.make_workload(2, n_sessions=24), W=40, n_blocks=24 * 5 + 3, max_new_tokens=4)
+    r = Runner(w, flags=0)
+    m = OracleMirror(r)
+    for i in range(24):
+        r.open(i); m.open(i)
+    rng = np.random.default_rng(21)
+    steps = []
+    for step in range(300):
+        idx = np.sort(rng.permutation(24)[: int(rng.integers(12, 25))]).astype(np.int32)
+        n_new = rng.integers(1, 4, size=len(idx)).astype(np.int32)
+        steps.append(r.make_step(("step", idx, n_new, True, step)))
+    # inputs first, so that nothing but the library's own kernels sits on the stream in the loop below
+    kvq = [(r.rows(synth.STREAM_K, 0, st.uid_rows, st.pos_rows), r.rows(synth.STREAM_V, 0, st.uid_rows, st.pos_rows),
+            r.rows(synth.STREAM_Q, 0, st.uid_rows, st.pos_rows)) for st in steps]
+    outs = [torch.empty_like(q) for _, _, q in kvq]
+    torch.cuda.synchronize()
+    for st, (k, v, q), o in zip(steps, kvq, outs):     # no host sync inside: the kernels run back to back
+        r.pool.append_kv(0, st.sids, st.n_new, k, v)
+        r.pool.attend_frame(0, st.sids, st.n_new, q, o)
+    torch.cuda.synchronize()
+    for st, out in zip(steps, outs):
+        m.append(st, 0)
+        assert_parity(out, m.attend(st, 0), f"early-mode step {st.frame}")
+    m.check_tables(r.pool)
+    _loaded_native()
