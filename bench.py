@@ -455,7 +455,10 @@ def main():
     cpu = None
     if not args.no_cpu_baseline and WORLD == 1:
         last = [it for it in timed if it[0] != "close"][-1][0]
-        cpu = cpu_baseline(w, r, {int(i): int(n) for i, n in zip(last.local, last.n_new)})
+        sample_steps = {int(i): int(n) for i, n in zip(last.local, last.n_new)}
+        cpu = cpu_baseline(w, r, sample_steps, budget_s=12.0)
+        one = cpu_baseline(w, r, sample_steps, budget_s=6.0, n_threads=1)      # 1 core and all cores
+        cpu["single_core_value"] = one["value"]
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": WORLD, "steps": K, "warmup": W,
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
