@@ -92,6 +92,19 @@ __device__ __forceinline__ void umma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64
                  "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
                  ::"r"(d_tmem), "r"(a_tmem), "l"(b), "r"(idesc), "r"(accum) : "memory");
 }
+// The same, issued by the lane whose `elect` is non-zero while EVERY lane of the warp carries the
+// (warp-uniform) operands: the descriptor arithmetic then stays on the uniform datapath instead of
+// running as a dependent chain of one lane plus R2UR moves (measured: ~130 -> ~45 cycles per MMA issued).
+__device__ __forceinline__ void umma_ss_e(uint32_t d_tmem, uint64_t a, uint64_t b, uint32_t idesc, uint32_t accum, uint32_t elect) {
+    asm volatile("{\n\t.reg .pred p, e;\n\tsetp.ne.b32 p, %4, 0;\n\tsetp.ne.b32 e, %5, 0;\n\t"
+                 "@e tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+                 ::"r"(d_tmem), "l"(a), "l"(b), "r"(idesc), "r"(accum), "r"(elect) : "memory");
+}
+__device__ __forceinline__ void umma_ts_e(uint32_t d_tmem, uint32_t a_tmem, uint64_t b, uint32_t idesc, uint32_t accum, uint32_t elect) {
+    asm volatile("{\n\t.reg .pred p, e;\n\tsetp.ne.b32 p, %4, 0;\n\tsetp.ne.b32 e, %5, 0;\n\t"
+                 "@e tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
+                 ::"r"(d_tmem), "r"(a_tmem), "l"(b), "r"(idesc), "r"(accum), "r"(elect) : "memory");
+}
 __device__ __forceinline__ void umma_commit(uint32_t bar) {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
 }
@@ -215,6 +228,25 @@ attend_umma_kernel(AttendParams p) {
         const int32_t* trow = p.table + (int64_t)it.sid * p.tbl_width;
         const uint8_t* head_base = p.kv_layer + (int64_t)kvh * p.L.head_bytes;
         const int32_t n_entries = two ? 2 * n_half : 4 * n_pair;
+        // Physical block ids of this segment's tiles, fetched ONCE (lane l holds tiles l, l+32, ...): a
+        // table lookup inside the loop is a dependent L2 round trip per ring entry and made the producer,
+        // not the tensor pipe or the softmax, set the pace of the whole kernel.
+        constexpr int kPhysPre = 8;                               // 256 tiles; longer segments look up the rest
+        int32_t phys_pre[kPhysPre];
+#pragma unroll
+        for (int j = 0; j < kPhysPre; ++j) {
+            const int32_t t = tl0 + j * 32 + lane;
+            phys_pre[j] = t < tl1 ? __ldg(trow + table_slot(tile_block(it, t), p.n_sink, p.ring)) : 0;
+        }
+        auto phys_of = [&](int32_t rel) {                         // rel = tile - tl0; rel >> 5 is warp-uniform
+            const int32_t j = rel >> 5;
+            int32_t v = phys_pre[0];
+#pragma unroll
+            for (int q = 1; q < kPhysPre; ++q) v = j == q ? phys_pre[q] : v;
+            v = __shfl_sync(0xffffffffu, v, rel & 31);
+            if (j >= kPhysPre) v = __ldg(trow + table_slot(tile_block(it, tl0 + rel), p.n_sink, p.ring));
+            return v;
+        };
         for (int32_t e = 0; e < n_entries; ++e) {
             // invert the order: which (K | V, half-stage) is entry e
             const int32_t es = two ? e : e >> 1, ns = two ? n_half : n_pair;
@@ -236,15 +268,13 @@ attend_umma_kernel(AttendParams p) {
             if (lane == 0) mbar_expect_tx(bar_full(b), (uint32_t)nt * C::kTileBytes);
             __syncwarp();
             const uint32_t dst = sRing + b * C::kBufBytes;
+            const int32_t blk = is_v ? lane : lane / C::NH, hh = lane % C::NH;
+            const int32_t phys = phys_of(h * C::KS + min(blk, C::KS - 1));      // (every lane takes part in the shuffle)
             if (is_v) {
-                if (lane < nt) {
-                    const int32_t phys = __ldg(trow + table_slot(tile_block(it, t0 + lane), p.n_sink, p.ring));
+                if (lane < nt)
                     bulk_g2s(dst + lane * C::kTileBytes, head_base + (int64_t)phys * p.L.block_bytes + p.L.tile_bytes,
                              C::kTileBytes, bar_full(b));
-                }
             } else if (lane < nt * C::NH) {
-                const int32_t blk = lane / C::NH, hh = lane % C::NH;
-                const int32_t phys = __ldg(trow + table_slot(tile_block(it, t0 + blk), p.n_sink, p.ring));
                 bulk_g2s(dst + hh * C::kKHalfBytes + blk * 2048, head_base + (int64_t)phys * p.L.block_bytes + hh * 2048, 2048,
                          bar_full(b));
             }
@@ -279,30 +309,34 @@ attend_umma_kernel(AttendParams p) {
         };
         auto release = [&](int32_t e) { if (lane == 0) umma_commit(bar_empty(e % C::NBUF)); };
         // S[buf] = Q K^T over the K half-stage in ring entry e
+        const uint32_t elect = lane == 0 ? 1u : 0u;
+        const uint64_t dq0 = umma_desc(qb, 16, 1024);
         auto issue_qk = [&](int32_t buf, int32_t e) {
-            if (lane == 0) {
-                const uint32_t kb = sRing + (e % C::NBUF) * C::kBufBytes;
+            // descriptors = base + (byte offset >> 4) in the address field (no carry: shared memory < 256 KB)
+            const uint64_t dk0 = umma_desc(sRing + (e % C::NBUF) * C::kBufBytes, 16, 1024);
+            const uint32_t ts = tSbase + 64 * buf;
 #pragma unroll
-                for (int kk = 0; kk < D / 16; ++kk)
-                    umma_ss(tSbase + 64 * buf, umma_desc(qb + (kk >> 2) * C::kQHalfBytes + (kk & 3) * 32, 16, 1024),
-                            umma_desc(kb + (kk >> 2) * C::kKHalfBytes + (kk & 3) * 32, 16, 1024), idesc_qk, kk > 0);
-                umma_commit(bar_s(slot, buf));
-            }
+            for (int kk = 0; kk < D / 16; ++kk)
+                umma_ss_e(ts, dq0 + (uint64_t)(((kk >> 2) * C::kQHalfBytes + (kk & 3) * 32) >> 4),
+                          dk0 + (uint64_t)(((kk >> 2) * C::kKHalfBytes + (kk & 3) * 32) >> 4), idesc_qk, kk > 0 ? 1u : 0u, elect);
+            if (lane == 0) umma_commit(bar_s(slot, buf));
             __syncwarp();
         };
         // O (+)= P V over the V half-stage in ring entry e: per valid block one K=16 MMA for the hi part of P
         // and one for the lo part (per 32-column chunk of the S buffer: hi in columns 0-15, lo in 16-31)
         auto issue_pv = [&](int32_t buf, int32_t e, int32_t nt, bool accumulate) {
-            if (lane == 0) {
-                const uint32_t vb = sRing + (e % C::NBUF) * C::kBufBytes;
-                for (int32_t b = 0; b < nt; ++b) {
-                    const uint32_t pa = tSbase + 64 * buf + 32 * (b >> 1) + 8 * (b & 1);
-                    const uint64_t vd = umma_desc(vb + b * C::kTileBytes, 2048, 1024);
-                    umma_ts(tOacc, pa, vd, idesc_pv, (accumulate || b > 0) ? 1u : 0u);
-                    umma_ts(tOacc, pa + 16, vd, idesc_pv, 1u);
+            const uint64_t vd0 = umma_desc(sRing + (e % C::NBUF) * C::kBufBytes, 2048, 1024);
+            const uint32_t pa0 = tSbase + 64 * buf;
+#pragma unroll
+            for (int b = 0; b < C::KS; ++b) {
+                if (b < nt) {                             // (warp-uniform)
+                    const uint32_t pa = pa0 + 32 * (b >> 1) + 8 * (b & 1);
+                    const uint64_t vd = vd0 + (uint64_t)((b * C::kTileBytes) >> 4);
+                    umma_ts_e(tOacc, pa, vd, idesc_pv, (accumulate || b > 0) ? 1u : 0u, elect);
+                    umma_ts_e(tOacc, pa + 16, vd, idesc_pv, 1u, elect);
                 }
-                umma_commit(bar_pv(slot));
             }
+            if (lane == 0) umma_commit(bar_pv(slot));
             __syncwarp();
         };
         // V rows past the session's length hold stale or poisoned bytes (0 * NaN = NaN): zero them
@@ -339,10 +373,12 @@ attend_umma_kernel(AttendParams p) {
             MTRACE(slot, 4 * k + 2);
             issue_pv(buf, e, nt, k > 0);
             release(e);
+            MTRACE(slot, 512 + 4 * k);
             if (k == n_mine - 1 && lane == 0) umma_commit(bar_o(slot));
             if (k + 2 < n_mine) {
                 const int32_t ek = entry_k(half_of(k + 2));
                 wait_full(ek);
+                MTRACE(slot, 512 + 4 * k + 1);
                 issue_qk(buf, ek);
                 release(ek);
             }
