@@ -60,7 +60,7 @@ struct UmmaCfg {
     static constexpr int kBarOff = 2 * kQBytes + NBUF * kBufBytes;
     static constexpr int kMlOff = kBarOff + 512;          // (m, l) of slot 1 for the in-CTA merge
     static constexpr int kSmemBytes = kMlOff + 1024 + 1024;   // + alignment slack
-    static constexpr int kThreads = 384;
+    static constexpr int kThreads = 384;                  // 12 warps: producer, 3 MMA issuers, 2 x 4 softmax
     static constexpr int kTmemCols = 512;
     static constexpr int kColS = 0, kColO = 256;          // S buffers of slot s at 128 s + {0, 64}; O_s at 256 + D s
     static_assert(kSmemBytes <= 232448, "shared memory budget");
@@ -189,9 +189,9 @@ attend_umma_kernel(AttendParams p) {
     auto bar_empty = [&](int b) { return sBar + 8u * (C::NBUF + b); };
     auto bar_s = [&](int s, int buf) { return sBar + 8u * (2 * C::NBUF + 2 * s + buf); };       // S ready  (MMA -> softmax)
     auto bar_p = [&](int s, int buf) { return sBar + 8u * (2 * C::NBUF + 4 + 2 * s + buf); };   // P written (softmax -> MMA)
-    auto bar_pv = [&](int s) { return sBar + 8u * (2 * C::NBUF + 8 + s); };                     // P V of a half-stage done
-    auto bar_o = [&](int s) { return sBar + 8u * (2 * C::NBUF + 10 + s); };                     // last P V of slot s done
-    volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(gen + C::kBarOff + 8 * (2 * C::NBUF + 12));
+    auto bar_pv = [&](int s, int buf) { return sBar + 8u * (2 * C::NBUF + 8 + 2 * s + buf); };  // P V out of that buffer done
+    auto bar_o = [&](int s) { return sBar + 8u * (2 * C::NBUF + 12 + s); };                     // last P V of slot s done
+    volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(gen + C::kBarOff + 8 * (2 * C::NBUF + 14));
 
     const int32_t kvh = blockIdx.x;
     // (no item is split when the grid has one row per item: no search)
@@ -217,8 +217,7 @@ attend_umma_kernel(AttendParams p) {
         if (lane == 0) {
             for (int b = 0; b < C::NBUF; ++b) { mbar_init(bar_full(b), 1); mbar_init(bar_empty(b), two ? 2 : 1); }
             for (int s = 0; s < 2; ++s) {
-                for (int buf = 0; buf < 2; ++buf) { mbar_init(bar_s(s, buf), 1); mbar_init(bar_p(s, buf), 4); }
-                mbar_init(bar_pv(s), 1);
+                for (int buf = 0; buf < 2; ++buf) { mbar_init(bar_s(s, buf), 1); mbar_init(bar_p(s, buf), 4); mbar_init(bar_pv(s, buf), 1); }
                 mbar_init(bar_o(s), 1);
             }
             asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -281,14 +280,14 @@ attend_umma_kernel(AttendParams p) {
         }
         return;
     }
-    if (warp == 3) {                                                  // spare warp of the first warpgroup
-        named_arrive(1, C::kThreads);
-        return;
-    }
-
-    if (warp == 1 || warp == 2) {
-        // ================================ MMA issuer of slot `slot` ================================
-        const int32_t slot = warp - 1;
+    if (warp >= 1 && warp <= 3) {
+        // ================================ MMA issuers ================================
+        // Warp 1 issues Q K^T for both slots, warps 2 / 3 issue P V of slot 0 / 1.  A single thread
+        // gets one tcgen05.mma out every ~110-130 cycles (measured), so the 32 MMAs of a half-stage
+        // are spread over three issuing threads (a fourth warp would put 4 warps on one SM
+        // sub-partition and cap everyone at 128 registers).
+        const bool is_pv = warp >= 2;
+        const int32_t slot = is_pv ? warp - 2 : 0;
         if (warp == 1) {
             asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;"
                          ::"r"(smem_u32(const_cast<uint32_t*>(tmem_slot))), "r"(C::kTmemCols));
@@ -300,8 +299,7 @@ attend_umma_kernel(AttendParams p) {
         const uint32_t tmem = *tmem_slot;
         constexpr uint32_t idesc_qk = umma_idesc(C::KS * kBlockTokens, false);
         constexpr uint32_t idesc_pv = umma_idesc(D, true);
-        const uint32_t tSbase = tmem + C::kColS + 128 * slot, tOacc = tmem + C::kColO + D * slot;
-        const uint32_t qb = sQ + (two ? slot : 0) * C::kQBytes;
+        const uint32_t tSbase = tmem + C::kColS + 128 * slot, tOacc = tmem + C::kColO + D * slot;      // (P V warps)
 
         auto wait_full = [&](int32_t e) {
             mbar_wait(bar_full(e % C::NBUF), (e / C::NBUF) & 1);
@@ -310,16 +308,16 @@ attend_umma_kernel(AttendParams p) {
         auto release = [&](int32_t e) { if (lane == 0) umma_commit(bar_empty(e % C::NBUF)); };
         // S[buf] = Q K^T over the K half-stage in ring entry e
         const uint32_t elect = lane == 0 ? 1u : 0u;
-        const uint64_t dq0 = umma_desc(qb, 16, 1024);
-        auto issue_qk = [&](int32_t buf, int32_t e) {
+        auto issue_qk = [&](int32_t qslot, int32_t buf, int32_t e) {
             // descriptors = base + (byte offset >> 4) in the address field (no carry: shared memory < 256 KB)
+            const uint64_t dq0 = umma_desc(sQ + (two ? qslot : 0) * C::kQBytes, 16, 1024);
             const uint64_t dk0 = umma_desc(sRing + (e % C::NBUF) * C::kBufBytes, 16, 1024);
-            const uint32_t ts = tSbase + 64 * buf;
+            const uint32_t ts = tmem + C::kColS + 128 * qslot + 64 * buf;
 #pragma unroll
             for (int kk = 0; kk < D / 16; ++kk)
                 umma_ss_e(ts, dq0 + (uint64_t)(((kk >> 2) * C::kQHalfBytes + (kk & 3) * 32) >> 4),
                           dk0 + (uint64_t)(((kk >> 2) * C::kKHalfBytes + (kk & 3) * 32) >> 4), idesc_qk, kk > 0 ? 1u : 0u, elect);
-            if (lane == 0) umma_commit(bar_s(slot, buf));
+            if (lane == 0) umma_commit(bar_s(qslot, buf));
             __syncwarp();
         };
         // O (+)= P V over the V half-stage in ring entry e: per valid block one K=16 MMA for the hi part of P
@@ -336,7 +334,7 @@ attend_umma_kernel(AttendParams p) {
                     umma_ts_e(tOacc, pa + 16, vd, idesc_pv, 1u, elect);
                 }
             }
-            if (lane == 0) umma_commit(bar_pv(slot));
+            if (lane == 0) umma_commit(bar_pv(slot, buf));
             __syncwarp();
         };
         // V rows past the session's length hold stale or poisoned bytes (0 * NaN = NaN): zero them
@@ -355,40 +353,47 @@ attend_umma_kernel(AttendParams p) {
         // this slot's half-stages: h(k) = k (two) or 2 k + slot
         const int32_t n_mine = two ? n_half : (n_half - slot + 1) >> 1;
         auto half_of = [&](int32_t k) { return two ? k : 2 * k + slot; };
-        for (int32_t k = 0; k < min(2, n_mine); ++k) {
-            const int32_t e = entry_k(half_of(k));
-            wait_full(e);
-            issue_qk(k, e);
-            release(e);
-        }
-        for (int32_t k = 0; k < n_mine; ++k) {
-            const int32_t h = half_of(k), e = entry_v(h), buf = k & 1;
-            const int32_t t0 = tl0 + h * C::KS, nt = min(C::KS, tl1 - t0);
-            MTRACE(slot, 4 * k);
-            wait_full(e);
-            MTRACE(slot, 4 * k + 1);
-            fix_ragged_v(e, t0, nt);
-            mbar_wait(bar_p(slot, buf), (k >> 1) & 1);
-            tc_fence_after();
-            MTRACE(slot, 4 * k + 2);
-            issue_pv(buf, e, nt, k > 0);
-            release(e);
-            MTRACE(slot, 512 + 4 * k);
-            if (k == n_mine - 1 && lane == 0) umma_commit(bar_o(slot));
-            if (k + 2 < n_mine) {
-                const int32_t ek = entry_k(half_of(k + 2));
-                wait_full(ek);
-                MTRACE(slot, 512 + 4 * k + 1);
-                issue_qk(buf, ek);
-                release(ek);
+        if (!is_pv) {
+            // ---- Q K^T of every half-stage h, for both slots (R > 128) or for slot h & 1: into S buffer
+            // k & 1 of the slot (k = the slot's own count), as soon as P V of k - 2 has drained that buffer ----
+            for (int32_t h = 0; h < n_half; ++h) {
+                const int32_t e = entry_k(h);
+                wait_full(e);
+                for (int32_t qs = two ? 0 : (h & 1); qs < (two ? 2 : (h & 1) + 1); ++qs) {
+                    const int32_t k = two ? h : h >> 1, buf = k & 1;
+                    if (k >= 2) {
+                        mbar_wait(bar_pv(qs, buf), ((k >> 1) - 1) & 1);
+                        tc_fence_after();
+                    }
+                    issue_qk(qs, buf, e);
+                    release(e);                          // (one arrival per consuming slot)
+                }
             }
-            MTRACE(slot, 4 * k + 3);
-        }
-        // a phantom half-stage (R <= 128, odd count) belongs to slot 1: hand its two entries back
-        if (!two && slot == 1 && (n_half & 1)) {
-            const int32_t ek = entry_k(n_half), ev = entry_v(n_half);
-            wait_full(ek); if (lane == 0) mbar_arrive(bar_empty(ek % C::NBUF));
-            wait_full(ev); if (lane == 0) mbar_arrive(bar_empty(ev % C::NBUF));
+            if (!two && (n_half & 1)) {                   // phantom half-stage of an odd count: hand the entry back
+                const int32_t ek = entry_k(n_half);
+                wait_full(ek); if (lane == 0) mbar_arrive(bar_empty(ek % C::NBUF));
+            }
+        } else {
+            // ---- P V: half-stage k out of S buffer k & 1, once the softmax has written P there ----
+            for (int32_t k = 0; k < n_mine; ++k) {
+                const int32_t h = half_of(k), e = entry_v(h), buf = k & 1;
+                const int32_t t0 = tl0 + h * C::KS, nt = min(C::KS, tl1 - t0);
+                MTRACE(slot, 4 * k);
+                wait_full(e);
+                MTRACE(slot, 4 * k + 1);
+                fix_ragged_v(e, t0, nt);
+                mbar_wait(bar_p(slot, buf), (k >> 1) & 1);
+                tc_fence_after();
+                MTRACE(slot, 4 * k + 2);
+                issue_pv(buf, e, nt, k > 0);
+                release(e);
+                if (k == n_mine - 1 && lane == 0) umma_commit(bar_o(slot));
+                MTRACE(slot, 4 * k + 3);
+            }
+            if (!two && slot == 1 && (n_half & 1)) {
+                const int32_t ev = entry_v(n_half);
+                wait_full(ev); if (lane == 0) mbar_arrive(bar_empty(ev % C::NBUF));
+            }
         }
         if (warp == 1) {
             // every softmax warp has finished reading TMEM
@@ -495,7 +500,7 @@ attend_umma_kernel(AttendParams p) {
                 const bool need = (m_run - m_used) > 8.f;             // (-inf) - (-inf) = NaN -> false
                 if (__any_sync(0xffffffffu, need)) {
                     // S is double buffered, so P V of the previous half-stage may still be running
-                    mbar_wait(bar_pv(slot), (k - 1) & 1);
+                    mbar_wait(bar_pv(slot, (k - 1) & 1), ((k - 1) >> 1) & 1);
                     tc_fence_after();
                     const float f = (need && m_used != -INFINITY) ? ex2(m_used - m_run) : 1.f;
                     l0 *= f; l1 *= f; l2 *= f; l3 *= f;
