@@ -7,15 +7,18 @@
 // (item, KV head, split-KV segment) and streams its KV ONCE from HBM in half-stages of 4 blocks
 // (64 keys):
 //
-//   warp 0      producer: per half-stage, bulk copies of the K tiles (one 2 KB copy per 64-dim half,
+//   warp 0      producer (physical block ids fetched once, then): per half-stage, bulk copies of the K tiles (one 2 KB copy per 64-dim half,
 //               so the halves of 4 blocks form one UMMA K-major operand) and of the V tiles (a V
 //               tile as laid out in HBM already IS a SWIZZLE_128B MN-major operand of one K=16
 //               MMA), into a ring of 16 KB buffers, mbarrier complete_tx
-//   warps 1, 2  MMA issuers, one per slot (warp 1 also allocates TMEM); per half-stage h:
+//   warps 1-3   MMA issuers (warp 1 also allocates TMEM): warp 1 issues Q K^T for both slots, warps
+//               2 / 3 issue P V of slot 0 / 1 -- one thread only gets a tcgen05.mma out every ~110-130
+//               cycles, so the 32 MMAs of a half-stage are spread over three threads; per half-stage h:
 //                 S = Q K_h^T   (SS form, D/16 instructions 128x64x16)   -> one of TWO S buffers
 //                 O += P_h V_h  (TS form: P read from TMEM, V from shared memory; hi and lo parts)
-//               S is double buffered, so Q K^T of half-stage h+1 is issued BEFORE P V of h: the
-//               softmax warps never wait for the tensor pipe in steady state
+//               S is double buffered, so Q K^T of half-stage h+1 is issued BEFORE P V of h (it only
+//               waits for P V of h-1 to have drained the buffer): the softmax warps never wait for
+//               the tensor pipe in steady state
 //   warps 4-7   softmax warpgroup of slot 0, warps 8-11 of slot 1: ONE THREAD PER QUERY ROW
 //               (tcgen05.ld 32x32b, 64 scores in registers): token-exact union mask on boundary
 //               half-stages, row max and row sum without any shuffle, exp2 in the log2 domain, P split
