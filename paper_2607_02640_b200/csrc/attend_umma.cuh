@@ -7,7 +7,8 @@
 // (item, KV head, split-KV segment) and streams its KV ONCE from HBM in half-stages of 4 blocks
 // (64 keys):
 //
-//   warp 0      producer (physical block ids fetched once, then): per half-stage, bulk copies of the K tiles (one 2 KB copy per 64-dim half,
+//   warp 0      producer (the segment's physical block ids are fetched once): per half-stage, bulk
+//               copies of the K tiles (one 2 KB copy per 64-dim half,
 //               so the halves of 4 blocks form one UMMA K-major operand) and of the V tiles (a V
 //               tile as laid out in HBM already IS a SWIZZLE_128B MN-major operand of one K=16
 //               MMA), into a ring of 16 KB buffers, mbarrier complete_tx
