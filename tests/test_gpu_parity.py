@@ -469,3 +469,19 @@ def test_early_mode_decode_with_constant_eviction_and_reuse():
         assert_parity(out, m.attend(st, 0), f"early-mode step {st.frame}")
     m.check_tables(r.pool)
     _loaded_native()
+
+
+@pytest.mark.parametrize("family", [1, 2])
+def test_two_layers_on_the_fused_path(family):
+    """Layers > 0 repeat layer 0's batch (reading R16): their append kernels only scatter K/V and the
+    work list planned at layer 0's append is reused by every layer's attend_frame (no poison flag here,
+    so this is the fused one-kernel-per-append path, in early mode for family 1)."""
+    _run_parity(wl.make_workload(1), n_layers=2, family=family, check_history_attend_every=4)
+
+
+def test_read_only_stream_microbenchmark_reports_a_plausible_bandwidth():
+    gbs = binding.stream_read_gbs(1 << 30, 3)
+    assert 1000.0 < gbs < 20000.0, gbs
+    with pytest.raises(binding.MetronomeError):
+        binding.stream_read_gbs(1024, 1)
+    _loaded_native()
