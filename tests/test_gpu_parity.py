@@ -485,3 +485,31 @@ def test_read_only_stream_microbenchmark_reports_a_plausible_bandwidth():
     with pytest.raises(binding.MetronomeError):
         binding.stream_read_gbs(1024, 1)
     _loaded_native()
+
+
+def test_chunk_kernel_on_a_segment_longer_than_256_tiles():
+    """A window of 4400 tokens gives a chunk-prefill segment of 276 tiles: beyond the 256 block ids the
+    producer warp keeps in registers, it looks the table up per entry.  Two row tiles (200 rows) and one."""
+    S, W, D, G = 4, 4400, 128, 8
+    rng = np.random.default_rng(31)
+    kw = dict(n_q_heads=G, n_kv_heads=1, head_dim=D, max_sessions=1, max_new_tokens=25)
+    pool = binding.Pool(n_sinks=S, window=W, n_blocks=300, **kw)
+    pool.set_tuning(0, 2)
+    ora = O.DefinitionOracle(O.PoolConfig(S=S, W=W, n_blocks=300, block_size=16, **kw))
+    sid = pool.session_open()
+    assert sid == ora.session_open()
+    total = 0
+    for step in range(255):
+        n = 25 if step % 2 == 0 else 11
+        k, v = rng.standard_normal((2, n, 1, D)).astype(np.float32)
+        q = rng.standard_normal((n, G, D)).astype(np.float32)
+        kb, vb, qb = (torch.from_numpy(a).to(torch.bfloat16).cuda() for a in (k, v, q))
+        pool.append_kv(0, [sid], [n], kb, vb)
+        ora.append_kv(0, [sid], [n], synth.to_u16(kb), synth.to_u16(vb))
+        total += n
+        if total > 4100:                     # attend only once the segment is long (keeps the oracle cheap)
+            out = torch.empty_like(qb)
+            pool.attend_frame(0, [sid], [n], qb, out)
+            assert_parity(out, ora.attend_frame(0, [sid], [n], synth.to_u16(qb)), f"long segment step {step} len {total}")
+    assert total > 16 * 256 + 25
+    _loaded_native()
