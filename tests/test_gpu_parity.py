@@ -437,7 +437,8 @@ def test_empty_batches_and_zero_length_items():
     _loaded_native()
 
 
-def test_early_mode_decode_with_constant_eviction_and_reuse():
+@pytest.mark.parametrize("side_stream", [False, True])
+def test_early_mode_decode_with_constant_eviction_and_reuse(side_stream):
     """Multi-head decode runs in 'early mode': the row kernel of step k streams the blocks the append of
     step k does not touch while that append (and the tail of step k-1's attention) is still running.
     A small window makes every session free a block every 16 steps, and the freed blocks are reused at
@@ -460,9 +461,11 @@ def test_early_mode_decode_with_constant_eviction_and_reuse():
             r.rows(synth.STREAM_Q, 0, st.uid_rows, st.pos_rows)) for st in steps]
     outs = [torch.empty_like(q) for _, _, q in kvq]
     torch.cuda.synchronize()
+    stream = torch.cuda.Stream() if side_stream else None      # the caller's own stream, or the default one
+    handle = stream.cuda_stream if side_stream else 0
     for st, (k, v, q), o in zip(steps, kvq, outs):     # no host sync inside: the kernels run back to back
-        r.pool.append_kv(0, st.sids, st.n_new, k, v)
-        r.pool.attend_frame(0, st.sids, st.n_new, q, o)
+        r.pool.append_kv(0, st.sids, st.n_new, k, v, handle)
+        r.pool.attend_frame(0, st.sids, st.n_new, q, o, handle)
     torch.cuda.synchronize()
     for st, out in zip(steps, outs):
         m.append(st, 0)
