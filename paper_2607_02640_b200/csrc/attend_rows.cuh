@@ -66,8 +66,9 @@ attend_rows_kernel(AttendParams p) {
     }
 
     float m = -INFINITY, l = 0.f, acc[8];
+    uint64_t acc2[4] = {0ull, 0ull, 0ull, 0ull}, q2[4];           // packed (even, odd) accumulators / query
 #pragma unroll
-    for (int k = 0; k < 8; ++k) acc[k] = 0.f;
+    for (int k = 0; k < 4; ++k) q2[k] = f2_pack(qf[2 * k], qf[2 * k + 1]);
 
     const int32_t* trow = p.table + (int64_t)it.sid * p.tbl_width;
     const int32_t tl0 = split * it.tiles_per_split;
@@ -111,12 +112,12 @@ attend_rows_kernel(AttendParams p) {
 #pragma unroll
         for (int j = 0; j < STEPS; ++j) {
             const uint32_t w[4] = {kr[j].x, kr[j].y, kr[j].z, kr[j].w};
-            float d = 0.f;
+            uint64_t d2 = 0ull;                                   // (even, odd) partial sums, FFMA2
 #pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                d = fmaf(qf[2 * k], bf16lo(w[k]), d);
-                d = fmaf(qf[2 * k + 1], bf16hi(w[k]), d);
-            }
+            for (int k = 0; k < 4; ++k) d2 = f2_fma(q2[k], f2_pack(bf16lo(w[k]), bf16hi(w[k])), d2);
+            float de, dodd;
+            f2_unpack(d2, de, dodd);
+            float d = de + dodd;
 #pragma unroll
             for (int o = LPT / 2; o >= 1; o >>= 1) d += __shfl_xor_sync(0xffffffffu, d, o);
             s[j] = d;
@@ -147,18 +148,17 @@ attend_rows_kernel(AttendParams p) {
         if (mn != -INFINITY) {            // (uniform inside a token group)
             const float corr = ex2(m - mn);
             l *= corr;
+            const uint64_t corr2 = f2_pack(corr, corr);
 #pragma unroll
-            for (int k = 0; k < 8; ++k) acc[k] *= corr;
+            for (int k = 0; k < 4; ++k) acc2[k] = f2_mul(acc2[k], corr2);
 #pragma unroll
             for (int j = 0; j < STEPS; ++j) {
                 const float pj = ex2(s[j] - mn);
                 l += pj;
+                const uint64_t pj2 = f2_pack(pj, pj);
                 const uint32_t w[4] = {vr[j].x, vr[j].y, vr[j].z, vr[j].w};
 #pragma unroll
-                for (int k = 0; k < 4; ++k) {
-                    acc[2 * k] = fmaf(pj, bf16lo(w[k]), acc[2 * k]);
-                    acc[2 * k + 1] = fmaf(pj, bf16hi(w[k]), acc[2 * k + 1]);
-                }
+                for (int k = 0; k < 4; ++k) acc2[k] = f2_fma(pj2, f2_pack(bf16lo(w[k]), bf16hi(w[k])), acc2[k]);
             }
             m = mn;
         }
@@ -171,6 +171,8 @@ attend_rows_kernel(AttendParams p) {
     }
 
     pdl_wait();       // nothing is written before the predecessor (and the kernels before it) are over
+#pragma unroll
+    for (int k = 0; k < 4; ++k) f2_unpack(acc2[k], acc[2 * k], acc[2 * k + 1]);
     // combine the token groups of the warp
 #pragma unroll
     for (int o = 16; o >= LPT; o >>= 1) {
