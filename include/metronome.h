@@ -136,6 +136,9 @@ int metronome_session_close(metronome_pool_t* pool, int32_t sid, void* cuda_stre
  *       check    free + freed >= needed, else POOL_EXHAUSTED and nothing has changed;
  *       phase 2  every session pops ceil(L1/B) - ceil(L0/B) blocks, ascending logical order.
  *   layer  > 0  : must repeat layer 0's most recent batch exactly; only writes K/V of that layer.
+ * One kernel launch (bookkeeping + K/V scatter); k_new / v_new are read by that kernel in stream order,
+ * the host arrays before the call returns.  Calls on one pool must be ordered on ONE stream.  The call
+ * also plans the usual attend_frame(q_lens = n_new) of this step, so that call needs no upload.
  * Errors: INVALID_ARG, INVALID_SESSION, DUPLICATE_SESSION, CHUNK_TOO_LARGE, LEN_OVERFLOW,
  *         POOL_EXHAUSTED, LAYER_SEQUENCE, CUDA. */
 int metronome_append_kv(metronome_pool_t* pool, int32_t layer, int32_t n_batch,
