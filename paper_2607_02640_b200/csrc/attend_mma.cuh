@@ -285,6 +285,21 @@ struct GqaPlan {
     __host__ __device__ int32_t max_pieces(int32_t n) const { return (int32_t)((n + q2 - 1) / q2) + 2; }
 };
 
+// Host: cut `total_tiles` into one static range per CTA and, when `dynamic`, keep the last 10 % for
+// small ranges (a sixth of a static one, at least 8 tiles) that the CTAs claim as they finish.
+inline GqaPlan make_gqa_plan(int32_t n_kv_heads, int64_t total_tiles, int64_t ctas, bool dynamic) {
+    GqaPlan g{};
+    g.n_kv_heads = n_kv_heads;
+    g.total_tiles = total_tiles;
+    const int64_t share = (total_tiles + ctas - 1) / ctas;
+    g.q1 = dynamic ? (share * 9 + 9) / 10 : share;
+    g.n_static = (int32_t)(dynamic ? ctas : (total_tiles + g.q1 - 1) / g.q1);
+    g.g1 = g.q1 * g.n_static < total_tiles ? g.q1 * g.n_static : total_tiles;
+    g.q2 = dynamic ? (g.q1 / 6 > 8 ? g.q1 / 6 : 8) : g.q1;
+    g.n_total = g.n_static + (int32_t)((total_tiles - g.g1 + g.q2 - 1) / g.q2);
+    return g;
+}
+
 // grid = n_SM * CTAs/SM (<= total tiles), block = 128.  items[].tile_off = exclusive prefix of n_tiles.
 template <int D>
 __global__ void __launch_bounds__(GqaCfg<D>::kThreads)

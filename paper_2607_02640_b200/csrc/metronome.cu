@@ -288,24 +288,18 @@ int plan_attend(metronome_pool* pool, int32_t n_batch, const int32_t* sids, cons
         if (family == 2 && cls == 0) {
             // stream-K: one wave of n_SM x 3 CTAs, equal static ranges (one per CTA); for long shares the
             // last 10 % of the flattened tile list is cut into small ranges claimed dynamically.
-            GqaPlan& g = pl.gplan;
-            g.n_kv_heads = c.n_kv_heads;
-            g.total_tiles = cls_tiles[0] * c.n_kv_heads;
+            const int64_t total_tiles = cls_tiles[0] * c.n_kv_heads;
             int64_t ctas = (int64_t)pool->n_sm * 3;
             const int64_t min_tiles = pool->tune_split_tokens > 0 ? (pool->tune_split_tokens + 15) / 16 : 8;
-            if (ctas > (g.total_tiles + min_tiles - 1) / min_tiles) ctas = (g.total_tiles + min_tiles - 1) / min_tiles;
-            if (pool->tune_split_tokens > 0) ctas = (g.total_tiles + min_tiles - 1) / min_tiles;
+            if (ctas > (total_tiles + min_tiles - 1) / min_tiles) ctas = (total_tiles + min_tiles - 1) / min_tiles;
+            if (pool->tune_split_tokens > 0) ctas = (total_tiles + min_tiles - 1) / min_tiles;
             if (ctas < 1) ctas = 1;
-            const int64_t share = (g.total_tiles + ctas - 1) / ctas;
             // measured on B200: the dynamic tail pays (-2 % on config 5) only when a CTA's share is long
             // (>= 512 tiles = 4 MB); for shorter shares the restart of a claimed range costs more than the
             // imbalance it removes (configs 3 and 4: +3..7 %), so they stay fully static
-            const bool dynamic = pool->tune_split_tokens <= 0 && share >= 512;
-            g.q1 = dynamic ? (share * 9 + 9) / 10 : share;
-            g.n_static = (int32_t)(dynamic ? ctas : (g.total_tiles + g.q1 - 1) / g.q1);
-            g.g1 = std::min<int64_t>(g.total_tiles, g.q1 * g.n_static);
-            g.q2 = dynamic ? std::max<int64_t>(8, g.q1 / 6) : g.q1;
-            g.n_total = g.n_static + (int32_t)((g.total_tiles - g.g1 + g.q2 - 1) / g.q2);
+            const bool dynamic = pool->tune_split_tokens <= 0 && (total_tiles + ctas - 1) / ctas >= 512;
+            pl.gplan = make_gqa_plan(c.n_kv_heads, total_tiles, ctas, dynamic);
+            GqaPlan& g = pl.gplan;
             pl.gqa_ctas = g.n_static;
             if (g.n_total <= kMaxRangeItems) {
                 int32_t* range_item = reinterpret_cast<int32_t*>(items + n_items);    // after ALL items
