@@ -12,7 +12,10 @@
  *
  * Conventions
  *   - All functions return an int status (METRONOME_OK = 0).  No exceptions, no aborts.
- *     On ANY error the pool's state (host and device) is unchanged.
+ *     On ANY error the pool's state (host and device) is unchanged.  (One exception, stated where it
+ *     applies: a CUDA launch failure that FOLLOWS a kernel the same call has already enqueued, which
+ *     only the poison / bookkeeping-only debug modes can see, leaves the CUDA context in its sticky
+ *     error state and the pool unusable.)
  *   - "host" pointers are ordinary CPU memory, read or written before the call returns.
  *     "device" pointers are CUDA global memory on the pool's device; they are consumed
  *     asynchronously on `cuda_stream` (a cudaStream_t passed as void*; NULL = default stream).
@@ -35,7 +38,7 @@
 extern "C" {
 #endif
 
-#define METRONOME_ABI_VERSION 1
+#define METRONOME_ABI_VERSION 2
 
 /* ---- status codes --------------------------------------------------------------------------- */
 enum {
@@ -80,7 +83,7 @@ typedef struct metronome_pool_config {
                                 METRONOME_FLAG_BOOKKEEPING_ONLY                                    */
     int32_t n_sinks;         /* S >= 0: pinned attention-sink tokens (L101)                        */
     int32_t window;          /* W >= 1: most recent tokens kept, the query's own included          */
-    int32_t max_sessions;    /* session slots, 1..65536                                            */
+    int32_t max_sessions;    /* session slots, 1..65534                                            */
     int32_t max_new_tokens;  /* largest n_new of one session in one append_kv (chunk length)       */
     int32_t n_blocks;        /* size of the fixed KV block pool (L60)                              */
     float   softmax_scale;   /* 0 -> 1/sqrt(D)                                                     */
@@ -152,6 +155,10 @@ int metronome_append_kv(metronome_pool_t* pool, int32_t layer, int32_t n_batch,
  *   sids, q_lens : host int32 [n_batch]; 0 <= q_lens[i] <= n_new of that session's last append
  *   q, out       : device bf16 [sum(q_lens), n_q_heads, head_dim], rows in batch order
  * The layer must have been appended in the current step (since the last layer-0 append).
+ * q must be complete on cuda_stream when the call is enqueued; when it repeats the batch of this
+ * step's append_kv (the usual case) its kernel may begin -- reading q and blocks no append is still
+ * writing -- while that append kernel runs, so q must not be produced by work enqueued on another
+ * stream without an event the caller has waited on.
  * Errors: INVALID_ARG, INVALID_SESSION, DUPLICATE_SESSION, QLEN_EXCEEDS_LAST_APPEND,
  *         LAYER_SEQUENCE, UNSUPPORTED, CUDA. */
 int metronome_attend_frame(metronome_pool_t* pool, int32_t layer, int32_t n_batch,
@@ -185,24 +192,6 @@ int metronome_pool_query(metronome_pool_t* pool, void* cuda_stream, int32_t* n_f
 int metronome_read_kv(metronome_pool_t* pool, int32_t layer, int32_t sid, int64_t pos0, int32_t n,
                       void* k_out, void* v_out, void* cuda_stream);
 
-/* Counters since pool_create: kernels launched by the library, append / attend calls.  host. */
-int metronome_pool_stats(metronome_pool_t* pool, int64_t* kernel_launches, int64_t* append_calls,
-                         int64_t* attend_calls);
-
-/* Tuning knob (0 = automatic): keys per split-KV segment target, and forcing the kernel family
- * (0 auto, 1 CUDA-core row kernel, 2 tensor-core kernels: mma.sync GQA decode + tcgen05 chunk prefill).
- * For benchmarks and tests of "both launch modes" (L258).
- * Errors: INVALID_ARG. */
-int metronome_pool_set_tuning(metronome_pool_t* pool, int32_t split_tokens, int32_t kernel_family);
-
-/* Measurement aid.  While enabled, attend_frame brackets its attention kernel (the dominant
- * kernel; not the metadata copy, not the merge) with CUDA events on the caller's stream.
- * read_profile waits for those events, returns the summed kernel time in milliseconds and the
- * number of bracketed launches since the last reset, and (reset != 0) clears them.  host. */
-int metronome_pool_set_profiling(metronome_pool_t* pool, int32_t enable);
-int metronome_pool_read_profile(metronome_pool_t* pool, double* attend_kernel_ms, int64_t* attend_kernel_launches,
-                                int32_t reset);
-
 /* ---- NEXT row f3: deadline-aware admission on the per-frame latency signal ----
  * PAPER.md:L105-111 sec. 4.2: "an AIMD loop on the measured per-frame latency, which lowers the
  * admission cap multiplicatively when latency nears a target fraction of the budget and raises it
@@ -227,14 +216,6 @@ int metronome_gate_create(const metronome_gate_config_t* cfg, metronome_gate_t**
 int metronome_gate_destroy(metronome_gate_t* gate);
 int metronome_gate_observe(metronome_gate_t* gate, float frame_latency_ms, float* cap_out);
 int metronome_gate_admit(metronome_gate_t* gate, int32_t n_live, int32_t* admitted_out);
-
-/* Measurement aid ("plus a read-only stream microbenchmark run in the same job").
- * Streams `bytes` of a scratch device buffer (allocated and freed inside) `reps` times with 16-byte
- * loads from every SM and returns the best read-only bandwidth in GB/s in *gbs_out: the ceiling a pure
- * KV stream can reach on this GPU, next to the read+write copy figure of MEASURED_PEAKS.json.
- * Blocking; uses the current device and `cuda_stream`.  Errors: INVALID_ARG (bytes < 1 MiB, reps < 1,
- * null), OUT_OF_MEMORY, CUDA. */
-int metronome_stream_read_gbs(size_t bytes, int32_t reps, void* cuda_stream, double* gbs_out);
 
 const char* metronome_strerror(int status);
 /* Text of the last CUDA error seen by this pool ("" if none).  Valid until the next call. */

@@ -1,0 +1,52 @@
+/*
+ * metronome_measure.h -- measurement and test aids of libmetronome.so.  NOT part of the product
+ * boundary (include/metronome.h): nothing here is needed to serve a frame.
+ * bench.py, the sweeps next to it and tests/ use these; a serving engine would not.
+ */
+#ifndef METRONOME_MEASURE_H_
+#define METRONOME_MEASURE_H_
+
+#include "metronome.h"
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* Counters since pool_create: kernels launched by the library, append / attend calls.  host. */
+int metronome_pool_stats(metronome_pool_t* pool, int64_t* kernel_launches, int64_t* append_calls,
+                         int64_t* attend_calls);
+
+/* Tuning knobs (0 = automatic): keys per split-KV segment target; the kernel family (1 CUDA-core row
+ * kernel, 2 tensor-core kernels: mma.sync GQA decode + tcgen05 chunk prefill); the GQA decode kernel's
+ * dynamically claimed tail ranges (1 forced on, 2 forced off; automatic = on for shares >= 512 tiles).
+ * For benchmarks and tests of "both launch modes" (L258).  Errors: INVALID_ARG. */
+int metronome_pool_set_tuning(metronome_pool_t* pool, int32_t split_tokens, int32_t kernel_family,
+                              int32_t gqa_dynamic);
+
+/* Test aid for the "no state change on error" contract: the NEXT append_kv(layer 0) fails as if
+ * (stage 1) growing the split-KV workspace had run out of memory, or (stage 2) the launch of the append
+ * kernel had failed -- both sit after the point where the shadow counts are tentatively committed.
+ * One-shot; stage 0 disarms.  Errors: INVALID_ARG. */
+int metronome_pool_debug_fail_next(metronome_pool_t* pool, int32_t stage);
+
+/* Measurement aid.  While enabled, attend_frame brackets its attention kernel (the dominant
+ * kernel; not the metadata copy, not the merge) with CUDA events on the caller's stream.
+ * read_profile waits for those events, returns the summed kernel time in milliseconds and the
+ * number of bracketed launches since the last reset, and (reset != 0) clears them.  host. */
+int metronome_pool_set_profiling(metronome_pool_t* pool, int32_t enable);
+int metronome_pool_read_profile(metronome_pool_t* pool, double* attend_kernel_ms, int64_t* attend_kernel_launches,
+                                int32_t reset);
+
+
+/* Measurement aid ("plus a read-only stream microbenchmark run in the same job").
+ * Streams `bytes` of a scratch device buffer (allocated and freed inside) `reps` times with 16-byte
+ * loads from every SM and returns the best read-only bandwidth in GB/s in *gbs_out: the ceiling a pure
+ * KV stream can reach on this GPU, next to the read+write copy figure of MEASURED_PEAKS.json.
+ * Blocking; uses the current device and `cuda_stream`.  Errors: INVALID_ARG (bytes < 1 MiB, reps < 1,
+ * null), OUT_OF_MEMORY, CUDA. */
+int metronome_stream_read_gbs(size_t bytes, int32_t reps, void* cuda_stream, double* gbs_out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* METRONOME_MEASURE_H_ */

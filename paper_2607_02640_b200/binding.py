@@ -1,4 +1,4 @@
-"""Thin ctypes mirror of include/metronome.h -- argument marshalling only.
+"""Thin ctypes mirror of include/metronome.h (+ the aids of include/metronome_measure.h) -- argument marshalling only.
 
 Every step of the path runs in libmetronome.so's CUDA kernels; torch is used by callers for device
 memory and streams.  There is NO fallback: if the library is missing or a call fails, this raises.
@@ -22,13 +22,13 @@ ERR_NAMES = {0: "OK", 1: "INVALID_ARG", 2: "INVALID_SESSION", 3: "DUPLICATE_SESS
              5: "POOL_EXHAUSTED", 6: "CHUNK_TOO_LARGE", 7: "QLEN_EXCEEDS_LAST_APPEND", 8: "LAYER_SEQUENCE",
              9: "LEN_OVERFLOW", 10: "CUDA", 11: "UNSUPPORTED", 12: "OUT_OF_MEMORY"}
 
-# every symbol include/metronome.h declares
+# every symbol include/metronome.h and include/metronome_measure.h declare
 EXPORTS = ["metronome_abi_version", "metronome_strerror", "metronome_last_cuda_error",
            "metronome_kv_storage_bytes", "metronome_max_blocks_per_session", "metronome_pool_create",
            "metronome_pool_destroy", "metronome_session_open", "metronome_session_close",
            "metronome_append_kv", "metronome_attend_frame", "metronome_step_host",
            "metronome_session_query", "metronome_pool_query", "metronome_read_kv", "metronome_pool_stats",
-           "metronome_pool_set_tuning", "metronome_pool_set_profiling", "metronome_pool_read_profile",
+           "metronome_pool_set_tuning", "metronome_pool_debug_fail_next", "metronome_pool_set_profiling", "metronome_pool_read_profile",
            "metronome_gate_create", "metronome_gate_destroy", "metronome_gate_observe", "metronome_gate_admit",
            "metronome_stream_read_gbs"]
 
@@ -81,7 +81,8 @@ def load():
     lib.metronome_pool_query.argtypes = [c_void_p, c_void_p, i32p, i32p]
     lib.metronome_read_kv.argtypes = [c_void_p, c_int32, c_int32, c_int64, c_int32, c_void_p, c_void_p, c_void_p]
     lib.metronome_pool_stats.argtypes = [c_void_p, POINTER(c_int64), POINTER(c_int64), POINTER(c_int64)]
-    lib.metronome_pool_set_tuning.argtypes = [c_void_p, c_int32, c_int32]
+    lib.metronome_pool_set_tuning.argtypes = [c_void_p, c_int32, c_int32, c_int32]
+    lib.metronome_pool_debug_fail_next.argtypes = [c_void_p, c_int32]
     lib.metronome_pool_set_profiling.argtypes = [c_void_p, c_int32]
     lib.metronome_pool_read_profile.argtypes = [c_void_p, POINTER(ctypes.c_double), POINTER(c_int64), c_int32]
     lib.metronome_gate_create.argtypes = [c_void_p, POINTER(c_void_p)]
@@ -199,8 +200,11 @@ class Pool:
         self._check(self._lib.metronome_pool_stats(self._h, byref(a), byref(b), byref(c)))
         return {"kernel_launches": a.value, "append_calls": b.value, "attend_calls": c.value}
 
-    def set_tuning(self, split_tokens=0, kernel_family=0):
-        self._check(self._lib.metronome_pool_set_tuning(self._h, split_tokens, kernel_family))
+    def set_tuning(self, split_tokens=0, kernel_family=0, gqa_dynamic=0):
+        self._check(self._lib.metronome_pool_set_tuning(self._h, split_tokens, kernel_family, gqa_dynamic))
+
+    def debug_fail_next(self, stage: int):
+        self._check(self._lib.metronome_pool_debug_fail_next(self._h, stage))
 
     def set_profiling(self, enable: bool):
         self._check(self._lib.metronome_pool_set_profiling(self._h, int(enable)))

@@ -24,7 +24,10 @@ struct AttendItem {
     int32_t tiles_per_split;
     int32_t tile_off;         // exclusive prefix sum of n_tiles over the items of this launch
     int32_t class_row_off;    // exclusive prefix sum of q_len over the items of this launch
+    int32_t fresh_blk;        // early mode: first logical block an append kernel may still be writing (see wait_work_list)
+    int32_t pad0, pad1, pad2; // 64 bytes: the list travels in 16-byte chunks
 };
+static_assert(sizeof(AttendItem) == 64, "AttendItem is copied in 16-byte chunks");
 
 struct AttendParams {
     const AttendItem* items;
@@ -52,9 +55,11 @@ struct AttendParams {
 // Start of an attention kernel.  In early mode (items_epoch >= 0: launched programmatically behind an
 // append kernel that triggered its dependents at once) the kernel may run NEXT TO the kernels before
 // it: it only waits for its work list here, streams every block the append does not touch, and calls
-// pdl_wait() before the first FRESH block of an item (blocks that hold the rows appended in this
-// step: logical block >= (len - q_len) / 16) and before it writes anything.  Otherwise the
-// predecessor is waited for right away.  One thread per CTA; the caller syncs.
+// pdl_wait() before the first FRESH block of an item (AttendItem::fresh_blk, from the host: the block
+// that holds the oldest row appended in this step OR in the step before it -- the append kernel of
+// step e-1 is only known to be past its own wait when this kernel starts, not to be complete) and
+// before it writes anything.  Otherwise the predecessor is waited for right away.  One thread per
+// CTA; the caller syncs.
 __device__ __forceinline__ void wait_work_list(const AttendParams& p) {
     if (p.items_epoch < 0) { pdl_wait(); return; }
     int32_t seen;                       // (>=: a later step's list may already be out, in the other buffer)
@@ -63,7 +68,6 @@ __device__ __forceinline__ void wait_work_list(const AttendParams& p) {
         if (seen - p.items_epoch < 0) __nanosleep(64);
     } while (seen - p.items_epoch < 0);
 }
-__device__ __forceinline__ int32_t fresh_block(const AttendItem& it) { return (it.len - it.q_len) / kBlockTokens; }
 
 __device__ __forceinline__ float ex2(float x) {
     float y;

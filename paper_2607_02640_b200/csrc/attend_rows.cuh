@@ -87,7 +87,7 @@ attend_rows_kernel(AttendParams p) {
         }
         return tile;
     };
-    const int32_t fresh = fresh_block(it);
+    const int32_t fresh = it.fresh_blk;
     auto tile_ptr = [&](int32_t tile) {
         if (block_of(tile) >= fresh) pdl_wait();        // rows (and maybe the block) of this step's append
         const int32_t phys = __ldg(trow + table_slot(block_of(tile), p.n_sink, p.ring));

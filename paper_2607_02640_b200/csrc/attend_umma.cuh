@@ -37,20 +37,6 @@
 
 namespace metronome {
 
-// Timeline probe for the microbenchmark harness (compiled out of the library): clock64 stamps of
-// one CTA's roles.
-#ifdef METRONOME_TRACE
-__device__ long long g_trace[4 * 1024];
-__device__ int g_trace_cta = 0;
-#define MTRACE(role, idx)                                                                        \
-    do {                                                                                        \
-        if (blockIdx.x == 0 && (int)blockIdx.y == g_trace_cta && (threadIdx.x & 31) == 0 && (idx) < 1024) \
-            g_trace[(role) * 1024 + (idx)] = clock64();                                         \
-    } while (0)
-#else
-#define MTRACE(role, idx) do { } while (0)
-#endif
-
 template <int D>
 struct UmmaCfg {
     static constexpr int KS = 4;                          // KV blocks per half-stage (64 keys)
@@ -360,17 +346,13 @@ attend_umma_kernel(AttendParams p) {
             for (int32_t k = 0; k < n_mine; ++k) {
                 const int32_t h = half_of(k), e = entry_v(h), buf = k & 1;
                 const int32_t t0 = tl0 + h * C::KS, nt = min(C::KS, tl1 - t0);
-                MTRACE(slot, 4 * k);
                 wait_full(e);
-                MTRACE(slot, 4 * k + 1);
                 fix_ragged_v(e, t0, nt);
                 mbar_wait(bar_p(slot, buf), (k >> 1) & 1);
                 tc_fence_after();
-                MTRACE(slot, 4 * k + 2);
                 issue_pv(buf, e, nt, k > 0);
                 release(e);
                 if (k == n_mine - 1 && lane == 0) umma_commit(bar_o(slot));
-                MTRACE(slot, 4 * k + 3);
             }
             if (!two && slot == 1 && (n_half & 1)) {
                 const int32_t ev = entry_v(n_half);
@@ -387,7 +369,6 @@ attend_umma_kernel(AttendParams p) {
     }
 
     // ================================ softmax warps ================================
-    if ((warp & 3) == 0) MTRACE(2 + ((warp - 4) >> 2), 1002);
     const int32_t slot = (warp - 4) >> 2, quarter = warp & 3;       // TMEM lanes 32 (warp % 4) .. + 31
     const int32_t row = quarter * 32 + lane;
     const int32_t tile_row0 = two ? 128 * slot : 0;
@@ -421,7 +402,6 @@ attend_umma_kernel(AttendParams p) {
     }
     named_sync(1, C::kThreads);
     tc_fence_after();
-    if ((warp & 3) == 0) MTRACE(2 + ((warp - 4) >> 2), 1003);
     const uint32_t tmem = *tmem_slot;
     const uint32_t lane_base = (uint32_t)(quarter * 32) << 16;
     const uint32_t tS = tmem + lane_base + C::kColS + 128 * slot;     // two 64-column S buffers; P (bf16 hi | lo) goes over S
@@ -434,10 +414,8 @@ attend_umma_kernel(AttendParams p) {
     const int32_t n_mine = two ? n_half : (n_half - slot + 1) >> 1;
     for (int32_t k = 0; k < n_mine; ++k) {
         const int32_t h = two ? k : 2 * k + slot, buf = k & 1;
-        if (quarter == 0) MTRACE(2 + slot, 4 * k);
         mbar_wait(bar_s(slot, buf), (k >> 1) & 1);
         tc_fence_after();
-        if (quarter == 0) MTRACE(2 + slot, 4 * k + 1);
         if (warp_active) {
             const uint32_t tSb = tS + 64 * buf;
             uint32_t sa[32], sb[32];
@@ -530,12 +508,10 @@ attend_umma_kernel(AttendParams p) {
             f2_unpack(lB, l2, l3);
             tmem_wait_st();
         }
-        if (quarter == 0) MTRACE(2 + slot, 4 * k + 2);
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(bar_p(slot, buf));
     }
-    if (quarter == 0) MTRACE(2 + slot, 1000);
     float l = (l0 + l1) + (l2 + l3);
     const int32_t n_it = n_mine;
 
@@ -618,7 +594,6 @@ attend_umma_kernel(AttendParams p) {
             }
         }
     }
-    if (quarter == 0) MTRACE(2 + slot, 1001);
     tc_fence_before();
     named_arrive(2, 32 + 256);
 }

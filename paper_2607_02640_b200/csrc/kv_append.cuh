@@ -12,32 +12,6 @@
 
 namespace metronome {
 
-// grid = (ceil(max_n_new * Hkv * D/8 / 256), n_items), block = 256
-__global__ void __launch_bounds__(256)
-kv_append_kernel(const AppendItem* __restrict__ items, const int32_t* __restrict__ table, int32_t tbl_width,
-                 int32_t n_sink, int32_t ring, const uint4* __restrict__ k_new, const uint4* __restrict__ v_new,
-                 uint8_t* __restrict__ kv_layer, KvLayout L) {
-    const AppendItem it = items[blockIdx.y];
-    const int32_t chunks_per_row = L.head_dim >> 3;
-    const int32_t chunks_per_tok = L.n_kv_heads * chunks_per_row;
-    const int32_t idx = blockIdx.x * blockDim.x + threadIdx.x;
-    if (idx >= it.n_new * chunks_per_tok) return;
-    const int32_t tok = idx / chunks_per_tok;
-    const int32_t rem = idx - tok * chunks_per_tok;
-    const int32_t h = rem / chunks_per_row;
-    const int32_t c = rem - h * chunks_per_row;
-    const int32_t pos = it.len0 + tok;
-    const int32_t blk = pos / kBlockTokens, r = pos % kBlockTokens;
-    const int32_t phys = table[(int64_t)it.sid * tbl_width + table_slot(blk, n_sink, ring)];
-    const int64_t src = (int64_t)(it.row_off + tok) * chunks_per_tok + rem;
-    uint8_t* tile = kv_layer + (int64_t)phys * L.block_bytes + (int64_t)h * L.head_bytes;
-    const int32_t off = tile_chunk_offset(r, c);
-    const uint4 kk = __ldg(k_new + src);
-    const uint4 vv = __ldg(v_new + src);
-    *reinterpret_cast<uint4*>(tile + off) = kk;
-    *reinterpret_cast<uint4*>(tile + L.tile_bytes + off) = vv;
-}
-
 // ------------------------------------------------------------------------------------------------
 // One launch per append_kv call: rows a2 + a3 (bookkeeping) and a4 (KV scatter) fused, and the
 // attention work list of the same step (row a8) carried to the device on the way.

@@ -5,6 +5,7 @@
 // raised synchronously and before anything changes, while the physical block ids (block tables,
 // free stack) live on the device and are only ever touched by kernels on the caller's stream.
 #include "../../include/metronome.h"
+#include "../../include/metronome_measure.h"
 
 #include <cmath>
 #include <cstdio>
@@ -31,6 +32,9 @@ struct Session {
     int64_t len = 0;
     int32_t first_live = 0;   // first logical non-sink block still resident
     int32_t last_n = 0;       // n_new of this session's most recent append
+    int64_t last_epoch = 0;   // pool epoch of that append
+    int32_t prev_n = 0;       // the same two for the append before it (early mode: rows the append kernel of
+    int64_t prev_epoch = 0;   // step e-1 wrote may still be in flight when the row kernel of step e starts)
 };
 
 constexpr int kStagingSlots = 64;      // per-call metadata slots (pinned host + device twin)
@@ -75,6 +79,9 @@ struct metronome_pool {
     std::vector<int64_t> layer_epoch;  // epoch of each layer's latest append
     std::vector<int32_t> last_sids, last_n_new;
     AttendPlan cached_plan;            // plan of attend_frame(q_lens = n_new) for the latest layer-0 append
+    std::vector<Session> undo_sessions;          // append_kv's rollback snapshot (members: no allocation per call)
+    std::vector<int32_t> undo_sids, undo_n_new;
+    int32_t inject_fault = 0;          // metronome_pool_debug_fail_next (one-shot, tests of the error path)
 
     // device
     int32_t* d_table = nullptr;
@@ -107,7 +114,7 @@ struct metronome_pool {
     std::vector<cudaEvent_t> prof_ev;  // start, stop, start, stop, ...
     size_t prof_used = 0;
 
-    int32_t tune_split_tokens = 0, tune_family = 0;
+    int32_t tune_split_tokens = 0, tune_family = 0, tune_gqa_dynamic = 0;
     int32_t n_sm = 148;
     int64_t n_launch = 0, n_append = 0, n_attend = 0;
     std::string cuda_err;
@@ -129,7 +136,7 @@ bool valid_cfg(const metronome_pool_config_t* c) {
     if (!c) return false;
     const bool bk = c->flags & METRONOME_FLAG_BOOKKEEPING_ONLY;
     if (c->n_layers < 1 || c->n_q_heads < 1 || c->n_kv_heads < 1 || c->n_q_heads % c->n_kv_heads) return false;
-    if (c->block_size < 1 || c->n_sinks < 0 || c->window < 1 || c->max_sessions < 1 || c->max_sessions > 65536)
+    if (c->block_size < 1 || c->n_sinks < 0 || c->window < 1 || c->max_sessions < 1 || c->max_sessions > 65534)
         return false;
     if (c->max_new_tokens < 1 || c->n_blocks < 1 || c->max_session_len < 0) return false;
     if (!bk && (c->block_size != kBlockTokens || (c->head_dim != 64 && c->head_dim != 128))) return false;
@@ -262,6 +269,12 @@ int plan_attend(metronome_pool* pool, int32_t n_batch, const int32_t* sids, cons
         it.n_sink_tiles = n_blk < pool->n_sink ? n_blk : pool->n_sink;
         it.first_blk = first_blk;
         it.n_tiles = it.n_sink_tiles + (n_blk > first_blk ? n_blk - first_blk : 0);
+        // Early mode: the row kernel of step e may run next to the append kernels of steps e AND e-1 (the
+        // one of step e-1 is only known to be past its own wait, not complete), so the first block it must
+        // not touch before griddepcontrol.wait is the one holding the oldest row either of them wrote.
+        const int64_t exposed = (s.last_epoch == pool->epoch && s.prev_epoch == pool->epoch - 1) ? s.prev_n : 0;
+        const int64_t fresh_pos = s.len - std::max<int64_t>(q_lens[i], s.last_epoch == pool->epoch ? s.last_n : 0) - exposed;
+        it.fresh_blk = (int32_t)((fresh_pos > 0 ? fresh_pos : 0) / kBlockTokens);
     }
     pl.n_items = n_items;
     if (family != 2) { n_cls[0] = n_items; n_cls[1] = 0; }
@@ -297,7 +310,8 @@ int plan_attend(metronome_pool* pool, int32_t n_batch, const int32_t* sids, cons
             // measured on B200: the dynamic tail pays (-2 % on config 5) only when a CTA's share is long
             // (>= 512 tiles = 4 MB); for shorter shares the restart of a claimed range costs more than the
             // imbalance it removes (configs 3 and 4: +3..7 %), so they stay fully static
-            const bool dynamic = pool->tune_split_tokens <= 0 && (total_tiles + ctas - 1) / ctas >= 512;
+            const bool dynamic = pool->tune_gqa_dynamic == 1 ||
+                                 (pool->tune_gqa_dynamic == 0 && pool->tune_split_tokens <= 0 && (total_tiles + ctas - 1) / ctas >= 512);
             pl.gplan = make_gqa_plan(c.n_kv_heads, total_tiles, ctas, dynamic);
             GqaPlan& g = pl.gplan;
             pl.gqa_ctas = g.n_static;
@@ -347,6 +361,7 @@ int plan_attend(metronome_pool* pool, int32_t n_batch, const int32_t* sids, cons
         const int rc = ensure_workspace(pool, (size_t)pl.total_rows * c.n_q_heads * pl.max_splits);
         if (rc) return rc;
     }
+    if (pool->inject_fault == 1) { pool->inject_fault = 0; return METRONOME_ERR_OUT_OF_MEMORY; }   // (as if the growth had failed)
     pl.valid = true;
     return METRONOME_OK;
 }
@@ -690,36 +705,51 @@ int metronome_append_kv(metronome_pool_t* pool, int32_t layer, int32_t n_batch, 
     }
     const AppendItem* h_items = reinterpret_cast<const AppendItem*>(h);     // pinned host memory, read by the kernels
     AttendItem* h_attend = reinterpret_cast<AttendItem*>(h + (size_t)n_batch * sizeof(AppendItem));
-    bool fused_bookkeeping = false, have_plan = false;
+    bool fused_bookkeeping = false, unfused_bookkeeping = false, have_plan = false;
     const int32_t n_free0 = pool->n_free;
+    // Everything that can fail comes BEFORE the shadow counts are final ("no state change on error"):
+    // the counts are committed tentatively (the work list of this step is planned from the lengths
+    // AFTER the append), and rolled back if the plan, the workspace growth or the first launch fails.
+    std::vector<Session>& undo_sessions = pool->undo_sessions;
+    undo_sessions.clear();
+    const int64_t undo_epoch = pool->epoch, undo_layer_epoch = pool->layer_epoch[layer];
+    const int32_t undo_last_early = pool->last_early_epoch;
+    std::vector<int32_t>&undo_sids = pool->undo_sids, &undo_n_new = pool->undo_n_new;
+    const AttendPlan undo_plan = pool->cached_plan;
+    auto rollback = [&]() {
+        if (layer == 0) {
+            for (int i = 0; i < n_batch; ++i) pool->sessions[sids[i]] = undo_sessions[i];
+            pool->n_free = n_free0;
+            pool->last_sids.swap(undo_sids);
+            pool->last_n_new.swap(undo_n_new);
+        }
+        pool->epoch = undo_epoch;
+        pool->layer_epoch[layer] = undo_layer_epoch;
+        pool->last_early_epoch = undo_last_early;
+        pool->cached_plan = undo_plan;
+    };
     if (layer == 0) {
         if (pool->n_free + total_freed < total_alloc) return METRONOME_ERR_POOL_EXHAUSTED;  // nothing changed
         if (n_batch > 0 && total_freed + total_alloc > 0) {
-            if (pool->poison || pool->bookkeeping_only) {
-                // unfused: the poison fill has to sit between the frees and the K/V writes
-                bookkeeping_kernel<<<1, 512, 0, st>>>(h_items, n_batch, pool->d_table, pool->tbl_width, pool->n_sink,
-                                                      pool->ring, pool->d_free, pool->n_free, total_freed);
-                ++pool->n_launch;
-                CU(cudaGetLastError());
-                if (pool->poison && !pool->bookkeeping_only && total_freed > 0) {
-                    poison_blocks_kernel<<<dim3(total_freed, c.n_layers), 256, 0, st>>>(pool->d_free, pool->n_free, pool->d_kv,
-                                                                                       pool->L.block_bytes, pool->L.layer_bytes);
-                    ++pool->n_launch;
-                    CU(cudaGetLastError());
-                }
-            } else {
-                fused_bookkeeping = true;
-            }
+            // unfused in poison / bookkeeping-only mode: the poison fill has to sit between the frees and
+            // the K/V writes
+            if (pool->poison || pool->bookkeeping_only) unfused_bookkeeping = true;
+            else fused_bookkeeping = true;
         }
-        // commit the shadow counts
+        // tentative commit of the shadow counts
+        undo_sessions.reserve(n_batch);
+        for (int i = 0; i < n_batch; ++i) undo_sessions.push_back(pool->sessions[sids[i]]);
+        undo_sids = pool->last_sids;
+        undo_n_new = pool->last_n_new;
+        ++pool->epoch;
         for (int i = 0; i < n_batch; ++i) {
             Session& s = pool->sessions[sids[i]];
             s.first_live += items[i].n_freed;
             s.len += n_new[i];
-            s.last_n = n_new[i];
+            s.prev_n = s.last_n; s.prev_epoch = s.last_epoch;
+            s.last_n = n_new[i]; s.last_epoch = pool->epoch;
         }
         pool->n_free += total_freed - total_alloc;
-        ++pool->epoch;
         pool->layer_epoch[0] = pool->epoch;
         pool->last_sids.assign(sids, sids + n_batch);
         pool->last_n_new.assign(n_new, n_new + n_batch);
@@ -728,14 +758,28 @@ int metronome_append_kv(metronome_pool_t* pool, int32_t layer, int32_t n_batch, 
         pool->cached_plan.valid = false;
         if (!pool->bookkeeping_only && total_new > 0) {
             rc = plan_attend(pool, n_batch, sids, n_new, h_attend, pool->cached_plan);
-            if (rc) return rc;
+            if (rc) { rollback(); return rc; }
             pool->cached_plan.epoch = pool->epoch;
             have_plan = true;
+        }
+        if (unfused_bookkeeping) {
+            bookkeeping_kernel<<<1, 512, 0, st>>>(h_items, n_batch, pool->d_table, pool->tbl_width, pool->n_sink,
+                                                  pool->ring, pool->d_free, n_free0, total_freed);
+            const cudaError_t e = cudaGetLastError();
+            if (e != cudaSuccess) { rollback(); return cuda_fail(pool, e, "bookkeeping_kernel"); }
+            ++pool->n_launch;
+            // (a failure from here on follows a kernel that is already enqueued: it is reported, and the
+            // CUDA context is in a sticky error state anyway)
+            if (pool->poison && !pool->bookkeeping_only && total_freed > 0) {
+                poison_blocks_kernel<<<dim3(total_freed, c.n_layers), 256, 0, st>>>(pool->d_free, n_free0, pool->d_kv,
+                                                                                   pool->L.block_bytes, pool->L.layer_bytes);
+                ++pool->n_launch;
+                CU(cudaGetLastError());
+            }
         }
     } else {
         pool->layer_epoch[layer] = pool->epoch;
     }
-    ++pool->n_append;
     if (n_batch > 0 && (fused_bookkeeping || (!pool->bookkeeping_only && total_new > 0))) {
         AppendParams a{};
         a.items = h_items;
@@ -764,11 +808,18 @@ int metronome_append_kv(metronome_pool_t* pool, int32_t layer, int32_t n_batch, 
         a.kv_layer = pool->bookkeeping_only ? nullptr : pool->d_kv + (int64_t)layer * pool->L.layer_bytes;
         a.L = pool->L;
         const int32_t chunks = max_n * c.n_kv_heads * (c.head_dim / 8);
-        dim3 grid(std::max(1, (chunks + 255) / 256), n_batch + 1);
+        dim3 grid(std::max(1, (chunks + 255) / 256), n_batch + 1);      // (n_batch <= max_sessions <= 65534)
         const size_t smem = (fused_bookkeeping && n_batch <= kAppendSmemItems) ? (size_t)n_batch * sizeof(AppendItem) : 0;
-        CU(launch_kernel(append_fused_kernel, grid, dim3(256), smem, st, true, a));
+        cudaError_t e = cudaSuccess;
+        if (pool->inject_fault == 2) { pool->inject_fault = 0; e = cudaErrorLaunchFailure; }
+        else e = launch_kernel(append_fused_kernel, grid, dim3(256), smem, st, true, a);
+        if (e != cudaSuccess) {
+            if (!unfused_bookkeeping) rollback();      // nothing was enqueued: the call never happened
+            return cuda_fail(pool, e, "append_fused_kernel");
+        }
         ++pool->n_launch;
     }
+    ++pool->n_append;
     if (n_batch > 0) return release_stage(pool, slot, st);
     return METRONOME_OK;
 }
@@ -1020,10 +1071,18 @@ int metronome_gate_admit(metronome_gate_t* g, int32_t n_live, int32_t* admitted_
     return METRONOME_OK;
 }
 
-int metronome_pool_set_tuning(metronome_pool_t* pool, int32_t split_tokens, int32_t kernel_family) {
-    if (!pool || split_tokens < 0 || kernel_family < 0 || kernel_family > 2) return METRONOME_ERR_INVALID_ARG;
+int metronome_pool_debug_fail_next(metronome_pool_t* pool, int32_t stage) {
+    if (!pool || stage < 0 || stage > 2) return METRONOME_ERR_INVALID_ARG;
+    pool->inject_fault = stage;
+    return METRONOME_OK;
+}
+
+int metronome_pool_set_tuning(metronome_pool_t* pool, int32_t split_tokens, int32_t kernel_family, int32_t gqa_dynamic) {
+    if (!pool || split_tokens < 0 || kernel_family < 0 || kernel_family > 2 || gqa_dynamic < 0 || gqa_dynamic > 2)
+        return METRONOME_ERR_INVALID_ARG;
     pool->tune_split_tokens = split_tokens;
     pool->tune_family = kernel_family;
+    pool->tune_gqa_dynamic = gqa_dynamic;
     pool->cached_plan.valid = false;
     return METRONOME_OK;
 }

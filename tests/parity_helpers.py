@@ -10,10 +10,11 @@ from paper_2607_02640_b200 import synth
 # north_star: "Attention outputs must match within max-abs 1e-2 and max-rel 2e-2 on bf16 outputs".
 # DESIGN.md reading R9.  Contract gate, every element:  |g - o| <= 1e-2 + 2e-2 * |o|   (the usual
 # atol/rtol pairing; a bare max-abs of 1e-2 cannot hold for ANY bf16 output once |o| > 5.1, and
-# config 4's x20 outlier channels reach |o| ~ 30).  The build's own tighter gates on top:
-#   * every (query, head) row:  ||g - o||_2 / ||o||_2 <= 1e-2
-#   * unit-scale workloads (no outlier channels; every config but 4):  max|g - o| <= 1e-2 over all
-#     elements AND max over rows of ||g - o||_inf / ||o||_inf <= 2e-2
+# config 4's x20 outlier channels reach |o| ~ 30).  On top, for every workload (both are scale-free):
+#   * every (query, head) row:  ||g - o||_inf / ||o||_inf <= 2e-2      (SURVEY.md sec. 8(c)'s reading of max-rel)
+#   * every (query, head) row:  ||g - o||_2 / ||o||_2 <= 1e-2          (the build's own tighter gate)
+# and for unit-scale workloads (no outlier channels; every config but 4) SURVEY sec. 8(c)'s bare
+# max|g - o| <= 1e-2 over all elements.
 ATOL = 1e-2
 RTOL = 2e-2
 ROW_L2 = 1e-2
@@ -36,9 +37,9 @@ def parity_report(got: torch.Tensor, ref: np.ndarray) -> dict:
 def assert_parity(got: torch.Tensor, ref: np.ndarray, what: str = "", unit_scale: bool = True):
     r = parity_report(got, ref)
     assert r["finite"], f"{what}: non-finite GPU output {r}"
-    assert r["allclose_excess"] <= 1.0 and r["row_l2"] <= ROW_L2, f"{what}: {r}"
+    assert r["allclose_excess"] <= 1.0 and r["row_l2"] <= ROW_L2 and r["max_rel"] <= RTOL, f"{what}: {r}"
     if unit_scale:
-        assert r["max_abs"] <= ATOL and r["max_rel"] <= RTOL, f"{what}: {r}"
+        assert r["max_abs"] <= ATOL, f"{what}: {r}"
     return r
 
 

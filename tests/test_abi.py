@@ -1,5 +1,5 @@
 """CPU-only checks of the boundary: the C-ABI library builds, loads, and exports every symbol
-include/metronome.h declares (no compute calls without a GPU)."""
+include/*.h declare (no compute calls without a GPU)."""
 import os
 import re
 import subprocess
@@ -18,7 +18,8 @@ def lib():
 
 
 def _declared():
-    text = open(os.path.join(ROOT, "include", "metronome.h")).read()
+    text = "".join(open(os.path.join(ROOT, "include", f)).read() for f in sorted(os.listdir(os.path.join(ROOT, "include")))
+                   if f.endswith(".h"))
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
     return sorted(set(re.findall(r"\b(metronome_[a-z_0-9]+)\s*\(", text)))
 
@@ -36,7 +37,7 @@ def test_every_declared_symbol_is_exported(lib):
 
 def test_host_only_entry_points(lib):
     from paper_2607_02640_b200 import binding
-    assert lib.metronome_abi_version() == 1
+    assert lib.metronome_abi_version() == 2
     assert lib.metronome_strerror(5) == b"POOL_EXHAUSTED"
     # closed form of the per-session cap for the five configs
     for (S, W, n), want in {(4, 128, 8): 11, (4, 750, 1): 49, (4, 2048, 25): 132, (4, 1024, 25): 68,

@@ -212,3 +212,36 @@ def test_synth_generator_is_deterministic_and_unit_variance():
     base = synth.rows(5, synth.STREAM_K, 0, torch.arange(8), torch.arange(8), 4, 64).float().reshape(8, -1)
     ratio = o[:, ch] / base[:, ch]
     assert torch.allclose(ratio[base[:, ch] != 0], torch.tensor(20.0), rtol=1e-2)
+
+
+@pytest.mark.parametrize("cls", ["definition", "paged"])
+@pytest.mark.parametrize("S,W,L,ql", [(4, 6, 40, 5), (0, 9, 33, 8), (17, 5, 70, 3), (2, 100, 30, 7)])
+def test_frame_queries_are_the_last_q_len_positions(cls, S, W, L, ql):
+    """Pins the ONE line both oracle layers share that places a frame's queries (reading R15:
+    the queries of attend_frame are the session's LAST q_len positions, row r at t = L - ql + r).
+    With zero keys every admitted key gets the same weight, so row r of the chunk must be the plain
+    mean of V over the paper's literal interval set [0,S) U (t-W, t] (reading R1) --
+    computed here from the intervals, not from the oracle's mask.  A query placed one position off, in
+    reverse order, or at the session's first positions moves that mean."""
+    Hq, Hkv, D, B = 2, 1, 8, 4
+    cfg = O.PoolConfig(n_q_heads=Hq, n_kv_heads=Hkv, head_dim=D, S=S, W=W, n_blocks=64, block_size=B,
+                       max_sessions=2, max_new_tokens=16)
+    ora = O.DefinitionOracle(cfg) if cls == "definition" else O.PagedOracle(cfg)
+    sid = ora.session_open()
+    g = torch.Generator().manual_seed(100 + L)
+    v = torch.randn(L, Hkv, D, generator=g).to(torch.bfloat16)
+    zeros = np.zeros((L, Hkv, D), np.uint16)
+    # history in appends of <= 16 tokens, the last one exactly ql long
+    cuts = list(range(0, L - ql, 11)) + [L - ql, L]
+    for a, b in zip(cuts[:-1], cuts[1:]):
+        if b > a:
+            ora.append_kv(0, [sid], [b - a], zeros[a:b], _bf16(v[a:b]))
+    q = _bf16(_rand(5, ql, Hq, D))
+    out = ora.attend_frame(0, [sid], [ql], q)
+    vf = v.double().numpy()
+    for r in range(ql):
+        t = L - ql + r
+        keys = sorted(set(range(0, min(S, t + 1))) | set(range(max(0, t - W + 1), t + 1)))
+        want = vf[keys, 0].mean(axis=0)
+        for h in range(Hq):
+            np.testing.assert_allclose(out[r, h], want, rtol=0, atol=1e-5)
