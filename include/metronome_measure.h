@@ -29,6 +29,11 @@ int metronome_pool_set_tuning(metronome_pool_t* pool, int32_t split_tokens, int3
  * One-shot; stage 0 disarms.  Errors: INVALID_ARG. */
 int metronome_pool_debug_fail_next(metronome_pool_t* pool, int32_t stage);
 
+/* Test aid: copies the pool's 16 internal device flag words to flags16 (host) after cuda_stream has
+ * drained: [0] bookkeeping epoch, [1] work-list epoch, [2] / [3] claim and exit counters of the GQA decode
+ * kernel's dynamic ranges (must be 0 between launches), [5] past-wait epoch.  Errors: INVALID_ARG, CUDA. */
+int metronome_pool_debug_read_flags(metronome_pool_t* pool, void* cuda_stream, int32_t* flags16);
+
 /* Measurement aid.  While enabled, attend_frame brackets its attention kernel (the dominant
  * kernel; not the metadata copy, not the merge) with CUDA events on the caller's stream.
  * read_profile waits for those events, returns the summed kernel time in milliseconds and the

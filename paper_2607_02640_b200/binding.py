@@ -28,7 +28,7 @@ EXPORTS = ["metronome_abi_version", "metronome_strerror", "metronome_last_cuda_e
            "metronome_pool_destroy", "metronome_session_open", "metronome_session_close",
            "metronome_append_kv", "metronome_attend_frame", "metronome_step_host",
            "metronome_session_query", "metronome_pool_query", "metronome_read_kv", "metronome_pool_stats",
-           "metronome_pool_set_tuning", "metronome_pool_debug_fail_next", "metronome_pool_set_profiling", "metronome_pool_read_profile",
+           "metronome_pool_set_tuning", "metronome_pool_debug_fail_next", "metronome_pool_debug_read_flags", "metronome_pool_set_profiling", "metronome_pool_read_profile",
            "metronome_gate_create", "metronome_gate_destroy", "metronome_gate_observe", "metronome_gate_admit",
            "metronome_stream_read_gbs"]
 
@@ -83,6 +83,7 @@ def load():
     lib.metronome_pool_stats.argtypes = [c_void_p, POINTER(c_int64), POINTER(c_int64), POINTER(c_int64)]
     lib.metronome_pool_set_tuning.argtypes = [c_void_p, c_int32, c_int32, c_int32]
     lib.metronome_pool_debug_fail_next.argtypes = [c_void_p, c_int32]
+    lib.metronome_pool_debug_read_flags.argtypes = [c_void_p, c_void_p, i32p]
     lib.metronome_pool_set_profiling.argtypes = [c_void_p, c_int32]
     lib.metronome_pool_read_profile.argtypes = [c_void_p, POINTER(ctypes.c_double), POINTER(c_int64), c_int32]
     lib.metronome_gate_create.argtypes = [c_void_p, POINTER(c_void_p)]
@@ -205,6 +206,11 @@ class Pool:
 
     def debug_fail_next(self, stage: int):
         self._check(self._lib.metronome_pool_debug_fail_next(self._h, stage))
+
+    def debug_read_flags(self, stream=0):
+        buf = (c_int32 * 16)()
+        self._check(self._lib.metronome_pool_debug_read_flags(self._h, c_void_p(stream), buf))
+        return list(buf)
 
     def set_profiling(self, enable: bool):
         self._check(self._lib.metronome_pool_set_profiling(self._h, int(enable)))

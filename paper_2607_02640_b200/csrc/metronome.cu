@@ -1077,6 +1077,14 @@ int metronome_pool_debug_fail_next(metronome_pool_t* pool, int32_t stage) {
     return METRONOME_OK;
 }
 
+int metronome_pool_debug_read_flags(metronome_pool_t* pool, void* cuda_stream, int32_t* flags16) {
+    if (!pool || !flags16) return METRONOME_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CU(cudaMemcpyAsync(flags16, pool->d_bk_flag, 64, cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    return METRONOME_OK;
+}
+
 int metronome_pool_set_tuning(metronome_pool_t* pool, int32_t split_tokens, int32_t kernel_family, int32_t gqa_dynamic) {
     if (!pool || split_tokens < 0 || kernel_family < 0 || kernel_family > 2 || gqa_dynamic < 0 || gqa_dynamic > 2)
         return METRONOME_ERR_INVALID_ARG;

@@ -1,0 +1,169 @@
+"""GPU tests (`-m gpu`) of launch paths that the workload-shaped parity tests do not reach on their own:
+the dynamically claimed tail ranges of the GQA decode kernel, early mode on grids that fit one wave, and
+append_kv's "no state change on error" contract past the point where the shadow counts are committed.
+Seeded inputs; the oracle gets the same bf16 bits.
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import bounded_kv as O
+from paper_2607_02640_b200 import binding, synth
+from parity_helpers import assert_parity
+
+pytestmark = pytest.mark.gpu
+
+
+def _rows(rng, n, H, D):
+    return torch.from_numpy(rng.standard_normal((n, H, D)).astype(np.float32)).to(torch.bfloat16)
+
+
+@pytest.mark.parametrize("split_tokens", [0, 1024, 4096])
+def test_gqa_decode_with_dynamic_ranges_forced(split_tokens):
+    """attend_gqa_kernel's dynamic regime (the last ~10 % of the flattened tile list is cut into small
+    ranges that CTAs claim with an atomic counter; the last CTA out resets the counters) is enabled by
+    itself only when a CTA's share is >= 512 tiles, i.e. on full config 5.  Here it is FORCED on a small
+    GQA-8 workload (split_tokens sets the static share: 64 / 256 tiles; 0 = the automatic one-wave cut),
+    for 12 consecutive launches with no host sync in between: every output against the oracle, and the
+    claim / exit counters back to zero after the launches (a stale counter would make the next launch skip
+    or repeat ranges)."""
+    Hq, Hkv, D, S, W, N, n_max = 32, 4, 128, 4, 2048, 6, 25
+    per = 1 + (W + n_max - 1) // 16 + 2
+    kw = dict(n_q_heads=Hq, n_kv_heads=Hkv, head_dim=D, max_sessions=N, max_new_tokens=n_max)
+    pool = binding.Pool(n_sinks=S, window=W, n_blocks=N * per, **kw)
+    pool.set_tuning(split_tokens, 2, 1)
+    ora = O.DefinitionOracle(O.PoolConfig(S=S, W=W, n_blocks=N * per, block_size=16, **kw))
+    sids = [pool.session_open() for _ in range(N)]
+    assert sids == [ora.session_open() for _ in range(N)]
+    rng = np.random.default_rng(4242 + split_tokens)
+    # ragged histories of 300 .. 2600 tokens, appended in 25-token chunks (no attention)
+    target = rng.integers(300, 2600, size=N)
+    done = np.zeros(N, np.int64)
+    while (done < target).any():
+        idx = [i for i in range(N) if done[i] < target[i]]
+        n_new = np.array([min(n_max, target[i] - done[i]) for i in idx], np.int32)
+        rows = int(n_new.sum())
+        k, v = _rows(rng, rows, Hkv, D), _rows(rng, rows, Hkv, D)
+        pool.append_kv(0, [sids[i] for i in idx], n_new, k.cuda(), v.cuda())
+        ora.append_kv(0, [sids[i] for i in idx], [int(x) for x in n_new], synth.to_u16(k), synth.to_u16(v))
+        done[idx] += n_new
+    # 12 decode steps back to back
+    ones = np.ones(N, np.int32)
+    ins = [(_rows(rng, N, Hkv, D), _rows(rng, N, Hkv, D), _rows(rng, N, Hq, D)) for _ in range(12)]
+    dev = [(k.cuda(), v.cuda(), q.cuda()) for k, v, q in ins]
+    outs = [torch.empty_like(q) for _, _, q in dev]
+    torch.cuda.synchronize()
+    for (k, v, q), o in zip(dev, outs):
+        pool.append_kv(0, sids, ones, k, v)
+        pool.attend_frame(0, sids, ones, q, o)
+    flags = pool.debug_read_flags()
+    assert flags[2] == 0 and flags[3] == 0, f"dynamic-range counters not reset: {flags[:6]}"
+    for step, ((k, v, q), o) in enumerate(zip(ins, outs)):
+        ora.append_kv(0, sids, [1] * N, synth.to_u16(k), synth.to_u16(v))
+        assert_parity(o, ora.attend_frame(0, sids, [1] * N, synth.to_u16(q)), f"dynamic ranges, split {split_tokens}, step {step}")
+    # the general path (a reordered subset: work list uploaded by attend_frame itself) under the same knob
+    k, v, q = _rows(rng, N, Hkv, D), _rows(rng, N, Hkv, D), _rows(rng, 3, Hq, D)
+    pool.append_kv(0, sids, ones, k.cuda(), v.cuda())
+    ora.append_kv(0, sids, [1] * N, synth.to_u16(k), synth.to_u16(v))
+    sub = [sids[4], sids[0], sids[2]]
+    o = torch.empty_like(q, device="cuda")
+    pool.attend_frame(0, sub, [1, 1, 1], q.cuda(), o)
+    assert_parity(o, ora.attend_frame(0, sub, [1, 1, 1], synth.to_u16(q)), "dynamic ranges, subset")
+    flags = pool.debug_read_flags()
+    assert flags[2] == 0 and flags[3] == 0
+
+
+@pytest.mark.parametrize("n_sessions,heads", [(1, 8), (2, 8), (4, 4), (3, 32)])
+def test_early_mode_on_grids_that_fit_one_wave(n_sessions, heads):
+    """Multi-head decode in early mode with FEW CTAs per launch (1-4 sessions x 4-32 heads x a few
+    segments: every launch fits one resident wave), so the append and row kernels of consecutive steps
+    can be co-resident: A(e-1), R(e-1), A(e), R(e).  R(e) may then read rows A(e-1) is still writing
+    unless it waits before the block that holds them (AttendItem::fresh_blk covers the previous step's
+    rows).  Session lengths cross multiples of 16 all the time (1-3 tokens per step); 600 steps with no
+    host sync; every output and every table against the oracle."""
+    D, S, W, n_max = 128, 4, 100, 3
+    per = 1 + (W + n_max - 1) // 16 + 2
+    kw = dict(n_q_heads=heads, n_kv_heads=heads, head_dim=D, max_sessions=n_sessions, max_new_tokens=n_max)
+    pool = binding.Pool(n_sinks=S, window=W, n_blocks=n_sessions * per + 1, **kw)
+    cfg = O.PoolConfig(S=S, W=W, n_blocks=n_sessions * per + 1, block_size=16, **kw)
+    defn, paged = O.DefinitionOracle(cfg), O.PagedOracle(cfg)
+    sids = [pool.session_open() for _ in range(n_sessions)]
+    assert sids == [defn.session_open() for _ in sids] == [paged.session_open() for _ in sids]
+    rng = np.random.default_rng(99 + n_sessions * 100 + heads)
+    steps = []
+    for step in range(600):
+        idx = np.sort(rng.permutation(n_sessions)[: int(rng.integers(1, n_sessions + 1))])
+        n_new = rng.integers(1, n_max + 1, size=len(idx)).astype(np.int32)
+        # every third step asks for fewer query rows than it appended (general path, plain launch order)
+        q_lens = np.maximum(1, n_new - 1).astype(np.int32) if step % 3 == 2 else n_new
+        rows, qrows = int(n_new.sum()), int(q_lens.sum())
+        steps.append(([sids[i] for i in idx], n_new, q_lens, _rows(rng, rows, heads, D), _rows(rng, rows, heads, D),
+                      _rows(rng, qrows, heads, D)))
+    dev = [(k.cuda(), v.cuda(), q.cuda()) for *_, k, v, q in steps]
+    outs = [torch.empty_like(q) for _, _, q in dev]
+    torch.cuda.synchronize()
+    for (ss, n_new, q_lens, *_), (k, v, q), o in zip(steps, dev, outs):
+        pool.append_kv(0, ss, n_new, k, v)
+        pool.attend_frame(0, ss, q_lens, q, o)
+    torch.cuda.synchronize()
+    for step, ((ss, n_new, q_lens, k, v, q), o) in enumerate(zip(steps, outs)):
+        defn.append_kv(0, ss, [int(x) for x in n_new], synth.to_u16(k), synth.to_u16(v))
+        paged.append_kv(0, ss, [int(x) for x in n_new])
+        assert_parity(o, defn.attend_frame(0, ss, [int(x) for x in q_lens], synth.to_u16(q)),
+                      f"one-wave early mode, {n_sessions} x {heads}, step {step}")
+    for s in sids:
+        got, want = pool.session_query(s), paged.session_query(s)
+        assert (got[0], got[1], list(got[2])) == (want[0], want[1], list(want[2]))
+    assert pool.pool_query()[1] == paged.pool_query()
+
+
+@pytest.mark.parametrize("stage", [1, 2])
+@pytest.mark.parametrize("family", [1, 2])
+def test_append_failure_after_the_tentative_commit_changes_nothing(stage, family):
+    """metronome_append_kv plans the step's attention (and may grow the split-KV workspace) and launches
+    its kernel AFTER the shadow counts are committed tentatively; a failure there (injected:
+    metronome_pool_debug_fail_next) must roll everything back: lengths, first live blocks, block tables,
+    the free list, the layer sequence -- and the same call must then succeed and match the oracle."""
+    Hq, Hkv, D, S, W, N, n_max = 8, 2, 64, 4, 40, 3, 16
+    per = 1 + (W + n_max - 1) // 16 + 2
+    kw = dict(n_q_heads=Hq, n_kv_heads=Hkv, head_dim=D, max_sessions=N, max_new_tokens=n_max)
+    pool = binding.Pool(n_sinks=S, window=W, n_blocks=N * per, **kw)
+    pool.set_tuning(16, family)                       # 16-token segments: the plan needs the split workspace
+    cfg = O.PoolConfig(S=S, W=W, n_blocks=N * per, block_size=16, **kw)
+    defn, paged = O.DefinitionOracle(cfg), O.PagedOracle(cfg)
+    sids = [pool.session_open() for _ in range(N)]
+    assert sids == [defn.session_open() for _ in sids] == [paged.session_open() for _ in sids]
+    rng = np.random.default_rng(5 + stage)
+
+    def state():
+        return [pool.session_query(s) for s in sids], pool.pool_query()
+
+    for step in range(30):
+        n_new = rng.integers(1, n_max + 1, size=N).astype(np.int32)
+        rows = int(n_new.sum())
+        k, v, q = _rows(rng, rows, Hkv, D), _rows(rng, rows, Hkv, D), _rows(rng, rows, Hq, D)
+        if step % 4 == 1:
+            before = state()
+            pool.debug_fail_next(stage)
+            with pytest.raises(binding.MetronomeError, match="OUT_OF_MEMORY" if stage == 1 else "CUDA"):
+                pool.append_kv(0, sids, n_new, k.cuda(), v.cuda())
+            assert state() == before, f"step {step}: a failed append_kv changed the pool"
+        pool.append_kv(0, sids, n_new, k.cuda(), v.cuda())
+        defn.append_kv(0, sids, [int(x) for x in n_new], synth.to_u16(k), synth.to_u16(v))
+        paged.append_kv(0, sids, [int(x) for x in n_new])
+        o = torch.empty(rows, Hq, D, dtype=torch.bfloat16, device="cuda")
+        pool.attend_frame(0, sids, n_new, q.cuda(), o)
+        assert_parity(o, defn.attend_frame(0, sids, [int(x) for x in n_new], synth.to_u16(q)), f"after rollback, step {step}")
+        for s in sids:
+            got, want = pool.session_query(s), paged.session_query(s)
+            assert (got[0], got[1], list(got[2])) == (want[0], want[1], list(want[2]))
+        assert pool.pool_query()[1] == paged.pool_query()
+
+
+def test_max_sessions_is_capped_where_the_append_grid_ends():
+    """n_batch + 1 is a gridDim.y of the append kernel (<= 65535): a pool may have at most 65534 slots."""
+    kw = dict(n_q_heads=1, n_kv_heads=1, head_dim=64, n_sinks=0, window=16, n_blocks=8, max_new_tokens=1,
+              flags=binding.FLAG_BOOKKEEPING_ONLY)
+    with pytest.raises(binding.MetronomeError, match="INVALID_ARG"):
+        binding.Pool(max_sessions=65535, **kw)
+    binding.Pool(max_sessions=65534, **kw).destroy()
