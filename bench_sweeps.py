@@ -1,4 +1,6 @@
-"""Shape checks and sweeps of SURVEY.md sec. 8(d)/(f), run by `bench.py --sweep ...` on one GPU.
+"""bench_sweeps.py -- measurement harness beside bench.py (not part of the product package).
+
+Shape checks and sweeps of SURVEY.md sec. 8(d)/(f), run by `bench.py --sweep ...` on one GPU.
 
   age       fixed N, every session at ONE age a in {1/4, 1/2, 1, 2, 5, 10, 20} x (S+W): per-frame
             latency must rise up to a ~ S+W and then stay FLAT ("O(W)")
@@ -24,9 +26,9 @@ from dataclasses import replace
 import numpy as np
 import torch
 
-from . import synth
-from . import workloads as wl
-from .runner import Runner
+from paper_2607_02640_b200 import synth
+from paper_2607_02640_b200 import workloads as wl
+from paper_2607_02640_b200.runner import Runner
 
 
 def _frames_of(events):
@@ -54,7 +56,7 @@ def time_frames(r: Runner, events, warmup: int = 2):
     + attend_frame of the frame, CUDA events), attend_ms (attention kernels only, the library's own
     event brackets), sessions, resident tokens.  The first `warmup` frames are dropped."""
     out = []
-    r.pool.set_profiling(True)
+    r.pool.set_profiling(1)
     for k, (pre, steps) in enumerate(_frames_of(events)):
         for ev in pre:
             if ev[0] == "open":
@@ -81,7 +83,7 @@ def time_frames(r: Runner, events, warmup: int = 2):
         if k >= warmup:
             sess = {int(i) for ev in steps for i in ev[1]}
             out.append({"ms": e0.elapsed_time(e1), "attend_ms": a_ms, "sessions": len(sess)})
-    r.pool.set_profiling(False)
+    r.pool.set_profiling(0)
     return out
 
 

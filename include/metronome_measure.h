@@ -34,13 +34,23 @@ int metronome_pool_debug_fail_next(metronome_pool_t* pool, int32_t stage);
  * kernel's dynamic ranges (must be 0 between launches), [5] past-wait epoch.  Errors: INVALID_ARG, CUDA. */
 int metronome_pool_debug_read_flags(metronome_pool_t* pool, void* cuda_stream, int32_t* flags16);
 
-/* Measurement aid.  While enabled, attend_frame brackets its attention kernel (the dominant
- * kernel; not the metadata copy, not the merge) with CUDA events on the caller's stream.
- * read_profile waits for those events, returns the summed kernel time in milliseconds and the
- * number of bracketed launches since the last reset, and (reset != 0) clears them.  host. */
-int metronome_pool_set_profiling(metronome_pool_t* pool, int32_t enable);
+/* Measurement aids for the time of the attention kernels (the dominant kernels; not the append kernel, not the merge).
+ *   mode 1  attend_frame brackets its attention kernel with CUDA events on the caller's stream.  Events between the
+ *           launches break their programmatic (PDL) edges, so in this mode every launch is plain and early mode is off:
+ *           the kernel is timed ALONE, not as it runs inside a normal step.  read_profile waits for the events, returns
+ *           the summed kernel time in milliseconds and the number of bracketed launches, and (reset != 0) clears them.
+ *   mode 2  the attention kernels stamp %globaltimer themselves (first CTA in, last CTA out; two atomics per CTA), the
+ *           launches stay exactly as in a normal step.  read_stamps synchronises the device, returns per attention launch
+ *           since the mode was set / the last read (at most max_launches, at most 32768 are kept) its kind (1 row kernel,
+ *           2 GQA decode kernel, 3 chunk-prefill kernel), its span and its start relative to the first launch, both in
+ *           milliseconds (-1: the kernel never stamped), and clears them.  All pointers host; kinds / span_ms / start_ms
+ *           may be NULL.
+ *   mode 0  off.  Errors: INVALID_ARG, CUDA. */
+int metronome_pool_set_profiling(metronome_pool_t* pool, int32_t mode);
 int metronome_pool_read_profile(metronome_pool_t* pool, double* attend_kernel_ms, int64_t* attend_kernel_launches,
                                 int32_t reset);
+int metronome_pool_read_stamps(metronome_pool_t* pool, int32_t max_launches, int32_t* kinds, double* span_ms,
+                               double* start_ms, int32_t* n_out);
 
 
 /* Measurement aid ("plus a read-only stream microbenchmark run in the same job").

@@ -28,7 +28,7 @@ EXPORTS = ["metronome_abi_version", "metronome_strerror", "metronome_last_cuda_e
            "metronome_pool_destroy", "metronome_session_open", "metronome_session_close",
            "metronome_append_kv", "metronome_attend_frame", "metronome_step_host",
            "metronome_session_query", "metronome_pool_query", "metronome_read_kv", "metronome_pool_stats",
-           "metronome_pool_set_tuning", "metronome_pool_debug_fail_next", "metronome_pool_debug_read_flags", "metronome_pool_set_profiling", "metronome_pool_read_profile",
+           "metronome_pool_set_tuning", "metronome_pool_debug_fail_next", "metronome_pool_debug_read_flags", "metronome_pool_set_profiling", "metronome_pool_read_profile", "metronome_pool_read_stamps",
            "metronome_gate_create", "metronome_gate_destroy", "metronome_gate_observe", "metronome_gate_admit",
            "metronome_stream_read_gbs"]
 
@@ -85,6 +85,7 @@ def load():
     lib.metronome_pool_debug_fail_next.argtypes = [c_void_p, c_int32]
     lib.metronome_pool_debug_read_flags.argtypes = [c_void_p, c_void_p, i32p]
     lib.metronome_pool_set_profiling.argtypes = [c_void_p, c_int32]
+    lib.metronome_pool_read_stamps.argtypes = [c_void_p, c_int32, i32p, POINTER(ctypes.c_double), POINTER(ctypes.c_double), i32p]
     lib.metronome_pool_read_profile.argtypes = [c_void_p, POINTER(ctypes.c_double), POINTER(c_int64), c_int32]
     lib.metronome_gate_create.argtypes = [c_void_p, POINTER(c_void_p)]
     lib.metronome_gate_destroy.argtypes = [c_void_p]
@@ -212,8 +213,20 @@ class Pool:
         self._check(self._lib.metronome_pool_debug_read_flags(self._h, c_void_p(stream), buf))
         return list(buf)
 
-    def set_profiling(self, enable: bool):
-        self._check(self._lib.metronome_pool_set_profiling(self._h, int(enable)))
+    def set_profiling(self, mode):
+        """0 off, 1 (or True) event brackets, 2 in-kernel %globaltimer stamps (launches unchanged)."""
+        self._check(self._lib.metronome_pool_set_profiling(self._h, int(mode)))
+
+    def read_stamps(self, max_launches=1 << 15):
+        """-> (kinds, span_ms, start_ms) numpy arrays, one entry per stamped attention launch; clears them."""
+        kinds = np.zeros(max_launches, np.int32)
+        span = np.zeros(max_launches, np.float64)
+        start = np.zeros(max_launches, np.float64)
+        n = c_int32()
+        self._check(self._lib.metronome_pool_read_stamps(
+            self._h, max_launches, kinds.ctypes.data_as(POINTER(c_int32)), span.ctypes.data_as(POINTER(ctypes.c_double)),
+            start.ctypes.data_as(POINTER(ctypes.c_double)), byref(n)))
+        return kinds[:n.value], span[:n.value], start[:n.value]
 
     def read_profile(self, reset=True):
         """-> (summed attention-kernel milliseconds, bracketed launches)"""

@@ -39,5 +39,43 @@ def build_library(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+CENSUS_OPS = ("UTCHMMA", "UTCBAR", "LDTM", "STTM", "UBLKCP", "SYNCS", "HMMA", "LDSM", "LDG", "STG", "MUFU.EX2", "FFMA2",
+              "ATOMG", "REDG", "ACQBULK", "LDGDEPBAR")
+
+
+def sass_census() -> dict:
+    """Per kernel of libmetronome.so: how often each SASS mnemonic of interest occurs (cuobjdump -sass).
+    UTCHMMA / LDTM / STTM = tcgen05.mma / tcgen05.ld / tcgen05.st, UBLKCP = cp.async.bulk, HMMA = mma.sync,
+    LDSM = ldmatrix, SYNCS = mbarrier operations (B200_PROFILING.md)."""
+    import re
+    out = subprocess.run(["cuobjdump", "-sass", LIB], capture_output=True, text=True, check=True).stdout
+    census, name = {}, None
+    for line in out.splitlines():
+        m = re.match(r"\s*Function : (\S+)", line)
+        if m:
+            name = subprocess.run(["c++filt", m.group(1)], capture_output=True, text=True).stdout.strip().replace("(anonymous namespace)::", "").split("(")[0]
+            name = name.replace("metronome::", "").replace("void ", "")
+            census[name] = {"instructions": 0}
+            continue
+        m = re.match(r"\s*/\*[0-9a-f]{4}\*/\s+(?:@!?U?P\d+\s+)?([A-Z0-9_.]+)", line)
+        if m and name:
+            census[name]["instructions"] += 1
+            op = m.group(1)
+            for key in CENSUS_OPS:
+                if op == key or op.startswith(key + "."):
+                    census[name][key] = census[name].get(key, 0) + 1
+    return census
+
+
 if __name__ == "__main__":
-    print(build_library(force=True, verbose=True))
+    import sys
+    if "--census" in sys.argv:
+        build_library()
+        c = sass_census()
+        cols = [k for k in CENSUS_OPS if any(k in v for v in c.values())]
+        print("| kernel | instructions | " + " | ".join(cols) + " |")
+        print("|---|---|" + "---|" * len(cols))
+        for name in sorted(c):
+            print(f"| `{name}` | {c[name]['instructions']} | " + " | ".join(str(c[name].get(k, 0)) for k in cols) + " |")
+    else:
+        print(build_library(force=True, verbose=True))

@@ -50,7 +50,18 @@ struct AttendParams {
     const int32_t* range_item; // GQA decode: item that holds the first tile of each range (null: binary search)
     int32_t* gqa_ctr;         // [2] claim / exit counters of the GQA decode kernel's dynamic ranges (zero between launches)
     int32_t* tickets;         // [item][Hkv] arrival counters of the stream-K pieces (zero between launches)
+    unsigned long long* stamp; // measurement aid (null: off): [0] <- min over CTAs of %globaltimer at start, [1] <- max at exit
 };
+
+// Measurement aid (metronome_pool_set_profiling mode 2): the kernel's own span in %globaltimer ns, first CTA
+// in to last CTA out, without events between the launches (those would break the programmatic launch edges).
+__device__ __forceinline__ unsigned long long global_ns() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+__device__ __forceinline__ void stamp_begin(const AttendParams& p) { if (p.stamp) atomicMin(p.stamp, global_ns()); }
+__device__ __forceinline__ void stamp_end(const AttendParams& p) { if (p.stamp) atomicMax(p.stamp + 1, global_ns()); }
 
 // Start of an attention kernel.  In early mode (items_epoch >= 0: launched programmatically behind an
 // append kernel that triggered its dependents at once) the kernel may run NEXT TO the kernels before

@@ -306,6 +306,7 @@ __global__ void __launch_bounds__(GqaCfg<D>::kThreads)
 attend_gqa_kernel(AttendParams p, GqaPlan plan) {
     using C = GqaCfg<D>;
     if (p.pdl_early) pdl_launch_dependents();
+    if (threadIdx.x == 0) stamp_begin(p);
     pdl_wait();                  // the work list and this step's K/V rows come from the append kernel
     extern __shared__ __align__(128) uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 127u) & ~127u;
@@ -522,6 +523,7 @@ attend_gqa_kernel(AttendParams p, GqaPlan plan) {
     if (plan.n_total != plan.n_static && threadIdx.x == 0) {
         if (atomicAdd(p.gqa_ctr + 1, 1) == (int32_t)gridDim.x - 1) { p.gqa_ctr[0] = 0; p.gqa_ctr[1] = 0; }
     }
+    if (threadIdx.x == 0) stamp_end(p);
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -34,7 +34,7 @@ template <int D>
 __global__ void __launch_bounds__(128)
 attend_rows_kernel(AttendParams p) {
     if (p.pdl_early) pdl_launch_dependents();
-    if (threadIdx.x == 0) wait_work_list(p);
+    if (threadIdx.x == 0) { stamp_begin(p); wait_work_list(p); }
     __syncthreads();
     if (p.items_epoch < 0) pdl_wait();
     constexpr int LPT = D / 8;         // lanes per token (16-byte chunks per row)
@@ -217,6 +217,7 @@ attend_rows_kernel(AttendParams p) {
             if (sub == 0) { p.ws_ml[slot * 2] = m; p.ws_ml[slot * 2 + 1] = l; }
         }
     }
+    if (threadIdx.x == 0) stamp_end(p);
 }
 
 }  // namespace metronome

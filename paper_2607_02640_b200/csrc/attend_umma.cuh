@@ -148,6 +148,7 @@ __global__ void __launch_bounds__(UmmaCfg<D>::kThreads, 1)
 attend_umma_kernel(AttendParams p) {
     using C = UmmaCfg<D>;
     if (p.pdl_early) pdl_launch_dependents();
+    if (threadIdx.x == 0) stamp_begin(p);
     pdl_wait();                  // the work list and this step's K/V rows come from the append kernel
     extern __shared__ __align__(1024) uint8_t smem_umma[];
     const uint32_t base = (smem_u32(smem_umma) + 1023u) & ~1023u;       // swizzle atoms are 1024-byte aligned
@@ -596,6 +597,7 @@ attend_umma_kernel(AttendParams p) {
     }
     tc_fence_before();
     named_arrive(2, 32 + 256);
+    if (threadIdx.x == 128) stamp_end(p);
 }
 
 // ------------------------------------------------------------------------------------------------

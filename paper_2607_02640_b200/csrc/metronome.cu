@@ -41,6 +41,7 @@ constexpr int kStagingSlots = 64;      // per-call metadata slots (pinned host +
 constexpr int kStagingGroup = 8;       // one completion event per 8 slots: an event between two kernels
                                        // would break their programmatic (PDL) launch edge
 constexpr int kMaxSplits = 64;
+constexpr int kStampSlots = 1 << 15;   // attention launches one stamped pass can hold
 constexpr int kMaxRangeItems = 4096;   // GQA decode ranges whose start item travels with the work list
 
 // Row a8: the launch plan of one attend_frame call (host side of the work list).  Items of class 0
@@ -110,9 +111,12 @@ struct metronome_pool {
     int next_slot = 0;
 
     // profiling (metronome_pool_set_profiling): event pairs around the attention kernel
-    bool profiling = false;
+    bool profiling = false;            // mode 1: event brackets (launches are then not programmatic)
     std::vector<cudaEvent_t> prof_ev;  // start, stop, start, stop, ...
     size_t prof_used = 0;
+    bool stamping = false;             // mode 2: %globaltimer stamps written by the attention kernels themselves
+    unsigned long long* d_stamps = nullptr;    // [kStampSlots][2]
+    std::vector<int32_t> stamp_kind;   // per used slot: 1 rows, 2 gqa decode, 3 chunk
 
     int32_t tune_split_tokens = 0, tune_family = 0, tune_gqa_dynamic = 0;
     int32_t n_sm = 148;
@@ -366,6 +370,20 @@ int plan_attend(metronome_pool* pool, int32_t n_batch, const int32_t* sids, cons
     return METRONOME_OK;
 }
 
+__global__ void init_stamps_kernel(unsigned long long* stamps, int n) {
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        stamps[2 * i] = ~0ull;
+        stamps[2 * i + 1] = 0ull;
+    }
+}
+
+// profiling mode 2: the stamp slot of the next attention launch (null when off or the ring is full)
+unsigned long long* next_stamp(metronome_pool* pool, int32_t kind) {
+    if (!pool->stamping || !pool->d_stamps || pool->stamp_kind.size() >= (size_t)kStampSlots) return nullptr;
+    pool->stamp_kind.push_back(kind);
+    return pool->d_stamps + 2 * (pool->stamp_kind.size() - 1);
+}
+
 // Launches the attention kernels (rows a5 / a7) and the split merge (a6) of one attend_frame call.
 // `pdl`: the work list was written by the append kernel that precedes this launch on the stream
 // (cached plan): launch programmatically so the prologue overlaps that kernel's tail.
@@ -410,17 +428,20 @@ int launch_attend(metronome_pool* pool, int32_t layer, const AttendPlan& pl, con
     if (pl.family == 2) {
         if (pl.n_cls[0] > 0) {
             p.items = d_items; p.n_items = pl.n_cls[0];
+            p.stamp = next_stamp(pool, 2);
             CU(launch_attend_gqa(p, pl.gplan, c.head_dim, pl.gqa_ctas, st, pdl));
             ++pool->n_launch;
         }
         if (pl.n_cls[1] > 0) {
             p.items = d_items + pl.n_cls[0]; p.n_items = pl.n_cls[1];
+            p.stamp = next_stamp(pool, 3);
             CU(launch_attend_umma(p, c.head_dim, c.n_kv_heads, pl.total_splits[1], st, pdl));
             ++pool->n_launch;
         }
     } else {
         p.items = d_items; p.n_items = pl.n_items;
         dim3 grid(c.n_q_heads, pl.total_splits[0], pl.cls_max_q[0]);
+        p.stamp = next_stamp(pool, 1);
         if (c.head_dim == 128) CU(launch_kernel(attend_rows_kernel<128>, grid, dim3(128), 0, st, pdl, p));
         else CU(launch_kernel(attend_rows_kernel<64>, grid, dim3(128), 0, st, pdl, p));
         ++pool->n_launch;
@@ -575,6 +596,7 @@ int metronome_pool_destroy(metronome_pool_t* pool) {
     if (pool->d_table) cudaFree(pool->d_table);
     if (pool->d_tickets) cudaFree(pool->d_tickets);
     if (pool->d_bk_flag) cudaFree(pool->d_bk_flag);
+    if (pool->d_stamps) cudaFree(pool->d_stamps);
     if (pool->d_attend_items) cudaFree(pool->d_attend_items);
     if (pool->d_free) cudaFree(pool->d_free);
     if (pool->own_kv && pool->d_kv) cudaFree(pool->d_kv);
@@ -971,9 +993,39 @@ int metronome_pool_stats(metronome_pool_t* pool, int64_t* kernel_launches, int64
     return METRONOME_OK;
 }
 
-int metronome_pool_set_profiling(metronome_pool_t* pool, int32_t enable) {
-    if (!pool) return METRONOME_ERR_INVALID_ARG;
-    pool->profiling = enable != 0;
+int metronome_pool_set_profiling(metronome_pool_t* pool, int32_t mode) {
+    if (!pool || mode < 0 || mode > 2) return METRONOME_ERR_INVALID_ARG;
+    pool->profiling = mode == 1;
+    pool->stamping = mode == 2;
+    if (mode == 2) {
+        if (!pool->d_stamps) CU(cudaMalloc(&pool->d_stamps, (size_t)kStampSlots * 2 * sizeof(unsigned long long)));
+        CU(cudaDeviceSynchronize());
+        init_stamps_kernel<<<64, 256>>>(pool->d_stamps, kStampSlots);
+        CU(cudaDeviceSynchronize());
+        pool->stamp_kind.clear();
+    }
+    return METRONOME_OK;
+}
+
+int metronome_pool_read_stamps(metronome_pool_t* pool, int32_t max_launches, int32_t* kinds, double* span_ms,
+                               double* start_ms, int32_t* n_out) {
+    if (!pool || max_launches < 0 || !n_out) return METRONOME_ERR_INVALID_ARG;
+    CU(cudaDeviceSynchronize());
+    const int32_t n = (int32_t)std::min<size_t>(pool->stamp_kind.size(), (size_t)max_launches);
+    std::vector<unsigned long long> h(2 * (size_t)n);
+    if (n > 0) CU(cudaMemcpy(h.data(), pool->d_stamps, h.size() * sizeof(unsigned long long), cudaMemcpyDeviceToHost));
+    for (int32_t i = 0; i < n; ++i) {
+        if (kinds) kinds[i] = pool->stamp_kind[i];
+        const bool ok = h[2 * i] != ~0ull && h[2 * i + 1] >= h[2 * i];
+        if (span_ms) span_ms[i] = ok ? (double)(h[2 * i + 1] - h[2 * i]) * 1e-6 : -1.0;
+        if (start_ms) start_ms[i] = ok ? (double)(h[2 * i] - h[0]) * 1e-6 : -1.0;
+    }
+    *n_out = n;
+    if (pool->d_stamps) {
+        init_stamps_kernel<<<64, 256>>>(pool->d_stamps, kStampSlots);
+        CU(cudaDeviceSynchronize());
+    }
+    pool->stamp_kind.clear();
     return METRONOME_OK;
 }
 

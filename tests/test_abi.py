@@ -56,6 +56,20 @@ def test_sass_is_sm100a_only():
     assert "sm_100a" in out and "sm_90" not in out and "sm_80" not in out
 
 
+def test_sass_census_shows_the_hardware_paths_each_kernel_claims():
+    """the chunk kernel is tcgen05 (UTCHMMA) with TMEM loads / stores (LDTM / STTM) and bulk
+    async copies (UBLKCP); the GQA decode kernel is mma.sync (HMMA) + ldmatrix + bulk copies; the row kernel
+    is CUDA cores only (packed FFMA2, no tensor instruction)."""
+    from paper_2607_02640_b200 import build
+    build.build_library()
+    c = build.sass_census()
+    for D in (64, 128):
+        u, g, r = c[f"attend_umma_kernel<{D}>"], c[f"attend_gqa_kernel<{D}>"], c[f"attend_rows_kernel<{D}>"]
+        assert u.get("UTCHMMA", 0) > 0 and u.get("LDTM", 0) > 0 and u.get("STTM", 0) > 0 and u.get("UBLKCP", 0) > 0, u
+        assert g.get("HMMA", 0) > 0 and g.get("LDSM", 0) > 0 and g.get("UBLKCP", 0) > 0 and "UTCHMMA" not in g, g
+        assert r.get("FFMA2", 0) > 0 and "HMMA" not in r and "UTCHMMA" not in r, r
+
+
 def test_product_never_imports_the_oracle():
     pkg = os.path.join(ROOT, "paper_2607_02640_b200")
     for dirpath, _, files in os.walk(pkg):
