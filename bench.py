@@ -38,7 +38,9 @@ UNIT = "session-frames/s (per layer)"
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=400)
+    ap.add_argument("--steps", type=int, default=0,
+                    help="timed frames (default: 400 for config 2; 20 for configs 3-5, whose sessions would otherwise age "
+                         "past the config's own age range during the run)")
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="metronome", choices=["metronome", "reference"])
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config index 1..5 (2 = the metric's)")
@@ -46,6 +48,11 @@ def parse():
     ap.add_argument("--sessions", type=int, default=0, help="override the session count (0 = the config's)")
     ap.add_argument("--family", type=int, default=0, help="0 auto, 1 CUDA-core rows, 2 tensor-core tiles")
     ap.add_argument("--split-tokens", type=int, default=0)
+    ap.add_argument("--two-calls", action="store_true",
+                    help="issue every sub-step as metronome_append_kv + metronome_attend_frame instead of the one-call "
+                         "metronome_append_attend (A/B of the fused decode step)")
+    ap.add_argument("--fused-step", action="store_true",
+                    help="run GQA decode steps as one launch (step_gqa.cuh; measured slower than the two launches, off by default)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--layers", type=int, default=1,
@@ -294,6 +301,8 @@ def run_reference(args):
 
 def main():
     args = parse()
+    if args.steps <= 0:
+        args.steps = 400 if args.config == 2 else 20
     if args.impl == "reference":
         return run_reference(args)
 
@@ -347,7 +356,7 @@ def main():
     events, info = wl.build_schedule(w, history_scale=args.history_scale)
     NL = max(1, args.layers)
     r = Runner(w, n_layers=NL, uid_base=replicas.uid_base(RANK))
-    r.pool.set_tuning(args.split_tokens, args.family)
+    r.pool.set_tuning(args.split_tokens, args.family, 0, 2 if args.fused_step else 0)
     t_hist = time.perf_counter()
     rest = r.run_history(events)
     torch.cuda.synchronize()
@@ -395,8 +404,11 @@ def main():
                 r.pool.session_close(item[1]); continue
             st, k, v, q, o, _ = item
             for layer in range(NL):                   # the same rows stand in for every layer's K/V/Q
-                r.pool.append_kv(layer, st.sids, st.n_new, k, v)
-                r.pool.attend_frame(layer, st.sids, st.n_new, q, o)
+                if args.two_calls:
+                    r.pool.append_kv(layer, st.sids, st.n_new, k, v)
+                    r.pool.attend_frame(layer, st.sids, st.n_new, q, o)
+                else:
+                    r.pool.append_attend(layer, st.sids, st.n_new, k, v, q, o)
 
     def finish_closes(prepped):
         for item in prepped:
@@ -440,6 +452,8 @@ def main():
             total += e0.elapsed_time(e1)
             if churn:
                 finish_closes(prepped)
+                # (one frame's K/V/Q at a time: keep the step records, drop the tensors)
+                prepped = [it if it[0] == "close" else (it[0], None, None, None, None, it[5]) for it in prepped]
             allp += prepped
         if not churn:
             finish_closes(allp)

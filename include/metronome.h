@@ -38,7 +38,7 @@
 extern "C" {
 #endif
 
-#define METRONOME_ABI_VERSION 2
+#define METRONOME_ABI_VERSION 3
 
 /* ---- status codes --------------------------------------------------------------------------- */
 enum {
@@ -164,6 +164,19 @@ int metronome_append_kv(metronome_pool_t* pool, int32_t layer, int32_t n_batch,
 int metronome_attend_frame(metronome_pool_t* pool, int32_t layer, int32_t n_batch,
                            const int32_t* sids, const int32_t* q_lens,
                            const void* q, void* out, void* cuda_stream);
+
+/* One sub-step of a frame in ONE call: exactly metronome_append_kv(layer, sids, n_new, k_new, v_new)
+ * followed by metronome_attend_frame(layer, sids, q_lens = n_new, q, out) -- same arguments, same
+ * results, same errors (union of the two; on any error nothing has changed) -- which is the shape of
+ * every sub-step of PAPER.md:L46 ("prefill the new chunk, then decode up to tau output tokens": each
+ * appends its tokens and attends from them), in one call: one validation, one plan, and the library is free
+ * to run both halves in one launch where that pays (a tuning knob of metronome_measure.h; today it runs the
+ * two kernels back to back).  k_new / v_new / q are read, out is written, in stream order by the kernels of
+ * this call.  Deviation from SURVEY.md sec. 8(b), which lists the two calls only; they remain. */
+int metronome_append_attend(metronome_pool_t* pool, int32_t layer, int32_t n_batch,
+                            const int32_t* sids, const int32_t* n_new,
+                            const void* k_new, const void* v_new,
+                            const void* q, void* out, void* cuda_stream);
 
 /* append_kv followed by attend_frame(q_lens = n_new) with HOST buffers: k_new, v_new, q are copied
  * host->device, out device->host, all on cuda_stream, and the stream is synchronised before

@@ -18,10 +18,19 @@ int metronome_pool_stats(metronome_pool_t* pool, int64_t* kernel_launches, int64
 
 /* Tuning knobs (0 = automatic): keys per split-KV segment target; the kernel family (1 CUDA-core row
  * kernel, 2 tensor-core kernels: mma.sync GQA decode + tcgen05 chunk prefill); the GQA decode kernel's
- * dynamically claimed tail ranges (1 forced on, 2 forced off; automatic = on for shares >= 512 tiles).
+ * dynamically claimed tail ranges (1 forced on, 2 forced off; automatic = on for shares >= 512 tiles);
+ * fused_step 2 = metronome_append_attend runs a decode step of a grouped-query pool as ONE launch (step_gqa.cuh;
+ * built and verified, but measured 0.4-4.5 % slower per frame than the two launches on B200, so it is off unless
+ * asked for: DESIGN.md sec. 5.2); setting it measures the SMs' streaming speeds once (metronome_pool_sm_speeds).
  * For benchmarks and tests of "both launch modes" (L258).  Errors: INVALID_ARG. */
 int metronome_pool_set_tuning(metronome_pool_t* pool, int32_t split_tokens, int32_t kernel_family,
-                              int32_t gqa_dynamic);
+                              int32_t gqa_dynamic, int32_t fused_step);
+
+/* What set_tuning(fused_step = 2) measured (otherwise 0 slow SMs, ratio 1): the SMs of one GPU do not
+ * stream at the same speed when all of them stream, and the fused decode step gives the warps that run on the slow
+ * ones shorter ranges.  n_sms = SMs of the device, n_slow_sms = those whose mean time was > 4 % above the median
+ * SM's, slow_ratio = their speed relative to the others (0.75 .. 1).  All pointers host, optional. */
+int metronome_pool_sm_speeds(metronome_pool_t* pool, int32_t* n_sms, int32_t* n_slow_sms, double* slow_ratio);
 
 /* Test aid for the "no state change on error" contract: the NEXT append_kv(layer 0) fails as if
  * (stage 1) growing the split-KV workspace had run out of memory, or (stage 2) the launch of the append

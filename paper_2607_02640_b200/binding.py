@@ -26,9 +26,9 @@ ERR_NAMES = {0: "OK", 1: "INVALID_ARG", 2: "INVALID_SESSION", 3: "DUPLICATE_SESS
 EXPORTS = ["metronome_abi_version", "metronome_strerror", "metronome_last_cuda_error",
            "metronome_kv_storage_bytes", "metronome_max_blocks_per_session", "metronome_pool_create",
            "metronome_pool_destroy", "metronome_session_open", "metronome_session_close",
-           "metronome_append_kv", "metronome_attend_frame", "metronome_step_host",
+           "metronome_append_kv", "metronome_attend_frame", "metronome_append_attend", "metronome_step_host",
            "metronome_session_query", "metronome_pool_query", "metronome_read_kv", "metronome_pool_stats",
-           "metronome_pool_set_tuning", "metronome_pool_debug_fail_next", "metronome_pool_debug_read_flags", "metronome_pool_set_profiling", "metronome_pool_read_profile", "metronome_pool_read_stamps",
+           "metronome_pool_set_tuning", "metronome_pool_sm_speeds", "metronome_pool_debug_fail_next", "metronome_pool_debug_read_flags", "metronome_pool_set_profiling", "metronome_pool_read_profile", "metronome_pool_read_stamps",
            "metronome_gate_create", "metronome_gate_destroy", "metronome_gate_observe", "metronome_gate_admit",
            "metronome_stream_read_gbs"]
 
@@ -75,13 +75,16 @@ def load():
     lib.metronome_session_close.argtypes = [c_void_p, c_int32, c_void_p]
     lib.metronome_append_kv.argtypes = [c_void_p, c_int32, c_int32, i32p, i32p, c_void_p, c_void_p, c_void_p]
     lib.metronome_attend_frame.argtypes = [c_void_p, c_int32, c_int32, i32p, i32p, c_void_p, c_void_p, c_void_p]
+    lib.metronome_append_attend.argtypes = [c_void_p, c_int32, c_int32, i32p, i32p, c_void_p, c_void_p, c_void_p,
+                                            c_void_p, c_void_p]
     lib.metronome_step_host.argtypes = [c_void_p, c_int32, c_int32, i32p, i32p, c_void_p, c_void_p, c_void_p,
                                         c_void_p, c_void_p]
     lib.metronome_session_query.argtypes = [c_void_p, c_int32, c_void_p, POINTER(c_int64), i32p, i32p, i32p]
     lib.metronome_pool_query.argtypes = [c_void_p, c_void_p, i32p, i32p]
     lib.metronome_read_kv.argtypes = [c_void_p, c_int32, c_int32, c_int64, c_int32, c_void_p, c_void_p, c_void_p]
     lib.metronome_pool_stats.argtypes = [c_void_p, POINTER(c_int64), POINTER(c_int64), POINTER(c_int64)]
-    lib.metronome_pool_set_tuning.argtypes = [c_void_p, c_int32, c_int32, c_int32]
+    lib.metronome_pool_set_tuning.argtypes = [c_void_p, c_int32, c_int32, c_int32, c_int32]
+    lib.metronome_pool_sm_speeds.argtypes = [c_void_p, i32p, i32p, POINTER(ctypes.c_double)]
     lib.metronome_pool_debug_fail_next.argtypes = [c_void_p, c_int32]
     lib.metronome_pool_debug_read_flags.argtypes = [c_void_p, c_void_p, i32p]
     lib.metronome_pool_set_profiling.argtypes = [c_void_p, c_int32]
@@ -172,6 +175,12 @@ class Pool:
         self._check(self._lib.metronome_attend_frame(self._h, layer, len(s), sp, np_, _ptr(q), _ptr(out),
                                                      c_void_p(stream)))
 
+    def append_attend(self, layer, sids, n_new, k_new, v_new, q, out, stream=0):
+        s, sp = _i32(sids)
+        n, np_ = _i32(n_new)
+        self._check(self._lib.metronome_append_attend(self._h, layer, len(s), sp, np_, _ptr(k_new), _ptr(v_new),
+                                                      _ptr(q), _ptr(out), c_void_p(stream)))
+
     def step_host(self, layer, sids, n_new, k_host, v_host, q_host, out_host, stream=0):
         s, sp = _i32(sids)
         n, np_ = _i32(n_new)
@@ -202,8 +211,14 @@ class Pool:
         self._check(self._lib.metronome_pool_stats(self._h, byref(a), byref(b), byref(c)))
         return {"kernel_launches": a.value, "append_calls": b.value, "attend_calls": c.value}
 
-    def set_tuning(self, split_tokens=0, kernel_family=0, gqa_dynamic=0):
-        self._check(self._lib.metronome_pool_set_tuning(self._h, split_tokens, kernel_family, gqa_dynamic))
+    def set_tuning(self, split_tokens=0, kernel_family=0, gqa_dynamic=0, fused_step=0):
+        self._check(self._lib.metronome_pool_set_tuning(self._h, split_tokens, kernel_family, gqa_dynamic, fused_step))
+
+    def sm_speeds(self):
+        """-> (SMs, slow SMs, their relative speed) as measured at pool creation."""
+        n, ns, r = c_int32(), c_int32(), ctypes.c_double()
+        self._check(self._lib.metronome_pool_sm_speeds(self._h, byref(n), byref(ns), byref(r)))
+        return n.value, ns.value, r.value
 
     def debug_fail_next(self, stage: int):
         self._check(self._lib.metronome_pool_debug_fail_next(self._h, stage))

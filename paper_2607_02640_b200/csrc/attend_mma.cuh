@@ -58,6 +58,8 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
 }
+// generic-proxy accesses to shared memory before, async-proxy (bulk copy / UMMA) accesses after
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void ldsm_x4(uint32_t addr, uint32_t& d0, uint32_t& d1, uint32_t& d2, uint32_t& d3) {
     asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];"
                  : "=r"(d0), "=r"(d1), "=r"(d2), "=r"(d3) : "r"(addr));
@@ -88,7 +90,8 @@ struct WarpTile {
     bool va, vb;
     int64_t qrow_a, qrow_b;                  // (query row, q head) flattened: row of q / out
 
-    __device__ __forceinline__ void init(const AttendParams& p, const AttendItem& it, int32_t kvh, int32_t mtile,
+    template <typename Item>                 // AttendItem, or the fused step kernel's StepGeo (same field names)
+    __device__ __forceinline__ void init(const AttendParams& p, const Item& it, int32_t kvh, int32_t mtile,
                                          int32_t lane) {
         const int32_t R = it.q_len * p.G;
         const int32_t t_first = it.len - it.q_len;            // reading R15: the last q_len positions
@@ -242,7 +245,8 @@ struct WarpTile {
 };
 
 // logical block and first token position of tile `tile` of an item (sinks first, then the window)
-__device__ __forceinline__ int32_t tile_block(const AttendItem& it, int32_t tile) {
+template <typename Item>
+__device__ __forceinline__ int32_t tile_block(const Item& it, int32_t tile) {
     return tile < it.n_sink_tiles ? tile : it.first_blk + (tile - it.n_sink_tiles);
 }
 

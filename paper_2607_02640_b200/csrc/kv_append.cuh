@@ -50,6 +50,31 @@ struct AppendParams {
 
 constexpr int kAppendSmemItems = 1024;       // AppendItems the bookkeeping CTA stages in shared memory
 
+// The two phases of bookkeeping.cuh over the whole batch by ONE CTA (any block size), then the call's
+// epoch is published in *bk_flag (release): table entries of blocks allocated in this call are valid
+// for whoever has seen it (acquire).
+__device__ __forceinline__ void bookkeeping_phases(const AppendParams& a, const AppendItem* items) {
+    // phase 1: evict (a2) -- PAPER.md:L256 "frees blocks that fall entirely behind the window"
+    for (int i = threadIdx.x; i < a.n_items; i += blockDim.x) {
+        const AppendItem it = items[i];
+        const int32_t* row = a.table + (int64_t)it.sid * a.tbl_width;
+        for (int k = 0; k < it.n_freed; ++k)
+            a.free_stack[a.n_free0 + it.free_off + k] = row[table_slot(it.free_lo + k, a.n_sink, a.ring)];
+    }
+    __syncthreads();
+    // phase 2: allocate (a3) -- pops from the top of the stack, batch order, ascending logical block
+    const int32_t top = a.n_free0 + a.total_freed - 1;
+    for (int i = threadIdx.x; i < a.n_items; i += blockDim.x) {
+        const AppendItem it = items[i];
+        int32_t* row = a.table + (int64_t)it.sid * a.tbl_width;
+        for (int k = 0; k < it.n_alloc; ++k)
+            row[table_slot(it.alloc_lo + k, a.n_sink, a.ring)] = a.free_stack[top - (it.alloc_off + k)];
+    }
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(a.bk_flag), "r"(a.epoch) : "memory");
+}
+
 __global__ void __launch_bounds__(256)
 append_fused_kernel(const AppendParams a) {
     extern __shared__ __align__(16) uint8_t smem_items[];
@@ -112,26 +137,7 @@ append_fused_kernel(const AppendParams a) {
         }
         if (!a.do_bookkeeping) return;
         __syncthreads();          // the staged AppendItems are complete in shared memory
-        const AppendItem* items = staged ? reinterpret_cast<const AppendItem*>(smem_items) : a.items;
-        // phase 1: evict (a2) -- PAPER.md:L256 "frees blocks that fall entirely behind the window"
-        for (int i = threadIdx.x; i < a.n_items; i += 256) {
-            const AppendItem it = items[i];
-            const int32_t* row = a.table + (int64_t)it.sid * a.tbl_width;
-            for (int k = 0; k < it.n_freed; ++k)
-                a.free_stack[a.n_free0 + it.free_off + k] = row[table_slot(it.free_lo + k, a.n_sink, a.ring)];
-        }
-        __syncthreads();
-        // phase 2: allocate (a3) -- pops from the top of the stack, batch order, ascending logical block
-        const int32_t top = a.n_free0 + a.total_freed - 1;
-        for (int i = threadIdx.x; i < a.n_items; i += 256) {
-            const AppendItem it = items[i];
-            int32_t* row = a.table + (int64_t)it.sid * a.tbl_width;
-            for (int k = 0; k < it.n_alloc; ++k)
-                row[table_slot(it.alloc_lo + k, a.n_sink, a.ring)] = a.free_stack[top - (it.alloc_off + k)];
-        }
-        __threadfence();
-        __syncthreads();
-        if (threadIdx.x == 0) asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(a.bk_flag), "r"(a.epoch) : "memory");
+        bookkeeping_phases(a, staged ? reinterpret_cast<const AppendItem*>(smem_items) : a.items);
         return;
     }
     // ---- scatter CTAs (a4) ----

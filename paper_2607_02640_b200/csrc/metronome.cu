@@ -22,6 +22,7 @@
 #include "attend_umma.cuh"
 #include "bookkeeping.cuh"
 #include "kv_append.cuh"
+#include "step_gqa.cuh"
 
 using namespace metronome;
 
@@ -60,6 +61,10 @@ struct AttendPlan {
     int32_t n_range_items = 0;        // int32 entries after the AttendItems (0: kernels search)
     bool early = false;               // the append kernel of this step runs in early mode (see append_fused_kernel)
     int64_t total_rows = 0;
+    // fused decode step (step_gqa.cuh): every item is decode class and the list fits the kernel parameters
+    bool step_ok = false;
+    GqaPlan step_plan{};              // its two lists of ranges (long: fast SMs, short: slow SMs)
+    int32_t step_workers = 0;         // warps of the launch (4 per CTA but the bookkeeping one)
 };
 
 }  // namespace
@@ -80,6 +85,7 @@ struct metronome_pool {
     std::vector<int64_t> layer_epoch;  // epoch of each layer's latest append
     std::vector<int32_t> last_sids, last_n_new;
     AttendPlan cached_plan;            // plan of attend_frame(q_lens = n_new) for the latest layer-0 append
+    std::vector<StepItem> step_items;  // the same work list in the fused step kernel's 16-byte form (cached_plan.step_ok)
     std::vector<Session> undo_sessions;          // append_kv's rollback snapshot (members: no allocation per call)
     std::vector<int32_t> undo_sids, undo_n_new;
     int32_t inject_fault = 0;          // metronome_pool_debug_fail_next (one-shot, tests of the error path)
@@ -118,10 +124,14 @@ struct metronome_pool {
     unsigned long long* d_stamps = nullptr;    // [kStampSlots][2]
     std::vector<int32_t> stamp_kind;   // per used slot: 1 rows, 2 gqa decode, 3 chunk
 
-    int32_t tune_split_tokens = 0, tune_family = 0, tune_gqa_dynamic = 0;
+    int32_t tune_split_tokens = 0, tune_family = 0, tune_gqa_dynamic = 0, tune_fused_step = 0;
     int32_t n_sm = 148;
     int64_t n_launch = 0, n_append = 0, n_attend = 0;
     std::string cuda_err;
+    StepParams step_params{};          // launch parameters of the fused step kernel (16 KB: not on the stack)
+    uint8_t sm_class[kStepMaxSms] = {};   // 1: an SM that streams slower than the rest (calibrate_sm_speeds)
+    int32_t n_slow_sms = 0;
+    double slow_ratio = 1.0;           // speed of the slow SMs relative to the fast ones
 };
 
 namespace {
@@ -223,6 +233,54 @@ int ensure_workspace(metronome_pool* pool, size_t slots) {
     return METRONOME_OK;
 }
 
+// Which SMs stream slower than the rest, and by how much (the fused step kernel cuts its ranges accordingly).
+// Three passes of step_calibrate_kernel over the pool's own KV storage; the first warms up.  An SM is "slow" when
+// its mean time is more than 4 % above the median SM's.  Leaves "no slow SMs" behind on any failure.
+void calibrate_sm_speeds(metronome_pool* pool) {
+    const metronome_pool_config_t& c = pool->cfg;
+    pool->n_slow_sms = 0;
+    pool->slow_ratio = 1.0;
+    memset(pool->sm_class, 0, sizeof(pool->sm_class));
+    if (pool->n_sm > kStepMaxSms || c.n_blocks < 64) return;
+    const int n_ctas = pool->n_sm * StepCfg<128, 1>::kCtasPerSm, n_warps = n_ctas * StepCfg<128, 1>::NWARP;
+    unsigned long long* d_out = nullptr;
+    if (cudaMalloc(&d_out, (size_t)n_warps * 2 * sizeof(unsigned long long)) != cudaSuccess) { cudaGetLastError(); return; }
+    std::vector<unsigned long long> h((size_t)n_warps * 2);
+    std::vector<double> t_sm(pool->n_sm, 0.0), n_sm_w(pool->n_sm, 0.0);
+    bool ok = true;
+    for (int pass = 0; pass < 3 && ok; ++pass) {
+        if (c.head_dim == 128)
+            step_calibrate_kernel<128><<<n_ctas, StepCfg<128, 1>::kThreads, StepCfg<128, 1>::kSmemBytes>>>(pool->d_kv, pool->L, c.n_blocks, 96, d_out);
+        else
+            step_calibrate_kernel<64><<<n_ctas, StepCfg<64, 1>::kThreads, StepCfg<64, 1>::kSmemBytes>>>(pool->d_kv, pool->L, c.n_blocks, 96, d_out);
+        ok = cudaMemcpy(h.data(), d_out, h.size() * sizeof(unsigned long long), cudaMemcpyDeviceToHost) == cudaSuccess;
+        if (!ok || pass == 0) continue;
+        for (int w = 0; w < n_warps; ++w) {
+            const unsigned long long sm = h[2 * (size_t)w];
+            if (sm < (unsigned long long)pool->n_sm) { t_sm[sm] += (double)h[2 * (size_t)w + 1]; n_sm_w[sm] += 1.0; }
+        }
+    }
+    cudaFree(d_out);
+    if (!ok) { cudaGetLastError(); return; }
+    std::vector<double> mean;
+    for (int s = 0; s < pool->n_sm; ++s)
+        if (n_sm_w[s] > 0) mean.push_back(t_sm[s] / n_sm_w[s]);
+    if ((int)mean.size() < pool->n_sm) return;                 // (an SM that got no CTA: leave the ranges equal)
+    std::vector<double> sorted = mean;
+    std::sort(sorted.begin(), sorted.end());
+    const double med = sorted[sorted.size() / 2];
+    double t_fast = 0.0, t_slow = 0.0;
+    int n_fast = 0, n_slow = 0;
+    for (int s = 0; s < pool->n_sm; ++s) {
+        const bool slow = mean[s] > 1.04 * med;
+        pool->sm_class[s] = slow ? 1 : 0;
+        if (slow) { t_slow += mean[s]; ++n_slow; } else { t_fast += mean[s]; ++n_fast; }
+    }
+    if (n_slow == 0 || n_fast == 0 || n_slow > pool->n_sm / 2) { memset(pool->sm_class, 0, sizeof(pool->sm_class)); return; }
+    pool->n_slow_sms = n_slow;
+    pool->slow_ratio = std::max(0.75, std::min(1.0, (t_fast / n_fast) / (t_slow / n_slow)));
+}
+
 // ---- row a8: the per-call work list, from the shadow counts ------------------------------------
 // Kernel families (north_star: "Tensor cores are used only for the GQA-group x chunk QK^T/PV tiles,
 // where the work really is a dense contraction"):
@@ -231,8 +289,9 @@ int ensure_workspace(metronome_pool* pool, size_t slots) {
 //   gqa    tensor-core stream-K decode kernel: items with R = G x q_len <= 16
 //   chunk  tcgen05 / TMEM chunk-prefill kernel: items with 16 < R <= 256
 // Fills items[0 .. plan.n_items) (host memory) and the plan; grows the split workspace if needed.
+// `step_items` (may be null): also plan the fused decode step and leave its work list there.
 int plan_attend(metronome_pool* pool, int32_t n_batch, const int32_t* sids, const int32_t* q_lens, AttendItem* items,
-                AttendPlan& pl) {
+                AttendPlan& pl, std::vector<StepItem>* step_items = nullptr) {
     const metronome_pool_config_t& c = pool->cfg;
     pl = AttendPlan();
     int32_t max_q = 0;
@@ -334,6 +393,42 @@ int plan_attend(metronome_pool* pool, int32_t n_batch, const int32_t* sids, cons
                 its[i].n_splits = pieces;      // upper bound on the pieces of one (item, head) pair
                 if (pieces > pl.max_splits) pl.max_splits = pieces;
             }
+            // The fused decode step (step_gqa.cuh): one contiguous range per WARP of a single wave (CTA 0 of
+            // that kernel does the bookkeeping), at least 8 tiles each; the work list in 16 bytes per item.
+            if (step_items && n_cls[1] == 0 && n <= kStepMaxItems && c.n_kv_heads <= 255 && pool->tune_fused_step == 2) {
+                // One contiguous range per warp of a single wave (minus the bookkeeping CTA), at least 8 tiles each:
+                // long ranges for the warps on fast SMs, ranges shorter by the measured speed ratio for those on slow SMs.
+                const int32_t wps = step_workers_per_sm(pool->G * pl.cls_max_q[0]);
+                const int64_t workers_max = (int64_t)pool->n_sm * wps - StepCfg<128, 1>::NWARP;
+                GqaPlan& sg = pl.step_plan;
+                sg = GqaPlan{};
+                sg.n_kv_heads = c.n_kv_heads;
+                sg.total_tiles = total_tiles;
+                const int64_t share = (total_tiles + workers_max - 1) / workers_max;
+                if (pool->tune_split_tokens > 0 || share < 16 || pool->n_slow_sms == 0) {
+                    sg.q1 = sg.q2 = pool->tune_split_tokens > 0 ? min_tiles : std::max<int64_t>(8, share);
+                    sg.n_static = sg.n_total = (int32_t)((total_tiles + sg.q1 - 1) / sg.q1);
+                    sg.g1 = total_tiles;
+                } else {
+                    const int64_t n_short = (int64_t)pool->n_slow_sms * wps;
+                    const int64_t n_long = workers_max - n_short;
+                    sg.q1 = (int64_t)std::ceil((double)total_tiles / ((double)n_long + pool->slow_ratio * (double)n_short));
+                    sg.q2 = std::max<int64_t>(1, (int64_t)std::ceil(pool->slow_ratio * (double)sg.q1));
+                    sg.n_static = (int32_t)std::min<int64_t>(n_long, (total_tiles + sg.q1 - 1) / sg.q1);
+                    sg.g1 = std::min<int64_t>(sg.q1 * sg.n_static, total_tiles);
+                    sg.n_total = sg.n_static + (int32_t)((total_tiles - sg.g1 + sg.q2 - 1) / sg.q2);
+                }
+                const int64_t ctas = std::min<int64_t>(workers_max / StepCfg<128, 1>::NWARP,
+                                                       ((int64_t)sg.n_total + StepCfg<128, 1>::NWARP - 1) / StepCfg<128, 1>::NWARP);
+                pl.step_workers = (int32_t)(ctas * StepCfg<128, 1>::NWARP);
+                step_items->resize(n);
+                for (int i = 0; i < n; ++i) {
+                    (*step_items)[i] = StepItem{its[i].sid | (its[i].q_len << 16), its[i].len, its[i].q_row_off, its[i].tile_off};
+                    const int32_t pieces = (int32_t)((its[i].n_tiles + sg.q2 - 1) / sg.q2) + 2;
+                    if (pieces > pl.max_splits) pl.max_splits = pieces;
+                }
+                pl.step_ok = true;
+            }
             continue;
         }
         // segments sized for >= 2 waves of CTAs, each with a useful run of tiles
@@ -387,8 +482,7 @@ unsigned long long* next_stamp(metronome_pool* pool, int32_t kind) {
 // Launches the attention kernels (rows a5 / a7) and the split merge (a6) of one attend_frame call.
 // `pdl`: the work list was written by the append kernel that precedes this launch on the stream
 // (cached plan): launch programmatically so the prologue overlaps that kernel's tail.
-int launch_attend(metronome_pool* pool, int32_t layer, const AttendPlan& pl, const AttendItem* d_items, const void* q,
-                  void* out, cudaStream_t st, bool pdl) {
+AttendParams make_attend_params(metronome_pool* pool, int32_t layer, const AttendPlan& pl, const void* q, void* out) {
     const metronome_pool_config_t& c = pool->cfg;
     AttendParams p{};
     p.table = pool->d_table;
@@ -403,15 +497,23 @@ int launch_attend(metronome_pool* pool, int32_t layer, const AttendPlan& pl, con
     p.ws_acc = pool->d_ws_acc; p.ws_ml = pool->d_ws_ml;
     p.max_splits = pl.max_splits;
     p.tickets = pool->d_tickets;
-    p.range_item = pl.n_range_items ? reinterpret_cast<const int32_t*>(d_items + pl.n_items) : nullptr;
     p.gqa_ctr = pool->d_bk_flag + 2;              // same 16-byte allocation: [flag, -, claims, exits]
     // measured on B200 (configs 2-4): letting the next append kernel launch early hides its host-memory
     // reads behind the attention kernel (-4..6 % per frame)
     p.pdl_early = 1;
+    p.items_flag = pool->d_bk_flag + 1;
+    p.items_epoch = -1;
+    return p;
+}
+
+int launch_attend(metronome_pool* pool, int32_t layer, const AttendPlan& pl, const AttendItem* d_items, const void* q,
+                  void* out, cudaStream_t st, bool pdl) {
+    const metronome_pool_config_t& c = pool->cfg;
+    AttendParams p = make_attend_params(pool, layer, pl, q, out);
+    p.range_item = pl.n_range_items ? reinterpret_cast<const int32_t*>(d_items + pl.n_items) : nullptr;
     // behind the fused append kernel of the same step the attention kernels may start early (they wait for
     // their work list, stream the untouched blocks, and wait for the append before the fresh ones); with the
     // poison fill or the profiling brackets in between, and on the general path, they wait at the top
-    p.items_flag = pool->d_bk_flag + 1;
     p.items_epoch = (pdl && pl.early && !pool->profiling) ? (int32_t)pl.epoch : -1;
 
     if (pool->profiling) {
@@ -585,7 +687,9 @@ int metronome_pool_create(const metronome_pool_config_t* cfg, metronome_pool_t**
     if (e != cudaSuccess) return fail(METRONOME_ERR_CUDA, e, "pool init kernels");
     e = configure_attend_mma_kernels();
     if (e == cudaSuccess) e = configure_attend_umma_kernels();
+    if (e == cudaSuccess) e = configure_step_kernels();
     if (e != cudaSuccess) return fail(METRONOME_ERR_CUDA, e, "cudaFuncSetAttribute");
+
     *out = pool;
     return METRONOME_OK;
 }
@@ -657,8 +761,15 @@ int metronome_session_close(metronome_pool_t* pool, int32_t sid, void* cuda_stre
     return METRONOME_OK;
 }
 
-int metronome_append_kv(metronome_pool_t* pool, int32_t layer, int32_t n_batch, const int32_t* sids,
-                        const int32_t* n_new, const void* k_new, const void* v_new, void* cuda_stream) {
+}  // extern "C"
+
+namespace {
+
+// metronome_append_kv, and the append half of metronome_append_attend.  `q` / `out` non-null: the caller
+// will attend exactly this batch next (q_lens = n_new); when the step can run as ONE launch
+// (step_gqa.cuh) it is launched here and *fused is set, else only the append is done.
+int append_impl(metronome_pool_t* pool, int32_t layer, int32_t n_batch, const int32_t* sids, const int32_t* n_new,
+                const void* k_new, const void* v_new, void* cuda_stream, const void* q, void* out, bool* fused) {
     if (!pool || layer < 0 || layer >= pool->cfg.n_layers) return METRONOME_ERR_INVALID_ARG;
     int rc = check_batch(pool, n_batch, sids, n_new);
     if (rc) return rc;
@@ -779,7 +890,7 @@ int metronome_append_kv(metronome_pool_t* pool, int32_t layer, int32_t n_batch, 
         // append kernel carries it to the device
         pool->cached_plan.valid = false;
         if (!pool->bookkeeping_only && total_new > 0) {
-            rc = plan_attend(pool, n_batch, sids, n_new, h_attend, pool->cached_plan);
+            rc = plan_attend(pool, n_batch, sids, n_new, h_attend, pool->cached_plan, &pool->step_items);
             if (rc) { rollback(); return rc; }
             pool->cached_plan.epoch = pool->epoch;
             have_plan = true;
@@ -833,17 +944,64 @@ int metronome_append_kv(metronome_pool_t* pool, int32_t layer, int32_t n_batch, 
         dim3 grid(std::max(1, (chunks + 255) / 256), n_batch + 1);      // (n_batch <= max_sessions <= 65534)
         const size_t smem = (fused_bookkeeping && n_batch <= kAppendSmemItems) ? (size_t)n_batch * sizeof(AppendItem) : 0;
         cudaError_t e = cudaSuccess;
+        const AttendPlan& cp = pool->cached_plan;
+        const bool fuse = q && out && fused && cp.valid && cp.epoch == pool->epoch && cp.step_ok && !unfused_bookkeeping &&
+                          !pool->poison && !pool->profiling && n_batch <= kAppendSmemItems;
         if (pool->inject_fault == 2) { pool->inject_fault = 0; e = cudaErrorLaunchFailure; }
-        else e = launch_kernel(append_fused_kernel, grid, dim3(256), smem, st, true, a);
+        else if (fuse) {
+            // rows a2-a6 of this step in ONE launch: CTA 0 does the bookkeeping, every other warp streams
+            // its share of the (item, head, tile) list and writes the new rows on the way
+            StepParams* sp = &pool->step_params;
+            sp->p = make_attend_params(pool, layer, cp, q, out);
+            sp->p.stamp = next_stamp(pool, 2);
+            sp->a = a;
+            sp->a.pdl_early = 0;
+            sp->a.attend_src = nullptr; sp->a.attend_n16 = 0;
+            sp->plan = cp.step_plan;
+            sp->n_workers = cp.step_workers;
+            sp->claim_ctr = pool->d_bk_flag + 8;
+            memcpy(sp->sm_class, pool->sm_class, sizeof(sp->sm_class));
+            sp->n_items = (int32_t)pool->step_items.size();
+            memcpy(sp->items, pool->step_items.data(), pool->step_items.size() * sizeof(StepItem));
+            e = launch_step_gqa(*sp, c.head_dim, pool->G * cp.cls_max_q[0], st, true);
+            if (e == cudaSuccess) { *fused = true; ++pool->n_attend; }
+        } else {
+            e = launch_kernel(append_fused_kernel, grid, dim3(256), smem, st, true, a);
+        }
         if (e != cudaSuccess) {
             if (!unfused_bookkeeping) rollback();      // nothing was enqueued: the call never happened
-            return cuda_fail(pool, e, "append_fused_kernel");
+            return cuda_fail(pool, e, fuse ? "step_gqa_kernel" : "append_fused_kernel");
         }
         ++pool->n_launch;
     }
     ++pool->n_append;
     if (n_batch > 0) return release_stage(pool, slot, st);
     return METRONOME_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int metronome_append_kv(metronome_pool_t* pool, int32_t layer, int32_t n_batch, const int32_t* sids,
+                        const int32_t* n_new, const void* k_new, const void* v_new, void* cuda_stream) {
+    return append_impl(pool, layer, n_batch, sids, n_new, k_new, v_new, cuda_stream, nullptr, nullptr, nullptr);
+}
+
+int metronome_append_attend(metronome_pool_t* pool, int32_t layer, int32_t n_batch, const int32_t* sids,
+                            const int32_t* n_new, const void* k_new, const void* v_new, const void* q, void* out,
+                            void* cuda_stream) {
+    if (!pool) return METRONOME_ERR_INVALID_ARG;
+    if (pool->bookkeeping_only) return METRONOME_ERR_UNSUPPORTED;
+    // (the attention half can only fail on arguments: check them before the append changes anything)
+    int64_t rows = 0;
+    if (n_batch > 0 && n_new)
+        for (int i = 0; i < n_batch; ++i) rows += n_new[i] > 0 ? n_new[i] : 0;
+    if (rows > 0 && (!q || !out)) return METRONOME_ERR_INVALID_ARG;
+    bool fused = false;
+    int rc = append_impl(pool, layer, n_batch, sids, n_new, k_new, v_new, cuda_stream, q, out, &fused);
+    if (rc || fused) return rc;
+    return metronome_attend_frame(pool, layer, n_batch, sids, n_new, q, out, cuda_stream);
 }
 
 int metronome_attend_frame(metronome_pool_t* pool, int32_t layer, int32_t n_batch, const int32_t* sids,
@@ -915,9 +1073,8 @@ int metronome_step_host(metronome_pool_t* pool, int32_t layer, int32_t n_batch, 
         CU(cudaMemcpyAsync(dv, v_new_host, kv_b, cudaMemcpyHostToDevice, st));
         CU(cudaMemcpyAsync(dq, q_host, q_b, cudaMemcpyHostToDevice, st));
     }
-    int rc = metronome_append_kv(pool, layer, n_batch, sids, n_new, rows ? dk : nullptr, rows ? dv : nullptr, cuda_stream);
-    if (rc) return rc;
-    rc = metronome_attend_frame(pool, layer, n_batch, sids, n_new, dq, dout, cuda_stream);
+    int rc = metronome_append_attend(pool, layer, n_batch, sids, n_new, rows ? dk : nullptr, rows ? dv : nullptr, dq, dout,
+                                     cuda_stream);
     if (rc) return rc;
     if (rows > 0) CU(cudaMemcpyAsync(out_host, dout, q_b, cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
@@ -990,6 +1147,14 @@ int metronome_pool_stats(metronome_pool_t* pool, int64_t* kernel_launches, int64
     if (kernel_launches) *kernel_launches = pool->n_launch;
     if (append_calls) *append_calls = pool->n_append;
     if (attend_calls) *attend_calls = pool->n_attend;
+    return METRONOME_OK;
+}
+
+int metronome_pool_sm_speeds(metronome_pool_t* pool, int32_t* n_sms, int32_t* n_slow_sms, double* slow_ratio) {
+    if (!pool) return METRONOME_ERR_INVALID_ARG;
+    if (n_sms) *n_sms = pool->n_sm;
+    if (n_slow_sms) *n_slow_sms = pool->n_slow_sms;
+    if (slow_ratio) *slow_ratio = pool->slow_ratio;
     return METRONOME_OK;
 }
 
@@ -1137,12 +1302,19 @@ int metronome_pool_debug_read_flags(metronome_pool_t* pool, void* cuda_stream, i
     return METRONOME_OK;
 }
 
-int metronome_pool_set_tuning(metronome_pool_t* pool, int32_t split_tokens, int32_t kernel_family, int32_t gqa_dynamic) {
-    if (!pool || split_tokens < 0 || kernel_family < 0 || kernel_family > 2 || gqa_dynamic < 0 || gqa_dynamic > 2)
+int metronome_pool_set_tuning(metronome_pool_t* pool, int32_t split_tokens, int32_t kernel_family, int32_t gqa_dynamic,
+                              int32_t fused_step) {
+    if (!pool || split_tokens < 0 || kernel_family < 0 || kernel_family > 2 || gqa_dynamic < 0 || gqa_dynamic > 2 ||
+        fused_step < 0 || fused_step > 2)
         return METRONOME_ERR_INVALID_ARG;
+    if (fused_step == 2 && pool->tune_fused_step != 2 && !pool->bookkeeping_only) {
+        cudaDeviceSynchronize();
+        calibrate_sm_speeds(pool);
+    }
     pool->tune_split_tokens = split_tokens;
     pool->tune_family = kernel_family;
     pool->tune_gqa_dynamic = gqa_dynamic;
+    pool->tune_fused_step = fused_step;
     pool->cached_plan.valid = false;
     return METRONOME_OK;
 }

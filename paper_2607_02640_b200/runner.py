@@ -94,6 +94,18 @@ class Runner:
         self.pool.attend_frame(layer, st.sids, st.n_new, q, out, stream)
         return out
 
+    def step(self, st: Step, layer: int, k=None, v=None, q=None, out=None, stream=0):
+        """append + attend of one sub-step in ONE call (metronome_append_attend)."""
+        if k is None:
+            k = self.rows(synth.STREAM_K, layer, st.uid_rows, st.pos_rows)
+            v = self.rows(synth.STREAM_V, layer, st.uid_rows, st.pos_rows)
+        if q is None:
+            q = self.rows(synth.STREAM_Q, layer, st.uid_rows, st.pos_rows)
+        if out is None:
+            out = torch.empty_like(q)
+        self.pool.append_attend(layer, st.sids, st.n_new, k, v, q, out, stream)
+        return out
+
     def run_history(self, events, rows_per_batch: int = 16384):
         """Executes the untimed prefix of a schedule (opens, closes, history appends on every layer)
         and returns the remaining events.  K/V rows of many steps are generated in one go, then

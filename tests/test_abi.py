@@ -37,7 +37,7 @@ def test_every_declared_symbol_is_exported(lib):
 
 def test_host_only_entry_points(lib):
     from paper_2607_02640_b200 import binding
-    assert lib.metronome_abi_version() == 2
+    assert lib.metronome_abi_version() == 3
     assert lib.metronome_strerror(5) == b"POOL_EXHAUSTED"
     # closed form of the per-session cap for the five configs
     for (S, W, n), want in {(4, 128, 8): 11, (4, 750, 1): 49, (4, 2048, 25): 132, (4, 1024, 25): 68,

@@ -157,9 +157,11 @@ def test_kv_write_reads_back_through_the_table():
 
 
 def _run_parity(w, history_scale=1.0, n_layers=1, flags=0, family=0, split_tokens=0, max_timed=None,
-                check_tables=True, check_history_attend_every=0):
+                check_tables=True, check_history_attend_every=0, one_call=False):
+    """one_call: every attended step goes through metronome_append_attend, with the fused decode step switched on
+    (one launch for a GQA decode step)."""
     r = Runner(w, n_layers=n_layers, flags=flags)
-    r.pool.set_tuning(split_tokens, family)
+    r.pool.set_tuning(split_tokens, family, 0, 2 if one_call else 0)
     m = OracleMirror(r)
     events, _ = wl.build_schedule(w, history_scale=history_scale)
     worst = {"max_abs": 0.0, "max_rel": 0.0, "row_l2": 0.0}
@@ -179,9 +181,13 @@ def _run_parity(w, history_scale=1.0, n_layers=1, flags=0, family=0, split_token
                 hist_i += 1
                 do_attend = hist_i % check_history_attend_every == 0
             for layer in range(n_layers):
-                r.append(st, layer); m.append(st, layer)
+                m.append(st, layer)
+                if do_attend and one_call:
+                    out = r.step(st, layer)
+                else:
+                    r.append(st, layer)
                 if do_attend:
-                    out = r.attend(st, layer)
+                    out = out if one_call else r.attend(st, layer)
                     ref = m.attend(st, layer)
                     rep = assert_parity(out, ref, f"{w.name} frame {st.frame} layer {layer} n={st.n_new[:4]}",
                                         unit_scale=w.outlier_frac == 0)
