@@ -187,6 +187,19 @@ int metronome_step_host(metronome_pool_t* pool, int32_t layer, int32_t n_batch,
                         const void* k_new_host, const void* v_new_host,
                         const void* q_host, void* out_host, void* cuda_stream);
 
+/* The same step, pipelined: returns once the copies and kernels are ENQUEUED -- k/v/q host->device on a copy
+ * stream of the pool's, the step on cuda_stream, out device->host on a second copy stream, chained by events --
+ * so that the uploads of step k+1 and the read-back of step k-1 run next to the kernels of step k (two staging
+ * slots).  The host buffers of a step must stay untouched, and out_host is not valid, until
+ * metronome_step_host_wait(pool, keep) has returned with that step among the finished ones: it blocks until at
+ * most `keep` (0, 1 or more) of the steps issued so far are still in flight.  Steps complete in issue order.
+ * Errors: as metronome_step_host; an error leaves the pool as it was (the step was not enqueued). */
+int metronome_step_host_async(metronome_pool_t* pool, int32_t layer, int32_t n_batch,
+                              const int32_t* sids, const int32_t* n_new,
+                              const void* k_new_host, const void* v_new_host,
+                              const void* q_host, void* out_host, void* cuda_stream);
+int metronome_step_host_wait(metronome_pool_t* pool, int32_t keep);
+
 /* ---- introspection (bit-exact parity of tables and free list; occupancy signal, L83) ---------- */
 
 /* All out-pointers are host and optional (NULL = skip).  Blocks the host until cuda_stream has

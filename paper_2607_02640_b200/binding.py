@@ -26,7 +26,7 @@ ERR_NAMES = {0: "OK", 1: "INVALID_ARG", 2: "INVALID_SESSION", 3: "DUPLICATE_SESS
 EXPORTS = ["metronome_abi_version", "metronome_strerror", "metronome_last_cuda_error",
            "metronome_kv_storage_bytes", "metronome_max_blocks_per_session", "metronome_pool_create",
            "metronome_pool_destroy", "metronome_session_open", "metronome_session_close",
-           "metronome_append_kv", "metronome_attend_frame", "metronome_append_attend", "metronome_step_host",
+           "metronome_append_kv", "metronome_attend_frame", "metronome_append_attend", "metronome_step_host", "metronome_step_host_async", "metronome_step_host_wait",
            "metronome_session_query", "metronome_pool_query", "metronome_read_kv", "metronome_pool_stats",
            "metronome_pool_set_tuning", "metronome_pool_sm_speeds", "metronome_pool_debug_fail_next", "metronome_pool_debug_read_flags", "metronome_pool_set_profiling", "metronome_pool_read_profile", "metronome_pool_read_stamps",
            "metronome_gate_create", "metronome_gate_destroy", "metronome_gate_observe", "metronome_gate_admit",
@@ -79,6 +79,8 @@ def load():
                                             c_void_p, c_void_p]
     lib.metronome_step_host.argtypes = [c_void_p, c_int32, c_int32, i32p, i32p, c_void_p, c_void_p, c_void_p,
                                         c_void_p, c_void_p]
+    lib.metronome_step_host_async.argtypes = lib.metronome_step_host.argtypes
+    lib.metronome_step_host_wait.argtypes = [c_void_p, c_int32]
     lib.metronome_session_query.argtypes = [c_void_p, c_int32, c_void_p, POINTER(c_int64), i32p, i32p, i32p]
     lib.metronome_pool_query.argtypes = [c_void_p, c_void_p, i32p, i32p]
     lib.metronome_read_kv.argtypes = [c_void_p, c_int32, c_int32, c_int64, c_int32, c_void_p, c_void_p, c_void_p]
@@ -186,6 +188,15 @@ class Pool:
         n, np_ = _i32(n_new)
         self._check(self._lib.metronome_step_host(self._h, layer, len(s), sp, np_, _ptr(k_host), _ptr(v_host),
                                                   _ptr(q_host), _ptr(out_host), c_void_p(stream)))
+
+    def step_host_async(self, layer, sids, n_new, k_host, v_host, q_host, out_host, stream=0):
+        s, sp = _i32(sids)
+        n, np_ = _i32(n_new)
+        self._check(self._lib.metronome_step_host_async(self._h, layer, len(s), sp, np_, _ptr(k_host), _ptr(v_host),
+                                                        _ptr(q_host), _ptr(out_host), c_void_p(stream)))
+
+    def step_host_wait(self, keep=0):
+        self._check(self._lib.metronome_step_host_wait(self._h, keep))
 
     def session_query(self, sid, stream=0):
         """-> (len, first_live_block, [physical block ids in logical order])"""

@@ -104,6 +104,14 @@ struct metronome_pool {
     size_t ws_slots = 0;               // capacity in (row, head, split) slots
     uint8_t* d_io = nullptr;           // staging for metronome_step_host
     size_t io_bytes = 0;
+    // metronome_step_host_async: two staging slots, a copy stream per direction, events that chain
+    // H2D(k) -> step(k) -> D2H(k) while H2D(k+1) and D2H(k-1) run next to step(k)
+    uint8_t* d_io2[2] = {nullptr, nullptr};
+    size_t io2_bytes[2] = {0, 0};
+    cudaStream_t s_h2d = nullptr, s_d2h = nullptr;
+    cudaEvent_t ev_h2d[2]{}, ev_comp[2]{}, ev_d2h[2]{};
+    bool slot_busy[2] = {false, false};
+    int64_t host_seq = 0;              // async steps issued so far (step k uses slot k & 1)
 
     // per-call metadata staging: pinned host ring + matching device ring
     uint8_t* h_stage = nullptr;
@@ -707,6 +715,14 @@ int metronome_pool_destroy(metronome_pool_t* pool) {
     if (pool->d_ws_acc) cudaFree(pool->d_ws_acc);
     if (pool->d_ws_ml) cudaFree(pool->d_ws_ml);
     if (pool->d_io) cudaFree(pool->d_io);
+    for (int b = 0; b < 2; ++b) {
+        if (pool->d_io2[b]) cudaFree(pool->d_io2[b]);
+        if (pool->ev_h2d[b]) cudaEventDestroy(pool->ev_h2d[b]);
+        if (pool->ev_comp[b]) cudaEventDestroy(pool->ev_comp[b]);
+        if (pool->ev_d2h[b]) cudaEventDestroy(pool->ev_d2h[b]);
+    }
+    if (pool->s_h2d) cudaStreamDestroy(pool->s_h2d);
+    if (pool->s_d2h) cudaStreamDestroy(pool->s_d2h);
     if (pool->h_stage) cudaFreeHost(pool->h_stage);
     if (pool->d_stage) cudaFree(pool->d_stage);
     for (int i = 0; i < kStagingSlots / kStagingGroup; ++i)
@@ -1078,6 +1094,76 @@ int metronome_step_host(metronome_pool_t* pool, int32_t layer, int32_t n_batch, 
     if (rc) return rc;
     if (rows > 0) CU(cudaMemcpyAsync(out_host, dout, q_b, cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
+    return METRONOME_OK;
+}
+
+int metronome_step_host_wait(metronome_pool_t* pool, int32_t keep) {
+    if (!pool || keep < 0) return METRONOME_ERR_INVALID_ARG;
+    // steps host_seq-1 (newest) and host_seq-2 may be outstanding; wait for all but the newest `keep`
+    for (int64_t k = pool->host_seq - 2; k <= pool->host_seq - 1 - keep; ++k) {
+        if (k < 0) continue;
+        const int b = (int)(k & 1);
+        if (!pool->slot_busy[b]) continue;
+        CU(cudaEventSynchronize(pool->ev_d2h[b]));
+        pool->slot_busy[b] = false;
+    }
+    return METRONOME_OK;
+}
+
+int metronome_step_host_async(metronome_pool_t* pool, int32_t layer, int32_t n_batch, const int32_t* sids,
+                              const int32_t* n_new, const void* k_new_host, const void* v_new_host,
+                              const void* q_host, void* out_host, void* cuda_stream) {
+    if (!pool || n_batch < 0 || (n_batch > 0 && (!sids || !n_new))) return METRONOME_ERR_INVALID_ARG;
+    if (pool->bookkeeping_only) return METRONOME_ERR_UNSUPPORTED;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const metronome_pool_config_t& c = pool->cfg;
+    int64_t rows = 0;
+    for (int i = 0; i < n_batch; ++i) {
+        if (n_new[i] < 0) return METRONOME_ERR_INVALID_ARG;
+        if (n_new[i] > c.max_new_tokens) return METRONOME_ERR_CHUNK_TOO_LARGE;
+        rows += n_new[i];
+    }
+    if (rows > 0 && (!k_new_host || !v_new_host || !q_host || !out_host)) return METRONOME_ERR_INVALID_ARG;
+    if (!pool->s_h2d) {
+        CU(cudaStreamCreateWithFlags(&pool->s_h2d, cudaStreamNonBlocking));
+        CU(cudaStreamCreateWithFlags(&pool->s_d2h, cudaStreamNonBlocking));
+        for (int b = 0; b < 2; ++b) {
+            CU(cudaEventCreateWithFlags(&pool->ev_h2d[b], cudaEventDisableTiming));
+            CU(cudaEventCreateWithFlags(&pool->ev_comp[b], cudaEventDisableTiming));
+            CU(cudaEventCreateWithFlags(&pool->ev_d2h[b], cudaEventDisableTiming));
+        }
+    }
+    const int b = (int)(pool->host_seq & 1);
+    const size_t kv_b = (size_t)rows * c.n_kv_heads * c.head_dim * 2, q_b = (size_t)rows * c.n_q_heads * c.head_dim * 2;
+    const size_t kv_al = (kv_b + 255) & ~(size_t)255, q_al = (q_b + 255) & ~(size_t)255;
+    const size_t need = 2 * kv_al + 2 * q_al;
+    if (need > pool->io2_bytes[b]) {
+        // (the slot's previous step must be through before its buffer goes away)
+        if (pool->slot_busy[b]) { CU(cudaEventSynchronize(pool->ev_d2h[b])); pool->slot_busy[b] = false; }
+        if (pool->d_io2[b]) cudaFree(pool->d_io2[b]);
+        pool->d_io2[b] = nullptr; pool->io2_bytes[b] = 0;
+        CU(cudaMalloc(&pool->d_io2[b], need + need / 2));
+        pool->io2_bytes[b] = need + need / 2;
+    }
+    uint8_t* dk = pool->d_io2[b]; uint8_t* dv = dk + kv_al; uint8_t* dq = dv + kv_al; uint8_t* dout = dq + q_al;
+    // H2D of this step: as soon as the slot's previous step (two steps back) has been read out
+    if (pool->slot_busy[b]) CU(cudaStreamWaitEvent(pool->s_h2d, pool->ev_d2h[b], 0));
+    if (rows > 0) {
+        CU(cudaMemcpyAsync(dk, k_new_host, kv_b, cudaMemcpyHostToDevice, pool->s_h2d));
+        CU(cudaMemcpyAsync(dv, v_new_host, kv_b, cudaMemcpyHostToDevice, pool->s_h2d));
+        CU(cudaMemcpyAsync(dq, q_host, q_b, cudaMemcpyHostToDevice, pool->s_h2d));
+    }
+    CU(cudaEventRecord(pool->ev_h2d[b], pool->s_h2d));
+    CU(cudaStreamWaitEvent(st, pool->ev_h2d[b], 0));
+    int rc = metronome_append_attend(pool, layer, n_batch, sids, n_new, rows ? dk : nullptr, rows ? dv : nullptr, dq, dout,
+                                     cuda_stream);
+    if (rc) return rc;          // (nothing of this step was enqueued but its input copies)
+    CU(cudaEventRecord(pool->ev_comp[b], st));
+    CU(cudaStreamWaitEvent(pool->s_d2h, pool->ev_comp[b], 0));
+    if (rows > 0) CU(cudaMemcpyAsync(out_host, dout, q_b, cudaMemcpyDeviceToHost, pool->s_d2h));
+    CU(cudaEventRecord(pool->ev_d2h[b], pool->s_d2h));
+    pool->slot_busy[b] = true;
+    ++pool->host_seq;
     return METRONOME_OK;
 }
 

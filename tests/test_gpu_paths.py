@@ -167,3 +167,33 @@ def test_max_sessions_is_capped_where_the_append_grid_ends():
     with pytest.raises(binding.MetronomeError, match="INVALID_ARG"):
         binding.Pool(max_sessions=65535, **kw)
     binding.Pool(max_sessions=65534, **kw).destroy()
+
+
+@pytest.mark.parametrize("Hkv", [8, 2])
+def test_pipelined_host_steps_match_the_blocking_ones(Hkv):
+    """metronome_step_host_async / _wait (two staging slots, copies on the pool's own streams) give what the oracle
+    gives, step by step, with up to two steps in flight and host buffers reused only after their wait."""
+    Hq, D, S, W, N = 8, 128, 4, 48, 3
+    per = 1 + (W + 8 - 1) // 16 + 2
+    kw = dict(n_q_heads=Hq, n_kv_heads=Hkv, head_dim=D, max_sessions=N, max_new_tokens=8)
+    pool = binding.Pool(n_sinks=S, window=W, n_blocks=N * per, **kw)
+    defn = O.DefinitionOracle(O.PoolConfig(S=S, W=W, n_blocks=N * per, block_size=16, **kw))
+    sids = [pool.session_open() for _ in range(N)]
+    assert sids == [defn.session_open() for _ in range(N)]
+    rng = np.random.default_rng(3 + Hkv)
+    pending = []                                       # (out_host, reference, label) of steps not yet waited for
+    for step in range(60):
+        n_new = rng.integers(1, 9, size=N).astype(np.int32) if step % 5 == 0 else np.ones(N, np.int32)
+        rows = int(n_new.sum())
+        k, v, q = (_rows(rng, rows, H, D).pin_memory() for H in (Hkv, Hkv, Hq))
+        out = torch.empty(rows, Hq, D, dtype=torch.bfloat16).pin_memory()
+        pool.step_host_async(0, sids, n_new, k, v, q, out)
+        defn.append_kv(0, sids, [int(x) for x in n_new], synth.to_u16(k), synth.to_u16(v))
+        pending.append((out, defn.attend_frame(0, sids, [int(x) for x in n_new], synth.to_u16(q)), f"step {step}", k, v, q))
+        pool.step_host_wait(1)
+        while len(pending) > 1:
+            o, ref, what, *_ = pending.pop(0)
+            assert_parity(o, ref, what)
+    pool.step_host_wait(0)
+    for o, ref, what, *_ in pending:
+        assert_parity(o, ref, what)
