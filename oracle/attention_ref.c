@@ -53,9 +53,11 @@ int oracle_admit(int64_t j, int64_t t, int64_t S, int64_t W) {
     return 0;
 }
 
-#define DEFINE_ORACLE_ATTEND(NAME, REAL, EXPF)                                                    \
+static float kv_identity(float x) { return x; }
+
+#define DEFINE_ORACLE_ATTEND(NAME, REAL, EXPF, KVT, KVLOAD)                                       \
     int NAME(const uint16_t* q, const int64_t* q_pos, int64_t n_q,                                \
-             const uint16_t* k, const uint16_t* v, const int64_t* k_pos, int64_t n_k,             \
+             const KVT* k, const KVT* v, const int64_t* k_pos, int64_t n_k,                       \
              int32_t Hq, int32_t Hkv, int32_t D, int64_t S, int64_t W, double scale,              \
              float* out, float* weights, int32_t n_threads) {                                     \
         if (Hkv <= 0 || Hq % Hkv != 0) return 1;                                                  \
@@ -74,10 +76,10 @@ int oracle_admit(int64_t j, int64_t t, int64_t S, int64_t W) {
                 int64_t n_adm = 0;                                                                \
                 for (int64_t i = 0; i < n_k; ++i) {                                               \
                     if (!oracle_admit(k_pos[i], t, S, W)) continue;                               \
-                    const uint16_t* kv = k + ((size_t)i * Hkv + hk) * D;                          \
+                    const KVT* kv = k + ((size_t)i * Hkv + hk) * D;                               \
                     REAL dot = 0;                                                                 \
                     for (int32_t d = 0; d < D; ++d)                                               \
-                        dot += (REAL)bf16_bits_to_float(qv[d]) * (REAL)bf16_bits_to_float(kv[d]); \
+                        dot += (REAL)bf16_bits_to_float(qv[d]) * (REAL)KVLOAD(kv[d]);             \
                     s[i] = (REAL)scale * dot;                                                     \
                     if (s[i] > m) m = s[i];                                                       \
                     ++n_adm;                                                                      \
@@ -95,9 +97,9 @@ int oracle_admit(int64_t j, int64_t t, int64_t S, int64_t W) {
                 if (!acc) { free(s); failed = 1; continue; }                                      \
                 for (int64_t i = 0; i < n_k; ++i) {            /* o = sum_i p_i v_i */            \
                     if (!oracle_admit(k_pos[i], t, S, W)) continue;                               \
-                    const uint16_t* vv = v + ((size_t)i * Hkv + hk) * D;                          \
+                    const KVT* vv = v + ((size_t)i * Hkv + hk) * D;                               \
                     for (int32_t d = 0; d < D; ++d)                                               \
-                        acc[d] += s[i] * (REAL)bf16_bits_to_float(vv[d]);                         \
+                        acc[d] += s[i] * (REAL)KVLOAD(vv[d]);                                     \
                 }                                                                                 \
                 float* o = out + ((size_t)r * Hq + h) * D;                                        \
                 for (int32_t d = 0; d < D; ++d) o[d] = (n_adm > 0) ? (float)acc[d] : 0.0f;        \
@@ -116,8 +118,13 @@ int oracle_admit(int64_t j, int64_t t, int64_t S, int64_t W) {
  * weights (optional, may be NULL) [n_q][Hq][n_k] float32 softmax weights (0 where not admitted).
  * A query with no admitted key (cannot happen when the query's own key is present) yields 0.
  * Returns 0 on success. */
-DEFINE_ORACLE_ATTEND(oracle_attend_f32, float, expf)
-DEFINE_ORACLE_ATTEND(oracle_attend_f64, double, exp)
+DEFINE_ORACLE_ATTEND(oracle_attend_f32, float, expf, uint16_t, bf16_bits_to_float)
+DEFINE_ORACLE_ATTEND(oracle_attend_f64, double, exp, uint16_t, bf16_bits_to_float)
+/* The same text with k / v given as float32 VALUES (q stays bf16 bits): the fp8 KV arm (oracle/kv_fp8.py), whose
+ * dequantised keys and values code x scale are not bf16 numbers ("we bound which tokens stay
+ * resident, and the two compose"). */
+DEFINE_ORACLE_ATTEND(oracle_attend_kvf32_f32, float, expf, float, kv_identity)
+DEFINE_ORACLE_ATTEND(oracle_attend_kvf32_f64, double, exp, float, kv_identity)
 
 int32_t oracle_max_threads(void) {
 #ifdef _OPENMP

@@ -61,10 +61,11 @@ def _load():
         u16p = ctypes.POINTER(ctypes.c_uint16)
         i64p = ctypes.POINTER(ctypes.c_int64)
         f32p = ctypes.POINTER(ctypes.c_float)
-        for name in ("oracle_attend_f32", "oracle_attend_f64"):
+        for name in ("oracle_attend_f32", "oracle_attend_f64", "oracle_attend_kvf32_f32", "oracle_attend_kvf32_f64"):
             fn = getattr(lib, name)
+            kvp = f32p if "kvf32" in name else u16p
             fn.restype = ctypes.c_int
-            fn.argtypes = [u16p, i64p, ctypes.c_int64, u16p, u16p, i64p, ctypes.c_int64,
+            fn.argtypes = [u16p, i64p, ctypes.c_int64, kvp, kvp, i64p, ctypes.c_int64,
                            ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, ctypes.c_int64,
                            ctypes.c_int64, ctypes.c_double, f32p, f32p, ctypes.c_int32]
         lib.oracle_admit.restype = ctypes.c_int
@@ -87,12 +88,14 @@ def attend(q, q_pos, k, v, k_pos, S, W, scale=None, precision="f32", want_weight
            n_threads=1):
     """Masked softmax attention for ONE session (definition in attention_ref.c's header).
 
-    q [n_q,Hq,D] uint16(bf16), q_pos [n_q] absolute positions; k,v [n_k,Hkv,D], k_pos [n_k]
-    ascending.  Returns float32 out [n_q,Hq,D] (and weights [n_q,Hq,n_k] if asked)."""
+    q [n_q,Hq,D] uint16(bf16), q_pos [n_q] absolute positions; k,v [n_k,Hkv,D] uint16(bf16) -- or float32 VALUES
+    (the fp8 KV arm: dequantised rows) --, k_pos [n_k] ascending.  Returns float32 out [n_q,Hq,D] (and weights
+    [n_q,Hq,n_k] if asked)."""
     lib = _load()
     q = np.ascontiguousarray(q, dtype=np.uint16)
-    k = np.ascontiguousarray(k, dtype=np.uint16)
-    v = np.ascontiguousarray(v, dtype=np.uint16)
+    kv_f32 = np.asarray(k).dtype == np.float32
+    k = np.ascontiguousarray(k, dtype=np.float32 if kv_f32 else np.uint16)
+    v = np.ascontiguousarray(v, dtype=np.float32 if kv_f32 else np.uint16)
     q_pos = np.ascontiguousarray(q_pos, dtype=np.int64)
     k_pos = np.ascontiguousarray(k_pos, dtype=np.int64)
     n_q, Hq, D = q.shape
@@ -103,12 +106,12 @@ def attend(q, q_pos, k, v, k_pos, S, W, scale=None, precision="f32", want_weight
         scale = 1.0 / math.sqrt(D)  # reading R7
     out = np.empty((n_q, Hq, D), dtype=np.float32)
     weights = np.empty((n_q, Hq, n_k), dtype=np.float32) if want_weights else None
-    fn = lib.oracle_attend_f32 if precision == "f32" else lib.oracle_attend_f64
+    fn = getattr(lib, ("oracle_attend_kvf32_" if kv_f32 else "oracle_attend_") + ("f32" if precision == "f32" else "f64"))
     u16p = ctypes.POINTER(ctypes.c_uint16)
     i64p = ctypes.POINTER(ctypes.c_int64)
     f32p = ctypes.POINTER(ctypes.c_float)
     rc = fn(q.ctypes.data_as(u16p), q_pos.ctypes.data_as(i64p), n_q,
-            k.ctypes.data_as(u16p), v.ctypes.data_as(u16p), k_pos.ctypes.data_as(i64p), n_k,
+            k.ctypes.data_as(f32p if kv_f32 else u16p), v.ctypes.data_as(f32p if kv_f32 else u16p), k_pos.ctypes.data_as(i64p), n_k,
             Hq, Hkv, D, int(S), int(W), float(scale),
             out.ctypes.data_as(f32p),
             weights.ctypes.data_as(f32p) if want_weights else None, int(n_threads))
@@ -136,6 +139,7 @@ class PoolConfig:
     scale: float | None = None
     max_session_len: int = 2**31 - 1 - 4096
     unbounded: bool = False  # the paper's vanilla arm: nothing is ever freed, full causal mask
+    kv_fp8: bool = False     # K / V rows are stored as e4m3 codes + one scale per (token, KV head): oracle/kv_fp8.py
 
     @property
     def n_sink(self) -> int:  # ceil(S / block)
@@ -187,9 +191,10 @@ class DefinitionOracle:
         self.length[sid] = 0
         self.last_n[sid] = 0
         c = self.cfg
+        dt = np.float32 if c.kv_fp8 else np.uint16
         for layer in range(c.n_layers):
-            self.hist[layer][sid] = [np.zeros((0, c.n_kv_heads, c.head_dim), np.uint16),
-                                     np.zeros((0, c.n_kv_heads, c.head_dim), np.uint16)]
+            self.hist[layer][sid] = [np.zeros((0, c.n_kv_heads, c.head_dim), dt),
+                                     np.zeros((0, c.n_kv_heads, c.head_dim), dt)]
         return sid
 
     def session_close(self, sid: int) -> None:
@@ -200,7 +205,11 @@ class DefinitionOracle:
             del self.hist[layer][sid]
 
     def append_kv(self, layer: int, sids, n_new, k_new, v_new) -> None:
-        """k_new/v_new: [sum n_new, Hkv, D] uint16 in batch order (PAPER.md:L46 'prefill the new chunk')."""
+        """k_new/v_new: [sum n_new, Hkv, D] uint16 in batch order (PAPER.md:L46 'prefill the new chunk').
+        In the fp8 arm every row is replaced by what its stored form decodes to (kv_fp8.roundtrip)."""
+        if self.cfg.kv_fp8:
+            from . import kv_fp8
+            k_new, v_new = kv_fp8.roundtrip(k_new), kv_fp8.roundtrip(v_new)
         row = 0
         for sid, n in zip(sids, n_new):
             if sid not in self.length:
