@@ -51,6 +51,9 @@ def parse():
     ap.add_argument("--two-calls", action="store_true",
                     help="issue every sub-step as metronome_append_kv + metronome_attend_frame instead of the one-call "
                          "metronome_append_attend (A/B of the fused decode step)")
+    ap.add_argument("--kv-fp8", action="store_true",
+                    help="store K / V as fp8 (E4M3 codes + a float32 scale per (token, KV head): METRONOME_FLAG_KV_FP8, NEXT row "
+                         "f4); algorithmic bytes per key drop from 4 D to 2 D + 8 per KV head")
     ap.add_argument("--fused-step", action="store_true",
                     help="run GQA decode steps as one launch (step_gqa.cuh; measured slower than the two launches, off by default)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -125,11 +128,15 @@ class ClockSampler:
         return out
 
 
+KV_FP8 = False      # --kv-fp8: a key costs 2 D + 8 bytes per KV head (codes + two scales) instead of 4 D
+
+
 def item_bytes(w, L, n):
     """per session keys_read x Hkv x 4D (K+V bf16) + q and out rows.
     keys_read = min(len, S+W) for decode; for a chunk the union over its rows min(L1, S+W+n-1)."""
     keys = min(L, w.S + w.W + n - 1)
-    return keys * w.n_kv_heads * 4 * w.head_dim + n * w.n_q_heads * 4 * w.head_dim
+    per_key = (2 * w.head_dim + 8) if KV_FP8 else 4 * w.head_dim
+    return keys * w.n_kv_heads * per_key + n * w.n_q_heads * 4 * w.head_dim
 
 
 def item_flops(w, L, n):
@@ -188,6 +195,7 @@ def config_dict(w, args, world):
     return {"workload": f"BASELINE.json configs[{w.index - 1}] {w.name}: {w.n_sessions} sessions, "
                         f"{w.n_q_heads}Q/{w.n_kv_heads}KV, D={w.head_dim}, S={w.S}, W={w.W}, block 16",
             "sessions_per_gpu": w.n_sessions, "n_layers": max(1, args.layers), "parallelism": f"replicas x{world}",
+            "kv_storage": "fp8 e4m3 + f32 scale per (token, kv head)" if getattr(args, "kv_fp8", False) else "bf16",
             "history_scale": args.history_scale,
             "l2": "inputs larger than L2: every step streams each session's whole window (GBs per step vs 126 MB "
                   "L2), no flush needed"}
@@ -355,7 +363,10 @@ def main():
     w = wl.make_workload(args.config, n_sessions=args.sessions or None, n_timed_frames=need)
     events, info = wl.build_schedule(w, history_scale=args.history_scale)
     NL = max(1, args.layers)
-    r = Runner(w, n_layers=NL, uid_base=replicas.uid_base(RANK))
+    global KV_FP8
+    KV_FP8 = bool(args.kv_fp8)
+    from paper_2607_02640_b200 import binding as _bind
+    r = Runner(w, n_layers=NL, uid_base=replicas.uid_base(RANK), flags=_bind.FLAG_KV_FP8 if args.kv_fp8 else 0)
     r.pool.set_tuning(args.split_tokens, args.family, 0, 2 if args.fused_step else 0)
     t_hist = time.perf_counter()
     rest = r.run_history(events)

@@ -72,6 +72,14 @@ enum {
  * mask is plain causal.  W is ignored. */
 #define METRONOME_FLAG_UNBOUNDED 0x4u
 
+/* NEXT row f4, sec. 4.1 "Orthogonal to KV compression, which shrinks each token
+ * ...: we bound which tokens stay resident, and the two compose": K / V rows are STORED as fp8 -- E4M3 codes plus one
+ * float32 scale per (token, KV head) row, scale = max |x| / 448, code = x / scale rounded to nearest even (DESIGN.md
+ * reading R18; the paper names no format).  k_new / v_new / q / out stay bf16; attention runs over what the codes
+ * decode to (value(code) x scale, float32).  A block-head takes 2 x 16 x D + 128 bytes instead of 2 x 16 x D x 2.
+ * All attention of such a pool runs on the CUDA-core row kernel.  metronome_read_kv returns FLOAT32 rows. */
+#define METRONOME_FLAG_KV_FP8 0x8u
+
 /* ---- configuration -------------------------------------------------------------------------- */
 typedef struct metronome_pool_config {
     int32_t n_layers;        /* >= 1; one block table is shared by all layers (L256: every decoder
@@ -98,7 +106,8 @@ typedef struct metronome_pool metronome_pool_t; /* opaque */
 /* ---- pool ----------------------------------------------------------------------------------- */
 
 /* Bytes of device memory the KV storage of `cfg` needs:
- * n_layers * n_blocks * n_kv_heads * 2 (K,V) * block_size * head_dim * 2.  0 if cfg is invalid. */
+ * n_layers * n_blocks * n_kv_heads * 2 (K,V) * block_size * head_dim * 2  (bf16), or
+ * n_layers * n_blocks * n_kv_heads * (2 * block_size * head_dim + 128)     (METRONOME_FLAG_KV_FP8).  0 if cfg is invalid. */
 size_t metronome_kv_storage_bytes(const metronome_pool_config_t* cfg);
 
 /* Worst-case resident blocks of one session: ceil(S/B) + floor((W + max_new_tokens - 1)/B) + 2.
@@ -213,7 +222,8 @@ int metronome_session_query(metronome_pool_t* pool, int32_t sid, void* cuda_stre
 int metronome_pool_query(metronome_pool_t* pool, void* cuda_stream, int32_t* n_free, int32_t* free_ids);
 
 /* Reads back, through the block table, K and V rows of positions [pos0, pos0+n) of `sid` in
- * `layer` into device bf16 [n, n_kv_heads, head_dim] buffers (verification of the KV write).
+ * `layer` into device bf16 [n, n_kv_heads, head_dim] buffers (verification of the KV write; float32
+ * buffers holding the decoded rows for a METRONOME_FLAG_KV_FP8 pool).
  * Positions whose block is not resident return bf16 NaN.  Errors: INVALID_*, UNSUPPORTED, CUDA. */
 int metronome_read_kv(metronome_pool_t* pool, int32_t layer, int32_t sid, int64_t pos0, int32_t n,
                       void* k_out, void* v_out, void* cuda_stream);

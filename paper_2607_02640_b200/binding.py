@@ -17,6 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libmetronome.so")
 FLAG_POISON_ON_FREE = 0x1
 FLAG_BOOKKEEPING_ONLY = 0x2
 FLAG_UNBOUNDED = 0x4
+FLAG_KV_FP8 = 0x8
 
 ERR_NAMES = {0: "OK", 1: "INVALID_ARG", 2: "INVALID_SESSION", 3: "DUPLICATE_SESSION", 4: "SESSIONS_FULL",
              5: "POOL_EXHAUSTED", 6: "CHUNK_TOO_LARGE", 7: "QLEN_EXCEEDS_LAST_APPEND", 8: "LAYER_SEQUENCE",

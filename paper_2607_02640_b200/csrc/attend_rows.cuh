@@ -15,6 +15,7 @@
 // round-robin, so there is no barrier inside the tile loop.
 #pragma once
 #include "attend_common.cuh"
+#include "kv_fp8.cuh"
 
 namespace metronome {
 
@@ -29,10 +30,28 @@ __device__ __forceinline__ void merge_state(float& m, float& l, float (&acc)[8],
     m = M;
 }
 
+// 8 consecutive elements of a K / V row as the lane holds them: 16 bytes of bf16, or 8 E4M3 codes (fp8 KV, NEXT row
+// f4: the row's float32 scale is applied to the finished dot product / folded into the softmax weight)
+template <bool FP8> struct RowChunk { using type = uint4; };
+template <> struct RowChunk<true> { using type = uint2; };
+// elements 2 k, 2 k + 1 of the chunk as a packed float pair
+__device__ __forceinline__ uint64_t chunk_pair(const uint4& c, int k) {
+    const uint32_t w = k == 0 ? c.x : k == 1 ? c.y : k == 2 ? c.z : c.w;
+    return f2_pack(bf16lo(w), bf16hi(w));
+}
+__device__ __forceinline__ uint64_t chunk_pair(const uint2& c, int k) {
+    const uint32_t w = (k < 2 ? c.x : c.y) >> (16 * (k & 1));
+    uint32_t h2;
+    asm("cvt.rn.f16x2.e4m3x2 %0, %1;" : "=r"(h2) : "h"((uint16_t)w));
+    const __half2 hv = *reinterpret_cast<const __half2*>(&h2);
+    return f2_pack(__low2float(hv), __high2float(hv));
+}
+
 // grid = (Hq, total_splits, max_q_len), block = 128
-template <int D>
+template <int D, bool FP8>
 __global__ void __launch_bounds__(128)
 attend_rows_kernel(AttendParams p) {
+    using Chunk = typename RowChunk<FP8>::type;
     if (p.pdl_early) pdl_launch_dependents();
     if (threadIdx.x == 0) { stamp_begin(p); wait_work_list(p); }
     __syncthreads();
@@ -93,16 +112,28 @@ attend_rows_kernel(AttendParams p) {
         const int32_t phys = __ldg(trow + table_slot(block_of(tile), p.n_sink, p.ring));
         return p.kv_layer + (int64_t)phys * p.L.block_bytes + (int64_t)kvh * p.L.head_bytes;
     };
-    uint4 kr[STEPS], vr[STEPS];
+    Chunk kr[STEPS], vr[STEPS];
+    float ks[FP8 ? STEPS : 1], vs[FP8 ? STEPS : 1];                 // fp8: the rows' scales
+    auto chunk_off = [&](int32_t row) { return FP8 ? row * D + sub * 8 : tile_chunk_offset(row, sub); };
+    auto load_k = [&](const uint8_t* kt) {
+#pragma unroll
+        for (int j = 0; j < STEPS; ++j) {
+            kr[j] = __ldg(reinterpret_cast<const Chunk*>(kt + chunk_off(j * TPS + grp)));
+            if (FP8) ks[j] = __ldg(reinterpret_cast<const float*>(kt + 2 * p.L.tile_bytes) + j * TPS + grp);
+        }
+    };
+    auto load_v = [&](const uint8_t* kt) {
+#pragma unroll
+        for (int j = 0; j < STEPS; ++j) {
+            vr[j] = __ldg(reinterpret_cast<const Chunk*>(kt + p.L.tile_bytes + chunk_off(j * TPS + grp)));
+            if (FP8) vs[j] = __ldg(reinterpret_cast<const float*>(kt + 2 * p.L.tile_bytes) + kBlockTokens + j * TPS + grp);
+        }
+    };
     int32_t tile = next_valid(tl0 + warp);
     if (tile < tl1) {
         const uint8_t* kt = tile_ptr(tile);
-#pragma unroll
-        for (int j = 0; j < STEPS; ++j) {
-            const int32_t off = tile_chunk_offset(j * TPS + grp, sub);
-            kr[j] = __ldg(reinterpret_cast<const uint4*>(kt + off));
-            vr[j] = __ldg(reinterpret_cast<const uint4*>(kt + p.L.tile_bytes + off));
-        }
+        load_k(kt);
+        load_v(kt);
     }
     while (tile < tl1) {
         const int32_t p0 = block_of(tile) * kBlockTokens;
@@ -111,22 +142,17 @@ attend_rows_kernel(AttendParams p) {
         float s[STEPS];
 #pragma unroll
         for (int j = 0; j < STEPS; ++j) {
-            const uint32_t w[4] = {kr[j].x, kr[j].y, kr[j].z, kr[j].w};
             uint64_t d2 = 0ull;                                   // (even, odd) partial sums, FFMA2
 #pragma unroll
-            for (int k = 0; k < 4; ++k) d2 = f2_fma(q2[k], f2_pack(bf16lo(w[k]), bf16hi(w[k])), d2);
+            for (int k = 0; k < 4; ++k) d2 = f2_fma(q2[k], chunk_pair(kr[j], k), d2);
             float de, dodd;
             f2_unpack(d2, de, dodd);
             float d = de + dodd;
 #pragma unroll
             for (int o = LPT / 2; o >= 1; o >>= 1) d += __shfl_xor_sync(0xffffffffu, d, o);
-            s[j] = d;
+            s[j] = FP8 ? d * ks[j] : d;
         }
-        if (kt_next) {
-#pragma unroll
-            for (int j = 0; j < STEPS; ++j)
-                kr[j] = __ldg(reinterpret_cast<const uint4*>(kt_next + tile_chunk_offset(j * TPS + grp, sub)));
-        }
+        if (kt_next) load_k(kt_next);
         const bool full = (p0 + kBlockTokens - 1 <= t) &&
                           (p0 + kBlockTokens - 1 < p.S || t - p0 < p.W);
         if (!full) {
@@ -137,7 +163,8 @@ attend_rows_kernel(AttendParams p) {
                 const int32_t pos = p0 + j * TPS + grp;
                 if (!admit(pos, t, p.S, p.W)) {
                     s[j] = -INFINITY;
-                    vr[j] = make_uint4(0u, 0u, 0u, 0u);
+                    vr[j] = Chunk{};
+                    if (FP8) vs[j] = 0.f;
                 }
             }
         }
@@ -155,18 +182,14 @@ attend_rows_kernel(AttendParams p) {
             for (int j = 0; j < STEPS; ++j) {
                 const float pj = ex2(s[j] - mn);
                 l += pj;
-                const uint64_t pj2 = f2_pack(pj, pj);
-                const uint32_t w[4] = {vr[j].x, vr[j].y, vr[j].z, vr[j].w};
+                const float pv = FP8 ? pj * vs[j] : pj;
+                const uint64_t pj2 = f2_pack(pv, pv);
 #pragma unroll
-                for (int k = 0; k < 4; ++k) acc2[k] = f2_fma(pj2, f2_pack(bf16lo(w[k]), bf16hi(w[k])), acc2[k]);
+                for (int k = 0; k < 4; ++k) acc2[k] = f2_fma(pj2, chunk_pair(vr[j], k), acc2[k]);
             }
             m = mn;
         }
-        if (kt_next) {
-#pragma unroll
-            for (int j = 0; j < STEPS; ++j)
-                vr[j] = __ldg(reinterpret_cast<const uint4*>(kt_next + p.L.tile_bytes + tile_chunk_offset(j * TPS + grp, sub)));
-        }
+        if (kt_next) load_v(kt_next);
         tile = nxt;
     }
 

@@ -9,6 +9,7 @@
 // decode step (n_new = 1) of 128-512 sessions still fills the machine.
 #pragma once
 #include "bookkeeping.cuh"
+#include "kv_fp8.cuh"
 
 namespace metronome {
 
@@ -174,6 +175,14 @@ append_fused_kernel(const AppendParams a) {
     const int32_t blk = pos / kBlockTokens, r = pos % kBlockTokens;
     const int32_t phys = __ldcg(a.table + (int64_t)it.sid * a.tbl_width + table_slot(blk, a.n_sink, a.ring));
     uint8_t* tile = a.kv_layer + (int64_t)phys * a.L.block_bytes + (int64_t)h * a.L.head_bytes;
+    if (a.L.fp8) {
+        // (the chunks_per_row threads of a row are consecutive lanes of one warp, all active or all not)
+        const uint2 kq = quantize_chunk_e4m3(kk, chunks_per_row, c == 0 ? reinterpret_cast<float*>(tile + 2 * a.L.tile_bytes) + r : nullptr);
+        const uint2 vq = quantize_chunk_e4m3(vv, chunks_per_row, c == 0 ? reinterpret_cast<float*>(tile + 2 * a.L.tile_bytes) + kBlockTokens + r : nullptr);
+        *reinterpret_cast<uint2*>(tile + r * a.L.head_dim + c * 8) = kq;
+        *reinterpret_cast<uint2*>(tile + a.L.tile_bytes + r * a.L.head_dim + c * 8) = vq;
+        return;
+    }
     const int32_t off = tile_chunk_offset(r, c);
     *reinterpret_cast<uint4*>(tile + off) = kk;
     *reinterpret_cast<uint4*>(tile + a.L.tile_bytes + off) = vv;
@@ -205,6 +214,36 @@ kv_read_kernel(const int32_t* __restrict__ row, int32_t n_sink, int32_t ring, in
     }
     k_out[idx] = kk;
     v_out[idx] = vv;
+}
+
+// The same for an fp8 pool: what the stored codes decode to, float32 [n, Hkv, D] (bit-exact check of the quantiser).
+__global__ void __launch_bounds__(256)
+kv_read_fp8_kernel(const int32_t* __restrict__ row, int32_t n_sink, int32_t ring, int32_t n_sink_res,
+                   int32_t first_live, int32_t n_blk, int32_t pos0, int32_t n, const uint8_t* __restrict__ kv_layer,
+                   KvLayout L, float* __restrict__ k_out, float* __restrict__ v_out) {
+    const int32_t chunks_per_row = L.head_dim >> 3;
+    const int32_t chunks_per_tok = L.n_kv_heads * chunks_per_row;
+    const int32_t idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= n * chunks_per_tok) return;
+    const int32_t tok = idx / chunks_per_tok;
+    const int32_t rem = idx - tok * chunks_per_tok;
+    const int32_t h = rem / chunks_per_row;
+    const int32_t c = rem - h * chunks_per_row;
+    const int32_t pos = pos0 + tok;
+    const int32_t blk = pos / kBlockTokens, r = pos % kBlockTokens;
+    const bool resident = blk < n_blk && (blk < n_sink_res || blk >= first_live);
+    float kf[8], vf[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) kf[k] = vf[k] = __int_as_float(0x7FC00000);
+    if (resident) {
+        const int32_t phys = row[table_slot(blk, n_sink, ring)];
+        const uint8_t* tile = kv_layer + (int64_t)phys * L.block_bytes + (int64_t)h * L.head_bytes;
+        const float* scales = reinterpret_cast<const float*>(tile + 2 * L.tile_bytes);
+        dequant8_e4m3(*reinterpret_cast<const uint2*>(tile + r * L.head_dim + c * 8), scales[r], kf);
+        dequant8_e4m3(*reinterpret_cast<const uint2*>(tile + L.tile_bytes + r * L.head_dim + c * 8), scales[kBlockTokens + r], vf);
+    }
+#pragma unroll
+    for (int k = 0; k < 8; ++k) { k_out[(int64_t)idx * 8 + k] = kf[k]; v_out[(int64_t)idx * 8 + k] = vf[k]; }
 }
 
 // Read-only stream over n16 x 16 bytes: 4 independent 16-byte loads in flight per thread, grid-stride.

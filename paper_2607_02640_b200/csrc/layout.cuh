@@ -23,18 +23,23 @@ constexpr int kHalfDim = 64;       // 128-byte rows: the swizzle span
 struct KvLayout {
     int32_t head_dim;       // D
     int32_t n_kv_heads;     // Hkv
-    int64_t tile_bytes;     // 16 * D * 2          (K or V of one block-head)
-    int64_t head_bytes;     // 2 * tile_bytes      (K then V)
+    int32_t fp8;            // METRONOME_FLAG_KV_FP8: rows are E4M3 codes + one float32 scale per (token, KV head)
+    int64_t tile_bytes;     // 16 * D * 2          (K or V of one block-head; 16 * D in the fp8 layout)
+    int64_t head_bytes;     // 2 * tile_bytes      (K then V; + 128 in the fp8 layout: 16 K scales, 16 V scales)
     int64_t block_bytes;    // Hkv * head_bytes
     int64_t layer_bytes;    // n_blocks * block_bytes
 };
 
-__host__ __device__ inline KvLayout make_layout(int32_t D, int32_t Hkv, int64_t n_blocks) {
+// fp8 layout of one (block, kv head):  [K codes 16 x D bytes, linear][V codes 16 x D][K scales 16 f32][V scales 16 f32]
+// (NEXT row f4, "the two compose"; quantiser: DESIGN.md reading R18).  Only the CUDA-core row kernel
+// reads it, so the rows are not swizzled.
+__host__ __device__ inline KvLayout make_layout(int32_t D, int32_t Hkv, int64_t n_blocks, bool fp8 = false) {
     KvLayout L;
     L.head_dim = D;
     L.n_kv_heads = Hkv;
-    L.tile_bytes = (int64_t)kBlockTokens * D * 2;
-    L.head_bytes = 2 * L.tile_bytes;
+    L.fp8 = fp8 ? 1 : 0;
+    L.tile_bytes = (int64_t)kBlockTokens * D * (fp8 ? 1 : 2);
+    L.head_bytes = 2 * L.tile_bytes + (fp8 ? 2 * kBlockTokens * 4 : 0);
     L.block_bytes = (int64_t)Hkv * L.head_bytes;
     L.layer_bytes = n_blocks * L.block_bytes;
     return L;

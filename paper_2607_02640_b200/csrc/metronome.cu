@@ -74,7 +74,7 @@ struct metronome_pool {
     int32_t n_sink = 0, tbl_width = 0, ring = 0, G = 1, W_eff = 0;
     float scale = 0.f;
     KvLayout L{};
-    bool bookkeeping_only = false, poison = false, unbounded = false, own_kv = false;
+    bool bookkeeping_only = false, poison = false, unbounded = false, own_kv = false, fp8 = false;
 
     std::vector<Session> sessions;
     std::vector<int32_t> stamp;        // duplicate detection
@@ -309,6 +309,7 @@ int plan_attend(metronome_pool* pool, int32_t n_batch, const int32_t* sids, cons
     }
     int family = pool->tune_family;
     if (family == 0) family = (pool->G * max_q >= 4) ? 2 : 1;
+    if (pool->fp8) family = 1;        // fp8 KV rows are read by the CUDA-core row kernel only (NEXT row f4)
     if (family == 2 && !attend_umma_supported(pool->G, max_q))
         family = 1;
     pl.family = family;
@@ -552,8 +553,13 @@ int launch_attend(metronome_pool* pool, int32_t layer, const AttendPlan& pl, con
         p.items = d_items; p.n_items = pl.n_items;
         dim3 grid(c.n_q_heads, pl.total_splits[0], pl.cls_max_q[0]);
         p.stamp = next_stamp(pool, 1);
-        if (c.head_dim == 128) CU(launch_kernel(attend_rows_kernel<128>, grid, dim3(128), 0, st, pdl, p));
-        else CU(launch_kernel(attend_rows_kernel<64>, grid, dim3(128), 0, st, pdl, p));
+        if (pool->fp8) {
+            if (c.head_dim == 128) CU(launch_kernel(attend_rows_kernel<128, true>, grid, dim3(128), 0, st, pdl, p));
+            else CU(launch_kernel(attend_rows_kernel<64, true>, grid, dim3(128), 0, st, pdl, p));
+        } else {
+            if (c.head_dim == 128) CU(launch_kernel(attend_rows_kernel<128, false>, grid, dim3(128), 0, st, pdl, p));
+            else CU(launch_kernel(attend_rows_kernel<64, false>, grid, dim3(128), 0, st, pdl, p));
+        }
         ++pool->n_launch;
     }
     if (pool->profiling) {
@@ -602,7 +608,7 @@ const char* metronome_last_cuda_error(metronome_pool_t* pool) { return pool ? po
 
 size_t metronome_kv_storage_bytes(const metronome_pool_config_t* c) {
     if (!valid_cfg(c) || (c->flags & METRONOME_FLAG_BOOKKEEPING_ONLY)) return 0;
-    return (size_t)c->n_layers * c->n_blocks * c->n_kv_heads * 2 * c->block_size * c->head_dim * 2;
+    return (size_t)c->n_layers * make_layout(c->head_dim, c->n_kv_heads, c->n_blocks, c->flags & METRONOME_FLAG_KV_FP8).layer_bytes;
 }
 
 int32_t metronome_max_blocks_per_session(int32_t S, int32_t W, int32_t B, int32_t max_new_tokens) {
@@ -660,7 +666,8 @@ int metronome_pool_create(const metronome_pool_config_t* cfg, metronome_pool_t**
     if (e != cudaSuccess) return fail(METRONOME_ERR_OUT_OF_MEMORY, e, "cudaMalloc free stack");
     cudaMemset(pool->d_table, 0xFF, (size_t)c.max_sessions * pool->tbl_width * sizeof(int32_t));
     if (!pool->bookkeeping_only) {
-        pool->L = make_layout(c.head_dim, c.n_kv_heads, c.n_blocks);
+        pool->fp8 = c.flags & METRONOME_FLAG_KV_FP8;
+        pool->L = make_layout(c.head_dim, c.n_kv_heads, c.n_blocks, pool->fp8);
         const size_t need = metronome_kv_storage_bytes(&pool->cfg);
         if (c.kv_storage) {
             if (c.kv_storage_bytes < need || ((uintptr_t)c.kv_storage & 127)) return fail(METRONOME_ERR_INVALID_ARG, e, "");
@@ -1220,9 +1227,14 @@ int metronome_read_kv(metronome_pool_t* pool, int32_t layer, int32_t sid, int64_
     const int32_t n_blk = (int32_t)((s.len + kBlockTokens - 1) / kBlockTokens);
     const int32_t n_sink_res = n_blk < pool->n_sink ? n_blk : pool->n_sink;
     const int64_t chunks = (int64_t)n * pool->cfg.n_kv_heads * (pool->cfg.head_dim / 8);
-    kv_read_kernel<<<(unsigned)((chunks + 255) / 256), 256, 0, (cudaStream_t)cuda_stream>>>(
-        pool->d_table + (int64_t)sid * pool->tbl_width, pool->n_sink, pool->ring, n_sink_res, s.first_live, n_blk,
-        (int32_t)pos0, n, pool->d_kv + (int64_t)layer * pool->L.layer_bytes, pool->L, (uint4*)k_out, (uint4*)v_out);
+    if (pool->fp8)
+        kv_read_fp8_kernel<<<(unsigned)((chunks + 255) / 256), 256, 0, (cudaStream_t)cuda_stream>>>(
+            pool->d_table + (int64_t)sid * pool->tbl_width, pool->n_sink, pool->ring, n_sink_res, s.first_live, n_blk,
+            (int32_t)pos0, n, pool->d_kv + (int64_t)layer * pool->L.layer_bytes, pool->L, (float*)k_out, (float*)v_out);
+    else
+        kv_read_kernel<<<(unsigned)((chunks + 255) / 256), 256, 0, (cudaStream_t)cuda_stream>>>(
+            pool->d_table + (int64_t)sid * pool->tbl_width, pool->n_sink, pool->ring, n_sink_res, s.first_live, n_blk,
+            (int32_t)pos0, n, pool->d_kv + (int64_t)layer * pool->L.layer_bytes, pool->L, (uint4*)k_out, (uint4*)v_out);
     ++pool->n_launch;
     CU(cudaGetLastError());
     return METRONOME_OK;

@@ -1,0 +1,127 @@
+"""GPU parity of the fp8 KV arm (`-m gpu`): METRONOME_FLAG_KV_FP8 pools (PAPER.md:L101
+"we bound which tokens stay resident, and the two compose"; quantiser = DESIGN.md reading R18, stated in
+oracle/kv_fp8.py and pinned in tests/test_oracle_kv_fp8.py).
+
+  * the stored rows: what metronome_read_kv decodes (float32) equals the oracle's round trip BIT FOR BIT -- both
+    sides take the rounding decision in float32 (scale = max|x| / 448, x / scale, nearest-even E4M3);
+  * attention over sinks + window of the decoded rows: same contract tolerance as the bf16 arm, against the oracle's
+    fp8 arm (which attends over the identical float32 rows), for decode / chunk / mixed steps, G = 1 and G = 4,
+    D = 64 and 128, several sink counts, split-KV on and off; block tables and free list bit-exact.
+Seeded inputs; nothing reads /root/reference.
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import bounded_kv as O
+from oracle import kv_fp8 as F
+from paper_2607_02640_b200 import binding, synth
+from parity_helpers import assert_parity
+
+pytestmark = pytest.mark.gpu
+
+
+def _bf16(rng, n, H, D, scale=1.0):
+    return torch.from_numpy((rng.standard_normal((n, H, D)) * scale).astype(np.float32)).to(torch.bfloat16)
+
+
+def _make(S, W, Hq, Hkv, D, N, n_max, split_tokens=0, extra_flags=0):
+    per = -(-S // 16) + (W + n_max - 1) // 16 + 2
+    kw = dict(n_q_heads=Hq, n_kv_heads=Hkv, head_dim=D, max_sessions=N, max_new_tokens=n_max)
+    pool = binding.Pool(n_sinks=S, window=W, n_blocks=N * per, flags=binding.FLAG_KV_FP8 | extra_flags, **kw)
+    pool.set_tuning(split_tokens, 0)
+    cfg = O.PoolConfig(S=S, W=W, n_blocks=N * per, block_size=16, kv_fp8=True, **kw)
+    return pool, O.DefinitionOracle(cfg), O.PagedOracle(cfg, store_kv=False)
+
+
+@pytest.mark.parametrize("D,Hkv", [(128, 4), (64, 2)])
+def test_stored_rows_decode_to_the_oracle_round_trip_bit_for_bit(D, Hkv):
+    pool, defn, book = _make(4, 64, Hkv * 2, Hkv, D, 3, 25)
+    assert pool.kv_storage_bytes() == pool.cfg.n_blocks * Hkv * (2 * 16 * D + 128)
+    sids = [pool.session_open() for _ in range(3)]
+    rng = np.random.default_rng(D)
+    hist = {s: ([], []) for s in sids}
+    for step in range(12):
+        n_new = rng.integers(0, 26, size=3).astype(np.int32) if step % 3 == 0 else np.ones(3, np.int32)
+        rows = int(n_new.sum())
+        scale = rng.choice([1e-3, 1.0, 30.0])
+        k, v = _bf16(rng, rows, Hkv, D, scale), _bf16(rng, rows, Hkv, D, 1.0)
+        if rows:
+            k[0] = 0                                                   # an all-zero row: scale 1, codes 0
+            v[-1, :, 1:] = 0                                           # a single non-zero element: it is the row's 448
+        pool.append_kv(0, sids, n_new, k.cuda(), v.cuda())
+        off = 0
+        for s, n in zip(sids, n_new):
+            hist[s][0].append(synth.to_u16(k[off:off + int(n)])); hist[s][1].append(synth.to_u16(v[off:off + int(n)]))
+            off += int(n)
+    for s in sids:
+        K, V = np.concatenate(hist[s][0]), np.concatenate(hist[s][1])
+        L = K.shape[0]
+        first_live = pool.session_query(s)[1]
+        for lo, hi in ((0, min(L, 16)), (first_live * 16, L)):           # the pinned sink block, the live window blocks
+            kb = torch.empty(hi - lo, Hkv, D, dtype=torch.float32, device="cuda")
+            vb = torch.empty_like(kb)
+            pool.read_kv(0, s, lo, hi - lo, kb, vb)
+            assert np.array_equal(kb.cpu().numpy().view(np.uint32), F.roundtrip(K[lo:hi]).view(np.uint32)), (s, lo, hi)
+            assert np.array_equal(vb.cpu().numpy().view(np.uint32), F.roundtrip(V[lo:hi]).view(np.uint32)), (s, lo, hi)
+
+
+@pytest.mark.parametrize("mode", ["decode", "chunk", "mixed"])
+@pytest.mark.parametrize("G,D", [(1, 128), (4, 128), (4, 64)])
+@pytest.mark.parametrize("S,split_tokens", [(4, 0), (0, 0), (17, 48)])
+def test_fp8_attention_parity(S, split_tokens, G, D, mode):
+    Hkv, W, n_max, N = 2, 72, 25, 3
+    Hq = Hkv * G
+    pool, defn, book = _make(S, W, Hq, Hkv, D, N, n_max, split_tokens)
+    sids = [pool.session_open() for _ in range(N)]
+    assert sids == [defn.session_open() for _ in range(N)] == [book.session_open() for _ in range(N)]
+    rng = np.random.default_rng(500 + 7 * S + G + D)
+    worst = 0.0
+    for step in range(120 if mode == "decode" else 30):
+        if mode == "decode" and step > 0:
+            n_new = np.ones(N, np.int64)
+        elif mode == "chunk" or step == 0:
+            n_new = rng.integers(5, n_max + 1, size=N)
+        else:
+            n_new = np.where(rng.random(N) < 0.5, 1, rng.integers(2, n_max + 1, size=N))
+        n_new = n_new.astype(np.int32)
+        rows = int(n_new.sum())
+        k, v, q = _bf16(rng, rows, Hkv, D), _bf16(rng, rows, Hkv, D), _bf16(rng, rows, Hq, D)
+        out = torch.empty_like(q, device="cuda")
+        pool.append_attend(0, sids, n_new, k.cuda(), v.cuda(), q.cuda(), out)
+        defn.append_kv(0, sids, [int(x) for x in n_new], synth.to_u16(k), synth.to_u16(v))
+        book.append_kv(0, sids, [int(x) for x in n_new])
+        ref = defn.attend_frame(0, sids, [int(x) for x in n_new], synth.to_u16(q))
+        rep = assert_parity(out, ref, f"fp8 S={S} G={G} D={D} {mode} step {step} n={n_new}")
+        worst = max(worst, rep["max_abs"])
+        for s in sids:
+            got, want = pool.session_query(int(s)), book.session_query(int(s))
+            assert (got[0], got[1], list(got[2])) == (want[0], want[1], list(want[2])), (step, s)
+    assert min(defn.length.values()) > S + W, "the sessions never left the full-causal regime"
+    assert pool.pool_query()[1] == book.pool_query()
+    print(f"fp8 S={S} G={G} D={D} {mode}: worst max_abs {worst:.2e}")
+
+
+def test_fp8_with_poisoned_frees_and_two_layers():
+    """Freed blocks are filled with NaN bytes ("freed blocks NaN-poisoned"): nothing outside sinks U
+    window may be read in the fp8 layout either; layer 1 repeats layer 0's batch with its own rows."""
+    S, W, Hq, Hkv, D, N = 4, 40, 8, 8, 128, 4
+    per = 1 + (W + 4 - 1) // 16 + 2
+    kw = dict(n_q_heads=Hq, n_kv_heads=Hkv, head_dim=D, max_sessions=N, max_new_tokens=4)
+    pool = binding.Pool(n_sinks=S, window=W, n_blocks=N * per, n_layers=2, flags=binding.FLAG_KV_FP8 | binding.FLAG_POISON_ON_FREE, **kw)
+    defn = O.DefinitionOracle(O.PoolConfig(S=S, W=W, n_blocks=N * per, block_size=16, n_layers=2, kv_fp8=True, **kw))
+    sids = [pool.session_open() for _ in range(N)]
+    assert sids == [defn.session_open() for _ in range(N)]
+    rng = np.random.default_rng(9)
+    for step in range(120):
+        due = sorted(rng.permutation(N)[:int(rng.integers(2, N + 1))].tolist())
+        n_new = rng.integers(1, 4, size=len(due)).astype(np.int32)
+        rows = int(n_new.sum())
+        for layer in range(2):
+            k, v, q = _bf16(rng, rows, Hkv, D), _bf16(rng, rows, Hkv, D), _bf16(rng, rows, Hq, D)
+            out = torch.empty_like(q, device="cuda")
+            pool.append_kv(layer, [sids[i] for i in due], n_new, k.cuda(), v.cuda())
+            pool.attend_frame(layer, [sids[i] for i in due], n_new, q.cuda(), out)
+            defn.append_kv(layer, [sids[i] for i in due], [int(x) for x in n_new], synth.to_u16(k), synth.to_u16(v))
+            ref = defn.attend_frame(layer, [sids[i] for i in due], [int(x) for x in n_new], synth.to_u16(q))
+            assert_parity(out, ref, f"fp8 poison step {step} layer {layer}")
