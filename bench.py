@@ -538,7 +538,7 @@ def main():
              "launches": d["launches"], "kernel_ms_avg": d["ms"] / d["launches"],
              "raw_span_ms_avg": d["span_ms"] / d["launches"],
              "algorithmic_bytes_per_launch": d["bytes"] / d["launches"], "share_of_step": d["ms"] / st_ms,
-             "frac_of_nominal_8TBs": gbs / 8000.0, "traffic": tj.get(f"config{w.index}_{KIND_NAME[kind]}")}
+             "frac_of_nominal_8TBs": gbs / 8000.0, "traffic": tj.get(f"config{w.index}{'_fp8' if KV_FP8 else ''}_{KIND_NAME[kind]}")}
         if kind == 3:
             tf_s = d["flops"] / (d["ms"] * 1e-3) / 1e12
             sustained = pk.get("bf16_tflops_sustained", 1423.1)

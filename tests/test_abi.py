@@ -64,7 +64,7 @@ def test_sass_census_shows_the_hardware_paths_each_kernel_claims():
     build.build_library()
     c = build.sass_census()
     for D in (64, 128):
-        u, g, r = c[f"attend_umma_kernel<{D}>"], c[f"attend_gqa_kernel<{D}>"], c[f"attend_rows_kernel<{D}>"]
+        u, g, r = c[f"attend_umma_kernel<{D}>"], c[f"attend_gqa_kernel<{D}>"], c[f"attend_rows_kernel<{D}, false>"]
         assert u.get("UTCHMMA", 0) > 0 and u.get("LDTM", 0) > 0 and u.get("STTM", 0) > 0 and u.get("UBLKCP", 0) > 0, u
         assert g.get("HMMA", 0) > 0 and g.get("LDSM", 0) > 0 and g.get("UBLKCP", 0) > 0 and "UTCHMMA" not in g, g
         assert r.get("FFMA2", 0) > 0 and "HMMA" not in r and "UTCHMMA" not in r, r
