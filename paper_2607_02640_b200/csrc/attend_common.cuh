@@ -50,6 +50,8 @@ struct AttendParams {
     const int32_t* range_item; // GQA decode: item that holds the first tile of each range (null: binary search)
     int32_t* gqa_ctr;         // [2] claim / exit counters of the GQA decode kernel's dynamic ranges (zero between launches)
     int32_t* tickets;         // [item][Hkv] arrival counters of the stream-K pieces (zero between launches)
+    int32_t* pastwait_flag;    // tensor-core kernels: <- pastwait_epoch once past griddepcontrol.wait, i.e. once this step's append
+    int32_t pastwait_epoch;    // kernel is complete (the NEXT append kernel may then do its bookkeeping while this kernel runs); null: off
     unsigned long long* stamp; // measurement aid (null: off): [0] <- min over CTAs of %globaltimer at start, [1] <- max at exit
 };
 
@@ -78,6 +80,11 @@ __device__ __forceinline__ void wait_work_list(const AttendParams& p) {
         asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(seen) : "l"(p.items_flag) : "memory");
         if (seen - p.items_epoch < 0) __nanosleep(64);
     } while (seen - p.items_epoch < 0);
+}
+
+// (one thread of the grid, right after pdl_wait)
+__device__ __forceinline__ void publish_past_wait(const AttendParams& p) {
+    if (p.pastwait_flag) asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p.pastwait_flag), "r"(p.pastwait_epoch) : "memory");
 }
 
 __device__ __forceinline__ float ex2(float x) {

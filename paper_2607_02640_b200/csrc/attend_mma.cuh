@@ -312,6 +312,7 @@ attend_gqa_kernel(AttendParams p, GqaPlan plan) {
     if (p.pdl_early) pdl_launch_dependents();
     if (threadIdx.x == 0) stamp_begin(p);
     pdl_wait();                  // the work list and this step's K/V rows come from the append kernel
+    if (blockIdx.x == 0 && threadIdx.x == 0) publish_past_wait(p);
     extern __shared__ __align__(128) uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 127u) & ~127u;
     uint8_t* smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));

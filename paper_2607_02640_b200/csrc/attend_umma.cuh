@@ -149,6 +149,7 @@ attend_umma_kernel(AttendParams p) {
     if (p.pdl_early) pdl_launch_dependents();
     if (threadIdx.x == 0) stamp_begin(p);
     pdl_wait();                  // the work list and this step's K/V rows come from the append kernel
+    if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) publish_past_wait(p);
     extern __shared__ __align__(1024) uint8_t smem_umma[];
     const uint32_t base = (smem_u32(smem_umma) + 1023u) & ~1023u;       // swizzle atoms are 1024-byte aligned
     uint8_t* gen = smem_umma + (base - smem_u32(smem_umma));

@@ -40,6 +40,9 @@ struct AppendParams {
     int32_t pdl_early;             // early mode: let the dependent (attention) kernel launch right away
     int32_t* items_flag;           // [0] <- epoch once the AttendItems are on the device; [4] <- epoch once past the wait
     int32_t gate_epoch;            // early mode: items_flag[4] must have reached this before the buffer is reused
+    int32_t early_bk;              // bookkeeping (and the work-list copy) BEFORE griddepcontrol.wait, i.e. while the previous
+    const int32_t* pastwait_flag;  // step's attention kernel still runs, as soon as *pastwait_flag has reached pastwait_gate
+    int32_t pastwait_gate;         // (= that kernel is past its own wait = the previous append kernel is complete)
     const uint4* attend_src;       // AttendItems of this step (host), attend_n16 x 16 bytes; may be null
     uint4* attend_dst;
     int32_t attend_n16;
@@ -128,6 +131,25 @@ append_fused_kernel(const AppendParams a) {
             __syncthreads();
             if (threadIdx.x == 0)
                 asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(a.items_flag), "r"(a.epoch) : "memory");
+        }
+        if (a.early_bk) {
+            // Rows a2 / a3 need nothing the previous step's ATTENTION kernel produces, only the tables and the free
+            // stack as the previous APPEND kernel left them: ~4 dependent round trips (table -> stack -> table -> flag)
+            // that used to sit between two attention kernels now run under the tail of the first.  What that kernel may
+            // still read is untouched: freed ids are only pushed, a new block's table slot is one that no block of any
+            // window it reads maps to (checked on the host), and K/V rows are written by the scatter CTAs AFTER the wait.
+            if (threadIdx.x == 0) {
+                int32_t seen;
+                do {
+                    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(seen) : "l"(a.pastwait_flag) : "memory");
+                    if (seen - a.pastwait_gate < 0) __nanosleep(64);
+                } while (seen - a.pastwait_gate < 0);
+            }
+            __syncthreads();
+            copy_items();          // (buffer of this epoch's parity: last read two steps back)
+            if (a.do_bookkeeping) bookkeeping_phases(a, staged ? reinterpret_cast<const AppendItem*>(smem_items) : a.items);
+            pdl_wait();
+            return;
         }
         pdl_wait();
         if (a.pdl_early) {

@@ -99,6 +99,8 @@ struct metronome_pool {
     int32_t* d_tickets = nullptr;      // [max_sessions][Hkv], zero between launches
     int32_t* d_bk_flag = nullptr;      // [0] bookkeeping epoch, [1] work-list epoch, [2..3] GQA claim counters, [5] past-wait epoch
     int32_t last_early_epoch = 0;      // epoch of the previous append kernel if it ran in early mode, else 0
+    int64_t pastwait_launches = -1;    // value of n_launch right after a tensor-core attention launch that publishes its epoch once
+    int32_t pastwait_epoch = 0;        // past its wait (d_bk_flag[12]); still equal to n_launch <=> nothing was launched since
     AttendItem* d_attend_items = nullptr;   // 2 x [max_sessions] (+ range items), written by the append kernel (cached plan)
     size_t attend_buf_bytes = 0;
     size_t ws_slots = 0;               // capacity in (row, head, split) slots
@@ -512,6 +514,7 @@ AttendParams make_attend_params(metronome_pool* pool, int32_t layer, const Atten
     p.pdl_early = 1;
     p.items_flag = pool->d_bk_flag + 1;
     p.items_epoch = -1;
+    p.pastwait_flag = nullptr;
     return p;
 }
 
@@ -536,6 +539,8 @@ int launch_attend(metronome_pool* pool, int32_t layer, const AttendPlan& pl, con
         CU(cudaEventRecord(pool->prof_ev[pool->prof_used], st));
         pdl = false;
     }
+    const bool publish = pl.family == 2 && pdl && !pool->profiling && !pool->poison;
+    if (publish) { p.pastwait_flag = pool->d_bk_flag + 12; p.pastwait_epoch = (int32_t)pool->epoch; }
     if (pl.family == 2) {
         if (pl.n_cls[0] > 0) {
             p.items = d_items; p.n_items = pl.n_cls[0];
@@ -575,6 +580,7 @@ int launch_attend(metronome_pool* pool, int32_t layer, const AttendPlan& pl, con
         else CU(launch_kernel(merge_kernel<64>, grid, dim3(16), 0, st, !pool->profiling, p));
         ++pool->n_launch;
     }
+    if (publish) { pool->pastwait_launches = pool->n_launch; pool->pastwait_epoch = (int32_t)pool->epoch; }
     return METRONOME_OK;
 }
 
@@ -955,6 +961,17 @@ int append_impl(metronome_pool_t* pool, int32_t layer, int32_t n_batch, const in
         a.items_flag = pool->d_bk_flag + 1;
         a.gate_epoch = pool->last_early_epoch;
         pool->last_early_epoch = early ? (int32_t)pool->epoch : 0;
+        // Early bookkeeping (tensor-core family): when the kernel right before this one on the stream is the previous
+        // step's attention kernel (nothing launched since, and it publishes when it is past its wait), rows a2 / a3
+        // run under its tail.  Not when a block allocated now would take the table slot of a block that kernel may
+        // still look up (a block freed in THIS call can hold the oldest key of the previous step's window).
+        bool early_bk = layer == 0 && have_plan && !early && pool->cached_plan.family == 2 && !pool->poison && !pool->profiling &&
+                        pool->pastwait_launches == pool->n_launch && pool->pastwait_epoch == (int32_t)pool->epoch - 1;
+        for (int i = 0; early_bk && i < n_batch; ++i)
+            if (items[i].n_alloc > 0 && items[i].alloc_lo + items[i].n_alloc - 1 - pool->ring >= undo_sessions[i].first_live) early_bk = false;
+        a.early_bk = early_bk ? 1 : 0;
+        a.pastwait_flag = pool->d_bk_flag + 12;
+        a.pastwait_gate = pool->pastwait_epoch;
         if (have_plan) {
             a.attend_src = reinterpret_cast<const uint4*>(h_attend);
             a.attend_dst = reinterpret_cast<uint4*>(reinterpret_cast<uint8_t*>(pool->d_attend_items) + (pool->epoch & 1) * pool->attend_buf_bytes);
