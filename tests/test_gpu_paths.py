@@ -197,3 +197,42 @@ def test_pipelined_host_steps_match_the_blocking_ones(Hkv):
     pool.step_host_wait(0)
     for o, ref, what, *_ in pending:
         assert_parity(o, ref, what)
+
+
+@pytest.mark.parametrize("n_max", [2, 25])
+def test_early_bookkeeping_under_the_previous_attention_kernel(n_max):
+    """Tensor-core family, two launches per step, 300 steps back to back with NOTHING else on the stream: the append
+    kernel of step e does rows a2 / a3 while the attention kernel of step e-1 is still running (early bookkeeping).  A
+    small window frees a block per session every few steps and the freed blocks are reallocated at once (LIFO); with
+    n_max = 25 the chunk steps fill the ring, so the host has to fall back whenever a new block would take the table slot
+    of a block freed in the same call.  Every output and the final tables against the oracle."""
+    Hq, Hkv, D, S, W, N = 16, 2, 128, 4, 40, 6
+    per = 1 + (W + n_max - 1) // 16 + 2
+    kw = dict(n_q_heads=Hq, n_kv_heads=Hkv, head_dim=D, max_sessions=N, max_new_tokens=n_max)
+    pool = binding.Pool(n_sinks=S, window=W, n_blocks=N * per, **kw)
+    cfg = O.PoolConfig(S=S, W=W, n_blocks=N * per, block_size=16, **kw)
+    defn, paged = O.DefinitionOracle(cfg), O.PagedOracle(cfg, store_kv=False)
+    sids = [pool.session_open() for _ in range(N)]
+    assert sids == [defn.session_open() for _ in range(N)] == [paged.session_open() for _ in range(N)]
+    rng = np.random.default_rng(40 + n_max)
+    steps = []
+    for e in range(300):
+        due = sorted(rng.permutation(N)[:int(rng.integers(3, N + 1))].tolist())
+        n_new = np.where(rng.random(len(due)) < 0.15, rng.integers(1, n_max + 1, size=len(due)), 1).astype(np.int32)
+        rows = int(n_new.sum())
+        steps.append(([sids[i] for i in due], n_new, _rows(rng, rows, Hkv, D), _rows(rng, rows, Hkv, D), _rows(rng, rows, Hq, D)))
+    dev = [(k.cuda(), v.cuda(), q.cuda(), torch.empty(q.shape, dtype=torch.bfloat16, device="cuda")) for _, _, k, v, q in steps]
+    torch.cuda.synchronize()
+    stream = torch.cuda.Stream()
+    for (ss, n_new, *_), (k, v, q, o) in zip(steps, dev):       # no host sync, no foreign kernel in between
+        pool.append_kv(0, ss, n_new, k, v, stream.cuda_stream)
+        pool.attend_frame(0, ss, n_new, q, o, stream.cuda_stream)
+    stream.synchronize()
+    for e, ((ss, n_new, k, v, q), (*_, o)) in enumerate(zip(steps, dev)):
+        for orc in (defn, paged):
+            orc.append_kv(0, ss, [int(x) for x in n_new], *((synth.to_u16(k), synth.to_u16(v)) if orc is defn else ()))
+        assert_parity(o, defn.attend_frame(0, ss, [int(x) for x in n_new], synth.to_u16(q)), f"step {e} n={n_new}")
+    for s in sids:
+        got, want = pool.session_query(s), paged.session_query(s)
+        assert (got[0], got[1], list(got[2])) == (want[0], want[1], list(want[2])), s
+    assert pool.pool_query()[1] == paged.pool_query()
