@@ -40,7 +40,9 @@ int metronome_pool_debug_fail_next(metronome_pool_t* pool, int32_t stage);
 
 /* Test aid: copies the pool's 16 internal device flag words to flags16 (host) after cuda_stream has
  * drained: [0] bookkeeping epoch, [1] work-list epoch, [2] / [3] claim and exit counters of the GQA decode
- * kernel's dynamic ranges (must be 0 between launches), [5] past-wait epoch.  Errors: INVALID_ARG, CUDA. */
+ * kernel's dynamic ranges (must be 0 between launches), [5] past-wait epoch of the early-mode append kernel, [8] / [9] / [10] range
+ * claims and exits of the fused step kernel (0 between launches), [12] epoch of the last tensor-core attention kernel that got
+ * past its wait (early bookkeeping).  Errors: INVALID_ARG, CUDA. */
 int metronome_pool_debug_read_flags(metronome_pool_t* pool, void* cuda_stream, int32_t* flags16);
 
 /* Measurement aids for the time of the attention kernels (the dominant kernels; not the append kernel, not the merge).
