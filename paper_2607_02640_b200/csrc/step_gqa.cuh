@@ -57,7 +57,7 @@ struct StepParams {
 static_assert(sizeof(StepParams) <= 32000, "kernel parameters are limited to 32764 bytes");
 
 // What plan_attend() keeps in an AttendItem, recomputed from the 16 bytes above (same formulas:
-// metronome.cu plan_attend; tests/native/gqa_plan_check.cu compares the two).
+// metronome.cu plan_attend; the one-call GPU tests compare the results).
 struct StepGeo {
     int32_t sid, len, q_len, q_row_off, n_sink_tiles, first_blk, n_tiles, tile_off;
     int32_t len0;             // length before this step's append: rows [len0, len) are in k_new / v_new
