@@ -172,7 +172,7 @@ def occupancy_trace(n_sessions: int = 128, n_frames: int = 200):
     returns POOL_EXHAUSTED and compares that frame with Eq. 1's closed form (a block is held from its
     first token, hence the ceil).  Windowed arm: same traffic, 3 x longer, plateau.  Occupancy is read
     from the device free list after every frame (metronome_pool_query)."""
-    from . import binding
+    from paper_2607_02640_b200 import binding
     base = wl.make_workload(3, n_sessions=n_sessions)
     frame = _frame_pattern(base)
     r_tok = sum(frame)
@@ -230,7 +230,7 @@ def admission_run(n_frames: int = 500, budget_ms: float = 2.5, target_frac: floa
     arrive as a Poisson stream far above what fits the deadline, live Exp(300) frames, and are admitted
     only while the gate's cap allows; every frame's measured GPU latency (one layer) feeds the gate.
     Returns one row: cap / live / latency every 25 frames and the steady-state summary."""
-    from . import binding
+    from paper_2607_02640_b200 import binding
     w = wl.make_workload(5)
     frame = _frame_pattern(w)
     rng = np.random.default_rng(seed)
@@ -286,3 +286,60 @@ def admission_run(n_frames: int = 500, budget_ms: float = 2.5, target_frac: floa
              "steady_latency_ms_median": float(np.median(lat_hist[tail])),
              "steady_latency_ms_p99": float(np.percentile(lat_hist[tail], 99)),
              "steady_frames_over_budget_frac": over, "pool_exhausted": 0, "trace_every_25_frames": trace}]
+
+
+# ---------------------------------------------------------------------------------------------------------------
+def summarize(paths) -> str:
+    """Markdown tables from the JSON lines `python bench.py --sweep ...` printed (no GPU needed):
+    python bench_sweeps.py gpurun_out/r02_sweep_*.jsonl > profiles/r02_sweeps.md"""
+    import json
+    rows = []
+    for p in paths:
+        rows += [json.loads(line) for line in open(p) if line.strip().startswith("{")]
+    out = []
+    by = lambda name: [r for r in rows if r.get("sweep") == name]
+    for cfg in sorted({r["config"] for r in by("age")}):
+        rs = [r for r in by("age") if r["config"] == cfg]
+        out += [f"## Latency vs session age, config {cfg}: {rs[0]['sessions']} sessions, S={rs[0]['S']}, W={rs[0]['W']}, every session at the same age",
+                "", "| age / (S+W) | age tokens | frame ms (median) | p99 | attend ms |", "|---|---|---|---|---|"]
+        out += [f"| {r['age_over_S_plus_W']} | {r['age_tokens']} | {r['ms_median']:.4f} | {r['ms_p99']:.4f} | {r['attend_ms_median']:.4f} |" for r in rs]
+        flat = [r["ms_median"] for r in rs if r["age_over_S_plus_W"] >= 1]
+        out += ["", f"Plateau from age = S+W on: {min(flat):.4f} .. {max(flat):.4f} ms (spread {100 * (max(flat) / min(flat) - 1):.1f} %).", ""]
+    rs = by("sessions")
+    if rs:
+        out += ["## Latency vs concurrency, config 5 pool churn (Poisson arrivals, Exp(300-frame) lifetimes)", "",
+                "| n_target | mean live sessions | frame ms (median) | p99 | attend ms | free blocks at end | POOL_EXHAUSTED | arrivals refused |", "|---|---|---|---|---|---|---|---|"]
+        out += [f"| {r['n_target']} | {r.get('sessions_mean', float('nan')):.1f} | {r['ms_median']:.3f} | {r['ms_p99']:.3f} | {r['attend_ms_median']:.3f} | "
+                f"{r['free_blocks_end']} | {r['pool_exhausted']} | {r['rejected_arrivals']} |" for r in rs]
+        med = [r["ms_median"] for r in rs]
+        out += ["", "Medians rise monotonically with load: " + str(all(b >= a for a, b in zip(med, med[1:]))) +
+                f"; pool {rs[0]['pool_blocks']} blocks, never exhausted.", ""]
+    rs = by("sw")
+    if rs:
+        out += ["## (S, W) sweep on config-3 shapes, every session at age 2 x (S+W) (NEXT f1)", "",
+                "| S | W | blocks / session | frame ms (median) | p99 | attend ms |", "|---|---|---|---|---|---|"]
+        out += [f"| {r['S']} | {r['W']} | {r['blocks_per_session']} | {r['ms_median']:.4f} | {r['ms_p99']:.4f} | {r['attend_ms_median']:.4f} |" for r in rs]
+        out += [""]
+    rs = by("occupancy")
+    if rs:
+        out += ["## Pool occupancy, unbounded vs windowed arm (NEXT f2, PAPER.md Eq. 1)", "",
+                "| arm | frames run | POOL_EXHAUSTED at frame | Eq. 1 t_sat (frame) | Eq. 1 slope / frame | fitted slope (first 20 frames) | occupancy max | occupancy at end |", "|---|---|---|---|---|---|---|---|"]
+        out += [f"| {r['arm']} | {r['frames_run']} | {r['pool_exhausted_at_frame']} | {r['eq1_t_sat_frame']} | {r['eq1_slope_per_frame']:.5f} | "
+                f"{(r['fit_slope_first_20_frames'] or 0):.5f} | {(r['occupancy_max'] or 0):.4f} | {(r['occupancy_end'] or 0):.4f} |" for r in rs]
+        out += [""]
+    rs = by("admission")
+    if rs:
+        r = rs[0]
+        out += ["## AIMD admission gate on the measured per-frame latency (NEXT f3)", "",
+                f"budget {r['budget_ms']} ms, target {r['target_ms']} ms, {r['arrivals_per_frame']} arrivals per frame, {r['frames']} frames: admitted {r['admitted']}, "
+                f"rejected {r['rejected']}; second half: live sessions {r['steady_live_mean']:.1f}, cap {r['steady_cap_mean']:.1f}, latency median "
+                f"{r['steady_latency_ms_median']:.3f} ms, p99 {r['steady_latency_ms_p99']:.3f} ms, frames over budget {100 * r['steady_frames_over_budget_frac']:.1f} %.", "",
+                "| frame | cap | live | latency ms |", "|---|---|---|---|"]
+        out += [f"| {t['frame']} | {t['cap']} | {t['live']} | {t['latency_ms']} |" for t in r["trace_every_25_frames"]]
+        out += [""]
+    return "\n".join(out)
+
+
+if __name__ == "__main__":
+    import sys
+    print(summarize(sys.argv[1:]))
