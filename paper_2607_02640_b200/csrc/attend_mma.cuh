@@ -272,7 +272,8 @@ struct GqaCfg {
 //            work is handed out in small pieces.
 struct GqaPlan {
     int32_t n_kv_heads;
-    int64_t total_tiles;      // Hkv * sum of the items' n_tiles
+    int32_t bnd;              // cost of starting an (item, head) pair, in tiles (see make_gqa_plan)
+    int64_t total_tiles;      // Hkv * sum of (the items' n_tiles + bnd): the list is cut in these COST units
     int64_t q1, g1;           // static regime
     int64_t q2;               // dynamic regime
     int32_t n_static, n_total;
@@ -286,14 +287,24 @@ struct GqaPlan {
         return g < g1 ? (int32_t)(g / q1) : n_static + (int32_t)((g - g1) / q2);
     }
     // upper bound on the pieces one (item, head) pair of n tiles can be cut into
-    __host__ __device__ int32_t max_pieces(int32_t n) const { return (int32_t)((n + q2 - 1) / q2) + 2; }
+    // (the shorter of the two range lengths: a forced dynamic plan of tiny shares has q2 = 8 > q1)
+    __host__ __device__ int32_t max_pieces(int32_t n) const {
+        const int64_t q = q1 < q2 ? q1 : q2;
+        return (int32_t)((n + q - 1) / q) + 2;
+    }
 };
 
 // Host: cut `total_tiles` into one static range per CTA and, when `dynamic`, keep the last 10 % for
 // small ranges (a sixth of a static one, at least 8 tiles) that the CTAs claim as they finish.
-inline GqaPlan make_gqa_plan(int32_t n_kv_heads, int64_t total_tiles, int64_t ctas, bool dynamic) {
+// The list is measured in COST units: pair (item i, head h) occupies n_tiles_i + bnd units starting at
+// (tile_off_i + bnd * i) * Hkv + h * (n_tiles_i + bnd); its first `bnd` units stand for the work of starting a pair
+// (item, table and Q fetch, merge of the four warps, write-out: ~4 us per pair on a B200, during which the CTA
+// streams nothing), the rest are its tiles.  Equal TILE shares ended 62 / 71 / 74 / 78 / 84 us after the wait for CTAs
+// that held 1 / 2 / 3 / 4 / 6 pairs (config 3), and the kernel ends with the last one.
+inline GqaPlan make_gqa_plan(int32_t n_kv_heads, int64_t total_tiles, int64_t ctas, bool dynamic, int32_t bnd) {
     GqaPlan g{};
     g.n_kv_heads = n_kv_heads;
+    g.bnd = bnd;
     g.total_tiles = total_tiles;
     const int64_t share = (total_tiles + ctas - 1) / ctas;
     g.q1 = dynamic ? (share * 9 + 9) / 10 : share;
@@ -302,6 +313,22 @@ inline GqaPlan make_gqa_plan(int32_t n_kv_heads, int64_t total_tiles, int64_t ct
     g.q2 = dynamic ? (g.q1 / 6 > 8 ? g.q1 / 6 : 8) : g.q1;
     g.n_total = g.n_static + (int32_t)((total_tiles - g.g1 + g.q2 - 1) / g.q2);
     return g;
+}
+
+// The piece of pair (item i, the head that holds unit g) that a range ending at unit g_end takes: tiles [a, b) of the
+// pair (b <= a: the range ends inside the pair's start-up units), pair_lo = the unit of the pair's tile 0.  A walk over a
+// range goes g -> pair_lo + b (and on to item i + 1 after the last head); tests/native/gqa_plan_check.cu walks every
+// range of random plans with this same function and checks that each tile is visited exactly once.
+struct GqaPiece { int32_t kvh, a, b; int64_t pair_lo; };
+__host__ __device__ inline GqaPiece gqa_piece(const GqaPlan& plan, int32_t i, int32_t tile_off, int32_t n_tiles, int64_t g, int64_t g_end) {
+    GqaPiece pc;
+    const int64_t item_lo = ((int64_t)tile_off + (int64_t)plan.bnd * i) * plan.n_kv_heads;
+    pc.kvh = (int32_t)((g - item_lo) / (n_tiles + plan.bnd));
+    pc.pair_lo = item_lo + (int64_t)pc.kvh * (n_tiles + plan.bnd) + plan.bnd;
+    const int64_t a = g - pc.pair_lo, b = g_end - pc.pair_lo;
+    pc.a = (int32_t)(a > 0 ? a : 0);
+    pc.b = (int32_t)(b < n_tiles ? b : n_tiles);
+    return pc;
 }
 
 // grid = n_SM * CTAs/SM (<= total tiles), block = 128.  items[].tile_off = exclusive prefix of n_tiles.
@@ -329,11 +356,12 @@ attend_gqa_kernel(AttendParams p, GqaPlan plan) {
     const int32_t Hkv = plan.n_kv_heads;
     __shared__ int32_t s_range;
     int32_t range = blockIdx.x;                          // first the CTA's static range, then claimed ones
+    const int32_t bnd = plan.bnd;
     while (range < plan.n_total) {
-    int64_t g = plan.range_lo(range);
+    int64_t g = plan.range_lo(range);                    // (cost units, see make_gqa_plan)
     const int64_t g_end = plan.range_hi(range);
-    // the item that holds the range's first tile: from the host's table, else by binary search
-    // (largest i with tile_off[i] * Hkv <= g); later pairs of the range follow without a search
+    // the item that holds the range's first unit: from the host's table, else by binary search
+    // (largest i with (tile_off[i] + bnd * i) * Hkv <= g); later pairs of the range follow without a search
     int32_t i = 0;
     if (p.range_item) {
         i = p.range_item[range];
@@ -341,19 +369,18 @@ attend_gqa_kernel(AttendParams p, GqaPlan plan) {
         int32_t lo = 0, hi = p.n_items - 1;
         while (lo < hi) {
             const int32_t mid = (lo + hi + 1) >> 1;
-            if ((int64_t)p.items[mid].tile_off * Hkv <= g) lo = mid; else hi = mid - 1;
+            if (((int64_t)p.items[mid].tile_off + (int64_t)bnd * mid) * Hkv <= g) lo = mid; else hi = mid - 1;
         }
         i = lo;
     }
     int32_t pre = 0;        // 1: the first tile of the coming pair is already in flight, in stage 1
     while (g < g_end) {
-        // ---- the (item, head) pair that holds global tile g, and this CTA's piece of it ----
+        // ---- the (item, head) pair that holds unit g, and this CTA's piece of it: tiles [a, b) ----
         const AttendItem it = p.items[i];
-        const int64_t item_lo = (int64_t)it.tile_off * Hkv;
-        const int32_t kvh = (int32_t)((g - item_lo) / it.n_tiles);
-        const int64_t pair_lo = item_lo + (int64_t)kvh * it.n_tiles;
-        const int32_t a = (int32_t)(g - pair_lo);
-        const int32_t b = (int32_t)min((int64_t)it.n_tiles, g_end - pair_lo);
+        const GqaPiece pc = gqa_piece(plan, i, it.tile_off, it.n_tiles, g, g_end);
+        const int32_t kvh = pc.kvh, a = pc.a, b = pc.b;
+        const int64_t pair_lo = pc.pair_lo;                                    // unit of the pair's tile 0
+        if (b <= a) break;                               // the range ends inside this pair's start-up units
         const int32_t first_cta = plan.range_of(pair_lo);                      // first / last range of this pair
         const int32_t last_cta = plan.range_of(pair_lo + it.n_tiles - 1);
 
@@ -390,14 +417,14 @@ attend_gqa_kernel(AttendParams p, GqaPlan plan) {
         // takes that tile now (saves the table -> HBM round trip after every (item, head) boundary) ----
         const int32_t R_rows = it.q_len * p.G;
         pre = 0;
-        if (R_rows * (D + 2) * 4 <= C::kHeadBytes && b == it.n_tiles && pair_lo + b < g_end) {
+        if (R_rows * (D + 2) * 4 <= C::kHeadBytes && b == it.n_tiles && pair_lo + b + bnd < g_end) {
             const bool same = kvh + 1 < Hkv;
             const int32_t i2 = same ? i : i + 1;
             const int32_t sid2 = same ? it.sid : p.items[i2].sid;
             const int32_t nt2 = same ? it.n_tiles : p.items[i2].n_tiles;
             const int32_t sink2 = same ? it.n_sink_tiles : p.items[i2].n_sink_tiles;
             const int32_t first2 = same ? it.first_blk : p.items[i2].first_blk;
-            const int32_t b2 = (int32_t)min((int64_t)nt2, g_end - (pair_lo + b));
+            const int32_t b2 = (int32_t)min((int64_t)nt2, g_end - (pair_lo + b + bnd));
             if (warp < b2) {
                 if (lane == 0) {
                     const int32_t blk = warp < sink2 ? warp : first2 + (warp - sink2);

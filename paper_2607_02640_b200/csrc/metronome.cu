@@ -43,6 +43,9 @@ constexpr int kStagingGroup = 8;       // one completion event per 8 slots: an e
                                        // would break their programmatic (PDL) launch edge
 constexpr int kMaxSplits = 64;
 constexpr int kStampSlots = 1 << 15;   // attention launches one stamped pass can hold
+#ifndef METRONOME_GQA_BND_BYTES
+#define METRONOME_GQA_BND_BYTES 65536
+#endif
 constexpr int kMaxRangeItems = 4096;   // GQA decode ranges whose start item travels with the work list
 
 // Row a8: the launch plan of one attend_frame call (host side of the work list).  Items of class 0
@@ -386,7 +389,10 @@ int plan_attend(metronome_pool* pool, int32_t n_batch, const int32_t* sids, cons
             // imbalance it removes (configs 3 and 4: +3..7 %), so they stay fully static
             const bool dynamic = pool->tune_gqa_dynamic == 1 ||
                                  (pool->tune_gqa_dynamic == 0 && pool->tune_split_tokens <= 0 && (total_tiles + ctas - 1) / ctas >= 512);
-            pl.gplan = make_gqa_plan(c.n_kv_heads, total_tiles, ctas, dynamic);
+            // ranges are cut in cost units: a pair's tiles + what starting a pair costs (make_gqa_plan), the latter
+            // ~4 us of one CTA's share of the stream = METRONOME_GQA_BND_BYTES of K/V tiles
+            const int32_t bnd = (int32_t)(METRONOME_GQA_BND_BYTES / (2 * kBlockTokens * c.head_dim * 2));
+            pl.gplan = make_gqa_plan(c.n_kv_heads, (cls_tiles[0] + (int64_t)bnd * n) * c.n_kv_heads, ctas, dynamic, bnd);
             GqaPlan& g = pl.gplan;
             pl.gqa_ctas = g.n_static;
             if (g.n_total <= kMaxRangeItems) {
@@ -394,7 +400,7 @@ int plan_attend(metronome_pool* pool, int32_t n_batch, const int32_t* sids, cons
                 int32_t ii = 0;
                 for (int32_t r = 0; r < g.n_total; ++r) {
                     const int64_t lo = g.range_lo(r);
-                    while (ii + 1 < n && (int64_t)its[ii + 1].tile_off * c.n_kv_heads <= lo) ++ii;
+                    while (ii + 1 < n && ((int64_t)its[ii + 1].tile_off + (int64_t)bnd * (ii + 1)) * c.n_kv_heads <= lo) ++ii;
                     range_item[r] = ii;
                 }
                 pl.n_range_items = g.n_total;
