@@ -40,7 +40,7 @@ def build_library(force: bool = False, verbose: bool = False) -> str:
 
 
 CENSUS_OPS = ("UTCHMMA", "UTCBAR", "LDTM", "STTM", "UBLKCP", "SYNCS", "HMMA", "LDSM", "LDG", "STG", "MUFU.EX2", "FFMA2",
-              "ATOMG", "REDG", "ACQBULK", "LDGDEPBAR")
+              "ATOMG", "REDG", "ACQBULK", "LDGDEPBAR", "F2FP.F16.E4M3", "PRMT")
 
 
 def sass_census() -> dict:

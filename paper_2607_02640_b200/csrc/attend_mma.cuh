@@ -30,6 +30,8 @@
 // head at G flop/byte; a 128-row UMMA tile would be > 87 % padding.  The shared helpers of this file
 // (mbarrier / bulk-copy wrappers, tile_block) are used by the chunk kernel too.
 #pragma once
+#include <type_traits>
+
 #include "attend_common.cuh"
 
 namespace metronome {
@@ -72,6 +74,36 @@ __device__ __forceinline__ void mma_bf16(float (&c)[4], const uint32_t (&a)[4], 
     asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
                  : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
                  : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+__device__ __forceinline__ void mma_f16(float (&c)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
+    asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                 : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+                 : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+// two E4M3 codes (low byte -> low half) as two fp16 values: exact, E4M3 is a subset of fp16
+__device__ __forceinline__ uint32_t e4m3x2_f16x2(uint16_t v) {
+    uint32_t d;
+    asm("cvt.rn.f16x2.e4m3x2 %0, %1;" : "=r"(d) : "h"(v));
+    return d;
+}
+__device__ __forceinline__ uint32_t pack_f16(float lo, float hi) {
+    __half2 v = __floats2half2_rn(lo, hi);
+    return *reinterpret_cast<uint32_t*>(&v);
+}
+__device__ __forceinline__ float2 lds_f2(uint32_t addr) {
+    float2 v;
+    asm volatile("ld.shared.v2.f32 {%0,%1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ uint4 lds_u4(uint32_t addr) {
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ uint2 lds_u2(uint32_t addr) {
+    uint2 v;
+    asm volatile("ld.shared.v2.u32 {%0,%1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr));
+    return v;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -216,6 +248,21 @@ struct WarpTile {
         }
     }
 
+    // this warp's state of the rows < R_rows into the CTA's merge scratch: [R][D + 2] floats = acc | m | l
+    __device__ __forceinline__ void to_scratch(float* scratch, int32_t R_rows, int32_t lane) const {
+        const int32_t ra = lane >> 2, c = (lane & 3) * 2;
+        const bool wa = ra < R_rows, wb = ra + 8 < R_rows;
+#pragma unroll
+        for (int n = 0; n < NT; ++n) {
+            if (wa) *reinterpret_cast<float2*>(scratch + ra * (D + 2) + n * 8 + c) = make_float2(o[n][0], o[n][1]);
+            if (wb) *reinterpret_cast<float2*>(scratch + (ra + 8) * (D + 2) + n * 8 + c) = make_float2(o[n][2], o[n][3]);
+        }
+        if ((lane & 3) == 0) {
+            if (wa) { scratch[ra * (D + 2) + D] = m_a; scratch[ra * (D + 2) + D + 1] = lsum[0]; }
+            if (wb) { scratch[(ra + 8) * (D + 2) + D] = m_b; scratch[(ra + 8) * (D + 2) + D + 1] = lsum[2]; }
+        }
+    }
+
     // final bf16 output (the piece covered every tile of this (item, head))
     __device__ __forceinline__ void store_final(const AttendParams& p, int32_t lane) const {
         const float ia = lsum[0] > 0.f ? 1.f / lsum[0] : 0.f, ib = lsum[2] > 0.f ? 1.f / lsum[2] : 0.f;
@@ -244,6 +291,245 @@ struct WarpTile {
     }
 };
 
+// ------------------------------------------------------------------------------------------------
+// The same m16 row tile over an fp8 (E4M3) KV pool (NEXT row f4, "the two compose"; DESIGN.md reading
+// R18: code x one float32 scale per (token, KV head) row).  The codes go to the tensor core as fp16 -- E4M3 is a subset
+// of fp16, so `cvt.rn.f16x2.e4m3x2` is exact -- and the scales never touch an operand:
+//   * S = (Q' C_K^T) * ks_j * qs_row: the K scale of key j multiplies the finished fp32 dot product; Q' is the bf16
+//     query row times a power of two that brings its largest element into [1, 2) (exact, undone by qs_row), rounded
+//     to fp16 (exact for every element within 2^-14 of the row's maximum, 2^-25 absolute below);
+//   * O = sum_j (p_j * vs_j / vref) C_V[j] * vref: the V scale of key j is folded into the softmax weight before it
+//     is rounded to fp16 (11 bits: no hi / lo split as in the bf16 tile), relative to a running reference vref >= every
+//     V scale seen so far and times 2^15, so the weights stay in [0, 2^13] whatever the magnitude of V and keep full
+//     fp16 precision down to p_j vs_j = 2^-29 vref (a one-hot row on a key whose V is 10^5 times smaller than its
+//     neighbours' still comes out to 11 bits); O is rescaled when vref grows (warp-uniform, rare: vref is raised with
+//     a factor 4 of headroom); the denominator is summed in fp32 from the unrounded p_j, each thread its own four
+//     keys of a tile, reduced over the quad once at the end.
+// Fragments without a transposing load: a k16 step of Q K^T takes 16-byte chunk c of the K rows (ldmatrix on code
+// bytes gives a thread 4 consecutive codes = its k = 2t, 2t+1 | 2t+8, 2t+9 operands, the Q fragment is fetched in the
+// same order); for P V a thread reads D/8 code bytes of rows 2t, 2t+1, 2t+8, 2t+9 and byte-permutes row pairs together,
+// so n8 tile j, column g is dim (D/8) g + j: the thread ends up with D/4 CONSECUTIVE dims of its two rows.
+template <int D>
+struct WarpTileF8 {
+    static constexpr int KSTEPS = D / 16;
+    static constexpr int NT = D / 8;
+    static constexpr int kTileBytes = kBlockTokens * D;
+    uint32_t qa[KSTEPS][4];
+    float o[NT][4];                          // [j][e] rows a (e = 0, 1) / b (e = 2, 3): dim (D/4) t + (e & 1) NT + j, in units of vref / 2^15
+    float m_a, m_b;
+    float lsum[4];                           // [0] row a, [2] row b: this thread's own keys only (see quad_sum)
+    float qs_a, qs_b;                        // scale_log2 * 2^e of the row's Q prescale
+    float vref, inv_vref;
+    int32_t ta, tb, t_min, t_max;
+    bool va, vb;
+    int64_t qrow_a, qrow_b;
+
+    template <typename Item>
+    __device__ __forceinline__ void init(const AttendParams& p, const Item& it, int32_t kvh, int32_t mtile,
+                                         int32_t lane) {
+        const int32_t R = it.q_len * p.G;
+        const int32_t t_first = it.len - it.q_len;            // reading R15: the last q_len positions
+        const int32_t rho_a = 16 * mtile + (lane >> 2), rho_b = rho_a + 8;
+        va = rho_a < R; vb = rho_b < R;
+        const int32_t ra = rho_a / p.G, rb = rho_b / p.G;
+        ta = va ? t_first + ra : -1;
+        tb = vb ? t_first + rb : -1;
+        qrow_a = (int64_t)(it.q_row_off + ra) * p.Hq + kvh * p.G + (rho_a - ra * p.G);
+        qrow_b = (int64_t)(it.q_row_off + rb) * p.Hq + kvh * p.G + (rho_b - rb * p.G);
+        t_min = t_first + (16 * mtile) / p.G;
+        t_max = t_first + (min(R, 16 * mtile + 16) - 1) / p.G;
+        // dims 16 kk + 4 t .. + 3 of the row: k = 2t, 2t+1 (first word) and 2t+8, 2t+9 (second word) of k-step kk
+        const uint2* pa = reinterpret_cast<const uint2*>(p.q + qrow_a * D);
+        const uint2* pb = reinterpret_cast<const uint2*>(p.q + qrow_b * D);
+        const int32_t c = lane & 3;
+        uint2 xa[KSTEPS], xb[KSTEPS];
+        float amax_a = 0.f, amax_b = 0.f;
+#pragma unroll
+        for (int kk = 0; kk < KSTEPS; ++kk) {
+            xa[kk] = va ? __ldg(pa + kk * 4 + c) : make_uint2(0u, 0u);
+            xb[kk] = vb ? __ldg(pb + kk * 4 + c) : make_uint2(0u, 0u);
+            amax_a = fmaxf(fmaxf(amax_a, fmaxf(fabsf(bf16lo(xa[kk].x)), fabsf(bf16hi(xa[kk].x)))),
+                           fmaxf(fabsf(bf16lo(xa[kk].y)), fabsf(bf16hi(xa[kk].y))));
+            amax_b = fmaxf(fmaxf(amax_b, fmaxf(fabsf(bf16lo(xb[kk].x)), fabsf(bf16hi(xb[kk].x)))),
+                           fmaxf(fabsf(bf16lo(xb[kk].y)), fabsf(bf16hi(xb[kk].y))));
+        }
+        amax_a = fmaxf(amax_a, __shfl_xor_sync(0xffffffffu, amax_a, 1));
+        amax_a = fmaxf(amax_a, __shfl_xor_sync(0xffffffffu, amax_a, 2));
+        amax_b = fmaxf(amax_b, __shfl_xor_sync(0xffffffffu, amax_b, 1));
+        amax_b = fmaxf(amax_b, __shfl_xor_sync(0xffffffffu, amax_b, 2));
+        // 2^(127 - E) brings the row's largest element into [1, 2); E = its biased exponent (a zero row: factor 1)
+        int32_t Ea = (__float_as_int(amax_a) >> 23) & 0xff, Eb = (__float_as_int(amax_b) >> 23) & 0xff;
+        Ea = Ea == 0 ? 127 : min(Ea, 253);
+        Eb = Eb == 0 ? 127 : min(Eb, 253);
+        const float da = __int_as_float((254 - Ea) << 23), db = __int_as_float((254 - Eb) << 23);
+        qs_a = p.scale_log2 * __int_as_float(Ea << 23);
+        qs_b = p.scale_log2 * __int_as_float(Eb << 23);
+#pragma unroll
+        for (int kk = 0; kk < KSTEPS; ++kk) {
+            qa[kk][0] = pack_f16(bf16lo(xa[kk].x) * da, bf16hi(xa[kk].x) * da);
+            qa[kk][1] = pack_f16(bf16lo(xb[kk].x) * db, bf16hi(xb[kk].x) * db);
+            qa[kk][2] = pack_f16(bf16lo(xa[kk].y) * da, bf16hi(xa[kk].y) * da);
+            qa[kk][3] = pack_f16(bf16lo(xb[kk].y) * db, bf16hi(xb[kk].y) * db);
+        }
+        reset();
+    }
+    __device__ __forceinline__ void reset() {
+#pragma unroll
+        for (int n = 0; n < NT; ++n) { o[n][0] = o[n][1] = o[n][2] = o[n][3] = 0.f; }
+        m_a = m_b = -INFINITY;
+        lsum[0] = lsum[1] = lsum[2] = lsum[3] = 0.f;
+        vref = 0.f; inv_vref = 0.f;
+    }
+    __device__ __forceinline__ bool skips(const AttendParams& p, int32_t p0) const {
+        return p0 > t_max || (p0 >= p.S && t_min - (p0 + kBlockTokens - 1) >= p.W);
+    }
+
+    // one 16-key tile at shared-memory address kt: [K codes][V codes][16 K scales][16 V scales]
+    template <int kLoInv>
+    __device__ __forceinline__ void step(const AttendParams& p, int32_t len, uint32_t kt, uint32_t vt, int32_t p0,
+                                         int32_t lane) {
+        const uint32_t sc = kt + 2 * kTileBytes;
+        const int32_t mat = lane >> 3, r8 = lane & 7;
+        const int32_t k_row = r8 + ((mat & 1) << 3), k_cs = mat >> 1;   // K: (rows 0-7 | 8-15) x (chunk, chunk+1)
+        const int32_t g = lane >> 2, t = lane & 3, col0 = 2 * t;
+        // ---- S = Q' C_K^T: two n8 tiles (keys 0-7 | 8-15) ----
+        float s0[4] = {0.f, 0.f, 0.f, 0.f}, s1[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+        for (int kk = 0; kk < KSTEPS; kk += 2) {
+            uint32_t d0, d1, d2, d3;
+            ldsm_x4(kt + fp8_chunk_offset(D, k_row, kk + k_cs), d0, d1, d2, d3);
+            mma_f16(s0, qa[kk], e4m3x2_f16x2((uint16_t)d0), e4m3x2_f16x2((uint16_t)(d0 >> 16)));
+            mma_f16(s1, qa[kk], e4m3x2_f16x2((uint16_t)d1), e4m3x2_f16x2((uint16_t)(d1 >> 16)));
+            mma_f16(s0, qa[kk + 1], e4m3x2_f16x2((uint16_t)d2), e4m3x2_f16x2((uint16_t)(d2 >> 16)));
+            mma_f16(s1, qa[kk + 1], e4m3x2_f16x2((uint16_t)d3), e4m3x2_f16x2((uint16_t)(d3 >> 16)));
+        }
+        // ---- the rows' scales: keys col0, col0+1 (.x, .y of *_lo) and col0+8, col0+9 (*_hi) ----
+        const float2 ks_lo = lds_f2(sc + col0 * 4), ks_hi = lds_f2(sc + (col0 + 8) * 4);
+        float2 vs_lo = lds_f2(sc + (kBlockTokens + col0) * 4), vs_hi = lds_f2(sc + (kBlockTokens + col0 + 8) * 4);
+        float sv[8];                            // log2 domain: [0] [1] row a, [2] [3] row b keys col0, col0+1; [4..7] keys col0+8, +9
+        sv[0] = s0[0] * (ks_lo.x * qs_a); sv[1] = s0[1] * (ks_lo.y * qs_a);
+        sv[2] = s0[2] * (ks_lo.x * qs_b); sv[3] = s0[3] * (ks_lo.y * qs_b);
+        sv[4] = s1[0] * (ks_hi.x * qs_a); sv[5] = s1[1] * (ks_hi.y * qs_a);
+        sv[6] = s1[2] * (ks_hi.x * qs_b); sv[7] = s1[3] * (ks_hi.y * qs_b);
+        // ---- union mask, boundary tiles only (a masked score may be anything, NaN included: it is replaced) ----
+        const bool full = (p0 + kBlockTokens - 1 <= t_min) && (p0 + kBlockTokens - 1 < p.S || t_max - p0 < p.W);
+        if (!full) {
+            const int32_t ja = p0 + col0, jb = ja + 8;
+            sv[0] = admit(ja, ta, p.S, p.W) ? sv[0] : -INFINITY;
+            sv[1] = admit(ja + 1, ta, p.S, p.W) ? sv[1] : -INFINITY;
+            sv[2] = admit(ja, tb, p.S, p.W) ? sv[2] : -INFINITY;
+            sv[3] = admit(ja + 1, tb, p.S, p.W) ? sv[3] : -INFINITY;
+            sv[4] = admit(jb, ta, p.S, p.W) ? sv[4] : -INFINITY;
+            sv[5] = admit(jb + 1, ta, p.S, p.W) ? sv[5] : -INFINITY;
+            sv[6] = admit(jb, tb, p.S, p.W) ? sv[6] : -INFINITY;
+            sv[7] = admit(jb + 1, tb, p.S, p.W) ? sv[7] : -INFINITY;
+        }
+        // ---- online softmax (log2 domain) ----
+        float mx_a = fmaxf(fmaxf(sv[0], sv[1]), fmaxf(sv[4], sv[5]));
+        float mx_b = fmaxf(fmaxf(sv[2], sv[3]), fmaxf(sv[6], sv[7]));
+        mx_a = fmaxf(mx_a, __shfl_xor_sync(0xffffffffu, mx_a, 1));
+        mx_a = fmaxf(mx_a, __shfl_xor_sync(0xffffffffu, mx_a, 2));
+        mx_b = fmaxf(mx_b, __shfl_xor_sync(0xffffffffu, mx_b, 1));
+        mx_b = fmaxf(mx_b, __shfl_xor_sync(0xffffffffu, mx_b, 2));
+        const float mn_a = fmaxf(m_a, mx_a), mn_b = fmaxf(m_b, mx_b);
+        // ---- V scales: rows past the session's length hold stale / poisoned bytes ----
+        const int32_t nvalid = len - p0;                     // < 16 only in the session's last block
+        if (nvalid < kBlockTokens) {
+            vs_lo.x = col0 < nvalid ? vs_lo.x : 0.f; vs_lo.y = col0 + 1 < nvalid ? vs_lo.y : 0.f;
+            vs_hi.x = col0 + 8 < nvalid ? vs_hi.x : 0.f; vs_hi.y = col0 + 9 < nvalid ? vs_hi.y : 0.f;
+        }
+        float vmax = fmaxf(fmaxf(vs_lo.x, vs_lo.y), fmaxf(vs_hi.x, vs_hi.y));
+        vmax = fmaxf(vmax, __shfl_xor_sync(0xffffffffu, vmax, 1));
+        vmax = fmaxf(vmax, __shfl_xor_sync(0xffffffffu, vmax, 2));       // (the same in every quad: warp-uniform)
+        const bool grow = vmax > vref;
+        if (grow || __any_sync(0xffffffffu, (mn_a != m_a) || (mn_b != m_b))) {
+            float ca = mn_a == -INFINITY ? 1.f : ex2(m_a - mn_a);
+            float cb = mn_b == -INFINITY ? 1.f : ex2(m_b - mn_b);
+            lsum[0] *= ca; lsum[2] *= cb;
+            if (grow) {
+                const float nv = vmax * 4.f, f = vref / nv;
+                ca *= f; cb *= f;
+                vref = nv; inv_vref = 32768.f / nv;
+            }
+#pragma unroll
+            for (int n = 0; n < NT; ++n) { o[n][0] *= ca; o[n][1] *= ca; o[n][2] *= cb; o[n][3] *= cb; }
+            m_a = mn_a; m_b = mn_b;
+        }
+        const float sub_a = m_a == -INFINITY ? 0.f : m_a, sub_b = m_b == -INFINITY ? 0.f : m_b;
+        float pr[8];
+        pr[0] = ex2(sv[0] - sub_a); pr[1] = ex2(sv[1] - sub_a); pr[2] = ex2(sv[2] - sub_b); pr[3] = ex2(sv[3] - sub_b);
+        pr[4] = ex2(sv[4] - sub_a); pr[5] = ex2(sv[5] - sub_a); pr[6] = ex2(sv[6] - sub_b); pr[7] = ex2(sv[7] - sub_b);
+        lsum[0] += (pr[0] + pr[1]) + (pr[4] + pr[5]);
+        lsum[2] += (pr[2] + pr[3]) + (pr[6] + pr[7]);
+        const float w0 = vs_lo.x * inv_vref, w1 = vs_lo.y * inv_vref, w8 = vs_hi.x * inv_vref, w9 = vs_hi.y * inv_vref;
+        uint32_t pw[4];                          // A fragment of P V: [0] row a keys col0.., [1] row b, [2] row a keys 8+col0.., [3] row b
+        pw[0] = pack_f16(pr[0] * w0, pr[1] * w1);
+        pw[1] = pack_f16(pr[2] * w0, pr[3] * w1);
+        pw[2] = pack_f16(pr[4] * w8, pr[5] * w9);
+        pw[3] = pack_f16(pr[6] * w8, pr[7] * w9);
+        // ---- O += P' C_V: code bytes (D/8) g .. of rows 2t, 2t+1 | 2t+8, 2t+9, row pairs zipped with byte permutes ----
+        uint32_t mk0 = 0xFFFFFFFFu, mk1 = 0xFFFFFFFFu;
+        if (nvalid < kBlockTokens) {
+            mk0 = (col0 < nvalid ? 0x00FF00FFu : 0u) | (col0 + 1 < nvalid ? 0xFF00FF00u : 0u);
+            mk1 = (col0 + 8 < nvalid ? 0x00FF00FFu : 0u) | (col0 + 9 < nvalid ? 0xFF00FF00u : 0u);
+        }
+        constexpr int WPR = D / 32;              // 32-bit words a thread takes from each row
+        uint32_t r0[WPR], r1[WPR], r2[WPR], r3[WPR];
+        if constexpr (D == 128) {
+            const uint4 a0 = lds_u4(vt + fp8_chunk_offset(D, col0, g)), a1 = lds_u4(vt + fp8_chunk_offset(D, col0 + 1, g));
+            const uint4 a2 = lds_u4(vt + fp8_chunk_offset(D, col0 + 8, g)), a3 = lds_u4(vt + fp8_chunk_offset(D, col0 + 9, g));
+            r0[0] = a0.x; r0[1] = a0.y; r0[2] = a0.z; r0[3] = a0.w;
+            r1[0] = a1.x; r1[1] = a1.y; r1[2] = a1.z; r1[3] = a1.w;
+            r2[0] = a2.x; r2[1] = a2.y; r2[2] = a2.z; r2[3] = a2.w;
+            r3[0] = a3.x; r3[1] = a3.y; r3[2] = a3.z; r3[3] = a3.w;
+        } else {
+            static_assert(D == 64 || D == 128, "head_dim");
+            const uint2 a0 = lds_u2(vt + fp8_unit_offset(D, col0, g)), a1 = lds_u2(vt + fp8_unit_offset(D, col0 + 1, g));
+            const uint2 a2 = lds_u2(vt + fp8_unit_offset(D, col0 + 8, g)), a3 = lds_u2(vt + fp8_unit_offset(D, col0 + 9, g));
+            r0[0] = a0.x; r0[1] = a0.y; r1[0] = a1.x; r1[1] = a1.y;
+            r2[0] = a2.x; r2[1] = a2.y; r3[0] = a3.x; r3[1] = a3.y;
+        }
+#pragma unroll
+        for (int i = 0; i < WPR; ++i) {
+            uint32_t x01 = __byte_perm(r0[i], r1[i], 0x5140), x23 = __byte_perm(r0[i], r1[i], 0x7362);
+            uint32_t y01 = __byte_perm(r2[i], r3[i], 0x5140), y23 = __byte_perm(r2[i], r3[i], 0x7362);
+            if (nvalid < kBlockTokens) { x01 &= mk0; x23 &= mk0; y01 &= mk1; y23 &= mk1; }
+            mma_f16(o[4 * i], pw, e4m3x2_f16x2((uint16_t)x01), e4m3x2_f16x2((uint16_t)y01));
+            mma_f16(o[4 * i + 1], pw, e4m3x2_f16x2((uint16_t)(x01 >> 16)), e4m3x2_f16x2((uint16_t)(y01 >> 16)));
+            mma_f16(o[4 * i + 2], pw, e4m3x2_f16x2((uint16_t)x23), e4m3x2_f16x2((uint16_t)y23));
+            mma_f16(o[4 * i + 3], pw, e4m3x2_f16x2((uint16_t)(x23 >> 16)), e4m3x2_f16x2((uint16_t)(y23 >> 16)));
+        }
+    }
+
+    __device__ __forceinline__ static float quad_sum(float x) {
+        x += __shfl_xor_sync(0xffffffffu, x, 1);
+        return x + __shfl_xor_sync(0xffffffffu, x, 2);
+    }
+    // this warp's state of the rows < R_rows into the CTA's merge scratch: [R][D + 2] floats = acc | m | l
+    // (all 32 lanes call it; acc in true units, dims in their natural order)
+    __device__ __forceinline__ void to_scratch(float* scratch, int32_t R_rows, int32_t lane) const {
+        const float la = quad_sum(lsum[0]), lb = quad_sum(lsum[2]);
+        const float vu = vref * (1.f / 32768.f);
+        const int32_t ra = lane >> 2, d0 = (lane & 3) * (D / 4);
+        const bool wa = ra < R_rows, wb = ra + 8 < R_rows;
+#pragma unroll
+        for (int n = 0; n < NT; n += 2) {
+            if (wa) {
+                *reinterpret_cast<float2*>(scratch + ra * (D + 2) + d0 + n) = make_float2(o[n][0] * vu, o[n + 1][0] * vu);
+                *reinterpret_cast<float2*>(scratch + ra * (D + 2) + d0 + NT + n) = make_float2(o[n][1] * vu, o[n + 1][1] * vu);
+            }
+            if (wb) {
+                *reinterpret_cast<float2*>(scratch + (ra + 8) * (D + 2) + d0 + n) = make_float2(o[n][2] * vu, o[n + 1][2] * vu);
+                *reinterpret_cast<float2*>(scratch + (ra + 8) * (D + 2) + d0 + NT + n) = make_float2(o[n][3] * vu, o[n + 1][3] * vu);
+            }
+        }
+        if ((lane & 3) == 0) {
+            if (wa) { scratch[ra * (D + 2) + D] = m_a; scratch[ra * (D + 2) + D + 1] = la; }
+            if (wb) { scratch[(ra + 8) * (D + 2) + D] = m_b; scratch[(ra + 8) * (D + 2) + D + 1] = lb; }
+        }
+    }
+};
+
 // logical block and first token position of tile `tile` of an item (sinks first, then the window)
 template <typename Item>
 __device__ __forceinline__ int32_t tile_block(const Item& it, int32_t tile) {
@@ -252,16 +538,21 @@ __device__ __forceinline__ int32_t tile_block(const Item& it, int32_t tile) {
 
 // ================================================================================================
 // GQA decode (R <= 16): stream-K partition of the flattened (item, KV head, tile) list.
-template <int D>
+template <int D, bool FP8>
 struct GqaCfg {
     static constexpr int NWARP = 4;
-    static constexpr int NS = 2;                        // private stages per warp, one 16-key tile each
-    static constexpr int kHeadBytes = 2 * kBlockTokens * D * 2;
+    // private stages per warp, one 16-key tile each (fp8 tiles are half the bytes: twice the stages keep the same
+    // number of bytes in flight)
+    static constexpr int NS = FP8 ? 4 : 2;
+    static constexpr int kPre = NS - 1;                 // the stage that takes the NEXT pair's first tile during a merge
+    static constexpr int kTileBytes = kBlockTokens * D * (FP8 ? 1 : 2);                   // K (or V) of one block-head
+    static constexpr int kHeadBytes = 2 * kTileBytes + (FP8 ? 2 * kBlockTokens * 4 : 0);   // = KvLayout::head_bytes
     static constexpr int kWarpBytes = NS * kHeadBytes;
     static constexpr int kSmemBytes = NWARP * kWarpBytes + NWARP * NS * 8 + 128;
     static constexpr int kThreads = 32 * NWARP;
     // the merge of the 4 warps reuses the rings: 16 rows x (D + 2) floats per warp must fit
     static_assert(16 * (D + 2) * 4 <= kWarpBytes, "merge scratch does not fit a warp's ring");
+    static_assert(kHeadBytes % 128 == 0, "stages stay 128-byte aligned");
 };
 
 // The flattened tile list [0, total_tiles) is cut into RANGES in two regimes:
@@ -332,10 +623,11 @@ __host__ __device__ inline GqaPiece gqa_piece(const GqaPlan& plan, int32_t i, in
 }
 
 // grid = n_SM * CTAs/SM (<= total tiles), block = 128.  items[].tile_off = exclusive prefix of n_tiles.
-template <int D>
-__global__ void __launch_bounds__(GqaCfg<D>::kThreads)
+template <int D, bool FP8>
+__global__ void __launch_bounds__(GqaCfg<D, FP8>::kThreads)
 attend_gqa_kernel(AttendParams p, GqaPlan plan) {
-    using C = GqaCfg<D>;
+    using C = GqaCfg<D, FP8>;
+    using Tile = typename std::conditional<FP8, WarpTileF8<D>, WarpTile<D>>::type;
     if (p.pdl_early) pdl_launch_dependents();
     if (threadIdx.x == 0) stamp_begin(p);
     pdl_wait();                  // the work list and this step's K/V rows come from the append kernel
@@ -373,7 +665,7 @@ attend_gqa_kernel(AttendParams p, GqaPlan plan) {
         }
         i = lo;
     }
-    int32_t pre = 0;        // 1: the first tile of the coming pair is already in flight, in stage 1
+    int32_t pre = 0;        // 1: the first tile of the coming pair is already in flight, in stage kPre
     while (g < g_end) {
         // ---- the (item, head) pair that holds unit g, and this CTA's piece of it: tiles [a, b) ----
         const AttendItem it = p.items[i];
@@ -388,7 +680,7 @@ attend_gqa_kernel(AttendParams p, GqaPlan plan) {
         const uint8_t* head_base = p.kv_layer + (int64_t)kvh * p.L.head_bytes;
         // this warp's tiles: a + warp, a + warp + 4, ...   (private ring, prologue fills NS stages)
         const int32_t n_mine = (b - a - warp + C::NWARP - 1) / C::NWARP;
-        const int32_t sbase = pre;         // k-th tile of this warp -> stage (k + sbase) % NS
+        const int32_t sbase = pre ? C::kPre : 0;   // k-th tile of this warp -> stage (k + sbase) % NS
         auto issue = [&](int32_t k) {
             if (lane == 0) {
                 const int32_t tile = a + warp + k * C::NWARP;
@@ -400,7 +692,7 @@ attend_gqa_kernel(AttendParams p, GqaPlan plan) {
             }
         };
         for (int32_t k = pre; k < min(n_mine, C::NS); ++k) issue(k);
-        WarpTile<D> wt;                                   // (Q rows are fetched while the first tiles fly)
+        Tile wt;                                          // (Q rows are fetched while the first tiles fly)
         wt.init(p, it, kvh, 0, lane);
         for (int32_t k = 0; k < n_mine; ++k) {
             const int32_t st = (k + sbase) % C::NS;
@@ -408,16 +700,16 @@ attend_gqa_kernel(AttendParams p, GqaPlan plan) {
             phase_bits ^= 1u << st;
             const int32_t p0 = tile_block(it, a + warp + k * C::NWARP) * kBlockTokens;
             const uint32_t kt = ring + st * C::kHeadBytes;
-            if (!wt.skips(p, p0)) wt.template step<256>(p, it.len, kt, kt + kBlockTokens * D * 2, p0, lane);
+            if (!wt.skips(p, p0)) wt.template step<256>(p, it.len, kt, kt + C::kTileBytes, p0, lane);
             __syncwarp();                                  // every lane is done reading the stage
             if (k + C::NS < n_mine) issue(k + C::NS);
         }
         // ---- while the warps are merged below, the first tile of the NEXT pair of this range is
-        // already on its way: the merge scratch of R <= 15 rows fits the warp's stage 0, so stage 1
+        // already on its way: when the merge scratch of the R rows fits the stages below kPre, stage kPre
         // takes that tile now (saves the table -> HBM round trip after every (item, head) boundary) ----
         const int32_t R_rows = it.q_len * p.G;
         pre = 0;
-        if (R_rows * (D + 2) * 4 <= C::kHeadBytes && b == it.n_tiles && pair_lo + b + bnd < g_end) {
+        if (R_rows * (D + 2) * 4 <= C::kPre * C::kHeadBytes && b == it.n_tiles && pair_lo + b + bnd < g_end) {
             const bool same = kvh + 1 < Hkv;
             const int32_t i2 = same ? i : i + 1;
             const int32_t sid2 = same ? it.sid : p.items[i2].sid;
@@ -429,9 +721,9 @@ attend_gqa_kernel(AttendParams p, GqaPlan plan) {
                 if (lane == 0) {
                     const int32_t blk = warp < sink2 ? warp : first2 + (warp - sink2);
                     const int32_t phys = __ldg(p.table + (int64_t)sid2 * p.tbl_width + table_slot(blk, p.n_sink, p.ring));
-                    const uint32_t bar = bars + 8;
+                    const uint32_t bar = bars + 8 * C::kPre;
                     mbar_expect_tx(bar, C::kHeadBytes);
-                    bulk_g2s(ring + C::kHeadBytes,
+                    bulk_g2s(ring + C::kPre * C::kHeadBytes,
                              p.kv_layer + (int64_t)phys * p.L.block_bytes + (int64_t)(same ? kvh + 1 : 0) * p.L.head_bytes,
                              C::kHeadBytes, bar);
                 }
@@ -440,20 +732,7 @@ attend_gqa_kernel(AttendParams p, GqaPlan plan) {
         }
         // ---- merge the four warps through shared memory (their rings are idle now) ----
         __syncthreads();
-        float* scratch = reinterpret_cast<float*>(smem_gen + warp * C::kWarpBytes);   // [R][D + 2], rows < R only
-        {
-            const int32_t ra = lane >> 2, c = (lane & 3) * 2;
-            const bool wa = ra < R_rows, wb = ra + 8 < R_rows;
-#pragma unroll
-            for (int n = 0; n < WarpTile<D>::NT; ++n) {
-                if (wa) *reinterpret_cast<float2*>(scratch + ra * (D + 2) + n * 8 + c) = make_float2(wt.o[n][0], wt.o[n][1]);
-                if (wb) *reinterpret_cast<float2*>(scratch + (ra + 8) * (D + 2) + n * 8 + c) = make_float2(wt.o[n][2], wt.o[n][3]);
-            }
-            if ((lane & 3) == 0) {
-                if (wa) { scratch[ra * (D + 2) + D] = wt.m_a; scratch[ra * (D + 2) + D + 1] = wt.lsum[0]; }
-                if (wb) { scratch[(ra + 8) * (D + 2) + D] = wt.m_b; scratch[(ra + 8) * (D + 2) + D + 1] = wt.lsum[2]; }
-            }
-        }
+        wt.to_scratch(reinterpret_cast<float*>(smem_gen + warp * C::kWarpBytes), R_rows, lane);   // [R][D + 2], rows < R only
         __syncthreads();
         {
             // 128 threads: row = tid / 8 (16 rows), 8 threads x (D/8) consecutive dims each
@@ -561,16 +840,24 @@ attend_gqa_kernel(AttendParams p, GqaPlan plan) {
 // ------------------------------------------------------------------------------------------------
 inline cudaError_t configure_attend_mma_kernels() {
     cudaError_t e;
-    if ((e = cudaFuncSetAttribute(attend_gqa_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  GqaCfg<128>::kSmemBytes)) != cudaSuccess) return e;
-    return cudaFuncSetAttribute(attend_gqa_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                GqaCfg<64>::kSmemBytes);
+    if ((e = cudaFuncSetAttribute(attend_gqa_kernel<128, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  GqaCfg<128, false>::kSmemBytes)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(attend_gqa_kernel<64, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  GqaCfg<64, false>::kSmemBytes)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(attend_gqa_kernel<128, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  GqaCfg<128, true>::kSmemBytes)) != cudaSuccess) return e;
+    return cudaFuncSetAttribute(attend_gqa_kernel<64, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                GqaCfg<64, true>::kSmemBytes);
 }
 
-// decode-class items (R <= 16)
+// decode-class items (R <= 16); `fp8`: the pool holds E4M3 codes + row scales (KvLayout::fp8)
 inline cudaError_t launch_attend_gqa(const AttendParams& p, const GqaPlan& plan, int32_t D, int32_t n_ctas, cudaStream_t st,
                                      bool pdl = false) {
-    if (D == 128) return launch_kernel(attend_gqa_kernel<128>, dim3(n_ctas), GqaCfg<128>::kThreads, GqaCfg<128>::kSmemBytes, st, pdl, p, plan);
-    return launch_kernel(attend_gqa_kernel<64>, dim3(n_ctas), GqaCfg<64>::kThreads, GqaCfg<64>::kSmemBytes, st, pdl, p, plan);
+    if (p.L.fp8) {
+        if (D == 128) return launch_kernel(attend_gqa_kernel<128, true>, dim3(n_ctas), GqaCfg<128, true>::kThreads, GqaCfg<128, true>::kSmemBytes, st, pdl, p, plan);
+        return launch_kernel(attend_gqa_kernel<64, true>, dim3(n_ctas), GqaCfg<64, true>::kThreads, GqaCfg<64, true>::kSmemBytes, st, pdl, p, plan);
+    }
+    if (D == 128) return launch_kernel(attend_gqa_kernel<128, false>, dim3(n_ctas), GqaCfg<128, false>::kThreads, GqaCfg<128, false>::kSmemBytes, st, pdl, p, plan);
+    return launch_kernel(attend_gqa_kernel<64, false>, dim3(n_ctas), GqaCfg<64, false>::kThreads, GqaCfg<64, false>::kSmemBytes, st, pdl, p, plan);
 }
 }  // namespace metronome

@@ -114,7 +114,7 @@ attend_rows_kernel(AttendParams p) {
     };
     Chunk kr[STEPS], vr[STEPS];
     float ks[FP8 ? STEPS : 1], vs[FP8 ? STEPS : 1];                 // fp8: the rows' scales
-    auto chunk_off = [&](int32_t row) { return FP8 ? row * D + sub * 8 : tile_chunk_offset(row, sub); };
+    auto chunk_off = [&](int32_t row) { return FP8 ? fp8_unit_offset(D, row, sub) : tile_chunk_offset(row, sub); };
     auto load_k = [&](const uint8_t* kt) {
 #pragma unroll
         for (int j = 0; j < STEPS; ++j) {

@@ -201,8 +201,9 @@ append_fused_kernel(const AppendParams a) {
         // (the chunks_per_row threads of a row are consecutive lanes of one warp, all active or all not)
         const uint2 kq = quantize_chunk_e4m3(kk, chunks_per_row, c == 0 ? reinterpret_cast<float*>(tile + 2 * a.L.tile_bytes) + r : nullptr);
         const uint2 vq = quantize_chunk_e4m3(vv, chunks_per_row, c == 0 ? reinterpret_cast<float*>(tile + 2 * a.L.tile_bytes) + kBlockTokens + r : nullptr);
-        *reinterpret_cast<uint2*>(tile + r * a.L.head_dim + c * 8) = kq;
-        *reinterpret_cast<uint2*>(tile + a.L.tile_bytes + r * a.L.head_dim + c * 8) = vq;
+        const int32_t off8 = fp8_unit_offset(a.L.head_dim, r, c);
+        *reinterpret_cast<uint2*>(tile + off8) = kq;
+        *reinterpret_cast<uint2*>(tile + a.L.tile_bytes + off8) = vq;
         return;
     }
     const int32_t off = tile_chunk_offset(r, c);
@@ -261,8 +262,9 @@ kv_read_fp8_kernel(const int32_t* __restrict__ row, int32_t n_sink, int32_t ring
         const int32_t phys = row[table_slot(blk, n_sink, ring)];
         const uint8_t* tile = kv_layer + (int64_t)phys * L.block_bytes + (int64_t)h * L.head_bytes;
         const float* scales = reinterpret_cast<const float*>(tile + 2 * L.tile_bytes);
-        dequant8_e4m3(*reinterpret_cast<const uint2*>(tile + r * L.head_dim + c * 8), scales[r], kf);
-        dequant8_e4m3(*reinterpret_cast<const uint2*>(tile + L.tile_bytes + r * L.head_dim + c * 8), scales[kBlockTokens + r], vf);
+        const int32_t off8 = fp8_unit_offset(L.head_dim, r, c);
+        dequant8_e4m3(*reinterpret_cast<const uint2*>(tile + off8), scales[r], kf);
+        dequant8_e4m3(*reinterpret_cast<const uint2*>(tile + L.tile_bytes + off8), scales[kBlockTokens + r], vf);
     }
 #pragma unroll
     for (int k = 0; k < 8; ++k) { k_out[(int64_t)idx * 8 + k] = kf[k]; v_out[(int64_t)idx * 8 + k] = vf[k]; }

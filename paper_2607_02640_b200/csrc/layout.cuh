@@ -30,9 +30,10 @@ struct KvLayout {
     int64_t layer_bytes;    // n_blocks * block_bytes
 };
 
-// fp8 layout of one (block, kv head):  [K codes 16 x D bytes, linear][V codes 16 x D][K scales 16 f32][V scales 16 f32]
-// (NEXT row f4, "the two compose"; quantiser: DESIGN.md reading R18).  Only the CUDA-core row kernel
-// reads it, so the rows are not swizzled.
+// fp8 layout of one (block, kv head):  [K codes 16 x D bytes][V codes 16 x D][K scales 16 f32][V scales 16 f32]
+// (NEXT row f4, "the two compose"; quantiser: DESIGN.md reading R18).  The 16-byte chunks of a code tile
+// are XOR-swizzled inside 128-byte lines (fp8_chunk_offset) so that `ldmatrix` and the 16-byte V-row loads of the GQA
+// decode kernel are conflict-free after a LINEAR copy HBM -> shared memory, as for the bf16 tiles.
 __host__ __device__ inline KvLayout make_layout(int32_t D, int32_t Hkv, int64_t n_blocks, bool fp8 = false) {
     KvLayout L;
     L.head_dim = D;
@@ -48,6 +49,19 @@ __host__ __device__ inline KvLayout make_layout(int32_t D, int32_t Hkv, int64_t 
 // Byte offset, inside a K or V tile, of 16-byte chunk `c` (0 .. D/8-1) of token row `r` (0..15).
 __host__ __device__ __forceinline__ int32_t tile_chunk_offset(int32_t r, int32_t c) {
     return ((c >> 3) * (kBlockTokens * 128)) + r * 128 + (((c & 7) ^ (r & 7)) << 4);
+}
+
+// fp8 KV: byte offset, inside a K or V code tile (16 rows x D bytes), of 16-byte chunk `c` (0 .. D/16-1) of token row
+// `r`.  The tile is a sequence of 128-byte lines (one row at D = 128, two rows at D = 64); chunk position p of line l is
+// stored at p ^ (l & 7).
+__host__ __device__ __forceinline__ int32_t fp8_chunk_offset(int32_t D, int32_t r, int32_t c) {
+    const int32_t q = r * (D >> 4) + c;
+    const int32_t line = q >> 3;
+    return line * 128 + (((q & 7) ^ (line & 7)) << 4);
+}
+// ... of the 8-byte unit `u` (8 codes, 0 .. D/8-1) of token row `r`
+__host__ __device__ __forceinline__ int32_t fp8_unit_offset(int32_t D, int32_t r, int32_t u) {
+    return fp8_chunk_offset(D, r, u >> 1) + ((u & 1) << 3);
 }
 
 // Slot of logical block `b` in a session's block table: the first n_sink entries are the pinned

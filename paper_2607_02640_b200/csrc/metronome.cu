@@ -314,8 +314,10 @@ int plan_attend(metronome_pool* pool, int32_t n_batch, const int32_t* sids, cons
     }
     int family = pool->tune_family;
     if (family == 0) family = (pool->G * max_q >= 4) ? 2 : 1;
-    if (pool->fp8) family = 1;        // fp8 KV rows are read by the CUDA-core row kernel only (NEXT row f4)
-    if (family == 2 && !attend_umma_supported(pool->G, max_q))
+    // fp8 KV (NEXT row f4): decode-class items go to the GQA decode kernel's fp8 tile, chunk-class items to the
+    // CUDA-core row kernel (the tcgen05 chunk kernel reads bf16 tiles only)
+    const bool rows_chunks = pool->fp8;
+    if (family == 2 && !rows_chunks && !attend_umma_supported(pool->G, max_q))
         family = 1;
     pl.family = family;
 
@@ -373,7 +375,7 @@ int plan_attend(metronome_pool* pool, int32_t n_batch, const int32_t* sids, cons
             cls_tiles[cls] += its[i].n_tiles;
             pl.cls_rows[cls] += its[i].q_len;
             if (its[i].q_len > pl.cls_max_q[cls]) pl.cls_max_q[cls] = its[i].q_len;
-            units += (int64_t)its[i].n_tiles * (family == 2 ? c.n_kv_heads : c.n_q_heads * its[i].q_len);
+            units += (int64_t)its[i].n_tiles * (family == 2 && !rows_chunks ? c.n_kv_heads : c.n_q_heads * its[i].q_len);
         }
         if (family == 2 && cls == 0) {
             // stream-K: one wave of n_SM x 3 CTAs, equal static ranges (one per CTA); for long shares the
@@ -391,7 +393,7 @@ int plan_attend(metronome_pool* pool, int32_t n_batch, const int32_t* sids, cons
                                  (pool->tune_gqa_dynamic == 0 && pool->tune_split_tokens <= 0 && (total_tiles + ctas - 1) / ctas >= 512);
             // ranges are cut in cost units: a pair's tiles + what starting a pair costs (make_gqa_plan), the latter
             // ~4 us of one CTA's share of the stream = METRONOME_GQA_BND_BYTES of K/V tiles
-            const int32_t bnd = (int32_t)(METRONOME_GQA_BND_BYTES / (2 * kBlockTokens * c.head_dim * 2));
+            const int32_t bnd = (int32_t)(METRONOME_GQA_BND_BYTES / pool->L.head_bytes);
             pl.gplan = make_gqa_plan(c.n_kv_heads, (cls_tiles[0] + (int64_t)bnd * n) * c.n_kv_heads, ctas, dynamic, bnd);
             GqaPlan& g = pl.gplan;
             pl.gqa_ctas = g.n_static;
@@ -412,7 +414,7 @@ int plan_attend(metronome_pool* pool, int32_t n_batch, const int32_t* sids, cons
             }
             // The fused decode step (step_gqa.cuh): one contiguous range per WARP of a single wave (CTA 0 of
             // that kernel does the bookkeeping), at least 8 tiles each; the work list in 16 bytes per item.
-            if (step_items && n_cls[1] == 0 && n <= kStepMaxItems && c.n_kv_heads <= 255 && pool->tune_fused_step == 2) {
+            if (step_items && n_cls[1] == 0 && n <= kStepMaxItems && c.n_kv_heads <= 255 && pool->tune_fused_step == 2 && !pool->fp8) {
                 // One contiguous range per warp of a single wave (minus the bookkeeping CTA), at least 8 tiles each:
                 // long ranges for the warps on fast SMs, ranges shorter by the measured speed ratio for those on slow SMs.
                 const int32_t wps = step_workers_per_sm(pool->G * pl.cls_max_q[0]);
@@ -449,11 +451,12 @@ int plan_attend(metronome_pool* pool, int32_t n_batch, const int32_t* sids, cons
             continue;
         }
         // segments sized for >= 2 waves of CTAs, each with a useful run of tiles
-        const int64_t target_ctas = (int64_t)pool->n_sm * (family == 2 ? 4 : 16);
+        const bool umma_cls = family == 2 && !rows_chunks;
+        const int64_t target_ctas = (int64_t)pool->n_sm * (umma_cls ? 4 : 16);
         int32_t tps = pool->tune_split_tokens > 0 ? (pool->tune_split_tokens + kBlockTokens - 1) / kBlockTokens
                                                   : (int32_t)((units + target_ctas - 1) / target_ctas);
         if (pool->tune_split_tokens <= 0 && tps < 8) tps = 8;
-        if (family == 2 && pool->tune_split_tokens <= 0) {
+        if (umma_cls && pool->tune_split_tokens <= 0) {
             // tcgen05 chunk kernel, one CTA per SM: whole (item, head) pairs when they alone give
             // >= 3 CTAs per SM (no partials to merge), else whole 128-key stages, >= 4 per segment
             if ((int64_t)n * c.n_kv_heads >= 3 * (int64_t)pool->n_sm) tps = INT32_MAX / 2;
@@ -545,7 +548,8 @@ int launch_attend(metronome_pool* pool, int32_t layer, const AttendPlan& pl, con
         CU(cudaEventRecord(pool->prof_ev[pool->prof_used], st));
         pdl = false;
     }
-    const bool publish = pl.family == 2 && pdl && !pool->profiling && !pool->poison;
+    // (the row kernel, which takes an fp8 pool's chunk-class items, does not publish)
+    const bool publish = pl.family == 2 && pdl && !pool->profiling && !pool->poison && (!pool->fp8 || pl.n_cls[0] > 0);
     if (publish) { p.pastwait_flag = pool->d_bk_flag + 12; p.pastwait_epoch = (int32_t)pool->epoch; }
     if (pl.family == 2) {
         if (pl.n_cls[0] > 0) {
@@ -556,8 +560,15 @@ int launch_attend(metronome_pool* pool, int32_t layer, const AttendPlan& pl, con
         }
         if (pl.n_cls[1] > 0) {
             p.items = d_items + pl.n_cls[0]; p.n_items = pl.n_cls[1];
-            p.stamp = next_stamp(pool, 3);
-            CU(launch_attend_umma(p, c.head_dim, c.n_kv_heads, pl.total_splits[1], st, pdl));
+            if (pool->fp8) {
+                dim3 grid(c.n_q_heads, pl.total_splits[1], pl.cls_max_q[1]);
+                p.stamp = next_stamp(pool, 1);
+                if (c.head_dim == 128) CU(launch_kernel(attend_rows_kernel<128, true>, grid, dim3(128), 0, st, pdl, p));
+                else CU(launch_kernel(attend_rows_kernel<64, true>, grid, dim3(128), 0, st, pdl, p));
+            } else {
+                p.stamp = next_stamp(pool, 3);
+                CU(launch_attend_umma(p, c.head_dim, c.n_kv_heads, pl.total_splits[1], st, pdl));
+            }
             ++pool->n_launch;
         }
     } else {

@@ -25,12 +25,13 @@ def _bf16(rng, n, H, D, scale=1.0):
     return torch.from_numpy((rng.standard_normal((n, H, D)) * scale).astype(np.float32)).to(torch.bfloat16)
 
 
-def _make(S, W, Hq, Hkv, D, N, n_max, split_tokens=0, extra_flags=0):
+def _make(S, W, Hq, Hkv, D, N, n_max, split_tokens=0, extra_flags=0, scale=None):
     per = -(-S // 16) + (W + n_max - 1) // 16 + 2
     kw = dict(n_q_heads=Hq, n_kv_heads=Hkv, head_dim=D, max_sessions=N, max_new_tokens=n_max)
-    pool = binding.Pool(n_sinks=S, window=W, n_blocks=N * per, flags=binding.FLAG_KV_FP8 | extra_flags, **kw)
+    pool = binding.Pool(n_sinks=S, window=W, n_blocks=N * per, flags=binding.FLAG_KV_FP8 | extra_flags,
+                        softmax_scale=scale or 0.0, **kw)
     pool.set_tuning(split_tokens, 0)
-    cfg = O.PoolConfig(S=S, W=W, n_blocks=N * per, block_size=16, kv_fp8=True, **kw)
+    cfg = O.PoolConfig(S=S, W=W, n_blocks=N * per, block_size=16, kv_fp8=True, scale=scale, **kw)
     return pool, O.DefinitionOracle(cfg), O.PagedOracle(cfg, store_kv=False)
 
 
@@ -125,3 +126,40 @@ def test_fp8_with_poisoned_frees_and_two_layers():
             defn.append_kv(layer, [sids[i] for i in due], [int(x) for x in n_new], synth.to_u16(k), synth.to_u16(v))
             ref = defn.attend_frame(layer, [sids[i] for i in due], [int(x) for x in n_new], synth.to_u16(q))
             assert_parity(out, ref, f"fp8 poison step {step} layer {layer}")
+
+
+@pytest.mark.parametrize("qmag", ["mixed", "huge"])
+@pytest.mark.parametrize("G,D", [(4, 128), (8, 128), (4, 64)])
+def test_fp8_gqa_decode_with_rows_of_very_different_magnitude(G, D, qmag):
+    """The GQA decode kernel's fp8 tile never applies a scale to a tensor-core operand: K scales multiply the finished
+    dot products, V scales are folded into the softmax weights relative to a running reference that is raised (and
+    the accumulator rescaled) when a larger scale arrives, and the query row is brought into fp16 range by a power of
+    two.  Here the rows' magnitudes span 1e-3 .. 1e2 for V (log-uniform per row, so the reference is raised many times,
+    also across split pieces) and {1e-3, 3e-2, 1} for K; Q rows are x {1e-2, 1, 300} ("mixed": flat to one-hot softmax
+    rows) or x {2.5e5, 1e6} with a softmax scale of 1e-6 / sqrt(D) ("huge": far outside fp16 range).  Freed blocks are
+    NaN-poisoned, S = 17 gives a partly filled second sink block, split-KV pieces of 64 tokens."""
+    Hkv, S, W, N = 2, 17, 150, 3
+    Hq = Hkv * G
+    scale = 1e-6 / np.sqrt(D) if qmag == "huge" else None
+    pool, defn, book = _make(S, W, Hq, Hkv, D, N, 4, split_tokens=64, extra_flags=binding.FLAG_POISON_ON_FREE, scale=scale)
+    sids = [pool.session_open() for _ in range(N)]
+    assert sids == [defn.session_open() for _ in range(N)] == [book.session_open() for _ in range(N)]
+    rng = np.random.default_rng(77 + G + D)
+
+    def mag(choices, shape):
+        return torch.from_numpy(np.asarray(choices, np.float32)[rng.integers(0, len(choices), size=shape)]).to(torch.bfloat16)
+
+    for step in range(260):
+        n_new = np.ones(N, np.int32) if step % 7 else rng.integers(1, 3, size=N).astype(np.int32)
+        rows = int(n_new.sum())
+        k = _bf16(rng, rows, Hkv, D) * mag([1e-3, 3e-2, 1.0], (rows, Hkv, 1))
+        v = _bf16(rng, rows, Hkv, D) * torch.from_numpy((10.0 ** rng.uniform(-3, 2, size=(rows, Hkv, 1))).astype(np.float32)).to(torch.bfloat16)
+        q = _bf16(rng, rows, Hq, D) * mag([2.5e5, 1e6] if qmag == "huge" else [1e-2, 1.0, 300.0], (rows, Hq, 1))
+        out = torch.empty_like(q, device="cuda")
+        pool.append_attend(0, sids, n_new, k.cuda(), v.cuda(), q.cuda(), out)
+        defn.append_kv(0, sids, [int(x) for x in n_new], synth.to_u16(k), synth.to_u16(v))
+        book.append_kv(0, sids, [int(x) for x in n_new])
+        ref = defn.attend_frame(0, sids, [int(x) for x in n_new], synth.to_u16(q))
+        assert_parity(out, ref, f"fp8 magnitudes G={G} D={D} {qmag} step {step}", unit_scale=False)
+    assert min(defn.length.values()) > S + W
+    assert pool.pool_query()[1] == book.pool_query()

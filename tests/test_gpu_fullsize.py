@@ -13,7 +13,8 @@ import pytest
 import torch
 
 from oracle import bounded_kv as O
-from paper_2607_02640_b200 import synth
+from oracle import kv_fp8 as F
+from paper_2607_02640_b200 import binding, synth
 from paper_2607_02640_b200 import workloads as wl
 from paper_2607_02640_b200.runner import Runner
 from parity_helpers import assert_parity, oracle_cfg
@@ -21,9 +22,9 @@ from parity_helpers import assert_parity, oracle_cfg
 pytestmark = pytest.mark.gpu
 
 
-def _reference_rows(r, w, local, n, layer=0):
+def _reference_rows(r, w, local, n, layer=0, kv_fp8=False):
     """oracle output for the last n rows of workload-local session `local` (definition layer on the
-    rows that can be admitted)."""
+    rows that can be admitted; kv_fp8: on what their stored fp8 form decodes to, oracle/kv_fp8.py)."""
     L = r.length[local]
     lo = max(0, L - n - w.W + 1)
     pos = np.concatenate([np.arange(0, min(w.S, lo)), np.arange(lo, L)]).astype(np.int64)
@@ -32,13 +33,15 @@ def _reference_rows(r, w, local, n, layer=0):
     v = synth.to_u16(r.rows(synth.STREAM_V, layer, uid, pos, device="cpu"))
     qpos = np.arange(L - n, L, dtype=np.int64)
     q = synth.to_u16(r.rows(synth.STREAM_Q, layer, np.full(n, r.uid[local], np.int64), qpos, device="cpu"))
+    if kv_fp8:
+        k, v = F.roundtrip(k), F.roundtrip(v)
     return O.attend(q, qpos, k, v, pos, w.S, w.W, None, "f32", False, O.max_threads())
 
 
-def _run_fullsize(index, n_frames, n_sample, history_scale=1.0, n_sessions=None):
+def _run_fullsize(index, n_frames, n_sample, history_scale=1.0, n_sessions=None, kv_fp8=False):
     w = wl.make_workload(index, n_sessions=n_sessions, n_timed_frames=n_frames)
     events, _ = wl.build_schedule(w, history_scale=history_scale)
-    r = Runner(w)
+    r = Runner(w, flags=binding.FLAG_KV_FP8 if kv_fp8 else 0)
     book = O.PagedOracle(oracle_cfg(w), store_kv=False)          # bookkeeping-only replay
     osid = {}
     rng = np.random.default_rng(w.seed + 5)
@@ -74,7 +77,7 @@ def _run_fullsize(index, n_frames, n_sample, history_scale=1.0, n_sessions=None)
         offs = np.concatenate([[0], np.cumsum(st.n_new)])
         for j in sorted(pick):
             n = int(st.n_new[j])
-            ref = _reference_rows(r, w, int(st.local[j]), n)
+            ref = _reference_rows(r, w, int(st.local[j]), n, kv_fp8=kv_fp8)
             rep = assert_parity(out[offs[j]:offs[j] + n], ref, f"{w.name} frame {st.frame} session {st.local[j]} len {lens[j]}",
                                 unit_scale=w.outlier_frac == 0)
             checked_rows += n
@@ -89,7 +92,7 @@ def _run_fullsize(index, n_frames, n_sample, history_scale=1.0, n_sessions=None)
         assert (got[0], got[1], got[2]) == (want[0], want[1], want[2]), i
         resident += len(got[2])
     assert n_free + resident == w.n_blocks
-    print(f"config {index}: {checked_rows} sampled rows x {w.n_q_heads} heads, worst {worst}")
+    print(f"config {index}{' fp8 KV' if kv_fp8 else ''}: {checked_rows} sampled rows x {w.n_q_heads} heads, worst {worst}")
     return worst
 
 
@@ -114,3 +117,20 @@ def test_config5_churn_sampled():
     the timed frames.  A CTA's share of the GQA decode kernel is >= 512 tiles here, so this is also the
     launch configuration that takes the dynamically claimed tail ranges by itself."""
     _run_fullsize(5, n_frames=3, n_sample=2)
+
+
+def test_config3_fp8_full_size_sampled():
+    """configs[2] on an fp8 (E4M3) KV pool (NEXT row f4, "the two compose"): the 8 decode steps of the
+    frame run on the GQA decode kernel's fp8 tile, the 25-token chunk on the row kernel."""
+    _run_fullsize(3, n_frames=1, n_sample=3, kv_fp8=True)
+
+
+def test_config4_fp8_full_size_sampled():
+    """configs[3] on an fp8 KV pool: the x20 outlier channels give rows whose scales differ by 20x inside one tile
+    (the V scale is folded into the softmax weight relative to a running reference)."""
+    _run_fullsize(4, n_frames=1, n_sample=2, kv_fp8=True)
+
+
+def test_config5_fp8_churn_sampled():
+    """configs[4] on an fp8 KV pool: the dynamically claimed tail ranges of the GQA decode kernel with fp8 tiles."""
+    _run_fullsize(5, n_frames=2, n_sample=2, kv_fp8=True)

@@ -18,21 +18,22 @@ def _rows(rng, n, H, D):
     return torch.from_numpy(rng.standard_normal((n, H, D)).astype(np.float32)).to(torch.bfloat16)
 
 
+@pytest.mark.parametrize("kv_fp8", [False, True])
 @pytest.mark.parametrize("split_tokens", [0, 1024, 4096])
-def test_gqa_decode_with_dynamic_ranges_forced(split_tokens):
+def test_gqa_decode_with_dynamic_ranges_forced(split_tokens, kv_fp8):
     """attend_gqa_kernel's dynamic regime (the last ~10 % of the flattened tile list is cut into small
     ranges that CTAs claim with an atomic counter; the last CTA out resets the counters) is enabled by
     itself only when a CTA's share is >= 512 tiles, i.e. on full config 5.  Here it is FORCED on a small
     GQA-8 workload (split_tokens sets the static share: 64 / 256 tiles; 0 = the automatic one-wave cut),
     for 12 consecutive launches with no host sync in between: every output against the oracle, and the
     claim / exit counters back to zero after the launches (a stale counter would make the next launch skip
-    or repeat ranges)."""
+    or repeat ranges).  kv_fp8: the same through the kernel's fp8 tile (four private stages per warp instead of two)."""
     Hq, Hkv, D, S, W, N, n_max = 32, 4, 128, 4, 2048, 6, 25
     per = 1 + (W + n_max - 1) // 16 + 2
     kw = dict(n_q_heads=Hq, n_kv_heads=Hkv, head_dim=D, max_sessions=N, max_new_tokens=n_max)
-    pool = binding.Pool(n_sinks=S, window=W, n_blocks=N * per, **kw)
+    pool = binding.Pool(n_sinks=S, window=W, n_blocks=N * per, flags=binding.FLAG_KV_FP8 if kv_fp8 else 0, **kw)
     pool.set_tuning(split_tokens, 2, 1)
-    ora = O.DefinitionOracle(O.PoolConfig(S=S, W=W, n_blocks=N * per, block_size=16, **kw))
+    ora = O.DefinitionOracle(O.PoolConfig(S=S, W=W, n_blocks=N * per, block_size=16, kv_fp8=kv_fp8, **kw))
     sids = [pool.session_open() for _ in range(N)]
     assert sids == [ora.session_open() for _ in range(N)]
     rng = np.random.default_rng(4242 + split_tokens)
