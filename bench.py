@@ -161,7 +161,7 @@ def launch_classes(w, n_new, family):
     n_new = np.asarray(n_new)
     G = w.n_q_heads // w.n_kv_heads
     fam = family or (2 if G * int(n_new.max()) >= 4 else 1)
-    if fam == 2 and G * int(n_new.max()) > 256 and not KV_FP8:
+    if fam == 2 and G * int(n_new.max()) > 256:
         fam = 1
     if fam == 1:
         return [(1, n_new > 0)]
@@ -171,7 +171,7 @@ def launch_classes(w, n_new, family):
     if dec.any():
         out.append((2, dec))
     if chk.any():
-        out.append((1 if KV_FP8 else 3, chk))      # (an fp8 pool's chunk-class items run on the row kernel)
+        out.append((3, chk))
     return out
 
 

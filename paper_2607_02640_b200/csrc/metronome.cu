@@ -20,6 +20,7 @@
 #include "attend_mma.cuh"
 #include "attend_rows.cuh"
 #include "attend_umma.cuh"
+#include "attend_umma_fp8.cuh"
 #include "bookkeeping.cuh"
 #include "kv_append.cuh"
 #include "step_gqa.cuh"
@@ -314,10 +315,9 @@ int plan_attend(metronome_pool* pool, int32_t n_batch, const int32_t* sids, cons
     }
     int family = pool->tune_family;
     if (family == 0) family = (pool->G * max_q >= 4) ? 2 : 1;
-    // fp8 KV (NEXT row f4): decode-class items go to the GQA decode kernel's fp8 tile, chunk-class items to the
-    // CUDA-core row kernel (the tcgen05 chunk kernel reads bf16 tiles only)
-    const bool rows_chunks = pool->fp8;
-    if (family == 2 && !rows_chunks && !attend_umma_supported(pool->G, max_q))
+    // (fp8 KV, NEXT row f4: the same three families -- fp8 rows in the row kernel, an fp8 tile in the GQA decode
+    // kernel, attend_umma_fp8_kernel for the chunk class)
+    if (family == 2 && !attend_umma_supported(pool->G, max_q))
         family = 1;
     pl.family = family;
 
@@ -375,7 +375,7 @@ int plan_attend(metronome_pool* pool, int32_t n_batch, const int32_t* sids, cons
             cls_tiles[cls] += its[i].n_tiles;
             pl.cls_rows[cls] += its[i].q_len;
             if (its[i].q_len > pl.cls_max_q[cls]) pl.cls_max_q[cls] = its[i].q_len;
-            units += (int64_t)its[i].n_tiles * (family == 2 && !rows_chunks ? c.n_kv_heads : c.n_q_heads * its[i].q_len);
+            units += (int64_t)its[i].n_tiles * (family == 2 ? c.n_kv_heads : c.n_q_heads * its[i].q_len);
         }
         if (family == 2 && cls == 0) {
             // stream-K: one wave of n_SM x 3 CTAs, equal static ranges (one per CTA); for long shares the
@@ -451,7 +451,7 @@ int plan_attend(metronome_pool* pool, int32_t n_batch, const int32_t* sids, cons
             continue;
         }
         // segments sized for >= 2 waves of CTAs, each with a useful run of tiles
-        const bool umma_cls = family == 2 && !rows_chunks;
+        const bool umma_cls = family == 2;
         const int64_t target_ctas = (int64_t)pool->n_sm * (umma_cls ? 4 : 16);
         int32_t tps = pool->tune_split_tokens > 0 ? (pool->tune_split_tokens + kBlockTokens - 1) / kBlockTokens
                                                   : (int32_t)((units + target_ctas - 1) / target_ctas);
@@ -548,8 +548,7 @@ int launch_attend(metronome_pool* pool, int32_t layer, const AttendPlan& pl, con
         CU(cudaEventRecord(pool->prof_ev[pool->prof_used], st));
         pdl = false;
     }
-    // (the row kernel, which takes an fp8 pool's chunk-class items, does not publish)
-    const bool publish = pl.family == 2 && pdl && !pool->profiling && !pool->poison && (!pool->fp8 || pl.n_cls[0] > 0);
+    const bool publish = pl.family == 2 && pdl && !pool->profiling && !pool->poison;
     if (publish) { p.pastwait_flag = pool->d_bk_flag + 12; p.pastwait_epoch = (int32_t)pool->epoch; }
     if (pl.family == 2) {
         if (pl.n_cls[0] > 0) {
@@ -560,15 +559,9 @@ int launch_attend(metronome_pool* pool, int32_t layer, const AttendPlan& pl, con
         }
         if (pl.n_cls[1] > 0) {
             p.items = d_items + pl.n_cls[0]; p.n_items = pl.n_cls[1];
-            if (pool->fp8) {
-                dim3 grid(c.n_q_heads, pl.total_splits[1], pl.cls_max_q[1]);
-                p.stamp = next_stamp(pool, 1);
-                if (c.head_dim == 128) CU(launch_kernel(attend_rows_kernel<128, true>, grid, dim3(128), 0, st, pdl, p));
-                else CU(launch_kernel(attend_rows_kernel<64, true>, grid, dim3(128), 0, st, pdl, p));
-            } else {
-                p.stamp = next_stamp(pool, 3);
-                CU(launch_attend_umma(p, c.head_dim, c.n_kv_heads, pl.total_splits[1], st, pdl));
-            }
+            p.stamp = next_stamp(pool, 3);
+            if (pool->fp8) CU(launch_attend_umma_fp8(p, c.head_dim, c.n_kv_heads, pl.total_splits[1], st, pdl));
+            else CU(launch_attend_umma(p, c.head_dim, c.n_kv_heads, pl.total_splits[1], st, pdl));
             ++pool->n_launch;
         }
     } else {
@@ -725,6 +718,7 @@ int metronome_pool_create(const metronome_pool_config_t* cfg, metronome_pool_t**
     if (e != cudaSuccess) return fail(METRONOME_ERR_CUDA, e, "pool init kernels");
     e = configure_attend_mma_kernels();
     if (e == cudaSuccess) e = configure_attend_umma_kernels();
+    if (e == cudaSuccess) e = configure_attend_umma_fp8_kernels();
     if (e == cudaSuccess) e = configure_step_kernels();
     if (e != cudaSuccess) return fail(METRONOME_ERR_CUDA, e, "cudaFuncSetAttribute");
 
