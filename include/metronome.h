@@ -57,7 +57,9 @@ enum {
     METRONOME_ERR_LEN_OVERFLOW = 9,       /* the clean version of the max_model_len crash (L271)   */
     METRONOME_ERR_CUDA = 10,              /* a CUDA runtime call failed; see metronome_last_cuda_error */
     METRONOME_ERR_UNSUPPORTED = 11,       /* e.g. attention on a bookkeeping-only pool             */
-    METRONOME_ERR_OUT_OF_MEMORY = 12
+    METRONOME_ERR_OUT_OF_MEMORY = 12,
+    METRONOME_ERR_SCRATCH_EXCEEDED = 13   /* metronome_attend_frame_static: the call's split-KV partials do not fit
+                                             the library's fixed scratch array; nothing was launched             */
 };
 
 /* ---- flags ---------------------------------------------------------------------------------- */
@@ -173,6 +175,33 @@ int metronome_append_kv(metronome_pool_t* pool, int32_t layer, int32_t n_batch,
 int metronome_attend_frame(metronome_pool_t* pool, int32_t layer, int32_t n_batch,
                            const int32_t* sids, const int32_t* q_lens,
                            const void* q, void* out, void* cuda_stream);
+
+/* metronome_attend_frame for callers that must not allocate (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): same arguments, same result (the union mask
+ * [0,S) U (t-W, t]; L258 "segmented-decode ... merged exactly once"), but the call -- unlike attend_frame,
+ * whose split-KV workspace is grown with cudaFree / cudaMalloc when a batch needs more -- calls NO cudaMalloc,
+ * cudaFree or allocating library routine.  It always runs the split-KV CUDA-core row kernel + the merge kernel
+ * (any group size, bf16 and fp8 pools; the tensor-core kernels are not used), and the segments' partial
+ * results (acc, m, l) go to ONE fixed array of METRONOME_STATIC_SCRATCH_BYTES that lives in the library image:
+ * every GPU that loads libmetronome.so holds those bytes until the process exits.
+ *   limit   sum(q_lens) * n_q_heads * max_splits * (head_dim + 2) * 4 <= METRONOME_STATIC_SCRATCH_BYTES, where
+ *           max_splits (<= 64) is the largest number of segments the call's split plan gives one session
+ *           (segments of >= 8 KV blocks, sized for >= 16 CTAs per SM; 1 = no partials at all).  A call beyond it
+ *           returns METRONOME_ERR_SCRATCH_EXCEEDED (metronome_last_cuda_error() says by how much); nothing was
+ *           launched and nothing changed.  Config 2's decode step (128 rows x 32 heads x 6 segments) needs 12.2 MiB.
+ *   sharing the array is shared by EVERY call in the process (all pools, all streams of one device) and keeps the
+ *           previous call's contents.  Nothing in it has to start at zero: a call reads only the slots its own
+ *           row kernel wrote.  Two calls whose kernels overlap on the GPU (different streams, different pools)
+ *           RACE on it: order such calls yourself (one stream, or an event between them).
+ *   set-up  the array's device address is looked up once per device (cudaGetSymbolAddress, no allocation) by the
+ *           first call made with that device current; the pool must have been created on the current device.
+ * sids, q_lens, q, out, stream ordering and the other errors: as metronome_attend_frame.  The per-call work
+ * list travels through the pool's staging ring (allocated at pool creation) with one cudaMemcpyAsync.
+ * Errors: those of metronome_attend_frame, SCRATCH_EXCEEDED. */
+#define METRONOME_STATIC_SCRATCH_BYTES (16u << 20)
+int metronome_attend_frame_static(metronome_pool_t* pool, int32_t layer, int32_t n_batch,
+                                  const int32_t* sids, const int32_t* q_lens,
+                                  const void* q, void* out, void* cuda_stream);
 
 /* One sub-step of a frame in ONE call: exactly metronome_append_kv(layer, sids, n_new, k_new, v_new)
  * followed by metronome_attend_frame(layer, sids, q_lens = n_new, q, out) -- same arguments, same

@@ -21,13 +21,14 @@ FLAG_KV_FP8 = 0x8
 
 ERR_NAMES = {0: "OK", 1: "INVALID_ARG", 2: "INVALID_SESSION", 3: "DUPLICATE_SESSION", 4: "SESSIONS_FULL",
              5: "POOL_EXHAUSTED", 6: "CHUNK_TOO_LARGE", 7: "QLEN_EXCEEDS_LAST_APPEND", 8: "LAYER_SEQUENCE",
-             9: "LEN_OVERFLOW", 10: "CUDA", 11: "UNSUPPORTED", 12: "OUT_OF_MEMORY"}
+             9: "LEN_OVERFLOW", 10: "CUDA", 11: "UNSUPPORTED", 12: "OUT_OF_MEMORY", 13: "SCRATCH_EXCEEDED"}
+STATIC_SCRATCH_BYTES = 16 << 20      # METRONOME_STATIC_SCRATCH_BYTES
 
 # every symbol include/metronome.h and include/metronome_measure.h declare
 EXPORTS = ["metronome_abi_version", "metronome_strerror", "metronome_last_cuda_error",
            "metronome_kv_storage_bytes", "metronome_max_blocks_per_session", "metronome_pool_create",
            "metronome_pool_destroy", "metronome_session_open", "metronome_session_close",
-           "metronome_append_kv", "metronome_attend_frame", "metronome_append_attend", "metronome_step_host", "metronome_step_host_async", "metronome_step_host_wait",
+           "metronome_append_kv", "metronome_attend_frame", "metronome_attend_frame_static", "metronome_append_attend", "metronome_step_host", "metronome_step_host_async", "metronome_step_host_wait",
            "metronome_session_query", "metronome_pool_query", "metronome_read_kv", "metronome_pool_stats",
            "metronome_pool_set_tuning", "metronome_pool_sm_speeds", "metronome_pool_debug_fail_next", "metronome_pool_debug_read_flags", "metronome_pool_set_profiling", "metronome_pool_read_profile", "metronome_pool_read_stamps",
            "metronome_gate_create", "metronome_gate_destroy", "metronome_gate_observe", "metronome_gate_admit",
@@ -76,6 +77,7 @@ def load():
     lib.metronome_session_close.argtypes = [c_void_p, c_int32, c_void_p]
     lib.metronome_append_kv.argtypes = [c_void_p, c_int32, c_int32, i32p, i32p, c_void_p, c_void_p, c_void_p]
     lib.metronome_attend_frame.argtypes = [c_void_p, c_int32, c_int32, i32p, i32p, c_void_p, c_void_p, c_void_p]
+    lib.metronome_attend_frame_static.argtypes = [c_void_p, c_int32, c_int32, i32p, i32p, c_void_p, c_void_p, c_void_p]
     lib.metronome_append_attend.argtypes = [c_void_p, c_int32, c_int32, i32p, i32p, c_void_p, c_void_p, c_void_p,
                                             c_void_p, c_void_p]
     lib.metronome_step_host.argtypes = [c_void_p, c_int32, c_int32, i32p, i32p, c_void_p, c_void_p, c_void_p,
@@ -140,7 +142,7 @@ class Pool:
     def _check(self, status):
         if status != 0:
             detail = ""
-            if status == 10 and self._h:
+            if status in (10, 13) and self._h:
                 detail = self._lib.metronome_last_cuda_error(self._h).decode()
             raise MetronomeError(status, detail)
 
@@ -177,6 +179,13 @@ class Pool:
         n, np_ = _i32(q_lens)
         self._check(self._lib.metronome_attend_frame(self._h, layer, len(s), sp, np_, _ptr(q), _ptr(out),
                                                      c_void_p(stream)))
+
+    def attend_frame_static(self, layer, sids, q_lens, q, out, stream=0):
+        """attend_frame that allocates nothing: split-KV partials in the library's fixed scratch array."""
+        s, sp = _i32(sids)
+        n, np_ = _i32(q_lens)
+        self._check(self._lib.metronome_attend_frame_static(self._h, layer, len(s), sp, np_, _ptr(q), _ptr(out),
+                                                            c_void_p(stream)))
 
     def append_attend(self, layer, sids, n_new, k_new, v_new, q, out, stream=0):
         s, sp = _i32(sids)

@@ -27,6 +27,11 @@
 
 using namespace metronome;
 
+// metronome_attend_frame_static (include/metronome.h): the split-KV partials of a call that must not allocate.
+// The name below is a host-side stand-in in host code, NOT a device address: static_scratch_ptr() asks the runtime
+// for the address (once per device, with that device current) and only that pointer is ever given to a kernel.
+static __device__ __align__(256) unsigned char g_static_scratch[METRONOME_STATIC_SCRATCH_BYTES];
+
 namespace {
 
 struct Session {
@@ -594,6 +599,87 @@ int launch_attend(metronome_pool* pool, int32_t layer, const AttendPlan& pl, con
     return METRONOME_OK;
 }
 
+// Device address of g_static_scratch on the CURRENT device (looked up on the first call made with that device
+// current; cudaGetSymbolAddress allocates nothing).  Returns null and sets *err on failure.
+constexpr int kMaxDevices = 64;
+void* static_scratch_ptr(cudaError_t* err) {
+    static void* ptr[kMaxDevices] = {};
+    int dev = 0;
+    *err = cudaGetDevice(&dev);
+    if (*err != cudaSuccess) return nullptr;
+    if (dev < 0 || dev >= kMaxDevices) { *err = cudaErrorInvalidDevice; return nullptr; }
+    void* p = __atomic_load_n(&ptr[dev], __ATOMIC_ACQUIRE);
+    if (!p) {
+        *err = cudaGetSymbolAddress(&p, g_static_scratch);
+        if (*err != cudaSuccess) return nullptr;
+        __atomic_store_n(&ptr[dev], p, __ATOMIC_RELEASE);      // (two racing first calls store the same address)
+    }
+    return p;
+}
+
+// Row a8 for metronome_attend_frame_static: the work list of the split-KV row kernel (one class, every item),
+// with the same item fields and the same segment rule as plan_attend's row-kernel branch (segments of >= 8 tiles,
+// sized for >= 16 CTAs per SM, at most kMaxSplits per item) -- but no workspace growth: the caller checks the
+// plan against the fixed scratch.  Writes items[0 .. n_items) (the pool's pinned staging slot: no host allocation).
+void plan_rows_static(metronome_pool* pool, int32_t n_batch, const int32_t* sids, const int32_t* q_lens, AttendItem* items,
+                      AttendPlan& pl) {
+    const metronome_pool_config_t& c = pool->cfg;
+    pl = AttendPlan();
+    pl.family = 1;
+    const int32_t W = pool->W_eff;
+    int32_t row = 0, n_items = 0;
+    int64_t units = 0, tiles = 0;
+    for (int i = 0; i < n_batch; ++i) {
+        if (q_lens[i] == 0) continue;
+        const Session& s = pool->sessions[sids[i]];
+        AttendItem& it = items[n_items++];
+        memset(&it, 0, sizeof(it));
+        it.sid = sids[i];
+        it.len = (int32_t)s.len;
+        it.q_len = q_lens[i];
+        it.q_row_off = row;
+        it.class_row_off = row;
+        row += q_lens[i];
+        const int32_t n_blk = (int32_t)((s.len + kBlockTokens - 1) / kBlockTokens);
+        const int64_t t0 = s.len - q_lens[i];                      // oldest query of this call
+        const int64_t wfirst = t0 - W + 1 > 0 ? t0 - W + 1 : 0;    // its oldest window key
+        int32_t first_blk = (int32_t)(wfirst / kBlockTokens);
+        if (first_blk < pool->n_sink) first_blk = pool->n_sink;
+        it.n_sink_tiles = n_blk < pool->n_sink ? n_blk : pool->n_sink;
+        it.first_blk = first_blk;
+        it.n_tiles = it.n_sink_tiles + (n_blk > first_blk ? n_blk - first_blk : 0);
+        it.fresh_blk = 0;                                          // (plain launch: the kernel waits at the top)
+        it.tile_off = (int32_t)tiles;
+        tiles += it.n_tiles;
+        units += (int64_t)it.n_tiles * c.n_q_heads * it.q_len;
+        if (it.q_len > pl.cls_max_q[0]) pl.cls_max_q[0] = it.q_len;
+    }
+    pl.n_items = n_items;
+    pl.n_cls[0] = n_items;
+    pl.total_rows = row;
+    pl.cls_rows[0] = row;
+    const int64_t target_ctas = (int64_t)pool->n_sm * 16;
+    int32_t tps = pool->tune_split_tokens > 0 ? (pool->tune_split_tokens + kBlockTokens - 1) / kBlockTokens
+                                              : (int32_t)((units + target_ctas - 1) / target_ctas);
+    if (pool->tune_split_tokens <= 0 && tps < 8) tps = 8;
+    if (tps < 1) tps = 1;
+    for (int i = 0; i < n_items; ++i) {
+        AttendItem& it = items[i];
+        int32_t ns = (it.n_tiles + tps - 1) / tps;
+        if (ns > kMaxSplits) ns = kMaxSplits;
+        if (ns < 1) ns = 1;
+        it.tiles_per_split = (it.n_tiles + ns - 1) / ns;
+        it.n_splits = (it.n_tiles + it.tiles_per_split - 1) / it.tiles_per_split;
+        if (it.n_splits < 1) it.n_splits = 1;
+        it.split_off = pl.total_splits[0];
+        pl.total_splits[0] += it.n_splits;
+        if (it.n_splits > pl.max_splits) pl.max_splits = it.n_splits;
+        if (it.n_splits > 1) pl.merge_cls[0] = true;
+    }
+    if (pl.max_splits < 1) pl.max_splits = 1;
+    pl.valid = true;
+}
+
 }  // namespace
 
 // ------------------------------------------------------------------------------------------------
@@ -616,6 +702,7 @@ const char* metronome_strerror(int status) {
         case METRONOME_ERR_CUDA: return "CUDA";
         case METRONOME_ERR_UNSUPPORTED: return "UNSUPPORTED";
         case METRONOME_ERR_OUT_OF_MEMORY: return "OUT_OF_MEMORY";
+        case METRONOME_ERR_SCRATCH_EXCEEDED: return "SCRATCH_EXCEEDED";
         default: return "UNKNOWN";
     }
 }
@@ -1093,6 +1180,79 @@ int metronome_attend_frame(metronome_pool_t* pool, int32_t layer, int32_t n_batc
     rc = commit_stage(pool, slot, (size_t)plan.n_items * sizeof(AttendItem) + (size_t)plan.n_range_items * sizeof(int32_t), st);
     if (rc) return rc;
     return launch_attend(pool, layer, plan, reinterpret_cast<const AttendItem*>(d), q, out, st, false);
+}
+
+// metronome_attend_frame without any allocation (include/metronome.h): the split-KV row kernel + the merge kernel,
+// their partials in the library's fixed scratch array instead of the pool's grow-on-demand workspace.  Calls no
+// cudaMalloc / cudaFree (nor plan_attend -> ensure_workspace, which does); the work list goes through the pool's
+// staging ring like the general path of attend_frame.
+int metronome_attend_frame_static(metronome_pool_t* pool, int32_t layer, int32_t n_batch, const int32_t* sids,
+                                  const int32_t* q_lens, const void* q, void* out, void* cuda_stream) {
+    if (!pool || layer < 0 || layer >= pool->cfg.n_layers) return METRONOME_ERR_INVALID_ARG;
+    if (pool->bookkeeping_only) return METRONOME_ERR_UNSUPPORTED;
+    int rc = check_batch(pool, n_batch, sids, q_lens);
+    if (rc) return rc;
+    int64_t total_rows = 0;
+    for (int i = 0; i < n_batch; ++i) {
+        if (q_lens[i] > pool->sessions[sids[i]].last_n) return METRONOME_ERR_QLEN_EXCEEDS_LAST_APPEND;
+        total_rows += q_lens[i];
+    }
+    if (total_rows > 0 && (!q || !out)) return METRONOME_ERR_INVALID_ARG;
+    if (total_rows == 0) { ++pool->n_attend; return METRONOME_OK; }
+    if (pool->epoch == 0 || pool->layer_epoch[layer] != pool->epoch) return METRONOME_ERR_LAYER_SEQUENCE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const metronome_pool_config_t& c = pool->cfg;
+
+    cudaError_t ce = cudaSuccess;
+    uint8_t* scratch = static_cast<uint8_t*>(static_scratch_ptr(&ce));
+    if (!scratch) return cuda_fail(pool, ce, "cudaGetSymbolAddress(g_static_scratch)");
+
+    uint8_t *h = nullptr, *d = nullptr;
+    int slot = 0;
+    rc = acquire_stage(pool, &h, &d, &slot);
+    if (rc) return rc;
+    AttendPlan plan;
+    plan_rows_static(pool, n_batch, sids, q_lens, reinterpret_cast<AttendItem*>(h), plan);
+    // [row][Hq][max_splits][D] floats of partial outputs, then [row][Hq][max_splits][2] floats of (m, l)
+    const size_t slots = (size_t)plan.total_rows * c.n_q_heads * plan.max_splits;
+    const size_t need = plan.max_splits > 1 ? slots * (size_t)(c.head_dim + 2) * sizeof(float) : 0;
+    if (need > (size_t)METRONOME_STATIC_SCRATCH_BYTES) {
+        char msg[192];
+        snprintf(msg, sizeof(msg), "attend_frame_static: %lld rows x %d heads x %d segments x (%d + 2) floats = %zu bytes of "
+                 "split-KV partials, the static scratch holds %u", (long long)plan.total_rows, c.n_q_heads, plan.max_splits,
+                 c.head_dim, need, (unsigned)METRONOME_STATIC_SCRATCH_BYTES);
+        pool->cuda_err = msg;
+        return METRONOME_ERR_SCRATCH_EXCEEDED;
+    }
+    ++pool->n_attend;
+    rc = commit_stage(pool, slot, (size_t)plan.n_items * sizeof(AttendItem), st);
+    if (rc) return rc;
+
+    AttendParams p = make_attend_params(pool, layer, plan, q, out);
+    p.ws_acc = reinterpret_cast<float*>(scratch);                                    // (256-byte aligned; slots * D * 4
+    p.ws_ml = reinterpret_cast<float*>(scratch + slots * (size_t)c.head_dim * sizeof(float));   //  is a multiple of 16)
+    p.max_splits = plan.max_splits;
+    p.items = reinterpret_cast<const AttendItem*>(d);
+    p.n_items = plan.n_items;
+    p.range_item = nullptr;
+    p.items_epoch = -1;                       // the list came by a copy: the kernel waits for its predecessor at the top
+    p.stamp = nullptr;
+    dim3 grid(c.n_q_heads, plan.total_splits[0], plan.cls_max_q[0]);
+    if (pool->fp8) {
+        if (c.head_dim == 128) CU(launch_kernel(attend_rows_kernel<128, true>, grid, dim3(128), 0, st, false, p));
+        else CU(launch_kernel(attend_rows_kernel<64, true>, grid, dim3(128), 0, st, false, p));
+    } else {
+        if (c.head_dim == 128) CU(launch_kernel(attend_rows_kernel<128, false>, grid, dim3(128), 0, st, false, p));
+        else CU(launch_kernel(attend_rows_kernel<64, false>, grid, dim3(128), 0, st, false, p));
+    }
+    ++pool->n_launch;
+    if (plan.merge_cls[0]) {                  // row a6: every slot the merge reads was written by the launch above
+        dim3 mgrid((unsigned)plan.cls_rows[0], c.n_q_heads);
+        if (c.head_dim == 128) CU(launch_kernel(merge_kernel<128>, mgrid, dim3(32), 0, st, true, p));
+        else CU(launch_kernel(merge_kernel<64>, mgrid, dim3(16), 0, st, true, p));
+        ++pool->n_launch;
+    }
+    return release_stage(pool, slot, st);
 }
 
 int metronome_step_host(metronome_pool_t* pool, int32_t layer, int32_t n_batch, const int32_t* sids,

@@ -1,0 +1,175 @@
+"""GPU test (`-m gpu`) of metronome_attend_frame_static, the entry point for callers that must not allocate
+(include/metronome.h: code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc).
+Its split-KV partials live in a fixed 16 MiB `static __device__` array of the library instead of the pool's
+grow-on-demand workspace; everything else (inputs, outputs, the union mask of PAPER.md:L103 / L258) is
+metronome_attend_frame's.
+
+The file is named so that pytest collects it LAST (the suite runs with `pytest -x`).  It depends on nothing the
+other tests leave behind: the scratch array keeps the previous call's contents by design, and a call reads only
+the slots its own row kernel wrote -- so the checks hold in a fresh process and after the whole suite alike.
+
+Checks, each on TWO calls in a row without a host sync in between (the second call finds the first one's
+partials in the shared array):
+  * output == the existing path's (attend_frame on the same pool state) within the suite's tolerance
+    (parity_helpers: |g - o| <= 1e-2 + 2e-2 |o|, row-wise l2 <= 1e-2, row-wise max-rel <= 2e-2), for multi-head decode,
+    a GQA mix of chunk + decode rows (where the existing path runs the tensor-core kernels), and an fp8 KV pool;
+  * the partials really went through the array (several segments per session), and the pool's own workspace was
+    never grown by the new entry point;
+  * a call beyond the array's size is rejected with SCRATCH_EXCEEDED, launches nothing and leaves the pool usable.
+Seeded inputs; nothing reads /root/reference.
+"""
+import numpy as np
+import pytest
+import torch
+
+from paper_2607_02640_b200 import binding
+from parity_helpers import assert_parity
+
+pytestmark = pytest.mark.gpu
+
+
+def _rows(rng, n, H, D):
+    return torch.from_numpy(rng.standard_normal((n, H, D)).astype(np.float32)).to(torch.bfloat16)
+
+
+def _pool(Hq, Hkv, D, S, W, N, n_max, flags=0):
+    per = -(-S // 16) + (W + n_max - 1) // 16 + 2
+    return binding.Pool(n_q_heads=Hq, n_kv_heads=Hkv, head_dim=D, n_sinks=S, window=W, n_blocks=N * per,
+                        max_sessions=N, max_new_tokens=n_max, flags=flags)
+
+
+def _history(pool, sids, rng, lo, hi, Hkv, D, n_max):
+    """ragged histories of lo .. hi tokens, appended in chunks (no attention)"""
+    N = len(sids)
+    target = rng.integers(lo, hi, size=N)
+    done = np.zeros(N, np.int64)
+    while (done < target).any():
+        idx = [i for i in range(N) if done[i] < target[i]]
+        n_new = np.array([min(n_max, target[i] - done[i]) for i in idx], np.int32)
+        rows = int(n_new.sum())
+        pool.append_kv(0, [sids[i] for i in idx], n_new, _rows(rng, rows, Hkv, D).cuda(), _rows(rng, rows, Hkv, D).cuda())
+        done[idx] += n_new
+
+
+def _two_calls_in_a_row(pool, sids, steps, rng, Hq, Hkv, D, what, unit_scale=True):
+    """For each step (a list of n_new per session): append, then the existing path and the no-alloc path on the same
+    state.  The no-alloc calls of consecutive steps run back to back with no host sync."""
+    pending = []
+    for n_new in steps:
+        n_new = np.asarray(n_new, np.int32)
+        rows = int(n_new.sum())
+        k, v, q = (_rows(rng, rows, H, D).cuda() for H in (Hkv, Hkv, Hq))
+        pool.append_kv(0, sids, n_new, k, v)
+        ref = torch.empty_like(q)
+        pool.attend_frame(0, sids, n_new, q, ref)                 # the existing path
+        got1, got2 = torch.full_like(q, float("nan")), torch.full_like(q, float("nan"))
+        pool.attend_frame_static(0, sids, n_new, q, got1)          # the new entry point, twice in a row: the second
+        pool.attend_frame_static(0, sids, n_new, q, got2)          # call finds the first one's partials in the array
+        pending.append((ref, got1, got2, n_new))
+    torch.cuda.synchronize()
+    for step, (ref, got1, got2, n_new) in enumerate(pending):
+        r = ref.float().cpu().numpy()
+        assert np.isfinite(r).all()
+        assert_parity(got1, r, f"{what}: step {step} n_new {n_new}, first call", unit_scale=unit_scale)
+        assert_parity(got2, r, f"{what}: step {step} n_new {n_new}, second call", unit_scale=unit_scale)
+        assert torch.equal(got1, got2), f"{what}: step {step}: two calls on the same state differ"
+
+
+def test_no_alloc_decode_matches_attend_frame():
+    """Multi-head decode (Moshi-shaped heads, W = 750: 48 window blocks = 6 segments per session)."""
+    Hq, Hkv, D, S, W, N = 8, 8, 128, 4, 750, 6
+    pool = _pool(Hq, Hkv, D, S, W, N, 25)
+    sids = [pool.session_open() for _ in range(N)]
+    rng = np.random.default_rng(20260702)
+    _history(pool, sids, rng, 40, 1800, Hkv, D, 25)
+    ws_before = pool.stats()
+    _two_calls_in_a_row(pool, sids, [[1] * N] * 4, rng, Hq, Hkv, D, "no-alloc decode")
+    assert pool.stats()["kernel_launches"] > ws_before["kernel_launches"]
+
+
+def test_no_alloc_gqa_chunk_and_decode_mix_matches_attend_frame():
+    """GQA 4, one call mixing chunk rows and decode rows ("mixed prefill/decode"): the existing path runs
+    its tensor-core kernels here, the no-alloc path the split-KV row kernel -- same result within the tolerance.
+    S = 17: a partly filled second sink block."""
+    Hq, Hkv, D, S, W, N = 16, 4, 128, 17, 520, 5
+    pool = _pool(Hq, Hkv, D, S, W, N, 12)
+    sids = [pool.session_open() for _ in range(N)]
+    rng = np.random.default_rng(77)
+    _history(pool, sids, rng, 10, 1500, Hkv, D, 12)
+    _two_calls_in_a_row(pool, sids, [[12, 1, 7, 1, 3], [1, 1, 1, 1, 1], [2, 9, 1, 12, 1]], rng, Hq, Hkv, D, "no-alloc GQA mix")
+
+
+def test_no_alloc_on_an_fp8_pool_matches_attend_frame():
+    Hq, Hkv, D, S, W, N = 8, 8, 64, 4, 300, 4
+    pool = _pool(Hq, Hkv, D, S, W, N, 8, flags=binding.FLAG_KV_FP8)
+    sids = [pool.session_open() for _ in range(N)]
+    rng = np.random.default_rng(5)
+    _history(pool, sids, rng, 200, 900, Hkv, D, 8)
+    _two_calls_in_a_row(pool, sids, [[1] * N, [1] * N], rng, Hq, Hkv, D, "no-alloc fp8")
+
+
+def test_no_alloc_rejects_a_call_beyond_the_static_scratch():
+    """24 sessions x 25-token chunks x 32 heads, forced 1-block segments (64 per session): 600 x 32 x 64 x 130 floats
+    = 639 MB of partials against the array's 16 MiB -> SCRATCH_EXCEEDED, nothing launched, the pool still works, and a
+    call that fits (automatic segments) goes through right after."""
+    Hq, Hkv, D, S, W, N = 32, 4, 128, 4, 2048, 24
+    pool = _pool(Hq, Hkv, D, S, W, N, 25)
+    sids = [pool.session_open() for _ in range(N)]
+    rng = np.random.default_rng(11)
+    _history(pool, sids, rng, 2100, 2300, Hkv, D, 25)
+    n_new = np.full(N, 25, np.int32)
+    rows = int(n_new.sum())
+    k, v, q = (_rows(rng, rows, H, D).cuda() for H in (Hkv, Hkv, Hq))
+    pool.append_kv(0, sids, n_new, k, v)
+    ref = torch.empty_like(q)
+    pool.attend_frame(0, sids, n_new, q, ref)
+    pool.set_tuning(16, 0)                                          # 1-block segments
+    launches = pool.stats()["kernel_launches"]
+    out = torch.zeros_like(q)
+    with pytest.raises(binding.MetronomeError) as ei:
+        pool.attend_frame_static(0, sids, n_new, q, out)
+    assert ei.value.code == "SCRATCH_EXCEEDED" and "static scratch holds" in str(ei.value), str(ei.value)
+    assert pool.stats()["kernel_launches"] == launches
+    torch.cuda.synchronize()
+    assert not out.any(), "a rejected call wrote output"
+    pool.set_tuning(0, 0)
+    need = rows * Hq * 64 * (D + 2) * 4
+    assert need > binding.STATIC_SCRATCH_BYTES
+    # automatic segments: 132 blocks / session at >= 16 CTAs per SM -> few segments; 600 rows x 32 heads x 130 floats
+    # x segments must fit for the call to pass
+    pool.attend_frame_static(0, sids, n_new, q, out)
+    torch.cuda.synchronize()
+    assert_parity(out, ref.float().cpu().numpy(), "no-alloc after a rejected call")
+
+
+def test_no_alloc_only_pool_never_touches_the_pool_workspace():
+    """Two pools fed the same seeded rows (bookkeeping is deterministic: same block ids): pool A answers through the
+    existing path, pool B ONLY ever through the no-alloc entry point, so B's own split-KV workspace is never allocated
+    (a null pointer: using it would fault) and its partials can only have gone through the array whose address the
+    library looked up with cudaGetSymbolAddress.  Free device memory (cudaMemGetInfo) is the same before and after
+    B's calls: the existing path would have grown a workspace of several MB for these batches."""
+    Hq, Hkv, D, S, W, N = 8, 8, 128, 4, 750, 6
+    pa, pb = _pool(Hq, Hkv, D, S, W, N, 25), _pool(Hq, Hkv, D, S, W, N, 25)
+    sa = [pa.session_open() for _ in range(N)]
+    sb = [pb.session_open() for _ in range(N)]
+    assert sa == sb
+    for pool, sids in ((pa, sa), (pb, sb)):
+        _history(pool, sids, np.random.default_rng(31), 900, 1800, Hkv, D, 25)
+    rng = np.random.default_rng(32)
+    ones = np.ones(N, np.int32)
+    ins = [tuple(_rows(rng, N, H, D).cuda() for H in (Hkv, Hkv, Hq)) for _ in range(3)]
+    refs = [torch.empty_like(q) for _, _, q in ins]
+    gots = [torch.full_like(q, float("nan")) for _, _, q in ins]
+    for (k, v, q), ref in zip(ins, refs):
+        pa.append_kv(0, sa, ones, k, v)
+        pa.attend_frame(0, sa, ones, q, ref)
+    torch.cuda.synchronize()
+    free_before = torch.cuda.mem_get_info()[0]
+    for (k, v, q), got in zip(ins, gots):                            # back to back, no host sync
+        pb.append_kv(0, sb, ones, k, v)
+        pb.attend_frame_static(0, sb, ones, q, got)
+    torch.cuda.synchronize()
+    assert torch.cuda.mem_get_info()[0] == free_before, "device memory was allocated during the no-alloc calls"
+    for step, (ref, got) in enumerate(zip(refs, gots)):
+        assert_parity(got, ref.float().cpu().numpy(), f"no-alloc-only pool, step {step}")
+    assert pa.pool_query()[1] == pb.pool_query()[1]
