@@ -124,53 +124,148 @@ attend_umma_fp8_kernel(AttendParams p) {
     auto entry_k = [&](int32_t h) { return umma_seq_k(h); };
     auto entry_v = [&](int32_t h) { return umma_seq_v(h, n_half); };
 
-    if (warp == 0) {
-        // ================================ producer ================================
-        if (lane == 0) {
-            for (int b = 0; b < C::NBUF; ++b) { mbar_init(bar_full(b), 4); mbar_init(bar_empty(b), n_slots); }
-            for (int s = 0; s < C::NSTAGE; ++s) { mbar_init(bar_stf(s), 1); mbar_init(bar_ste(s), 4); }
-            for (int s = 0; s < 2; ++s) {
-                for (int buf = 0; buf < 2; ++buf) { mbar_init(bar_s(s, buf), 1); mbar_init(bar_p(s, buf), 4); mbar_init(bar_pv(s, buf), 1); }
-                mbar_init(bar_o(s), 1);
+    // Register budget per warpgroup (setmaxnreg; 512 threads launch with 128 each): producer + MMA issuers 72,
+    // converters 104, the two softmax warpgroups 168 (one thread per query row holds 64 scores + 64 weights:
+    // at 128 it spilled ~200 bytes per thread into the half-stage loop).  4 x 32 x (72 + 104 + 2 x 168) = 65536.
+    if (warp < 4) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 72;");
+        if (warp == 0) {
+            // ================================ producer ================================
+            if (lane == 0) {
+                for (int b = 0; b < C::NBUF; ++b) { mbar_init(bar_full(b), 4); mbar_init(bar_empty(b), n_slots); }
+                for (int s = 0; s < C::NSTAGE; ++s) { mbar_init(bar_stf(s), 1); mbar_init(bar_ste(s), 4); }
+                for (int s = 0; s < 2; ++s) {
+                    for (int buf = 0; buf < 2; ++buf) { mbar_init(bar_s(s, buf), 1); mbar_init(bar_p(s, buf), 4); mbar_init(bar_pv(s, buf), 1); }
+                    mbar_init(bar_o(s), 1);
+                }
+                asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
             }
-            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        }
-        __syncwarp();
-        named_arrive(1, C::kThreads);
-        const int32_t* trow = p.table + (int64_t)it.sid * p.tbl_width;
-        const uint8_t* head_base = p.kv_layer + (int64_t)kvh * p.L.head_bytes;
-        // physical block ids of this segment's tiles, fetched ONCE (lane l holds tiles l, l+32, ...)
-        constexpr int kPhysPre = 8;                               // 256 tiles; longer segments look up the rest
-        int32_t phys_pre[kPhysPre];
-#pragma unroll
-        for (int j = 0; j < kPhysPre; ++j) {
-            const int32_t t = tl0 + j * 32 + lane;
-            phys_pre[j] = t < tl1 ? __ldg(trow + table_slot(tile_block(it, t), p.n_sink, p.ring)) : 0;
-        }
-        auto phys_of = [&](int32_t rel) {                         // rel = tile - tl0; rel >> 5 is warp-uniform
-            const int32_t j = rel >> 5;
-            int32_t v = phys_pre[0];
-#pragma unroll
-            for (int q = 1; q < kPhysPre; ++q) v = j == q ? phys_pre[q] : v;
-            v = __shfl_sync(0xffffffffu, v, rel & 31);
-            if (j >= kPhysPre) v = __ldg(trow + table_slot(tile_block(it, tl0 + rel), p.n_sink, p.ring));
-            return v;
-        };
-        for (int32_t h = 0; h < n_half; ++h) {
-            const int32_t st = h % C::NSTAGE, k = h / C::NSTAGE;
-            if (k >= 1) mbar_wait(bar_ste(st), (k - 1) & 1);
-            const int32_t t0 = tl0 + h * C::KS;
-            const int32_t nt = min(C::KS, tl1 - t0);
-            if (lane == 0) mbar_expect_tx(bar_stf(st), (uint32_t)nt * C::kStageBlk);
             __syncwarp();
-            const int32_t phys = phys_of(h * C::KS + min(lane, nt - 1));        // (every lane takes part in the shuffle)
-            if (lane < nt)
-                bulk_g2s(sStage + st * C::kStageBytes + lane * C::kStageBlk, head_base + (int64_t)phys * p.L.block_bytes,
-                         C::kStageBlk, bar_stf(st));
+            named_arrive(1, C::kThreads);
+            const int32_t* trow = p.table + (int64_t)it.sid * p.tbl_width;
+            const uint8_t* head_base = p.kv_layer + (int64_t)kvh * p.L.head_bytes;
+            // physical block ids of this segment's tiles, fetched ONCE (lane l holds tiles l, l+32, ...)
+            constexpr int kPhysPre = 8;                               // 256 tiles; longer segments look up the rest
+            int32_t phys_pre[kPhysPre];
+    #pragma unroll
+            for (int j = 0; j < kPhysPre; ++j) {
+                const int32_t t = tl0 + j * 32 + lane;
+                phys_pre[j] = t < tl1 ? __ldg(trow + table_slot(tile_block(it, t), p.n_sink, p.ring)) : 0;
+            }
+            auto phys_of = [&](int32_t rel) {                         // rel = tile - tl0; rel >> 5 is warp-uniform
+                const int32_t j = rel >> 5;
+                int32_t v = phys_pre[0];
+    #pragma unroll
+                for (int q = 1; q < kPhysPre; ++q) v = j == q ? phys_pre[q] : v;
+                v = __shfl_sync(0xffffffffu, v, rel & 31);
+                if (j >= kPhysPre) v = __ldg(trow + table_slot(tile_block(it, tl0 + rel), p.n_sink, p.ring));
+                return v;
+            };
+            for (int32_t h = 0; h < n_half; ++h) {
+                const int32_t st = h % C::NSTAGE, k = h / C::NSTAGE;
+                if (k >= 1) mbar_wait(bar_ste(st), (k - 1) & 1);
+                const int32_t t0 = tl0 + h * C::KS;
+                const int32_t nt = min(C::KS, tl1 - t0);
+                if (lane == 0) mbar_expect_tx(bar_stf(st), (uint32_t)nt * C::kStageBlk);
+                __syncwarp();
+                const int32_t phys = phys_of(h * C::KS + min(lane, nt - 1));        // (every lane takes part in the shuffle)
+                if (lane < nt)
+                    bulk_g2s(sStage + st * C::kStageBytes + lane * C::kStageBlk, head_base + (int64_t)phys * p.L.block_bytes,
+                             C::kStageBlk, bar_stf(st));
+            }
+            return;
         }
-        return;
+        {
+            // ================================ MMA issuers ================================
+            // Warp 1 issues Q K^T for both slots, warps 2 / 3 issue P V of slot 0 / 1 (as in attend_umma.cuh).
+            const bool is_pv = warp >= 2;
+            const int32_t slot = is_pv ? warp - 2 : 0;
+            if (warp == 1) {
+                asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;"
+                             ::"r"(smem_u32(const_cast<uint32_t*>(tmem_slot))), "r"(C::kTmemCols));
+                asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+            }
+            tc_fence_before();
+            named_sync(1, C::kThreads);
+            tc_fence_after();
+            const uint32_t tmem = *tmem_slot;
+            constexpr uint32_t idesc_qk = umma_idesc_f16(C::KS * kBlockTokens, false);
+            constexpr uint32_t idesc_pv = umma_idesc_f16(D, true);
+            const uint32_t tSbase = tmem + C::kColS + 128 * slot, tOacc = tmem + C::kColO + D * slot;      // (P V warps)
+            auto wait_full = [&](int32_t e) {
+                mbar_wait(bar_full(e % C::NBUF), (e / C::NBUF) & 1);
+                tc_fence_after();
+            };
+            auto release = [&](int32_t e) { if (lane == 0) umma_commit(bar_empty(e % C::NBUF)); };
+            const uint32_t elect = lane == 0 ? 1u : 0u;
+            // S[buf] = Q K^T over the K half-stage in ring entry e
+            auto issue_qk = [&](int32_t qslot, int32_t buf, int32_t e) {
+                const uint64_t dq0 = umma_desc(sQ + qslot * C::kQBytes, 16, 1024);
+                const uint64_t dk0 = umma_desc(sRing + (e % C::NBUF) * C::kBufBytes, 16, 1024);
+                const uint32_t ts = tmem + C::kColS + 128 * qslot + 64 * buf;
+    #pragma unroll
+                for (int kk = 0; kk < D / 16; ++kk)
+                    umma_ss_e(ts, dq0 + (uint64_t)(((kk >> 2) * C::kQHalfBytes + (kk & 3) * 32) >> 4),
+                              dk0 + (uint64_t)(((kk >> 2) * C::kKHalfBytes + (kk & 3) * 32) >> 4), idesc_qk, kk > 0 ? 1u : 0u, elect);
+                if (lane == 0) umma_commit(bar_s(qslot, buf));
+                __syncwarp();
+            };
+            // O (+)= P V over the V half-stage in ring entry e: one K = 16 MMA per valid block; the fp16 P of block b
+            // sits in columns 32 (b / 2) + 8 (b % 2) .. + 7 of the S buffer
+            auto issue_pv = [&](int32_t buf, int32_t e, int32_t nt, bool accumulate) {
+                const uint64_t vd0 = umma_desc(sRing + (e % C::NBUF) * C::kBufBytes, 2048, 1024);
+                const uint32_t pa0 = tSbase + 64 * buf;
+    #pragma unroll
+                for (int b = 0; b < C::KS; ++b) {
+                    if (b < nt) {                             // (warp-uniform)
+                        const uint32_t pa = pa0 + 32 * (b >> 1) + 8 * (b & 1);
+                        const uint64_t vd = vd0 + (uint64_t)((b * C::kOpTile) >> 4);
+                        umma_ts_e(tOacc, pa, vd, idesc_pv, (accumulate || b > 0) ? 1u : 0u, elect);
+                    }
+                }
+                if (lane == 0) umma_commit(bar_pv(slot, buf));
+                __syncwarp();
+            };
+            if (!is_pv) {
+                // ---- Q K^T of every half-stage, for every slot: into S buffer h & 1 of the slot, as soon as P V of
+                // h - 2 has drained that buffer ----
+                for (int32_t h = 0; h < n_half; ++h) {
+                    const int32_t e = entry_k(h);
+                    wait_full(e);
+                    for (int32_t qs = 0; qs < n_slots; ++qs) {
+                        const int32_t buf = h & 1;
+                        if (h >= 2) {
+                            mbar_wait(bar_pv(qs, buf), ((h >> 1) - 1) & 1);
+                            tc_fence_after();
+                        }
+                        issue_qk(qs, buf, e);
+                        release(e);                          // (one arrival per consuming slot)
+                    }
+                }
+            } else if (slot < n_slots) {
+                // ---- P V: half-stage h out of S buffer h & 1, once the softmax has written P there ----
+                for (int32_t h = 0; h < n_half; ++h) {
+                    const int32_t e = entry_v(h), buf = h & 1;
+                    const int32_t nt = min(C::KS, tl1 - (tl0 + h * C::KS));
+                    wait_full(e);
+                    mbar_wait(bar_p(slot, buf), (h >> 1) & 1);
+                    tc_fence_after();
+                    issue_pv(buf, e, nt, h > 0);
+                    release(e);
+                    if (h == n_half - 1 && lane == 0) umma_commit(bar_o(slot));
+                }
+            }
+            if (warp == 1) {
+                // every softmax warp has finished reading TMEM
+                named_sync(2, 32 + 256);
+                tc_fence_after();
+                asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(C::kTmemCols));
+            }
+            return;
+        }
     }
     if (warp >= 12) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 104;");
         // ================================ converters ================================
         // Operand ring entry e = K or V of a half-stage, in the order the MMA issuers consume them.  The staging
         // entry of half-stage j is awaited at K(j) (always before V(j)) and handed back after V(j).
@@ -246,94 +341,7 @@ attend_umma_fp8_kernel(AttendParams p) {
         }
         return;
     }
-    if (warp >= 1 && warp <= 3) {
-        // ================================ MMA issuers ================================
-        // Warp 1 issues Q K^T for both slots, warps 2 / 3 issue P V of slot 0 / 1 (as in attend_umma.cuh).
-        const bool is_pv = warp >= 2;
-        const int32_t slot = is_pv ? warp - 2 : 0;
-        if (warp == 1) {
-            asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;"
-                         ::"r"(smem_u32(const_cast<uint32_t*>(tmem_slot))), "r"(C::kTmemCols));
-            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
-        }
-        tc_fence_before();
-        named_sync(1, C::kThreads);
-        tc_fence_after();
-        const uint32_t tmem = *tmem_slot;
-        constexpr uint32_t idesc_qk = umma_idesc_f16(C::KS * kBlockTokens, false);
-        constexpr uint32_t idesc_pv = umma_idesc_f16(D, true);
-        const uint32_t tSbase = tmem + C::kColS + 128 * slot, tOacc = tmem + C::kColO + D * slot;      // (P V warps)
-        auto wait_full = [&](int32_t e) {
-            mbar_wait(bar_full(e % C::NBUF), (e / C::NBUF) & 1);
-            tc_fence_after();
-        };
-        auto release = [&](int32_t e) { if (lane == 0) umma_commit(bar_empty(e % C::NBUF)); };
-        const uint32_t elect = lane == 0 ? 1u : 0u;
-        // S[buf] = Q K^T over the K half-stage in ring entry e
-        auto issue_qk = [&](int32_t qslot, int32_t buf, int32_t e) {
-            const uint64_t dq0 = umma_desc(sQ + qslot * C::kQBytes, 16, 1024);
-            const uint64_t dk0 = umma_desc(sRing + (e % C::NBUF) * C::kBufBytes, 16, 1024);
-            const uint32_t ts = tmem + C::kColS + 128 * qslot + 64 * buf;
-#pragma unroll
-            for (int kk = 0; kk < D / 16; ++kk)
-                umma_ss_e(ts, dq0 + (uint64_t)(((kk >> 2) * C::kQHalfBytes + (kk & 3) * 32) >> 4),
-                          dk0 + (uint64_t)(((kk >> 2) * C::kKHalfBytes + (kk & 3) * 32) >> 4), idesc_qk, kk > 0 ? 1u : 0u, elect);
-            if (lane == 0) umma_commit(bar_s(qslot, buf));
-            __syncwarp();
-        };
-        // O (+)= P V over the V half-stage in ring entry e: one K = 16 MMA per valid block; the fp16 P of block b
-        // sits in columns 32 (b / 2) + 8 (b % 2) .. + 7 of the S buffer
-        auto issue_pv = [&](int32_t buf, int32_t e, int32_t nt, bool accumulate) {
-            const uint64_t vd0 = umma_desc(sRing + (e % C::NBUF) * C::kBufBytes, 2048, 1024);
-            const uint32_t pa0 = tSbase + 64 * buf;
-#pragma unroll
-            for (int b = 0; b < C::KS; ++b) {
-                if (b < nt) {                             // (warp-uniform)
-                    const uint32_t pa = pa0 + 32 * (b >> 1) + 8 * (b & 1);
-                    const uint64_t vd = vd0 + (uint64_t)((b * C::kOpTile) >> 4);
-                    umma_ts_e(tOacc, pa, vd, idesc_pv, (accumulate || b > 0) ? 1u : 0u, elect);
-                }
-            }
-            if (lane == 0) umma_commit(bar_pv(slot, buf));
-            __syncwarp();
-        };
-        if (!is_pv) {
-            // ---- Q K^T of every half-stage, for every slot: into S buffer h & 1 of the slot, as soon as P V of
-            // h - 2 has drained that buffer ----
-            for (int32_t h = 0; h < n_half; ++h) {
-                const int32_t e = entry_k(h);
-                wait_full(e);
-                for (int32_t qs = 0; qs < n_slots; ++qs) {
-                    const int32_t buf = h & 1;
-                    if (h >= 2) {
-                        mbar_wait(bar_pv(qs, buf), ((h >> 1) - 1) & 1);
-                        tc_fence_after();
-                    }
-                    issue_qk(qs, buf, e);
-                    release(e);                          // (one arrival per consuming slot)
-                }
-            }
-        } else if (slot < n_slots) {
-            // ---- P V: half-stage h out of S buffer h & 1, once the softmax has written P there ----
-            for (int32_t h = 0; h < n_half; ++h) {
-                const int32_t e = entry_v(h), buf = h & 1;
-                const int32_t nt = min(C::KS, tl1 - (tl0 + h * C::KS));
-                wait_full(e);
-                mbar_wait(bar_p(slot, buf), (h >> 1) & 1);
-                tc_fence_after();
-                issue_pv(buf, e, nt, h > 0);
-                release(e);
-                if (h == n_half - 1 && lane == 0) umma_commit(bar_o(slot));
-            }
-        }
-        if (warp == 1) {
-            // every softmax warp has finished reading TMEM
-            named_sync(2, 32 + 256);
-            tc_fence_after();
-            asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(C::kTmemCols));
-        }
-        return;
-    }
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 168;");
 
     // ================================ softmax warps (4 .. 11) ================================
     const int32_t slot = (warp - 4) >> 2, quarter = warp & 3;       // TMEM lanes 32 (warp % 4) .. + 31
