@@ -534,7 +534,7 @@ def main():
     def kind_obj(kind):
         d = per_kind[kind]
         gbs = d["bytes"] / (d["ms"] * 1e-3) / 1e9
-        o = {"kernel": KIND_NAME[kind], "bound": "hbm", "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak,
+        o = {"kernel": "attend_umma_fp8_kernel" if (KV_FP8 and kind == 3) else KIND_NAME[kind], "bound": "hbm", "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak,
              "launches": d["launches"], "kernel_ms_avg": d["ms"] / d["launches"],
              "raw_span_ms_avg": d["span_ms"] / d["launches"],
              "algorithmic_bytes_per_launch": d["bytes"] / d["launches"], "share_of_step": d["ms"] / st_ms,
