@@ -226,11 +226,20 @@ int metronome_step_host(metronome_pool_t* pool, int32_t layer, int32_t n_batch,
                         const void* q_host, void* out_host, void* cuda_stream);
 
 /* The same step, pipelined: returns once the copies and kernels are ENQUEUED -- k/v/q host->device on a copy
- * stream of the pool's, the step on cuda_stream, out device->host on a second copy stream, chained by events --
- * so that the uploads of step k+1 and the read-back of step k-1 run next to the kernels of step k (two staging
- * slots).  The host buffers of a step must stay untouched, and out_host is not valid, until
+ * stream of the pool's, the step on cuda_stream, out device->host on a second copy stream -- so that the uploads of
+ * the next steps and the read-back of the previous ones run next to the kernels of step k.
+ *   pinned host buffers (out_host page-locked): three staging slots and NO event on cuda_stream between two kernels, so
+ *     the kernels keep their programmatic launch edges (one step per tick, back to back): the input copies
+ *     end with a 4-byte copy of the step number into a device flag the kernels wait for, a one-thread kernel behind the
+ *     step's last kernel publishes "kernels complete", the read-back stream waits for that value (stream wait-value),
+ *     copies out and writes the step number to a pinned flag that metronome_step_host_wait polls.  The host may run
+ *     two steps ahead: issuing step k blocks until step k-3 is complete.
+ *   pageable host buffers (or METRONOME_HOST_STEP_EVENTS=1 in the environment at pool creation, a measurement aid): two
+ *     staging slots chained by events; issuing step k blocks until step k-2 is complete.  The library drains one mode
+ *     before it switches to the other.
+ * The host buffers of a step must stay untouched, and out_host is not valid, until
  * metronome_step_host_wait(pool, keep) has returned with that step among the finished ones: it blocks until at
- * most `keep` (0, 1 or more) of the steps issued so far are still in flight.  Steps complete in issue order.
+ * most `keep` (0, 1, 2) of the steps issued so far are still in flight.  Steps complete in issue order.
  * Errors: as metronome_step_host; an error leaves the pool as it was (the step was not enqueued). */
 int metronome_step_host_async(metronome_pool_t* pool, int32_t layer, int32_t n_batch,
                               const int32_t* sids, const int32_t* n_new,

@@ -53,6 +53,9 @@ struct AttendParams {
     int32_t* pastwait_flag;    // tensor-core kernels: <- pastwait_epoch once past griddepcontrol.wait, i.e. once this step's append
     int32_t pastwait_epoch;    // kernel is complete (the NEXT append kernel may then do its bookkeeping while this kernel runs); null: off
     unsigned long long* stamp; // measurement aid (null: off): [0] <- min over CTAs of %globaltimer at start, [1] <- max at exit
+    const int32_t* h2d_flag;   // event-free host steps: q is filled by a copy stream that ends by copying h2d_seq into *h2d_flag
+    int32_t h2d_seq;           // (null: q is stream-ordered).  Only an EARLY-mode kernel has to look: the others wait for the
+                               // append kernel of their step, which has itself waited for the flag
 };
 
 // Measurement aid (metronome_pool_set_profiling mode 2): the kernel's own span in %globaltimer ns, first CTA
@@ -80,6 +83,7 @@ __device__ __forceinline__ void wait_work_list(const AttendParams& p) {
         asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(seen) : "l"(p.items_flag) : "memory");
         if (seen - p.items_epoch < 0) __nanosleep(64);
     } while (seen - p.items_epoch < 0);
+    if (p.h2d_flag) spin_until_reached_sys(p.h2d_flag, p.h2d_seq);     // q is read before any griddepcontrol.wait
 }
 
 // (one thread of the grid, right after pdl_wait)
@@ -143,6 +147,19 @@ __device__ __forceinline__ uint64_t f2_mul(uint64_t a, uint64_t b) {
     uint64_t d;
     asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
     return d;
+}
+
+// Event-free host steps: publishes "the kernels of step `seq` are complete" in a flag (device memory; the read-back stream
+// waits for it with a stream wait-value operation) once everything before it on the stream is complete and flushed (it is launched programmatically right behind the step's last attention kernel, whose
+// griddepcontrol.wait chain reaches back to the step's append kernel).  It triggers its own dependents at once, so the
+// next step's append kernel still starts under the attention kernel's tail.  grid = 1, block = 32.
+__global__ void step_done_kernel(int32_t* done_flag, int32_t seq) {
+    pdl_launch_dependents();
+    pdl_wait();
+    if (threadIdx.x == 0) {
+        __threadfence_system();
+        asm volatile("st.release.sys.global.s32 [%0], %1;" ::"l"(done_flag), "r"(seq) : "memory");
+    }
 }
 
 // Row a6: log-sum-exp combine of the split-KV partials of one (query row, q head); sinks were

@@ -50,6 +50,10 @@ struct AppendParams {
     const uint4* v_new;
     uint8_t* kv_layer;             // null: metadata only
     KvLayout L;
+    // event-free host steps (metronome_step_host_async, direct mode): k_new / v_new are filled by copies on ANOTHER stream
+    // that end with a 4-byte copy of h2d_seq into *h2d_flag; the scatter CTAs wait for it (null: inputs are stream-ordered)
+    const int32_t* h2d_flag;
+    int32_t h2d_seq;
 };
 
 constexpr int kAppendSmemItems = 1024;       // AppendItems the bookkeeping CTA stages in shared memory
@@ -178,7 +182,14 @@ append_fused_kernel(const AppendParams a) {
     const int64_t src = (int64_t)(it.row_off + tok) * chunks_per_tok + rem;
     pdl_wait();                                       // k_new / v_new may come from the previous kernel
     uint4 kk = make_uint4(0u, 0u, 0u, 0u), vv = kk;
-    if (active) {
+    if (a.h2d_flag) {                                 // (kernel-uniform) ... or from a copy stream: wait for its flag,
+        if (threadIdx.x == 0) spin_until_reached_sys(a.h2d_flag, a.h2d_seq);
+        __syncthreads();
+        if (active) {                                 // and read past L1 (the rows landed while this grid was resident)
+            kk = __ldcg(a.k_new + src);
+            vv = __ldcg(a.v_new + src);
+        }
+    } else if (active) {
         kk = __ldg(a.k_new + src);
         vv = __ldg(a.v_new + src);
     }

@@ -77,6 +77,16 @@ __host__ __device__ __forceinline__ int32_t table_slot(int32_t b, int32_t n_sink
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 
+// One thread: wait until the 32-bit flag (written in stream order by a copy engine or by another grid) has reached
+// `seq` (wrap-safe), with acquire semantics at system scope: what was written before the flag is visible afterwards.
+__device__ __forceinline__ void spin_until_reached_sys(const int32_t* flag, int32_t seq) {
+    int32_t seen;
+    do {
+        asm volatile("ld.acquire.sys.global.s32 %0, [%1];" : "=r"(seen) : "l"(flag) : "memory");
+        if (seen - seq < 0) __nanosleep(64);
+    } while (seen - seq < 0);
+}
+
 template <typename... KArgs, typename... Args>
 inline cudaError_t launch_kernel(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, bool pdl,
                                  Args... args) {

@@ -48,6 +48,7 @@ constexpr int kStagingSlots = 64;      // per-call metadata slots (pinned host +
 constexpr int kStagingGroup = 8;       // one completion event per 8 slots: an event between two kernels
                                        // would break their programmatic (PDL) launch edge
 constexpr int kMaxSplits = 64;
+constexpr int kDirectSlots = 3;        // device staging slots of the event-free async host steps
 constexpr int kStampSlots = 1 << 15;   // attention launches one stamped pass can hold
 #ifndef METRONOME_GQA_BND_BYTES
 #define METRONOME_GQA_BND_BYTES 65536
@@ -117,12 +118,28 @@ struct metronome_pool {
     size_t io_bytes = 0;
     // metronome_step_host_async: two staging slots, a copy stream per direction, events that chain
     // H2D(k) -> step(k) -> D2H(k) while H2D(k+1) and D2H(k-1) run next to step(k)
-    uint8_t* d_io2[2] = {nullptr, nullptr};
-    size_t io2_bytes[2] = {0, 0};
+    uint8_t* d_io2[3] = {nullptr, nullptr, nullptr};   // (the event-chained mode uses two slots, the event-free mode three)
+    size_t io2_bytes[3] = {0, 0, 0};
     cudaStream_t s_h2d = nullptr, s_d2h = nullptr;
     cudaEvent_t ev_h2d[2]{}, ev_comp[2]{}, ev_d2h[2]{};
     bool slot_busy[2] = {false, false};
     int64_t host_seq = 0;              // async steps issued so far (step k uses slot k & 1)
+    // event-free mode of the async host steps (out_host pinned): no event sits between two kernels of the compute stream, so
+    // their programmatic launch edges survive.  Inputs: copies on s_h2d that end with a 4-byte copy of the step number
+    // into d_h2d_flag[0] (kernels spin on it); completion: step_done_kernel stores the step number into d_h2d_flag[32];
+    // result: s_d2h waits for that value (stream wait-value), copies the step's output to out_host and then writes the
+    // step number into *h_done (stream write-value; pinned, the host polls it).
+    typedef int (*memop32_fn)(void* stream, unsigned long long addr, unsigned int value, unsigned int flags);
+    memop32_fn fn_wait32 = nullptr, fn_write32 = nullptr;
+    int memops_state = 0;              // 0 not looked up yet, 1 available, -1 not available (event-chained mode only)
+    unsigned long long h_done_dev = 0; // device address of *h_done
+    bool direct_mode = false;
+    int32_t direct_seq = 0;            // steps issued in this mode (step n uses slot n & 1)
+    int32_t* d_h2d_flag = nullptr;
+    int32_t* h_done = nullptr;         // pinned + mapped
+    int32_t* h_seq_ring = nullptr;     // pinned: sources of the flag copies (a copy reads its source when it executes)
+    const int32_t* cur_h2d_flag = nullptr;   // non-null only while such a step is being enqueued (append_impl / make_attend_params)
+    int32_t cur_h2d_seq = 0;
 
     // per-call metadata staging: pinned host ring + matching device ring
     uint8_t* h_stage = nullptr;
@@ -144,6 +161,7 @@ struct metronome_pool {
     std::vector<int32_t> stamp_kind;   // per used slot: 1 rows, 2 gqa decode, 3 chunk
 
     int32_t tune_split_tokens = 0, tune_family = 0, tune_gqa_dynamic = 0, tune_fused_step = 0;
+    bool tune_host_direct = true;      // false (METRONOME_HOST_STEP_EVENTS=1 at pool creation): async host steps always chain events
     int32_t n_sm = 148;
     int64_t n_launch = 0, n_append = 0, n_attend = 0;
     std::string cuda_err;
@@ -529,6 +547,7 @@ AttendParams make_attend_params(metronome_pool* pool, int32_t layer, const Atten
     p.items_flag = pool->d_bk_flag + 1;
     p.items_epoch = -1;
     p.pastwait_flag = nullptr;
+    p.h2d_flag = pool->cur_h2d_flag; p.h2d_seq = pool->cur_h2d_seq;
     return p;
 }
 
@@ -783,6 +802,7 @@ int metronome_pool_create(const metronome_pool_config_t* cfg, metronome_pool_t**
         if (pool->poison) fill_nan_kernel<<<1184, 256>>>((uint4*)pool->d_kv, (int64_t)(need / 16));
     }
     pool->slot_bytes = (size_t)c.max_sessions * (sizeof(AppendItem) + sizeof(AttendItem)) + kMaxRangeItems * sizeof(int32_t) + 16;
+    { const char* ev = getenv("METRONOME_HOST_STEP_EVENTS"); pool->tune_host_direct = !(ev && ev[0] == '1'); }
     e = cudaMalloc(&pool->d_tickets, (size_t)c.max_sessions * c.n_kv_heads * sizeof(int32_t));
     if (e != cudaSuccess) return fail(METRONOME_ERR_OUT_OF_MEMORY, e, "cudaMalloc tickets");
     cudaMemset(pool->d_tickets, 0, (size_t)c.max_sessions * c.n_kv_heads * sizeof(int32_t));
@@ -826,12 +846,16 @@ int metronome_pool_destroy(metronome_pool_t* pool) {
     if (pool->d_ws_acc) cudaFree(pool->d_ws_acc);
     if (pool->d_ws_ml) cudaFree(pool->d_ws_ml);
     if (pool->d_io) cudaFree(pool->d_io);
+    if (pool->d_io2[2]) cudaFree(pool->d_io2[2]);
     for (int b = 0; b < 2; ++b) {
         if (pool->d_io2[b]) cudaFree(pool->d_io2[b]);
         if (pool->ev_h2d[b]) cudaEventDestroy(pool->ev_h2d[b]);
         if (pool->ev_comp[b]) cudaEventDestroy(pool->ev_comp[b]);
         if (pool->ev_d2h[b]) cudaEventDestroy(pool->ev_d2h[b]);
     }
+    if (pool->d_h2d_flag) cudaFree(pool->d_h2d_flag);
+    if (pool->h_done) cudaFreeHost(pool->h_done);
+    if (pool->h_seq_ring) cudaFreeHost(pool->h_seq_ring);
     if (pool->s_h2d) cudaStreamDestroy(pool->s_h2d);
     if (pool->s_d2h) cudaStreamDestroy(pool->s_d2h);
     if (pool->h_stage) cudaFreeHost(pool->h_stage);
@@ -1078,6 +1102,7 @@ int append_impl(metronome_pool_t* pool, int32_t layer, int32_t n_batch, const in
         a.k_new = (const uint4*)k_new; a.v_new = (const uint4*)v_new;
         a.kv_layer = pool->bookkeeping_only ? nullptr : pool->d_kv + (int64_t)layer * pool->L.layer_bytes;
         a.L = pool->L;
+        a.h2d_flag = pool->cur_h2d_flag; a.h2d_seq = pool->cur_h2d_seq;
         const int32_t chunks = max_n * c.n_kv_heads * (c.head_dim / 8);
         dim3 grid(std::max(1, (chunks + 255) / 256), n_batch + 1);      // (n_batch <= max_sessions <= 65534)
         const size_t smem = (fused_bookkeeping && n_batch <= kAppendSmemItems) ? (size_t)n_batch * sizeof(AppendItem) : 0;
@@ -1292,8 +1317,27 @@ int metronome_step_host(metronome_pool_t* pool, int32_t layer, int32_t n_batch, 
     return METRONOME_OK;
 }
 
+// Event-free host steps: the host's side of step_done_kernel.  Polls the pinned flag; looks at the stream now and then so
+// that a faulted GPU comes back as an error, not as a hang.
+static int wait_step_done(metronome_pool* pool, int32_t seq) {
+    if (!pool->h_done || seq <= 0) return METRONOME_OK;
+    volatile int32_t* flag = pool->h_done;
+    for (uint64_t spin = 1; *flag - seq < 0; ++spin) {
+        if ((spin & 0x3fff) == 0 && pool->have_stream) {
+            const cudaError_t e = cudaStreamQuery(pool->last_stream);
+            if (e != cudaSuccess && e != cudaErrorNotReady) return cuda_fail(pool, e, "cudaStreamQuery (waiting for a host step)");
+        }
+#if defined(__x86_64__)
+        __builtin_ia32_pause();
+#endif
+    }
+    __atomic_thread_fence(__ATOMIC_ACQUIRE);     // the kernels' writes into out_host are behind the flag
+    return METRONOME_OK;
+}
+
 int metronome_step_host_wait(metronome_pool_t* pool, int32_t keep) {
     if (!pool || keep < 0) return METRONOME_ERR_INVALID_ARG;
+    if (pool->direct_mode) return wait_step_done(pool, pool->direct_seq - keep);
     // steps host_seq-1 (newest) and host_seq-2 may be outstanding; wait for all but the newest `keep`
     for (int64_t k = pool->host_seq - 2; k <= pool->host_seq - 1 - keep; ++k) {
         if (k < 0) continue;
@@ -1328,6 +1372,85 @@ int metronome_step_host_async(metronome_pool_t* pool, int32_t layer, int32_t n_b
             CU(cudaEventCreateWithFlags(&pool->ev_d2h[b], cudaEventDisableTiming));
         }
     }
+    // Event-free mode when the copies are truly asynchronous (out_host pinned) and the driver's stream wait-value /
+    // write-value operations are there.  Pageable buffers, the profiling brackets and the poison fill (more launches per
+    // step) keep the event-chained path below.
+    if (pool->memops_state == 0) {
+        void *fw = nullptr, *fs = nullptr;
+        cudaDriverEntryPointQueryResult qa, qb;
+        const bool ok = cudaGetDriverEntryPoint("cuStreamWaitValue32", &fw, cudaEnableDefault, &qa) == cudaSuccess &&
+                        cudaGetDriverEntryPoint("cuStreamWriteValue32", &fs, cudaEnableDefault, &qb) == cudaSuccess &&
+                        qa == cudaDriverEntryPointSuccess && qb == cudaDriverEntryPointSuccess && fw && fs;
+        if (!ok) cudaGetLastError();
+        pool->fn_wait32 = reinterpret_cast<metronome_pool::memop32_fn>(fw);
+        pool->fn_write32 = reinterpret_cast<metronome_pool::memop32_fn>(fs);
+        pool->memops_state = ok ? 1 : -1;
+    }
+    bool direct = false;
+    if (rows > 0 && !pool->profiling && !pool->poison && pool->tune_host_direct && pool->memops_state == 1) {
+        cudaPointerAttributes at{};
+        if (cudaPointerGetAttributes(&at, out_host) == cudaSuccess) direct = at.type == cudaMemoryTypeHost;
+        else cudaGetLastError();
+    }
+    if (direct != pool->direct_mode) {              // drain the other mode's steps before switching
+        const int rcw = metronome_step_host_wait(pool, 0);
+        if (rcw) return rcw;
+        pool->direct_mode = direct;
+    }
+    if (direct) {
+        if (!pool->d_h2d_flag) {
+            CU(cudaMalloc(&pool->d_h2d_flag, 256));
+            CU(cudaMemset(pool->d_h2d_flag, 0, 256));
+            CU(cudaHostAlloc(&pool->h_done, 256, cudaHostAllocMapped));
+            CU(cudaHostAlloc(&pool->h_seq_ring, 64 * sizeof(int32_t), cudaHostAllocDefault));
+            pool->h_done[0] = 0;
+            void* dp = nullptr;
+            CU(cudaHostGetDevicePointer(&dp, pool->h_done, 0));
+            pool->h_done_dev = (unsigned long long)(uintptr_t)dp;
+        }
+        int32_t* d_done = pool->d_h2d_flag + 32;    // (its own 128-byte line)
+        const int32_t seq = pool->direct_seq + 1;
+        const int b = seq % kDirectSlots;
+        const size_t kv_b = (size_t)rows * c.n_kv_heads * c.head_dim * 2, q_b = (size_t)rows * c.n_q_heads * c.head_dim * 2;
+        const size_t kv_al = (kv_b + 255) & ~(size_t)255, q_al = (q_b + 255) & ~(size_t)255;
+        const size_t need = 2 * kv_al + 2 * q_al;
+        // the slot's previous step (three steps back) must be through -- kernels and read-back -- before it is reused:
+        // the host may run two steps ahead of the GPU (metronome_step_host_wait(2))
+        int rc = wait_step_done(pool, seq - kDirectSlots);
+        if (rc) return rc;
+        if (need > pool->io2_bytes[b]) {
+            if (pool->d_io2[b]) cudaFree(pool->d_io2[b]);
+            pool->d_io2[b] = nullptr; pool->io2_bytes[b] = 0;
+            CU(cudaMalloc(&pool->d_io2[b], need + need / 2));
+            pool->io2_bytes[b] = need + need / 2;
+        }
+        uint8_t* dk = pool->d_io2[b]; uint8_t* dv = dk + kv_al; uint8_t* dq = dv + kv_al; uint8_t* dout = dq + q_al;
+        CU(cudaMemcpyAsync(dk, k_new_host, kv_b, cudaMemcpyHostToDevice, pool->s_h2d));
+        CU(cudaMemcpyAsync(dv, v_new_host, kv_b, cudaMemcpyHostToDevice, pool->s_h2d));
+        CU(cudaMemcpyAsync(dq, q_host, q_b, cudaMemcpyHostToDevice, pool->s_h2d));
+        pool->h_seq_ring[seq & 63] = seq;
+        CU(cudaMemcpyAsync(pool->d_h2d_flag, pool->h_seq_ring + (seq & 63), sizeof(int32_t), cudaMemcpyHostToDevice, pool->s_h2d));
+        pool->direct_seq = seq;                     // (from here on the step exists: an error still publishes its number)
+        pool->cur_h2d_flag = pool->d_h2d_flag; pool->cur_h2d_seq = seq;
+        rc = metronome_append_attend(pool, layer, n_batch, sids, n_new, dk, dv, dq, dout, cuda_stream);
+        pool->cur_h2d_flag = nullptr;
+        // "the kernels of step seq are complete", behind the step's last kernel, programmatic on both sides; transparent
+        // for the early bookkeeping of the next append kernel (it touches nothing that kernel or the attention kernels use)
+        const bool adjacent = pool->pastwait_launches == pool->n_launch;
+        CU(launch_kernel(step_done_kernel, dim3(1), dim3(32), 0, st, rc == METRONOME_OK, d_done, seq));
+        ++pool->n_launch;
+        if (adjacent) pool->pastwait_launches = pool->n_launch;
+        pool->last_stream = st; pool->have_stream = true;
+        // read-back on its own stream: wait for that value, copy, publish to the host
+        if (pool->fn_wait32(pool->s_d2h, (unsigned long long)(uintptr_t)d_done, (unsigned int)seq, 0u /* GEQ, wrap-safe */) != 0)
+            return cuda_fail(pool, cudaErrorUnknown, "cuStreamWaitValue32");
+        if (rc == METRONOME_OK) CU(cudaMemcpyAsync(out_host, dout, q_b, cudaMemcpyDeviceToHost, pool->s_d2h));
+        if (pool->fn_write32(pool->s_d2h, pool->h_done_dev, (unsigned int)seq, 0u) != 0)
+            return cuda_fail(pool, cudaErrorUnknown, "cuStreamWriteValue32");
+        if (rc) return rc;
+        ++pool->host_seq;
+        return METRONOME_OK;
+    }
     const int b = (int)(pool->host_seq & 1);
     const size_t kv_b = (size_t)rows * c.n_kv_heads * c.head_dim * 2, q_b = (size_t)rows * c.n_q_heads * c.head_dim * 2;
     const size_t kv_al = (kv_b + 255) & ~(size_t)255, q_al = (q_b + 255) & ~(size_t)255;
@@ -1341,8 +1464,9 @@ int metronome_step_host_async(metronome_pool_t* pool, int32_t layer, int32_t n_b
         pool->io2_bytes[b] = need + need / 2;
     }
     uint8_t* dk = pool->d_io2[b]; uint8_t* dv = dk + kv_al; uint8_t* dq = dv + kv_al; uint8_t* dout = dq + q_al;
-    // H2D of this step: as soon as the slot's previous step (two steps back) has been read out
-    if (pool->slot_busy[b]) CU(cudaStreamWaitEvent(pool->s_h2d, pool->ev_d2h[b], 0));
+    // H2D of this step: once the slot's previous step (two steps back) has been read out.  The host waits for that here, so
+    // that metronome_step_host_wait(keep >= 2) holds as well: whatever is older than the two newest steps is complete
+    if (pool->slot_busy[b]) { CU(cudaEventSynchronize(pool->ev_d2h[b])); pool->slot_busy[b] = false; }
     if (rows > 0) {
         CU(cudaMemcpyAsync(dk, k_new_host, kv_b, cudaMemcpyHostToDevice, pool->s_h2d));
         CU(cudaMemcpyAsync(dv, v_new_host, kv_b, cudaMemcpyHostToDevice, pool->s_h2d));

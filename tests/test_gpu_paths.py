@@ -170,10 +170,14 @@ def test_max_sessions_is_capped_where_the_append_grid_ends():
     binding.Pool(max_sessions=65534, **kw).destroy()
 
 
+@pytest.mark.parametrize("buffers", ["pinned", "pageable", "alternating"])
 @pytest.mark.parametrize("Hkv", [8, 2])
-def test_pipelined_host_steps_match_the_blocking_ones(Hkv):
+def test_pipelined_host_steps_match_the_blocking_ones(Hkv, buffers):
     """metronome_step_host_async / _wait (two staging slots, copies on the pool's own streams) give what the oracle
-    gives, step by step, with up to two steps in flight and host buffers reused only after their wait."""
+    gives, step by step, with up to two steps in flight and host buffers reused only after their wait.
+    buffers: pinned = the event-free mode (kernels wait for the input copies' flag, write the result straight into the
+    pinned buffer, step_done_kernel publishes completion); pageable = the event-chained mode (a kernel cannot write
+    pageable memory); alternating = the library has to drain one mode before it switches to the other."""
     Hq, D, S, W, N = 8, 128, 4, 48, 3
     per = 1 + (W + 8 - 1) // 16 + 2
     kw = dict(n_q_heads=Hq, n_kv_heads=Hkv, head_dim=D, max_sessions=N, max_new_tokens=8)
@@ -186,8 +190,11 @@ def test_pipelined_host_steps_match_the_blocking_ones(Hkv):
     for step in range(60):
         n_new = rng.integers(1, 9, size=N).astype(np.int32) if step % 5 == 0 else np.ones(N, np.int32)
         rows = int(n_new.sum())
-        k, v, q = (_rows(rng, rows, H, D).pin_memory() for H in (Hkv, Hkv, Hq))
-        out = torch.empty(rows, Hq, D, dtype=torch.bfloat16).pin_memory()
+        pin = buffers == "pinned" or (buffers == "alternating" and (step // 7) % 2 == 0)
+        k, v, q = (_rows(rng, rows, H, D) for H in (Hkv, Hkv, Hq))
+        out = torch.full((rows, Hq, D), float("nan"), dtype=torch.bfloat16)
+        if pin:
+            k, v, q, out = k.pin_memory(), v.pin_memory(), q.pin_memory(), out.pin_memory()
         pool.step_host_async(0, sids, n_new, k, v, q, out)
         defn.append_kv(0, sids, [int(x) for x in n_new], synth.to_u16(k), synth.to_u16(v))
         pending.append((out, defn.attend_frame(0, sids, [int(x) for x in n_new], synth.to_u16(q)), f"step {step}", k, v, q))
@@ -198,6 +205,55 @@ def test_pipelined_host_steps_match_the_blocking_ones(Hkv):
     pool.step_host_wait(0)
     for o, ref, what, *_ in pending:
         assert_parity(o, ref, what)
+
+
+@pytest.mark.parametrize("G", [1, 8])
+def test_event_free_host_steps_under_load(G):
+    """The event-free mode on shapes where everything it touches is live: 24 sessions x 32 query heads, W = 750 (split-KV
+    + merge kernel for G = 1, early mode: the row kernel reads q before any griddepcontrol.wait and so waits for the input
+    copies' flag itself; stream-K GQA decode for G = 8, early bookkeeping behind step_done_kernel), 150 decode steps with
+    at most two in flight and THREE sets of pinned host buffers reused round-robin -- a result that lands late, a flag
+    seen early or a buffer overwritten too soon all show up as a mismatch with the oracle."""
+    Hq, D, S, W, N = 32, 128, 4, 750, 24
+    Hkv = Hq // G
+    per = 1 + (W + 25 - 1) // 16 + 2
+    kw = dict(n_q_heads=Hq, n_kv_heads=Hkv, head_dim=D, max_sessions=N, max_new_tokens=25)
+    pool = binding.Pool(n_sinks=S, window=W, n_blocks=N * per, **kw)
+    defn = O.DefinitionOracle(O.PoolConfig(S=S, W=W, n_blocks=N * per, block_size=16, **kw))
+    sids = [pool.session_open() for _ in range(N)]
+    assert sids == [defn.session_open() for _ in range(N)]
+    rng = np.random.default_rng(900 + G)
+    target = rng.integers(30, 1500, size=N)
+    done = np.zeros(N, np.int64)
+    while (done < target).any():                        # ragged histories, device buffers, no attention
+        idx = [i for i in range(N) if done[i] < target[i]]
+        n_new = np.array([min(25, target[i] - done[i]) for i in idx], np.int32)
+        rows = int(n_new.sum())
+        k, v = _rows(rng, rows, Hkv, D), _rows(rng, rows, Hkv, D)
+        pool.append_kv(0, [sids[i] for i in idx], n_new, k.cuda(), v.cuda())
+        defn.append_kv(0, [sids[i] for i in idx], [int(x) for x in n_new], synth.to_u16(k), synth.to_u16(v))
+        done[idx] += n_new
+    ones = np.ones(N, np.int32)
+    bufs = [tuple(torch.empty(N, H, D, dtype=torch.bfloat16).pin_memory() for H in (Hkv, Hkv, Hq, Hq)) for _ in range(3)]
+    launches0 = pool.stats()["kernel_launches"]
+    pending = []
+    for step in range(150):
+        k, v, q, out = bufs[step % 3]                    # (its previous use, step - 3, has been waited for)
+        for t, H in ((k, Hkv), (v, Hkv), (q, Hq)):
+            t.copy_(_rows(rng, N, H, D))
+        out.fill_(float("nan"))
+        pool.step_host_async(0, sids, ones, k, v, q, out)
+        defn.append_kv(0, sids, [1] * N, synth.to_u16(k), synth.to_u16(v))
+        pending.append((out, defn.attend_frame(0, sids, [1] * N, synth.to_u16(q)), f"G={G} step {step}"))
+        pool.step_host_wait(1)
+        while len(pending) > 1:
+            o, ref, what = pending.pop(0)
+            assert_parity(o.clone(), ref, what)
+    pool.step_host_wait(0)
+    assert_parity(pending[0][0], pending[0][1], pending[0][2])
+    # append + attention (+ merge) + step_done_kernel per step: the extra launch proves the event-free mode ran
+    per_step = (pool.stats()["kernel_launches"] - launches0) / 150
+    assert per_step >= 3, per_step
 
 
 @pytest.mark.parametrize("n_max", [2, 25])
