@@ -681,10 +681,19 @@ attend_gqa_kernel(AttendParams p, GqaPlan plan) {
         // this warp's tiles: a + warp, a + warp + 4, ...   (private ring, prologue fills NS stages)
         const int32_t n_mine = (b - a - warp + C::NWARP - 1) / C::NWARP;
         const int32_t sbase = pre ? C::kPre : 0;   // k-th tile of this warp -> stage (k + sbase) % NS
-        auto issue = [&](int32_t k) {
+        // Physical block ids of this warp's tiles, fetched 32 at a time (lane j: the warp's tiles j and 32 + j of the
+        // piece) and handed out by shuffle: a refill is then shuffle -> bulk copy instead of logical block -> table slot
+        // (an integer modulo) -> dependent table load (an L2 round trip) -> bulk copy, by one lane, for every tile.
+        // A piece of more than 64 tiles per warp (W > 4096) looks the rest up one by one.
+        auto lookup = [&](int32_t k) {
+            return __ldg(trow + table_slot(tile_block(it, a + warp + k * C::NWARP), p.n_sink, p.ring));
+        };
+        const int32_t phys_c0 = lane < n_mine ? lookup(lane) : 0;
+        const int32_t phys_c1 = lane + 32 < n_mine ? lookup(lane + 32) : 0;
+        auto issue = [&](int32_t k) {                      // (all lanes)
+            int32_t phys = __shfl_sync(0xffffffffu, (k & 32) ? phys_c1 : phys_c0, k & 31);
+            if (k >= 64) phys = lookup(k);
             if (lane == 0) {
-                const int32_t tile = a + warp + k * C::NWARP;
-                const int32_t phys = __ldg(trow + table_slot(tile_block(it, tile), p.n_sink, p.ring));
                 const int32_t st = (k + sbase) % C::NS;
                 const uint32_t bar = bars + 8 * st;
                 mbar_expect_tx(bar, C::kHeadBytes);
