@@ -300,9 +300,9 @@ struct WarpTile {
 //     to fp16 (exact for every element within 2^-14 of the row's maximum, 2^-25 absolute below);
 //   * O = sum_j (p_j * vs_j / vref) C_V[j] * vref: the V scale of key j is folded into the softmax weight before it
 //     is rounded to fp16 (11 bits: no hi / lo split as in the bf16 tile), relative to a running reference vref >= every
-//     V scale seen so far and times 2^15, so the weights stay in [0, 2^13] whatever the magnitude of V and keep full
-//     fp16 precision down to p_j vs_j = 2^-29 vref (a one-hot row on a key whose V is 10^5 times smaller than its
-//     neighbours' still comes out to 11 bits); O is rescaled when vref grows (warp-uniform, rare: vref is raised with
+//     V scale seen so far and times 2^9, so the weights stay in [0, 2^15] whatever the magnitude of V (p_j reaches 2^6
+//     under the lazily updated row maximum, vs_j / vref reaches 1) and keep full fp16 precision down to p_j vs_j = 2^-23 vref (a one-hot row
+//     on a key whose V is 10^5 times smaller than its neighbours' still comes out to 11 bits); O is rescaled when vref grows (warp-uniform, rare: vref is raised with
 //     a factor 4 of headroom); the denominator is summed in fp32 from the unrounded p_j, each thread its own four
 //     keys of a tile, reduced over the quad once at the end.
 // Fragments without a transposing load: a k16 step of Q K^T takes 16-byte chunk c of the K rows (ldmatrix on code
@@ -314,8 +314,11 @@ struct WarpTileF8 {
     static constexpr int KSTEPS = D / 16;
     static constexpr int NT = D / 8;
     static constexpr int kTileBytes = kBlockTokens * D;
+    // fp16 weight = p (<= 2^6, lazy reference) x vs / vref (<= 1: vref is only raised when a scale exceeds it)
+    // x kWScale <= 2^15 < 65504; full fp16 precision down to p vs / vref = 2^-23
+    static constexpr float kWScale = 512.f;
     uint32_t qa[KSTEPS][4];
-    float o[NT][4];                          // [j][e] rows a (e = 0, 1) / b (e = 2, 3): dim (D/4) t + (e & 1) NT + j, in units of vref / 2^15
+    float o[NT][4];                          // [j][e] rows a (e = 0, 1) / b (e = 2, 3): dim (D/4) t + (e & 1) NT + j, in units of vref / 2^9
     float m_a, m_b;
     float lsum[4];                           // [0] row a, [2] row b: this thread's own keys only (see quad_sum)
     float qs_a, qs_b;                        // scale_log2 * 2^e of the row's Q prescale
@@ -431,7 +434,12 @@ struct WarpTileF8 {
         mx_a = fmaxf(mx_a, __shfl_xor_sync(0xffffffffu, mx_a, 2));
         mx_b = fmaxf(mx_b, __shfl_xor_sync(0xffffffffu, mx_b, 1));
         mx_b = fmaxf(mx_b, __shfl_xor_sync(0xffffffffu, mx_b, 2));
-        const float mn_a = fmaxf(m_a, mx_a), mn_b = fmaxf(m_b, mx_b);
+        // lazy reference: a row keeps its stale maximum while the true one is within 2^kLazy of it (its weights then
+        // reach 2^kLazy instead of 1, which the fp16 weight factor below leaves room for); the 4 NT accumulators are
+        // rescaled on ~1 tile in 20 instead of 2 in 3 (8 rows, each with a new maximum every few tiles)
+        constexpr float kLazy = 6.f;
+        const bool need_a = mx_a > m_a + kLazy, need_b = mx_b > m_b + kLazy;        // (-inf + 6 = -inf: the first key counts)
+        const float mn_a = need_a ? mx_a : m_a, mn_b = need_b ? mx_b : m_b;
         // ---- V scales: rows past the session's length hold stale / poisoned bytes ----
         const int32_t nvalid = len - p0;                     // < 16 only in the session's last block
         if (nvalid < kBlockTokens) {
@@ -442,14 +450,14 @@ struct WarpTileF8 {
         vmax = fmaxf(vmax, __shfl_xor_sync(0xffffffffu, vmax, 1));
         vmax = fmaxf(vmax, __shfl_xor_sync(0xffffffffu, vmax, 2));       // (the same in every quad: warp-uniform)
         const bool grow = vmax > vref;
-        if (grow || __any_sync(0xffffffffu, (mn_a != m_a) || (mn_b != m_b))) {
+        if (grow || __any_sync(0xffffffffu, need_a || need_b)) {
             float ca = mn_a == -INFINITY ? 1.f : ex2(m_a - mn_a);
             float cb = mn_b == -INFINITY ? 1.f : ex2(m_b - mn_b);
             lsum[0] *= ca; lsum[2] *= cb;
             if (grow) {
                 const float nv = vmax * 4.f, f = vref / nv;
                 ca *= f; cb *= f;
-                vref = nv; inv_vref = 32768.f / nv;
+                vref = nv; inv_vref = kWScale / nv;
             }
 #pragma unroll
             for (int n = 0; n < NT; ++n) { o[n][0] *= ca; o[n][1] *= ca; o[n][2] *= cb; o[n][3] *= cb; }
@@ -509,7 +517,7 @@ struct WarpTileF8 {
     // (all 32 lanes call it; acc in true units, dims in their natural order)
     __device__ __forceinline__ void to_scratch(float* scratch, int32_t R_rows, int32_t lane) const {
         const float la = quad_sum(lsum[0]), lb = quad_sum(lsum[2]);
-        const float vu = vref * (1.f / 32768.f);
+        const float vu = vref * (1.f / kWScale);
         const int32_t ra = lane >> 2, d0 = (lane & 3) * (D / 4);
         const bool wa = ra < R_rows, wb = ra + 8 < R_rows;
 #pragma unroll

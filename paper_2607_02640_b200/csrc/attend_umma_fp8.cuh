@@ -9,15 +9,16 @@
 //   * The tensor-core operands are fp16, not bf16: E4M3 is a subset of fp16, so the codes convert EXACTLY and no scale
 //     ever touches an operand.  The K scale of key j multiplies the finished fp32 score (softmax thread), the V scale is
 //     folded into the softmax weight before it is rounded to fp16 -- relative to a running reference vref >= every V
-//     scale seen so far, times 2^9: weights stay below 2^15 even with the lazily updated row maximum (p <= 2^8) and keep
-//     full fp16 precision down to p vs = 2^-23 vref.  fp16's 11 bits replace the bf16 hi + lo pair of the bf16 kernel:
+//     scale seen so far, times 2^7: weights stay at or below 2^15 < 65504 even with the lazily updated row maximum
+//     (p <= 2^8) and a key whose scale equals the reference (vref is only raised when a scale exceeds it), and keep
+//     full fp16 precision down to p vs = 2^-21 vref.  fp16's 11 bits replace the bf16 hi + lo pair of the bf16 kernel:
 //     ONE P V instruction per block instead of two.
 //   * Q is staged as fp16 after an exact power-of-two prescale per row (its largest element into [1, 2)), undone in the
 //     softmax's scale factor: |q| > 65504 and tiny rows both survive.
 //   * Four CONVERTER warps sit between the producer and the MMA issuers: the producer bulk-copies whole (block, head)
 //     units (K codes | V codes | scales, 4224 B at D = 128, contiguous in HBM) into a staging ring; the converters turn
 //     the code tiles into the K-major / MN-major SWIZZLE_128B fp16 operands the MMAs read, zero V rows past the
-//     session's length, and publish the half-stage's scales (ks_j, vs_j 2^9 / vref, vref) for the softmax threads.
+//     session's length, and publish the half-stage's scales (ks_j, vs_j 2^7 / vref, vref) for the softmax threads.
 //     HBM traffic per key and KV head: 2 D + 8 bytes instead of 4 D.
 //   * A row tile count of one (R <= 128) runs on slot 0 alone (the bf16 kernel alternates half-stages between the two
 //     softmax warpgroups there).
@@ -41,7 +42,7 @@ struct UmmaF8Cfg {
     static constexpr int kQBytes = 128 * D * 2;                   // Q rows of one slot
     static constexpr int NBUF = 5;                                // operand ring buffers
     static constexpr int NSC = 16;                                // scale slots (one per half-stage in flight)
-    static constexpr int kScFloats = 136;                         // 64 ks | 64 vs 2^9 / vref | vref | pad
+    static constexpr int kScFloats = 136;                         // 64 ks | 64 vs 2^7 / vref | vref | pad
     static constexpr int kRingOff = 2 * kQBytes;
     static constexpr int kStageOff = kRingOff + NBUF * kBufBytes;
     static constexpr int kScOff = kStageOff + NSTAGE * kStageBytes;
@@ -51,7 +52,7 @@ struct UmmaF8Cfg {
     static constexpr int kThreads = 512;                          // 16 warps: producer, 3 MMA issuers, 2 x 4 softmax, 4 converters
     static constexpr int kTmemCols = 512;
     static constexpr int kColS = 0, kColO = 256;
-    static constexpr float kPScale = 512.f;                       // 2^9 (see the header)
+    static constexpr float kPScale = 128.f;                       // 2^7 (see the header)
     static_assert(kSmemBytes <= 232448, "shared memory budget");
     static_assert(kStageBlk % 128 == 0, "staging units stay 128-byte aligned");
 };
@@ -530,7 +531,7 @@ attend_umma_fp8_kernel(AttendParams p) {
     }
     const float l = (l0 + l1) + (l2 + l3);
 
-    // ---- epilogue: O (in units of vref / 2^9) -> bf16 output, or the unnormalised partial of a split, 32 columns at a time ----
+    // ---- epilogue: O (in units of vref / 2^7) -> bf16 output, or the unnormalised partial of a split, 32 columns at a time ----
     if (n_mine > 0) {
         mbar_wait(bar_o(slot), 0);
         tc_fence_after();

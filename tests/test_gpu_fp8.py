@@ -163,3 +163,52 @@ def test_fp8_gqa_decode_with_rows_of_very_different_magnitude(G, D, qmag):
         assert_parity(out, ref, f"fp8 magnitudes G={G} D={D} {qmag} step {step}", unit_scale=False)
     assert min(defn.length.values()) > S + W
     assert pool.pool_query()[1] == book.pool_query()
+
+
+@pytest.mark.parametrize("mode", ["decode", "chunk"])
+def test_fp8_weights_stay_inside_fp16_when_the_row_maximum_lags(mode):
+    """Both fp8 tensor-core kernels round softmax weight x V scale to fp16 relative to a LAZILY updated row maximum (the
+    accumulators are rescaled only when the true maximum has moved by more than 2^6 (GQA decode tile) / 2^8 (chunk
+    kernel)) and to a V reference that is raised only when a scale exceeds it.  Worst case for the fp16 range: scores
+    that rise key after key (0.12 per key in the log2 domain: the stale maximum lags by almost the whole bound) while the
+    keys' V scales sit just under the reference (first 64 keys x 1, the rest x 3.9 with a reference of 4 x the first
+    maximum).  A weight factor that forgets either effect overflows to inf (this did happen: the decode tile at 2^11, and
+    2^9 in the chunk kernel was only safe by luck); outputs must be finite and match the oracle."""
+    G, Hkv, D, S, W, N = 4, 2, 128, 4, 640, 2
+    Hq = G * Hkv
+    n_max = 20
+    pool, defn, book = _make(S, W, Hq, Hkv, D, N, n_max)
+    sids = [pool.session_open() for _ in range(N)]
+    assert sids == [defn.session_open() for _ in range(N)] == [book.session_open() for _ in range(N)]
+    rng = np.random.default_rng(321)
+    length = np.zeros(N, np.int64)
+    beta, delta = 8.0, 0.12 / (1.4426950408889634 / np.sqrt(D)) / 8.0          # score rises 0.12 per key (log2 domain)
+
+    def rows_for(n_new):
+        ks, vs, qs = [], [], []
+        for i, n in enumerate(n_new):
+            pos = length[i] + np.arange(n)
+            k = rng.standard_normal((n, Hkv, D)).astype(np.float32) * 0.05
+            k[:, :, 0] = (delta * pos)[:, None]
+            v = rng.standard_normal((n, Hkv, D)).astype(np.float32) * np.where(pos < 64, 1.0, 3.9)[:, None, None]
+            q = rng.standard_normal((n, Hq, D)).astype(np.float32) * 0.05
+            q[:, :, 0] = beta
+            ks.append(k); vs.append(v); qs.append(q)
+            length[i] += n
+        t = lambda xs: torch.from_numpy(np.concatenate(xs)).to(torch.bfloat16)
+        return t(ks), t(vs), t(qs)
+
+    for step in range(60):
+        if mode == "chunk" or step < 12:
+            n_new = np.full(N, n_max, np.int32)                 # (R = 80 rows: chunk class; also builds the decode history)
+        else:
+            n_new = np.ones(N, np.int32)
+        k, v, q = rows_for(n_new)
+        out = torch.empty_like(q, device="cuda")
+        pool.append_attend(0, sids, n_new, k.cuda(), v.cuda(), q.cuda(), out)
+        assert torch.isfinite(out.float()).all(), f"{mode} step {step}: non-finite output (fp16 weight overflow)"
+        defn.append_kv(0, sids, [int(x) for x in n_new], synth.to_u16(k), synth.to_u16(v))
+        book.append_kv(0, sids, [int(x) for x in n_new])
+        ref = defn.attend_frame(0, sids, [int(x) for x in n_new], synth.to_u16(q))
+        assert_parity(out, ref, f"fp8 lagging maximum, {mode} step {step}", unit_scale=False)
+    assert pool.pool_query()[1] == book.pool_query()
