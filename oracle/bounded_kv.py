@@ -397,6 +397,8 @@ class PagedOracle:
 
     def attend_frame(self, layer: int, sids, q_lens, q, precision="f32", want_weights=False):
         c = self.cfg
+        if c.kv_fp8:       # (the fp8 KV arm is stated at the definition layer only; this layer then checks bookkeeping)
+            raise OracleError("PagedOracle has no fp8 arm: attend through DefinitionOracle")
         B = c.block_size
         outs, weights = [], []
         row = 0

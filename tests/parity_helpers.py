@@ -43,21 +43,23 @@ def assert_parity(got: torch.Tensor, ref: np.ndarray, what: str = "", unit_scale
     return r
 
 
-def oracle_cfg(w, n_layers=1, unbounded=False, scale=None) -> O.PoolConfig:
+def oracle_cfg(w, n_layers=1, unbounded=False, scale=None, kv_fp8=False) -> O.PoolConfig:
     return O.PoolConfig(n_q_heads=w.n_q_heads, n_kv_heads=w.n_kv_heads, head_dim=w.head_dim, S=w.S, W=w.W,
                         n_blocks=w.n_blocks, block_size=w.block_size, max_sessions=w.slots,
-                        max_new_tokens=w.max_new_tokens, n_layers=n_layers, scale=scale, unbounded=unbounded)
+                        max_new_tokens=w.max_new_tokens, n_layers=n_layers, scale=scale, unbounded=unbounded,
+                        kv_fp8=kv_fp8)
 
 
 class OracleMirror:
     """Replays the same opens / closes / steps into both oracle layers, regenerating every row on the
     CPU from its (uid, position) coordinates -- no value ever comes from the CUDA path."""
 
-    def __init__(self, runner, layers=(0,), paged=True, definition=True, unbounded=False):
+    def __init__(self, runner, layers=(0,), paged=True, definition=True, unbounded=False, kv_fp8=False):
         self.r = runner
-        cfg = oracle_cfg(runner.w, runner.n_layers, unbounded)
+        cfg = oracle_cfg(runner.w, runner.n_layers, unbounded, kv_fp8=kv_fp8)
         self.defn = O.DefinitionOracle(cfg) if definition else None
-        self.paged = O.PagedOracle(cfg, poison_on_free=True) if paged else None
+        # (the fp8 KV arm exists at the definition layer only: the paged layer then checks the bookkeeping alone)
+        self.paged = (O.PagedOracle(cfg, store_kv=False) if kv_fp8 else O.PagedOracle(cfg, poison_on_free=True)) if paged else None
         self.layers = layers
         self.osid = {}
 
