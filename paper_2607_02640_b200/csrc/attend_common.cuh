@@ -49,6 +49,7 @@ struct AttendParams {
     int32_t items_epoch;      // -1: the list came by a copy / plain launch: wait for the predecessor at the top
     const int32_t* range_item; // GQA decode: item that holds the first tile of each range (null: binary search)
     int32_t* gqa_ctr;         // [2] claim / exit counters of the GQA decode kernel's dynamic ranges (zero between launches)
+    const uint8_t* sm_class;  // [SM id] 1: an SM that streams slower than the rest (GqaPlan::sm_mode; its claim counters: gqa_ctr[4], [5])
     int32_t* tickets;         // [item][Hkv] arrival counters of the stream-K pieces (zero between launches)
     int32_t* pastwait_flag;    // tensor-core kernels: <- pastwait_epoch once past griddepcontrol.wait, i.e. once this step's append
     int32_t pastwait_epoch;    // kernel is complete (the NEXT append kernel may then do its bookkeeping while this kernel runs); null: off

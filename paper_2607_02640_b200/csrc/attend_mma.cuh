@@ -576,6 +576,8 @@ struct GqaPlan {
     int64_t q1, g1;           // static regime
     int64_t q2;               // dynamic regime
     int32_t n_static, n_total;
+    int32_t sm_mode;          // 1: ranges 0 .. n_static-1 are for CTAs on fast SMs, the rest (shorter) for CTAs on slow SMs: one range
+                              // per CTA, claimed from the list of the CTA's SM class (make_gqa_plan_smclass)
     __host__ __device__ int64_t range_lo(int32_t r) const { return r < n_static ? r * q1 : g1 + (int64_t)(r - n_static) * q2; }
     __host__ __device__ int64_t range_hi(int32_t r) const {
         const int64_t hi = r < n_static ? (r + 1) * q1 : g1 + (int64_t)(r - n_static + 1) * q2;
@@ -611,6 +613,27 @@ inline GqaPlan make_gqa_plan(int32_t n_kv_heads, int64_t total_tiles, int64_t ct
     g.g1 = g.q1 * g.n_static < total_tiles ? g.q1 * g.n_static : total_tiles;
     g.q2 = dynamic ? (g.q1 / 6 > 8 ? g.q1 / 6 : 8) : g.q1;
     g.n_total = g.n_static + (int32_t)((total_tiles - g.g1 + g.q2 - 1) / g.q2);
+    return g;
+}
+
+// The same list cut for a GPU whose SMs do not stream at the same speed (on a B200 the same ~26-40 SMs run at ~0.9 of the
+// others' rate, launch after launch, and a launch ends with its slowest CTA): n_fast long ranges of q1 units for the CTAs
+// that land on fast SMs, then n_slow ranges shorter by `ratio` for those on slow SMs.  Which CTA lands where is the
+// hardware's choice: a CTA reads %smid and CLAIMS a range from its class's list (or from the other one if its own is
+// used up, which keeps any placement correct: there are exactly as many ranges as CTAs).
+inline GqaPlan make_gqa_plan_smclass(int32_t n_kv_heads, int64_t total_tiles, int64_t n_fast, int64_t n_slow, double ratio, int32_t bnd) {
+    GqaPlan g{};
+    g.n_kv_heads = n_kv_heads;
+    g.bnd = bnd;
+    g.total_tiles = total_tiles;
+    g.sm_mode = 1;
+    const double weight = (double)n_fast + ratio * (double)n_slow;
+    g.q1 = (int64_t)((double)total_tiles / weight) + 1;
+    g.g1 = g.q1 * n_fast < total_tiles ? g.q1 * n_fast : total_tiles;
+    g.n_static = (int32_t)((g.g1 + g.q1 - 1) / g.q1);
+    const int64_t rem = total_tiles - g.g1;
+    g.q2 = rem > 0 ? (rem + n_slow - 1) / n_slow : g.q1;
+    g.n_total = g.n_static + (int32_t)((rem + g.q2 - 1) / g.q2);
     return g;
 }
 
@@ -650,12 +673,27 @@ attend_gqa_kernel(AttendParams p, GqaPlan plan) {
         for (int s = 0; s < C::NS; ++s) mbar_init(bars + 8 * s, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    __shared__ int32_t s_range;
+    if (plan.sm_mode && threadIdx.x == 0) {
+        // one range per CTA, from the list of this SM's class (GqaPlan::sm_mode); if that list is used up (the hardware
+        // placed the CTAs otherwise than 3 per SM) from the other one: ranges and CTAs are equally many, so one of the
+        // two claims succeeds
+        unsigned int smid;
+        asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+        int32_t cls = __ldg(p.sm_class + smid) ? 1 : 0;
+        int32_t idx = atomicAdd(p.gqa_ctr + 4 + cls, 1);
+        if (idx >= (cls ? plan.n_total - plan.n_static : plan.n_static)) {
+            cls ^= 1;
+            idx = atomicAdd(p.gqa_ctr + 4 + cls, 1);
+        }
+        const bool got = idx < (cls ? plan.n_total - plan.n_static : plan.n_static);
+        s_range = got ? (cls ? plan.n_static + idx : idx) : plan.n_total;
+    }
     __syncthreads();
     uint32_t phase_bits = 0;                             // parity of each private stage
 
     const int32_t Hkv = plan.n_kv_heads;
-    __shared__ int32_t s_range;
-    int32_t range = blockIdx.x;                          // first the CTA's static range, then claimed ones
+    int32_t range = plan.sm_mode ? s_range : (int32_t)blockIdx.x;   // first the CTA's static range, then claimed ones
     const int32_t bnd = plan.bnd;
     while (range < plan.n_total) {
     int64_t g = plan.range_lo(range);                    // (cost units, see make_gqa_plan)
@@ -841,14 +879,16 @@ attend_gqa_kernel(AttendParams p, GqaPlan plan) {
         if (kvh + 1 == Hkv) ++i;                          // (a pair left unfinished ends the range anyway)
     }
     // ---- next range: one of the small dynamic ones, first come first served ----
-    if (plan.n_total == plan.n_static) break;
+    if (plan.n_total == plan.n_static || plan.sm_mode) break;
     if (threadIdx.x == 0) s_range = plan.n_static + atomicAdd(p.gqa_ctr, 1);
     __syncthreads();
     range = s_range;
     }
     // every CTA leaves through exactly one failed claim: the last one out zeroes the counters for
     // the next launch
-    if (plan.n_total != plan.n_static && threadIdx.x == 0) {
+    if (plan.sm_mode) {
+        if (threadIdx.x == 0 && atomicAdd(p.gqa_ctr + 1, 1) == (int32_t)gridDim.x - 1) { p.gqa_ctr[1] = 0; p.gqa_ctr[4] = 0; p.gqa_ctr[5] = 0; }
+    } else if (plan.n_total != plan.n_static && threadIdx.x == 0) {
         if (atomicAdd(p.gqa_ctr + 1, 1) == (int32_t)gridDim.x - 1) { p.gqa_ctr[0] = 0; p.gqa_ctr[1] = 0; }
     }
     if (threadIdx.x == 0) stamp_end(p);

@@ -48,6 +48,7 @@ constexpr int kStagingSlots = 64;      // per-call metadata slots (pinned host +
 constexpr int kStagingGroup = 8;       // one completion event per 8 slots: an event between two kernels
                                        // would break their programmatic (PDL) launch edge
 constexpr int kMaxSplits = 64;
+constexpr int kGqaSmClassDefault = 0;  // (set to 1 once measured)
 constexpr int kDirectSlots = 3;        // device staging slots of the event-free async host steps
 constexpr int kStampSlots = 1 << 15;   // attention launches one stamped pass can hold
 #ifndef METRONOME_GQA_BND_BYTES
@@ -107,7 +108,7 @@ struct metronome_pool {
     float* d_ws_acc = nullptr;
     float* d_ws_ml = nullptr;
     int32_t* d_tickets = nullptr;      // [max_sessions][Hkv], zero between launches
-    int32_t* d_bk_flag = nullptr;      // [0] bookkeeping epoch, [1] work-list epoch, [2..3] GQA claim counters, [5] past-wait epoch
+    int32_t* d_bk_flag = nullptr;      // [0] bookkeeping epoch, [1] work-list epoch, [2..3] GQA claim counters, [5] past-wait epoch, [6..7] GQA SM-class claims
     int32_t last_early_epoch = 0;      // epoch of the previous append kernel if it ran in early mode, else 0
     int64_t pastwait_launches = -1;    // value of n_launch right after a tensor-core attention launch that publishes its epoch once
     int32_t pastwait_epoch = 0;        // past its wait (d_bk_flag[12]); still equal to n_launch <=> nothing was launched since
@@ -161,6 +162,8 @@ struct metronome_pool {
     std::vector<int32_t> stamp_kind;   // per used slot: 1 rows, 2 gqa decode, 3 chunk
 
     int32_t tune_split_tokens = 0, tune_family = 0, tune_gqa_dynamic = 0, tune_fused_step = 0;
+    int tune_gqa_smclass = 0;          // GQA decode ranges sized by the SM's streaming speed (METRONOME_GQA_SMCLASS at pool creation)
+    uint8_t* d_sm_class = nullptr;     // device copy of sm_class (256 bytes)
     bool tune_host_direct = true;      // false (METRONOME_HOST_STEP_EVENTS=1 at pool creation): async host steps always chain events
     int32_t n_sm = 148;
     int64_t n_launch = 0, n_append = 0, n_attend = 0;
@@ -417,9 +420,17 @@ int plan_attend(metronome_pool* pool, int32_t n_batch, const int32_t* sids, cons
             // ranges are cut in cost units: a pair's tiles + what starting a pair costs (make_gqa_plan), the latter
             // ~4 us of one CTA's share of the stream = METRONOME_GQA_BND_BYTES of K/V tiles
             const int32_t bnd = (int32_t)(METRONOME_GQA_BND_BYTES / pool->L.head_bytes);
+            // a full one-wave launch on a GPU with a known set of slow SMs: long ranges for the CTAs that land on fast SMs,
+            // ranges shorter by the measured speed ratio for those on slow SMs (each CTA claims from its SM's list)
+            const bool smclass = pool->d_sm_class && pool->n_slow_sms > 0 && !dynamic && pool->tune_split_tokens <= 0 &&
+                                 pool->tune_gqa_dynamic != 2 && ctas == (int64_t)pool->n_sm * 3;
+            if (smclass)
+                pl.gplan = make_gqa_plan_smclass(c.n_kv_heads, (cls_tiles[0] + (int64_t)bnd * n) * c.n_kv_heads,
+                                                 3 * (pool->n_sm - pool->n_slow_sms), 3 * pool->n_slow_sms, pool->slow_ratio, bnd);
+            else
             pl.gplan = make_gqa_plan(c.n_kv_heads, (cls_tiles[0] + (int64_t)bnd * n) * c.n_kv_heads, ctas, dynamic, bnd);
             GqaPlan& g = pl.gplan;
-            pl.gqa_ctas = g.n_static;
+            pl.gqa_ctas = g.sm_mode ? g.n_total : g.n_static;     // (SM-class ranges: one CTA per range, long and short)
             if (g.n_total <= kMaxRangeItems) {
                 int32_t* range_item = reinterpret_cast<int32_t*>(items + n_items);    // after ALL items
                 int32_t ii = 0;
@@ -541,6 +552,7 @@ AttendParams make_attend_params(metronome_pool* pool, int32_t layer, const Atten
     p.max_splits = pl.max_splits;
     p.tickets = pool->d_tickets;
     p.gqa_ctr = pool->d_bk_flag + 2;              // same 16-byte allocation: [flag, -, claims, exits]
+    p.sm_class = pool->d_sm_class;                // (null: off) its claim counters are gqa_ctr[4], [5] = d_bk_flag[6], [7]
     // measured on B200 (configs 2-4): letting the next append kernel launch early hides its host-memory
     // reads behind the attention kernel (-4..6 % per frame)
     p.pdl_early = 1;
@@ -803,6 +815,7 @@ int metronome_pool_create(const metronome_pool_config_t* cfg, metronome_pool_t**
     }
     pool->slot_bytes = (size_t)c.max_sessions * (sizeof(AppendItem) + sizeof(AttendItem)) + kMaxRangeItems * sizeof(int32_t) + 16;
     { const char* ev = getenv("METRONOME_HOST_STEP_EVENTS"); pool->tune_host_direct = !(ev && ev[0] == '1'); }
+    { const char* ev = getenv("METRONOME_GQA_SMCLASS"); pool->tune_gqa_smclass = ev ? atoi(ev) : kGqaSmClassDefault; }
     e = cudaMalloc(&pool->d_tickets, (size_t)c.max_sessions * c.n_kv_heads * sizeof(int32_t));
     if (e != cudaSuccess) return fail(METRONOME_ERR_OUT_OF_MEMORY, e, "cudaMalloc tickets");
     cudaMemset(pool->d_tickets, 0, (size_t)c.max_sessions * c.n_kv_heads * sizeof(int32_t));
@@ -829,6 +842,16 @@ int metronome_pool_create(const metronome_pool_config_t* cfg, metronome_pool_t**
     if (e == cudaSuccess) e = configure_step_kernels();
     if (e != cudaSuccess) return fail(METRONOME_ERR_CUDA, e, "cudaFuncSetAttribute");
 
+    // GQA decode ranges sized by the SMs' streaming speeds: classify the SMs once (a few ms), keep the table on the device
+    if (pool->tune_gqa_smclass && !pool->bookkeeping_only && pool->G > 1) {
+        calibrate_sm_speeds(pool);
+        if (pool->n_slow_sms > 0) {
+            e = cudaMalloc(&pool->d_sm_class, sizeof(pool->sm_class));
+            if (e == cudaSuccess) e = cudaMemcpy(pool->d_sm_class, pool->sm_class, sizeof(pool->sm_class), cudaMemcpyHostToDevice);
+            if (e != cudaSuccess) return fail(METRONOME_ERR_CUDA, e, "SM class table");
+        }
+    }
+
     *out = pool;
     return METRONOME_OK;
 }
@@ -853,6 +876,7 @@ int metronome_pool_destroy(metronome_pool_t* pool) {
         if (pool->ev_comp[b]) cudaEventDestroy(pool->ev_comp[b]);
         if (pool->ev_d2h[b]) cudaEventDestroy(pool->ev_d2h[b]);
     }
+    if (pool->d_sm_class) cudaFree(pool->d_sm_class);
     if (pool->d_h2d_flag) cudaFree(pool->d_h2d_flag);
     if (pool->h_done) cudaFreeHost(pool->h_done);
     if (pool->h_seq_ring) cudaFreeHost(pool->h_seq_ring);

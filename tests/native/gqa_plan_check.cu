@@ -1,4 +1,4 @@
-// Host-only check of GqaPlan (csrc/attend_mma.cuh): the static + dynamic ranges must partition the
+// Host-only check of GqaPlan (csrc/attend_mma.cuh): the static + dynamic (or long + short, by SM class) ranges must partition the
 // flattened list of cost units exactly, range_of() must invert range_lo() / range_hi(), and the walk a CTA makes
 // over its range (gqa_piece, the function the kernel itself calls) must visit every (item, head, tile) exactly once,
 // with the pieces of a pair numbered 0 .. last - first without a gap.  Built and run by tests/test_host_logic.py
@@ -11,8 +11,20 @@
 using metronome::GqaPlan;
 using metronome::GqaPiece;
 
-static int check(int64_t total, int64_t ctas, bool dynamic, int32_t bnd) {
-    const GqaPlan g = metronome::make_gqa_plan(4, total, ctas, dynamic, bnd);      // the launcher's own rule
+// mode 0 static, 1 static + dynamic tail, 2 ranges by SM class (a random split of the CTAs into fast / slow, a random
+// speed ratio): the launcher's own rules
+static GqaPlan plan_for(int32_t Hkv, int64_t total, int64_t ctas, int mode, int32_t bnd) {
+    if (mode < 2) return metronome::make_gqa_plan(Hkv, total, ctas, mode == 1, bnd);
+    int64_t n_slow = 3 * (rand() % 60);
+    if (n_slow >= ctas) n_slow = ctas - 1;
+    const double ratio = 0.75 + 0.25 * (rand() % 1000) / 999.0;
+    const GqaPlan g = metronome::make_gqa_plan_smclass(Hkv, total, ctas - n_slow, n_slow, ratio, bnd);
+    if (g.n_total > ctas || g.n_static > ctas - n_slow) { printf("SM-class plan: %d ranges (%d long) for %lld CTAs (%lld fast)\n", g.n_total, g.n_static, (long long)ctas, (long long)(ctas - n_slow)); exit(1); }
+    return g;
+}
+
+static int check(int64_t total, int64_t ctas, int mode, int32_t bnd) {
+    const GqaPlan g = plan_for(4, total, ctas, mode, bnd);
     int64_t expect = 0;
     for (int32_t r = 0; r < g.n_total; ++r) {
         const int64_t lo = g.range_lo(r), hi = g.range_hi(r);
@@ -26,13 +38,14 @@ static int check(int64_t total, int64_t ctas, bool dynamic, int32_t bnd) {
 }
 
 // the kernel's walk, on the host: items with random tile counts, Hkv heads
-static int walk(int n_items, int Hkv, int max_tiles, int64_t ctas, bool dynamic, int32_t bnd) {
+static int walk(int n_items, int Hkv, int max_tiles, int64_t ctas, int mode, int32_t bnd) {
+    const bool dynamic = mode == 1;
     std::vector<int32_t> n_tiles(n_items), tile_off(n_items);
     int64_t sum = 0;
     for (int i = 0; i < n_items; ++i) { n_tiles[i] = 1 + rand() % max_tiles; tile_off[i] = (int32_t)sum; sum += n_tiles[i]; }
     const int64_t total = (sum + (int64_t)bnd * n_items) * Hkv;
     if (ctas > sum * Hkv) ctas = sum * Hkv;
-    const GqaPlan g = metronome::make_gqa_plan(Hkv, total, ctas, dynamic, bnd);
+    const GqaPlan g = plan_for(Hkv, total, ctas, mode, bnd);
     std::vector<std::vector<int>> seen(n_items * Hkv);
     std::vector<std::vector<int>> pieces(n_items * Hkv);
     for (int i = 0; i < n_items; ++i) for (int h = 0; h < Hkv; ++h) seen[i * Hkv + h].assign(n_tiles[i], 0);
@@ -75,16 +88,18 @@ int main() {
         const int64_t ctas = 1 + rand() % 600;
         const int64_t total = ctas + rand() % 400000;
         const int32_t bnd = (it & 1) ? 8 : 0;
-        bad += check(total, ctas, false, bnd);
-        if ((total + ctas - 1) / ctas >= 48) bad += check(total, ctas, true, bnd);
+        bad += check(total, ctas, 0, bnd);
+        if ((total + ctas - 1) / ctas >= 48) bad += check(total, ctas, 1, bnd);
+        if (ctas >= 2) bad += check(total, ctas, 2, bnd);
         ++n;
     }
-    bad += check(1, 1, false, 0);
-    bad += check(444, 444, false, 8);
+    bad += check(1, 1, 0, 0);
+    bad += check(444, 444, 0, 8);
+    bad += check(444, 444, 2, 8);
     const int32_t bnds[4] = {0, 1, 8, 16};
     for (int it = 0; it < 3000; ++it) {
         const int n_items = 1 + rand() % 200, Hkv = 1 + rand() % 8, max_tiles = (it % 3 == 0) ? 3 : 1 + rand() % 140;
-        bad += walk(n_items, Hkv, max_tiles, 1 + rand() % 600, (it & 1) != 0, bnds[it & 3]);
+        bad += walk(n_items, Hkv, max_tiles, 2 + rand() % 600, it % 3, bnds[it & 3]);
         ++n;
     }
     printf("%d cases, %d bad\n", n, bad);

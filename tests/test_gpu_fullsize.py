@@ -68,7 +68,9 @@ def _run_fullsize(index, n_frames, n_sample, history_scale=1.0, n_sessions=None,
         st = r.make_step(ev)
         r.append(st, 0)
         book.append_kv(0, [osid[int(i)] for i in st.local], [int(n) for n in st.n_new])
-        out = r.attend(st, 0)
+        rows = int(st.n_new.sum())
+        out = torch.full((rows, w.n_q_heads, w.head_dim), float("nan"), dtype=torch.bfloat16, device="cuda")
+        out = r.attend(st, 0, out=out)                 # (NaN first: a row no CTA wrote cannot pass as finite)
         assert torch.isfinite(out.float()).all()
         # sampled sessions of this step: always include the youngest and the oldest due session
         lens = np.array([r.length[int(i)] for i in st.local])

@@ -256,6 +256,51 @@ def test_event_free_host_steps_under_load(G):
     assert per_step >= 3, per_step
 
 
+def test_gqa_ranges_by_sm_class(monkeypatch):
+    """GqaPlan::sm_mode (METRONOME_GQA_SMCLASS=1 at pool creation; off by default): the GQA decode kernel's CTAs read %smid
+    and claim a long range (fast SMs) or a shorter one (the SMs that a calibration pass found to stream slower) from two
+    lists.  Every range must be processed exactly once whatever the placement: outputs are pre-filled with NaN (a range
+    nobody claimed leaves NaN rows -- the first version of this mode launched one CTA per LONG range only, skipped a sixth
+    of the work and still passed every sampled check), compared with the oracle on every row, over 8 launches back to
+    back, and the claim counters must be back to zero."""
+    monkeypatch.setenv("METRONOME_GQA_SMCLASS", "1")
+    Hq, Hkv, D, S, W, N = 32, 4, 128, 4, 750, 24
+    per = 1 + (W + 25 - 1) // 16 + 2
+    kw = dict(n_q_heads=Hq, n_kv_heads=Hkv, head_dim=D, max_sessions=N, max_new_tokens=25)
+    pool = binding.Pool(n_sinks=S, window=W, n_blocks=N * per, **kw)
+    n_sm, n_slow, ratio = pool.sm_speeds()
+    if n_slow == 0:
+        pytest.skip("the calibration found no slow SMs on this GPU: the mode stays off")
+    assert 0.75 <= ratio <= 1.0
+    defn = O.DefinitionOracle(O.PoolConfig(S=S, W=W, n_blocks=N * per, block_size=16, **kw))
+    sids = [pool.session_open() for _ in range(N)]
+    assert sids == [defn.session_open() for _ in range(N)]
+    rng = np.random.default_rng(1234)
+    target = rng.integers(500, 1500, size=N)
+    done = np.zeros(N, np.int64)
+    while (done < target).any():
+        idx = [i for i in range(N) if done[i] < target[i]]
+        n_new = np.array([min(25, target[i] - done[i]) for i in idx], np.int32)
+        rows = int(n_new.sum())
+        k, v = _rows(rng, rows, Hkv, D), _rows(rng, rows, Hkv, D)
+        pool.append_kv(0, [sids[i] for i in idx], n_new, k.cuda(), v.cuda())
+        defn.append_kv(0, [sids[i] for i in idx], [int(x) for x in n_new], synth.to_u16(k), synth.to_u16(v))
+        done[idx] += n_new
+    ones = np.ones(N, np.int32)
+    ins = [(_rows(rng, N, Hkv, D), _rows(rng, N, Hkv, D), _rows(rng, N, Hq, D)) for _ in range(8)]
+    dev = [(k.cuda(), v.cuda(), q.cuda()) for k, v, q in ins]
+    outs = [torch.full_like(q, float("nan")) for _, _, q in dev]
+    torch.cuda.synchronize()
+    for (k, v, q), o in zip(dev, outs):
+        pool.append_attend(0, sids, ones, k, v, q, o)
+    flags = pool.debug_read_flags()
+    assert flags[3] == 0 and flags[6] == 0 and flags[7] == 0, f"SM-class claim counters not reset: {flags[:8]}"
+    for step, ((k, v, q), o) in enumerate(zip(ins, outs)):
+        assert torch.isfinite(o.float()).all(), f"step {step}: rows no CTA wrote"
+        defn.append_kv(0, sids, [1] * N, synth.to_u16(k), synth.to_u16(v))
+        assert_parity(o, defn.attend_frame(0, sids, [1] * N, synth.to_u16(q)), f"SM-class ranges, step {step}")
+
+
 @pytest.mark.parametrize("n_max", [2, 25])
 def test_early_bookkeeping_under_the_previous_attention_kernel(n_max):
     """Tensor-core family, two launches per step, 300 steps back to back with NOTHING else on the stream: the append
