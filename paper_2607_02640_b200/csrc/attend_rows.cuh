@@ -114,18 +114,28 @@ attend_rows_kernel(AttendParams p) {
     };
     Chunk kr[STEPS], vr[STEPS];
     float ks[FP8 ? STEPS : 1], vs[FP8 ? STEPS : 1];                 // fp8: the rows' scales
-    auto chunk_off = [&](int32_t row) { return FP8 ? fp8_unit_offset(D, row, sub) : tile_chunk_offset(row, sub); };
+    // fp8 code tiles are XOR-swizzled in 128-byte lines (layout.cuh: fp8_chunk_offset, for the tensor-core kernels'
+    // ldmatrix); this thread's offsets take four distinct swizzle patterns (step j and j + 4 are eight rows apart: the
+    // same pattern, 4 TPS D bytes further), computed once instead of per load -- the fp8 arm of this kernel is issue-bound
+    int32_t xo[4] = {0, 0, 0, 0};
+    if (FP8) {
+#pragma unroll
+        for (int jj = 0; jj < (STEPS < 4 ? STEPS : 4); ++jj) xo[jj] = fp8_unit_offset(D, jj * TPS + grp, sub);
+    }
+    auto chunk_off_j = [&](int j) {
+        return FP8 ? xo[j & 3] + (j >> 2) * (4 * TPS * D) : tile_chunk_offset(j * TPS + grp, sub);
+    };
     auto load_k = [&](const uint8_t* kt) {
 #pragma unroll
         for (int j = 0; j < STEPS; ++j) {
-            kr[j] = __ldg(reinterpret_cast<const Chunk*>(kt + chunk_off(j * TPS + grp)));
+            kr[j] = __ldg(reinterpret_cast<const Chunk*>(kt + chunk_off_j(j)));
             if (FP8) ks[j] = __ldg(reinterpret_cast<const float*>(kt + 2 * p.L.tile_bytes) + j * TPS + grp);
         }
     };
     auto load_v = [&](const uint8_t* kt) {
 #pragma unroll
         for (int j = 0; j < STEPS; ++j) {
-            vr[j] = __ldg(reinterpret_cast<const Chunk*>(kt + p.L.tile_bytes + chunk_off(j * TPS + grp)));
+            vr[j] = __ldg(reinterpret_cast<const Chunk*>(kt + p.L.tile_bytes + chunk_off_j(j)));
             if (FP8) vs[j] = __ldg(reinterpret_cast<const float*>(kt + 2 * p.L.tile_bytes) + kBlockTokens + j * TPS + grp);
         }
     };
