@@ -54,9 +54,6 @@ struct AttendParams {
     int32_t* pastwait_flag;    // tensor-core kernels: <- pastwait_epoch once past griddepcontrol.wait, i.e. once this step's append
     int32_t pastwait_epoch;    // kernel is complete (the NEXT append kernel may then do its bookkeeping while this kernel runs); null: off
     unsigned long long* stamp; // measurement aid (null: off): [0] <- min over CTAs of %globaltimer at start, [1] <- max at exit
-    const int32_t* h2d_flag;   // event-free host steps: q is filled by a copy stream that ends by copying h2d_seq into *h2d_flag
-    int32_t h2d_seq;           // (null: q is stream-ordered).  Only an EARLY-mode kernel has to look: the others wait for the
-                               // append kernel of their step, which has itself waited for the flag
 };
 
 // Measurement aid (metronome_pool_set_profiling mode 2): the kernel's own span in %globaltimer ns, first CTA
@@ -76,7 +73,8 @@ __device__ __forceinline__ void stamp_end(const AttendParams& p) { if (p.stamp) 
 // that holds the oldest row appended in this step OR in the step before it -- the append kernel of
 // step e-1 is only known to be past its own wait when this kernel starts, not to be complete) and
 // before it writes anything.  Otherwise the predecessor is waited for right away.  One thread per
-// CTA; the caller syncs.
+// CTA; the caller syncs.  (Event-free host steps: q comes from a copy stream; the append kernel waits for the copies' flag
+// before it publishes the epoch this function waits for, so q is complete here as well.)
 __device__ __forceinline__ void wait_work_list(const AttendParams& p) {
     if (p.items_epoch < 0) { pdl_wait(); return; }
     int32_t seen;                       // (>=: a later step's list may already be out, in the other buffer)
@@ -84,7 +82,6 @@ __device__ __forceinline__ void wait_work_list(const AttendParams& p) {
         asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(seen) : "l"(p.items_flag) : "memory");
         if (seen - p.items_epoch < 0) __nanosleep(64);
     } while (seen - p.items_epoch < 0);
-    if (p.h2d_flag) spin_until_reached_sys(p.h2d_flag, p.h2d_seq);     // q is read before any griddepcontrol.wait
 }
 
 // (one thread of the grid, right after pdl_wait)

@@ -128,6 +128,10 @@ append_fused_kernel(const AppendParams a) {
                     asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(seen) : "l"(a.items_flag + 4) : "memory");
                     if (seen - a.gate_epoch < 0) __nanosleep(64);
                 } while (seen - a.gate_epoch < 0);
+                // event-free host steps: the early-mode row kernel reads q as soon as it has seen this step's epoch below, so
+                // the input copies (k_new, v_new, q: one flag behind all three) must have landed before it is published --
+                // one system-scope wait per launch here instead of one per CTA of the row kernel
+                if (a.h2d_flag) spin_until_reached_sys(a.h2d_flag, a.h2d_seq);
             }
             __syncthreads();
             copy_items();

@@ -139,7 +139,7 @@ struct metronome_pool {
     int32_t* d_h2d_flag = nullptr;
     int32_t* h_done = nullptr;         // pinned + mapped
     int32_t* h_seq_ring = nullptr;     // pinned: sources of the flag copies (a copy reads its source when it executes)
-    const int32_t* cur_h2d_flag = nullptr;   // non-null only while such a step is being enqueued (append_impl / make_attend_params)
+    const int32_t* cur_h2d_flag = nullptr;   // non-null only while such a step is being enqueued (append_impl passes it to the append kernel)
     int32_t cur_h2d_seq = 0;
 
     // per-call metadata staging: pinned host ring + matching device ring
@@ -559,7 +559,6 @@ AttendParams make_attend_params(metronome_pool* pool, int32_t layer, const Atten
     p.items_flag = pool->d_bk_flag + 1;
     p.items_epoch = -1;
     p.pastwait_flag = nullptr;
-    p.h2d_flag = pool->cur_h2d_flag; p.h2d_seq = pool->cur_h2d_seq;
     return p;
 }
 
