@@ -146,8 +146,9 @@ def test_no_alloc_only_pool_never_touches_the_pool_workspace():
     """Two pools fed the same seeded rows (bookkeeping is deterministic: same block ids): pool A answers through the
     existing path, pool B ONLY ever through the no-alloc entry point, so B's own split-KV workspace is never allocated
     (a null pointer: using it would fault) and its partials can only have gone through the array whose address the
-    library looked up with cudaGetSymbolAddress.  Free device memory (cudaMemGetInfo) is the same before and after
-    B's calls: the existing path would have grown a workspace of several MB for these batches."""
+    library looked up with cudaGetSymbolAddress.  Free device memory (cudaMemGetInfo) is also the same before and after
+    B's calls -- a coarse guard only (the driver hands out device memory in 2 MiB steps and the existing path's workspace
+    for these batches is ~190 KB); the null workspace pointer is the real one."""
     Hq, Hkv, D, S, W, N = 8, 8, 128, 4, 750, 6
     pa, pb = _pool(Hq, Hkv, D, S, W, N, 25), _pool(Hq, Hkv, D, S, W, N, 25)
     sa = [pa.session_open() for _ in range(N)]
