@@ -207,6 +207,44 @@ def test_pipelined_host_steps_match_the_blocking_ones(Hkv, buffers):
         assert_parity(o, ref, what)
 
 
+def test_event_free_host_step_that_fails_does_not_stall_the_pipeline():
+    """metronome_step_host_async, event-free mode: a step that fails validation inside the library (here: a session named
+    twice, a session that is not open) has already had its input copies enqueued and its step number taken; the library
+    still publishes that number, so the waits of the surrounding good steps return, the pool is as it was before the bad
+    step (no state change on error), and the good steps' results match the oracle."""
+    Hq, Hkv, D, S, W, N = 8, 8, 128, 4, 48, 3
+    per = 1 + (W + 8 - 1) // 16 + 2
+    kw = dict(n_q_heads=Hq, n_kv_heads=Hkv, head_dim=D, max_sessions=N + 1, max_new_tokens=8)
+    pool = binding.Pool(n_sinks=S, window=W, n_blocks=(N + 1) * per, **kw)
+    defn = O.DefinitionOracle(O.PoolConfig(S=S, W=W, n_blocks=(N + 1) * per, block_size=16, **kw))
+    sids = [pool.session_open() for _ in range(N)]
+    assert sids == [defn.session_open() for _ in range(N)]
+    rng = np.random.default_rng(77)
+    ones = np.ones(N, np.int32)
+    pending = []
+    for step in range(40):
+        k, v, q = (_rows(rng, N, H, D).pin_memory() for H in (Hkv, Hkv, Hq))
+        out = torch.full((N, Hq, D), float("nan"), dtype=torch.bfloat16).pin_memory()
+        if step % 4 == 2:                                 # a bad step between good ones: nothing may change, nothing may hang
+            bad = [sids[0], sids[0], sids[1]] if step % 8 == 2 else [sids[0], N, sids[1]]      # (slot N was never opened)
+            with pytest.raises(binding.MetronomeError) as ei:
+                pool.step_host_async(0, bad, ones, k, v, q, out)
+            assert ei.value.code in ("DUPLICATE_SESSION", "INVALID_SESSION"), ei.value.code
+            continue
+        pool.step_host_async(0, sids, ones, k, v, q, out)
+        defn.append_kv(0, sids, [1] * N, synth.to_u16(k), synth.to_u16(v))
+        pending.append((out, defn.attend_frame(0, sids, [1] * N, synth.to_u16(q)), f"step {step}", k, v, q))
+        pool.step_host_wait(1)
+        while len(pending) > 1:
+            o, ref, what, *_ = pending.pop(0)
+            assert_parity(o, ref, what)
+    pool.step_host_wait(0)
+    for o, ref, what, *_ in pending:
+        assert_parity(o, ref, what)
+    for s_ in sids:
+        assert pool.session_query(s_)[0] == defn.length[s_]
+
+
 @pytest.mark.parametrize("G", [1, 8])
 def test_event_free_host_steps_under_load(G):
     """The event-free mode on shapes where everything it touches is live: 24 sessions x 32 query heads, W = 750 (split-KV
