@@ -37,7 +37,10 @@
 
 namespace metronome {
 
-template <int D>
+// HALF: the variant for items of R <= 128 rows (one row tile): one softmax warpgroup, 256 TMEM columns and a ring of 4
+// buffers, so that TWO CTAs fit an SM and each runs under the other's prologue (Q staging, TMEM allocation, first tiles)
+// and epilogue (O read-out, normalisation, store): ~7 us of a ~22 us (item, head) pair on config 4.
+template <int D, bool HALF = false>
 struct UmmaCfg {
     static constexpr int KS = 4;                          // KV blocks per half-stage (64 keys)
     static constexpr int NH = D / 64;                     // 64-dim halves (128-byte swizzle span)
@@ -46,14 +49,17 @@ struct UmmaCfg {
     static constexpr int kKHalfBytes = KS * kBlockTokens * 128;   // [64 keys][64 dims]
     static constexpr int kQHalfBytes = 128 * 128;         // [128 rows][64 dims]
     static constexpr int kQBytes = 128 * D * 2;           // Q rows of one slot
-    static constexpr int NBUF = D == 128 ? 10 : 12;       // ring buffers
-    static constexpr int kBarOff = 2 * kQBytes + NBUF * kBufBytes;
+    static constexpr int NQ = HALF ? 1 : 2;               // row tiles (slots) a CTA can hold
+    static constexpr int NBUF = HALF ? 4 : (D == 128 ? 10 : 12);       // ring buffers
+    static constexpr int kBarOff = NQ * kQBytes + NBUF * kBufBytes;
     static constexpr int kMlOff = kBarOff + 512;          // (m, l) of slot 1 for the in-CTA merge
     static constexpr int kSmemBytes = kMlOff + 1024 + 1024;   // + alignment slack
-    static constexpr int kThreads = 384;                  // 12 warps: producer, 3 MMA issuers, 2 x 4 softmax
-    static constexpr int kTmemCols = 512;
-    static constexpr int kColS = 0, kColO = 256;          // S buffers of slot s at 128 s + {0, 64}; O_s at 256 + D s
-    static_assert(kSmemBytes <= 232448, "shared memory budget");
+    static constexpr int kThreads = HALF ? 256 : 384;     // 12 warps: producer, 3 MMA issuers, 2 x 4 softmax (HALF: 8 warps, one softmax warpgroup)
+    static constexpr int kSoftmaxThreads = HALF ? 128 : 256;
+    static constexpr int kTmemCols = HALF ? 256 : 512;
+    static constexpr int kColS = 0, kColO = HALF ? 128 : 256;   // S buffers of slot s at 128 s + {0, 64}; O_s at kColO + D s
+    static_assert(kSmemBytes <= (HALF ? 115712 : 232448), "shared memory budget");
+    static_assert(!HALF || kColO + D <= kTmemCols, "TMEM budget of the half-size variant");
 };
 
 // ---- tcgen05 / UMMA primitives --------------------------------------------------------------
@@ -137,10 +143,10 @@ __device__ __forceinline__ int32_t umma_seq_k(int32_t j) { return j == 0 ? 0 : 2
 __device__ __forceinline__ int32_t umma_seq_v(int32_t j, int32_t n) { return j == n - 1 ? 2 * n - 1 : 2 * j + 2; }
 
 // grid = (Hkv, total segments of the chunk-class items), block = 384, one CTA per SM
-template <int D>
-__global__ void __launch_bounds__(UmmaCfg<D>::kThreads, 1)
+template <int D, bool HALF>
+__global__ void __launch_bounds__(UmmaCfg<D, HALF>::kThreads, HALF ? 2 : 1)
 attend_umma_kernel(AttendParams p) {
-    using C = UmmaCfg<D>;
+    using C = UmmaCfg<D, HALF>;
     if (p.pdl_early) pdl_launch_dependents();
     if (threadIdx.x == 0) stamp_begin(p);
     pdl_wait();                  // the work list and this step's K/V rows come from the append kernel
@@ -148,7 +154,7 @@ attend_umma_kernel(AttendParams p) {
     extern __shared__ __align__(1024) uint8_t smem_umma[];
     const uint32_t base = (smem_u32(smem_umma) + 1023u) & ~1023u;       // swizzle atoms are 1024-byte aligned
     uint8_t* gen = smem_umma + (base - smem_u32(smem_umma));
-    const uint32_t sQ = base, sRing = base + 2 * C::kQBytes, sBar = base + C::kBarOff;
+    const uint32_t sQ = base, sRing = base + C::NQ * C::kQBytes, sBar = base + C::kBarOff;
     auto bar_full = [&](int b) { return sBar + 8u * b; };
     auto bar_empty = [&](int b) { return sBar + 8u * (C::NBUF + b); };
     auto bar_s = [&](int s, int buf) { return sBar + 8u * (2 * C::NBUF + 2 * s + buf); };       // S ready  (MMA -> softmax)
@@ -166,208 +172,216 @@ attend_umma_kernel(AttendParams p) {
     const int32_t split = (int32_t)blockIdx.y - it.split_off;
     const int32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int32_t R = it.q_len * p.G;
-    const bool two = R > 128;
+    const bool two = !HALF && R > 128;
+    const bool seq = two || HALF;                                       // every consuming slot takes every half-stage, in order
     const int32_t tl0 = split * it.tiles_per_split;
     const int32_t tl1 = min(it.n_tiles, tl0 + it.tiles_per_split);
     const int32_t n_half = (tl1 - tl0 + C::KS - 1) / C::KS;             // half-stages of this segment
     const int32_t n_pair = (n_half + 1) >> 1;
     const int32_t t_first = it.len - it.q_len;                          // reading R15: the last q_len positions
     // ring entry of K / V of half-stage h (see umma_seq_k / umma_seq_v)
-    auto entry_k = [&](int32_t h) { return two ? umma_seq_k(h) : 2 * umma_seq_k(h >> 1) + (h & 1); };
-    auto entry_v = [&](int32_t h) { return two ? umma_seq_v(h, n_half) : 2 * umma_seq_v(h >> 1, n_pair) + (h & 1); };
+    auto entry_k = [&](int32_t h) { return seq ? umma_seq_k(h) : 2 * umma_seq_k(h >> 1) + (h & 1); };
+    auto entry_v = [&](int32_t h) { return seq ? umma_seq_v(h, n_half) : 2 * umma_seq_v(h >> 1, n_pair) + (h & 1); };
 
-    if (warp == 0) {
-        // ================================ producer ================================
-        if (lane == 0) {
-            for (int b = 0; b < C::NBUF; ++b) { mbar_init(bar_full(b), 1); mbar_init(bar_empty(b), two ? 2 : 1); }
-            for (int s = 0; s < 2; ++s) {
-                for (int buf = 0; buf < 2; ++buf) { mbar_init(bar_s(s, buf), 1); mbar_init(bar_p(s, buf), 4); mbar_init(bar_pv(s, buf), 1); }
-                mbar_init(bar_o(s), 1);
+    // HALF: two CTAs of 256 threads share an SM (128 registers each at launch): the producer / MMA warpgroup keeps 64,
+    // the softmax warpgroup (one thread per query row, 64 scores + P in registers) takes 192.  4 x 32 x (64 + 192) = 32768.
+    if (warp < 4) {
+        if constexpr (HALF) asm volatile("setmaxnreg.dec.sync.aligned.u32 64;");
+        if (warp == 0) {
+            // ================================ producer ================================
+            if (lane == 0) {
+                for (int b = 0; b < C::NBUF; ++b) { mbar_init(bar_full(b), 1); mbar_init(bar_empty(b), two ? 2 : 1); }
+                for (int s = 0; s < C::NQ; ++s) {
+                    for (int buf = 0; buf < 2; ++buf) { mbar_init(bar_s(s, buf), 1); mbar_init(bar_p(s, buf), 4); mbar_init(bar_pv(s, buf), 1); }
+                    mbar_init(bar_o(s), 1);
+                }
+                asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
             }
-            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        }
-        __syncwarp();
-        named_arrive(1, C::kThreads);
-        const int32_t* trow = p.table + (int64_t)it.sid * p.tbl_width;
-        const uint8_t* head_base = p.kv_layer + (int64_t)kvh * p.L.head_bytes;
-        const int32_t n_entries = two ? 2 * n_half : 4 * n_pair;
-        // Physical block ids of this segment's tiles, fetched ONCE (lane l holds tiles l, l+32, ...): a
-        // table lookup inside the loop is a dependent L2 round trip per ring entry and made the producer,
-        // not the tensor pipe or the softmax, set the pace of the whole kernel.
-        constexpr int kPhysPre = 8;                               // 256 tiles; longer segments look up the rest
-        int32_t phys_pre[kPhysPre];
-#pragma unroll
-        for (int j = 0; j < kPhysPre; ++j) {
-            const int32_t t = tl0 + j * 32 + lane;
-            phys_pre[j] = t < tl1 ? __ldg(trow + table_slot(tile_block(it, t), p.n_sink, p.ring)) : 0;
-        }
-        auto phys_of = [&](int32_t rel) {                         // rel = tile - tl0; rel >> 5 is warp-uniform
-            const int32_t j = rel >> 5;
-            int32_t v = phys_pre[0];
-#pragma unroll
-            for (int q = 1; q < kPhysPre; ++q) v = j == q ? phys_pre[q] : v;
-            v = __shfl_sync(0xffffffffu, v, rel & 31);
-            if (j >= kPhysPre) v = __ldg(trow + table_slot(tile_block(it, tl0 + rel), p.n_sink, p.ring));
-            return v;
-        };
-        for (int32_t e = 0; e < n_entries; ++e) {
-            // invert the order: which (K | V, half-stage) is entry e
-            const int32_t es = two ? e : e >> 1, ns = two ? n_half : n_pair;
-            bool is_v;
-            int32_t j;
-            if (es == 0) { is_v = false; j = 0; }
-            else if (es == 2 * ns - 1) { is_v = true; j = ns - 1; }
-            else if (es & 1) { is_v = false; j = (es + 1) >> 1; }
-            else { is_v = true; j = (es >> 1) - 1; }
-            const int32_t h = two ? j : 2 * j + (e & 1);
-            const int32_t b = e % C::NBUF, k = e / C::NBUF;
-            if (k >= 1) mbar_wait(bar_empty(b), (k - 1) & 1);
-            if (h >= n_half) {                                        // phantom half-stage of an odd count
-                if (lane == 0) mbar_arrive(bar_full(b));
-                continue;
-            }
-            const int32_t t0 = tl0 + h * C::KS;
-            const int32_t nt = min(C::KS, tl1 - t0);
-            if (lane == 0) mbar_expect_tx(bar_full(b), (uint32_t)nt * C::kTileBytes);
             __syncwarp();
-            const uint32_t dst = sRing + b * C::kBufBytes;
-            const int32_t blk = is_v ? lane : lane / C::NH, hh = lane % C::NH;
-            const int32_t phys = phys_of(h * C::KS + min(blk, C::KS - 1));      // (every lane takes part in the shuffle)
-            if (is_v) {
-                if (lane < nt)
-                    bulk_g2s(dst + lane * C::kTileBytes, head_base + (int64_t)phys * p.L.block_bytes + p.L.tile_bytes,
-                             C::kTileBytes, bar_full(b));
-            } else if (lane < nt * C::NH) {
-                bulk_g2s(dst + hh * C::kKHalfBytes + blk * 2048, head_base + (int64_t)phys * p.L.block_bytes + hh * 2048, 2048,
-                         bar_full(b));
+            named_arrive(1, C::kThreads);
+            const int32_t* trow = p.table + (int64_t)it.sid * p.tbl_width;
+            const uint8_t* head_base = p.kv_layer + (int64_t)kvh * p.L.head_bytes;
+            const int32_t n_entries = seq ? 2 * n_half : 4 * n_pair;
+            // Physical block ids of this segment's tiles, fetched ONCE (lane l holds tiles l, l+32, ...): a
+            // table lookup inside the loop is a dependent L2 round trip per ring entry and made the producer,
+            // not the tensor pipe or the softmax, set the pace of the whole kernel.
+            constexpr int kPhysPre = 8;                               // 256 tiles; longer segments look up the rest
+            int32_t phys_pre[kPhysPre];
+    #pragma unroll
+            for (int j = 0; j < kPhysPre; ++j) {
+                const int32_t t = tl0 + j * 32 + lane;
+                phys_pre[j] = t < tl1 ? __ldg(trow + table_slot(tile_block(it, t), p.n_sink, p.ring)) : 0;
             }
+            auto phys_of = [&](int32_t rel) {                         // rel = tile - tl0; rel >> 5 is warp-uniform
+                const int32_t j = rel >> 5;
+                int32_t v = phys_pre[0];
+    #pragma unroll
+                for (int q = 1; q < kPhysPre; ++q) v = j == q ? phys_pre[q] : v;
+                v = __shfl_sync(0xffffffffu, v, rel & 31);
+                if (j >= kPhysPre) v = __ldg(trow + table_slot(tile_block(it, tl0 + rel), p.n_sink, p.ring));
+                return v;
+            };
+            for (int32_t e = 0; e < n_entries; ++e) {
+                // invert the order: which (K | V, half-stage) is entry e
+                const int32_t es = seq ? e : e >> 1, ns = seq ? n_half : n_pair;
+                bool is_v;
+                int32_t j;
+                if (es == 0) { is_v = false; j = 0; }
+                else if (es == 2 * ns - 1) { is_v = true; j = ns - 1; }
+                else if (es & 1) { is_v = false; j = (es + 1) >> 1; }
+                else { is_v = true; j = (es >> 1) - 1; }
+                const int32_t h = seq ? j : 2 * j + (e & 1);
+                const int32_t b = e % C::NBUF, k = e / C::NBUF;
+                if (k >= 1) mbar_wait(bar_empty(b), (k - 1) & 1);
+                if (h >= n_half) {                                        // phantom half-stage of an odd count
+                    if (lane == 0) mbar_arrive(bar_full(b));
+                    continue;
+                }
+                const int32_t t0 = tl0 + h * C::KS;
+                const int32_t nt = min(C::KS, tl1 - t0);
+                if (lane == 0) mbar_expect_tx(bar_full(b), (uint32_t)nt * C::kTileBytes);
+                __syncwarp();
+                const uint32_t dst = sRing + b * C::kBufBytes;
+                const int32_t blk = is_v ? lane : lane / C::NH, hh = lane % C::NH;
+                const int32_t phys = phys_of(h * C::KS + min(blk, C::KS - 1));      // (every lane takes part in the shuffle)
+                if (is_v) {
+                    if (lane < nt)
+                        bulk_g2s(dst + lane * C::kTileBytes, head_base + (int64_t)phys * p.L.block_bytes + p.L.tile_bytes,
+                                 C::kTileBytes, bar_full(b));
+                } else if (lane < nt * C::NH) {
+                    bulk_g2s(dst + hh * C::kKHalfBytes + blk * 2048, head_base + (int64_t)phys * p.L.block_bytes + hh * 2048, 2048,
+                             bar_full(b));
+                }
+            }
+            return;
         }
-        return;
-    }
-    if (warp >= 1 && warp <= 3) {
-        // ================================ MMA issuers ================================
-        // Warp 1 issues Q K^T for both slots, warps 2 / 3 issue P V of slot 0 / 1.  A single thread
-        // gets one tcgen05.mma out every ~110-130 cycles (measured), so the 32 MMAs of a half-stage
-        // are spread over three issuing threads (a fourth warp would put 4 warps on one SM
-        // sub-partition and cap everyone at 128 registers).
-        const bool is_pv = warp >= 2;
-        const int32_t slot = is_pv ? warp - 2 : 0;
-        if (warp == 1) {
-            asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;"
-                         ::"r"(smem_u32(const_cast<uint32_t*>(tmem_slot))), "r"(C::kTmemCols));
-            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
-        }
-        tc_fence_before();
-        named_sync(1, C::kThreads);
-        tc_fence_after();
-        const uint32_t tmem = *tmem_slot;
-        constexpr uint32_t idesc_qk = umma_idesc(C::KS * kBlockTokens, false);
-        constexpr uint32_t idesc_pv = umma_idesc(D, true);
-        const uint32_t tSbase = tmem + C::kColS + 128 * slot, tOacc = tmem + C::kColO + D * slot;      // (P V warps)
-
-        auto wait_full = [&](int32_t e) {
-            mbar_wait(bar_full(e % C::NBUF), (e / C::NBUF) & 1);
+        {
+            // ================================ MMA issuers ================================
+            // Warp 1 issues Q K^T for both slots, warps 2 / 3 issue P V of slot 0 / 1.  A single thread
+            // gets one tcgen05.mma out every ~110-130 cycles (measured), so the 32 MMAs of a half-stage
+            // are spread over three issuing threads (a fourth warp would put 4 warps on one SM
+            // sub-partition and cap everyone at 128 registers).
+            const bool is_pv = warp >= 2;
+            const int32_t slot = is_pv ? warp - 2 : 0;
+            if (warp == 1) {
+                asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;"
+                             ::"r"(smem_u32(const_cast<uint32_t*>(tmem_slot))), "r"(C::kTmemCols));
+                asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+            }
+            tc_fence_before();
+            named_sync(1, C::kThreads);
             tc_fence_after();
-        };
-        auto release = [&](int32_t e) { if (lane == 0) umma_commit(bar_empty(e % C::NBUF)); };
-        // S[buf] = Q K^T over the K half-stage in ring entry e
-        const uint32_t elect = lane == 0 ? 1u : 0u;
-        auto issue_qk = [&](int32_t qslot, int32_t buf, int32_t e) {
-            // descriptors = base + (byte offset >> 4) in the address field (no carry: shared memory < 256 KB)
-            const uint64_t dq0 = umma_desc(sQ + (two ? qslot : 0) * C::kQBytes, 16, 1024);
-            const uint64_t dk0 = umma_desc(sRing + (e % C::NBUF) * C::kBufBytes, 16, 1024);
-            const uint32_t ts = tmem + C::kColS + 128 * qslot + 64 * buf;
-#pragma unroll
-            for (int kk = 0; kk < D / 16; ++kk)
-                umma_ss_e(ts, dq0 + (uint64_t)(((kk >> 2) * C::kQHalfBytes + (kk & 3) * 32) >> 4),
-                          dk0 + (uint64_t)(((kk >> 2) * C::kKHalfBytes + (kk & 3) * 32) >> 4), idesc_qk, kk > 0 ? 1u : 0u, elect);
-            if (lane == 0) umma_commit(bar_s(qslot, buf));
-            __syncwarp();
-        };
-        // O (+)= P V over the V half-stage in ring entry e: per valid block one K=16 MMA for the hi part of P
-        // and one for the lo part (per 32-column chunk of the S buffer: hi in columns 0-15, lo in 16-31)
-        auto issue_pv = [&](int32_t buf, int32_t e, int32_t nt, bool accumulate) {
-            const uint64_t vd0 = umma_desc(sRing + (e % C::NBUF) * C::kBufBytes, 2048, 1024);
-            const uint32_t pa0 = tSbase + 64 * buf;
-#pragma unroll
-            for (int b = 0; b < C::KS; ++b) {
-                if (b < nt) {                             // (warp-uniform)
-                    const uint32_t pa = pa0 + 32 * (b >> 1) + 8 * (b & 1);
-                    const uint64_t vd = vd0 + (uint64_t)((b * C::kTileBytes) >> 4);
-                    umma_ts_e(tOacc, pa, vd, idesc_pv, (accumulate || b > 0) ? 1u : 0u, elect);
-                    umma_ts_e(tOacc, pa + 16, vd, idesc_pv, 1u, elect);
-                }
-            }
-            if (lane == 0) umma_commit(bar_pv(slot, buf));
-            __syncwarp();
-        };
-        // V rows past the session's length hold stale or poisoned bytes (0 * NaN = NaN): zero them
-        auto fix_ragged_v = [&](int32_t e, int32_t t0, int32_t nt) {
-            const int32_t last = it.n_tiles - 1, nvalid = it.len & (kBlockTokens - 1);
-            if (nvalid == 0 || last < t0 || last >= t0 + nt) return;
-            uint8_t* vt = gen + 2 * C::kQBytes + (e % C::NBUF) * C::kBufBytes + (last - t0) * C::kTileBytes;
-            const int32_t per_row = C::NH * 8;
-            for (int32_t idx = lane; idx < (kBlockTokens - nvalid) * per_row; idx += 32) {
-                const int32_t row = nvalid + idx / per_row, rem = idx % per_row;
-                *reinterpret_cast<uint4*>(vt + (rem >> 3) * 2048 + row * 128 + (rem & 7) * 16) = make_uint4(0u, 0u, 0u, 0u);
-            }
-            fence_async_smem();
-            __syncwarp();
-        };
-        // this slot's half-stages: h(k) = k (two) or 2 k + slot
-        const int32_t n_mine = two ? n_half : (n_half - slot + 1) >> 1;
-        auto half_of = [&](int32_t k) { return two ? k : 2 * k + slot; };
-        if (!is_pv) {
-            // ---- Q K^T of every half-stage h, for both slots (R > 128) or for slot h & 1: into S buffer
-            // k & 1 of the slot (k = the slot's own count), as soon as P V of k - 2 has drained that buffer ----
-            for (int32_t h = 0; h < n_half; ++h) {
-                const int32_t e = entry_k(h);
-                wait_full(e);
-                for (int32_t qs = two ? 0 : (h & 1); qs < (two ? 2 : (h & 1) + 1); ++qs) {
-                    const int32_t k = two ? h : h >> 1, buf = k & 1;
-                    if (k >= 2) {
-                        mbar_wait(bar_pv(qs, buf), ((k >> 1) - 1) & 1);
-                        tc_fence_after();
-                    }
-                    issue_qk(qs, buf, e);
-                    release(e);                          // (one arrival per consuming slot)
-                }
-            }
-            if (!two && (n_half & 1)) {                   // phantom half-stage of an odd count: hand the entry back
-                const int32_t ek = entry_k(n_half);
-                wait_full(ek); if (lane == 0) mbar_arrive(bar_empty(ek % C::NBUF));
-            }
-        } else {
-            // ---- P V: half-stage k out of S buffer k & 1, once the softmax has written P there ----
-            for (int32_t k = 0; k < n_mine; ++k) {
-                const int32_t h = half_of(k), e = entry_v(h), buf = k & 1;
-                const int32_t t0 = tl0 + h * C::KS, nt = min(C::KS, tl1 - t0);
-                wait_full(e);
-                fix_ragged_v(e, t0, nt);
-                mbar_wait(bar_p(slot, buf), (k >> 1) & 1);
+            const uint32_t tmem = *tmem_slot;
+            constexpr uint32_t idesc_qk = umma_idesc(C::KS * kBlockTokens, false);
+            constexpr uint32_t idesc_pv = umma_idesc(D, true);
+            const uint32_t tSbase = tmem + C::kColS + 128 * slot, tOacc = tmem + C::kColO + D * slot;      // (P V warps)
+            if (HALF && warp == 3) return;                    // (one row tile: no second P V issuer; warp 1 frees the TMEM)
+
+            auto wait_full = [&](int32_t e) {
+                mbar_wait(bar_full(e % C::NBUF), (e / C::NBUF) & 1);
                 tc_fence_after();
-                issue_pv(buf, e, nt, k > 0);
-                release(e);
-                if (k == n_mine - 1 && lane == 0) umma_commit(bar_o(slot));
+            };
+            auto release = [&](int32_t e) { if (lane == 0) umma_commit(bar_empty(e % C::NBUF)); };
+            // S[buf] = Q K^T over the K half-stage in ring entry e
+            const uint32_t elect = lane == 0 ? 1u : 0u;
+            auto issue_qk = [&](int32_t qslot, int32_t buf, int32_t e) {
+                // descriptors = base + (byte offset >> 4) in the address field (no carry: shared memory < 256 KB)
+                const uint64_t dq0 = umma_desc(sQ + (two ? qslot : 0) * C::kQBytes, 16, 1024);
+                const uint64_t dk0 = umma_desc(sRing + (e % C::NBUF) * C::kBufBytes, 16, 1024);
+                const uint32_t ts = tmem + C::kColS + 128 * qslot + 64 * buf;
+    #pragma unroll
+                for (int kk = 0; kk < D / 16; ++kk)
+                    umma_ss_e(ts, dq0 + (uint64_t)(((kk >> 2) * C::kQHalfBytes + (kk & 3) * 32) >> 4),
+                              dk0 + (uint64_t)(((kk >> 2) * C::kKHalfBytes + (kk & 3) * 32) >> 4), idesc_qk, kk > 0 ? 1u : 0u, elect);
+                if (lane == 0) umma_commit(bar_s(qslot, buf));
+                __syncwarp();
+            };
+            // O (+)= P V over the V half-stage in ring entry e: per valid block one K=16 MMA for the hi part of P
+            // and one for the lo part (per 32-column chunk of the S buffer: hi in columns 0-15, lo in 16-31)
+            auto issue_pv = [&](int32_t buf, int32_t e, int32_t nt, bool accumulate) {
+                const uint64_t vd0 = umma_desc(sRing + (e % C::NBUF) * C::kBufBytes, 2048, 1024);
+                const uint32_t pa0 = tSbase + 64 * buf;
+    #pragma unroll
+                for (int b = 0; b < C::KS; ++b) {
+                    if (b < nt) {                             // (warp-uniform)
+                        const uint32_t pa = pa0 + 32 * (b >> 1) + 8 * (b & 1);
+                        const uint64_t vd = vd0 + (uint64_t)((b * C::kTileBytes) >> 4);
+                        umma_ts_e(tOacc, pa, vd, idesc_pv, (accumulate || b > 0) ? 1u : 0u, elect);
+                        umma_ts_e(tOacc, pa + 16, vd, idesc_pv, 1u, elect);
+                    }
+                }
+                if (lane == 0) umma_commit(bar_pv(slot, buf));
+                __syncwarp();
+            };
+            // V rows past the session's length hold stale or poisoned bytes (0 * NaN = NaN): zero them
+            auto fix_ragged_v = [&](int32_t e, int32_t t0, int32_t nt) {
+                const int32_t last = it.n_tiles - 1, nvalid = it.len & (kBlockTokens - 1);
+                if (nvalid == 0 || last < t0 || last >= t0 + nt) return;
+                uint8_t* vt = gen + C::NQ * C::kQBytes + (e % C::NBUF) * C::kBufBytes + (last - t0) * C::kTileBytes;
+                const int32_t per_row = C::NH * 8;
+                for (int32_t idx = lane; idx < (kBlockTokens - nvalid) * per_row; idx += 32) {
+                    const int32_t row = nvalid + idx / per_row, rem = idx % per_row;
+                    *reinterpret_cast<uint4*>(vt + (rem >> 3) * 2048 + row * 128 + (rem & 7) * 16) = make_uint4(0u, 0u, 0u, 0u);
+                }
+                fence_async_smem();
+                __syncwarp();
+            };
+            // this slot's half-stages: h(k) = k (two) or 2 k + slot
+            const int32_t n_mine = seq ? n_half : (n_half - slot + 1) >> 1;
+            auto half_of = [&](int32_t k) { return seq ? k : 2 * k + slot; };
+            if (!is_pv) {
+                // ---- Q K^T of every half-stage h, for both slots (R > 128) or for slot h & 1: into S buffer
+                // k & 1 of the slot (k = the slot's own count), as soon as P V of k - 2 has drained that buffer ----
+                for (int32_t h = 0; h < n_half; ++h) {
+                    const int32_t e = entry_k(h);
+                    wait_full(e);
+                    for (int32_t qs = seq ? 0 : (h & 1); qs < (two ? 2 : HALF ? 1 : (h & 1) + 1); ++qs) {
+                        const int32_t k = seq ? h : h >> 1, buf = k & 1;
+                        if (k >= 2) {
+                            mbar_wait(bar_pv(qs, buf), ((k >> 1) - 1) & 1);
+                            tc_fence_after();
+                        }
+                        issue_qk(qs, buf, e);
+                        release(e);                          // (one arrival per consuming slot)
+                    }
+                }
+                if (!seq && (n_half & 1)) {                   // phantom half-stage of an odd count: hand the entry back
+                    const int32_t ek = entry_k(n_half);
+                    wait_full(ek); if (lane == 0) mbar_arrive(bar_empty(ek % C::NBUF));
+                }
+            } else {
+                // ---- P V: half-stage k out of S buffer k & 1, once the softmax has written P there ----
+                for (int32_t k = 0; k < n_mine; ++k) {
+                    const int32_t h = half_of(k), e = entry_v(h), buf = k & 1;
+                    const int32_t t0 = tl0 + h * C::KS, nt = min(C::KS, tl1 - t0);
+                    wait_full(e);
+                    fix_ragged_v(e, t0, nt);
+                    mbar_wait(bar_p(slot, buf), (k >> 1) & 1);
+                    tc_fence_after();
+                    issue_pv(buf, e, nt, k > 0);
+                    release(e);
+                    if (k == n_mine - 1 && lane == 0) umma_commit(bar_o(slot));
+                }
+                if (!seq && slot == 1 && (n_half & 1)) {
+                    const int32_t ev = entry_v(n_half);
+                    wait_full(ev); if (lane == 0) mbar_arrive(bar_empty(ev % C::NBUF));
+                }
             }
-            if (!two && slot == 1 && (n_half & 1)) {
-                const int32_t ev = entry_v(n_half);
-                wait_full(ev); if (lane == 0) mbar_arrive(bar_empty(ev % C::NBUF));
+            if (warp == 1) {
+                // every softmax warp has finished reading TMEM
+                named_sync(2, 32 + C::kSoftmaxThreads);
+                tc_fence_after();
+                asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(C::kTmemCols));
             }
+            return;
         }
-        if (warp == 1) {
-            // every softmax warp has finished reading TMEM
-            named_sync(2, 32 + 256);
-            tc_fence_after();
-            asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(C::kTmemCols));
-        }
-        return;
     }
+    if constexpr (HALF) asm volatile("setmaxnreg.inc.sync.aligned.u32 192;");
 
     // ================================ softmax warps ================================
     const int32_t slot = (warp - 4) >> 2, quarter = warp & 3;       // TMEM lanes 32 (warp % 4) .. + 31
     const int32_t row = quarter * 32 + lane;
-    const int32_t tile_row0 = two ? 128 * slot : 0;
+    const int32_t tile_row0 = two ? 128 * slot : 0;                   // (HALF: slot is always 0)
     const int32_t rho = tile_row0 + row;                              // rho = r * G + g
     const bool valid = rho < R;
     const int32_t rq = rho / p.G, gq = rho - rq * p.G;
@@ -379,10 +393,10 @@ attend_umma_kernel(AttendParams p) {
     // ---- Q rows -> shared memory, K-major SWIZZLE_128B, one [128][64] region per 64-dim half ----
     {
         const int32_t tid2 = threadIdx.x - 128;
-        const int32_t n_rows = two ? 256 : 128;
+        const int32_t n_rows = two ? 256 : 128;                       // (HALF: 128, one Q region)
         constexpr int CPR = D / 8;                                    // 16-byte chunks per row
         // 16-byte cp.async per chunk: all of a thread's copies are in flight together
-        for (int32_t idx = tid2; idx < n_rows * CPR; idx += 256) {
+        for (int32_t idx = tid2; idx < n_rows * CPR; idx += C::kSoftmaxThreads) {
             const int32_t rr = idx / CPR, c = idx % CPR;
             const uint32_t dst = (rr >> 7) * C::kQBytes + (c >> 3) * C::kQHalfBytes + (rr & 127) * 128 + (((c & 7) ^ (rr & 7)) << 4);
             if (rr < R) {
@@ -407,9 +421,9 @@ attend_umma_kernel(AttendParams p) {
     // (two tcgen05.ld of 32 columns), row max, exp2, and P written back over the columns just read.
     float m_run = -INFINITY, m_used = -INFINITY;
     float l0 = 0.f, l1 = 0.f, l2 = 0.f, l3 = 0.f;                     // four partial sums (ILP)
-    const int32_t n_mine = two ? n_half : (n_half - slot + 1) >> 1;
+    const int32_t n_mine = seq ? n_half : (n_half - slot + 1) >> 1;
     for (int32_t k = 0; k < n_mine; ++k) {
-        const int32_t h = two ? k : 2 * k + slot, buf = k & 1;
+        const int32_t h = seq ? k : 2 * k + slot, buf = k & 1;
         mbar_wait(bar_s(slot, buf), (k >> 1) & 1);
         tc_fence_after();
         if (warp_active) {
@@ -537,7 +551,7 @@ attend_umma_kernel(AttendParams p) {
         for (int c = 0; c < D / 32; ++c) tmem_ld32(tO + 32 * c, reinterpret_cast<uint32_t*>(o) + 32 * c);
         tmem_wait_ld();
     };
-    if (two) {
+    if (seq) {
         if (n_it > 0) {
             mbar_wait(bar_o(slot), 0);
             tc_fence_after();
@@ -591,7 +605,7 @@ attend_umma_kernel(AttendParams p) {
         }
     }
     tc_fence_before();
-    named_arrive(2, 32 + 256);
+    named_arrive(2, 32 + C::kSoftmaxThreads);
     if (threadIdx.x == 128) stamp_end(p);
 }
 
@@ -602,18 +616,29 @@ inline bool attend_umma_supported(int32_t G, int32_t max_q) { return (int64_t)G 
 
 inline cudaError_t configure_attend_umma_kernels() {
     cudaError_t e;
-    if ((e = cudaFuncSetAttribute(attend_umma_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  UmmaCfg<128>::kSmemBytes)) != cudaSuccess) return e;
-    return cudaFuncSetAttribute(attend_umma_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                UmmaCfg<64>::kSmemBytes);
+    if ((e = cudaFuncSetAttribute(attend_umma_kernel<128, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  UmmaCfg<128, false>::kSmemBytes)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(attend_umma_kernel<64, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  UmmaCfg<64, false>::kSmemBytes)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(attend_umma_kernel<128, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  UmmaCfg<128, true>::kSmemBytes)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(attend_umma_kernel<128, true>, cudaFuncAttributePreferredSharedMemoryCarveout, 100)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(attend_umma_kernel<64, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  UmmaCfg<64, true>::kSmemBytes)) != cudaSuccess) return e;
+    return cudaFuncSetAttribute(attend_umma_kernel<64, true>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
 }
 
-// chunk-class items (16 < R <= 256): p.items / p.n_items must point at them
+// chunk-class items (16 < R <= 256): p.items / p.n_items must point at them.  `half`: every item of the launch has
+// R <= 128 rows -- the half-size variant, two CTAs per SM (UmmaCfg<D, true>)
 inline cudaError_t launch_attend_umma(const AttendParams& p, int32_t D, int32_t Hkv, int32_t total_splits, cudaStream_t st,
-                                      bool pdl = false) {
+                                      bool pdl = false, bool half = false) {
     dim3 grid(Hkv, total_splits);
-    if (D == 128) return launch_kernel(attend_umma_kernel<128>, grid, UmmaCfg<128>::kThreads, UmmaCfg<128>::kSmemBytes, st, pdl, p);
-    return launch_kernel(attend_umma_kernel<64>, grid, UmmaCfg<64>::kThreads, UmmaCfg<64>::kSmemBytes, st, pdl, p);
+    if (half) {
+        if (D == 128) return launch_kernel(attend_umma_kernel<128, true>, grid, UmmaCfg<128, true>::kThreads, UmmaCfg<128, true>::kSmemBytes, st, pdl, p);
+        return launch_kernel(attend_umma_kernel<64, true>, grid, UmmaCfg<64, true>::kThreads, UmmaCfg<64, true>::kSmemBytes, st, pdl, p);
+    }
+    if (D == 128) return launch_kernel(attend_umma_kernel<128, false>, grid, UmmaCfg<128, false>::kThreads, UmmaCfg<128, false>::kSmemBytes, st, pdl, p);
+    return launch_kernel(attend_umma_kernel<64, false>, grid, UmmaCfg<64, false>::kThreads, UmmaCfg<64, false>::kSmemBytes, st, pdl, p);
 }
 
 }  // namespace metronome

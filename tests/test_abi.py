@@ -64,9 +64,11 @@ def test_sass_census_shows_the_hardware_paths_each_kernel_claims():
     build.build_library()
     c = build.sass_census()
     for D in (64, 128):
-        u, g, r = c[f"attend_umma_kernel<{D}>"], c[f"attend_gqa_kernel<{D}, false>"], c[f"attend_rows_kernel<{D}, false>"]
+        u, g, r = c[f"attend_umma_kernel<{D}, false>"], c[f"attend_gqa_kernel<{D}, false>"], c[f"attend_rows_kernel<{D}, false>"]
         assert u.get("UTCHMMA", 0) > 0 and u.get("LDTM", 0) > 0 and u.get("STTM", 0) > 0 and u.get("UBLKCP", 0) > 0, u
         assert g.get("HMMA", 0) > 0 and g.get("LDSM", 0) > 0 and g.get("UBLKCP", 0) > 0 and "UTCHMMA" not in g, g
+        uh = c[f"attend_umma_kernel<{D}, true>"]          # half-size variant (R <= 128 rows, two CTAs per SM): the same tcgen05 path
+        assert uh.get("UTCHMMA", 0) > 0 and uh.get("LDTM", 0) > 0 and uh.get("STTM", 0) > 0 and uh.get("UBLKCP", 0) > 0, uh
         g8 = c[f"attend_gqa_kernel<{D}, true>"]         # fp8 KV tile: E4M3 -> fp16 conversions feed the same mma.sync path
         assert g8.get("HMMA", 0) > 0 and g8.get("LDSM", 0) > 0 and g8.get("UBLKCP", 0) > 0 and g8.get("F2FP.F16.E4M3", 0) > 0, g8
         assert r.get("FFMA2", 0) > 0 and "HMMA" not in r and "UTCHMMA" not in r, r
