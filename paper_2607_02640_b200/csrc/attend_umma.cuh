@@ -163,7 +163,10 @@ attend_umma_kernel(AttendParams p) {
     auto bar_o = [&](int s) { return sBar + 8u * (2 * C::NBUF + 12 + s); };                     // last P V of slot s done
     volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(gen + C::kBarOff + 8 * (2 * C::NBUF + 14));
 
-    const int32_t kvh = blockIdx.x;
+    // HALF: an item of more than 128 rows is run as several CTAs of 128 rows each (gridDim.x = Hkv x row tiles, the row
+    // tile fastest: the CTAs that stream the same K / V tiles are dispatched next to each other, the second pass hits L2)
+    const int32_t n_rt = HALF ? (int32_t)gridDim.x / p.L.n_kv_heads : 1;
+    const int32_t kvh = (int32_t)blockIdx.x / n_rt, r0 = ((int32_t)blockIdx.x % n_rt) * 128;
     // (no item is split when the grid has one row per item: no search)
     const int32_t i = (int32_t)gridDim.y == p.n_items
                           ? (int32_t)blockIdx.y
@@ -171,7 +174,9 @@ attend_umma_kernel(AttendParams p) {
     const AttendItem it = p.items[i];
     const int32_t split = (int32_t)blockIdx.y - it.split_off;
     const int32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int32_t R = it.q_len * p.G;
+    const int32_t R_all = it.q_len * p.G;
+    if (HALF && r0 >= R_all) return;                                    // (CTA-uniform, before anything is set up)
+    const int32_t R = HALF ? min(128, R_all - r0) : R_all;              // rows of THIS CTA: global rows r0 .. r0 + R - 1
     const bool two = !HALF && R > 128;
     const bool seq = two || HALF;                                       // every consuming slot takes every half-stage, in order
     const int32_t tl0 = split * it.tiles_per_split;
@@ -382,13 +387,13 @@ attend_umma_kernel(AttendParams p) {
     const int32_t slot = (warp - 4) >> 2, quarter = warp & 3;       // TMEM lanes 32 (warp % 4) .. + 31
     const int32_t row = quarter * 32 + lane;
     const int32_t tile_row0 = two ? 128 * slot : 0;                   // (HALF: slot is always 0)
-    const int32_t rho = tile_row0 + row;                              // rho = r * G + g
-    const bool valid = rho < R;
+    const int32_t rho = r0 + tile_row0 + row;                         // (global row) rho = r * G + g
+    const bool valid = tile_row0 + row < R;
     const int32_t rq = rho / p.G, gq = rho - rq * p.G;
     const int32_t t = valid ? t_first + rq : -1;                      // -1: padding row, admits nothing
     const bool warp_active = tile_row0 + quarter * 32 < R;
-    const int32_t t_wmin = t_first + (tile_row0 + quarter * 32) / p.G;
-    const int32_t t_wmax = t_first + (min(R, tile_row0 + quarter * 32 + 32) - 1) / p.G;
+    const int32_t t_wmin = t_first + (r0 + tile_row0 + quarter * 32) / p.G;
+    const int32_t t_wmax = t_first + (r0 + min(R, tile_row0 + quarter * 32 + 32) - 1) / p.G;
 
     // ---- Q rows -> shared memory, K-major SWIZZLE_128B, one [128][64] region per 64-dim half ----
     {
@@ -400,7 +405,7 @@ attend_umma_kernel(AttendParams p) {
             const int32_t rr = idx / CPR, c = idx % CPR;
             const uint32_t dst = (rr >> 7) * C::kQBytes + (c >> 3) * C::kQHalfBytes + (rr & 127) * 128 + (((c & 7) ^ (rr & 7)) << 4);
             if (rr < R) {
-                const int32_t r2 = rr / p.G, g2 = rr - r2 * p.G;
+                const int32_t r2 = (r0 + rr) / p.G, g2 = (r0 + rr) - r2 * p.G;
                 const __nv_bfloat16* src = p.q + ((int64_t)(it.q_row_off + r2) * p.Hq + kvh * p.G + g2) * D + c * 8;
                 asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sQ + dst), "l"(src) : "memory");
             } else {
@@ -628,12 +633,13 @@ inline cudaError_t configure_attend_umma_kernels() {
     return cudaFuncSetAttribute(attend_umma_kernel<64, true>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
 }
 
-// chunk-class items (16 < R <= 256): p.items / p.n_items must point at them.  `half`: every item of the launch has
-// R <= 128 rows -- the half-size variant, two CTAs per SM (UmmaCfg<D, true>)
+// chunk-class items (16 < R <= 256): p.items / p.n_items must point at them.  `half`: the half-size variant, two CTAs
+// per SM (UmmaCfg<D, true>), `row_tiles` = ceil(largest R / 128) CTAs of 128 rows per (item, head) segment
 inline cudaError_t launch_attend_umma(const AttendParams& p, int32_t D, int32_t Hkv, int32_t total_splits, cudaStream_t st,
-                                      bool pdl = false, bool half = false) {
+                                      bool pdl = false, bool half = false, int32_t row_tiles = 1) {
     dim3 grid(Hkv, total_splits);
     if (half) {
+        grid.x = Hkv * row_tiles;                        // (row tile fastest)
         if (D == 128) return launch_kernel(attend_umma_kernel<128, true>, grid, UmmaCfg<128, true>::kThreads, UmmaCfg<128, true>::kSmemBytes, st, pdl, p);
         return launch_kernel(attend_umma_kernel<64, true>, grid, UmmaCfg<64, true>::kThreads, UmmaCfg<64, true>::kSmemBytes, st, pdl, p);
     }

@@ -48,6 +48,7 @@ constexpr int kStagingSlots = 64;      // per-call metadata slots (pinned host +
 constexpr int kStagingGroup = 8;       // one completion event per 8 slots: an event between two kernels
                                        // would break their programmatic (PDL) launch edge
 constexpr int kMaxSplits = 64;
+constexpr int kUmmaHalfDefault = 2;
 constexpr int kGqaSmClassDefault = 0;  // (set to 1 once measured)
 constexpr int kDirectSlots = 3;        // device staging slots of the event-free async host steps
 constexpr int kStampSlots = 1 << 15;   // attention launches one stamped pass can hold
@@ -162,7 +163,8 @@ struct metronome_pool {
     std::vector<int32_t> stamp_kind;   // per used slot: 1 rows, 2 gqa decode, 3 chunk
 
     int32_t tune_split_tokens = 0, tune_family = 0, tune_gqa_dynamic = 0, tune_fused_step = 0;
-    bool tune_umma_half = true;        // chunk items of R <= 128 rows on the half-size kernel, two CTAs per SM (METRONOME_UMMA_HALF=0: off)
+    int tune_umma_half = 1;            // METRONOME_UMMA_HALF: 0 full-size chunk kernel only, 1 half-size kernel (two CTAs per SM) when every
+                                       // chunk item of the launch has R <= 128 rows, 2 always (larger items as two CTAs of 128 rows)
     int tune_gqa_smclass = 0;          // GQA decode ranges sized by the SM's streaming speed (METRONOME_GQA_SMCLASS at pool creation)
     uint8_t* d_sm_class = nullptr;     // device copy of sm_class (256 bytes)
     bool tune_host_direct = true;      // false (METRONOME_HOST_STEP_EVENTS=1 at pool creation): async host steps always chain events
@@ -597,8 +599,11 @@ int launch_attend(metronome_pool* pool, int32_t layer, const AttendPlan& pl, con
             p.items = d_items + pl.n_cls[0]; p.n_items = pl.n_cls[1];
             p.stamp = next_stamp(pool, 3);
             if (pool->fp8) CU(launch_attend_umma_fp8(p, c.head_dim, c.n_kv_heads, pl.total_splits[1], st, pdl));
-            else CU(launch_attend_umma(p, c.head_dim, c.n_kv_heads, pl.total_splits[1], st, pdl,
-                                       pool->tune_umma_half && pool->G * pl.cls_max_q[1] <= 128));
+            else {
+                const int32_t R_max = pool->G * pl.cls_max_q[1];
+                const bool half = pool->tune_umma_half >= 2 || (pool->tune_umma_half == 1 && R_max <= 128);
+                CU(launch_attend_umma(p, c.head_dim, c.n_kv_heads, pl.total_splits[1], st, pdl, half, (R_max + 127) / 128));
+            }
             ++pool->n_launch;
         }
     } else {
@@ -816,7 +821,7 @@ int metronome_pool_create(const metronome_pool_config_t* cfg, metronome_pool_t**
     }
     pool->slot_bytes = (size_t)c.max_sessions * (sizeof(AppendItem) + sizeof(AttendItem)) + kMaxRangeItems * sizeof(int32_t) + 16;
     { const char* ev = getenv("METRONOME_HOST_STEP_EVENTS"); pool->tune_host_direct = !(ev && ev[0] == '1'); }
-    { const char* ev = getenv("METRONOME_UMMA_HALF"); pool->tune_umma_half = !(ev && ev[0] == '0'); }
+    { const char* ev = getenv("METRONOME_UMMA_HALF"); pool->tune_umma_half = ev ? atoi(ev) : kUmmaHalfDefault; }
     { const char* ev = getenv("METRONOME_GQA_SMCLASS"); pool->tune_gqa_smclass = ev ? atoi(ev) : kGqaSmClassDefault; }
     e = cudaMalloc(&pool->d_tickets, (size_t)c.max_sessions * c.n_kv_heads * sizeof(int32_t));
     if (e != cudaSuccess) return fail(METRONOME_ERR_OUT_OF_MEMORY, e, "cudaMalloc tickets");
