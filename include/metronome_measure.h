@@ -23,7 +23,9 @@ int metronome_pool_stats(metronome_pool_t* pool, int64_t* kernel_launches, int64
  * built and verified, but measured 0.4-4.5 % slower per frame than the two launches on B200, so it is off unless
  * asked for: DESIGN.md sec. 5.2); setting it measures the SMs' streaming speeds once (metronome_pool_sm_speeds).
  * For benchmarks and tests of "both launch modes" (L258).  Errors: INVALID_ARG.
- * Two more switches are read from the environment at pool creation (measurement aids):
+ * Three more switches are read from the environment at pool creation (measurement aids):
+ * METRONOME_UMMA_HALF=0 | 1 | 2 picks the chunk-prefill kernel: full-size (one CTA per SM) only, half-size (two CTAs per SM) for
+ * launches whose items have at most 128 query rows, or half-size always (default 2);
  * METRONOME_GQA_SMCLASS=1 sizes the GQA decode kernel's ranges by the SMs' measured streaming speeds (a calibration pass per
  * pool; off by default), METRONOME_HOST_STEP_EVENTS=1 makes metronome_step_host_async chain events even for pinned buffers. */
 int metronome_pool_set_tuning(metronome_pool_t* pool, int32_t split_tokens, int32_t kernel_family,
