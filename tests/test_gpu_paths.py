@@ -294,6 +294,37 @@ def test_event_free_host_steps_under_load(G):
     assert per_step >= 3, per_step
 
 
+@pytest.mark.parametrize("mode", ["0", "1", "2"])
+def test_chunk_kernel_variants(monkeypatch, mode):
+    """METRONOME_UMMA_HALF (read at pool creation): 0 = the full-size chunk kernel only (one CTA per SM, two row tiles),
+    1 = the half-size variant (two CTAs per SM, one row tile) when every chunk item of a launch has R <= 128 rows, 2 (the
+    default) = always, items of more than 128 rows as two CTAs of 128 rows each.  GQA 8: launches of 25-token chunks
+    (R = 200: two row tiles / two CTAs), of 9-token chunks (R = 72), mixed ones (25, 5, 13 tokens + decode rows, so CTAs whose
+    row offset lies past a small item's rows exit at once), S = 17 (a partly filled second sink block), windows that
+    slide; outputs pre-filled with NaN and compared with the oracle on every row."""
+    monkeypatch.setenv("METRONOME_UMMA_HALF", mode)
+    Hq, Hkv, D, S, W, N, n_max = 16, 2, 128, 17, 300, 4, 25
+    per = 2 + (W + n_max - 1) // 16 + 2
+    kw = dict(n_q_heads=Hq, n_kv_heads=Hkv, head_dim=D, max_sessions=N, max_new_tokens=n_max)
+    pool = binding.Pool(n_sinks=S, window=W, n_blocks=N * per, **kw)
+    defn = O.DefinitionOracle(O.PoolConfig(S=S, W=W, n_blocks=N * per, block_size=16, **kw))
+    sids = [pool.session_open() for _ in range(N)]
+    assert sids == [defn.session_open() for _ in range(N)]
+    rng = np.random.default_rng(2607 + int(mode))
+    plans = [[25] * N, [9] * N, [25, 5, 13, 1], [1] * N, [25, 25, 1, 9], [3, 25, 25, 25]]
+    for step in range(36):
+        n_new = np.asarray(plans[step % len(plans)], np.int32)
+        rows = int(n_new.sum())
+        k, v, q = _rows(rng, rows, Hkv, D), _rows(rng, rows, Hkv, D), _rows(rng, rows, Hq, D)
+        out = torch.full((rows, Hq, D), float("nan"), dtype=torch.bfloat16, device="cuda")
+        pool.append_attend(0, sids, n_new, k.cuda(), v.cuda(), q.cuda(), out)
+        defn.append_kv(0, sids, [int(x) for x in n_new], synth.to_u16(k), synth.to_u16(v))
+        ref = defn.attend_frame(0, sids, [int(x) for x in n_new], synth.to_u16(q))
+        assert torch.isfinite(out.float()).all(), f"mode {mode} step {step}: rows no CTA wrote"
+        assert_parity(out, ref, f"chunk kernel mode {mode}, step {step}, n_new {n_new}")
+    assert min(defn.length.values()) > S + W
+
+
 def test_gqa_ranges_by_sm_class(monkeypatch):
     """GqaPlan::sm_mode (METRONOME_GQA_SMCLASS=1 at pool creation; off by default): the GQA decode kernel's CTAs read %smid
     and claim a long range (fast SMs) or a shorter one (the SMs that a calibration pass found to stream slower) from two
